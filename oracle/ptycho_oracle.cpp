@@ -1,0 +1,608 @@
+// ptycho_oracle.cpp — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// Plain, slow, double-precision CPU restatement of one forward+adjoint iteration of the
+// mixed-state multislice ptychography model of arxiv 2505.14372 ("phaser"), written from the
+// paper and from the readings R1..R22 listed in DESIGN.md §3.  It shares no code,
+// header, table or constant generator with the CUDA path in paper_2505_14372_b200/csrc and
+// neither side includes the other.  Only tests/, __graft_entry__.smoke() and bench.py's
+// cpu_baseline / --impl reference leg may load this library.
+//
+// Everything is the plain definition: naive O(N^2) 1-D DFT (row-column for 2-D) and a simple
+// recursive radix-2 FFT, std::complex<double>, no blocking, no fusion.  OpenMP only splits the
+// loop over probe positions ("operates on a group of probe positions in parallel").
+//
+// Pins (tests/test_oracle_pins.py, -m "not gpu"): brute-force DFT, Parseval, identity
+// propagator at dz=0, propagator composition, integer tilt shift, vacuum-object invariant, SPOA
+// special case, phase-ramp object, loss closed forms, dot-product adjoint tests, central finite
+// differences of the whole loss, zero gradient at the truth, torch.fft+autograd (complex128)
+// cross-check, LSQML line-search optimum.  "Absolute values vs the paper": parity unpinned —
+// the paper prints no numeric example.
+//
+// Notation follows PAPER.md §III: probe modes P_k, object slices O_i with gaps dz_i, positions
+// X_j, exit waves Psi_{i,k}, measured I_exp.  F is the unnormalised forward DFT
+// (F a)[q] = sum_r a[r] exp(-2 pi i (qy y + qx x)/N), Finv = F^H / N^2.
+
+#include <cmath>
+#include <complex>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+typedef std::complex<double> cd;
+static const double PI = 3.14159265358979323846264338327950288;
+
+extern "C" {
+
+// ------------------------------------------------------------------------------------------
+// problem description (mirrors the paper's problem statement)
+// ------------------------------------------------------------------------------------------
+struct orc_problem {
+  int32_t n;                 // N, probe / pattern side
+  int32_t n_modes;           // M incoherent probe modes
+  int32_t n_slices;          // S object slices
+  int32_t obj_ny, obj_nx;    // object slice size (px)
+  int32_t n_pos_total;       // rows of positions / intensity
+  int32_t n_batch;           // J positions in this group
+  float pixel_size;          // Angstrom / px (float32: the same value the GPU receives)
+  float wavelength;          // Angstrom
+  const float* slice_thickness;  // S entries, last unused (reading R10)
+  float tilt_x_mrad, tilt_y_mrad;  // propagator tilt (reading R8)
+  float bandlimit;           // fraction of Nyquist, <=0: off (reading R9)
+  int32_t loss;              // 0 amplitude, 1 Poisson
+  float loss_c;              // c of the variance-stabilising transform
+  float eps;                 // epsilon offset (readings R11..R13)
+  float lsqml_delta_o;       // delta_O of PAPER.md:219
+  float lsqml_delta_p;       // probe analogue (reading R19)
+};
+
+// ------------------------------------------------------------------------------------------
+// DFT / FFT
+// ------------------------------------------------------------------------------------------
+// naive 1-D DFT, sign=-1 forward, +1 backward (unnormalised). stride in elements.
+static void dft1_naive(int n, const cd* in, int sin, cd* out, int sout, int sign) {
+  for (int k = 0; k < n; ++k) {
+    cd acc = 0.0;
+    for (int r = 0; r < n; ++r) {
+      // reduce k*r mod n before forming the angle so the argument stays accurate
+      long kr = ((long)k * (long)r) % n;
+      double ang = sign * 2.0 * PI * (double)kr / (double)n;
+      acc += in[(long)r * sin] * cd(std::cos(ang), std::sin(ang));
+    }
+    out[(long)k * sout] = acc;
+  }
+}
+
+// simple recursive radix-2 decimation-in-time FFT, n power of two, unnormalised
+static void fft1_rec(int n, const cd* in, int sin, cd* out, int sign) {
+  if (n == 1) { out[0] = in[0]; return; }
+  int h = n / 2;
+  std::vector<cd> ev(h), od(h);
+  fft1_rec(h, in, sin * 2, ev.data(), sign);
+  fft1_rec(h, in + sin, sin * 2, od.data(), sign);
+  for (int k = 0; k < h; ++k) {
+    double ang = sign * 2.0 * PI * (double)k / (double)n;
+    cd t = cd(std::cos(ang), std::sin(ang)) * od[k];
+    out[k] = ev[k] + t;
+    out[k + h] = ev[k] - t;
+  }
+}
+
+static bool is_pow2(int n) { return n > 0 && (n & (n - 1)) == 0; }
+
+// 2-D transform of an n x n row-major field, in place. naive!=0 uses the O(n^2) 1-D DFT.
+static void xform2(int n, cd* a, int sign, int naive) {
+  std::vector<cd> line(n), res(n);
+  for (int y = 0; y < n; ++y) {           // rows (x direction)
+    for (int x = 0; x < n; ++x) line[x] = a[(long)y * n + x];
+    if (naive || !is_pow2(n)) dft1_naive(n, line.data(), 1, res.data(), 1, sign);
+    else fft1_rec(n, line.data(), 1, res.data(), sign);
+    for (int x = 0; x < n; ++x) a[(long)y * n + x] = res[x];
+  }
+  for (int x = 0; x < n; ++x) {           // columns (y direction)
+    for (int y = 0; y < n; ++y) line[y] = a[(long)y * n + x];
+    if (naive || !is_pow2(n)) dft1_naive(n, line.data(), 1, res.data(), 1, sign);
+    else fft1_rec(n, line.data(), 1, res.data(), sign);
+    for (int y = 0; y < n; ++y) a[(long)y * n + x] = res[y];
+  }
+}
+static void F2(int n, cd* a) { xform2(n, a, -1, 0); }
+static void Finv2(int n, cd* a) {
+  xform2(n, a, +1, 0);
+  double s = 1.0 / ((double)n * (double)n);
+  for (long i = 0; i < (long)n * n; ++i) a[i] *= s;
+}
+
+// exported for the pins: out = F(in) (sign=-1) or F^H(in) (sign=+1), unnormalised
+void orc_dft2_naive(int32_t n, const double* in, double* out, int32_t sign) {
+  std::vector<cd> a((long)n * n);
+  for (long i = 0; i < (long)n * n; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  xform2(n, a.data(), sign, 1);
+  for (long i = 0; i < (long)n * n; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+}
+// direct O(N^4) double sum, no row-column split (for 8x8 brute force)
+void orc_dft2_bruteforce(int32_t n, const double* in, double* out, int32_t sign) {
+  for (int qy = 0; qy < n; ++qy)
+    for (int qx = 0; qx < n; ++qx) {
+      cd acc = 0.0;
+      for (int y = 0; y < n; ++y)
+        for (int x = 0; x < n; ++x) {
+          double ang = sign * 2.0 * PI * ((double)(qy * y) + (double)(qx * x)) / (double)n;
+          acc += cd(in[2 * ((long)y * n + x)], in[2 * ((long)y * n + x) + 1]) * cd(std::cos(ang), std::sin(ang));
+        }
+      out[2 * ((long)qy * n + qx)] = acc.real();
+      out[2 * ((long)qy * n + qx) + 1] = acc.imag();
+    }
+}
+void orc_fft2(int32_t n, const double* in, double* out, int32_t sign) {
+  std::vector<cd> a((long)n * n);
+  for (long i = 0; i < (long)n * n; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  xform2(n, a.data(), sign, 0);
+  for (long i = 0; i < (long)n * n; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+}
+
+// signed frequency in cycles / px: f(n) = n/N for n < N/2, (n-N)/N otherwise (Nyquist at -1/2)
+static double freq(int n, int N) { return (n < N / 2) ? (double)n / N : (double)(n - N) / N; }
+
+// ------------------------------------------------------------------------------------------
+// O1: position split, reading R2 — done in float32, the same arithmetic as the GPU, so a
+// rounding flip at a half pixel cannot break parity; promoted to double afterwards.
+// ------------------------------------------------------------------------------------------
+void orc_position_split(float X, float px, int32_t N, int32_t* r0, float* delta) {
+  volatile float p = X / px;
+  volatile float c = p - (float)(N / 2);
+  volatile float ch = c + 0.5f;
+  float fl = std::floor(ch);
+  volatile float d = c - fl;
+  *r0 = (int32_t)fl;
+  *delta = d;
+}
+
+// O1: sub-pixel shift ramp R[q] = exp(-2 pi i (f(qy) dy + f(qx) dx))  (PAPER.md:115 P_k(r - X_j))
+static void shift_ramp(int N, double dy, double dx, cd* R) {
+  for (int qy = 0; qy < N; ++qy)
+    for (int qx = 0; qx < N; ++qx) {
+      double ang = -2.0 * PI * (freq(qy, N) * dy + freq(qx, N) * dx);
+      R[(long)qy * N + qx] = cd(std::cos(ang), std::sin(ang));
+    }
+}
+
+// O4: Fresnel propagator with tilt and band limit (readings R7,R8,R9)
+// H[q] = B[q] exp(-i pi lambda dz (kx^2+ky^2)) exp(+2 pi i dz (kx tan tx + ky tan ty))
+static void propagator(int N, double px, double lambda, double dz, double tx_mrad, double ty_mrad,
+                       double bandlimit, cd* H) {
+  double tx = std::tan(tx_mrad * 1e-3), ty = std::tan(ty_mrad * 1e-3);
+  for (int qy = 0; qy < N; ++qy)
+    for (int qx = 0; qx < N; ++qx) {
+      double fy = freq(qy, N), fx = freq(qx, N);
+      double ky = fy / px, kx = fx / px;   // cycles / Angstrom
+      double ang = -PI * lambda * dz * (kx * kx + ky * ky) + 2.0 * PI * dz * (kx * tx + ky * ty);
+      double B = 1.0;
+      if (bandlimit > 0.0) {
+        // sharp inclusive circular mask at bandlimit x Nyquist; compared on integer frequency
+        // indices (exact) against (0.5*bandlimit*N)^2
+        int iy = (qy < N / 2) ? qy : qy - N, ix = (qx < N / 2) ? qx : qx - N;
+        double lim = 0.5 * bandlimit * N;
+        B = ((double)(iy * iy + ix * ix) <= lim * lim) ? 1.0 : 0.0;
+      }
+      H[(long)qy * N + qx] = B * cd(std::cos(ang), std::sin(ang));
+    }
+}
+void orc_propagator(int32_t N, double px, double lambda, double dz, double tx_mrad, double ty_mrad,
+                    double bandlimit, double* H_out) {
+  std::vector<cd> H((long)N * N);
+  propagator(N, px, lambda, dz, tx_mrad, ty_mrad, bandlimit, H.data());
+  for (long i = 0; i < (long)N * N; ++i) { H_out[2 * i] = H[i].real(); H_out[2 * i + 1] = H[i].imag(); }
+}
+
+// the linear pieces, exported so that the dot-product tests pin the very code the model uses -----
+// out = Finv(R(dy,dx) .* F(in))        (O2 with in = P_k)
+void orc_shift(int32_t N, const double* in, double dy, double dx, double* out, int32_t adjoint) {
+  std::vector<cd> a((long)N * N), R((long)N * N);
+  for (long i = 0; i < (long)N * N; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  shift_ramp(N, dy, dx, R.data());
+  F2(N, a.data());
+  for (long i = 0; i < (long)N * N; ++i) a[i] *= adjoint ? std::conj(R[i]) : R[i];
+  Finv2(N, a.data());
+  for (long i = 0; i < (long)N * N; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+}
+// out = Finv(H .* F(in)), or with adjoint: Finv(conj(H) .* F(in))   (O3 / O8)
+void orc_propagate(int32_t N, const double* in, double px, double lambda, double dz, double tx_mrad,
+                   double ty_mrad, double bandlimit, double* out, int32_t adjoint) {
+  std::vector<cd> a((long)N * N), H((long)N * N);
+  for (long i = 0; i < (long)N * N; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  propagator(N, px, lambda, dz, tx_mrad, ty_mrad, bandlimit, H.data());
+  F2(N, a.data());
+  for (long i = 0; i < (long)N * N; ++i) a[i] *= adjoint ? std::conj(H[i]) : H[i];
+  Finv2(N, a.data());
+  for (long i = 0; i < (long)N * N; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+}
+// patch[r] = obj[r0 + r]   (O3)
+void orc_gather(int32_t N, int32_t ony, int32_t onx, const double* obj, int32_t r0y, int32_t r0x, double* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x)
+      for (int c = 0; c < 2; ++c)
+        patch[2 * ((long)y * N + x) + c] = obj[2 * ((long)(r0y + y) * onx + (r0x + x)) + c];
+  (void)ony;
+}
+// obj[r0 + r] += patch[r]  (O8 last line)
+void orc_scatter_add(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t r0y, int32_t r0x, const double* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x)
+      for (int c = 0; c < 2; ++c)
+        obj[2 * ((long)(r0y + y) * onx + (r0x + x)) + c] += patch[2 * ((long)y * N + x) + c];
+  (void)ony;
+}
+
+// O6: per-pixel loss l(I, Iexp) and detector weight w = dl/dI
+// Poisson (PAPER.md:151 Stirling form, epsilon inside both logarithms — reading R11; w = PAPER.md:165)
+// Amplitude/Anscombe (PAPER.md:157 as printed; w = its derivative regularised as PAPER.md:167 — reading R12)
+void orc_loss_pixel(int32_t kind, double I, double Iexp, double c, double eps, double* l, double* w) {
+  if (kind == 1) {
+    *l = I - Iexp * (std::log(I + eps) - std::log(Iexp + eps) + 1.0);
+    *w = 1.0 - Iexp / (I + eps);
+  } else {
+    double a = std::sqrt(I + c), ae = std::sqrt(Iexp + c);
+    *l = 0.5 * (a - ae) * (a - ae);
+    *w = 0.5 * (1.0 - ae / (a + eps));
+  }
+}
+
+}  // extern "C" (helpers below are C++)
+
+// ------------------------------------------------------------------------------------------
+// one position: forward (O1..O6) and, optionally, adjoint (O7..O10)
+// ------------------------------------------------------------------------------------------
+struct PosWork {
+  int N, M, S;
+  std::vector<cd> R;                 // shift ramp
+  std::vector<std::vector<cd>> Psi;  // [i*M+k] entering wave of slice i, mode k
+  std::vector<std::vector<cd>> T;    // [i] object patch
+  std::vector<std::vector<cd>> psit; // [k] far field / N
+  std::vector<std::vector<cd>> gPhi; // [i*M+k] gradient wrt the exit wave of slice i (only kept when asked)
+  std::vector<double> I;
+  int r0y, r0x; double dy, dx;
+};
+
+struct Model {
+  orc_problem p;
+  int N, M, S;
+  long NN;
+  std::vector<std::vector<cd>> Pt;   // F(P_k)           (O0)
+  std::vector<std::vector<cd>> H;    // H_i, i<S-1       (O4)
+  std::vector<cd> obj;               // [S][ony][onx]
+  const float* positions; const float* intensity; const int32_t* batch_idx;
+};
+
+static void model_init(Model& m, const orc_problem* p, const float* object, const float* probe,
+                       const float* positions, const float* intensity, const int32_t* batch_idx) {
+  m.p = *p; m.N = p->n; m.M = p->n_modes; m.S = p->n_slices; m.NN = (long)p->n * p->n;
+  m.positions = positions; m.intensity = intensity; m.batch_idx = batch_idx;
+  long on = (long)p->n_slices * p->obj_ny * p->obj_nx;
+  m.obj.resize(on);
+  for (long i = 0; i < on; ++i) m.obj[i] = cd(object[2 * i], object[2 * i + 1]);
+  m.Pt.assign(m.M, std::vector<cd>(m.NN));
+  for (int k = 0; k < m.M; ++k) {
+    for (long i = 0; i < m.NN; ++i) m.Pt[k][i] = cd(probe[2 * (k * m.NN + i)], probe[2 * (k * m.NN + i) + 1]);
+    F2(m.N, m.Pt[k].data());                                                    // O0
+  }
+  m.H.assign(m.S > 1 ? m.S - 1 : 0, std::vector<cd>(m.NN));
+  for (int i = 0; i + 1 < m.S; ++i)
+    propagator(m.N, (double)p->pixel_size, (double)p->wavelength, (double)p->slice_thickness[i],
+               (double)p->tilt_x_mrad, (double)p->tilt_y_mrad, (double)p->bandlimit, m.H[i].data());
+}
+
+// returns 0, or -1 if the window leaves the object (reading R4)
+static int forward_pos(const Model& m, int jrow, PosWork& w) {
+  const int N = m.N, M = m.M, S = m.S; const long NN = m.NN;
+  const orc_problem& p = m.p;
+  w.N = N; w.M = M; w.S = S;
+  float dyf, dxf; int32_t r0y, r0x;
+  orc_position_split(m.positions[2 * jrow + 0], p.pixel_size, N, &r0y, &dyf);   // O1
+  orc_position_split(m.positions[2 * jrow + 1], p.pixel_size, N, &r0x, &dxf);
+  if (r0y < 0 || r0x < 0 || r0y + N > p.obj_ny || r0x + N > p.obj_nx) return -1;
+  w.r0y = r0y; w.r0x = r0x; w.dy = (double)dyf; w.dx = (double)dxf;
+  w.R.resize(NN); shift_ramp(N, w.dy, w.dx, w.R.data());
+  w.Psi.assign((long)S * M, std::vector<cd>()); w.T.assign(S, std::vector<cd>(NN));
+  w.psit.assign(M, std::vector<cd>(NN)); w.I.assign(NN, 0.0);
+  for (int i = 0; i < S; ++i)                                                    // O3: T_i[r] = O_i[r0 + r]
+    for (int y = 0; y < N; ++y)
+      for (int x = 0; x < N; ++x)
+        w.T[i][(long)y * N + x] = m.obj[((long)i * p.obj_ny + (r0y + y)) * p.obj_nx + (r0x + x)];
+  for (int k = 0; k < M; ++k) {
+    std::vector<cd> cur(NN);
+    for (long q = 0; q < NN; ++q) cur[q] = w.R[q] * m.Pt[k][q];                  // O2
+    Finv2(N, cur.data());
+    for (int i = 0; i < S; ++i) {
+      w.Psi[(long)i * M + k] = cur;                                              // entering wave Psi_{i,k}
+      for (long r = 0; r < NN; ++r) cur[r] *= w.T[i][r];                         // Phi_{i,k} = Psi .* T
+      if (i < S - 1) {                                                           // O3 propagate (reading R10: none after the last slice)
+        F2(N, cur.data());
+        for (long q = 0; q < NN; ++q) cur[q] *= m.H[i][q];
+        Finv2(N, cur.data());
+      }
+    }
+    F2(N, cur.data());                                                           // O5 far field, orthonormal (reading R5)
+    for (long q = 0; q < NN; ++q) { cur[q] /= (double)N; w.I[q] += std::norm(cur[q]); }
+    w.psit[k] = cur;
+  }
+  return 0;
+}
+
+// adjoint O7..O10 for one position. gT[i] (N x N) is overwritten; gPt_acc[k] += conj(R) .* G~_k;
+// gdelta[2] = dL/d(delta_y, delta_x).  If keep_gphi, w.gPhi[i*M+k] keeps gPhi_{i,k} (for O14).
+static void adjoint_pos(const Model& m, int jrow, PosWork& w, double* loss_j,
+                        std::vector<std::vector<cd>>& gT, std::vector<std::vector<cd>>* gPt_acc,
+                        double* gdelta, bool keep_gphi) {
+  const int N = m.N, M = m.M, S = m.S; const long NN = m.NN; const orc_problem& p = m.p;
+  std::vector<double> wdet(NN);
+  double L = 0.0;
+  const float* Iexp = m.intensity + (long)jrow * NN;
+  for (long q = 0; q < NN; ++q) {                                                // O6
+    double l, ww; orc_loss_pixel(p.loss, w.I[q], (double)Iexp[q], (double)p.loss_c, (double)p.eps, &l, &ww);
+    L += l; wdet[q] = ww;
+  }
+  *loss_j = L;
+  gT.assign(S, std::vector<cd>(NN, cd(0.0)));
+  if (keep_gphi) w.gPhi.assign((long)S * M, std::vector<cd>());
+  gdelta[0] = gdelta[1] = 0.0;
+  for (int k = 0; k < M; ++k) {
+    std::vector<cd> g(NN);
+    for (long q = 0; q < NN; ++q) g[q] = wdet[q] * w.psit[k][q];                 // O7: g~ = w .* psi~
+    Finv2(N, g.data());
+    for (long r = 0; r < NN; ++r) g[r] *= (double)N;                             //     gPhi_{S-1} = N Finv(g~)
+    for (int i = S - 1; i >= 0; --i) {                                           // O8
+      if (keep_gphi) w.gPhi[(long)i * M + k] = g;
+      const std::vector<cd>& Psi = w.Psi[(long)i * M + k];
+      for (long r = 0; r < NN; ++r) gT[i][r] += std::conj(Psi[r]) * g[r];        // gT_i += conj(Psi) .* gPhi
+      for (long r = 0; r < NN; ++r) g[r] = std::conj(w.T[i][r]) * g[r];          // gPsi = conj(T) .* gPhi
+      if (i > 0) {
+        F2(N, g.data());
+        for (long q = 0; q < NN; ++q) g[q] *= std::conj(m.H[i - 1][q]);
+        Finv2(N, g.data());                                                      // gPhi_{i-1}
+      }
+    }
+    F2(N, g.data());                                                             // O9: G~ = F(gPsi_0)
+    if (gPt_acc)
+      for (long q = 0; q < NN; ++q) (*gPt_acc)[k][q] += std::conj(w.R[q]) * g[q];
+    for (int a = 0; a < 2; ++a) {                                                // O10
+      cd acc = 0.0;
+      for (int qy = 0; qy < N; ++qy)
+        for (int qx = 0; qx < N; ++qx) {
+          long q = (long)qy * N + qx;
+          double fa = (a == 0) ? freq(qy, N) : freq(qx, N);
+          acc += std::conj(g[q]) * cd(0.0, -2.0 * PI * fa) * w.R[q] * m.Pt[k][q];
+        }
+      gdelta[a] += 2.0 * acc.real() / ((double)N * N);
+    }
+  }
+}
+
+static int row_of(const Model& m, int jb) { return m.batch_idx ? m.batch_idx[jb] : jb; }
+
+extern "C" {
+
+// ------------------------------------------------------------------------------------------
+// forward + loss (O0..O6).  Outputs may be NULL.  Returns 0, -1 out of bounds.
+// ------------------------------------------------------------------------------------------
+int32_t orc_forward_loss(const orc_problem* p, const float* object, const float* probe,
+                         const float* positions, const float* intensity, const int32_t* batch_idx,
+                         double* loss, double* loss_per_pos, double* model_intensity) {
+  Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
+  const int J = p->n_batch; int err = 0;
+  std::vector<double> Lj(J, 0.0);
+#pragma omp parallel for schedule(dynamic)
+  for (int jb = 0; jb < J; ++jb) {
+    PosWork w; int jrow = row_of(m, jb);
+    if (forward_pos(m, jrow, w) != 0) {
+#pragma omp atomic write
+      err = -1;
+      continue;
+    }
+    if (model_intensity) for (long q = 0; q < m.NN; ++q) model_intensity[(long)jb * m.NN + q] = w.I[q];
+    if (intensity) {
+      double L = 0.0; const float* Iexp = intensity + (long)jrow * m.NN;
+      for (long q = 0; q < m.NN; ++q) { double l, ww; orc_loss_pixel(p->loss, w.I[q], (double)Iexp[q], (double)p->loss_c, (double)p->eps, &l, &ww); L += l; }
+      Lj[jb] = L;
+    }
+  }
+  double L = 0.0; for (int jb = 0; jb < J; ++jb) { L += Lj[jb]; if (loss_per_pos) loss_per_pos[jb] = Lj[jb]; }
+  if (loss) *loss = L;
+  return err;
+}
+
+// ------------------------------------------------------------------------------------------
+// loss + gradients (O0..O11) and the illumination map (O12).
+//   grad_object [S][ony][onx] complex, grad_probe [M][N][N] complex   (dL/d conj(.))
+//   grad_pos [J][2]  dL/dX per Angstrom (O10), illum [S][ony][onx] real — any may be NULL
+// ------------------------------------------------------------------------------------------
+int32_t orc_gradient(const orc_problem* p, const float* object, const float* probe,
+                     const float* positions, const float* intensity, const int32_t* batch_idx,
+                     double* grad_object, double* grad_probe, double* grad_pos, double* illum,
+                     double* loss, double* loss_per_pos) {
+  Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
+  const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const long NN = m.NN;
+  const long on = (long)S * p->obj_ny * p->obj_nx;
+  int err = 0;
+  std::vector<double> Lj(J, 0.0);
+  std::vector<cd> gO(on, cd(0.0)); std::vector<double> il(illum ? on : 0, 0.0);
+  std::vector<std::vector<cd>> gPt(M, std::vector<cd>(NN, cd(0.0)));
+#pragma omp parallel
+  {
+    std::vector<cd> gO_loc(on, cd(0.0)); std::vector<double> il_loc(illum ? on : 0, 0.0);
+    std::vector<std::vector<cd>> gPt_loc(M, std::vector<cd>(NN, cd(0.0)));
+#pragma omp for schedule(dynamic)
+    for (int jb = 0; jb < J; ++jb) {
+      PosWork w; int jrow = row_of(m, jb);
+      if (forward_pos(m, jrow, w) != 0) {
+#pragma omp atomic write
+        err = -1;
+        continue;
+      }
+      std::vector<std::vector<cd>> gT; double gd[2];
+      adjoint_pos(m, jrow, w, &Lj[jb], gT, &gPt_loc, gd, false);
+      for (int i = 0; i < S; ++i)                                               // O8 last line: scatter-add
+        for (int y = 0; y < N; ++y)
+          for (int x = 0; x < N; ++x) {
+            long o = ((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x);
+            gO_loc[o] += gT[i][(long)y * N + x];
+            if (illum) {                                                        // O12
+              double s = 0.0; for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][(long)y * N + x]);
+              il_loc[o] += s;
+            }
+          }
+      if (grad_pos) { grad_pos[2 * jb + 0] = gd[0] / (double)p->pixel_size; grad_pos[2 * jb + 1] = gd[1] / (double)p->pixel_size; }
+    }
+#pragma omp critical
+    {
+      for (long o = 0; o < on; ++o) gO[o] += gO_loc[o];
+      if (illum) for (long o = 0; o < on; ++o) il[o] += il_loc[o];
+      for (int k = 0; k < M; ++k) for (long q = 0; q < NN; ++q) gPt[k][q] += gPt_loc[k][q];
+    }
+  }
+  if (grad_object) for (long o = 0; o < on; ++o) { grad_object[2 * o] = gO[o].real(); grad_object[2 * o + 1] = gO[o].imag(); }
+  if (illum) for (long o = 0; o < on; ++o) illum[o] = il[o];
+  if (grad_probe)
+    for (int k = 0; k < M; ++k) {                                               // O11
+      Finv2(N, gPt[k].data());
+      for (long r = 0; r < NN; ++r) { grad_probe[2 * (k * NN + r)] = gPt[k][r].real(); grad_probe[2 * (k * NN + r) + 1] = gPt[k][r].imag(); }
+    }
+  double L = 0.0; for (int jb = 0; jb < J; ++jb) { L += Lj[jb]; if (loss_per_pos) loss_per_pos[jb] = Lj[jb]; }
+  if (loss) *loss = L;
+  return err;
+}
+
+// ------------------------------------------------------------------------------------------
+// O13/O14: LSQML-style step-size terms, second sweep over the batch.
+//   grad_object/grad_probe: the batch-aggregated gradients (double, as returned by orc_gradient)
+//   illum_prev: [S][ony][onx] running probe-intensity sum of the previous iteration
+//   step_terms: [J][2S+6]:  (numO,denO) per slice, (numP,denP), (numX_y,denX_y), (numX_x,denX_x)
+// chi_{i,k} := -gPhi_{i,k} (steepest-descent wavefront update, reading R20)
+// ------------------------------------------------------------------------------------------
+int32_t orc_step_terms(const orc_problem* p, const float* object, const float* probe,
+                       const float* positions, const float* intensity, const int32_t* batch_idx,
+                       const double* grad_object, const double* grad_probe, const double* illum_prev,
+                       double* step_terms) {
+  Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
+  const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const long NN = m.NN;
+  const long on = (long)S * p->obj_ny * p->obj_nx;
+  std::vector<cd> dOhat(on);
+  for (long o = 0; o < on; ++o)                                                 // O13
+    dOhat[o] = -cd(grad_object[2 * o], grad_object[2 * o + 1]) / (illum_prev[o] + (double)p->lsqml_delta_o);
+  std::vector<std::vector<cd>> dPhat_t(M, std::vector<cd>(NN));                 // F(dPhat_k)
+  for (int k = 0; k < M; ++k) {
+    for (long r = 0; r < NN; ++r) dPhat_t[k][r] = -cd(grad_probe[2 * (k * NN + r)], grad_probe[2 * (k * NN + r) + 1]) / ((double)p->lsqml_delta_p + 1.0);
+    F2(N, dPhat_t[k].data());
+  }
+  int err = 0; const int W = 2 * S + 6;
+#pragma omp parallel for schedule(dynamic)
+  for (int jb = 0; jb < J; ++jb) {
+    PosWork w; int jrow = row_of(m, jb);
+    if (forward_pos(m, jrow, w) != 0) {
+#pragma omp atomic write
+      err = -1;
+      continue;
+    }
+    std::vector<std::vector<cd>> gT; double gd[2], Lj;
+    adjoint_pos(m, jrow, w, &Lj, gT, nullptr, gd, true);
+    double* out = step_terms + (long)jb * W;
+    for (int i = 0; i < S; ++i) {                                               // O14 object
+      double num = 0.0, den = 0.0;
+      for (int k = 0; k < M; ++k)
+        for (int y = 0; y < N; ++y)
+          for (int x = 0; x < N; ++x) {
+            long r = (long)y * N + x;
+            cd u = dOhat[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] * w.Psi[(long)i * M + k][r];
+            cd chi = -w.gPhi[(long)i * M + k][r];
+            num += (chi * std::conj(u)).real(); den += std::norm(u);
+          }
+      out[2 * i] = num; out[2 * i + 1] = den;
+    }
+    double numP = 0, denP = 0, numX[2] = {0, 0}, denX[2] = {0, 0};
+    for (int k = 0; k < M; ++k) {
+      std::vector<cd> v(NN);
+      for (long q = 0; q < NN; ++q) v[q] = w.R[q] * dPhat_t[k][q];              // shift_j(dPhat_k)
+      Finv2(N, v.data());
+      for (long r = 0; r < NN; ++r) {
+        cd vv = v[r] * w.T[0][r]; cd chi = -w.gPhi[k][r];                       // slice 0: index 0*M+k
+        numP += (chi * std::conj(vv)).real(); denP += std::norm(vv);
+      }
+      for (int a = 0; a < 2; ++a) {
+        std::vector<cd> s(NN);
+        for (int qy = 0; qy < N; ++qy)
+          for (int qx = 0; qx < N; ++qx) {
+            long q = (long)qy * N + qx; double fa = (a == 0) ? freq(qy, N) : freq(qx, N);
+            s[q] = cd(0.0, -2.0 * PI * fa) * w.R[q] * m.Pt[k][q];               // d Psi_0 / d delta_a, Fourier side
+          }
+        Finv2(N, s.data());
+        for (long r = 0; r < NN; ++r) {
+          cd ss = s[r] * w.T[0][r]; cd chi = -w.gPhi[k][r];
+          numX[a] += (chi * std::conj(ss)).real(); denX[a] += std::norm(ss);
+        }
+      }
+    }
+    out[2 * S + 0] = numP; out[2 * S + 1] = denP;
+    out[2 * S + 2] = numX[0]; out[2 * S + 3] = denX[0];
+    out[2 * S + 4] = numX[1]; out[2 * S + 5] = denX[1];
+  }
+  return err;
+}
+
+// ------------------------------------------------------------------------------------------
+// O15 / H15 update.  mode 0: SGD z <- z - lr g.  mode 1: LSQML-style (R18):
+//   alpha_{O,i} = sum_j numO / (sum_j denO + gamma);  O_i += beta_O alpha_{O,i} dOhat_i   etc.
+// object/probe/positions are double in/out here (the test converts); positions rows batch_idx only.
+// ------------------------------------------------------------------------------------------
+int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, double* probe, double* positions,
+                         const double* grad_object, const double* grad_probe, const double* grad_pos,
+                         const double* illum_prev, const double* step_terms, const int32_t* batch_idx,
+                         double lr_obj, double lr_probe, double lr_pos, double beta_obj, double beta_probe,
+                         double gamma) {
+  const int J = p->n_batch, M = p->n_modes, S = p->n_slices; const long NN = (long)p->n * p->n;
+  const long os = (long)p->obj_ny * p->obj_nx;
+  if (mode == 0) {
+    if (object && grad_object) for (long o = 0; o < 2 * S * os; ++o) object[o] -= lr_obj * grad_object[o];
+    if (probe && grad_probe) for (long r = 0; r < 2 * M * NN; ++r) probe[r] -= lr_probe * grad_probe[r];
+    if (positions && grad_pos)
+      for (int jb = 0; jb < J; ++jb) { int row = batch_idx ? batch_idx[jb] : jb;
+        positions[2 * row] -= lr_pos * grad_pos[2 * jb]; positions[2 * row + 1] -= lr_pos * grad_pos[2 * jb + 1]; }
+    return 0;
+  }
+  const int W = 2 * S + 6;
+  if (object && grad_object)
+    for (int i = 0; i < S; ++i) {
+      double num = 0, den = 0;
+      for (int jb = 0; jb < J; ++jb) { num += step_terms[(long)jb * W + 2 * i]; den += step_terms[(long)jb * W + 2 * i + 1]; }
+      double alpha = num / (den + gamma);
+      for (long o = 0; o < os; ++o) {
+        long g = (long)i * os + o; double d = illum_prev[g] + (double)p->lsqml_delta_o;
+        object[2 * g] += beta_obj * alpha * (-grad_object[2 * g] / d);
+        object[2 * g + 1] += beta_obj * alpha * (-grad_object[2 * g + 1] / d);
+      }
+    }
+  if (probe && grad_probe) {
+    double num = 0, den = 0;
+    for (int jb = 0; jb < J; ++jb) { num += step_terms[(long)jb * W + 2 * S]; den += step_terms[(long)jb * W + 2 * S + 1]; }
+    double alpha = num / (den + gamma);
+    for (long r = 0; r < 2 * M * NN; ++r) probe[r] += beta_probe * alpha * (-grad_probe[r] / ((double)p->lsqml_delta_p + 1.0));
+  }
+  if (positions)
+    for (int jb = 0; jb < J; ++jb) { int row = batch_idx ? batch_idx[jb] : jb;
+      for (int a = 0; a < 2; ++a) {
+        double num = step_terms[(long)jb * W + 2 * S + 2 + 2 * a], den = step_terms[(long)jb * W + 2 * S + 3 + 2 * a];
+        positions[2 * row + a] += (double)p->pixel_size * num / (den + gamma);
+      } }
+  return 0;
+}
+
+int32_t orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

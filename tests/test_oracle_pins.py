@@ -1,0 +1,497 @@
+"""Pins for the CPU oracle (oracle/ptycho_oracle.cpp) against what the paper and the mathematics fix.
+
+None of these call the CUDA path.  Each test names the passage (PAPER.md line / DESIGN.md reading) it pins.
+The paper prints no numeric worked example, so the pins are closed forms, invariants,
+library routines on special cases (numpy.fft), brute force on tiny inputs, central finite differences and
+an autograd (torch, complex128) re-derivation of the adjoint.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+
+RNG = np.random.default_rng(12345)
+
+
+def crandn(*shape):
+    return RNG.standard_normal(shape) + 1j * RNG.standard_normal(shape)
+
+
+# ------------------------------------------------------------------------------------------------
+# FFT (O0, O2, O3, O5)  — definitions block of DESIGN.md §2
+# ------------------------------------------------------------------------------------------------
+def test_dft_bruteforce_8x8():
+    a = crandn(8, 8)
+    ref = orc.dft2_bruteforce(a, -1)           # direct O(N^4) double sum
+    assert np.abs(orc.fft2(a, -1) - ref).max() < 1e-12
+    assert np.abs(orc.dft2_naive(a, -1) - ref).max() < 1e-12
+    # sign convention: forward kernel exp(-2 pi i q r / N) == numpy.fft.fft2
+    assert np.abs(ref - np.fft.fft2(a)).max() < 1e-12
+    assert np.abs(orc.dft2_bruteforce(a, +1) - np.fft.ifft2(a) * 64).max() < 1e-12
+
+
+def test_fft_inverse_parseval_delta():
+    for n in (8, 64):
+        a = crandn(n, n)
+        A = orc.fft2(a, -1)
+        assert np.abs(orc.fft2(A, +1) / n ** 2 - a).max() < 1e-12            # Finv F = id
+        assert abs(np.sum(np.abs(A) ** 2) - n ** 2 * np.sum(np.abs(a) ** 2)) < 1e-9 * n ** 2 * np.sum(np.abs(a) ** 2)
+        d = np.zeros((n, n), complex); d[0, 0] = 1.0
+        assert np.abs(orc.fft2(d, -1) - 1.0).max() < 1e-13                   # delta <-> constant
+        d = np.zeros((n, n), complex); d[3, 5] = 1.0                         # shifted delta <-> plane wave
+        qy, qx = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+        assert np.abs(orc.fft2(d, -1) - np.exp(-2j * np.pi * (3 * qy + 5 * qx) / n)).max() < 1e-12
+
+
+def test_recursive_fft_vs_naive_dft_64_and_128():
+    for n in (64, 128):
+        a = crandn(n, n)
+        assert np.abs(orc.fft2(a, -1) - orc.dft2_naive(a, -1)).max() < 1e-9
+        assert np.abs(orc.fft2(a, -1) - np.fft.fft2(a)).max() < 1e-9
+
+
+# ------------------------------------------------------------------------------------------------
+# position split (O1, reading R2)
+# ------------------------------------------------------------------------------------------------
+def test_position_split():
+    # p = X/px, c = p - N/2, r0 = floor(c + 1/2), delta = c - r0 in [-1/2, 1/2)
+    assert orc.position_split(40.0, 1.0, 64) == (8, 0.0)
+    r0, d = orc.position_split(40.25, 1.0, 64); assert r0 == 8 and abs(d - 0.25) < 1e-7
+    r0, d = orc.position_split(40.5, 1.0, 64); assert r0 == 9 and abs(d + 0.5) < 1e-7     # round half up
+    r0, d = orc.position_split(40.75, 1.0, 64); assert r0 == 9 and abs(d + 0.25) < 1e-7
+    r0, d = orc.position_split(4.06, 0.1, 64); assert r0 == 9 and abs(d - (-0.4)) < 1e-5
+    for X in RNG.uniform(10, 40, 200):
+        r0, d = orc.position_split(float(np.float32(X)), 0.1, 128)
+        assert -0.5 <= d < 0.5
+        assert abs((r0 + d) - (np.float32(X) / np.float32(0.1) - 64)) < 1e-4
+
+
+# ------------------------------------------------------------------------------------------------
+# sub-pixel shift (O1, O2; PAPER.md:115 P_k(r - X_j))
+# ------------------------------------------------------------------------------------------------
+def test_shift_integer_is_roll_and_inverse():
+    a = crandn(16, 16)
+    # delta = +1 moves content to the next higher index: out[r] = in[r - delta]
+    assert np.abs(orc.shift(a, 1.0, 0.0) - np.roll(a, 1, axis=0)).max() < 1e-12
+    assert np.abs(orc.shift(a, 0.0, -3.0) - np.roll(a, -3, axis=1)).max() < 1e-12
+    b = orc.shift(orc.shift(a, 0.3, -0.2), -0.3, 0.2)
+    assert np.abs(b - a).max() < 1e-12
+    s = orc.shift(a, 0.37, 0.11)
+    assert abs(np.sum(np.abs(s) ** 2) - np.sum(np.abs(a) ** 2)) < 1e-10
+    # band-limited signal: shift equals evaluating the trigonometric interpolant
+    n = 16; y, x = np.meshgrid(np.arange(n), np.arange(n), indexing="ij")
+    f = lambda yy, xx: np.exp(2j * np.pi * (2 * yy - 3 * xx) / n) + 0.5 * np.exp(2j * np.pi * (-5 * yy + 1 * xx) / n)
+    assert np.abs(orc.shift(f(y, x), 0.3, -0.45) - f(y - 0.3, x + 0.45)).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# propagator (O3, O4; readings R7, R8, R9)
+# ------------------------------------------------------------------------------------------------
+def test_propagator_identity_composition_unit_modulus():
+    a = crandn(16, 16)
+    assert np.abs(orc.propagate(a, 0.1, 0.0197, 0.0, 0.8, 0.6) - a).max() < 1e-12         # dz = 0 -> identity
+    H1 = orc.propagator(16, 0.1, 0.0197, 7.0, 0.8, 0.6)
+    H2 = orc.propagator(16, 0.1, 0.0197, 5.0, 0.8, 0.6)
+    H3 = orc.propagator(16, 0.1, 0.0197, 12.0, 0.8, 0.6)
+    assert np.abs(H1 * H2 - H3).max() < 1e-12                                             # H(a)H(b) = H(a+b)
+    assert np.abs(np.abs(H1) - 1.0).max() < 1e-14                                         # |H| = 1 without mask
+    b = orc.propagate(a, 0.1, 0.0197, 9.0, 0.8, 0.6)
+    assert abs(np.sum(np.abs(b) ** 2) - np.sum(np.abs(a) ** 2)) < 1e-10
+
+
+def test_propagator_tilt_integer_shift_sign():
+    # R8: exp(+2 pi i dz (kx tan tx + ky tan ty)); with dz*tan(theta)/px = +m px the field moves by -m px.
+    n, px = 16, 0.1
+    a = crandn(n, n)
+    dz = 100.0
+    tx_mrad = np.arctan(2 * px / dz) * 1e3         # dz tan(tx) = +2 px
+    ty_mrad = np.arctan(-3 * px / dz) * 1e3        # dz tan(ty) = -3 px
+    # lambda = 0 removes the Fresnel term, leaving the pure tilt
+    out = orc.propagate(a, px, 0.0, dz, tx_mrad, ty_mrad)
+    assert np.abs(out - np.roll(np.roll(a, -2, axis=1), +3, axis=0)).max() < 1e-10
+
+
+def test_propagator_gaussian_closed_form():
+    # Fresnel sign/units (R7): H = exp(-i pi lambda dz k^2), k in cycles/Angstrom.  A Gaussian
+    # exp(-r^2/(2 s^2)) propagates to (s^2/s'^2) exp(-r^2/(2 s'^2)) with s'^2 = s^2 + i lambda dz/(2 pi).
+    n, px, lam, dz, s = 128, 0.1, 0.0197, 40.0, 0.5
+    r = (np.arange(n) - n // 2) * px
+    Y, X = np.meshgrid(r, r, indexing="ij")
+    g = np.exp(-(X ** 2 + Y ** 2) / (2 * s ** 2))
+    s2 = s ** 2 + 1j * lam * dz / (2 * np.pi)
+    ref = (s ** 2 / s2) * np.exp(-(X ** 2 + Y ** 2) / (2 * s2))
+    out = orc.propagate(g, px, lam, dz)
+    assert np.abs(out - ref).max() < 1e-8
+
+
+def test_bandlimit_mask():
+    n = 32
+    H = orc.propagator(n, 0.1, 0.0197, 10.0, 0.0, 0.0, 2.0 / 3.0)
+    s = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n)
+    QY, QX = np.meshgrid(s, s, indexing="ij")
+    inside = (QY ** 2 + QX ** 2) <= (0.5 * (2.0 / 3.0) * n) ** 2
+    assert np.all(np.abs(np.abs(H) - inside) < 1e-14)
+    assert 0 < inside.sum() < n * n
+
+
+# ------------------------------------------------------------------------------------------------
+# whole forward (O1..O5; readings R5, R6, R10)
+# ------------------------------------------------------------------------------------------------
+def small_problem(n=8, M=2, S=3, on=20, J=3, loss=orc.LOSS_POISSON, eps=0.3, bandlimit=0.0, c=0.0, tilt=(30.0, -20.0)):
+    pb = orc.Problem(n=n, n_modes=M, n_slices=S, obj_ny=on, obj_nx=on + 2, pixel_size=0.2, wavelength=0.05,
+                     slice_thickness=[3.0 + 0.5 * i for i in range(S)], tilt_x_mrad=tilt[0], tilt_y_mrad=tilt[1],
+                     bandlimit=bandlimit, loss=loss, loss_c=c, eps=eps)
+    obj = (np.exp(0.3 * crandn(S, on, on + 2))).astype(np.complex64)
+    probe = crandn(M, n, n).astype(np.complex64)
+    pos_px = RNG.uniform(n / 2 + 1.0, on - n / 2 - 1.0, size=(J, 2))
+    pos = (pos_px * 0.2).astype(np.float32)
+    return pb, obj, probe, pos
+
+
+def test_forward_vacuum_invariant():
+    # O == 1: every pattern equals sum_k |F(P_k)|^2 / N^2, for any S, dz, tilt, positions
+    pb, obj, probe, pos = small_problem(n=16, M=3, S=4, on=40, J=5)
+    obj[:] = 1.0
+    out = orc.forward_loss(pb, obj, probe, pos)
+    ref = sum(np.abs(np.fft.fft2(probe[k].astype(complex))) ** 2 for k in range(3)) / 16 ** 2
+    for j in range(5):
+        assert np.abs(out["intensity"][j] - ref).max() < 1e-10 * ref.max()
+
+
+def test_forward_spoa_single_slice_matches_numpy():
+    # S = 1 reduces to |F(P_shift . O_patch)|^2 / N^2 (SPOA; BASELINE.json config 1)
+    n, on = 16, 40
+    pb, obj, probe, pos = small_problem(n=n, M=2, S=1, on=on, J=4)
+    out = orc.forward_loss(pb, obj, probe, pos)
+    s = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n) / n
+    for j in range(4):
+        c = pos[j].astype(np.float64) / 0.2 - n / 2          # exact here: compare r0/delta to the fp32 split
+        r0 = np.floor(c + 0.5).astype(int); d = c - r0
+        r0y, dy = orc.position_split(float(pos[j, 0]), 0.2, n); r0x, dx = orc.position_split(float(pos[j, 1]), 0.2, n)
+        assert (r0y, r0x) == (r0[0], r0[1]) and abs(dy - d[0]) < 1e-5 and abs(dx - d[1]) < 1e-5
+        R = np.exp(-2j * np.pi * (s[:, None] * dy + s[None, :] * dx))
+        I = np.zeros((n, n))
+        for k in range(2):
+            Ps = np.fft.ifft2(R * np.fft.fft2(probe[k].astype(complex)))
+            patch = obj[0, r0y:r0y + n, r0x:r0x + n].astype(complex)
+            I += np.abs(np.fft.fft2(Ps * patch)) ** 2 / n ** 2
+        assert np.abs(out["intensity"][j] - I).max() < 1e-10 * I.max()
+        # electron count (Parseval, reading R5)
+        assert abs(out["intensity"][j].sum() - sum(np.sum(np.abs(np.fft.ifft2(R * np.fft.fft2(probe[k].astype(complex))) * patch) ** 2) for k in range(2))) < 1e-9 * I.sum()
+
+
+def test_forward_phase_ramp_object_shifts_pattern():
+    # integer-linear phase ramp exp(2 pi i a.r/N) at S = 1 circularly shifts the pattern by a
+    n, on = 16, 40
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=2)
+    y, x = np.meshgrid(np.arange(on), np.arange(on + 2), indexing="ij")
+    obj0 = np.ones_like(obj)
+    obj1 = np.exp(2j * np.pi * (3 * y - 2 * x) / n)[None].astype(np.complex64)
+    I0 = orc.forward_loss(pb, obj0, probe, pos)["intensity"]
+    I1 = orc.forward_loss(pb, obj1, probe, pos)["intensity"]
+    for j in range(2):
+        assert np.abs(I1[j] - np.roll(np.roll(I0[j], 3, axis=0), -2, axis=1)).max() < 1e-5 * I0[j].max()
+
+
+def test_forward_translation_covariance_and_scaling_ambiguity():
+    pb, obj, probe, pos = small_problem(n=8, M=2, S=3, on=24, J=3)
+    pos = np.clip(pos, (8 / 2 + 1) * 0.2, (24 - 8 / 2 - 4) * 0.2).astype(np.float32)
+    I0 = orc.forward_loss(pb, obj, probe, pos)["intensity"]
+    obj_s = np.roll(np.roll(obj, 2, axis=1), 1, axis=2)
+    pos_s = (pos.astype(np.float64) + np.array([2, 1]) * 0.2).astype(np.float32)
+    I1 = orc.forward_loss(pb, obj_s, probe, pos_s)["intensity"]
+    assert np.abs(I1 - I0).max() < 2e-4 * I0.max()      # fp32 positions: delta differs by ~1e-6 px
+    # P -> aP, O_0 -> O_0 / a leaves I unchanged
+    obj2 = obj.copy(); obj2[0] /= 2.0
+    I2 = orc.forward_loss(pb, obj2, (probe * 2.0).astype(np.complex64), pos)["intensity"]
+    assert np.abs(I2 - I0).max() < 1e-6 * I0.max()
+
+
+# ------------------------------------------------------------------------------------------------
+# loss (O6; readings R11, R12)
+# ------------------------------------------------------------------------------------------------
+def test_loss_closed_forms():
+    # amplitude loss exactly as printed: hand-computed 2x2 example
+    I = [4.0, 9.0, 1.0, 0.0]; Ie = [1.0, 16.0, 1.0, 2.0]
+    tot = sum(orc.loss_pixel(orc.LOSS_AMPLITUDE, a, b, 0.0, 1e-12)[0] for a, b in zip(I, Ie))
+    assert abs(tot - (0.5 + 0.5 + 0.0 + 1.0)) < 1e-12
+    # Anscombe c = 3/8
+    l, w = orc.loss_pixel(orc.LOSS_AMPLITUDE, 4.0 - 0.375, 9.0 - 0.375, 0.375, 1e-12)
+    assert abs(l - 0.5) < 1e-12 and abs(w - 0.5 * (1 - 3.0 / 2.0)) < 1e-11
+    # zero loss and weight at I = Iexp
+    for kind in (0, 1):
+        l, w = orc.loss_pixel(kind, 7.3, 7.3, 0.0, 1e-14)
+        assert abs(l) < 1e-12 and abs(w) < 1e-12
+    # Poisson: l = I where Iexp = 0; w = 1 - Iexp/(I + eps)
+    l, w = orc.loss_pixel(1, 2.5, 0.0, 0.0, 0.8); assert abs(l - 2.5) < 1e-14 and abs(w - 1.0) < 1e-14
+    l, w = orc.loss_pixel(1, 2.0, 3.0, 0.0, 0.5)
+    assert abs(l - (2.0 - 3.0 * (np.log(2.5) - np.log(3.5) + 1.0))) < 1e-14 and abs(w - (1 - 3.0 / 2.5)) < 1e-14
+    # Stirling form vs exact Poisson NLL: difference is 0.5 log(2 pi Iexp) + O(1/Iexp)
+    from math import lgamma
+    Ie, I = 400.0, 380.0
+    exact = I - Ie * np.log(I) + lgamma(Ie + 1)
+    l, _ = orc.loss_pixel(1, I, Ie, 0.0, 0.0)
+    assert abs((exact - l) - 0.5 * np.log(2 * np.pi * Ie)) < 1e-3
+    # w is the derivative of l (both losses), convexity in I
+    for kind, eps in ((0, 1e-12), (1, 0.8)):
+        for I0 in (0.7, 3.0, 50.0):
+            h = 1e-6
+            lp, _ = orc.loss_pixel(kind, I0 + h, 5.0, 0.0, eps); lm, _ = orc.loss_pixel(kind, I0 - h, 5.0, 0.0, eps)
+            l0, w0 = orc.loss_pixel(kind, I0, 5.0, 0.0, eps)
+            assert abs((lp - lm) / (2 * h) - w0) < 1e-6
+            lp, _ = orc.loss_pixel(kind, I0 + 0.25, 5.0, 0.0, eps); lm, _ = orc.loss_pixel(kind, I0 - 0.25, 5.0, 0.0, eps)
+            assert lp + lm - 2 * l0 > 0
+
+
+# ------------------------------------------------------------------------------------------------
+# linear adjoint pieces (O7..O11): <A x, y> = <x, A^H y>
+# ------------------------------------------------------------------------------------------------
+def test_adjoint_dot_products():
+    n = 16
+    x, y = crandn(n, n), crandn(n, n)
+    assert abs(np.vdot(y, orc.shift(x, 0.3, -0.2)) - np.vdot(orc.shift(y, 0.3, -0.2, adjoint=True), x)) < 1e-11
+    args = (0.1, 0.0197, 12.0, 0.8, 0.6, 2.0 / 3.0)
+    assert abs(np.vdot(y, orc.propagate(x, *args)) - np.vdot(orc.propagate(y, *args, adjoint=True), x)) < 1e-11
+    obj = crandn(30, 33); patch = crandn(n, n)
+    acc = np.zeros((30, 33), np.complex128); orc.scatter_add(acc, 5, 9, patch)
+    assert abs(np.vdot(patch, orc.gather(obj, 5, 9, n)) - np.vdot(acc, obj)) < 1e-11
+
+
+def test_scatter_add_coverage_map():
+    # all-ones patch gradients on an integer raster -> coverage = outer product of 1-D overlap counts
+    n, on = 8, 24
+    acc = np.zeros((on, on), np.complex128)
+    starts = [0, 4, 8, 12, 16]
+    for r0y in starts:
+        for r0x in starts:
+            orc.scatter_add(acc, r0y, r0x, np.ones((n, n)))
+    c1 = np.zeros(on); [c1.__setitem__(slice(s, s + n), c1[s:s + n] + 1) for s in starts]
+    assert np.abs(acc - np.outer(c1, c1)).max() == 0
+
+
+# ------------------------------------------------------------------------------------------------
+# full gradient: central finite differences (O7..O11; PAPER.md:181-185 Wirtinger convention, reading R15)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("loss,eps,bandlimit", [(orc.LOSS_POISSON, 0.3, 0.0), (orc.LOSS_POISSON, 0.3, 2.0 / 3.0),
+                                                (orc.LOSS_AMPLITUDE, 1e-12, 0.0)])
+def test_gradient_finite_differences(loss, eps, bandlimit):
+    pb, obj, probe, pos = small_problem(loss=loss, eps=eps, bandlimit=bandlimit)
+    obj_t = (obj * np.exp(0.2 * crandn(*obj.shape))).astype(np.complex64)
+    Iexp = orc.forward_loss(pb, obj_t, probe, pos)["intensity"].astype(np.float32) + 0.05
+    g = orc.gradient(pb, obj, probe, pos, Iexp)
+    L0 = orc.forward_loss(pb, obj, probe, pos, Iexp)["loss"]
+    assert abs(L0 - g["loss"]) < 1e-12 * abs(L0)
+
+    # perturbations must be exactly representable in the float32 inputs: use h = 2^-k and work on copies
+    def L(o, p):
+        return orc.forward_loss(pb, o, p, pos, Iexp, want_intensity=False)["loss"]
+
+    h = 2.0 ** -9
+    for which in ("obj", "probe"):
+        base = obj if which == "obj" else probe
+        D = crandn(*base.shape).astype(np.complex64)
+        # keep everything on the fp32 grid: z +- h*D evaluated in fp64 then cast would round; instead
+        # compute in complex128 and feed the oracle complex64 casts of both, measuring the actual step
+        zp = (base.astype(np.complex128) + h * D).astype(np.complex64)
+        zm = (base.astype(np.complex128) - h * D).astype(np.complex64)
+        Dact = (zp.astype(np.complex128) - zm.astype(np.complex128)) / 2.0
+        if which == "obj":
+            fd = (L(zp, probe) - L(zm, probe)) / 2.0
+            lin = 2.0 * np.real(np.vdot(g["grad_object"], Dact))
+        else:
+            fd = (L(obj, zp) - L(obj, zm)) / 2.0
+            lin = 2.0 * np.real(np.vdot(g["grad_probe"], Dact))
+        assert abs(fd - lin) < 2e-4 * abs(lin) + 1e-9, (which, fd, lin)
+
+
+def test_position_gradient_finite_differences():
+    pb, obj, probe, pos = small_problem(J=4)
+    Iexp = orc.forward_loss(pb, (obj * 1.1).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.05
+    # keep delta away from +-1/2 so r0 does not flip
+    for j in range(4):
+        for a in range(2):
+            r0, d = orc.position_split(float(pos[j, a]), 0.2, 8)
+            if abs(d) > 0.3:
+                pos[j, a] = np.float32((r0 + 8 / 2 + 0.1 * np.sign(d)) * 0.2)
+    g = orc.gradient(pb, obj, probe, pos, Iexp)
+    h = 2e-3 * 0.2
+    for j in range(4):
+        for a in range(2):
+            pp = pos.copy(); pm = pos.copy()
+            pp[j, a] += np.float32(h); pm[j, a] -= np.float32(h)
+            step = float(pp[j, a]) - float(pm[j, a])
+            fd = (orc.forward_loss(pb, obj, probe, pp, Iexp)["loss"] - orc.forward_loss(pb, obj, probe, pm, Iexp)["loss"]) / step
+            assert abs(fd - g["grad_pos"][j, a]) < 2e-3 * abs(fd) + 1e-6, (j, a, fd, g["grad_pos"][j, a])
+
+
+def test_zero_gradient_at_truth_noiseless():
+    # noiseless data, eps -> 0: loss and all gradients vanish at the true state (both losses)
+    for loss in (orc.LOSS_POISSON, orc.LOSS_AMPLITUDE):
+        pb, obj, probe, pos = small_problem(loss=loss, eps=1e-20)
+        Iexp = orc.forward_loss(pb, obj, probe, pos)["intensity"]
+        # fp32 storage of Iexp limits this to ~1e-7 relative
+        g = orc.gradient(pb, obj, probe, pos, Iexp.astype(np.float32))
+        scale = np.abs(obj).max() * np.abs(probe).max() ** 2
+        assert abs(g["loss"]) < 1e-9 * Iexp.sum()
+        assert np.abs(g["grad_object"]).max() < 1e-5 * scale
+        assert np.abs(g["grad_probe"]).max() < 1e-5 * scale
+        assert np.abs(g["grad_pos"]).max() < 1e-4 * Iexp.sum()
+
+
+# ------------------------------------------------------------------------------------------------
+# autograd re-derivation (torch, complex128): guards against a derivation error shared by the
+# hand-written adjoints (SURVEY.md §8(c) "optional independent check")
+# ------------------------------------------------------------------------------------------------
+def _torch_model(pb, obj, probe, pos, Iexp, retain=False):
+    import torch
+    n, M, S = pb.n, pb.n_modes, pb.n_slices
+    dt = torch.complex128
+    O = torch.tensor(obj.astype(np.complex128), requires_grad=True)
+    P = torch.tensor(probe.astype(np.complex128), requires_grad=True)
+    s = torch.tensor(np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n) / n)
+    px = float(np.float32(pb.pixel_size)); lam = float(np.float32(pb.wavelength))
+    tx = np.tan(float(np.float32(pb.tilt_x_mrad)) * 1e-3); ty = np.tan(float(np.float32(pb.tilt_y_mrad)) * 1e-3)
+    ky = (s / px)[:, None]; kx = (s / px)[None, :]
+    deltas = []; L = 0.0; inter = []
+    for j in range(pos.shape[0]):
+        r0y, dy = orc.position_split(float(pos[j, 0]), pb.pixel_size, n)
+        r0x, dx = orc.position_split(float(pos[j, 1]), pb.pixel_size, n)
+        d = torch.tensor([dy, dx], dtype=torch.float64, requires_grad=True); deltas.append(d)
+        R = torch.exp(-2j * np.pi * (s[:, None] * d[0] + s[None, :] * d[1]))
+        I = torch.zeros((n, n), dtype=torch.float64)
+        for k in range(M):
+            psi = torch.fft.ifft2(R * torch.fft.fft2(P[k]))
+            for i in range(S):
+                phi = psi * O[i, r0y:r0y + n, r0x:r0x + n]
+                if retain:
+                    phi.retain_grad(); inter.append((j, i, k, psi, phi))
+                if i < S - 1:
+                    dz = float(np.float32(pb.slice_thickness[i]))
+                    H = torch.exp(-1j * np.pi * lam * dz * (kx ** 2 + ky ** 2) + 2j * np.pi * dz * (kx * tx + ky * ty))
+                    if pb.bandlimit > 0:
+                        si = torch.tensor(np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n))
+                        H = H * ((si[:, None] ** 2 + si[None, :] ** 2) <= (0.5 * float(np.float32(pb.bandlimit)) * n) ** 2)
+                    psi = torch.fft.ifft2(H * torch.fft.fft2(phi))
+            I = I + torch.abs(torch.fft.fft2(phi) / n) ** 2
+        Ie = torch.tensor(Iexp[j].astype(np.float64)); eps = float(np.float32(pb.eps)); c = float(np.float32(pb.loss_c))
+        if pb.loss == orc.LOSS_POISSON:
+            L = L + torch.sum(I - Ie * (torch.log(I + eps) - torch.log(Ie + eps) + 1.0))
+        else:
+            L = L + torch.sum(0.5 * (torch.sqrt(I + c) - torch.sqrt(Ie + c)) ** 2)
+    L.backward()
+    gd = np.array([d.grad.numpy() for d in deltas])
+    return L.item(), O.grad.numpy() / 2.0, P.grad.numpy() / 2.0, gd, inter     # torch returns 2 dL/dconj(z) (R15)
+
+
+@pytest.mark.parametrize("loss,eps,S,bandlimit", [(orc.LOSS_POISSON, 0.8, 3, 0.0), (orc.LOSS_POISSON, 0.8, 2, 2.0 / 3.0),
+                                                  (orc.LOSS_AMPLITUDE, 1e-12, 1, 0.0), (orc.LOSS_AMPLITUDE, 1e-12, 3, 0.0)])
+def test_gradient_vs_torch_autograd(loss, eps, S, bandlimit):
+    pb, obj, probe, pos = small_problem(n=16, M=2, S=S, on=36, J=4, loss=loss, eps=eps, bandlimit=bandlimit)
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp)
+    L, gO, gP, gd, _ = _torch_model(pb, obj, probe, pos, Iexp)
+    rel = lambda a, b: np.linalg.norm(a - b) / np.linalg.norm(b)
+    assert abs(g["loss"] - L) < 1e-10 * abs(L)
+    assert rel(g["grad_object"], gO) < 1e-9
+    assert rel(g["grad_probe"], gP) < 1e-9
+    assert rel(g["grad_pos"], gd / float(np.float32(pb.pixel_size))) < 1e-8
+
+
+def test_single_slice_epie_relation():
+    # in single slice, gO|patch = -conj(P_shift) chi and gP-contribution = -conj(O) chi,
+    # chi = -N Finv(w psi~)  — i.e. ePIE's Delta O ~ P* chi is the negative Wirtinger gradient.
+    n, on = 16, 36
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=1, loss=orc.LOSS_POISSON, eps=0.8)
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp)
+    r0y, dy = orc.position_split(float(pos[0, 0]), pb.pixel_size, n); r0x, dx = orc.position_split(float(pos[0, 1]), pb.pixel_size, n)
+    Ps = orc.shift(probe[0].astype(complex), dy, dx)
+    patch = obj[0, r0y:r0y + n, r0x:r0x + n].astype(complex)
+    psit = np.fft.fft2(Ps * patch) / n
+    I = np.abs(psit) ** 2
+    w = 1 - Iexp[0] / (I + float(np.float32(0.8)))
+    chi = -n * np.fft.ifft2(w * psit)
+    assert np.abs(g["grad_object"][0, r0y:r0y + n, r0x:r0x + n] - (-np.conj(Ps) * chi)).max() < 1e-9 * np.abs(chi).max() * np.abs(Ps).max()
+    gP_ref = orc.shift(-np.conj(patch) * chi, dy, dx, adjoint=True)
+    assert np.abs(g["grad_probe"][0] - gP_ref).max() < 1e-9 * np.abs(gP_ref).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# LSQML-style terms (O12..O15; readings R18..R21)
+# ------------------------------------------------------------------------------------------------
+def test_lsqml_terms_vs_torch_intermediates():
+    pb, obj, probe, pos = small_problem(n=16, M=2, S=3, on=36, J=3, loss=orc.LOSS_POISSON, eps=0.8)
+    pb.lsqml_delta_o = 0.7; pb.lsqml_delta_p = 0.2
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    illum_prev = g["illum"] * 1.3 + 0.1
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], illum_prev)
+    # numX = -1/2 dL/d delta  (O14)
+    px = float(np.float32(pb.pixel_size)); S = 3
+    assert np.abs(st[:, 2 * S + 2] + 0.5 * g["grad_pos"][:, 0] * px).max() < 1e-9 * np.abs(g["grad_pos"]).max()
+    assert np.abs(st[:, 2 * S + 4] + 0.5 * g["grad_pos"][:, 1] * px).max() < 1e-9 * np.abs(g["grad_pos"]).max()
+    # illumination map (O12) and object terms against autograd intermediates chi = -gPhi
+    _, _, _, _, inter = _torch_model(pb, obj, probe, pos, Iexp, retain=True)
+    n = 16
+    dOhat = -g["grad_object"] / (illum_prev + float(np.float32(0.7)))
+    num = np.zeros((3, S)); den = np.zeros((3, S)); il = np.zeros_like(g["illum"])
+    for (j, i, k, psi, phi) in inter:
+        r0y, _ = orc.position_split(float(pos[j, 0]), pb.pixel_size, n); r0x, _ = orc.position_split(float(pos[j, 1]), pb.pixel_size, n)
+        chi = -(phi.grad.numpy() / 2.0); Psi = psi.detach().numpy()
+        u = dOhat[i, r0y:r0y + n, r0x:r0x + n] * Psi
+        num[j, i] += np.sum(np.real(chi * np.conj(u))); den[j, i] += np.sum(np.abs(u) ** 2)
+        il[i, r0y:r0y + n, r0x:r0x + n] += np.abs(Psi) ** 2
+    assert np.abs(il - g["illum"]).max() < 1e-10 * il.max()
+    assert np.abs(st[:, 0:2 * S:2] - num).max() < 1e-9 * np.abs(num).max()
+    assert np.abs(st[:, 1:2 * S:2] - den).max() < 1e-9 * np.abs(den).max()
+
+
+def test_lsqml_alpha_closed_form_single_position():
+    # single position, single slice, one mode, illum_prev = this position's |Psi|^2, delta_O -> 0, gamma = 0:
+    # dOhat|patch = conj(Psi) chi / |Psi|^2, so dOhat Psi = chi and alpha_O = sum|chi|^2 / sum|chi|^2 = 1,
+    # i.e. the step that zeroes the linearised exit-wave residual.
+    n, on = 16, 36
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=1, loss=orc.LOSS_POISSON, eps=0.8)
+    pb.lsqml_delta_o = 1e-30
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    illum_prev = np.where(g["illum"] > 0, g["illum"], 1.0)
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], illum_prev)
+    assert abs(st[0, 0] / st[0, 1] - 1.0) < 1e-9
+    # and the update moves the object by exactly beta * alpha * dOhat
+    o2, p2, x2 = orc.apply_update(pb, 1, obj, probe, pos, g["grad_object"], None, None, illum_prev, st, beta_obj=0.5)
+    assert np.abs((o2 - obj) - 0.5 * (-g["grad_object"] / (illum_prev + 1e-30))).max() < 1e-9
+
+
+def test_lsqml_position_step_recovers_offset():
+    # reading R21 (parity unpinned against the paper): the least-squares shift num/(den+gamma) walks a
+    # known sub-pixel offset back monotonically on a noiseless single-position toy with a strong object.
+    # (chi from an intensity-only loss sees only the amplitude part of the residual, so the contraction
+    # per step is ~0.8, not a one-step Newton solve.)
+    n, on = 16, 40
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=1, loss=orc.LOSS_AMPLITUDE, eps=1e-6)
+    s = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n)
+    Pt = (s[:, None] ** 2 + s[None, :] ** 2 <= 16) * np.exp(1j * 0.25 * (s[:, None] ** 2 + s[None, :] ** 2))
+    probe = (np.fft.fftshift(np.fft.ifft2(Pt))[None] * 30).astype(np.complex64)
+    yy, xx = np.meshgrid(np.arange(on), np.arange(on + 2), indexing="ij")
+    ph = 1.5 * (np.sin(2 * np.pi * yy / 9.0) + np.cos(2 * np.pi * xx / 7.0) + np.sin(2 * np.pi * (yy + xx) / 5.0))
+    obj = np.exp(1j * ph)[None].astype(np.complex64)
+    true = np.array([[(20.0 + 0.12) * 0.2, (21.0 - 0.08) * 0.2]], np.float32)
+    Iexp = orc.forward_loss(pb, obj, probe, true)["intensity"].astype(np.float32)
+    x = np.array([[20.0 * 0.2, 21.0 * 0.2]], np.float32)
+    errs = [np.abs(x - true).max()]
+    for _ in range(8):
+        g = orc.gradient(pb, obj, probe, x, Iexp, want_illum=True)
+        st = orc.step_terms(pb, obj, probe, x, Iexp, g["grad_object"], g["grad_probe"], g["illum"] + 1.0)
+        _, _, x2 = orc.apply_update(pb, 1, obj, probe, x, None, None, None, g["illum"] + 1.0, st)
+        x = x2.astype(np.float32); errs.append(np.abs(x - true).max())
+    assert all(b < a for a, b in zip(errs, errs[1:]))
+    assert errs[-1] < 0.3 * errs[0]
+
+
+def test_sgd_update():
+    pb, obj, probe, pos = small_problem()
+    gO = crandn(*obj.shape); gP = crandn(*probe.shape); gX = RNG.standard_normal(pos.shape)
+    o, p, x = orc.apply_update(pb, 0, obj, probe, pos, gO, gP, gX, lr_obj=0.1, lr_probe=0.2, lr_pos=0.3)
+    assert np.abs(o - (obj - 0.1 * gO)).max() < 1e-12 and np.abs(p - (probe - 0.2 * gP)).max() < 1e-12
+    assert np.abs(x - (pos - 0.3 * gX)).max() < 1e-12
