@@ -1,0 +1,156 @@
+/* ptycho.h — C ABI of the B200 hot path of mixed-state multislice ptychography
+ * (arxiv 2505.14372, "phaser").  One call = one batched forward(+adjoint) pass of the model of
+ * PAPER.md:113-123 over a group of probe positions, on one GPU, on the caller's stream.
+ *
+ * Conventions (DESIGN.md §2/§3 give the citations and the readings R1..R22 of the paper):
+ *   - complex64 is interleaved (re, im) float32; all arrays are C-contiguous, row-major, last index fastest.
+ *   - F is the unnormalised forward DFT with kernel exp(-2 pi i q.r/N); zero frequency at index [0][0].
+ *   - gradients are g = dL/d conj(z); a descent step is z <- z - lr*g.
+ *   - pointers ending in _d are DEVICE pointers, _h HOST pointers.  The library never allocates device
+ *     memory, keeps no pointer after a call returns and has no global state (re-entrant across streams).
+ *     pt_problem / pt_update / slice_thickness are HOST memory, read synchronously during the call.
+ *   - all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*); nothing synchronises except
+ *     ptycho_status() and the *_host convenience entry point.
+ *   - every function returns int32 status: 0 = PT_OK, < 0 = error.  No exceptions, no printing, no abort.
+ */
+#ifndef PTYCHO_H_
+#define PTYCHO_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct { float re, im; } pt_c64;
+
+enum { PT_LOSS_AMPLITUDE = 0,   /* PAPER.md:157, l = 1/2 (sqrt(I+c) - sqrt(Iexp+c))^2 ; c = 3/8 gives Anscombe */
+       PT_LOSS_POISSON = 1 };   /* PAPER.md:151, l = I - Iexp (ln(I+eps) - ln(Iexp+eps) + 1)                  */
+
+enum { PT_SHIFT_FOURIER_PROBE = 0,    /* integer window on the object + Fourier shift of the probe (R1) */
+       PT_SHIFT_BILINEAR_OBJECT = 1 };/* not built yet: returns PT_ERR_UNSUPPORTED                                    */
+
+enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                                                        */
+       PT_WANT_ILLUM = 2,             /* fill illum_d with sum_{j,k} |Psi_{i,k,j}|^2             */
+       PT_WANT_STEP_SIZES = 4,        /* fill step_terms_d, needs illum_prev_d               */
+       PT_ACCUMULATE = 16 };          /* add into grad_object_d/grad_probe_d/illum_d/loss_d instead of overwriting */
+
+enum { PT_OK = 0, PT_ERR_NULL = -1, PT_ERR_BAD_SIZE = -2, PT_ERR_BAD_PARAM = -3, PT_ERR_WORKSPACE = -4,
+       PT_ERR_CUDA = -5, PT_ERR_OUT_OF_BOUNDS = -6, PT_ERR_NONFINITE = -7, PT_ERR_UNSUPPORTED = -8 };
+
+/* Problem statement. HOST struct. */
+typedef struct {
+  int32_t n;                      /* N: probe / pattern side in px; supported: 64, 128, 256                      */
+  int32_t n_modes;                /* M >= 1 incoherent probe modes P_k                           */
+  int32_t n_slices;               /* S >= 1 object slices O_i                                    */
+  int32_t obj_ny, obj_nx;         /* object slice size in px (>= N)                                             */
+  int32_t n_pos_total;            /* rows of positions_d / intensity_d                                          */
+  int32_t n_batch;                /* J: positions in this call; batch_idx_d has J entries (NULL: rows 0..J-1)   */
+  float pixel_size;               /* Angstrom / px (probe and object)                                           */
+  float wavelength;               /* Angstrom                                                                   */
+  const float *slice_thickness;   /* HOST, S entries (Angstrom); entry S-1 unused (R10)                         */
+  float tilt_x_mrad, tilt_y_mrad; /* propagator tilt (R8: exp(+2 pi i dz (kx tan tx + ky tan ty)))*/
+  float bandlimit;                /* fraction of Nyquist of the sharp circular mask (R9); <=0 off */
+  int32_t loss;                   /* PT_LOSS_*                                                                   */
+  float loss_c;                   /* c of the variance-stabilising transform                     */
+  float eps;                      /* epsilon > 0 (R11..R13)                                       */
+  int32_t shift_mode;             /* PT_SHIFT_*                                                                  */
+  int32_t flags;                  /* PT_WANT_* | PT_ACCUMULATE                                                   */
+  float lsqml_delta_o;            /* delta_O of PAPER.md:219 (PT_WANT_STEP_SIZES only)                          */
+  float lsqml_delta_p;            /* probe analogue: dPhat = -gP / (delta_p + 1) (R19)                          */
+} pt_problem;
+
+enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1 };
+typedef struct {                  /* HOST struct */
+  int32_t mode;                   /* PT_UPDATE_SGD:   z <- z - lr * g   */
+                                  /* PT_UPDATE_LSQML: O_i += beta_O alpha_{O,i} dOhat_i etc.   (R18) */
+  float lr_obj, lr_probe, lr_pos;
+  float beta_obj, beta_probe;
+  float gamma;                    /* step-size regulariser of PAPER.md:221                                      */
+} pt_update;
+
+/* Number of floats per position in step_terms_d:  (numO_i, denO_i) i = 0..S-1, (numP, denP),
+ * (numX_y, denX_y), (numX_x, denX_x)  => 2*S + 6. */
+#define PT_STEP_TERMS_PER_POS(S) (2 * (S) + 6)
+
+/* Device scratch the caller must supply.  ptycho_workspace_bytes returns the RECOMMENDED size (positions are
+ * processed in chunks; a larger workspace means larger chunks, capped at 32 GiB); ptycho_workspace_min_bytes the
+ * smallest size the calls accept.  The first 64 bytes hold the deferred status word. */
+size_t ptycho_workspace_bytes(const pt_problem *p);
+size_t ptycho_workspace_min_bytes(const pt_problem *p);
+
+/* Forward model + loss.
+ *   object_d     [S][obj_ny][obj_nx]  transmission functions O_i
+ *   probe_d      [M][N][N]            probe modes in real space, centred at (N/2, N/2); mode weights folded in (R16)
+ *   positions_d  [n_pos_total][2]     (y, x) probe-centre coordinates in Angstrom; object pixel (0,0) at 0 (R3)
+ *   intensity_d  [n_pos_total][N][N]  measured I_exp, zero frequency at [0][0] (R6); may be NULL if only
+ *                                     model_intensity_d is wanted (loss outputs are then zero)
+ *   batch_idx_d  [n_batch] int32 rows of positions/intensity, or NULL
+ *   loss_d       [1] double  L = sum_j sum_q l   (NULL allowed)
+ *   loss_per_pos_d [n_batch] float L_j           (NULL allowed)
+ *   model_intensity_d [n_batch][N][N] float I_j  (NULL allowed)
+ * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE, PT_ERR_BAD_PARAM, PT_ERR_WORKSPACE, PT_ERR_CUDA immediately;
+ * PT_ERR_OUT_OF_BOUNDS (a window [r0, r0+N) leaves the object: the kernel clamps r0 so it never reads
+ * outside, and raises the flag — R4) and PT_ERR_NONFINITE deferred through ptycho_status(). */
+int32_t ptycho_forward_loss(const pt_problem *p, const pt_c64 *object_d, const pt_c64 *probe_d,
+                            const float *positions_d, const float *intensity_d, const int32_t *batch_idx_d,
+                            double *loss_d, float *loss_per_pos_d, float *model_intensity_d,
+                            void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* Loss + gradients: the adjoint of the chain above.
+ *   grad_object_d [S][obj_ny][obj_nx]  dL/d conj(O_i), deterministic scatter-add over overlapping patches
+ *   grad_probe_d  [M][N][N]            dL/d conj(P_k)
+ *   grad_pos_d    [n_batch][2]         dL/dX (per Angstrom), PT_WANT_POS_GRAD            (NULL allowed)
+ *   illum_d       [S][obj_ny][obj_nx]  float, this batch's sum_{j,k}|Psi_{i,k}|^2, PT_WANT_ILLUM (NULL allowed)
+ *   illum_prev_d  [S][obj_ny][obj_nx]  float, running sum of the previous iteration (R19);
+ *                                      needed with PT_WANT_STEP_SIZES
+ *   step_terms_d  [n_batch][2S+6]      float, PT_WANT_STEP_SIZES                          (NULL allowed)
+ * Bitwise reproducible: the same inputs give the same outputs on every run (no float atomics). */
+int32_t ptycho_gradient(const pt_problem *p, const pt_c64 *object_d, const pt_c64 *probe_d,
+                        const float *positions_d, const float *intensity_d, const int32_t *batch_idx_d,
+                        pt_c64 *grad_object_d, pt_c64 *grad_probe_d, float *grad_pos_d,
+                        float *illum_d, const float *illum_prev_d, float *step_terms_d,
+                        double *loss_d, float *loss_per_pos_d,
+                        void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* Update step (PAPER.md:187 SGD; PAPER.md:225 LSQML-style with per-group step sizes, R18).  In place.
+ * Any of object_d/probe_d/positions_d may be NULL (that variable is left alone). positions rows batch_idx_d only. */
+int32_t ptycho_apply_update(const pt_problem *p, pt_c64 *object_d, pt_c64 *probe_d, float *positions_d,
+                            const pt_c64 *grad_object_d, const pt_c64 *grad_probe_d, const float *grad_pos_d,
+                            const float *illum_prev_d, const float *step_terms_d, const int32_t *batch_idx_d,
+                            const pt_update *u, void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* End-to-end convenience with HOST buffers (pinned memory recommended): copies object/probe/positions and the
+ * batch rows' intensities host->device into the workspace, runs ptycho_gradient, copies gradients and loss
+ * back, and synchronises the stream.  Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL. */
+size_t ptycho_workspace_host_bytes(const pt_problem *p);
+int32_t ptycho_gradient_host(const pt_problem *p, const pt_c64 *object_h, const pt_c64 *probe_h,
+                             const float *positions_h, const float *intensity_h, const int32_t *batch_idx_h,
+                             pt_c64 *grad_object_h, pt_c64 *grad_probe_h, float *grad_pos_h,
+                             double *loss_h, float *loss_per_pos_h,
+                             void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* Synchronises the stream and returns the deferred device-side status (PT_OK, PT_ERR_OUT_OF_BOUNDS,
+ * PT_ERR_NONFINITE, or PT_ERR_CUDA); clears it. */
+int32_t ptycho_status(void *workspace_d, void *cuda_stream);
+
+/* Number of the library's own kernel launches enqueued by the calls made so far on this thread (for bench.py). */
+int64_t ptycho_launch_count(void);
+
+/* Optional per-kernel device timing, for bench.py's roofline line (the profiling recipe: CUDA events on the
+ * launching stream).  After ptycho_profile_enable(1) every kernel this THREAD launches through the calls above is
+ * followed by a CUDA event on its stream; ptycho_profile_read synchronises those events, writes per kernel kind
+ * (0 <= kind < ptycho_profile_num_kernels()) the summed device time in ms and the number of launches to the two
+ * HOST arrays, and resets the record.  ptycho_profile_enable(0) switches it off.  Off by default. */
+int32_t ptycho_profile_enable(int32_t on);
+int32_t ptycho_profile_num_kernels(void);
+const char *ptycho_profile_kernel_name(int32_t kind);
+int32_t ptycho_profile_read(float *ms_h, int64_t *launches_h);
+
+const char *ptycho_strerror(int32_t code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PTYCHO_H_ */

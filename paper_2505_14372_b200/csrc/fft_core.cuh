@@ -1,0 +1,320 @@
+// fft_core.cuh — register-resident 2-D complex FFT of an N x N field held by one CTA (N = 64, 128).
+//
+// A field of N*N complex64 lives in the REGISTERS of T = N*N/32 threads, 32 elements per thread.  One 2-D
+// FFT is three in-register phases joined by two shared-memory exchanges (the minimum for 2^14 points at 2^5
+// per thread):
+//
+//   R-layout (real space)  thread (a, b), reg (n1y, n1x):  x = a + N2X*n1x,  y = b + N2Y*n1y
+//     phase 1: DFT-N1X over n1x and DFT-N1Y over n1y, then twiddles W_N^(a*k1x) W_N^(b*k1y)
+//   exchange X1 (warp-local 32x32 transpose: lane <-> register)
+//     phase 2: DFT-N2X over a  (LP2 lines per thread)           -> qx = k1x + N1X*k2x
+//   exchange X2 (CTA-wide: for each k1y a [b] x [qx] transpose)
+//     phase 3: DFT-N2Y over b  (LP3 lines per thread)           -> qy = k1y + N1Y*k2y
+//   F-layout (Fourier space) thread (qx, c), reg (ksel, k2y): k1y = c*LP3 + ksel, qy = k1y + N1Y*k2y
+//
+// The inverse runs the same phases backwards (conjugated constants), so no bit reversal is ever
+// materialised: pointwise operators are indexed through the layout maps below.  Both exchanges use
+// padded/skewed slots whose addresses are thread-base + compile-time immediates and are bank-conflict free
+// for 8-byte accesses in both directions.
+//
+// Everything here is __host__ __device__ so that tests/test_fft_layout.py can emulate one CTA on the host
+// (index maps only; the host build is a test harness, never a product path).
+#pragma once
+#include <cuda_runtime.h>
+
+#if defined(__CUDACC__)
+#define PTK_HD __host__ __device__ __forceinline__
+#else
+#define PTK_HD inline
+#endif
+
+namespace ptk {
+
+typedef float2 cf;
+
+PTK_HD cf cmul(cf a, cf b) { return make_float2(fmaf(-a.y, b.y, a.x * b.x), fmaf(a.y, b.x, a.x * b.y)); }
+PTK_HD cf cmulc(cf a, cf b) { /* a * conj(b) */ return make_float2(fmaf(a.y, b.y, a.x * b.x), fmaf(a.y, b.x, -(a.x * b.y))); }
+PTK_HD cf cadd(cf a, cf b) { return make_float2(a.x + b.x, a.y + b.y); }
+PTK_HD cf csub(cf a, cf b) { return make_float2(a.x - b.x, a.y - b.y); }
+PTK_HD cf cconj(cf a) { return make_float2(a.x, -a.y); }
+PTK_HD cf cscale(cf a, float s) { return make_float2(a.x * s, a.y * s); }
+
+// cos / sin (2 pi m / 32), correctly rounded float literals
+PTK_HD constexpr float c32(int m) {
+  switch (m & 31) {
+    case 0: return 1.0f; case 1: return 0.98078525066375732f; case 2: return 0.92387950420379639f;
+    case 3: return 0.83146959543228149f; case 4: return 0.70710676908493042f; case 5: return 0.55557024478912354f;
+    case 6: return 0.38268342614173889f; case 7: return 0.19509032368659973f; case 8: return 0.0f;
+    case 9: return -0.19509032368659973f; case 10: return -0.38268342614173889f; case 11: return -0.55557024478912354f;
+    case 12: return -0.70710676908493042f; case 13: return -0.83146959543228149f; case 14: return -0.92387950420379639f;
+    case 15: return -0.98078525066375732f; case 16: return -1.0f; case 17: return -0.98078525066375732f;
+    case 18: return -0.92387950420379639f; case 19: return -0.83146959543228149f; case 20: return -0.70710676908493042f;
+    case 21: return -0.55557024478912354f; case 22: return -0.38268342614173889f; case 23: return -0.19509032368659973f;
+    case 24: return 0.0f; case 25: return 0.19509032368659973f; case 26: return 0.38268342614173889f;
+    case 27: return 0.55557024478912354f; case 28: return 0.70710676908493042f; case 29: return 0.83146959543228149f;
+    case 30: return 0.92387950420379639f; default: return 0.98078525066375732f;
+  }
+}
+PTK_HD constexpr float s32(int m) { return c32(m - 8); }
+
+// (x) * exp(DIR * 2 pi i * m / 32), m compile-time after unrolling; trivial cases cost no multiply
+template <int DIR>
+PTK_HD cf twiddle32(cf x, int m) {
+  m &= 31;
+  if (m == 0) return x;
+  if (m == 16) return make_float2(-x.x, -x.y);
+  if (m == 8) return DIR > 0 ? make_float2(-x.y, x.x) : make_float2(x.y, -x.x);    // * (+-i)
+  if (m == 24) return DIR > 0 ? make_float2(x.y, -x.x) : make_float2(-x.y, x.x);
+  const float c = c32(m), s = DIR > 0 ? s32(m) : -s32(m);
+  return make_float2(fmaf(-x.y, s, x.x * c), fmaf(x.x, s, x.y * c));
+}
+
+// in-register DFT of R = 2^k points, natural order in and out.  DIR = -1 forward (exp(-2 pi i ..)), +1 backward.
+// Decimation in frequency, radix 2, constant twiddles; all indices are compile-time after unrolling.
+template <int R, int DIR>
+struct Dft {
+  static PTK_HD void run(cf* x) {
+    cf e[R / 2], o[R / 2];
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) {
+      e[k] = cadd(x[k], x[k + R / 2]);
+      o[k] = twiddle32<DIR>(csub(x[k], x[k + R / 2]), k * (32 / R));
+    }
+    Dft<R / 2, DIR>::run(e);
+    Dft<R / 2, DIR>::run(o);
+#pragma unroll
+    for (int k = 0; k < R / 2; ++k) { x[2 * k] = e[k]; x[2 * k + 1] = o[k]; }
+  }
+};
+template <int DIR>
+struct Dft<1, DIR> { static PTK_HD void run(cf*) {} };
+
+// ---------------------------------------------------------------------------------------------------
+template <int N_> struct Geo;
+template <> struct Geo<128> {
+  static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
+};
+template <> struct Geo<64> {
+  static constexpr int N = 64, LOGN = 6, T = 128, N1X = 8, N2X = 8, N1Y = 4, N2Y = 16, LX2 = 3, LY2 = 4, LP2 = 4, LP3 = 2;
+};
+
+template <class G>
+struct Lay {
+  static constexpr int N = G::N, T = G::T;
+  static constexpr int X1_WARP = 33 * 32;                 // float2 slots per warp region (32 rows padded to 33)
+  static constexpr int X2_PLANE = G::N2Y * G::N + 8;      // float2 slots per k1y plane, skewed by 8
+  static constexpr int XBUF = (T / 32) * X1_WARP > 4 * X2_PLANE ? (T / 32) * X1_WARP : 4 * X2_PLANE;  // float2 slots
+  static constexpr int TW = G::N1X * G::N2X + G::N1Y * G::N2Y;   // twiddle table entries (float2)
+
+  // ---- R-layout: thread t, reg r -> (y, x)
+  static PTK_HD int r_x(int t, int r) { return (t & (G::N2X - 1)) + G::N2X * (r & (G::N1X - 1)); }
+  static PTK_HD int r_y(int t, int r) { return (t >> G::LX2) + G::N2Y * (r / G::N1X); }
+  // ---- F-layout: thread t, reg r -> (qy, qx)
+  static PTK_HD int f_qx(int t, int) { return t & (N - 1); }
+  static PTK_HD int f_qy(int t, int r) { return ((t >> G::LOGN) * G::LP3 + r / G::N2Y) + G::N1Y * (r & (G::N2Y - 1)); }
+  // native (coalesced) storage index of (thread, reg) in float2 units — used for stashes in both layouts
+  static PTK_HD int native(int t, int r) { return r * T + t; }
+  // position of real-space pixel (y, x) in R-native storage (used by the object-gradient gather)
+  static PTK_HD int r_native_of(int y, int x) {
+    int a = x & (G::N2X - 1), n1x = x >> G::LX2, b = y & (G::N2Y - 1), n1y = y >> G::LY2;
+    return (n1y * G::N1X + n1x) * T + (a + G::N2X * b);
+  }
+  static PTK_HD int f_native_of(int qy, int qx) {
+    int k1y = qy & (G::N1Y - 1), k2y = qy / G::N1Y;
+    int c = k1y / G::LP3, ksel = k1y % G::LP3;
+    return (ksel * G::N2Y + k2y) * T + (qx + N * c);
+  }
+
+  // fill the twiddle table: tw[k1x*N2X + a] = W_N^(a k1x), tw[N1X*N2X + k1y*N2Y + b] = W_N^(b k1y)   (forward sign)
+  static PTK_HD void fill_twiddle(cf* tw, int idx) {
+    int m;
+    if (idx < G::N1X * G::N2X) m = (idx / G::N2X) * (idx % G::N2X);
+    else { int i = idx - G::N1X * G::N2X; m = (i / G::N2Y) * (i % G::N2Y); }
+    float s, c;
+    sincospif(-2.0f * (float)(m % N) / (float)N, &s, &c);
+    tw[idx] = make_float2(c, s);
+  }
+
+  // ---- phase 1 (forward): R-layout regs -> (k1y, k1x) regs with twiddles
+  static PTK_HD void phase1_fwd(cf (&v)[32], const cf* tw, int t) {
+    const int a = t & (G::N2X - 1), b = t >> G::LX2;
+#pragma unroll
+    for (int n1y = 0; n1y < G::N1Y; ++n1y) {
+      cf x[G::N1X];
+#pragma unroll
+      for (int i = 0; i < G::N1X; ++i) x[i] = v[n1y * G::N1X + i];
+      Dft<G::N1X, -1>::run(x);
+#pragma unroll
+      for (int i = 0; i < G::N1X; ++i) v[n1y * G::N1X + i] = x[i];
+    }
+#pragma unroll
+    for (int k1x = 0; k1x < G::N1X; ++k1x) {
+      cf x[G::N1Y];
+#pragma unroll
+      for (int i = 0; i < G::N1Y; ++i) x[i] = v[i * G::N1X + k1x];
+      Dft<G::N1Y, -1>::run(x);
+      if (k1x > 0) {
+        cf wx = tw[k1x * G::N2X + a];
+#pragma unroll
+        for (int i = 0; i < G::N1Y; ++i) x[i] = cmul(x[i], wx);
+      }
+#pragma unroll
+      for (int i = 0; i < G::N1Y; ++i) v[i * G::N1X + k1x] = x[i];
+    }
+#pragma unroll
+    for (int k1y = 1; k1y < G::N1Y; ++k1y) {
+      cf wy = tw[G::N1X * G::N2X + k1y * G::N2Y + b];
+#pragma unroll
+      for (int k1x = 0; k1x < G::N1X; ++k1x) v[k1y * G::N1X + k1x] = cmul(v[k1y * G::N1X + k1x], wy);
+    }
+  }
+  // ---- phase 1 (inverse): (k1y, k1x) regs -> R-layout regs
+  static PTK_HD void phase1_inv(cf (&v)[32], const cf* tw, int t) {
+    const int a = t & (G::N2X - 1), b = t >> G::LX2;
+#pragma unroll
+    for (int k1y = 1; k1y < G::N1Y; ++k1y) {
+      cf wy = tw[G::N1X * G::N2X + k1y * G::N2Y + b];
+#pragma unroll
+      for (int k1x = 0; k1x < G::N1X; ++k1x) v[k1y * G::N1X + k1x] = cmulc(v[k1y * G::N1X + k1x], wy);
+    }
+#pragma unroll
+    for (int k1x = 0; k1x < G::N1X; ++k1x) {
+      cf x[G::N1Y];
+#pragma unroll
+      for (int i = 0; i < G::N1Y; ++i) x[i] = v[i * G::N1X + k1x];
+      if (k1x > 0) {
+        cf wx = tw[k1x * G::N2X + a];
+#pragma unroll
+        for (int i = 0; i < G::N1Y; ++i) x[i] = cmulc(x[i], wx);
+      }
+      Dft<G::N1Y, +1>::run(x);
+#pragma unroll
+      for (int i = 0; i < G::N1Y; ++i) v[i * G::N1X + k1x] = x[i];
+    }
+#pragma unroll
+    for (int n1y = 0; n1y < G::N1Y; ++n1y) {
+      cf x[G::N1X];
+#pragma unroll
+      for (int i = 0; i < G::N1X; ++i) x[i] = v[n1y * G::N1X + i];
+      Dft<G::N1X, +1>::run(x);
+#pragma unroll
+      for (int i = 0; i < G::N1X; ++i) v[n1y * G::N1X + i] = x[i];
+    }
+  }
+  // ---- phase 2: LP2 lines of N2X points (reg = line*N2X + point)
+  template <int DIR>
+  static PTK_HD void phase2(cf (&v)[32]) {
+#pragma unroll
+    for (int l = 0; l < G::LP2; ++l) {
+      cf x[G::N2X];
+#pragma unroll
+      for (int i = 0; i < G::N2X; ++i) x[i] = v[l * G::N2X + i];
+      Dft<G::N2X, DIR>::run(x);
+#pragma unroll
+      for (int i = 0; i < G::N2X; ++i) v[l * G::N2X + i] = x[i];
+    }
+  }
+  // ---- phase 3: LP3 lines of N2Y points
+  template <int DIR>
+  static PTK_HD void phase3(cf (&v)[32]) {
+#pragma unroll
+    for (int l = 0; l < G::LP3; ++l) {
+      cf x[G::N2Y];
+#pragma unroll
+      for (int i = 0; i < G::N2Y; ++i) x[i] = v[l * G::N2Y + i];
+      Dft<G::N2Y, DIR>::run(x);
+#pragma unroll
+      for (int i = 0; i < G::N2Y; ++i) v[l * G::N2Y + i] = x[i];
+    }
+  }
+
+  // ---- exchange X1: warp-local transpose lane <-> reg.  "p1" side: thread t (lane L), reg R = k1y*N1X + k1x.
+  // "p2" side: lane L' = R, reg R' = L (= a + N2X*bsel).  slot(L, R) = warp*X1_WARP + R*33 + L.
+  static PTK_HD void x1_store_p1(const cf (&v)[32], cf* sm, int t) {
+    cf* base = sm + (t >> 5) * X1_WARP + (t & 31);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) base[r * 33] = v[r];
+  }
+  static PTK_HD void x1_load_p1(cf (&v)[32], const cf* sm, int t) {
+    const cf* base = sm + (t >> 5) * X1_WARP + (t & 31);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = base[r * 33];
+  }
+  static PTK_HD void x1_store_p2(const cf (&v)[32], cf* sm, int t) {
+    cf* base = sm + (t >> 5) * X1_WARP + (t & 31) * 33;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) base[r] = v[r];
+  }
+  static PTK_HD void x1_load_p2(cf (&v)[32], const cf* sm, int t) {
+    const cf* base = sm + (t >> 5) * X1_WARP + (t & 31) * 33;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = base[r];
+  }
+  // ---- exchange X2: slot(k1y, b, qx) = k1y*X2_PLANE + b*N + qx.
+  // "p2" side: thread t = warp w, lane (k1y, k1x); reg (bsel, k2x): b = w*LP2 + bsel, qx = k1x + N1X*k2x.
+  static PTK_HD int x2_base_p2(int t) {
+    const int w = t >> 5, k1y = (t & 31) / G::N1X, k1x = t & (G::N1X - 1);
+    return k1y * X2_PLANE + (w * G::LP2) * N + k1x;
+  }
+  static PTK_HD void x2_store_p2(const cf (&v)[32], cf* sm, int t) {
+    cf* base = sm + x2_base_p2(t);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) base[(r / G::N2X) * N + (r & (G::N2X - 1)) * G::N1X] = v[r];
+  }
+  static PTK_HD void x2_load_p2(cf (&v)[32], const cf* sm, int t) {
+    const cf* base = sm + x2_base_p2(t);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = base[(r / G::N2X) * N + (r & (G::N2X - 1)) * G::N1X];
+  }
+  // "p3" side: thread t = (qx, c); reg (ksel, b): k1y = c*LP3 + ksel.
+  static PTK_HD int x2_base_p3(int t) { return ((t >> G::LOGN) * G::LP3) * X2_PLANE + (t & (N - 1)); }
+  static PTK_HD void x2_store_p3(const cf (&v)[32], cf* sm, int t) {
+    cf* base = sm + x2_base_p3(t);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) base[(r / G::N2Y) * X2_PLANE + (r & (G::N2Y - 1)) * N] = v[r];
+  }
+  static PTK_HD void x2_load_p3(cf (&v)[32], const cf* sm, int t) {
+    const cf* base = sm + x2_base_p3(t);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = base[(r / G::N2Y) * X2_PLANE + (r & (G::N2Y - 1)) * N];
+  }
+};
+
+#if defined(__CUDACC__)
+// Whole transforms for one CTA.  `sm` = exchange buffer (Lay::XBUF float2), `tw` = twiddle table (Lay::TW).
+// Contract: fft2_fwd must follow an fft2_inv or a __syncthreads() (it starts by overwriting the calling warp's
+// own X1 region, which only that warp read last); fft2_inv may follow anything (it starts with a CTA barrier
+// because it overwrites the whole buffer).  Unnormalised.
+template <class G>
+__device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int t) {
+  typedef Lay<G> L;
+  L::phase1_fwd(v, tw, t);
+  __syncwarp();
+  L::x1_store_p1(v, sm, t);
+  __syncwarp();
+  L::x1_load_p2(v, sm, t);
+  L::template phase2<-1>(v);
+  __syncthreads();                 // every warp is done with its X1 region before X2 overwrites the buffer
+  L::x2_store_p2(v, sm, t);
+  __syncthreads();
+  L::x2_load_p3(v, sm, t);
+  L::template phase3<-1>(v);
+}
+template <class G>
+__device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int t) {
+  typedef Lay<G> L;
+  L::template phase3<+1>(v);
+  __syncthreads();
+  L::x2_store_p3(v, sm, t);
+  __syncthreads();
+  L::x2_load_p2(v, sm, t);
+  L::template phase2<+1>(v);
+  __syncthreads();                 // all X2 reads done before the warp-local X1 regions are overwritten
+  L::x1_store_p2(v, sm, t);
+  __syncwarp();
+  L::x1_load_p1(v, sm, t);
+  L::phase1_inv(v, tw, t);
+}
+#endif
+
+}  // namespace ptk

@@ -1,0 +1,1048 @@
+// ptycho_kernels.cu — sm_100a kernels and the C ABI (include/ptycho.h) of the multislice ptychography hot path.
+//
+// Path, all on the caller's stream:
+//   k_setup_prop     H5 tables  hx_i[qx], hy_i[qy] (separable Fresnel + tilt phases, fp64 math -> fp32)
+//   k_setup_pos      H0 position split (fp32, reading R2) + H2 shift ramps rx_j, ry_j + bounds flag (R4)
+//   k_probe_fft      H1 P~_k = F(P_k)
+//   k_forward        H2..H6 one CTA per (position j, mode k): field in registers, 2S in-register 2-D FFTs,
+//                    entering waves Psi_{i,k} stashed for the adjoint, far field psi~_k written out
+//   k_loss           H7,H8 mode-summed intensity, per-pixel loss in fp64, detector weight w
+//   k_backward       H9,H10,H12,H13 one CTA per (j,k): adjoint chain, per-(j,k,i) patch gradients,
+//                    per-(j,k) probe-gradient spectra and position-gradient terms
+//   k_gather_object  H11 deterministic owner-computes scatter-add: every object pixel sums the patch
+//                    gradients that cover it in fixed (j,k) order — no float atomics
+//   k_reduce_probe / k_probe_ifft / k_finalize   H12 tail, loss and position-gradient sums
+//   k_step_*         H14 LSQML-style step-size terms (second sweep), k_update_* H15
+// The CPU oracle under oracle/ shares nothing with this file.
+#include <cuda_runtime.h>
+#include <math_constants.h>
+#include <stdint.h>
+#include <string.h>
+
+#include <vector>
+
+#include "../../include/ptycho.h"
+#include "fft_core.cuh"
+
+using namespace ptk;
+
+namespace {
+
+constexpr int kStatusOOB = 1, kStatusNonfinite = 2;
+
+// ------------------------------------------------------------------------------------------------
+// workspace layout (host + device agree through this POD)
+// ------------------------------------------------------------------------------------------------
+struct Ws {
+  int32_t* status;     // [16]
+  cf* hx;              // [max(S-1,1)][N]   pre-scaled by 1/N^2
+  cf* hy;              // [max(S-1,1)][N]
+  cf* ramps;           // [J][2][N]  (rx, ry)
+  int32_t* r0;         // [J][2]  (y, x)
+  float* delta;        // [J][2]
+  cf* Pt;              // [M][N^2]  F-native, unscaled
+  cf* Qt;              // [M][N^2]  F-native: F(dPhat_k) for the step-size sweep
+  double2* gPt_acc;    // [M][N^2]  F-native accumulators
+  double* loss_pp;     // [J]
+  double* posg_part;   // [J][M][2]
+  double* step_part;   // [J][M][2S+6]
+  cf* dOhat;           // [S][ony][onx]      (step sizes only)
+  // chunked
+  cf* psit;            // [Jc][M][N^2]  F-native
+  float* wdet;         // [Jc][N^2]     F-native
+  cf* stash;           // [Jc][M][S][N^2]  R-native
+  cf* gTpart;          // [Jc][M][S][N^2]  R-native
+  cf* Gpart;           // [Jc][M][N^2]     F-native
+  cf* scratch;         // [Jc][M][N^2]     (step sizes: gPhi_0)
+  int32_t Jc;
+  size_t total;
+};
+
+inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+
+// per-chunk-position bytes and fixed bytes
+void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
+  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch;
+  const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
+  size_t f = 256;
+  f += 2 * align_up((S > 1 ? S - 1 : 1) * N * sizeof(cf));
+  f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float));
+  f += 2 * align_up(M * NN * sizeof(cf)) + align_up(M * NN * sizeof(double2));
+  f += align_up(J * sizeof(double)) + align_up(J * M * 2 * sizeof(double));
+  f += align_up(J * M * (2 * S + 6) * sizeof(double));
+  if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
+  size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
+  if (steps) pp += M * NN * sizeof(cf);
+  *fixed = f + 8 * 256;   // slack for the per-array alignment of the chunked part
+  *per_pos = pp;
+}
+
+int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
+  size_t fixed, pp;
+  ws_sizes(p, &fixed, &pp);
+  if (bytes < fixed + pp) return PT_ERR_WORKSPACE;
+  size_t jc = (bytes - fixed) / pp;
+  if (jc > (size_t)p->n_batch) jc = p->n_batch;
+  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch;
+  const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
+  char* c = (char*)base;
+  size_t off = 0;
+  auto take = [&](size_t n) { char* r = c + off; off += align_up(n); return (void*)r; };
+  w->status = (int32_t*)take(256);
+  w->hx = (cf*)take((S > 1 ? S - 1 : 1) * N * sizeof(cf));
+  w->hy = (cf*)take((S > 1 ? S - 1 : 1) * N * sizeof(cf));
+  w->ramps = (cf*)take(J * 2 * N * sizeof(cf));
+  w->r0 = (int32_t*)take(J * 2 * sizeof(int32_t));
+  w->delta = (float*)take(J * 2 * sizeof(float));
+  w->Pt = (cf*)take(M * NN * sizeof(cf));
+  w->Qt = (cf*)take(M * NN * sizeof(cf));
+  w->gPt_acc = (double2*)take(M * NN * sizeof(double2));
+  w->loss_pp = (double*)take(J * sizeof(double));
+  w->posg_part = (double*)take(J * M * 2 * sizeof(double));
+  w->step_part = (double*)take(J * M * (2 * S + 6) * sizeof(double));
+  w->dOhat = steps ? (cf*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf)) : nullptr;
+  w->psit = (cf*)take(jc * M * NN * sizeof(cf));
+  w->wdet = (float*)take(jc * NN * sizeof(float));
+  w->stash = (cf*)take(jc * M * S * NN * sizeof(cf));
+  w->gTpart = (cf*)take(jc * M * S * NN * sizeof(cf));
+  w->Gpart = (cf*)take(jc * M * NN * sizeof(cf));
+  w->scratch = steps ? (cf*)take(jc * M * NN * sizeof(cf)) : nullptr;
+  w->Jc = (int32_t)jc;
+  w->total = off;
+  return off <= bytes ? PT_OK : PT_ERR_WORKSPACE;
+}
+
+// ------------------------------------------------------------------------------------------------
+// kernel parameter block
+// ------------------------------------------------------------------------------------------------
+struct KP {
+  int N, M, S, ony, onx, J;          // J = batch size
+  int j0, jc;                        // current chunk: batch-local offset and count
+  float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
+  int loss; float loss_c, eps;
+  const cf* object; const cf* probe; const float* positions; const float* intensity; const int32_t* batch_idx;
+  Ws w;
+};
+
+__device__ __forceinline__ int signed_freq(int q, int N) { return q < N / 2 ? q : q - N; }
+
+// ------------------------------------------------------------------------------------------------
+// H5 tables: hx_i[q] = exp(-i pi lambda dz kx^2 + 2 pi i dz kx tan(tx)) / N^2, hy_i likewise without the scale
+// (readings R7, R8).  fp64 math, one thread per (i, axis, q).
+// ------------------------------------------------------------------------------------------------
+struct PropArgs { int N, nprop; double px, lambda, tx, ty; cf* hx; cf* hy; float dz[64]; int i0; };
+__global__ void k_setup_prop(PropArgs a) {
+  int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= a.nprop * 2 * a.N) return;
+  int q = idx % a.N, axis = (idx / a.N) & 1, il = idx / (2 * a.N);
+  double dz = (double)a.dz[il];
+  double k = (double)signed_freq(q, a.N) / (double)a.N / a.px;
+  double t = axis == 0 ? tan(a.tx * 1e-3) : tan(a.ty * 1e-3);
+  double ang = -CUDART_PI * a.lambda * dz * k * k + 2.0 * CUDART_PI * dz * k * t;
+  double s, c;
+  sincos(ang, &s, &c);
+  if (axis == 0) {
+    double sc = 1.0 / ((double)a.N * (double)a.N);
+    a.hx[(size_t)(a.i0 + il) * a.N + q] = make_float2((float)(c * sc), (float)(s * sc));
+  } else {
+    a.hy[(size_t)(a.i0 + il) * a.N + q] = make_float2((float)c, (float)s);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// H0 + H2 tables: position split in fp32 exactly as the reading R2 states it (no FMA contraction), bounds
+// flag (R4: clamp + raise), shift ramps rx[q] = exp(-2 pi i f(q) dx), ry likewise.
+// One block per position, N threads.
+// ------------------------------------------------------------------------------------------------
+__global__ void k_setup_pos(KP P) {
+  const int jb = blockIdx.x, q = threadIdx.x, N = P.N;
+  const int row = P.batch_idx ? P.batch_idx[jb] : jb;
+  float d[2]; int r0[2];
+#pragma unroll
+  for (int a = 0; a < 2; ++a) {
+    float X = P.positions[2 * row + a];
+    float p = __fdiv_rn(X, P.px);
+    float c = __fsub_rn(p, (float)(N / 2));
+    float fl = floorf(__fadd_rn(c, 0.5f));
+    d[a] = __fsub_rn(c, fl);
+    int r = (int)fl;
+    int lim = (a == 0 ? P.ony : P.onx) - N;
+    if (r < 0 || r > lim) {
+      if (q == 0) atomicOr(P.w.status, kStatusOOB);
+      r = r < 0 ? 0 : lim;
+    }
+    r0[a] = r;
+  }
+  if (q == 0) {
+    P.w.r0[2 * jb] = r0[0]; P.w.r0[2 * jb + 1] = r0[1];
+    P.w.delta[2 * jb] = d[0]; P.w.delta[2 * jb + 1] = d[1];
+  }
+  const float f = (float)signed_freq(q, N) / (float)N;
+  float s, c;
+  sincospif(-2.0f * f * d[1], &s, &c);
+  P.w.ramps[((size_t)jb * 2 + 0) * N + q] = make_float2(c, s);     // rx
+  sincospif(-2.0f * f * d[0], &s, &c);
+  P.w.ramps[((size_t)jb * 2 + 1) * N + q] = make_float2(c, s);     // ry
+}
+
+// ------------------------------------------------------------------------------------------------
+// block-wide deterministic sum of NV doubles per thread; result valid in thread 0
+// ------------------------------------------------------------------------------------------------
+template <int T, int NV>
+__device__ __forceinline__ void block_sum(double (&val)[NV], double* red /* [T/32][NV] */) {
+#pragma unroll
+  for (int i = 0; i < NV; ++i)
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) val[i] += __shfl_xor_sync(0xffffffffu, val[i], o);
+  const int w = threadIdx.x >> 5, l = threadIdx.x & 31;
+  if (l == 0)
+#pragma unroll
+    for (int i = 0; i < NV; ++i) red[w * NV + i] = val[i];
+  __syncthreads();
+  if (threadIdx.x == 0) {
+#pragma unroll
+    for (int i = 0; i < NV; ++i) {
+      double s = 0.0;
+      for (int ww = 0; ww < T / 32; ++ww) s += red[ww * NV + i];
+      val[i] = s;
+    }
+  }
+  __syncthreads();
+}
+
+template <class G> constexpr int min_blocks() { return G::N == 128 ? 1 : 4; }
+template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::XBUF + Lay<G>::TW) * sizeof(cf) + 1024; }
+
+// ------------------------------------------------------------------------------------------------
+// H1: P~_k = F(P_k), stored F-native.  Also used for Q~_k = F(dPhat_k) with scale/accumulator input.
+//   mode 0: in = raster complex64 field [k][N][N]
+//   mode 1: in = -gP_k / (delta_p + 1) from raster grad_probe (step-size sweep, O14)
+// ------------------------------------------------------------------------------------------------
+template <class G>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* in, cf* out, float scale) {
+  typedef Lay<G> L;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
+  const int t = threadIdx.x, k = blockIdx.x, N = G::N;
+  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  __syncthreads();
+  cf v[32];
+  const cf* src = in + (size_t)k * N * N;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) v[r] = cscale(src[L::r_y(t, r) * N + L::r_x(t, r)], scale);
+  fft2_fwd<G>(v, sm, tw, t);
+  cf* dst = out + (size_t)k * N * N;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) dst[L::native(t, r)] = v[r];
+}
+
+// H12 tail: gP_k = Finv(gP~_k): F-native double accumulators -> raster complex64 (overwrite or add)
+template <class G>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const double2* acc, cf* out, int accumulate) {
+  typedef Lay<G> L;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
+  const int t = threadIdx.x, k = blockIdx.x, N = G::N;
+  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  __syncthreads();
+  cf v[32];
+  const double sc = 1.0 / ((double)N * (double)N);
+#pragma unroll
+  for (int r = 0; r < 32; ++r) { double2 a = acc[(size_t)k * N * N + L::native(t, r)]; v[r] = make_float2((float)(a.x * sc), (float)(a.y * sc)); }
+  fft2_inv<G>(v, sm, tw, t);
+  cf* dst = out + (size_t)k * N * N;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    cf* d = dst + L::r_y(t, r) * N + L::r_x(t, r);
+    if (accumulate) { cf o = *d; *d = make_float2(o.x + v[r].x, o.y + v[r].y); } else *d = v[r];
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// pointwise helpers on the register field
+// ------------------------------------------------------------------------------------------------
+// v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9)
+template <class G, bool CONJ>
+__device__ __forceinline__ void apply_prop(cf (&v)[32], const cf* hx, const cf* hy, float bandlim2, int t) {
+  typedef Lay<G> L;
+  const int qx = L::f_qx(t, 0);
+  cf wx = hx[qx];
+  if (CONJ) wx.y = -wx.y;
+  const int sx = signed_freq(qx, G::N);
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int qy = L::f_qy(t, r);
+    cf wy = hy[qy];
+    if (CONJ) wy.y = -wy.y;
+    cf h = cmul(wx, wy);
+    if (bandlim2 >= 0.0f) {
+      const int sy = signed_freq(qy, G::N);
+      if ((float)(sx * sx + sy * sy) > bandlim2) h = make_float2(0.f, 0.f);
+    }
+    v[r] = cmul(v[r], h);
+  }
+}
+
+// object patch pointer for (slice i, position window r0)
+__device__ __forceinline__ const cf* patch_ptr(const KP& P, int i, int r0y, int r0x) {
+  return P.object + ((size_t)i * P.ony + r0y) * P.onx + r0x;
+}
+
+// ------------------------------------------------------------------------------------------------
+// H2..H6 forward: one CTA per (j,k) pair of the chunk
+// ------------------------------------------------------------------------------------------------
+template <class G, bool STASH>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
+  typedef Lay<G> L;
+  constexpr int N = G::N, NN = N * N;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
+  const int t = threadIdx.x;
+  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  __syncthreads();
+  const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
+  const cf* ry = rx + N;
+  cf v[32];
+  {   // H2: R .* P~_k / N^2   (F-layout)
+    const cf* pt = P.w.Pt + (size_t)k * NN;
+    cf wx = cscale(rx[L::f_qx(t, 0)], 1.0f / (float)NN);
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = cmul(pt[L::native(t, r)], cmul(wx, ry[L::f_qy(t, r)]));
+  }
+  const int S = P.S;
+  for (int i = 0; i < S; ++i) {
+    fft2_inv<G>(v, sm, tw, t);                                   // Psi_{i,k}  (R-layout)
+    if (STASH) {
+      cf* st = P.w.stash + ((size_t)(jl * P.M + k) * S + i) * NN;
+#pragma unroll
+      for (int r = 0; r < 32; ++r) st[L::native(t, r)] = v[r];
+    }
+    const cf* ob = patch_ptr(P, i, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
+#pragma unroll
+    for (int r = 0; r < 32; ++r)                                 // H3+H4: Phi = Psi .* T_i
+      v[r] = cmul(v[r], ob[(size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X]);
+    fft2_fwd<G>(v, sm, tw, t);                                   // F(Phi)    (F-layout)
+    if (i < S - 1) apply_prop<G, false>(v, P.w.hx + (size_t)i * N, P.w.hy + (size_t)i * N, P.bandlim2, t);   // H5
+  }
+  cf* out = P.w.psit + (size_t)(jl * P.M + k) * NN;              // H6: psi~ = F(Phi_{S-1}) / N
+  const float sc = 1.0f / (float)N;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) out[L::native(t, r)] = cscale(v[r], sc);
+}
+
+// ------------------------------------------------------------------------------------------------
+// H7 + H8: I = sum_k |psi~_k|^2 ; per-pixel loss in fp64 ; w = dl/dI.  One CTA per position of the chunk.
+// ------------------------------------------------------------------------------------------------
+template <class G>
+__global__ void __launch_bounds__(G::T) k_loss(KP P, float* loss_per_pos, float* model_intensity, int want_w) {
+  typedef Lay<G> L;
+  constexpr int N = G::N, NN = N * N;
+  __shared__ double red[(G::T / 32) * 1];
+  const int t = threadIdx.x, jl = blockIdx.x, jb = P.j0 + jl;
+  const int row = P.batch_idx ? P.batch_idx[jb] : jb;
+  float I[32];
+#pragma unroll
+  for (int r = 0; r < 32; ++r) I[r] = 0.f;
+  for (int k = 0; k < P.M; ++k) {
+    const cf* ps = P.w.psit + (size_t)(jl * P.M + k) * NN;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) { cf z = ps[L::native(t, r)]; I[r] = fmaf(z.x, z.x, fmaf(z.y, z.y, I[r])); }
+  }
+  double acc[1] = {0.0};
+  const float* Ie = P.intensity ? P.intensity + (size_t)row * NN : nullptr;
+  const double eps = (double)P.eps, c = (double)P.loss_c;
+#pragma unroll 4
+  for (int r = 0; r < 32; ++r) {
+    const int qy = L::f_qy(t, r), qx = L::f_qx(t, r);
+    if (model_intensity) model_intensity[(size_t)jb * NN + qy * N + qx] = I[r];
+    if (Ie) {
+      const double Im = (double)I[r], Ix = (double)Ie[qy * N + qx];
+      double l, w;
+      if (P.loss == PT_LOSS_POISSON) {
+        l = Im - Ix * (log(Im + eps) - log(Ix + eps) + 1.0);
+        w = 1.0 - Ix / (Im + eps);
+      } else {
+        const double a = sqrt(Im + c), ae = sqrt(Ix + c);
+        l = 0.5 * (a - ae) * (a - ae);
+        w = 0.5 * (1.0 - ae / (a + eps));
+      }
+      acc[0] += l;
+      if (want_w) P.w.wdet[(size_t)jl * NN + L::native(t, r)] = (float)w;
+    }
+  }
+  block_sum<G::T, 1>(acc, red);
+  if (t == 0) {
+    P.w.loss_pp[jb] = acc[0];
+    if (loss_per_pos) loss_per_pos[jb] = (float)acc[0];
+    if (!(acc[0] == acc[0]) || fabs(acc[0]) > 1e300) atomicOr(P.w.status, kStatusNonfinite);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// H9, H10, H12, H13 backward: one CTA per (j,k) pair of the chunk.
+// MODE 0: gradient pass — writes gT partials, probe partials, position terms.
+// MODE 1: step-size sweep (H14) — instead accumulates numO/denO per slice and the probe / position terms.
+// ------------------------------------------------------------------------------------------------
+template <class G, int MODE>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int want_pos) {
+  typedef Lay<G> L;
+  constexpr int N = G::N, NN = N * N;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
+  double* red = (double*)(tw + L::TW);          // [(T/32)*4] doubles (<= 64*8 = 512 B... sized in fft_smem_bytes)
+  const int t = threadIdx.x;
+  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  __syncthreads();
+  const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const int S = P.S;
+  cf v[32];
+  {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = N Finv(g~) = F^H(g~) / N
+    const cf* ps = P.w.psit + (size_t)(jl * P.M + k) * NN;
+    const float* wd = P.w.wdet + (size_t)jl * NN;
+    const float sc = 1.0f / (float)N;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) v[r] = cscale(ps[L::native(t, r)], wd[L::native(t, r)] * sc);
+  }
+  for (int i = S - 1; i >= 0; --i) {
+    fft2_inv<G>(v, sm, tw, t);                                   // gPhi_{i,k}  (R-layout)
+    const size_t fld = ((size_t)(jl * P.M + k) * S + i) * NN;
+    const cf* st = P.w.stash + fld;
+    const cf* ob = patch_ptr(P, i, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
+    if (MODE == 0) {
+      cf* gt = P.w.gTpart + fld;
+#pragma unroll
+      for (int r = 0; r < 32; ++r) {
+        cf psi = st[L::native(t, r)];
+        cf T = ob[(size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X];
+        gt[L::native(t, r)] = cmulc(v[r], psi);                  // H10: gT_i contribution conj(Psi) .* gPhi
+        v[r] = cmulc(v[r], T);                                   //      gPsi = conj(T) .* gPhi
+      }
+    } else {
+      // H14 object terms: u = dOhat|patch .* Psi ; chi = -gPhi ; num += Re(chi conj(u)) ; den += |u|^2
+      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * P.onx + r0x + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
+      float num = 0.f, den = 0.f;
+      if (i == 0) {                                              // keep gPhi_0 for the probe / position terms
+        cf* sc0 = P.w.scratch + (size_t)(jl * P.M + k) * NN;
+#pragma unroll
+        for (int r = 0; r < 32; ++r) sc0[L::native(t, r)] = v[r];
+      }
+#pragma unroll
+      for (int r = 0; r < 32; ++r) {
+        const size_t o = (size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X;
+        cf psi = st[L::native(t, r)];
+        cf u = cmul(dO[o], psi);
+        num -= fmaf(v[r].x, u.x, v[r].y * u.y);
+        den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
+        v[r] = cmulc(v[r], ob[o]);
+      }
+      double acc[2] = {(double)num, (double)den};
+      block_sum<G::T, 2>(acc, red);
+      if (t == 0) {
+        double* sp = P.w.step_part + (size_t)(jb * P.M + k) * (2 * S + 6);
+        sp[2 * i] = acc[0]; sp[2 * i + 1] = acc[1];
+      }
+      if (i == 0) break;                                         // probe / position terms handled below
+    }
+    fft2_fwd<G>(v, sm, tw, t);                                   // F(gPsi_i)  (F-layout)
+    if (i > 0) apply_prop<G, true>(v, P.w.hx + (size_t)(i - 1) * N, P.w.hy + (size_t)(i - 1) * N, P.bandlim2, t);
+  }
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
+  const cf* ry = rx + N;
+  const cf* pt = P.w.Pt + (size_t)k * NN;
+  if (MODE == 0) {
+    // v = G~ = F(gPsi_0).  H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
+    cf* gp = P.w.Gpart + (size_t)(jl * P.M + k) * NN;
+    const int qx = L::f_qx(t, 0);
+    const cf wx = rx[qx];
+    const float fx = (float)signed_freq(qx, N) / (float)N;
+    float sy = 0.f, sx = 0.f;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+      const int qy = L::f_qy(t, r);
+      const cf R = cmul(wx, ry[qy]);
+      gp[L::native(t, r)] = cmulc(v[r], R);
+      if (want_pos) {
+        const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);  // conj(G~) R P~
+        const float fy = (float)signed_freq(qy, N) / (float)N;
+        sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
+      }
+    }
+    if (want_pos) {
+      double acc[2] = {(double)sy, (double)sx};
+      block_sum<G::T, 2>(acc, red);
+      if (t == 0) {
+        const double f = 4.0 * CUDART_PI / ((double)N * (double)N);
+        P.w.posg_part[(size_t)(jb * P.M + k) * 2 + 0] = f * acc[0];
+        P.w.posg_part[(size_t)(jb * P.M + k) * 2 + 1] = f * acc[1];
+      }
+    }
+  } else {
+    // H14 probe and position terms at slice 0 (O14): three more fields from the Fourier side, each
+    // compared with chi_0 = -gPhi_0 (kept in scratch) after multiplication by T_0.
+    const cf* sc0 = P.w.scratch + (size_t)(jl * P.M + k) * NN;
+    const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
+    const cf* qt = P.w.Qt + (size_t)k * NN;
+    const int qx = L::f_qx(t, 0);
+    const cf wx = cscale(rx[qx], 1.0f / (float)NN);
+    const float fx = (float)signed_freq(qx, N) / (float)N;
+    double* sp = P.w.step_part + (size_t)(jb * P.M + k) * (2 * S + 6) + 2 * S;
+    for (int term = 0; term < 3; ++term) {
+#pragma unroll
+      for (int r = 0; r < 32; ++r) {
+        const int qy = L::f_qy(t, r);
+        const cf R = cmul(wx, ry[qy]);
+        if (term == 0) v[r] = cmul(R, qt[L::native(t, r)]);                       // shift_j(dPhat_k)
+        else {
+          const float f = term == 1 ? (float)signed_freq(qy, N) / (float)N : fx;  // d Psi_0 / d delta_a
+          const cf z = cmul(R, pt[L::native(t, r)]);
+          const float g = -2.0f * CUDART_PI_F * f;
+          v[r] = make_float2(-g * z.y, g * z.x);                                  // (i g) z
+        }
+      }
+      fft2_inv<G>(v, sm, tw, t);
+      float num = 0.f, den = 0.f;
+#pragma unroll
+      for (int r = 0; r < 32; ++r) {
+        const size_t o = (size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X;
+        const cf u = cmul(v[r], ob[o]);
+        const cf g = sc0[L::native(t, r)];
+        num -= fmaf(g.x, u.x, g.y * u.y);
+        den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
+      }
+      double acc[2] = {(double)num, (double)den};
+      block_sum<G::T, 2>(acc, red);
+      if (t == 0) { sp[2 * term] = acc[0]; sp[2 * term + 1] = acc[1]; }
+      __syncthreads();
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// H11: deterministic object-gradient scatter-add as an owner-computes gather.  Block = 32 x 8 object pixels of
+// one slice; each pixel sums, in fixed (j ascending, k ascending) order, the patch-gradient entries that
+// land on it, in fp64, then adds the chunk total to gO once.  Optionally the illumination map (O12).
+// ------------------------------------------------------------------------------------------------
+template <class G, bool ILLUM>
+__global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illum) {
+  typedef Lay<G> L;
+  constexpr int N = G::N, NN = N * N;
+  __shared__ int2 sr0[256];
+  const int i = blockIdx.z;
+  const int ox0 = blockIdx.x * 32, oy0 = blockIdx.y * 8;
+  const int ox = ox0 + threadIdx.x, oy = oy0 + threadIdx.y;
+  const int tid = threadIdx.y * 32 + threadIdx.x;
+  double ar = 0.0, ai = 0.0, al = 0.0;
+  for (int jbase = 0; jbase < P.jc; jbase += 256) {
+    const int cnt = min(256, P.jc - jbase);
+    if (tid < cnt) sr0[tid] = make_int2(P.w.r0[2 * (P.j0 + jbase + tid) + 1], P.w.r0[2 * (P.j0 + jbase + tid)]);  // (x, y)
+    __syncthreads();
+    for (int jj = 0; jj < cnt; ++jj) {
+      const int2 r0 = sr0[jj];
+      if (r0.x > ox0 + 31 || r0.x + N <= ox0 || r0.y > oy0 + 7 || r0.y + N <= oy0) continue;   // block-uniform reject
+      const int px = ox - r0.x, py = oy - r0.y;
+      if (px >= 0 && px < N && py >= 0 && py < N) {
+        const int idx = L::r_native_of(py, px);
+        const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
+        for (int k = 0; k < P.M; ++k) {
+          const cf g = P.w.gTpart[base + (size_t)k * P.S * NN];
+          ar += (double)g.x; ai += (double)g.y;
+          if (ILLUM) { const cf s = P.w.stash[base + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
+        }
+      }
+    }
+    __syncthreads();
+  }
+  if (ox < P.onx && oy < P.ony) {
+    const size_t o = ((size_t)i * P.ony + oy) * P.onx + ox;
+    cf cur = gO[o];
+    gO[o] = make_float2((float)((double)cur.x + ar), (float)((double)cur.y + ai));
+    if (ILLUM) illum[o] = (float)((double)illum[o] + al);
+  }
+}
+
+// H12: gP~_k[q] += sum_j (chunk) conj(R_j) G~_{k,j}[q], fixed order, fp64
+__global__ void k_reduce_probe(KP P) {
+  const int NN = P.N * P.N;
+  const int e = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
+  if (e >= NN) return;
+  double ar = 0.0, ai = 0.0;
+  for (int jl = 0; jl < P.jc; ++jl) {
+    const cf g = P.w.Gpart[(size_t)(jl * P.M + k) * NN + e];
+    ar += (double)g.x; ai += (double)g.y;
+  }
+  double2 a = P.w.gPt_acc[(size_t)k * NN + e];
+  a.x += ar; a.y += ai;
+  P.w.gPt_acc[(size_t)k * NN + e] = a;
+}
+
+// loss total (fixed-order fp64), position gradients (sum over modes, / px), step-term sums over modes
+__global__ void k_finalize(KP P, double* loss, int accumulate, float* grad_pos, float* step_terms) {
+  __shared__ double red[1024 / 32];
+  const int t = threadIdx.x;
+  if (loss) {
+    double acc[1] = {0.0};
+    for (int j = t; j < P.J; j += 1024) acc[0] += P.w.loss_pp[j];
+    block_sum<1024, 1>(acc, red);
+    if (t == 0) *loss = (accumulate ? *loss : 0.0) + acc[0];
+  }
+  if (grad_pos)
+    for (int j = t; j < P.J; j += 1024) {
+      double sy = 0.0, sx = 0.0;
+      for (int k = 0; k < P.M; ++k) { sy += P.w.posg_part[(size_t)(j * P.M + k) * 2]; sx += P.w.posg_part[(size_t)(j * P.M + k) * 2 + 1]; }
+      grad_pos[2 * j] = (float)(sy / (double)P.px);
+      grad_pos[2 * j + 1] = (float)(sx / (double)P.px);
+    }
+  if (step_terms) {
+    const int W = 2 * P.S + 6;
+    for (int idx = t; idx < P.J * W; idx += 1024) {
+      const int j = idx / W, c = idx - j * W;
+      double s = 0.0;
+      for (int k = 0; k < P.M; ++k) s += P.w.step_part[(size_t)(j * P.M + k) * W + c];
+      step_terms[idx] = (float)s;
+    }
+  }
+}
+
+__global__ void k_zero(float* p, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  const size_t stride = (size_t)gridDim.x * blockDim.x;
+  for (; i < n; i += stride) p[i] = 0.f;
+}
+
+// O13: dOhat = -gO / (illum_prev + delta_O)
+__global__ void k_dohat(const cf* gO, const float* illum_prev, float delta_o, cf* out, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float d = -1.0f / (illum_prev[i] + delta_o);
+  out[i] = make_float2(gO[i].x * d, gO[i].y * d);
+}
+
+// ------------------------------------------------------------------------------------------------
+// H15 update kernels
+// ------------------------------------------------------------------------------------------------
+__global__ void k_axpy(float* z, const float* g, float a, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i < n) z[i] = fmaf(a, g[i], z[i]);
+}
+__global__ void k_pos_sgd(float* pos, const float* g, const int32_t* idx, float lr, int J) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= J) return;
+  int row = idx ? idx[j] : j;
+  pos[2 * row] -= lr * g[2 * j]; pos[2 * row + 1] -= lr * g[2 * j + 1];
+}
+// alpha[c] = sum_j num / (sum_j den + gamma) for c = 0..S (S object slices, then the probe); one block per c
+__global__ void k_lsqml_alpha(const float* step_terms, int J, int S, float gamma, float* alpha) {
+  __shared__ double red[(256 / 32) * 2];
+  const int c = blockIdx.x, W = 2 * S + 6;
+  double acc[2] = {0.0, 0.0};
+  for (int j = threadIdx.x; j < J; j += 256) { acc[0] += step_terms[(size_t)j * W + 2 * c]; acc[1] += step_terms[(size_t)j * W + 2 * c + 1]; }
+  block_sum<256, 2>(acc, red);
+  if (threadIdx.x == 0) alpha[c] = (float)(acc[0] / (acc[1] + (double)gamma));
+}
+__global__ void k_lsqml_object(cf* O, const cf* gO, const float* illum_prev, const float* alpha, float beta, float delta_o,
+                               size_t slice_elems, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float a = beta * alpha[i / slice_elems] * (-1.0f / (illum_prev[i] + delta_o));
+  O[i] = make_float2(fmaf(a, gO[i].x, O[i].x), fmaf(a, gO[i].y, O[i].y));
+}
+__global__ void k_lsqml_probe(cf* Pr, const cf* gP, const float* alpha, int S, float beta, float delta_p, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float a = beta * alpha[S] * (-1.0f / (delta_p + 1.0f));
+  Pr[i] = make_float2(fmaf(a, gP[i].x, Pr[i].x), fmaf(a, gP[i].y, Pr[i].y));
+}
+__global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* idx, int J, int S, float px, float gamma) {
+  int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j >= J) return;
+  const int W = 2 * S + 6; int row = idx ? idx[j] : j;
+  const float* s = step_terms + (size_t)j * W + 2 * S + 2;
+  pos[2 * row] += px * s[0] / (s[1] + gamma);
+  pos[2 * row + 1] += px * s[2] / (s[3] + gamma);
+}
+
+// ------------------------------------------------------------------------------------------------
+// launch accounting + optional per-kernel timing (ptycho_profile_*): when enabled, one CUDA event is recorded on
+// the launching stream after every kernel (and one at the start of each public call); a stream runs its work in
+// order, so the time between consecutive events is that kernel's duration as seen on the device.
+// ------------------------------------------------------------------------------------------------
+enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
+            K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
+            K_lsqml_pos, K_COUNT };
+const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
+                                         "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
+                                         "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos"};
+thread_local int64_t g_launches = 0;
+thread_local bool g_prof_on = false;
+struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
+thread_local std::vector<ProfMark> g_prof;
+
+inline void prof_mark(int kind, cudaStream_t st) {
+  if (!g_prof_on) return;
+  ProfMark m; m.kind = kind;
+  if (cudaEventCreate(&m.ev) != cudaSuccess) return;
+  cudaEventRecord(m.ev, st);
+  g_prof.push_back(m);
+}
+
+#define LAUNCH_CHECK(kind, st)                                  \
+  do {                                                          \
+    ++g_launches;                                               \
+    if (cudaGetLastError() != cudaSuccess) return PT_ERR_CUDA;  \
+    prof_mark(kind, st);                                        \
+  } while (0)
+
+int validate(const pt_problem* p) {
+  if (!p) return PT_ERR_NULL;
+  if (p->n != 64 && p->n != 128) return p->n == 256 ? PT_ERR_UNSUPPORTED : PT_ERR_BAD_SIZE;
+  if (p->n_modes < 1 || p->n_slices < 1 || p->n_batch < 1 || p->n_pos_total < p->n_batch) return PT_ERR_BAD_SIZE;
+  if (p->obj_ny < p->n || p->obj_nx < p->n) return PT_ERR_BAD_SIZE;
+  if (!(p->pixel_size > 0.f) || !(p->wavelength > 0.f) || !(p->eps > 0.f)) return PT_ERR_BAD_PARAM;
+  if (p->loss != PT_LOSS_AMPLITUDE && p->loss != PT_LOSS_POISSON) return PT_ERR_BAD_PARAM;
+  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
+  if (p->shift_mode != PT_SHIFT_FOURIER_PROBE) return PT_ERR_BAD_PARAM;
+  if (p->n_slices > 1 && !p->slice_thickness) return PT_ERR_NULL;
+  if (p->loss_c < 0.f) return PT_ERR_BAD_PARAM;
+  return PT_OK;
+}
+
+KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64* probe, const float* positions,
+           const float* intensity, const int32_t* batch_idx) {
+  KP k;
+  k.N = p->n; k.M = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch;
+  k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
+  const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
+  k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
+  k.loss = p->loss; k.loss_c = p->loss_c; k.eps = p->eps;
+  k.object = (const cf*)object; k.probe = (const cf*)probe; k.positions = positions; k.intensity = intensity;
+  k.batch_idx = batch_idx; k.w = w;
+  return k;
+}
+
+template <class G>
+int set_smem_attrs() {
+  const int b = (int)fft_smem_bytes<G>();
+  if (cudaFuncSetAttribute(k_forward<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_forward<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  return PT_OK;
+}
+
+// common prologue: tables, position split, probe spectrum
+template <class G>
+int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
+  int rc = set_smem_attrs<G>();
+  if (rc != PT_OK) return rc;
+  const int nprop = p->n_slices - 1;
+  for (int i0 = 0; i0 < nprop; i0 += 64) {
+    PropArgs a;
+    a.N = p->n; a.nprop = nprop - i0 < 64 ? nprop - i0 : 64; a.px = (double)p->pixel_size; a.lambda = (double)p->wavelength;
+    a.tx = (double)p->tilt_x_mrad; a.ty = (double)p->tilt_y_mrad; a.hx = kp.w.hx; a.hy = kp.w.hy; a.i0 = i0;
+    for (int i = 0; i < a.nprop; ++i) a.dz[i] = p->slice_thickness[i0 + i];
+    const int n = a.nprop * 2 * a.N;
+    k_setup_prop<<<(n + 255) / 256, 256, 0, st>>>(a);
+    LAUNCH_CHECK(K_setup_prop, st);
+  }
+  k_setup_pos<<<p->n_batch, p->n, 0, st>>>(kp);
+  LAUNCH_CHECK(K_setup_pos, st);
+  k_probe_fft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp.probe, kp.w.Pt, 1.0f);
+  LAUNCH_CHECK(K_probe_fft, st);
+  return PT_OK;
+}
+
+template <class G>
+int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_d, float* model_intensity_d, cudaStream_t st) {
+  int rc = prologue<G>(p, kp, st);
+  if (rc != PT_OK) return rc;
+  for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
+    kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+    k_forward<G, false><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+    LAUNCH_CHECK(K_forward, st);
+    k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, model_intensity_d, 0);
+    LAUNCH_CHECK(K_loss, st);
+  }
+  if (loss_d) {
+    k_finalize<<<1, 1024, 0, st>>>(kp, loss_d, (p->flags & PT_ACCUMULATE) != 0, nullptr, nullptr);
+    LAUNCH_CHECK(K_finalize, st);
+  }
+  return PT_OK;
+}
+
+template <class G>
+int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, float* illum, const float* illum_prev,
+                 float* step_terms, double* loss_d, float* loss_per_pos_d, cudaStream_t st) {
+  int rc = prologue<G>(p, kp, st);
+  if (rc != PT_OK) return rc;
+  const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
+  const bool acc = (p->flags & PT_ACCUMULATE) != 0;
+  const bool want_illum = (p->flags & PT_WANT_ILLUM) && illum;
+  const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX;
+  const bool want_steps = (p->flags & PT_WANT_STEP_SIZES) && step_terms;
+  k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
+  LAUNCH_CHECK(K_zero, st);
+  if (!acc) {
+    k_zero<<<592, 256, 0, st>>>((float*)gO, on * 2);
+    LAUNCH_CHECK(K_zero, st);
+    if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, on); LAUNCH_CHECK(K_zero, st); }
+  }
+  const dim3 ggrid((p->obj_nx + 31) / 32, (p->obj_ny + 7) / 8, p->n_slices), gblock(32, 8);
+  for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
+    kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+    k_forward<G, true><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+    LAUNCH_CHECK(K_forward, st);
+    k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, nullptr, 1);
+    LAUNCH_CHECK(K_loss, st);
+    k_backward<G, 0><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp, want_pos ? 1 : 0);
+    LAUNCH_CHECK(K_backward, st);
+    if (want_illum) k_gather_object<G, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
+    else k_gather_object<G, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
+    LAUNCH_CHECK(K_gather_object, st);
+    k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp);
+    LAUNCH_CHECK(K_reduce_probe, st);
+  }
+  k_probe_ifft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0);
+  LAUNCH_CHECK(K_probe_ifft, st);
+  if (want_steps) {
+    // H14 second sweep (O13/O14): needs the batch-aggregated gO, gP
+    k_dohat<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((const cf*)gO, illum_prev, p->lsqml_delta_o, kp.w.dOhat, on);
+    LAUNCH_CHECK(K_dohat, st);
+    k_probe_fft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>((const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f));
+    LAUNCH_CHECK(K_probe_fft, st);
+    for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
+      kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+      if (kp.w.Jc < p->n_batch) {   // stash of this chunk was overwritten: recompute it
+        k_forward<G, true><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+        LAUNCH_CHECK(K_forward, st);
+        k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, nullptr, nullptr, 1);
+        LAUNCH_CHECK(K_loss, st);
+      }
+      k_backward<G, 1><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp, 0);
+      LAUNCH_CHECK(K_backward, st);
+    }
+  }
+  k_finalize<<<1, 1024, 0, st>>>(kp, loss_d, acc ? 1 : 0, want_pos ? gX : nullptr, want_steps ? step_terms : nullptr);
+  LAUNCH_CHECK(K_finalize, st);
+  return PT_OK;
+}
+
+}  // namespace
+
+// ==================================================================================================
+// C ABI
+// ==================================================================================================
+extern "C" {
+
+size_t ptycho_workspace_min_bytes(const pt_problem* p) {
+  if (validate(p) != PT_OK) return 0;
+  size_t f, pp; ws_sizes(p, &f, &pp);
+  return f + pp;
+}
+
+size_t ptycho_workspace_bytes(const pt_problem* p) {
+  if (validate(p) != PT_OK) return 0;
+  size_t f, pp; ws_sizes(p, &f, &pp);
+  const size_t cap = (size_t)32 << 30;
+  size_t jc = p->n_batch;
+  if (f + jc * pp > cap) {
+    jc = (cap - f) / pp;
+    // whole waves of 148 CTAs per chunk where possible
+    const size_t wave = 148;
+    size_t pairs = jc * p->n_modes;
+    if (pairs > wave) { pairs -= pairs % wave; jc = pairs / p->n_modes; }
+    if (jc < 1) jc = 1;
+  }
+  return f + jc * pp;
+}
+
+int32_t ptycho_forward_loss(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
+                            const float* intensity_d, const int32_t* batch_idx_d, double* loss_d, float* loss_per_pos_d,
+                            float* model_intensity_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!object_d || !probe_d || !positions_d || !workspace_d) return PT_ERR_NULL;
+  Ws w;
+  pt_problem q = *p; q.flags &= ~PT_WANT_STEP_SIZES;
+  rc = ws_layout(&q, workspace_d, workspace_bytes, &w);
+  if (rc != PT_OK) return rc;
+  KP kp = make_kp(p, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  return p->n == 128 ? run_forward<Geo<128>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st)
+                     : run_forward<Geo<64>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st);
+}
+
+int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
+                        const float* intensity_d, const int32_t* batch_idx_d, pt_c64* grad_object_d, pt_c64* grad_probe_d,
+                        float* grad_pos_d, float* illum_d, const float* illum_prev_d, float* step_terms_d, double* loss_d,
+                        float* loss_per_pos_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
+  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
+  Ws w;
+  pt_problem q = *p;
+  if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
+  rc = ws_layout(&q, workspace_d, workspace_bytes, &w);
+  if (rc != PT_OK) return rc;
+  KP kp = make_kp(&q, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  return p->n == 128 ? run_gradient<Geo<128>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st)
+                     : run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st);
+}
+
+int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe_d, float* positions_d,
+                            const pt_c64* grad_object_d, const pt_c64* grad_probe_d, const float* grad_pos_d,
+                            const float* illum_prev_d, const float* step_terms_d, const int32_t* batch_idx_d,
+                            const pt_update* u, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!u) return PT_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  const size_t NN = (size_t)p->n * p->n, os = (size_t)p->obj_ny * p->obj_nx, on = os * p->n_slices, pn = NN * p->n_modes;
+  if (u->mode == PT_UPDATE_SGD) {
+    if (object_d && grad_object_d) { k_axpy<<<(unsigned)((2 * on + 255) / 256), 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, -u->lr_obj, 2 * on); LAUNCH_CHECK(K_axpy, st); }
+    if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, -u->lr_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
+    if (positions_d && grad_pos_d) { k_pos_sgd<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, grad_pos_d, batch_idx_d, u->lr_pos, p->n_batch); LAUNCH_CHECK(K_pos_sgd, st); }
+    return PT_OK;
+  }
+  if (u->mode != PT_UPDATE_LSQML) return PT_ERR_BAD_PARAM;
+  if (!step_terms_d || !workspace_d) return PT_ERR_NULL;
+  if (workspace_bytes < 256 + (size_t)(p->n_slices + 1) * sizeof(float)) return PT_ERR_WORKSPACE;
+  float* alpha = (float*)((char*)workspace_d + 256);
+  k_lsqml_alpha<<<p->n_slices + 1, 256, 0, st>>>(step_terms_d, p->n_batch, p->n_slices, u->gamma, alpha);
+  LAUNCH_CHECK(K_lsqml_alpha, st);
+  if (object_d && grad_object_d) {
+    if (!illum_prev_d) return PT_ERR_NULL;
+    k_lsqml_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, alpha, u->beta_obj, p->lsqml_delta_o, os, on);
+    LAUNCH_CHECK(K_lsqml_object, st);
+  }
+  if (probe_d && grad_probe_d) {
+    k_lsqml_probe<<<(unsigned)((pn + 255) / 256), 256, 0, st>>>((cf*)probe_d, (const cf*)grad_probe_d, alpha, p->n_slices, u->beta_probe, p->lsqml_delta_p, pn);
+    LAUNCH_CHECK(K_lsqml_probe, st);
+  }
+  if (positions_d) {
+    k_lsqml_pos<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, step_terms_d, batch_idx_d, p->n_batch, p->n_slices, p->pixel_size, u->gamma);
+    LAUNCH_CHECK(K_lsqml_pos, st);
+  }
+  return PT_OK;
+}
+
+size_t ptycho_workspace_host_bytes(const pt_problem* p) {
+  if (validate(p) != PT_OK) return 0;
+  const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx, pn = NN * p->n_modes, J = p->n_batch;
+  size_t s = align_up(on * 8) * 2 + align_up(pn * 8) * 2 + align_up(J * 8) * 2 + align_up(J * NN * 4) + align_up(J * 4) + 256;
+  return s + ptycho_workspace_bytes(p);
+}
+
+int32_t ptycho_gradient_host(const pt_problem* p, const pt_c64* object_h, const pt_c64* probe_h, const float* positions_h,
+                             const float* intensity_h, const int32_t* batch_idx_h, pt_c64* grad_object_h, pt_c64* grad_probe_h,
+                             float* grad_pos_h, double* loss_h, float* loss_per_pos_h, void* workspace_d, size_t workspace_bytes,
+                             void* cuda_stream) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!object_h || !probe_h || !positions_h || !intensity_h || !grad_object_h || !grad_probe_h || !workspace_d) return PT_ERR_NULL;
+  if (workspace_bytes < ptycho_workspace_host_bytes(p)) return PT_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx, pn = NN * p->n_modes, J = p->n_batch;
+  char* c = (char*)workspace_d; size_t off = 0;
+  auto take = [&](size_t n) { char* r = c + off; off += align_up(n); return (void*)r; };
+  pt_c64* obj_d = (pt_c64*)take(on * 8); pt_c64* gO_d = (pt_c64*)take(on * 8);
+  pt_c64* pr_d = (pt_c64*)take(pn * 8); pt_c64* gP_d = (pt_c64*)take(pn * 8);
+  float* pos_d = (float*)take(J * 8); float* gX_d = (float*)take(J * 8);
+  float* int_d = (float*)take(J * NN * 4); float* lpp_d = (float*)take(J * 4);
+  double* loss_d = (double*)take(256);
+  void* ws = c + off;
+  // the batch rows are compacted on the way in: the device sees rows 0..J-1
+  if (cudaMemcpyAsync(obj_d, object_h, on * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaMemcpyAsync(pr_d, probe_h, pn * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (!batch_idx_h) {
+    if (cudaMemcpyAsync(pos_d, positions_h, J * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+    if (cudaMemcpyAsync(int_d, intensity_h, J * NN * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+  } else {
+    for (size_t j = 0; j < J; ++j) {
+      const size_t row = batch_idx_h[j];
+      if (cudaMemcpyAsync(pos_d + 2 * j, positions_h + 2 * row, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+      if (cudaMemcpyAsync(int_d + j * NN, intensity_h + row * NN, NN * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+    }
+  }
+  pt_problem q = *p;
+  q.n_pos_total = (int32_t)J; q.flags &= ~(PT_ACCUMULATE | PT_WANT_STEP_SIZES | PT_WANT_ILLUM);
+  if (grad_pos_h) q.flags |= PT_WANT_POS_GRAD;
+  rc = ptycho_gradient(&q, obj_d, pr_d, pos_d, int_d, nullptr, gO_d, gP_d, grad_pos_h ? gX_d : nullptr, nullptr, nullptr, nullptr,
+                       loss_d, lpp_d, ws, workspace_bytes - off, st);
+  if (rc != PT_OK) return rc;
+  if (cudaMemcpyAsync(grad_object_h, gO_d, on * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaMemcpyAsync(grad_probe_h, gP_d, pn * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (grad_pos_h && cudaMemcpyAsync(grad_pos_h, gX_d, J * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (loss_h && cudaMemcpyAsync(loss_h, loss_d, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (loss_per_pos_h && cudaMemcpyAsync(loss_per_pos_h, lpp_d, J * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return PT_ERR_CUDA;
+  return PT_OK;
+}
+
+int32_t ptycho_status(void* workspace_d, void* cuda_stream) {
+  if (!workspace_d) return PT_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int32_t s = 0;
+  if (cudaMemcpyAsync(&s, workspace_d, sizeof(s), cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaMemsetAsync(workspace_d, 0, sizeof(s), st) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaStreamSynchronize(st) != cudaSuccess) return PT_ERR_CUDA;
+  if (s & kStatusOOB) return PT_ERR_OUT_OF_BOUNDS;
+  if (s & kStatusNonfinite) return PT_ERR_NONFINITE;
+  return PT_OK;
+}
+
+int64_t ptycho_launch_count(void) { return g_launches; }
+
+int32_t ptycho_profile_enable(int32_t on) {
+  for (auto& m : g_prof) cudaEventDestroy(m.ev);
+  g_prof.clear();
+  g_prof_on = on != 0;
+  return PT_OK;
+}
+
+int32_t ptycho_profile_num_kernels(void) { return K_COUNT; }
+
+const char* ptycho_profile_kernel_name(int32_t kind) { return kind >= 0 && kind < K_COUNT ? kKindNames[kind] : ""; }
+
+int32_t ptycho_profile_read(float* ms_h, int64_t* launches_h) {
+  if (!ms_h || !launches_h) return PT_ERR_NULL;
+  for (int k = 0; k < K_COUNT; ++k) { ms_h[k] = 0.f; launches_h[k] = 0; }
+  for (size_t i = 0; i < g_prof.size(); ++i) {
+    if (cudaEventSynchronize(g_prof[i].ev) != cudaSuccess) return PT_ERR_CUDA;
+    if (g_prof[i].kind < 0 || i == 0) continue;
+    float ms = 0.f;
+    if (cudaEventElapsedTime(&ms, g_prof[i - 1].ev, g_prof[i].ev) != cudaSuccess) return PT_ERR_CUDA;
+    ms_h[g_prof[i].kind] += ms;
+    launches_h[g_prof[i].kind] += 1;
+  }
+  for (auto& m : g_prof) cudaEventDestroy(m.ev);
+  g_prof.clear();
+  return PT_OK;
+}
+
+const char* ptycho_strerror(int32_t code) {
+  switch (code) {
+    case PT_OK: return "ok";
+    case PT_ERR_NULL: return "null pointer";
+    case PT_ERR_BAD_SIZE: return "unsupported or inconsistent size";
+    case PT_ERR_BAD_PARAM: return "bad parameter";
+    case PT_ERR_WORKSPACE: return "workspace too small";
+    case PT_ERR_CUDA: return "CUDA error";
+    case PT_ERR_OUT_OF_BOUNDS: return "a probe window leaves the object";
+    case PT_ERR_NONFINITE: return "non-finite loss";
+    case PT_ERR_UNSUPPORTED: return "not supported by this build";
+    default: return "unknown error";
+  }
+}
+
+}  // extern "C"

@@ -1,0 +1,300 @@
+"""Parity of the CUDA path (through the C ABI, include/ptycho.h) against the CPU oracle, element by element,
+on the same seeded inputs.  Tolerances are north_star's: loss <= 1e-5 relative, gradients <= 1e-4 relative L2
+(fp32 complex on the GPU vs fp64 in the oracle).  Everything here needs a B200: marked gpu.
+"""
+import numpy as np
+import pytest
+
+from oracle import oracle as orc
+from paper_2505_14372_b200 import synth
+from tests._cases import make_case, oracle_problem, gpu_problem, rel_l2
+
+pytestmark = pytest.mark.gpu
+
+TOL_LOSS = 1e-5     # relative (north_star)
+TOL_GRAD = 1e-4     # relative L2 per array (north_star)
+TOL_INT = 2e-6      # model intensity, relative L2 (fp32 FFT chain)
+
+
+def _t(a, dtype=None):
+    import torch
+    t = torch.from_numpy(np.ascontiguousarray(a))
+    if dtype is not None:
+        t = t.to(dtype)
+    return t.cuda()
+
+
+def gpu_gradient(case, pbg, batch_idx=None, flags=0, want_pos=True, want_illum=False, max_ws=None, obj=None,
+                 positions=None, acc_into=None):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = case.cfg
+    obj_d = _t(case.obj_start if obj is None else obj)
+    pr_d = _t(case.probe)
+    pos_d = _t(case.positions if positions is None else positions)
+    I_d = _t(case.intensity)
+    b_d = None if batch_idx is None else _t(np.asarray(batch_idx, np.int32))
+    J = pos_d.shape[0] if b_d is None else b_d.numel()
+    if acc_into is None:
+        gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+        loss = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+        illum = torch.full(obj_d.shape, float("nan"), dtype=torch.float32, device="cuda") if want_illum else None
+    else:
+        gO, gP, loss, illum = acc_into
+    gX = torch.full((J, 2), float("nan"), dtype=torch.float32, device="cuda") if want_pos else None
+    lpp = torch.full((J,), float("nan"), dtype=torch.float32, device="cuda")
+    ws = ptycho.make_workspace(pbg, pos_d.shape[0], J, flags, max_bytes=max_ws)
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, b_d, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX,
+                    illum=illum, loss=loss, loss_per_pos=lpp, flags=flags)
+    assert ptycho.status(ws) == 0
+    out = dict(loss=float(loss.item()), loss_per_pos=lpp.cpu().numpy(), grad_object=gO.cpu().numpy(),
+               grad_probe=gP.cpu().numpy(), grad_pos=None if gX is None else gX.cpu().numpy(),
+               illum=None if illum is None else illum.cpu().numpy(), _dev=(gO, gP, loss, illum))
+    return out
+
+
+def check(g, o, tol_grad=TOL_GRAD, pos=True):
+    assert abs(g["loss"] - o["loss"]) <= TOL_LOSS * abs(o["loss"]), (g["loss"], o["loss"])
+    assert np.max(np.abs(g["loss_per_pos"] - o["loss_per_pos"]) / np.maximum(np.abs(o["loss_per_pos"]), 1e-30)) <= 2e-5
+    assert rel_l2(g["grad_object"], o["grad_object"]) <= tol_grad
+    assert rel_l2(g["grad_probe"], o["grad_probe"]) <= tol_grad
+    if pos:
+        assert rel_l2(g["grad_pos"], o["grad_pos"]) <= tol_grad
+
+
+# ------------------------------------------------------------------------------------------------
+# config 1 at full size: N=64, 256 positions, 1 mode, 1 slice, amplitude loss, vacuum start
+# ------------------------------------------------------------------------------------------------
+def test_cfg1_full():
+    cfg = synth.config(1)
+    case = make_case(cfg, start_scale=0.0, noise=False)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
+def test_cfg1_forward_intensity():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(1)
+    case = make_case(cfg, noise=False)
+    pbg = gpu_problem(cfg)
+    J = cfg.n_pos
+    mi = torch.empty((J, cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda"); lpp = torch.zeros(J, dtype=torch.float32, device="cuda")
+    ws = ptycho.make_workspace(pbg, J, J)
+    ptycho.forward_loss(pbg, _t(case.obj_true), _t(case.probe), _t(case.positions_true), _t(case.intensity),
+                        workspace=ws, loss=loss, loss_per_pos=lpp, model_intensity=mi)
+    assert ptycho.status(ws) == 0
+    o = orc.forward_loss(oracle_problem(cfg), case.obj_true, case.probe, case.positions_true, case.intensity)
+    assert rel_l2(mi.cpu().numpy(), o["intensity"]) <= TOL_INT
+    # noiseless data at the true state: the loss is ~0 on both sides (absolute check, electrons)
+    assert abs(loss.item() - o["loss"]) <= 1e-5 * cfg.dose * J * 1e-3
+    # and without measured data only the model intensity is produced
+    mi2 = torch.empty_like(mi)
+    ptycho.forward_loss(pbg, _t(case.obj_true), _t(case.probe), _t(case.positions_true), None, workspace=ws, model_intensity=mi2)
+    assert torch.equal(mi, mi2)
+
+
+# ------------------------------------------------------------------------------------------------
+# config 2 (reduced scan, full N / modes): N=128, 4 modes, amplitude loss, Poisson data, states (a) and (b)
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("start", [0.0, 0.8])
+def test_cfg2_reduced(start):
+    cfg = synth.config(2, scan=(7, 9))
+    case = make_case(cfg, start_scale=start)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
+# ------------------------------------------------------------------------------------------------
+# config 3 (reduced scan, full N / modes / slices): 8 modes, 20 slices, tilt, Poisson loss.
+# The workspace is capped so the batch runs in several chunks with a ragged last chunk.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("start", [0.0, 0.8])
+def test_cfg3_reduced_chunked(start):
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(3, scan=(5, 6))
+    case = make_case(cfg, start_scale=start)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    pbg = gpu_problem(cfg)
+    min_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos, minimum=True)
+    full_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos)
+    cap = min_ws + (full_ws - min_ws) * 7 // 29 + 4096          # room for 8 positions per chunk: 30 = 8+8+8+6
+    g = gpu_gradient(case, pbg, want_illum=True, max_ws=cap)
+    check(g, o)
+    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    g1 = gpu_gradient(case, pbg, want_illum=True)                # one chunk
+    check(g1, o)
+
+
+def test_bandlimit_and_anscombe():
+    cfg = synth.config(3, scan=(3, 4), n_modes=2, n_slices=3, bandlimit=2.0 / 3.0, loss=synth.LOSS_AMPLITUDE,
+                       loss_c=0.375, eps=0.5)
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
+def test_n64_multislice_multimode():
+    cfg = synth.config(3, n=64, scan=(6, 5), n_modes=3, n_slices=4, obj_n=200, pixel_size=0.2, step_px=3.0)
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
+# ------------------------------------------------------------------------------------------------
+# mini-batches: batch_idx subsets + PT_ACCUMULATE over the batches == one call over all positions
+# ------------------------------------------------------------------------------------------------
+def test_batches_accumulate():
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(2, scan=(6, 6), n_modes=2)
+    case = make_case(cfg, start_scale=0.8)
+    pbo, pbg = oracle_problem(cfg), gpu_problem(cfg)
+    o_all = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity)
+    bs = synth.batches(cfg, 13)                                  # 13 + 13 + 10, seeded permutation
+    acc = None
+    for i, b in enumerate(bs):
+        ob = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, batch_idx=b)
+        g = gpu_gradient(case, pbg, batch_idx=b, flags=(ptycho.ACCUMULATE if i else 0), acc_into=acc)
+        acc = g["_dev"]
+        assert rel_l2(g["grad_pos"], ob["grad_pos"]) <= TOL_GRAD
+        assert np.max(np.abs(g["loss_per_pos"] - ob["loss_per_pos"]) / np.abs(ob["loss_per_pos"])) <= 2e-5
+    assert abs(g["loss"] - o_all["loss"]) <= TOL_LOSS * abs(o_all["loss"])
+    assert rel_l2(g["grad_object"], o_all["grad_object"]) <= TOL_GRAD
+    assert rel_l2(g["grad_probe"], o_all["grad_probe"]) <= TOL_GRAD
+
+
+def test_deterministic_bitwise():
+    cfg = synth.config(3, scan=(4, 5), n_modes=3, n_slices=4)
+    case = make_case(cfg, start_scale=0.8)
+    pbg = gpu_problem(cfg)
+    a = gpu_gradient(case, pbg)
+    for _ in range(2):
+        b = gpu_gradient(case, pbg)
+        for k in ("grad_object", "grad_probe", "grad_pos", "loss_per_pos"):
+            assert a[k].tobytes() == b[k].tobytes()
+        assert a["loss"] == b["loss"]
+
+
+# ------------------------------------------------------------------------------------------------
+# config 5: position gradients at offset positions, illumination map, LSQML-style step terms and update
+# ------------------------------------------------------------------------------------------------
+def test_cfg5_step_terms_and_lsqml_update():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(5, scan=(4, 5), n_modes=4, n_slices=6)
+    case = make_case(cfg, start_scale=0.8)
+    pbo, pbg = oracle_problem(cfg, lsqml_delta_o=50.0, lsqml_delta_p=0.5), gpu_problem(cfg, lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    illum_prev = (o["illum"] * 0.9).astype(np.float32)
+    J, S = cfg.n_pos, cfg.n_slices
+    st_o = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity,
+                          o["grad_object"], o["grad_probe"], illum_prev)
+    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity)
+    ip_d = _t(illum_prev)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d); gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
+    il = torch.empty(obj_d.shape, dtype=torch.float32, device="cuda")
+    st = torch.empty((J, 2 * S + 6), dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    fl = ptycho.WANT_POS_GRAD | ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES
+    ws = ptycho.make_workspace(pbg, J, J, fl)
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il,
+                    illum_prev=ip_d, step_terms=st, loss=loss)
+    assert ptycho.status(ws) == 0
+    assert rel_l2(gO.cpu().numpy(), o["grad_object"]) <= TOL_GRAD
+    assert rel_l2(gX.cpu().numpy(), o["grad_pos"]) <= TOL_GRAD
+    assert rel_l2(il.cpu().numpy(), o["illum"]) <= TOL_GRAD
+    stg = st.cpu().numpy().astype(np.float64)
+    # numerators / denominators column by column (each an L2 over positions)
+    for c in range(2 * S + 6):
+        assert rel_l2(stg[:, c], st_o[:, c]) <= 3e-4, c
+    # the update itself, from the GPU's own gradients and step terms, against the oracle's from its own
+    o_new, p_new, x_new = orc.apply_update(pbo, 1, case.obj_start, case.probe, case.positions, o["grad_object"], o["grad_probe"],
+                                           None, illum_prev, st_o, beta_obj=0.9, beta_probe=0.8, gamma=1e-3)
+    ptycho.apply_update(pbg, obj_d, pr_d, pos_d, grad_object=gO, grad_probe=gP, illum_prev=ip_d, step_terms=st,
+                        mode=ptycho.UPDATE_LSQML, beta_obj=0.9, beta_probe=0.8, gamma=1e-3, workspace=ws)
+    torch.cuda.synchronize()
+    assert rel_l2(obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start) <= 5e-4
+    assert rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe) <= 5e-4
+    assert rel_l2(pos_d.cpu().numpy() - case.positions, x_new - case.positions) <= 5e-3   # fp32 positions: ulp(20 A) ~ 2e-6 on steps ~ 1e-2
+    # chunked second sweep (the stash is recomputed per chunk) gives the same step terms
+    min_ws = ptycho.workspace_bytes(pbg, J, J, fl, minimum=True)
+    full_ws = ptycho.workspace_bytes(pbg, J, J, fl)
+    ws2 = ptycho.make_workspace(pbg, J, J, fl, max_bytes=min_ws + (full_ws - min_ws) * 6 // 19 + 4096)
+    st2 = torch.empty_like(st)
+    ptycho.gradient(pbg, _t(case.obj_start), _t(case.probe), _t(case.positions), I_d, None, workspace=ws2, grad_object=gO,
+                    grad_probe=gP, grad_pos=gX, illum=il, illum_prev=ip_d, step_terms=st2, loss=loss)
+    assert ptycho.status(ws2) == 0
+    for c in range(2 * S + 6):
+        assert rel_l2(st2.cpu().numpy()[:, c], st_o[:, c]) <= 3e-4, c
+
+
+def test_sgd_update():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(2, scan=(3, 3), n_modes=2)
+    case = make_case(cfg, start_scale=0.8)
+    pbo, pbg = oracle_problem(cfg), gpu_problem(cfg)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity)
+    b = np.array([7, 2, 5], np.int32)
+    gX = o["grad_pos"][b]
+    o_new, p_new, x_new = orc.apply_update(pbo, 0, case.obj_start, case.probe, case.positions, o["grad_object"], o["grad_probe"],
+                                           gX, batch_idx=b, lr_obj=1e-3, lr_probe=2e-3, lr_pos=1e-4)
+    obj_d, pr_d, pos_d = _t(case.obj_start), _t(case.probe), _t(case.positions)
+    ptycho.apply_update(pbg, obj_d, pr_d, pos_d, grad_object=_t(o["grad_object"].astype(np.complex64)),
+                        grad_probe=_t(o["grad_probe"].astype(np.complex64)), grad_pos=_t(gX.astype(np.float32)),
+                        batch_idx=_t(b), mode=ptycho.UPDATE_SGD, lr_obj=1e-3, lr_probe=2e-3, lr_pos=1e-4)
+    torch.cuda.synchronize()
+    assert rel_l2(obj_d.cpu().numpy(), o_new) <= 1e-6
+    assert rel_l2(pr_d.cpu().numpy(), p_new) <= 1e-6
+    assert np.max(np.abs(pos_d.cpu().numpy() - x_new)) <= 4e-6
+
+
+# ------------------------------------------------------------------------------------------------
+# boundary behaviour
+# ------------------------------------------------------------------------------------------------
+def test_out_of_bounds_flag_and_errors():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(1, scan=(2, 2))
+    case = make_case(cfg, noise=False)
+    pbg = gpu_problem(cfg)
+    bad = case.positions.copy(); bad[1, 0] = 5.0                  # window would start at a negative row
+    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(bad), _t(case.intensity)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d)
+    ws = ptycho.make_workspace(pbg, 4, 4)
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP)
+    assert ptycho.status(ws) == -6                                # PT_ERR_OUT_OF_BOUNDS, deferred (R4)
+    assert ptycho.status(ws) == 0                                 # cleared
+    assert torch.isfinite(torch.view_as_real(gO)).all()           # clamped window: no wild reads
+    with pytest.raises(ptycho.PtychoError) as e:                  # workspace too small
+        ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws[:1024], grad_object=gO, grad_probe=gP)
+    assert e.value.code == -4
+    import dataclasses
+    with pytest.raises(ptycho.PtychoError) as e:                  # eps must be positive (R13)
+        ptycho.gradient(dataclasses.replace(pbg, eps=0.0), obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP)
+    assert e.value.code == -3
+
+
+def test_gradient_host_matches_device_path():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(2, scan=(4, 4), n_modes=2)
+    case = make_case(cfg, start_scale=0.8)
+    pbg = gpu_problem(cfg)
+    g = gpu_gradient(case, pbg)
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    obj_h, pr_h, pos_h, I_h = pin(case.obj_start), pin(case.probe), pin(case.positions), pin(case.intensity)
+    gO_h = torch.empty_like(obj_h).pin_memory(); gP_h = torch.empty_like(pr_h).pin_memory()
+    gX_h = torch.empty((cfg.n_pos, 2), dtype=torch.float32).pin_memory()
+    loss_h = torch.zeros(1, dtype=torch.float64).pin_memory()
+    ws = ptycho.make_workspace(pbg, cfg.n_pos, cfg.n_pos, host=True)
+    ptycho.gradient_host(pbg, obj_h, pr_h, pos_h, I_h, workspace=ws, grad_object_h=gO_h, grad_probe_h=gP_h, grad_pos_h=gX_h, loss_h=loss_h)
+    assert gO_h.numpy().tobytes() == g["grad_object"].tobytes()
+    assert gP_h.numpy().tobytes() == g["grad_probe"].tobytes()
+    assert gX_h.numpy().tobytes() == g["grad_pos"].tobytes()
+    assert loss_h.item() == g["loss"]
