@@ -1,0 +1,331 @@
+"""bench.py — probe positions/s for one full forward+adjoint iteration of the multislice hot path on B200.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--impl reference] [--config 3]
+    python -m torch.distributed.run --nnodes=1 --nproc-per-node N --master-addr 127.0.0.1 --master-port P \
+           bench.py --gpus N --steps K --warmup W
+
+A step = one pass of the whole hot path over ALL positions of the workload:
+ptycho_gradient (loss + object / probe / position gradients) then ptycho_apply_update (SGD), through the C ABI.
+Workload at N=1: BASELINE.json config 3 (128x128 patterns, 64x64 scan = 4096 positions, 8 modes, 20 slices, tilt,
+Poisson loss), the configuration north_star's target is quoted on.  Inputs are seeded and synthetic.
+Rank 0 prints ONE JSON line.
+"""
+import argparse
+import json
+import os
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "probe positions/s per full forward+adjoint iteration"
+UNIT = "positions/s"
+PAPER_CONTEXT = "paper: <3 s/iter for 6400 positions x 20 slices on an RTX 3080, whole engine iteration (PAPER.md:266) - context only"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 5])
+    ap.add_argument("--cpu-sample", type=int, default=0, help="positions in the oracle sample (0: per-config default)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--ws-gib", type=float, default=0.0, help="cap of the device workspace in GiB (0: library default)")
+    return ap.parse_args()
+
+
+def workload(idx):
+    from paper_2505_14372_b200 import synth
+    cfg = synth.config(idx)
+    return cfg, dict(workload=f"BASELINE.json configs[{idx - 1}] ({cfg.name})", n=cfg.n, positions_per_gpu=cfg.n_pos, modes=cfg.n_modes,
+                     slices=cfg.n_slices, object_px=cfg.obj_n, loss="poisson" if cfg.loss == synth.LOSS_POISSON else "amplitude",
+                     start_state="O = exp((i-0.05) 0.8 phi_true), true probe, nominal positions",
+                     patterns="seeded closed-form stand-in + Poisson (synth.standin_patterns)")
+
+
+def problem_kwargs(cfg):
+    return dict(n=cfg.n, n_modes=cfg.n_modes, n_slices=cfg.n_slices, obj_ny=cfg.obj_n, obj_nx=cfg.obj_n,
+                pixel_size=cfg.pixel_size, wavelength=cfg.wavelength, slice_thickness=[cfg.dz] * cfg.n_slices,
+                tilt_x_mrad=cfg.tilt_mrad[0], tilt_y_mrad=cfg.tilt_mrad[1], bandlimit=cfg.bandlimit, loss=cfg.loss,
+                loss_c=cfg.loss_c, eps=cfg.eps)
+
+
+def host_inputs(cfg, rows=None):
+    from paper_2505_14372_b200 import synth
+    phi = synth.object_phase(cfg)
+    obj = synth.object_from_phase(phi, 0.8)
+    pr = synth.probe(cfg)
+    pos = synth.positions(cfg)
+    if rows is not None:
+        pos = pos[rows]
+    inten = synth.standin_patterns(cfg, rows)
+    return obj, pr, pos, inten
+
+
+LR = dict(lr_obj=1e-7, lr_probe=1e-7, lr_pos=1e-9)   # a real (tiny) SGD step so every timed step does the update
+
+
+# ----------------------------------------------------------------------------------------------------
+# clocks during the timed region (profiling recipe)
+# ----------------------------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits", "-lms", "100",
+                                       "-i", str(index)], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        out = dict(sm_mhz=None, sm_max_mhz=None, reasons=[], samples=0)
+        if self.p is None:
+            return out
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f.read().splitlines():
+            c = [x.strip() for x in line.split(",")]
+            if len(c) < 7:
+                continue
+            try:
+                sm.append(float(c[0])); mx.append(float(c[1])); pw.append(float(c[2]))
+            except ValueError:
+                continue
+            for n, v in zip(names, c[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(n)
+        self.f.close(); os.unlink(self.f.name)
+        if sm:
+            out.update(sm_mhz=float(np.median(sm)), sm_max_mhz=float(max(mx)), power_w_max=float(max(pw)),
+                       reasons=sorted(reasons), samples=len(sm))
+        return out
+
+
+def measured_peaks():
+    p = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(p):
+        d = json.load(open(p))
+        return float(d["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs)", float(d.get("sm_max_mhz", 1965.0))
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)", 1965.0
+
+
+# per-position ALGORITHMIC bytes of the two FFT-chain kernels: the slice-wave stash of the
+# reverse-mode adjoint (written once by k_forward, read once by k_backward: SURVEY §8(d) B_act) plus the
+# far-field hand-over; the per-mode patch-gradient staging of the current build is NOT algorithmic.
+def algorithmic_bytes_per_position(cfg, kernel):
+    NN = cfg.n * cfg.n
+    stash = cfg.n_modes * cfg.n_slices * NN * 8
+    far = cfg.n_modes * NN * 8
+    if kernel == "k_forward":
+        return stash + far
+    if kernel == "k_backward":
+        return stash + far + NN * 4
+    return None
+
+
+def nominal_flops_per_position(cfg):
+    NN = cfg.n * cfg.n
+    fft = 5.0 * NN * np.log2(NN)                      # one 2-D complex FFT
+    return cfg.n_modes * (4 * cfg.n_slices * fft + (32 * cfg.n_slices + 20) * NN)
+
+
+# ----------------------------------------------------------------------------------------------------
+def run_reference(args):
+    """The reference arm of this tier = the CPU oracle as it stands, on the host cores, on a bounded sample."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from oracle import oracle as orc
+    cfg, conf = workload(args.config)
+    n = args.cpu_sample or {1: 256, 2: 64, 3: 16, 5: 16}[args.config]
+    rows = np.arange(n)
+    obj, pr, pos, inten = host_inputs(cfg, rows)
+    pbo = orc.Problem(**problem_kwargs(cfg))
+
+    def step():
+        g = orc.gradient(pbo, obj, pr, pos, inten)
+        orc.apply_update(pbo, 0, obj, pr, pos, g["grad_object"], g["grad_probe"], g["grad_pos"], **LR)
+
+    for _ in range(args.warmup):
+        step()
+    t0 = time.perf_counter()
+    for _ in range(args.steps):
+        step()
+    dt = (time.perf_counter() - t0) / args.steps
+    v = n / dt
+    sample = f"first {n} positions of the scan, forward+adjoint+SGD update per step"
+    conf.update(sample_positions=n)
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": v, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": dt * 1e3, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": conf,
+        "cpu_baseline": {"value": v, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
+
+
+def run_b200(args):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    cfg, conf = workload(args.config)
+    J = cfg.n_pos
+    obj_h, pr_h, pos_h, I_h = host_inputs(cfg)
+    pbg = ptycho.Problem(**problem_kwargs(cfg))
+    dev = lambda a: torch.from_numpy(np.ascontiguousarray(a)).cuda()
+    obj, pr, pos, inten = dev(obj_h), dev(pr_h), dev(pos_h), dev(I_h)
+    gO, gP = torch.empty_like(obj), torch.empty_like(pr)
+    gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    cap = int(args.ws_gib * (1 << 30)) if args.ws_gib > 0 else None
+    ws = ptycho.make_workspace(pbg, J, J, ptycho.WANT_POS_GRAD, max_bytes=cap)
+
+    def step():
+        # weak scaling over ranks: every rank owns J positions of the scan; object / probe are replicated, so the
+        # only exchange is the sum of the object / probe gradients and the loss before the update.
+        ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
+        if dist is not None:
+            dist.all_reduce(torch.view_as_real(gO)); dist.all_reduce(torch.view_as_real(gP)); dist.all_reduce(loss)
+        ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, **LR)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    assert ptycho.status(ws) == 0, "device-side error flag set during warm-up"
+    clocks = ClockSampler(local) if rank == 0 else None
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    barrier()
+    n0 = ptycho.launch_count()
+    e0.record()
+    for _ in range(args.steps):
+        step()
+    e1.record()
+    barrier()
+    launches = ptycho.launch_count() - n0
+    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(ms, op=dist.ReduceOp.MAX)
+    ms_step = ms.item() / args.steps
+    clk = clocks.stop() if clocks else None
+    loss_val = loss.item()
+    assert np.isfinite(loss_val) and ptycho.status(ws) == 0
+
+    # per-kernel device time over the same K steps (CUDA events on the launching stream, inside the library)
+    ptycho.profile_enable(True)
+    torch.cuda.synchronize()
+    for _ in range(args.steps):
+        step()
+    prof = ptycho.profile_read()
+    ptycho.profile_enable(False)
+    tot = sum(v[0] for v in prof.values())
+    top = max(prof, key=lambda k: prof[k][0])
+    top_ms, top_n = prof[top]
+    hbm, which, sm_max = measured_peaks()
+    units_per_launch = J * args.steps / top_n
+    ab = algorithmic_bytes_per_position(cfg, top)
+    roof = {"bound": "hbm", "kernel": top, "achieved": None, "peak": hbm, "unit": "GB/s", "frac": None, "traffic": None,
+            "peak_source": which, "share_of_step": top_ms / tot, "avg_launch_ms": top_ms / top_n,
+            "kernel_ms_per_step": {k: v[0] / args.steps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
+    if ab is not None:
+        ach = ab * units_per_launch / (top_ms / top_n * 1e-3) / 1e9
+        roof.update(achieved=ach, frac=ach / hbm, algorithmic_bytes_per_launch=ab * units_per_launch)
+    # whole-step view against both roofs of SURVEY §8(d): the io+act byte model and nominal FFT flops on the FP32 ALUs
+    rate = J / (ms_step * 1e-3)
+    b_model = 2 * cfg.n_modes * cfg.n_slices * cfg.n * cfg.n * 8 + cfg.n * cfg.n * 4
+    fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    roof["step_model"] = {"hbm_frac_io_act_model": b_model * rate / 1e9 / hbm,
+                          "fp32_frac_nominal_fft_flops": nominal_flops_per_position(cfg) * rate / 1e12 / fp32_peak,
+                          "fp32_peak_tflops_at_max_clock": fp32_peak}
+
+    # end to end through the host-buffer entry point: pinned host memory in, gradients + loss back, every step
+    e2e = None
+    if not args.no_e2e:
+        del ws
+        torch.cuda.empty_cache()
+        pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+        obj_p, pr_p, pos_p, I_p = pin(obj_h), pin(pr_h), pin(pos_h), pin(I_h)
+        gO_p = torch.empty(obj_p.shape, dtype=torch.complex64).pin_memory(); gP_p = torch.empty(pr_p.shape, dtype=torch.complex64).pin_memory()
+        gX_p = torch.empty((J, 2), dtype=torch.float32).pin_memory(); loss_p = torch.zeros(1, dtype=torch.float64).pin_memory()
+        wsh = ptycho.make_workspace(pbg, J, J, ptycho.WANT_POS_GRAD, host=True)
+
+        def step_host():
+            ptycho.gradient_host(pbg, obj_p, pr_p, pos_p, I_p, workspace=wsh, grad_object_h=gO_p, grad_probe_h=gP_p,
+                                 grad_pos_h=gX_p, loss_h=loss_p)
+
+        for _ in range(max(1, min(args.warmup, 2))):
+            step_host()
+        barrier()
+        e0.record()
+        for _ in range(args.steps):
+            step_host()
+        e1.record()
+        barrier()
+        msh = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(msh, op=dist.ReduceOp.MAX)
+        h2d = obj_p.numel() * 8 + pr_p.numel() * 8 + pos_p.numel() * 4 + I_p.numel() * 4
+        d2h = gO_p.numel() * 8 + gP_p.numel() * 8 + gX_p.numel() * 4 + 8
+        e2e = {"value": world * J / (msh.item() / args.steps * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h, "api": "ptycho_gradient_host (loss + gradients; pinned host buffers)"}
+
+    cpu = None
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        from oracle import oracle as orc
+        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 5: 24}[args.config]
+        pbo = orc.Problem(**problem_kwargs(cfg))
+        t0 = time.perf_counter()
+        g = orc.gradient(pbo, obj_h, pr_h, pos_h, I_h, batch_idx=np.arange(n, dtype=np.int32))
+        orc.apply_update(pbo, 0, obj_h, pr_h, pos_h[:n], g["grad_object"], g["grad_probe"], g["grad_pos"], **LR)
+        dt = time.perf_counter() - t0
+        cpu = {"value": n / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
+               "sample": f"first {n} of {J} positions, one forward+adjoint+update, {dt:.1f} s"}
+
+    if rank == 0:
+        conf.update(parallelism=f"positions sharded over {world} GPU(s), gradients all-reduced" if world > 1 else "1 GPU",
+                    global_positions=world * J, l2_policy="inputs larger than L2 (268 MB patterns + multi-GB stash per step), no flush",
+                    context=PAPER_CONTEXT)
+        print(json.dumps({
+            "metric": METRIC, "value": world * rate, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 (complex64)",
+            "data": "synthetic", "config": conf, "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roof,
+            "cpu_baseline": cpu, "loss": loss_val}))
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    a = parse()
+    if a.impl == "reference":
+        run_reference(a)
+    else:
+        run_b200(a)

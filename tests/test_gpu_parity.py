@@ -53,13 +53,19 @@ def gpu_gradient(case, pbg, batch_idx=None, flags=0, want_pos=True, want_illum=F
     return out
 
 
-def check(g, o, tol_grad=TOL_GRAD, pos=True):
+def check(g, o, tol_grad=TOL_GRAD, pos=True, px=1.0):
     assert abs(g["loss"] - o["loss"]) <= TOL_LOSS * abs(o["loss"]), (g["loss"], o["loss"])
     assert np.max(np.abs(g["loss_per_pos"] - o["loss_per_pos"]) / np.maximum(np.abs(o["loss_per_pos"]), 1e-30)) <= 2e-5
     assert rel_l2(g["grad_object"], o["grad_object"]) <= tol_grad
     assert rel_l2(g["grad_probe"], o["grad_probe"]) <= tol_grad
     if pos:
         assert rel_l2(g["grad_pos"], o["grad_pos"]) <= tol_grad
+    else:
+        # vacuum start: the pattern does not depend on the position (vacuum invariant), so dL/dX == 0 exactly and
+        # the oracle returns ~1e-10; a relative error is undefined.  Bound the fp32 noise against the natural
+        # scale "loss per pixel of shift" instead.
+        assert np.max(np.abs(o["grad_pos"])) <= 1e-6
+        assert np.max(np.abs(g["grad_pos"])) <= 1e-5 * np.max(np.abs(o["loss_per_pos"])) / px
 
 
 # ------------------------------------------------------------------------------------------------
@@ -70,7 +76,7 @@ def test_cfg1_full():
     case = make_case(cfg, start_scale=0.0, noise=False)
     o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
     g = gpu_gradient(case, gpu_problem(cfg))
-    check(g, o)
+    check(g, o, pos=False, px=cfg.pixel_size)
 
 
 def test_cfg1_forward_intensity():
@@ -105,7 +111,7 @@ def test_cfg2_reduced(start):
     case = make_case(cfg, start_scale=start)
     o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
     g = gpu_gradient(case, gpu_problem(cfg))
-    check(g, o)
+    check(g, o, pos=start > 0, px=cfg.pixel_size)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -123,10 +129,10 @@ def test_cfg3_reduced_chunked(start):
     full_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos)
     cap = min_ws + (full_ws - min_ws) * 7 // 29 + 4096          # room for 8 positions per chunk: 30 = 8+8+8+6
     g = gpu_gradient(case, pbg, want_illum=True, max_ws=cap)
-    check(g, o)
+    check(g, o, pos=start > 0, px=cfg.pixel_size)
     assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
     g1 = gpu_gradient(case, pbg, want_illum=True)                # one chunk
-    check(g1, o)
+    check(g1, o, pos=start > 0, px=cfg.pixel_size)
 
 
 def test_bandlimit_and_anscombe():
