@@ -93,9 +93,11 @@ struct Dft<1, DIR> { static PTK_HD void run(cf*) {} };
 template <int N_> struct Geo;
 template <> struct Geo<128> {
   static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
+  static constexpr int PF16 = 11;   // 16-byte prefetch slots per thread beside the exchange buffer (1 CTA / SM)
 };
 template <> struct Geo<64> {
   static constexpr int N = 64, LOGN = 6, T = 128, N1X = 8, N2X = 8, N1Y = 4, N2Y = 16, LX2 = 3, LY2 = 4, LP2 = 4, LP3 = 2;
+  static constexpr int PF16 = 8;    // 4 CTAs / SM: 56 KB each
 };
 
 template <class G>
@@ -112,17 +114,19 @@ struct Lay {
   // ---- F-layout: thread t, reg r -> (qy, qx)
   static PTK_HD int f_qx(int t, int) { return t & (N - 1); }
   static PTK_HD int f_qy(int t, int r) { return ((t >> G::LOGN) * G::LP3 + r / G::N2Y) + G::N1Y * (r & (G::N2Y - 1)); }
-  // native (coalesced) storage index of (thread, reg) in float2 units — used for stashes in both layouts
-  static PTK_HD int native(int t, int r) { return r * T + t; }
+  // native (coalesced) storage index of (thread, reg) in float2 units — used for every field kept in the
+  // workspace, in both layouts.  Registers (2p, 2p+1) of a thread are adjacent, so one thread moves 16 bytes
+  // and a warp 512 contiguous bytes per access: as a float4 array the index is p*T + t.
+  static PTK_HD int native(int t, int r) { return (((r >> 1) * T + t) << 1) | (r & 1); }
   // position of real-space pixel (y, x) in R-native storage (used by the object-gradient gather)
   static PTK_HD int r_native_of(int y, int x) {
     int a = x & (G::N2X - 1), n1x = x >> G::LX2, b = y & (G::N2Y - 1), n1y = y >> G::LY2;
-    return (n1y * G::N1X + n1x) * T + (a + G::N2X * b);
+    return native(a + G::N2X * b, n1y * G::N1X + n1x);
   }
   static PTK_HD int f_native_of(int qy, int qx) {
     int k1y = qy & (G::N1Y - 1), k2y = qy / G::N1Y;
     int c = k1y / G::LP3, ksel = k1y % G::LP3;
-    return (ksel * G::N2Y + k2y) * T + (qx + N * c);
+    return native(qx + N * c, ksel * G::N2Y + k2y);
   }
 
   // fill the twiddle table: tw[k1x*N2X + a] = W_N^(a k1x), tw[N1X*N2X + k1y*N2Y + b] = W_N^(b k1y)   (forward sign)
@@ -300,8 +304,11 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   L::x2_load_p3(v, sm, t);
   L::template phase3<-1>(v);
 }
+// The inverse in two pieces: after the head, the calling warp's own X1 region (Lay::X1_WARP float2 slots at
+// sm + warp*X1_WARP) is free until that warp's next fft2_fwd / fft2_inv_head — the chain kernels land their
+// late cp.async prefetches there while phase 1 runs.
 template <class G>
-__device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int t) {
+__device__ __forceinline__ void fft2_inv_head(cf (&v)[32], cf* sm, int t) {
   typedef Lay<G> L;
   L::template phase3<+1>(v);
   __syncthreads();
@@ -313,7 +320,12 @@ __device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int 
   L::x1_store_p2(v, sm, t);
   __syncwarp();
   L::x1_load_p1(v, sm, t);
-  L::phase1_inv(v, tw, t);
+  __syncwarp();                    // every lane has read its part: the warp's X1 region is free
+}
+template <class G>
+__device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int t) {
+  fft2_inv_head<G>(v, sm, t);
+  Lay<G>::phase1_inv(v, tw, t);
 }
 #endif
 

@@ -214,6 +214,41 @@ template <class G> constexpr int min_blocks() { return G::N == 128 ? 1 : 4; }
 template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::XBUF + Lay<G>::TW) * sizeof(cf) + 1024; }
 
 // ------------------------------------------------------------------------------------------------
+// Shared memory of the chain kernels (k_forward / k_backward):
+//   [ exchange buffer XBUF | twiddles TW | reduction scratch 1 KB | hy tables 2 x N | prefetch slots PF16 x T x 16 B ]
+// Global data a slice needs (object patch T_i, stashed wave Psi_i) is brought in with cp.async into slots that
+// belong to the thread that will consume them, so no barrier or mbarrier is involved: "early" slots (the PF16
+// region) are filled one whole FFT pair ahead, "late" slots live in the calling warp's own X1 exchange region,
+// which is idle between the end of fft2_inv_head and the next fft2_fwd (16 slots of 16 B per lane).
+// ------------------------------------------------------------------------------------------------
+template <class G> constexpr size_t chain_smem_bytes() {
+  return (size_t)(Lay<G>::XBUF + Lay<G>::TW + 2 * G::N) * sizeof(cf) + 1024 + (size_t)G::PF16 * G::T * 16;
+}
+template <class G>
+struct ChainSmem {
+  cf* sm; cf* tw; double* red; cf* hyS; float4* pf; float4* xs;
+  __device__ __forceinline__ ChainSmem(unsigned char* raw, int t) {
+    typedef Lay<G> L;
+    sm = (cf*)raw; tw = sm + L::XBUF; red = (double*)(tw + L::TW);
+    hyS = (cf*)((unsigned char*)red + 1024);
+    pf = (float4*)(hyS + 2 * G::N) + t;                                 // early slot s: pf[s * T]
+    xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late slot s:  xs[s * 32]
+  }
+};
+__device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
+
+// offset (in object pixels) of register r's pixel from the thread's first pixel of the patch
+template <class G>
+__device__ __forceinline__ size_t patch_off(int r, int onx) { return (size_t)((r / G::N1X) * G::N2Y) * onx + (r & (G::N1X - 1)) * G::N2X; }
+
+// ------------------------------------------------------------------------------------------------
 // H1: P~_k = F(P_k), stored F-native.  Also used for Q~_k = F(dPhat_k) with scale/accumulator input.
 //   mode 0: in = raster complex64 field [k][N][N]
 //   mode 1: in = -gP_k / (delta_p + 1) from raster grad_probe (step-size sweep, O14)
@@ -289,47 +324,95 @@ __device__ __forceinline__ const cf* patch_ptr(const KP& P, int i, int r0y, int 
 }
 
 // ------------------------------------------------------------------------------------------------
+// pointwise helpers on the register field
+// ------------------------------------------------------------------------------------------------
+// v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9); hy from shared memory
+template <class G, bool CONJ>
+__device__ __forceinline__ void apply_prop_s(cf (&v)[32], cf wx, const cf* hyS, float bandlim2, int t) {
+  typedef Lay<G> L;
+  if (CONJ) wx.y = -wx.y;
+  const int sx = signed_freq(L::f_qx(t, 0), G::N);
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int qy = L::f_qy(t, r);
+    cf wy = hyS[qy];
+    if (CONJ) wy.y = -wy.y;
+    cf h = cmul(wx, wy);
+    if (bandlim2 >= 0.0f) {
+      const int sy = signed_freq(qy, G::N);
+      if ((float)(sx * sx + sy * sy) > bandlim2) h = make_float2(0.f, 0.f);
+    }
+    v[r] = cmul(v[r], h);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // H2..H6 forward: one CTA per (j,k) pair of the chunk
 // ------------------------------------------------------------------------------------------------
 template <class G, bool STASH>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N;
+  constexpr int N = G::N, NN = N * N, T = G::T, E = G::PF16;     // E pair slots early, 16 - E late
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
   const int t = threadIdx.x;
-  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
-  __syncthreads();
+  ChainSmem<G> cs(smem_raw, t);
+  cf* sm = cs.sm; cf* tw = cs.tw;
+  for (int i = t; i < L::TW; i += T) L::fill_twiddle(tw, i);
   const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const int S = P.S, onx = P.onx;
+  const size_t slice = (size_t)P.ony * onx;
+  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);   // this thread's first pixel, slice 0
+  // H3 prefetch: patch values of registers [0, 2E) one FFT pair ahead into the thread's early slots
+  auto early = [&](int i) {
+    const cf* o = ob + (size_t)i * slice;
+#pragma unroll
+    for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.pf + (r >> 1) * T) + (r & 1), o + patch_off<G>(r, onx));
+    if (i < S - 1 && t < N) cp_async8(cs.hyS + (i & 1) * N + t, P.w.hy + (size_t)i * N + t);
+    cp_async_commit();
+  };
+  early(0);
+  __syncthreads();                                               // twiddle table ready
   const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
   const cf* ry = rx + N;
+  const int qx = L::f_qx(t, 0);
   cf v[32];
   {   // H2: R .* P~_k / N^2   (F-layout)
-    const cf* pt = P.w.Pt + (size_t)k * NN;
-    cf wx = cscale(rx[L::f_qx(t, 0)], 1.0f / (float)NN);
+    const float4* pt = (const float4*)(P.w.Pt + (size_t)k * NN);
+    const cf wx = cscale(rx[qx], 1.0f / (float)NN);
 #pragma unroll
-    for (int r = 0; r < 32; ++r) v[r] = cmul(pt[L::native(t, r)], cmul(wx, ry[L::f_qy(t, r)]));
-  }
-  const int S = P.S;
-  for (int i = 0; i < S; ++i) {
-    fft2_inv<G>(v, sm, tw, t);                                   // Psi_{i,k}  (R-layout)
-    if (STASH) {
-      cf* st = P.w.stash + ((size_t)(jl * P.M + k) * S + i) * NN;
-#pragma unroll
-      for (int r = 0; r < 32; ++r) st[L::native(t, r)] = v[r];
+    for (int p = 0; p < 16; ++p) {
+      const float4 q = pt[p * T + t];
+      v[2 * p] = cmul(make_float2(q.x, q.y), cmul(wx, ry[L::f_qy(t, 2 * p)]));
+      v[2 * p + 1] = cmul(make_float2(q.z, q.w), cmul(wx, ry[L::f_qy(t, 2 * p + 1)]));
     }
-    const cf* ob = patch_ptr(P, i, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
-#pragma unroll
-    for (int r = 0; r < 32; ++r)                                 // H3+H4: Phi = Psi .* T_i
-      v[r] = cmul(v[r], ob[(size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X]);
-    fft2_fwd<G>(v, sm, tw, t);                                   // F(Phi)    (F-layout)
-    if (i < S - 1) apply_prop<G, false>(v, P.w.hx + (size_t)i * N, P.w.hy + (size_t)i * N, P.bandlim2, t);   // H5
   }
-  cf* out = P.w.psit + (size_t)(jl * P.M + k) * NN;              // H6: psi~ = F(Phi_{S-1}) / N
+  for (int i = 0; i < S; ++i) {
+    fft2_inv_head<G>(v, sm, t);
+    {   // registers [2E, 32) of T_i into the warp's idle X1 region
+      const cf* o = ob + (size_t)i * slice;
+#pragma unroll
+      for (int r = 2 * E; r < 32; ++r) cp_async8((cf*)(cs.xs + ((r >> 1) - E) * 32) + (r & 1), o + patch_off<G>(r, onx));
+      cp_async_commit();
+    }
+    L::phase1_inv(v, tw, t);                                     // Psi_{i,k}  (R-layout)
+    cp_async_wait_all();
+    float4* st = (float4*)(P.w.stash + ((size_t)(jl * P.M + k) * S + i) * NN);
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {                               // stash Psi_i ; H3+H4: Phi = Psi .* T_i
+      if (STASH) st[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
+      const float4 q = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+      v[2 * p] = cmul(v[2 * p], make_float2(q.x, q.y));
+      v[2 * p + 1] = cmul(v[2 * p + 1], make_float2(q.z, q.w));
+    }
+    if (i + 1 < S) early(i + 1);
+    fft2_fwd<G>(v, sm, tw, t);                                   // F(Phi)    (F-layout)
+    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx[(size_t)i * N + qx], cs.hyS + (i & 1) * N, P.bandlim2, t);   // H5
+  }
+  float4* out = (float4*)(P.w.psit + (size_t)(jl * P.M + k) * NN);   // H6: psi~ = F(Phi_{S-1}) / N
   const float sc = 1.0f / (float)N;
 #pragma unroll
-  for (int r = 0; r < 32; ++r) out[L::native(t, r)] = cscale(v[r], sc);
+  for (int p = 0; p < 16; ++p) out[p * T + t] = make_float4(v[2 * p].x * sc, v[2 * p].y * sc, v[2 * p + 1].x * sc, v[2 * p + 1].y * sc);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -388,56 +471,92 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* loss_per_pos, float*
 template <class G, int MODE>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int want_pos) {
   typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N;
+  constexpr int N = G::N, NN = N * N, T = G::T, E = G::PF16;     // stash pairs [0,E) early, [E,16) late; T pairs [0,E) late
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
-  double* red = (double*)(tw + L::TW);          // [(T/32)*4] doubles (<= 64*8 = 512 B... sized in fft_smem_bytes)
   const int t = threadIdx.x;
-  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
-  __syncthreads();
+  ChainSmem<G> cs(smem_raw, t);
+  cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
+  for (int i = t; i < L::TW; i += T) L::fill_twiddle(tw, i);
   const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
-  const int S = P.S;
+  const int S = P.S, onx = P.onx;
+  const size_t slice = (size_t)P.ony * onx;
+  const size_t fld0 = (size_t)(jl * P.M + k) * S * NN;
+  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);
+  const int qx = L::f_qx(t, 0);
+  // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
+  auto early = [&](int i) {
+    const float4* st = (const float4*)(P.w.stash + fld0 + (size_t)i * NN) + t;
+#pragma unroll
+    for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+    if (i > 0 && t < N) cp_async8(cs.hyS + ((i - 1) & 1) * N + t, P.w.hy + (size_t)(i - 1) * N + t);
+    cp_async_commit();
+  };
+  early(S - 1);
+  __syncthreads();
   cf v[32];
   {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = N Finv(g~) = F^H(g~) / N
-    const cf* ps = P.w.psit + (size_t)(jl * P.M + k) * NN;
-    const float* wd = P.w.wdet + (size_t)jl * NN;
+    const float4* ps = (const float4*)(P.w.psit + (size_t)(jl * P.M + k) * NN);
+    const float2* wd = (const float2*)(P.w.wdet + (size_t)jl * NN);
     const float sc = 1.0f / (float)N;
 #pragma unroll
-    for (int r = 0; r < 32; ++r) v[r] = cscale(ps[L::native(t, r)], wd[L::native(t, r)] * sc);
+    for (int p = 0; p < 16; ++p) {
+      const float4 q = ps[p * T + t]; const float2 w = wd[p * T + t];
+      v[2 * p] = make_float2(q.x * (w.x * sc), q.y * (w.x * sc));
+      v[2 * p + 1] = make_float2(q.z * (w.y * sc), q.w * (w.y * sc));
+    }
   }
   for (int i = S - 1; i >= 0; --i) {
-    fft2_inv<G>(v, sm, tw, t);                                   // gPhi_{i,k}  (R-layout)
-    const size_t fld = ((size_t)(jl * P.M + k) * S + i) * NN;
-    const cf* st = P.w.stash + fld;
-    const cf* ob = patch_ptr(P, i, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
-    if (MODE == 0) {
-      cf* gt = P.w.gTpart + fld;
+    fft2_inv_head<G>(v, sm, t);
+    const cf* o = ob + (size_t)i * slice;
+    {   // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
+      const float4* st = (const float4*)(P.w.stash + fld0 + (size_t)i * NN) + t;
 #pragma unroll
-      for (int r = 0; r < 32; ++r) {
-        cf psi = st[L::native(t, r)];
-        cf T = ob[(size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X];
-        gt[L::native(t, r)] = cmulc(v[r], psi);                  // H10: gT_i contribution conj(Psi) .* gPhi
-        v[r] = cmulc(v[r], T);                                   //      gPsi = conj(T) .* gPhi
+      for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
+#pragma unroll
+      for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.xs + (16 - E + (r >> 1)) * 32) + (r & 1), o + patch_off<G>(r, onx));
+      cp_async_commit();
+    }
+    L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
+    cp_async_wait_all();
+    if (MODE == 0) {
+      float4* gt = (float4*)(P.w.gTpart + fld0 + (size_t)i * NN);
+#pragma unroll
+      for (int p = 0; p < 16; ++p) {
+        const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+        cf T0, T1;
+        if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
+        else { T0 = o[patch_off<G>(2 * p, onx)]; T1 = o[patch_off<G>(2 * p + 1, onx)]; }
+        const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+        gt[p * T + t] = make_float4(g0.x, g0.y, g1.x, g1.y);    // H10: gT_i contribution conj(Psi) .* gPhi
+        v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
+        v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
       }
+      if (i > 0) early(i - 1);
     } else {
       // H14 object terms: u = dOhat|patch .* Psi ; chi = -gPhi ; num += Re(chi conj(u)) ; den += |u|^2
-      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * P.onx + r0x + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
+      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);
       float num = 0.f, den = 0.f;
       if (i == 0) {                                              // keep gPhi_0 for the probe / position terms
-        cf* sc0 = P.w.scratch + (size_t)(jl * P.M + k) * NN;
+        float4* sc0 = (float4*)(P.w.scratch + (size_t)(jl * P.M + k) * NN);
 #pragma unroll
-        for (int r = 0; r < 32; ++r) sc0[L::native(t, r)] = v[r];
+        for (int p = 0; p < 16; ++p) sc0[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
       }
 #pragma unroll
-      for (int r = 0; r < 32; ++r) {
-        const size_t o = (size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X;
-        cf psi = st[L::native(t, r)];
-        cf u = cmul(dO[o], psi);
-        num -= fmaf(v[r].x, u.x, v[r].y * u.y);
-        den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
-        v[r] = cmulc(v[r], ob[o]);
+      for (int p = 0; p < 16; ++p) {
+        const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+        cf T0, T1;
+        if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
+        else { T0 = o[patch_off<G>(2 * p, onx)]; T1 = o[patch_off<G>(2 * p + 1, onx)]; }
+        const cf u0 = cmul(dO[patch_off<G>(2 * p, onx)], make_float2(ps.x, ps.y));
+        const cf u1 = cmul(dO[patch_off<G>(2 * p + 1, onx)], make_float2(ps.z, ps.w));
+        num -= fmaf(v[2 * p].x, u0.x, v[2 * p].y * u0.y) + fmaf(v[2 * p + 1].x, u1.x, v[2 * p + 1].y * u1.y);
+        den = fmaf(u0.x, u0.x, fmaf(u0.y, u0.y, den));
+        den = fmaf(u1.x, u1.x, fmaf(u1.y, u1.y, den));
+        v[2 * p] = cmulc(v[2 * p], T0);
+        v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
       }
+      if (i > 0) early(i - 1);
       double acc[2] = {(double)num, (double)den};
       block_sum<G::T, 2>(acc, red);
       if (t == 0) {
@@ -447,7 +566,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       if (i == 0) break;                                         // probe / position terms handled below
     }
     fft2_fwd<G>(v, sm, tw, t);                                   // F(gPsi_i)  (F-layout)
-    if (i > 0) apply_prop<G, true>(v, P.w.hx + (size_t)(i - 1) * N, P.w.hy + (size_t)(i - 1) * N, P.bandlim2, t);
+    if (i > 0) apply_prop_s<G, true>(v, P.w.hx[(size_t)(i - 1) * N + qx], cs.hyS + ((i - 1) & 1) * N, P.bandlim2, t);
   }
   const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
   const cf* ry = rx + N;
@@ -725,10 +844,11 @@ KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64*
 template <class G>
 int set_smem_attrs() {
   const int b = (int)fft_smem_bytes<G>();
-  if (cudaFuncSetAttribute(k_forward<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_forward<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
+  const int c = (int)chain_smem_bytes<G>();
+  if (cudaFuncSetAttribute(k_forward<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_forward<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   return PT_OK;
@@ -762,7 +882,7 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
   if (rc != PT_OK) return rc;
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    k_forward<G, false><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+    k_forward<G, false><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, model_intensity_d, 0);
     LAUNCH_CHECK(K_loss, st);
@@ -794,11 +914,11 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const dim3 ggrid((p->obj_nx + 31) / 32, (p->obj_ny + 7) / 8, p->n_slices), gblock(32, 8);
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    k_forward<G, true><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+    k_forward<G, true><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
-    k_backward<G, 0><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp, want_pos ? 1 : 0);
+    k_backward<G, 0><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp, want_pos ? 1 : 0);
     LAUNCH_CHECK(K_backward, st);
     if (want_illum) k_gather_object<G, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
     else k_gather_object<G, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
@@ -817,12 +937,12 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
       if (kp.w.Jc < p->n_batch) {   // stash of this chunk was overwritten: recompute it
-        k_forward<G, true><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp);
+        k_forward<G, true><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
         LAUNCH_CHECK(K_forward, st);
         k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, nullptr, nullptr, 1);
         LAUNCH_CHECK(K_loss, st);
       }
-      k_backward<G, 1><<<kp.jc * p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp, 0);
+      k_backward<G, 1><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp, 0);
       LAUNCH_CHECK(K_backward, st);
     }
   }
