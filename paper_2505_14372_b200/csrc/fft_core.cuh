@@ -91,13 +91,24 @@ struct Dft<1, DIR> { static PTK_HD void run(cf*) {} };
 
 // ---------------------------------------------------------------------------------------------------
 template <int N_> struct Geo;
+// N = side of the transform one CTA holds in registers; NF = side of the whole field; CL = CTAs per field.
+// CL = 4 (NF = 256): a cluster of four CTAs, CTA (a, b) = rank a + 2 b holds the sub-lattice x = 2 x' + a,
+// y = 2 y' + b and the four 128 x 128 transforms are combined by one radix-2 x 2 stage over distributed shared
+// memory (struct Cross below).
 template <> struct Geo<128> {
   static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
+  static constexpr int NF = 128, CL = 1;
   static constexpr int PF16 = 11;   // 16-byte prefetch slots per thread beside the exchange buffer (1 CTA / SM)
 };
 template <> struct Geo<64> {
   static constexpr int N = 64, LOGN = 6, T = 128, N1X = 8, N2X = 8, N1Y = 4, N2Y = 16, LX2 = 3, LY2 = 4, LP2 = 4, LP3 = 2;
+  static constexpr int NF = 64, CL = 1;
   static constexpr int PF16 = 8;    // 4 CTAs / SM: 56 KB each
+};
+template <> struct Geo<256> {
+  static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
+  static constexpr int NF = 256, CL = 4;
+  static constexpr int PF16 = 10;
 };
 
 template <class G>
@@ -284,7 +295,78 @@ struct Lay {
   }
 };
 
+// ---------------------------------------------------------------------------------------------------
+// Field-level maps (cluster-aware).  For CL = 1 they are Lay's.  For CL = 4 the CTA of rank p = a + 2 b holds
+//   real space   : reg r of thread t  <->  pixel (2 r_y(t,r) + b, 2 r_x(t,r) + a)                    ("R-layout")
+//   Fourier space: reg r = 8 c + e of thread t, quadrant c = cx + 2 cy, e = 0..7  <->
+//                  qx = f_qx(t) + N cx,  qy = f_qy(t, 8 p + e) + N cy                                ("C-layout")
+// i.e. after the four sub-lattice transforms, CTA p owns registers [8p, 8p+8) of every thread of all four
+// CTAs and combines them into the four frequency quadrants (decimation in time, PAPER-independent textbook
+// identity  F[q' + N c] = sum_a (-1)^(a c) W_2N^(a q') F_a[q']  per axis).
+// Fields kept in the workspace are stored as [rank][N*N] blocks of Lay::native order in both spaces.
+// ---------------------------------------------------------------------------------------------------
+template <class G>
+struct FL {
+  typedef Lay<G> L;
+  static constexpr int CL = G::CL, NF = G::NF, NS = G::N, NNS = NS * NS, NNF = NF * NF, NXV = CL == 1 ? 1 : 2;
+  static PTK_HD int pix_x(int rank, int t, int r) { return CL == 1 ? L::r_x(t, r) : 2 * L::r_x(t, r) + (rank & 1); }
+  static PTK_HD int pix_y(int rank, int t, int r) { return CL == 1 ? L::r_y(t, r) : 2 * L::r_y(t, r) + (rank >> 1); }
+  static PTK_HD int fq_xsel(int r) { return CL == 1 ? 0 : (r >> 3) & 1; }       // which of the thread's NXV qx values
+  static PTK_HD int fq_x(int rank, int t, int r) { return CL == 1 ? L::f_qx(t, r) : L::f_qx(t, 0) + NS * ((r >> 3) & 1); }
+  static PTK_HD int fq_y(int rank, int t, int r) { return CL == 1 ? L::f_qy(t, r) : L::f_qy(t, 8 * rank + (r & 7)) + NS * (r >> 4); }
+  // storage index (float2 units, inside one field of NNF elements) of real-space pixel (y, x)
+  static PTK_HD int r_native_of(int y, int x) {
+    return CL == 1 ? L::r_native_of(y, x) : ((x & 1) + 2 * (y & 1)) * NNS + L::r_native_of(y >> 1, x >> 1);
+  }
+  // object-pixel offset of register r from the thread's first pixel
+  static PTK_HD size_t patch_off(int r, int onx) {
+    return (size_t)(CL == 1 ? 1 : 2) * ((size_t)((r / G::N1X) * G::N2Y) * onx + (r & (G::N1X - 1)) * G::N2X);
+  }
+  // in-place 2 x 2 butterfly over the block index s = r / 8 (self-inverse up to the factor 4)
+  static PTK_HD void butterfly(cf (&v)[32]) {
+#pragma unroll
+    for (int e = 0; e < 8; ++e) {
+      const cf s0 = cadd(v[e], v[8 + e]), d0 = csub(v[e], v[8 + e]);
+      const cf s1 = cadd(v[16 + e], v[24 + e]), d1 = csub(v[16 + e], v[24 + e]);
+      v[e] = cadd(s0, s1); v[8 + e] = cadd(d0, d1); v[16 + e] = csub(s0, s1); v[24 + e] = csub(d0, d1);
+    }
+  }
+  // tw2[m] = exp(-2 pi i m / (2 N)), m < N
+  static PTK_HD void fill_tw2(cf* tw2, int m) {
+    float s, c;
+    sincospif(-(float)m / (float)NS, &s, &c);
+    tw2[m] = make_float2(c, s);
+  }
+  // sub-lattice twiddle W_2N^(a qx' + b qy') on sub-F-layout registers (INV: conjugate)
+  template <bool INV>
+  static PTK_HD void twiddle(cf (&v)[32], const cf* tw2, int t, int rank) {
+    if (CL == 1 || rank == 0) return;
+    cf wx = make_float2(1.f, 0.f);
+    if (rank & 1) wx = tw2[L::f_qx(t, 0)];
+    if (rank >> 1) {
+#pragma unroll
+      for (int r = 0; r < 32; ++r) { const cf w = cmul(wx, tw2[L::f_qy(t, r)]); v[r] = INV ? cmulc(v[r], w) : cmul(v[r], w); }
+    } else {
+#pragma unroll
+      for (int r = 0; r < 32; ++r) v[r] = INV ? cmulc(v[r], wx) : cmul(v[r], wx);
+    }
+  }
+  // exchange slots in the exchange buffer, float4 units: block src, register pair ep, thread t
+  static PTK_HD int xslot(int src, int ep, int t) { return (src * 4 + ep) * G::T + t; }
+};
+
 #if defined(__CUDACC__)
+// ---- cluster primitives (CL = 4 only)
+__device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
+__device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
+__device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+__device__ __forceinline__ unsigned mapa_u32(unsigned saddr, unsigned rank) {
+  unsigned r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
+}
+__device__ __forceinline__ void st_cluster_v4(unsigned addr, cf a, cf b) {
+  asm volatile("st.shared::cluster.v4.f32 [%0], {%1, %2, %3, %4};" ::"r"(addr), "f"(a.x), "f"(a.y), "f"(b.x), "f"(b.y) : "memory");
+}
+
 // Whole transforms for one CTA.  `sm` = exchange buffer (Lay::XBUF float2), `tw` = twiddle table (Lay::TW).
 // Contract: fft2_fwd must follow an fft2_inv or a __syncthreads() (it starts by overwriting the calling warp's
 // own X1 region, which only that warp read last); fft2_inv may follow anything (it starts with a CTA barrier
@@ -302,6 +384,7 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   L::x2_store_p2(v, sm, t);
   __syncthreads();
   L::x2_load_p3(v, sm, t);
+  if (G::CL > 1) cluster_arrive();  // this thread no longer reads the exchange buffer: peers may overwrite it (Cross)
   L::template phase3<-1>(v);
 }
 // The inverse in two pieces: after the head, the calling warp's own X1 region (Lay::X1_WARP float2 slots at
@@ -327,6 +410,81 @@ __device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int 
   fft2_inv_head<G>(v, sm, t);
   Lay<G>::phase1_inv(v, tw, t);
 }
+
+// ---------------------------------------------------------------------------------------------------
+// Cross-CTA radix-2 x 2 stage of the CL = 4 field transform, over distributed shared memory.
+// Every CTA sends registers [8 d, 8 d + 8) of each thread to CTA d (its own block included, through the same
+// path) with 16-byte remote stores into the destination's exchange buffer, slot FL::xslot(source, pair, t):
+// a warp writes 512 contiguous bytes.  One hardware cluster barrier phase protects the buffer before the
+// stores (write-after-read: the matching arrive is issued as soon as a thread has finished reading the
+// buffer) and one makes them visible.  Protocol invariant: whenever the registers are in Fourier space
+// (C-layout), exactly one cluster arrive of this thread is pending.
+// ---------------------------------------------------------------------------------------------------
+template <class G>
+struct Cross {
+  typedef FL<G> F;
+  static __device__ __forceinline__ void send(const cf (&v)[32], cf* sm, int t, unsigned rank) {
+    const unsigned base = (unsigned)__cvta_generic_to_shared((float4*)sm + F::xslot((int)rank, 0, t));
+#pragma unroll
+    for (int d = 0; d < 4; ++d) {
+      const unsigned ra = mapa_u32(base, (unsigned)d);
+#pragma unroll
+      for (int ep = 0; ep < 4; ++ep) st_cluster_v4(ra + (unsigned)(ep * G::T * 16), v[8 * d + 2 * ep], v[8 * d + 2 * ep + 1]);
+    }
+  }
+  static __device__ __forceinline__ void recv(cf (&v)[32], const cf* sm, int t) {
+    const float4* b = (const float4*)sm;
+#pragma unroll
+    for (int s = 0; s < 4; ++s)
+#pragma unroll
+      for (int ep = 0; ep < 4; ++ep) {
+        const float4 q = b[F::xslot(s, ep, t)];
+        v[8 * s + 2 * ep] = make_float2(q.x, q.y);
+        v[8 * s + 2 * ep + 1] = make_float2(q.z, q.w);
+      }
+  }
+  // sub-F-layout (after fft2_fwd, whose last exchange-buffer read issued the pending arrive) -> C-layout
+  static __device__ __forceinline__ void fwd(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rank) {
+    F::template twiddle<false>(v, tw2, t, (int)rank);
+    cluster_wait();
+    send(v, sm, t, rank);
+    cluster_arrive();
+    cluster_wait();
+    recv(v, sm, t);
+    cluster_arrive();
+    F::butterfly(v);
+  }
+  // C-layout -> sub-F-layout (ready for fft2_inv_head); consumes the pending arrive
+  static __device__ __forceinline__ void inv(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rank) {
+    F::butterfly(v);
+    cluster_wait();
+    send(v, sm, t, rank);
+    cluster_arrive();
+    cluster_wait();
+    recv(v, sm, t);
+    F::template twiddle<true>(v, tw2, t, (int)rank);
+  }
+};
+
+// Field-level transforms of one CTA (of a CL-cluster): R-layout <-> Fourier layout (F-layout / C-layout)
+template <class G>
+struct Fft {
+  static __device__ __forceinline__ unsigned rank() { return G::CL > 1 ? cluster_ctarank() : 0u; }
+  static __device__ __forceinline__ void begin_fourier() { if (G::CL > 1) cluster_arrive(); }   // registers (re)start in Fourier space
+  static __device__ __forceinline__ void end_fourier() { if (G::CL > 1) cluster_wait(); }       // kernel ends in Fourier space
+  static __device__ __forceinline__ void fwd(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
+    fft2_fwd<G>(v, sm, tw, t);
+    if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
+  }
+  static __device__ __forceinline__ void inv_head(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rk) {
+    if (G::CL > 1) Cross<G>::inv(v, sm, tw2, t, rk);
+    fft2_inv_head<G>(v, sm, t);
+  }
+  static __device__ __forceinline__ void inv(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
+    inv_head(v, sm, tw2, t, rk);
+    Lay<G>::phase1_inv(v, tw, t);
+  }
+};
 #endif
 
 }  // namespace ptk

@@ -43,9 +43,9 @@ struct Ws {
   cf* Pt;              // [M][N^2]  F-native, unscaled
   cf* Qt;              // [M][N^2]  F-native: F(dPhat_k) for the step-size sweep
   double2* gPt_acc;    // [M][N^2]  F-native accumulators
-  double* loss_pp;     // [J]
-  double* posg_part;   // [J][M][2]
-  double* step_part;   // [J][M][2S+6]
+  double* loss_pp;     // [J][CL]
+  double* posg_part;   // [J][M][CL][2]
+  double* step_part;   // [J][M][CL][2S+6]
   cf* dOhat;           // [S][ony][onx]      (step sizes only)
   // chunked
   cf* psit;            // [Jc][M][N^2]  F-native
@@ -59,17 +59,18 @@ struct Ws {
 };
 
 inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+inline size_t cluster_of(int n) { return n == 256 ? 4 : 1; }   // CTAs per field (Geo<n>::CL)
 
 // per-chunk-position bytes and fixed bytes
 void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
-  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch;
+  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch, CL = cluster_of(p->n);
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   size_t f = 256;
   f += 2 * align_up((S > 1 ? S - 1 : 1) * N * sizeof(cf));
   f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float));
   f += 2 * align_up(M * NN * sizeof(cf)) + align_up(M * NN * sizeof(double2));
-  f += align_up(J * sizeof(double)) + align_up(J * M * 2 * sizeof(double));
-  f += align_up(J * M * (2 * S + 6) * sizeof(double));
+  f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
+  f += align_up(J * M * CL * (2 * S + 6) * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
   size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   if (steps) pp += M * NN * sizeof(cf);
@@ -83,7 +84,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   if (bytes < fixed + pp) return PT_ERR_WORKSPACE;
   size_t jc = (bytes - fixed) / pp;
   if (jc > (size_t)p->n_batch) jc = p->n_batch;
-  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch;
+  const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch, CL = cluster_of(p->n);
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   char* c = (char*)base;
   size_t off = 0;
@@ -97,9 +98,9 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->Pt = (cf*)take(M * NN * sizeof(cf));
   w->Qt = (cf*)take(M * NN * sizeof(cf));
   w->gPt_acc = (double2*)take(M * NN * sizeof(double2));
-  w->loss_pp = (double*)take(J * sizeof(double));
-  w->posg_part = (double*)take(J * M * 2 * sizeof(double));
-  w->step_part = (double*)take(J * M * (2 * S + 6) * sizeof(double));
+  w->loss_pp = (double*)take(J * CL * sizeof(double));
+  w->posg_part = (double*)take(J * M * CL * 2 * sizeof(double));
+  w->step_part = (double*)take(J * M * CL * (2 * S + 6) * sizeof(double));
   w->dOhat = steps ? (cf*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf)) : nullptr;
   w->psit = (cf*)take(jc * M * NN * sizeof(cf));
   w->wdet = (float*)take(jc * NN * sizeof(float));
@@ -210,29 +211,33 @@ __device__ __forceinline__ void block_sum(double (&val)[NV], double* red /* [T/3
   __syncthreads();
 }
 
-template <class G> constexpr int min_blocks() { return G::N == 128 ? 1 : 4; }
-template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::XBUF + Lay<G>::TW) * sizeof(cf) + 1024; }
+template <class G> constexpr int min_blocks() { return G::T == 512 ? 1 : 4; }
 
 // ------------------------------------------------------------------------------------------------
-// Shared memory of the chain kernels (k_forward / k_backward):
-//   [ exchange buffer XBUF | twiddles TW | reduction scratch 1 KB | hy tables 2 x N | prefetch slots PF16 x T x 16 B ]
+// Shared memory of the FFT kernels:
+//   [ exchange buffer XBUF | twiddles TW | cluster twiddles TW2 (CL = 4 only) | reduction scratch 1 KB |
+//     chain kernels only: hy tables 2 x NF | prefetch slots PF16 x T x 16 B ]
 // Global data a slice needs (object patch T_i, stashed wave Psi_i) is brought in with cp.async into slots that
 // belong to the thread that will consume them, so no barrier or mbarrier is involved: "early" slots (the PF16
 // region) are filled one whole FFT pair ahead, "late" slots live in the calling warp's own X1 exchange region,
 // which is idle between the end of fft2_inv_head and the next fft2_fwd (16 slots of 16 B per lane).
 // ------------------------------------------------------------------------------------------------
-template <class G> constexpr size_t chain_smem_bytes() {
-  return (size_t)(Lay<G>::XBUF + Lay<G>::TW + 2 * G::N) * sizeof(cf) + 1024 + (size_t)G::PF16 * G::T * 16;
-}
+template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::XBUF + Lay<G>::TW + (G::CL > 1 ? G::N : 0)) * sizeof(cf) + 1024; }
+template <class G> constexpr size_t chain_smem_bytes() { return fft_smem_bytes<G>() + (size_t)2 * G::NF * sizeof(cf) + (size_t)G::PF16 * G::T * 16; }
 template <class G>
 struct ChainSmem {
-  cf* sm; cf* tw; double* red; cf* hyS; float4* pf; float4* xs;
+  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs;
   __device__ __forceinline__ ChainSmem(unsigned char* raw, int t) {
     typedef Lay<G> L;
-    sm = (cf*)raw; tw = sm + L::XBUF; red = (double*)(tw + L::TW);
+    sm = (cf*)raw; tw = sm + L::XBUF; tw2 = tw + L::TW; red = (double*)(tw2 + (G::CL > 1 ? G::N : 0));
     hyS = (cf*)((unsigned char*)red + 1024);
-    pf = (float4*)(hyS + 2 * G::N) + t;                                 // early slot s: pf[s * T]
+    pf = (float4*)(hyS + 2 * G::NF) + t;                                // early slot s: pf[s * T]
     xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late slot s:  xs[s * 32]
+  }
+  // twiddle tables; the caller synchronises the CTA before the first transform
+  __device__ __forceinline__ void fill_tables(int t) {
+    for (int i = t; i < Lay<G>::TW; i += G::T) Lay<G>::fill_twiddle(tw, i);
+    for (int i = t; i < (G::CL > 1 ? G::N : 0); i += G::T) FL<G>::fill_tw2(tw2, i);
   }
 };
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
@@ -244,51 +249,51 @@ __device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 
-// offset (in object pixels) of register r's pixel from the thread's first pixel of the patch
-template <class G>
-__device__ __forceinline__ size_t patch_off(int r, int onx) { return (size_t)((r / G::N1X) * G::N2Y) * onx + (r & (G::N1X - 1)) * G::N2X; }
-
 // ------------------------------------------------------------------------------------------------
-// H1: P~_k = F(P_k), stored F-native.  Also used for Q~_k = F(dPhat_k) with scale/accumulator input.
-//   mode 0: in = raster complex64 field [k][N][N]
-//   mode 1: in = -gP_k / (delta_p + 1) from raster grad_probe (step-size sweep, O14)
+// H1: P~_k = F(P_k), stored Fourier-native.  Also used for Q~_k = F(dPhat_k) with a scale (step-size sweep, O14:
+// in = raster grad_probe, scale = -1 / (delta_p + 1)).  One CTA (CL = 4: one cluster) per mode.
 // ------------------------------------------------------------------------------------------------
 template <class G>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* in, cf* out, float scale) {
-  typedef Lay<G> L;
+  typedef Lay<G> L; typedef FL<G> F;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
-  const int t = threadIdx.x, k = blockIdx.x, N = G::N;
-  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  const int t = threadIdx.x, k = blockIdx.x / G::CL;
+  const unsigned rk = Fft<G>::rank();
+  ChainSmem<G> cs(smem_raw, t);
+  cs.fill_tables(t);
   __syncthreads();
   cf v[32];
-  const cf* src = in + (size_t)k * N * N;
+  const cf* src = in + (size_t)k * F::NNF;
 #pragma unroll
-  for (int r = 0; r < 32; ++r) v[r] = cscale(src[L::r_y(t, r) * N + L::r_x(t, r)], scale);
-  fft2_fwd<G>(v, sm, tw, t);
-  cf* dst = out + (size_t)k * N * N;
+  for (int r = 0; r < 32; ++r) v[r] = cscale(src[F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r)], scale);
+  Fft<G>::fwd(v, cs.sm, cs.tw, cs.tw2, t, rk);
+  cf* dst = out + ((size_t)k * G::CL + rk) * F::NNS;
 #pragma unroll
   for (int r = 0; r < 32; ++r) dst[L::native(t, r)] = v[r];
+  Fft<G>::end_fourier();
 }
 
-// H12 tail: gP_k = Finv(gP~_k): F-native double accumulators -> raster complex64 (overwrite or add)
+// H12 tail: gP_k = Finv(gP~_k): Fourier-native double accumulators -> raster complex64 (overwrite or add)
 template <class G>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const double2* acc, cf* out, int accumulate) {
-  typedef Lay<G> L;
+  typedef Lay<G> L; typedef FL<G> F;
   extern __shared__ __align__(16) unsigned char smem_raw[];
-  cf* sm = (cf*)smem_raw; cf* tw = sm + L::XBUF;
-  const int t = threadIdx.x, k = blockIdx.x, N = G::N;
-  for (int i = t; i < L::TW; i += G::T) L::fill_twiddle(tw, i);
+  const int t = threadIdx.x, k = blockIdx.x / G::CL;
+  const unsigned rk = Fft<G>::rank();
+  ChainSmem<G> cs(smem_raw, t);
+  cs.fill_tables(t);
+  Fft<G>::begin_fourier();
   __syncthreads();
   cf v[32];
-  const double sc = 1.0 / ((double)N * (double)N);
+  const double sc = 1.0 / ((double)F::NF * (double)F::NF);
+  const double2* a0 = acc + ((size_t)k * G::CL + rk) * F::NNS;
 #pragma unroll
-  for (int r = 0; r < 32; ++r) { double2 a = acc[(size_t)k * N * N + L::native(t, r)]; v[r] = make_float2((float)(a.x * sc), (float)(a.y * sc)); }
-  fft2_inv<G>(v, sm, tw, t);
-  cf* dst = out + (size_t)k * N * N;
+  for (int r = 0; r < 32; ++r) { double2 a = a0[L::native(t, r)]; v[r] = make_float2((float)(a.x * sc), (float)(a.y * sc)); }
+  Fft<G>::inv(v, cs.sm, cs.tw, cs.tw2, t, rk);
+  cf* dst = out + (size_t)k * F::NNF;
 #pragma unroll
   for (int r = 0; r < 32; ++r) {
-    cf* d = dst + L::r_y(t, r) * N + L::r_x(t, r);
+    cf* d = dst + F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r);
     if (accumulate) { cf o = *d; *d = make_float2(o.x + v[r].x, o.y + v[r].y); } else *d = v[r];
   }
 }
@@ -296,50 +301,32 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const doub
 // ------------------------------------------------------------------------------------------------
 // pointwise helpers on the register field
 // ------------------------------------------------------------------------------------------------
-// v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9)
-template <class G, bool CONJ>
-__device__ __forceinline__ void apply_prop(cf (&v)[32], const cf* hx, const cf* hy, float bandlim2, int t) {
-  typedef Lay<G> L;
-  const int qx = L::f_qx(t, 0);
-  cf wx = hx[qx];
-  if (CONJ) wx.y = -wx.y;
-  const int sx = signed_freq(qx, G::N);
-#pragma unroll
-  for (int r = 0; r < 32; ++r) {
-    const int qy = L::f_qy(t, r);
-    cf wy = hy[qy];
-    if (CONJ) wy.y = -wy.y;
-    cf h = cmul(wx, wy);
-    if (bandlim2 >= 0.0f) {
-      const int sy = signed_freq(qy, G::N);
-      if ((float)(sx * sx + sy * sy) > bandlim2) h = make_float2(0.f, 0.f);
-    }
-    v[r] = cmul(v[r], h);
-  }
-}
-
 // object patch pointer for (slice i, position window r0)
 __device__ __forceinline__ const cf* patch_ptr(const KP& P, int i, int r0y, int r0x) {
   return P.object + ((size_t)i * P.ony + r0y) * P.onx + r0x;
 }
 
-// ------------------------------------------------------------------------------------------------
-// pointwise helpers on the register field
-// ------------------------------------------------------------------------------------------------
+// the thread's NXV values of an x-table (hx row or shift ramp rx), optionally scaled
+template <class G>
+__device__ __forceinline__ void load_xv(cf (&wxv)[FL<G>::NXV], const cf* row, int t, float scale) {
+#pragma unroll
+  for (int c = 0; c < FL<G>::NXV; ++c) wxv[c] = cscale(row[Lay<G>::f_qx(t, 0) + c * G::N], scale);
+}
+
 // v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9); hy from shared memory
 template <class G, bool CONJ>
-__device__ __forceinline__ void apply_prop_s(cf (&v)[32], cf wx, const cf* hyS, float bandlim2, int t) {
-  typedef Lay<G> L;
-  if (CONJ) wx.y = -wx.y;
-  const int sx = signed_freq(L::f_qx(t, 0), G::N);
+__device__ __forceinline__ void apply_prop_s(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, int t, unsigned rk) {
+  typedef FL<G> F;
+  cf wxv[F::NXV];
+  load_xv<G>(wxv, hxrow, t, 1.0f);
 #pragma unroll
   for (int r = 0; r < 32; ++r) {
-    const int qy = L::f_qy(t, r);
-    cf wy = hyS[qy];
-    if (CONJ) wy.y = -wy.y;
+    const int qy = F::fq_y(rk, t, r);
+    cf wx = wxv[F::fq_xsel(r)], wy = hyS[qy];
+    if (CONJ) { wx.y = -wx.y; wy.y = -wy.y; }
     cf h = cmul(wx, wy);
     if (bandlim2 >= 0.0f) {
-      const int sy = signed_freq(qy, G::N);
+      const int sx = signed_freq(F::fq_x(rk, t, r), F::NF), sy = signed_freq(qy, F::NF);
       if ((float)(sx * sx + sy * sy) > bandlim2) h = make_float2(0.f, 0.f);
     }
     v[r] = cmul(v[r], h);
@@ -347,57 +334,59 @@ __device__ __forceinline__ void apply_prop_s(cf (&v)[32], cf wx, const cf* hyS, 
 }
 
 // ------------------------------------------------------------------------------------------------
-// H2..H6 forward: one CTA per (j,k) pair of the chunk
+// H2..H6 forward: one CTA (CL = 4: one cluster of four) per (j,k) pair of the chunk
 // ------------------------------------------------------------------------------------------------
 template <class G, bool STASH>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
-  typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N, T = G::T, E = G::PF16;     // E pair slots early, 16 - E late
+  typedef Lay<G> L; typedef FL<G> F;
+  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL;     // E pair slots early, 16 - E late
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x;
+  const unsigned rk = Fft<G>::rank();
   ChainSmem<G> cs(smem_raw, t);
   cf* sm = cs.sm; cf* tw = cs.tw;
-  for (int i = t; i < L::TW; i += T) L::fill_twiddle(tw, i);
-  const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  cs.fill_tables(t);
+  Fft<G>::begin_fourier();
+  const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int S = P.S, onx = P.onx;
   const size_t slice = (size_t)P.ony * onx;
-  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);   // this thread's first pixel, slice 0
+  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);   // this thread's first pixel, slice 0
   // H3 prefetch: patch values of registers [0, 2E) one FFT pair ahead into the thread's early slots
   auto early = [&](int i) {
     const cf* o = ob + (size_t)i * slice;
 #pragma unroll
-    for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.pf + (r >> 1) * T) + (r & 1), o + patch_off<G>(r, onx));
-    if (i < S - 1 && t < N) cp_async8(cs.hyS + (i & 1) * N + t, P.w.hy + (size_t)i * N + t);
+    for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.pf + (r >> 1) * T) + (r & 1), o + F::patch_off(r, onx));
+    if (i < S - 1 && t < NF) cp_async8(cs.hyS + (i & 1) * NF + t, P.w.hy + (size_t)i * NF + t);
     cp_async_commit();
   };
   early(0);
-  __syncthreads();                                               // twiddle table ready
-  const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
-  const cf* ry = rx + N;
-  const int qx = L::f_qx(t, 0);
+  __syncthreads();                                               // twiddle tables ready
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
+  const cf* ry = rx + NF;
   cf v[32];
-  {   // H2: R .* P~_k / N^2   (F-layout)
-    const float4* pt = (const float4*)(P.w.Pt + (size_t)k * NN);
-    const cf wx = cscale(rx[qx], 1.0f / (float)NN);
+  {   // H2: R .* P~_k / N^2   (Fourier layout)
+    const float4* pt = (const float4*)(P.w.Pt + ((size_t)k * CL + rk) * NNS);
+    cf wxv[F::NXV];
+    load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 q = pt[p * T + t];
-      v[2 * p] = cmul(make_float2(q.x, q.y), cmul(wx, ry[L::f_qy(t, 2 * p)]));
-      v[2 * p + 1] = cmul(make_float2(q.z, q.w), cmul(wx, ry[L::f_qy(t, 2 * p + 1)]));
+      v[2 * p] = cmul(make_float2(q.x, q.y), cmul(wxv[F::fq_xsel(2 * p)], ry[F::fq_y(rk, t, 2 * p)]));
+      v[2 * p + 1] = cmul(make_float2(q.z, q.w), cmul(wxv[F::fq_xsel(2 * p + 1)], ry[F::fq_y(rk, t, 2 * p + 1)]));
     }
   }
   for (int i = 0; i < S; ++i) {
-    fft2_inv_head<G>(v, sm, t);
+    Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     {   // registers [2E, 32) of T_i into the warp's idle X1 region
       const cf* o = ob + (size_t)i * slice;
 #pragma unroll
-      for (int r = 2 * E; r < 32; ++r) cp_async8((cf*)(cs.xs + ((r >> 1) - E) * 32) + (r & 1), o + patch_off<G>(r, onx));
+      for (int r = 2 * E; r < 32; ++r) cp_async8((cf*)(cs.xs + ((r >> 1) - E) * 32) + (r & 1), o + F::patch_off(r, onx));
       cp_async_commit();
     }
     L::phase1_inv(v, tw, t);                                     // Psi_{i,k}  (R-layout)
     cp_async_wait_all();
-    float4* st = (float4*)(P.w.stash + ((size_t)(jl * P.M + k) * S + i) * NN);
+    float4* st = (float4*)(P.w.stash + (((size_t)pair * S + i) * CL + rk) * NNS);
 #pragma unroll
     for (int p = 0; p < 16; ++p) {                               // stash Psi_i ; H3+H4: Phi = Psi .* T_i
       if (STASH) st[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
@@ -406,42 +395,43 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
       v[2 * p + 1] = cmul(v[2 * p + 1], make_float2(q.z, q.w));
     }
     if (i + 1 < S) early(i + 1);
-    fft2_fwd<G>(v, sm, tw, t);                                   // F(Phi)    (F-layout)
-    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx[(size_t)i * N + qx], cs.hyS + (i & 1) * N, P.bandlim2, t);   // H5
+    Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(Phi)    (Fourier layout)
+    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, t, rk);   // H5
   }
-  float4* out = (float4*)(P.w.psit + (size_t)(jl * P.M + k) * NN);   // H6: psi~ = F(Phi_{S-1}) / N
-  const float sc = 1.0f / (float)N;
+  float4* out = (float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);   // H6: psi~ = F(Phi_{S-1}) / N
+  const float sc = 1.0f / (float)NF;
 #pragma unroll
   for (int p = 0; p < 16; ++p) out[p * T + t] = make_float4(v[2 * p].x * sc, v[2 * p].y * sc, v[2 * p + 1].x * sc, v[2 * p + 1].y * sc);
+  Fft<G>::end_fourier();
 }
 
 // ------------------------------------------------------------------------------------------------
-// H7 + H8: I = sum_k |psi~_k|^2 ; per-pixel loss in fp64 ; w = dl/dI.  One CTA per position of the chunk.
+// H7 + H8: I = sum_k |psi~_k|^2 ; per-pixel loss in fp64 ; w = dl/dI.  One CTA per (position of the chunk, rank).
 // ------------------------------------------------------------------------------------------------
 template <class G>
-__global__ void __launch_bounds__(G::T) k_loss(KP P, float* loss_per_pos, float* model_intensity, int want_w) {
-  typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N;
+__global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int want_w) {
+  typedef Lay<G> L; typedef FL<G> F;
+  constexpr int NF = F::NF, NNS = F::NNS, CL = G::CL;
   __shared__ double red[(G::T / 32) * 1];
-  const int t = threadIdx.x, jl = blockIdx.x, jb = P.j0 + jl;
+  const int t = threadIdx.x, jl = blockIdx.x / CL, rk = blockIdx.x - jl * CL, jb = P.j0 + jl;
   const int row = P.batch_idx ? P.batch_idx[jb] : jb;
   float I[32];
 #pragma unroll
   for (int r = 0; r < 32; ++r) I[r] = 0.f;
   for (int k = 0; k < P.M; ++k) {
-    const cf* ps = P.w.psit + (size_t)(jl * P.M + k) * NN;
+    const cf* ps = P.w.psit + (((size_t)jl * P.M + k) * CL + rk) * NNS;
 #pragma unroll
     for (int r = 0; r < 32; ++r) { cf z = ps[L::native(t, r)]; I[r] = fmaf(z.x, z.x, fmaf(z.y, z.y, I[r])); }
   }
   double acc[1] = {0.0};
-  const float* Ie = P.intensity ? P.intensity + (size_t)row * NN : nullptr;
+  const float* Ie = P.intensity ? P.intensity + (size_t)row * F::NNF : nullptr;
   const double eps = (double)P.eps, c = (double)P.loss_c;
 #pragma unroll 4
   for (int r = 0; r < 32; ++r) {
-    const int qy = L::f_qy(t, r), qx = L::f_qx(t, r);
-    if (model_intensity) model_intensity[(size_t)jb * NN + qy * N + qx] = I[r];
+    const int qy = F::fq_y(rk, t, r), qx = F::fq_x(rk, t, r);
+    if (model_intensity) model_intensity[(size_t)jb * F::NNF + qy * NF + qx] = I[r];
     if (Ie) {
-      const double Im = (double)I[r], Ix = (double)Ie[qy * N + qx];
+      const double Im = (double)I[r], Ix = (double)Ie[qy * NF + qx];
       double l, w;
       if (P.loss == PT_LOSS_POISSON) {
         l = Im - Ix * (log(Im + eps) - log(Ix + eps) + 1.0);
@@ -452,53 +442,55 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* loss_per_pos, float*
         w = 0.5 * (1.0 - ae / (a + eps));
       }
       acc[0] += l;
-      if (want_w) P.w.wdet[(size_t)jl * NN + L::native(t, r)] = (float)w;
+      if (want_w) P.w.wdet[((size_t)jl * CL + rk) * NNS + L::native(t, r)] = (float)w;
     }
   }
   block_sum<G::T, 1>(acc, red);
   if (t == 0) {
-    P.w.loss_pp[jb] = acc[0];
-    if (loss_per_pos) loss_per_pos[jb] = (float)acc[0];
+    P.w.loss_pp[(size_t)jb * CL + rk] = acc[0];
     if (!(acc[0] == acc[0]) || fabs(acc[0]) > 1e300) atomicOr(P.w.status, kStatusNonfinite);
   }
 }
 
 // ------------------------------------------------------------------------------------------------
-// H9, H10, H12, H13 backward: one CTA per (j,k) pair of the chunk.
+// H9, H10, H12, H13 backward: one CTA (CL = 4: one cluster) per (j,k) pair of the chunk.
 // MODE 0: gradient pass — writes gT partials, probe partials, position terms.
 // MODE 1: step-size sweep (H14) — instead accumulates numO/denO per slice and the probe / position terms.
 // ------------------------------------------------------------------------------------------------
 template <class G, int MODE>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int want_pos) {
-  typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N, T = G::T, E = G::PF16;     // stash pairs [0,E) early, [E,16) late; T pairs [0,E) late
+  typedef Lay<G> L; typedef FL<G> F;
+  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL;   // stash pairs [0,E) early, [E,16) late; T pairs [0,E) late
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x;
+  const unsigned rk = Fft<G>::rank();
   ChainSmem<G> cs(smem_raw, t);
   cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
-  for (int i = t; i < L::TW; i += T) L::fill_twiddle(tw, i);
-  const int pair = blockIdx.x, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  cs.fill_tables(t);
+  Fft<G>::begin_fourier();
+  const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  const int unit = (jb * P.M + k) * CL + (int)rk;                 // index of this CTA's fp64 partials
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int S = P.S, onx = P.onx;
   const size_t slice = (size_t)P.ony * onx;
-  const size_t fld0 = (size_t)(jl * P.M + k) * S * NN;
-  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);
-  const int qx = L::f_qx(t, 0);
+  auto fld = [&](int i) { return (((size_t)pair * S + i) * CL + rk) * NNS; };   // field (pair, slice i), this rank's block
+  const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
+  const cf* ob = patch_ptr(P, 0, r0y, r0x) + pix0;
   // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
   auto early = [&](int i) {
-    const float4* st = (const float4*)(P.w.stash + fld0 + (size_t)i * NN) + t;
+    const float4* st = (const float4*)(P.w.stash + fld(i)) + t;
 #pragma unroll
     for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
-    if (i > 0 && t < N) cp_async8(cs.hyS + ((i - 1) & 1) * N + t, P.w.hy + (size_t)(i - 1) * N + t);
+    if (i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
     cp_async_commit();
   };
   early(S - 1);
   __syncthreads();
   cf v[32];
   {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = N Finv(g~) = F^H(g~) / N
-    const float4* ps = (const float4*)(P.w.psit + (size_t)(jl * P.M + k) * NN);
-    const float2* wd = (const float2*)(P.w.wdet + (size_t)jl * NN);
-    const float sc = 1.0f / (float)N;
+    const float4* ps = (const float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);
+    const float2* wd = (const float2*)(P.w.wdet + ((size_t)jl * CL + rk) * NNS);
+    const float sc = 1.0f / (float)NF;
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 q = ps[p * T + t]; const float2 w = wd[p * T + t];
@@ -507,26 +499,26 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     }
   }
   for (int i = S - 1; i >= 0; --i) {
-    fft2_inv_head<G>(v, sm, t);
+    Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
     {   // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
-      const float4* st = (const float4*)(P.w.stash + fld0 + (size_t)i * NN) + t;
+      const float4* st = (const float4*)(P.w.stash + fld(i)) + t;
 #pragma unroll
       for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
 #pragma unroll
-      for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.xs + (16 - E + (r >> 1)) * 32) + (r & 1), o + patch_off<G>(r, onx));
+      for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.xs + (16 - E + (r >> 1)) * 32) + (r & 1), o + F::patch_off(r, onx));
       cp_async_commit();
     }
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     if (MODE == 0) {
-      float4* gt = (float4*)(P.w.gTpart + fld0 + (size_t)i * NN);
+      float4* gt = (float4*)(P.w.gTpart + fld(i));
 #pragma unroll
       for (int p = 0; p < 16; ++p) {
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
         if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
-        else { T0 = o[patch_off<G>(2 * p, onx)]; T1 = o[patch_off<G>(2 * p + 1, onx)]; }
+        else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
         const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
         gt[p * T + t] = make_float4(g0.x, g0.y, g1.x, g1.y);    // H10: gT_i contribution conj(Psi) .* gPhi
         v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
@@ -535,10 +527,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       if (i > 0) early(i - 1);
     } else {
       // H14 object terms: u = dOhat|patch .* Psi ; chi = -gPhi ; num += Re(chi conj(u)) ; den += |u|^2
-      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x + (size_t)L::r_y(t, 0) * onx + L::r_x(t, 0);
+      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x + pix0;
       float num = 0.f, den = 0.f;
       if (i == 0) {                                              // keep gPhi_0 for the probe / position terms
-        float4* sc0 = (float4*)(P.w.scratch + (size_t)(jl * P.M + k) * NN);
+        float4* sc0 = (float4*)(P.w.scratch + ((size_t)pair * CL + rk) * NNS);
 #pragma unroll
         for (int p = 0; p < 16; ++p) sc0[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
       }
@@ -547,9 +539,9 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
         if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
-        else { T0 = o[patch_off<G>(2 * p, onx)]; T1 = o[patch_off<G>(2 * p + 1, onx)]; }
-        const cf u0 = cmul(dO[patch_off<G>(2 * p, onx)], make_float2(ps.x, ps.y));
-        const cf u1 = cmul(dO[patch_off<G>(2 * p + 1, onx)], make_float2(ps.z, ps.w));
+        else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
+        const cf u0 = cmul(dO[F::patch_off(2 * p, onx)], make_float2(ps.x, ps.y));
+        const cf u1 = cmul(dO[F::patch_off(2 * p + 1, onx)], make_float2(ps.z, ps.w));
         num -= fmaf(v[2 * p].x, u0.x, v[2 * p].y * u0.y) + fmaf(v[2 * p + 1].x, u1.x, v[2 * p + 1].y * u1.y);
         den = fmaf(u0.x, u0.x, fmaf(u0.y, u0.y, den));
         den = fmaf(u1.x, u1.x, fmaf(u1.y, u1.y, den));
@@ -560,32 +552,31 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       double acc[2] = {(double)num, (double)den};
       block_sum<G::T, 2>(acc, red);
       if (t == 0) {
-        double* sp = P.w.step_part + (size_t)(jb * P.M + k) * (2 * S + 6);
+        double* sp = P.w.step_part + (size_t)unit * (2 * S + 6);
         sp[2 * i] = acc[0]; sp[2 * i + 1] = acc[1];
       }
       if (i == 0) break;                                         // probe / position terms handled below
     }
-    fft2_fwd<G>(v, sm, tw, t);                                   // F(gPsi_i)  (F-layout)
-    if (i > 0) apply_prop_s<G, true>(v, P.w.hx[(size_t)(i - 1) * N + qx], cs.hyS + ((i - 1) & 1) * N, P.bandlim2, t);
+    Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(gPsi_i)  (Fourier layout)
+    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
   }
-  const cf* rx = P.w.ramps + (size_t)jb * 2 * N;
-  const cf* ry = rx + N;
-  const cf* pt = P.w.Pt + (size_t)k * NN;
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
+  const cf* ry = rx + NF;
+  const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
   if (MODE == 0) {
     // v = G~ = F(gPsi_0).  H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
-    cf* gp = P.w.Gpart + (size_t)(jl * P.M + k) * NN;
-    const int qx = L::f_qx(t, 0);
-    const cf wx = rx[qx];
-    const float fx = (float)signed_freq(qx, N) / (float)N;
+    cf* gp = P.w.Gpart + ((size_t)pair * CL + rk) * NNS;
+    cf wxv[F::NXV];
+    load_xv<G>(wxv, rx, t, 1.0f);
     float sy = 0.f, sx = 0.f;
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
-      const int qy = L::f_qy(t, r);
-      const cf R = cmul(wx, ry[qy]);
+      const int qy = F::fq_y(rk, t, r);
+      const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
       gp[L::native(t, r)] = cmulc(v[r], R);
       if (want_pos) {
         const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);  // conj(G~) R P~
-        const float fy = (float)signed_freq(qy, N) / (float)N;
+        const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(rk, t, r), NF) / (float)NF;
         sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
       }
     }
@@ -593,40 +584,39 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       double acc[2] = {(double)sy, (double)sx};
       block_sum<G::T, 2>(acc, red);
       if (t == 0) {
-        const double f = 4.0 * CUDART_PI / ((double)N * (double)N);
-        P.w.posg_part[(size_t)(jb * P.M + k) * 2 + 0] = f * acc[0];
-        P.w.posg_part[(size_t)(jb * P.M + k) * 2 + 1] = f * acc[1];
+        const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
+        P.w.posg_part[(size_t)unit * 2 + 0] = f * acc[0];
+        P.w.posg_part[(size_t)unit * 2 + 1] = f * acc[1];
       }
     }
+    Fft<G>::end_fourier();
   } else {
     // H14 probe and position terms at slice 0 (O14): three more fields from the Fourier side, each
     // compared with chi_0 = -gPhi_0 (kept in scratch) after multiplication by T_0.
-    const cf* sc0 = P.w.scratch + (size_t)(jl * P.M + k) * NN;
-    const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)L::r_y(t, 0) * P.onx + L::r_x(t, 0);
-    const cf* qt = P.w.Qt + (size_t)k * NN;
-    const int qx = L::f_qx(t, 0);
-    const cf wx = cscale(rx[qx], 1.0f / (float)NN);
-    const float fx = (float)signed_freq(qx, N) / (float)N;
-    double* sp = P.w.step_part + (size_t)(jb * P.M + k) * (2 * S + 6) + 2 * S;
+    const cf* sc0 = P.w.scratch + ((size_t)pair * CL + rk) * NNS;
+    const cf* qt = P.w.Qt + ((size_t)k * CL + rk) * NNS;
+    cf wxv[F::NXV];
+    load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
+    double* sp = P.w.step_part + (size_t)unit * (2 * S + 6) + 2 * S;
     for (int term = 0; term < 3; ++term) {
 #pragma unroll
       for (int r = 0; r < 32; ++r) {
-        const int qy = L::f_qy(t, r);
-        const cf R = cmul(wx, ry[qy]);
+        const int qy = F::fq_y(rk, t, r);
+        const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
         if (term == 0) v[r] = cmul(R, qt[L::native(t, r)]);                       // shift_j(dPhat_k)
         else {
-          const float f = term == 1 ? (float)signed_freq(qy, N) / (float)N : fx;  // d Psi_0 / d delta_a
+          const float f = (float)signed_freq(term == 1 ? qy : F::fq_x(rk, t, r), NF) / (float)NF;   // d Psi_0 / d delta_a
           const cf z = cmul(R, pt[L::native(t, r)]);
           const float g = -2.0f * CUDART_PI_F * f;
           v[r] = make_float2(-g * z.y, g * z.x);                                  // (i g) z
         }
       }
-      fft2_inv<G>(v, sm, tw, t);
+      Fft<G>::begin_fourier();
+      Fft<G>::inv(v, sm, tw, cs.tw2, t, rk);
       float num = 0.f, den = 0.f;
 #pragma unroll
       for (int r = 0; r < 32; ++r) {
-        const size_t o = (size_t)((r / G::N1X) * G::N2Y) * P.onx + (r & (G::N1X - 1)) * G::N2X;
-        const cf u = cmul(v[r], ob[o]);
+        const cf u = cmul(v[r], ob[F::patch_off(r, onx)]);
         const cf g = sc0[L::native(t, r)];
         num -= fmaf(g.x, u.x, g.y * u.y);
         den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
@@ -646,8 +636,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 // ------------------------------------------------------------------------------------------------
 template <class G, bool ILLUM>
 __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illum) {
-  typedef Lay<G> L;
-  constexpr int N = G::N, NN = N * N;
+  typedef FL<G> F;
+  constexpr int N = F::NF, NN = F::NNF;
   __shared__ int2 sr0[256];
   const int i = blockIdx.z;
   const int ox0 = blockIdx.x * 32, oy0 = blockIdx.y * 8;
@@ -663,7 +653,7 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
       if (r0.x > ox0 + 31 || r0.x + N <= ox0 || r0.y > oy0 + 7 || r0.y + N <= oy0) continue;   // block-uniform reject
       const int px = ox - r0.x, py = oy - r0.y;
       if (px >= 0 && px < N && py >= 0 && py < N) {
-        const int idx = L::r_native_of(py, px);
+        const int idx = F::r_native_of(py, px);
         const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
         for (int k = 0; k < P.M; ++k) {
           const cf g = P.w.gTpart[base + (size_t)k * P.S * NN];
@@ -698,19 +688,25 @@ __global__ void k_reduce_probe(KP P) {
 }
 
 // loss total (fixed-order fp64), position gradients (sum over modes, / px), step-term sums over modes
-__global__ void k_finalize(KP P, double* loss, int accumulate, float* grad_pos, float* step_terms) {
+// (cl = CTAs per field: every per-(position, mode) partial exists once per cluster rank)
+__global__ void k_finalize(KP P, int cl, double* loss, int accumulate, float* loss_per_pos, float* grad_pos, float* step_terms) {
   __shared__ double red[1024 / 32];
-  const int t = threadIdx.x;
-  if (loss) {
+  const int t = threadIdx.x, MU = P.M * cl;
+  if (loss || loss_per_pos) {
     double acc[1] = {0.0};
-    for (int j = t; j < P.J; j += 1024) acc[0] += P.w.loss_pp[j];
+    for (int j = t; j < P.J; j += 1024) {
+      double lj = 0.0;
+      for (int c = 0; c < cl; ++c) lj += P.w.loss_pp[(size_t)j * cl + c];
+      if (loss_per_pos) loss_per_pos[j] = (float)lj;
+      acc[0] += lj;
+    }
     block_sum<1024, 1>(acc, red);
-    if (t == 0) *loss = (accumulate ? *loss : 0.0) + acc[0];
+    if (t == 0 && loss) *loss = (accumulate ? *loss : 0.0) + acc[0];
   }
   if (grad_pos)
     for (int j = t; j < P.J; j += 1024) {
       double sy = 0.0, sx = 0.0;
-      for (int k = 0; k < P.M; ++k) { sy += P.w.posg_part[(size_t)(j * P.M + k) * 2]; sx += P.w.posg_part[(size_t)(j * P.M + k) * 2 + 1]; }
+      for (int k = 0; k < MU; ++k) { sy += P.w.posg_part[((size_t)j * MU + k) * 2]; sx += P.w.posg_part[((size_t)j * MU + k) * 2 + 1]; }
       grad_pos[2 * j] = (float)(sy / (double)P.px);
       grad_pos[2 * j + 1] = (float)(sx / (double)P.px);
     }
@@ -719,7 +715,7 @@ __global__ void k_finalize(KP P, double* loss, int accumulate, float* grad_pos, 
     for (int idx = t; idx < P.J * W; idx += 1024) {
       const int j = idx / W, c = idx - j * W;
       double s = 0.0;
-      for (int k = 0; k < P.M; ++k) s += P.w.step_part[(size_t)(j * P.M + k) * W + c];
+      for (int k = 0; k < MU; ++k) s += P.w.step_part[((size_t)j * MU + k) * W + c];
       step_terms[idx] = (float)s;
     }
   }
@@ -816,7 +812,7 @@ inline void prof_mark(int kind, cudaStream_t st) {
 
 int validate(const pt_problem* p) {
   if (!p) return PT_ERR_NULL;
-  if (p->n != 64 && p->n != 128) return p->n == 256 ? PT_ERR_UNSUPPORTED : PT_ERR_BAD_SIZE;
+  if (p->n != 64 && p->n != 128 && p->n != 256) return PT_ERR_BAD_SIZE;
   if (p->n_modes < 1 || p->n_slices < 1 || p->n_batch < 1 || p->n_pos_total < p->n_batch) return PT_ERR_BAD_SIZE;
   if (p->obj_ny < p->n || p->obj_nx < p->n) return PT_ERR_BAD_SIZE;
   if (!(p->pixel_size > 0.f) || !(p->wavelength > 0.f) || !(p->eps > 0.f)) return PT_ERR_BAD_PARAM;
@@ -839,6 +835,18 @@ KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64*
   k.object = (const cf*)object; k.probe = (const cf*)probe; k.positions = positions; k.intensity = intensity;
   k.batch_idx = batch_idx; k.w = w;
   return k;
+}
+
+// launch on `st`; CL = 4 geometries launch clusters of four consecutive CTAs (one field per cluster)
+template <class G, class... KArgs, class... Args>
+cudaError_t launch_fft(void (*kern)(KArgs...), unsigned grid, size_t smem, cudaStream_t st, Args... args) {
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(grid, 1, 1); cfg.blockDim = dim3(G::T, 1, 1); cfg.dynamicSmemBytes = smem; cfg.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeClusterDimension;
+  at[0].val.clusterDim.x = G::CL; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+  cfg.attrs = at; cfg.numAttrs = G::CL > 1 ? 1 : 0;
+  return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
 template <class G>
@@ -871,7 +879,7 @@ int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
   }
   k_setup_pos<<<p->n_batch, p->n, 0, st>>>(kp);
   LAUNCH_CHECK(K_setup_pos, st);
-  k_probe_fft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp.probe, kp.w.Pt, 1.0f);
+  launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f);
   LAUNCH_CHECK(K_probe_fft, st);
   return PT_OK;
 }
@@ -882,13 +890,13 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
   if (rc != PT_OK) return rc;
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    k_forward<G, false><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
+    launch_fft<G>(k_forward<G, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
-    k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, model_intensity_d, 0);
+    k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, model_intensity_d, 0);
     LAUNCH_CHECK(K_loss, st);
   }
-  if (loss_d) {
-    k_finalize<<<1, 1024, 0, st>>>(kp, loss_d, (p->flags & PT_ACCUMULATE) != 0, nullptr, nullptr);
+  if (loss_d || loss_per_pos_d) {
+    k_finalize<<<1, 1024, 0, st>>>(kp, G::CL, loss_d, (p->flags & PT_ACCUMULATE) != 0, loss_per_pos_d, nullptr, nullptr);
     LAUNCH_CHECK(K_finalize, st);
   }
   return PT_OK;
@@ -914,11 +922,11 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const dim3 ggrid((p->obj_nx + 31) / 32, (p->obj_ny + 7) / 8, p->n_slices), gblock(32, 8);
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    k_forward<G, true><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
+    launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
-    k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, loss_per_pos_d, nullptr, 1);
+    k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
-    k_backward<G, 0><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp, want_pos ? 1 : 0);
+    launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos ? 1 : 0);
     LAUNCH_CHECK(K_backward, st);
     if (want_illum) k_gather_object<G, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
     else k_gather_object<G, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
@@ -926,27 +934,27 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp);
     LAUNCH_CHECK(K_reduce_probe, st);
   }
-  k_probe_ifft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>(kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0);
+  launch_fft<G>(k_probe_ifft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const double2*)kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0);
   LAUNCH_CHECK(K_probe_ifft, st);
   if (want_steps) {
     // H14 second sweep (O13/O14): needs the batch-aggregated gO, gP
     k_dohat<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((const cf*)gO, illum_prev, p->lsqml_delta_o, kp.w.dOhat, on);
     LAUNCH_CHECK(K_dohat, st);
-    k_probe_fft<G><<<p->n_modes, G::T, fft_smem_bytes<G>(), st>>>((const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f));
+    launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f));
     LAUNCH_CHECK(K_probe_fft, st);
     for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
       if (kp.w.Jc < p->n_batch) {   // stash of this chunk was overwritten: recompute it
-        k_forward<G, true><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp);
+        launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
         LAUNCH_CHECK(K_forward, st);
-        k_loss<G><<<kp.jc, G::T, 0, st>>>(kp, nullptr, nullptr, 1);
+        k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
         LAUNCH_CHECK(K_loss, st);
       }
-      k_backward<G, 1><<<kp.jc * p->n_modes, G::T, chain_smem_bytes<G>(), st>>>(kp, 0);
+      launch_fft<G>(k_backward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
       LAUNCH_CHECK(K_backward, st);
     }
   }
-  k_finalize<<<1, 1024, 0, st>>>(kp, loss_d, acc ? 1 : 0, want_pos ? gX : nullptr, want_steps ? step_terms : nullptr);
+  k_finalize<<<1, 1024, 0, st>>>(kp, G::CL, loss_d, acc ? 1 : 0, loss_per_pos_d, want_pos ? gX : nullptr, want_steps ? step_terms : nullptr);
   LAUNCH_CHECK(K_finalize, st);
   return PT_OK;
 }
@@ -973,8 +981,8 @@ size_t ptycho_workspace_bytes(const pt_problem* p) {
     jc = (cap - f) / pp;
     // whole waves of 148 CTAs per chunk where possible
     const size_t wave = 148;
-    size_t pairs = jc * p->n_modes;
-    if (pairs > wave) { pairs -= pairs % wave; jc = pairs / p->n_modes; }
+    size_t pairs = jc * p->n_modes * cluster_of(p->n);
+    if (pairs > wave) { pairs -= pairs % wave; jc = pairs / (p->n_modes * cluster_of(p->n)); }
     if (jc < 1) jc = 1;
   }
   return f + jc * pp;
@@ -994,7 +1002,8 @@ int32_t ptycho_forward_loss(const pt_problem* p, const pt_c64* object_d, const p
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
   return p->n == 128 ? run_forward<Geo<128>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st)
-                     : run_forward<Geo<64>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st);
+       : p->n == 64 ? run_forward<Geo<64>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st)
+                    : run_forward<Geo<256>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st);
 }
 
 int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
@@ -1014,7 +1023,8 @@ int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c6
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
   return p->n == 128 ? run_gradient<Geo<128>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st)
-                     : run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st);
+       : p->n == 64 ? run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st)
+                    : run_gradient<Geo<256>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st);
 }
 
 int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe_d, float* positions_d,

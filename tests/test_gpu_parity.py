@@ -153,6 +153,40 @@ def test_n64_multislice_multimode():
 
 
 # ------------------------------------------------------------------------------------------------
+# config 4 geometry (N = 256: one field = a cluster of four CTAs) on a reduced scan / modes / slices, chunked
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("start", [0.0, 0.8])
+def test_cfg4_reduced_n256(start):
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(4, scan=(3, 4), n_modes=3, n_slices=4, obj_n=300)
+    case = make_case(cfg, start_scale=start)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    pbg = gpu_problem(cfg)
+    g = gpu_gradient(case, pbg, want_illum=True)
+    check(g, o, pos=start > 0, px=cfg.pixel_size)
+    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    min_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos, minimum=True)
+    full_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos)
+    g2 = gpu_gradient(case, pbg, max_ws=min_ws + (full_ws - min_ws) * 4 // 11 + 4096)   # 5 + 5 + 2 positions
+    check(g2, o, pos=start > 0, px=cfg.pixel_size)
+
+
+def test_n256_forward_intensity_bandlimit():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(4, scan=(2, 3), n_modes=2, n_slices=3, obj_n=300, bandlimit=2.0 / 3.0)
+    case = make_case(cfg, noise=False)
+    pbg = gpu_problem(cfg)
+    J = cfg.n_pos
+    mi = torch.empty((J, cfg.n, cfg.n), dtype=torch.float32, device="cuda")
+    ws = ptycho.make_workspace(pbg, J, J)
+    ptycho.forward_loss(pbg, _t(case.obj_true), _t(case.probe), _t(case.positions_true), None, workspace=ws, model_intensity=mi)
+    assert ptycho.status(ws) == 0
+    o = orc.forward_loss(oracle_problem(cfg), case.obj_true, case.probe, case.positions_true, case.intensity)
+    assert rel_l2(mi.cpu().numpy(), o["intensity"]) <= TOL_INT
+
+
+# ------------------------------------------------------------------------------------------------
 # mini-batches: batch_idx subsets + PT_ACCUMULATE over the batches == one call over all positions
 # ------------------------------------------------------------------------------------------------
 def test_batches_accumulate():
