@@ -35,7 +35,7 @@ def parse():
     ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="b200", choices=["b200", "reference"])
-    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 5])
+    ap.add_argument("--config", type=int, default=3, choices=[1, 2, 3, 4, 5])
     ap.add_argument("--cpu-sample", type=int, default=0, help="positions in the oracle sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
@@ -67,10 +67,17 @@ def host_inputs(cfg, rows=None):
     pos = synth.positions(cfg)
     if rows is not None:
         pos = pos[rows]
-    inten = synth.standin_patterns(cfg, rows)
+    if rows is None and cfg.n_pos > UNIQUE_PATTERN_ROWS:
+        # config 4 (16384 x 256 x 256 floats): draw UNIQUE_PATTERN_ROWS stand-in patterns and repeat them over the scan;
+        # the work per position does not depend on the pattern values (no data-dependent branches)
+        inten = np.tile(synth.standin_patterns(cfg, np.arange(UNIQUE_PATTERN_ROWS)), (cfg.n_pos // UNIQUE_PATTERN_ROWS, 1, 1))
+    else:
+        inten = synth.standin_patterns(cfg, rows)
     return obj, pr, pos, inten
 
 
+UNIQUE_PATTERN_ROWS = 1024
+MINIBATCH = {4: 1024}                                  # BASELINE.json configs[3]: mini-batches of 1024 positions
 LR = dict(lr_obj=1e-7, lr_probe=1e-7, lr_pos=1e-9)   # a real (tiny) SGD step so every timed step does the update
 
 
@@ -155,7 +162,7 @@ def run_reference(args):
         return
     from oracle import oracle as orc
     cfg, conf = workload(args.config)
-    n = args.cpu_sample or {1: 256, 2: 64, 3: 16, 5: 16}[args.config]
+    n = args.cpu_sample or {1: 256, 2: 64, 3: 16, 4: 4, 5: 16}[args.config]
     rows = np.arange(n)
     obj, pr, pos, inten = host_inputs(cfg, rows)
     pbo = orc.Problem(**problem_kwargs(cfg))
@@ -203,15 +210,33 @@ def run_b200(args):
     gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
     loss = torch.zeros(1, dtype=torch.float64, device="cuda")
     cap = int(args.ws_gib * (1 << 30)) if args.ws_gib > 0 else None
-    ws = ptycho.make_workspace(pbg, J, J, ptycho.WANT_POS_GRAD, max_bytes=cap)
+    mb = MINIBATCH.get(args.config)
+    from paper_2505_14372_b200 import synth as _synth
+    batches = None if mb is None else [torch.from_numpy(b).cuda() for b in _synth.batches(cfg, mb)]
+    ws = ptycho.make_workspace(pbg, J, mb or J, ptycho.WANT_POS_GRAD, max_bytes=cap)
+    if batches is not None:
+        conf.update(minibatch=mb, grouping="seeded permutation (sparse), gradients accumulated over the batches, one update")
+        args.no_e2e = True      # the host-buffer entry point takes one batch per call: no whole-iteration e2e at this size
 
     def step():
         # weak scaling over ranks: every rank owns J positions of the scan; object / probe are replicated, so the
         # only exchange is the sum of the object / probe gradients and the loss before the update.
-        ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
+        if batches is None:
+            ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
+        else:
+            o = 0
+            for i, b in enumerate(batches):
+                ptycho.gradient(pbg, obj, pr, pos, inten, b, workspace=ws, grad_object=gO, grad_probe=gP,
+                                grad_pos=gX[o:o + b.numel()], loss=loss, flags=ptycho.ACCUMULATE if i else 0)
+                o += b.numel()
         if dist is not None:
             dist.all_reduce(torch.view_as_real(gO)); dist.all_reduce(torch.view_as_real(gP)); dist.all_reduce(loss)
-        ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, **LR)
+        if batches is None:
+            ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, **LR)
+        else:
+            ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, batch_idx=order, **LR)
+
+    order = None if batches is None else torch.cat(batches)
 
     def barrier():
         torch.cuda.synchronize()
@@ -253,16 +278,26 @@ def run_b200(args):
     hbm, which, sm_max = measured_peaks()
     units_per_launch = J * args.steps / top_n
     ab = algorithmic_bytes_per_position(cfg, top)
-    roof = {"bound": "hbm", "kernel": top, "achieved": None, "peak": hbm, "unit": "GB/s", "frac": None, "traffic": None,
-            "peak_source": which, "share_of_step": top_ms / tot, "avg_launch_ms": top_ms / top_n,
+    # The FFT chain kernels are bound by plain FP32 arithmetic (19.5 flop/B against a machine balance of
+    # 11.4), so the line reports "alu": nominal FFT flops (5 N^2 log2 N^2 per 2-D FFT + pointwise) per launch over the
+    # launch duration, against 148 SM x 128 lanes x 2 flop x max SM clock.  The HBM view of the same kernel
+    # (algorithmic bytes: stash + far field) is given beside it.
+    fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    roof = {"bound": "alu", "kernel": top, "achieved": None, "peak": fp32_peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
+            "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md §6)",
+            "share_of_step": top_ms / tot, "avg_launch_ms": top_ms / top_n,
             "kernel_ms_per_step": {k: v[0] / args.steps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
     if ab is not None:
-        ach = ab * units_per_launch / (top_ms / top_n * 1e-3) / 1e9
-        roof.update(achieved=ach, frac=ach / hbm, algorithmic_bytes_per_launch=ab * units_per_launch)
+        sec = top_ms / top_n * 1e-3
+        fl = 0.5 * nominal_flops_per_position(cfg)              # the forward and the backward chain each do half of the FFTs
+        ach = fl * units_per_launch / sec / 1e12
+        achb = ab * units_per_launch / sec / 1e9
+        roof.update(achieved=ach, frac=ach / fp32_peak, nominal_flops_per_launch=fl * units_per_launch,
+                    hbm_view={"achieved": achb, "peak": hbm, "unit": "GB/s", "frac": achb / hbm, "peak_source": which,
+                              "algorithmic_bytes_per_launch": ab * units_per_launch})
     # whole-step view against both roofs of SURVEY §8(d): the io+act byte model and nominal FFT flops on the FP32 ALUs
     rate = J / (ms_step * 1e-3)
     b_model = 2 * cfg.n_modes * cfg.n_slices * cfg.n * cfg.n * 8 + cfg.n * cfg.n * 4
-    fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12
     roof["step_model"] = {"hbm_frac_io_act_model": b_model * rate / 1e9 / hbm,
                           "fp32_frac_nominal_fft_flops": nominal_flops_per_position(cfg) * rate / 1e12 / fp32_peak,
                           "fp32_peak_tflops_at_max_clock": fp32_peak}
@@ -301,7 +336,7 @@ def run_b200(args):
     cpu = None
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         from oracle import oracle as orc
-        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 5: 24}[args.config]
+        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 4: 4, 5: 24}[args.config]
         pbo = orc.Problem(**problem_kwargs(cfg))
         t0 = time.perf_counter()
         g = orc.gradient(pbo, obj_h, pr_h, pos_h, I_h, batch_idx=np.arange(n, dtype=np.int32))
