@@ -39,6 +39,7 @@ def parse():
     ap.add_argument("--cpu-sample", type=int, default=0, help="positions in the oracle sample (0: per-config default)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--batch", type=int, default=0, help="config 5: mini-batch size of the LSQML sweep (0: sweep 64/256/1024/4096)")
     ap.add_argument("--ws-gib", type=float, default=0.0, help="cap of the device workspace in GiB (0: library default)")
     return ap.parse_args()
 
@@ -190,7 +191,7 @@ def run_reference(args):
 
 def run_b200(args):
     import torch
-    from paper_2505_14372_b200 import ptycho
+    from paper_2505_14372_b200 import ptycho, shard
     rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
     local = int(os.environ.get("LOCAL_RANK", "0"))
     if not torch.cuda.is_available():
@@ -211,16 +212,39 @@ def run_b200(args):
     loss = torch.zeros(1, dtype=torch.float64, device="cuda")
     cap = int(args.ws_gib * (1 << 30)) if args.ws_gib > 0 else None
     mb = MINIBATCH.get(args.config)
+    lsqml = args.config == 5
+    if lsqml:
+        mb = args.batch or 1024
     from paper_2505_14372_b200 import synth as _synth
     batches = None if mb is None else [torch.from_numpy(b).cuda() for b in _synth.batches(cfg, mb)]
-    ws = ptycho.make_workspace(pbg, J, mb or J, ptycho.WANT_POS_GRAD, max_bytes=cap)
-    if batches is not None:
+    fl = ptycho.WANT_POS_GRAD | ((ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES) if lsqml else 0)
+    ws = ptycho.make_workspace(pbg, J, J if lsqml else (mb or J), fl, max_bytes=cap)
+    if batches is not None and not lsqml:
         conf.update(minibatch=mb, grouping="seeded permutation (sparse), gradients accumulated over the batches, one update")
         args.no_e2e = True      # the host-buffer entry point takes one batch per call: no whole-iteration e2e at this size
+    if lsqml:
+        # config 5: per batch, gradient + illumination map + step-size sweep (second pass over the chain) + LSQML update
+        conf.update(minibatch=mb, grouping="seeded permutation (sparse); per batch: gradient, step-size sweep, LSQML update",
+                    flags="POS_GRAD | ILLUM | STEP_SIZES")
+        illum = torch.zeros(obj.shape, dtype=torch.float32, device="cuda")
+        illum_prev = torch.full(obj.shape, float(cfg.dose) / (cfg.step_px ** 2), dtype=torch.float32, device="cuda")   # ~ dose per scan-step area
+        args.no_e2e = True      # the host-buffer entry point has no step-size outputs
+        st_terms = torch.empty((J, 2 * cfg.n_slices + 6), dtype=torch.float32, device="cuda")
+        LS = dict(mode=ptycho.UPDATE_LSQML, beta_obj=1e-3, beta_probe=1e-3, gamma=1e-2)
+
+    def lsqml_iteration(bl):
+        for b in bl:
+            nb = b.numel()
+            ptycho.gradient(pbg, obj, pr, pos, inten, b, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX[:nb], illum=illum,
+                            illum_prev=illum_prev, step_terms=st_terms[:nb], loss=loss)
+            ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, illum_prev=illum_prev, step_terms=st_terms[:nb],
+                                batch_idx=b, workspace=ws, **LS)
 
     def step():
         # weak scaling over ranks: every rank owns J positions of the scan; object / probe are replicated, so the
         # only exchange is the sum of the object / probe gradients and the loss before the update.
+        if lsqml:
+            return lsqml_iteration(batches)
         if batches is None:
             ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
         else:
@@ -230,7 +254,7 @@ def run_b200(args):
                                 grad_pos=gX[o:o + b.numel()], loss=loss, flags=ptycho.ACCUMULATE if i else 0)
                 o += b.numel()
         if dist is not None:
-            dist.all_reduce(torch.view_as_real(gO)); dist.all_reduce(torch.view_as_real(gP)); dist.all_reduce(loss)
+            shard.allreduce_sums(dist, gO, gP, loss)
         if batches is None:
             ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, **LR)
         else:
@@ -264,6 +288,17 @@ def run_b200(args):
     clk = clocks.stop() if clocks else None
     loss_val = loss.item()
     assert np.isfinite(loss_val) and ptycho.status(ws) == 0
+
+    sweep = None
+    if lsqml and not args.batch:
+        # the paper's grouping sweep: whole-iteration rate at each mini-batch size, one timed iteration each
+        sweep = {str(mb): J / (ms_step * 1e-3)}
+        for bsz in (64, 256, 4096):
+            bl = [torch.from_numpy(b).cuda() for b in _synth.batches(cfg, bsz)]
+            lsqml_iteration(bl)
+            torch.cuda.synchronize(); e0.record(); lsqml_iteration(bl); e1.record(); torch.cuda.synchronize()
+            sweep[str(bsz)] = J / (e0.elapsed_time(e1) * 1e-3)
+        conf.update(batch_sweep_positions_per_s=sweep)
 
     # per-kernel device time over the same K steps (CUDA events on the launching stream, inside the library)
     ptycho.profile_enable(True)
