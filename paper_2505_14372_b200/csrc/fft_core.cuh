@@ -98,7 +98,7 @@ template <int N_> struct Geo;
 template <> struct Geo<128> {
   static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
   static constexpr int NF = 128, CL = 1;
-  static constexpr int PF16 = 11;   // 16-byte prefetch slots per thread beside the exchange buffer (1 CTA / SM)
+  static constexpr int PF16 = 10;   // 16-byte prefetch slots per thread beside the exchange buffer (1 CTA / SM)
 };
 template <> struct Geo<64> {
   static constexpr int N = 64, LOGN = 6, T = 128, N1X = 8, N2X = 8, N1Y = 4, N2Y = 16, LX2 = 3, LY2 = 4, LP2 = 4, LP3 = 2;
@@ -114,9 +114,15 @@ template <> struct Geo<256> {
 template <class G>
 struct Lay {
   static constexpr int N = G::N, T = G::T;
-  static constexpr int X1_WARP = 33 * 32;                 // float2 slots per warp region (32 rows padded to 33)
-  static constexpr int X2_PLANE = G::N2Y * G::N + 8;      // float2 slots per k1y plane, skewed by 8
-  static constexpr int XBUF = (T / 32) * X1_WARP > 4 * X2_PLANE ? (T / 32) * X1_WARP : 4 * X2_PLANE;  // float2 slots
+  // The exchange buffer is one region of X1_WARP float2 slots per warp.  X1 (warp-local) lives in the calling
+  // warp's region; X2 is laid out so that its "p2" side (warp w holds rows b = w*LP2 .. w*LP2+LP2-1 of every
+  // k1y plane) also touches ONLY the calling warp's region: slot(b, k1y, qx) = (b / LP2)*X1_WARP +
+  // (b % LP2)*N1Y*X2_ROW + k1y*X2_ROW + qx.  Hence no CTA barrier is needed between an X1 access and a p2-side
+  // X2 access of the same warp; only the p3 side (which reads / writes every region) is fenced by CTA barriers.
+  static constexpr int X2_ROW = G::N + 8;                 // float2 slots per (b, k1y) row, skewed by 8 (ROW mod 16 = 8)
+  static constexpr int X2_WARP = G::LP2 * G::N1Y * X2_ROW;
+  static constexpr int X1_WARP = 33 * 32 > X2_WARP ? 33 * 32 : X2_WARP;   // float2 slots per warp region
+  static constexpr int XBUF = (T / 32) * X1_WARP;         // float2 slots
   static constexpr int TW = G::N1X * G::N2X + G::N1Y * G::N2Y;   // twiddle table entries (float2)
 
   // ---- R-layout: thread t, reg r -> (y, x)
@@ -265,33 +271,41 @@ struct Lay {
 #pragma unroll
     for (int r = 0; r < 32; ++r) v[r] = base[r];
   }
-  // ---- exchange X2: slot(k1y, b, qx) = k1y*X2_PLANE + b*N + qx.
+  // ---- exchange X2: slot(b, k1y, qx) as above.
   // "p2" side: thread t = warp w, lane (k1y, k1x); reg (bsel, k2x): b = w*LP2 + bsel, qx = k1x + N1X*k2x.
+  static PTK_HD int x2_slot(int b, int k1y, int qx) {
+    return (b / G::LP2) * X1_WARP + (b % G::LP2) * (G::N1Y * X2_ROW) + k1y * X2_ROW + qx;
+  }
   static PTK_HD int x2_base_p2(int t) {
     const int w = t >> 5, k1y = (t & 31) / G::N1X, k1x = t & (G::N1X - 1);
-    return k1y * X2_PLANE + (w * G::LP2) * N + k1x;
+    return w * X1_WARP + k1y * X2_ROW + k1x;
   }
+  static PTK_HD int x2_off_p2(int r) { return (r / G::N2X) * (G::N1Y * X2_ROW) + (r & (G::N2X - 1)) * G::N1X; }
   static PTK_HD void x2_store_p2(const cf (&v)[32], cf* sm, int t) {
     cf* base = sm + x2_base_p2(t);
 #pragma unroll
-    for (int r = 0; r < 32; ++r) base[(r / G::N2X) * N + (r & (G::N2X - 1)) * G::N1X] = v[r];
+    for (int r = 0; r < 32; ++r) base[x2_off_p2(r)] = v[r];
   }
   static PTK_HD void x2_load_p2(cf (&v)[32], const cf* sm, int t) {
     const cf* base = sm + x2_base_p2(t);
 #pragma unroll
-    for (int r = 0; r < 32; ++r) v[r] = base[(r / G::N2X) * N + (r & (G::N2X - 1)) * G::N1X];
+    for (int r = 0; r < 32; ++r) v[r] = base[x2_off_p2(r)];
   }
   // "p3" side: thread t = (qx, c); reg (ksel, b): k1y = c*LP3 + ksel.
-  static PTK_HD int x2_base_p3(int t) { return ((t >> G::LOGN) * G::LP3) * X2_PLANE + (t & (N - 1)); }
+  static PTK_HD int x2_base_p3(int t) { return ((t >> G::LOGN) * G::LP3) * X2_ROW + (t & (N - 1)); }
+  static PTK_HD int x2_off_p3(int r) {
+    const int ksel = r / G::N2Y, b = r & (G::N2Y - 1);
+    return ksel * X2_ROW + (b / G::LP2) * X1_WARP + (b % G::LP2) * (G::N1Y * X2_ROW);
+  }
   static PTK_HD void x2_store_p3(const cf (&v)[32], cf* sm, int t) {
     cf* base = sm + x2_base_p3(t);
 #pragma unroll
-    for (int r = 0; r < 32; ++r) base[(r / G::N2Y) * X2_PLANE + (r & (G::N2Y - 1)) * N] = v[r];
+    for (int r = 0; r < 32; ++r) base[x2_off_p3(r)] = v[r];
   }
   static PTK_HD void x2_load_p3(cf (&v)[32], const cf* sm, int t) {
     const cf* base = sm + x2_base_p3(t);
 #pragma unroll
-    for (int r = 0; r < 32; ++r) v[r] = base[(r / G::N2Y) * X2_PLANE + (r & (G::N2Y - 1)) * N];
+    for (int r = 0; r < 32; ++r) v[r] = base[x2_off_p3(r)];
   }
 };
 
@@ -368,9 +382,12 @@ __device__ __forceinline__ void st_cluster_v4(unsigned addr, cf a, cf b) {
 }
 
 // Whole transforms for one CTA.  `sm` = exchange buffer (Lay::XBUF float2), `tw` = twiddle table (Lay::TW).
-// Contract: fft2_fwd must follow an fft2_inv or a __syncthreads() (it starts by overwriting the calling warp's
-// own X1 region, which only that warp read last); fft2_inv may follow anything (it starts with a CTA barrier
-// because it overwrites the whole buffer).  Unnormalised.
+// Buffer protocol (one region of Lay::X1_WARP slots per warp, see Lay): X1 and the p2 side of X2 touch only the
+// calling warp's region and are ordered by __syncwarp(); the p3 side of X2 touches every region and is fenced
+// by two CTA barriers: one between the stores and the loads of the exchange (a true dependency) and one right
+// after the p3-side LOADS of the forward transform (cheap: every warp issues them at the same moment), after
+// which the whole buffer is free again.  Consequences: fft2_fwd may start whenever the calling warp is done
+// with its own region; fft2_inv_head may start after an fft2_fwd or any CTA barrier.  Unnormalised.
 template <class G>
 __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int t) {
   typedef Lay<G> L;
@@ -380,30 +397,31 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   __syncwarp();
   L::x1_load_p2(v, sm, t);
   L::template phase2<-1>(v);
-  __syncthreads();                 // every warp is done with its X1 region before X2 overwrites the buffer
+  __syncwarp();                    // every lane has read its X1 values: the warp's region may be overwritten
   L::x2_store_p2(v, sm, t);
   __syncthreads();
   L::x2_load_p3(v, sm, t);
+  __syncthreads();                 // all p3-side reads issued: the buffer is free for the next transform
   if (G::CL > 1) cluster_arrive();  // this thread no longer reads the exchange buffer: peers may overwrite it (Cross)
   L::template phase3<-1>(v);
 }
-// The inverse in two pieces: after the head, the calling warp's own X1 region (Lay::X1_WARP float2 slots at
+// The inverse in two pieces: after the head, the calling warp's own region (Lay::X1_WARP float2 slots at
 // sm + warp*X1_WARP) is free until that warp's next fft2_fwd / fft2_inv_head — the chain kernels land their
 // late cp.async prefetches there while phase 1 runs.
 template <class G>
 __device__ __forceinline__ void fft2_inv_head(cf (&v)[32], cf* sm, int t) {
   typedef Lay<G> L;
   L::template phase3<+1>(v);
-  __syncthreads();
+  if (G::CL > 1) __syncthreads();  // Cross::inv: other warps may still be reading what peers sent into this buffer
   L::x2_store_p3(v, sm, t);
   __syncthreads();
   L::x2_load_p2(v, sm, t);
   L::template phase2<+1>(v);
-  __syncthreads();                 // all X2 reads done before the warp-local X1 regions are overwritten
+  __syncwarp();                    // own-region X2 reads done before the warp-local X1 exchange overwrites them
   L::x1_store_p2(v, sm, t);
   __syncwarp();
   L::x1_load_p1(v, sm, t);
-  __syncwarp();                    // every lane has read its part: the warp's X1 region is free
+  __syncwarp();                    // every lane has read its part: the warp's region is free
 }
 template <class G>
 __device__ __forceinline__ void fft2_inv(cf (&v)[32], cf* sm, const cf* tw, int t) {

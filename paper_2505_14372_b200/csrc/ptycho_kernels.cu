@@ -226,13 +226,16 @@ template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::X
 template <class G> constexpr size_t chain_smem_bytes() { return fft_smem_bytes<G>() + (size_t)2 * G::NF * sizeof(cf) + (size_t)G::PF16 * G::T * 16; }
 template <class G>
 struct ChainSmem {
-  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs;
+  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs; cf* pf8; cf* xs8;
   __device__ __forceinline__ ChainSmem(unsigned char* raw, int t) {
     typedef Lay<G> L;
     sm = (cf*)raw; tw = sm + L::XBUF; tw2 = tw + L::TW; red = (double*)(tw2 + (G::CL > 1 ? G::N : 0));
     hyS = (cf*)((unsigned char*)red + 1024);
-    pf = (float4*)(hyS + 2 * G::NF) + t;                                // early slot s: pf[s * T]
-    xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late slot s:  xs[s * 32]
+    pf = (float4*)(hyS + 2 * G::NF) + t;                                // early 16-byte slot s: pf[s * T]
+    xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late 16-byte slot s:  xs[s * 32]
+    // the same two regions viewed as 8-byte slots (lanes 8 bytes apart: conflict-free cp.async writes and reads)
+    pf8 = (cf*)(hyS + 2 * G::NF) + t;                                   // early 8-byte slot s: pf8[s * T]
+    xs8 = sm + (t >> 5) * L::X1_WARP + (t & 31);                        // late 8-byte slot s:  xs8[s * 32]
   }
   // twiddle tables; the caller synchronises the CTA before the first transform
   __device__ __forceinline__ void fill_tables(int t) {
@@ -356,7 +359,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   auto early = [&](int i) {
     const cf* o = ob + (size_t)i * slice;
 #pragma unroll
-    for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.pf + (r >> 1) * T) + (r & 1), o + F::patch_off(r, onx));
+    for (int r = 0; r < 2 * E; ++r) cp_async8(cs.pf8 + r * T, o + F::patch_off(r, onx));
     if (i < S - 1 && t < NF) cp_async8(cs.hyS + (i & 1) * NF + t, P.w.hy + (size_t)i * NF + t);
     cp_async_commit();
   };
@@ -381,7 +384,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     {   // registers [2E, 32) of T_i into the warp's idle X1 region
       const cf* o = ob + (size_t)i * slice;
 #pragma unroll
-      for (int r = 2 * E; r < 32; ++r) cp_async8((cf*)(cs.xs + ((r >> 1) - E) * 32) + (r & 1), o + F::patch_off(r, onx));
+      for (int r = 2 * E; r < 32; ++r) cp_async8(cs.xs8 + (r - 2 * E) * 32, o + F::patch_off(r, onx));
       cp_async_commit();
     }
     L::phase1_inv(v, tw, t);                                     // Psi_{i,k}  (R-layout)
@@ -390,9 +393,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
 #pragma unroll
     for (int p = 0; p < 16; ++p) {                               // stash Psi_i ; H3+H4: Phi = Psi .* T_i
       if (STASH) st[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
-      const float4 q = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
-      v[2 * p] = cmul(v[2 * p], make_float2(q.x, q.y));
-      v[2 * p + 1] = cmul(v[2 * p + 1], make_float2(q.z, q.w));
+      const cf T0 = p < E ? cs.pf8[(2 * p) * T] : cs.xs8[(2 * p - 2 * E) * 32];
+      const cf T1 = p < E ? cs.pf8[(2 * p + 1) * T] : cs.xs8[(2 * p + 1 - 2 * E) * 32];
+      v[2 * p] = cmul(v[2 * p], T0);
+      v[2 * p + 1] = cmul(v[2 * p + 1], T1);
     }
     if (i + 1 < S) early(i + 1);
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(Phi)    (Fourier layout)
@@ -506,7 +510,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 #pragma unroll
       for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
 #pragma unroll
-      for (int r = 0; r < 2 * E; ++r) cp_async8((cf*)(cs.xs + (16 - E + (r >> 1)) * 32) + (r & 1), o + F::patch_off(r, onx));
+      for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
       cp_async_commit();
     }
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
@@ -517,7 +521,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       for (int p = 0; p < 16; ++p) {
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
-        if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
+        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
         else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
         const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
         gt[p * T + t] = make_float4(g0.x, g0.y, g1.x, g1.y);    // H10: gT_i contribution conj(Psi) .* gPhi
@@ -538,7 +542,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       for (int p = 0; p < 16; ++p) {
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
-        if (p < E) { const float4 q = cs.xs[(16 - E + p) * 32]; T0 = make_float2(q.x, q.y); T1 = make_float2(q.z, q.w); }
+        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
         else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
         const cf u0 = cmul(dO[F::patch_off(2 * p, onx)], make_float2(ps.x, ps.y));
         const cf u1 = cmul(dO[F::patch_off(2 * p + 1, onx)], make_float2(ps.z, ps.w));
