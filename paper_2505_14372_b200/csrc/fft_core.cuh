@@ -384,9 +384,9 @@ __device__ __forceinline__ void st_cluster_v4(unsigned addr, cf a, cf b) {
 // Whole transforms for one CTA.  `sm` = exchange buffer (Lay::XBUF float2), `tw` = twiddle table (Lay::TW).
 // Buffer protocol (one region of Lay::X1_WARP slots per warp, see Lay): X1 and the p2 side of X2 touch only the
 // calling warp's region and are ordered by __syncwarp(); the p3 side of X2 touches every region and is fenced
-// by two CTA barriers: one between the stores and the loads of the exchange (a true dependency) and one right
-// after the p3-side LOADS of the forward transform (cheap: every warp issues them at the same moment), after
-// which the whole buffer is free again.  Consequences: fft2_fwd may start whenever the calling warp is done
+// by two CTA barriers: one between the stores and the loads of the exchange (a true dependency) and one at the
+// end of the forward transform (inside an arithmetic-only stretch, so it costs only the skew between warps),
+// after which the whole buffer is free again.  Consequences: fft2_fwd may start whenever the calling warp is done
 // with its own region; fft2_inv_head may start after an fft2_fwd or any CTA barrier.  Unnormalised.
 template <class G>
 __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int t) {
@@ -401,9 +401,11 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   L::x2_store_p2(v, sm, t);
   __syncthreads();
   L::x2_load_p3(v, sm, t);
-  __syncthreads();                 // all p3-side reads issued: the buffer is free for the next transform
   if (G::CL > 1) cluster_arrive();  // this thread no longer reads the exchange buffer: peers may overwrite it (Cross)
   L::template phase3<-1>(v);
+  __syncthreads();                 // all p3-side reads are long done: the buffer is free for the next transform.
+                                   // Placed after the arithmetic, not after the loads: a barrier behind a burst of
+                                   // LDS releases only when the LAST warp got its loads into the queue (~1k cycles)
 }
 // The inverse in two pieces: after the head, the calling warp's own region (Lay::X1_WARP float2 slots at
 // sm + warp*X1_WARP) is free until that warp's next fft2_fwd / fft2_inv_head — the chain kernels land their

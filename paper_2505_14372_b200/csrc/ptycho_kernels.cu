@@ -249,9 +249,14 @@ __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
 __device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
 }
+// 8-byte read-only load pinned where it is written (asm volatile keeps its place among the other memory operations)
+__device__ __forceinline__ cf ld_nc8(const cf* p) {
+  cf v;
+  asm volatile("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
+  return v;
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
-
 // ------------------------------------------------------------------------------------------------
 // H1: P~_k = F(P_k), stored Fourier-native.  Also used for Q~_k = F(dPhat_k) with a scale (step-size sweep, O14:
 // in = raster grad_probe, scale = -1 / (delta_p + 1)).  One CTA (CL = 4: one cluster) per mode.
@@ -316,24 +321,30 @@ __device__ __forceinline__ void load_xv(cf (&wxv)[FL<G>::NXV], const cf* row, in
   for (int c = 0; c < FL<G>::NXV; ++c) wxv[c] = cscale(row[Lay<G>::f_qx(t, 0) + c * G::N], scale);
 }
 
-// v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9); hy from shared memory
-template <class G, bool CONJ>
-__device__ __forceinline__ void apply_prop_s(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, int t, unsigned rk) {
+// v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9); hy from shared memory.
+// The mask test is hoisted out of the unrolled loop (block-uniform branch): the five configs run with the mask off.
+template <class G, bool CONJ, bool MASK>
+__device__ __forceinline__ void apply_prop_body(cf (&v)[32], const cf (&wxv)[FL<G>::NXV], const cf* hyS, float bandlim2, int t, unsigned rk) {
   typedef FL<G> F;
-  cf wxv[F::NXV];
-  load_xv<G>(wxv, hxrow, t, 1.0f);
 #pragma unroll
   for (int r = 0; r < 32; ++r) {
     const int qy = F::fq_y(rk, t, r);
     cf wx = wxv[F::fq_xsel(r)], wy = hyS[qy];
     if (CONJ) { wx.y = -wx.y; wy.y = -wy.y; }
     cf h = cmul(wx, wy);
-    if (bandlim2 >= 0.0f) {
+    if (MASK) {
       const int sx = signed_freq(F::fq_x(rk, t, r), F::NF), sy = signed_freq(qy, F::NF);
       if ((float)(sx * sx + sy * sy) > bandlim2) h = make_float2(0.f, 0.f);
     }
     v[r] = cmul(v[r], h);
   }
+}
+template <class G, bool CONJ>
+__device__ __forceinline__ void apply_prop_s(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, int t, unsigned rk) {
+  cf wxv[FL<G>::NXV];
+  load_xv<G>(wxv, hxrow, t, 1.0f);
+  if (bandlim2 >= 0.0f) apply_prop_body<G, CONJ, true>(v, wxv, hyS, bandlim2, t, rk);
+  else apply_prop_body<G, CONJ, false>(v, wxv, hyS, bandlim2, t, rk);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -513,6 +524,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
       cp_async_commit();
     }
+    // T registers [2E, 32) have no slot left in shared memory: plain loads, issued a whole phase ahead of their use
+    cf Tr[32 - 2 * E];
+#pragma unroll
+    for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     if (MODE == 0) {
@@ -522,7 +537,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
         if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
+        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
         const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
         gt[p * T + t] = make_float4(g0.x, g0.y, g1.x, g1.y);    // H10: gT_i contribution conj(Psi) .* gPhi
         v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
@@ -543,7 +558,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
         cf T0, T1;
         if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = o[F::patch_off(2 * p, onx)]; T1 = o[F::patch_off(2 * p + 1, onx)]; }
+        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
         const cf u0 = cmul(dO[F::patch_off(2 * p, onx)], make_float2(ps.x, ps.y));
         const cf u1 = cmul(dO[F::patch_off(2 * p + 1, onx)], make_float2(ps.z, ps.w));
         num -= fmaf(v[2 * p].x, u0.x, v[2 * p].y * u0.y) + fmaf(v[2 * p + 1].x, u1.x, v[2 * p + 1].y * u1.y);
@@ -634,19 +649,23 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 }
 
 // ------------------------------------------------------------------------------------------------
-// H11: deterministic object-gradient scatter-add as an owner-computes gather.  Block = 32 x 8 object pixels of
+// H11: deterministic object-gradient scatter-add as an owner-computes gather.  Block = 64 x 4 object pixels of
 // one slice; each pixel sums, in fixed (j ascending, k ascending) order, the patch-gradient entries that
 // land on it, in fp64, then adds the chunk total to gO once.  Optionally the illumination map (O12).
 // ------------------------------------------------------------------------------------------------
+#ifndef GATHER_TW
+#define GATHER_TW 64     // tile width in object pixels (256 threads per block)
+#endif
 template <class G, bool ILLUM>
 __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illum) {
   typedef FL<G> F;
   constexpr int N = F::NF, NN = F::NNF;
   __shared__ int2 sr0[256];
   const int i = blockIdx.z;
-  const int ox0 = blockIdx.x * 32, oy0 = blockIdx.y * 8;
+  constexpr int TW_ = GATHER_TW, TH_ = 256 / GATHER_TW;
+  const int ox0 = blockIdx.x * TW_, oy0 = blockIdx.y * TH_;
   const int ox = ox0 + threadIdx.x, oy = oy0 + threadIdx.y;
-  const int tid = threadIdx.y * 32 + threadIdx.x;
+  const int tid = threadIdx.y * TW_ + threadIdx.x;
   double ar = 0.0, ai = 0.0, al = 0.0;
   for (int jbase = 0; jbase < P.jc; jbase += 256) {
     const int cnt = min(256, P.jc - jbase);
@@ -654,7 +673,7 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
     __syncthreads();
     for (int jj = 0; jj < cnt; ++jj) {
       const int2 r0 = sr0[jj];
-      if (r0.x > ox0 + 31 || r0.x + N <= ox0 || r0.y > oy0 + 7 || r0.y + N <= oy0) continue;   // block-uniform reject
+      if (r0.x > ox0 + TW_ - 1 || r0.x + N <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + N <= oy0) continue;   // block-uniform reject
       const int px = ox - r0.x, py = oy - r0.y;
       if (px >= 0 && px < N && py >= 0 && py < N) {
         const int idx = F::r_native_of(py, px);
@@ -923,7 +942,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     LAUNCH_CHECK(K_zero, st);
     if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, on); LAUNCH_CHECK(K_zero, st); }
   }
-  const dim3 ggrid((p->obj_nx + 31) / 32, (p->obj_ny + 7) / 8, p->n_slices), gblock(32, 8);
+  const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
     launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
