@@ -79,6 +79,9 @@ typedef struct {                  /* HOST struct */
  * smallest size the calls accept.  The first 64 bytes hold the deferred status word. */
 size_t ptycho_workspace_bytes(const pt_problem *p);
 size_t ptycho_workspace_min_bytes(const pt_problem *p);
+/* Positions kept in flight per chunk (the memory unit, as opposed to the mini-batch p->n_batch, the optimisation
+ * unit) for a workspace of workspace_bytes; 0 if the problem is invalid or the size too small. */
+int32_t ptycho_positions_in_flight(const pt_problem *p, size_t workspace_bytes);
 
 /* Forward model + loss.
  *   object_d     [S][obj_ny][obj_nx]  transmission functions O_i

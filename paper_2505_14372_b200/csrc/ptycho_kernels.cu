@@ -995,6 +995,14 @@ size_t ptycho_workspace_min_bytes(const pt_problem* p) {
   return f + pp;
 }
 
+int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) {
+  if (validate(p) != PT_OK) return 0;
+  size_t f, pp; ws_sizes(p, &f, &pp);
+  if (workspace_bytes < f + pp) return 0;
+  size_t jc = (workspace_bytes - f) / pp;
+  return (int32_t)(jc > (size_t)p->n_batch ? (size_t)p->n_batch : jc);
+}
+
 size_t ptycho_workspace_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
   size_t f, pp; ws_sizes(p, &f, &pp);

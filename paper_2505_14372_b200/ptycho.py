@@ -21,7 +21,7 @@ SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
 WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE = 1, 2, 4, 16
 UPDATE_SGD, UPDATE_LSQML = 0, 1
 OK = 0
-EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_forward_loss", "ptycho_gradient",
+EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
            "ptycho_apply_update", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
            "ptycho_launch_count", "ptycho_strerror", "ptycho_profile_enable", "ptycho_profile_num_kernels",
            "ptycho_profile_kernel_name", "ptycho_profile_read"]
@@ -145,6 +145,15 @@ def workspace_bytes(pb: Problem, n_pos_total: int, n_batch: int, flags: int = 0,
     if n == 0:
         raise PtychoError(-2)
     return n
+
+
+def positions_in_flight(pb: Problem, n_pos_total: int, n_batch: int, flags: int = 0, workspace_bytes_: Optional[int] = None) -> int:
+    """ptycho_positions_in_flight: chunk size for a workspace of the given (default: recommended) size."""
+    cs = pb.c_struct(n_pos_total, n_batch, flags)
+    n = workspace_bytes(pb, n_pos_total, n_batch, flags) if workspace_bytes_ is None else workspace_bytes_
+    f = lib().ptycho_positions_in_flight
+    f.restype = C.c_int32
+    return int(f(C.byref(cs), C.c_size_t(n)))
 
 
 def make_workspace(pb: Problem, n_pos_total: int, n_batch: int, flags: int = 0, max_bytes: Optional[int] = None, host: bool = False):

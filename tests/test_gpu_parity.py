@@ -338,3 +338,60 @@ def test_gradient_host_matches_device_path():
     assert gP_h.numpy().tobytes() == g["grad_probe"].tobytes()
     assert gX_h.numpy().tobytes() == g["grad_pos"].tobytes()
     assert loss_h.item() == g["loss"]
+
+
+# ------------------------------------------------------------------------------------------------
+# config 3 at FULL size, in the launch configuration bench.py times (4096 positions, default workspace: chunks of
+# ~777 positions, stand-in patterns): the oracle cannot do the whole pass in seconds, so it checks
+#   (1) per-position loss and position gradient of SAMPLED positions (first, last, both sides of a chunk edge,
+#       two in the middle) — each depends on that position alone, so the oracle computes them one by one;
+#   (2) the object gradient on a patch at the corner of the scan footprint, where only a handful of windows
+#       overlap: the oracle's gradient over exactly those positions is the whole sum there;
+#   (3) properties that hold at any size: sum of per-position losses = loss; object gradient exactly zero where no
+#       window reaches; finite everywhere.
+# ------------------------------------------------------------------------------------------------
+def test_cfg3_full_size_sampled():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(3)
+    N, J = cfg.n, cfg.n_pos
+    phi = synth.object_phase(cfg)
+    obj = synth.object_from_phase(phi, 0.8)
+    pr = synth.probe(cfg)
+    pos = synth.positions(cfg)
+    inten = synth.standin_patterns(cfg)
+    pbg, pbo = gpu_problem(cfg), oracle_problem(cfg)
+    obj_d, pr_d, pos_d, I_d = _t(obj), _t(pr), _t(pos), _t(inten)
+    gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+    gX = torch.full((J, 2), float("nan"), dtype=torch.float32, device="cuda")
+    lpp = torch.full((J,), float("nan"), dtype=torch.float32, device="cuda")
+    loss = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+    ws = ptycho.make_workspace(pbg, J, J)                                 # library default: what bench.py uses
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX,
+                    loss=loss, loss_per_pos=lpp)
+    assert ptycho.status(ws) == 0
+    gO_h, gX_h, lpp_h = gO.cpu().numpy(), gX.cpu().numpy(), lpp.cpu().numpy()
+    assert np.isfinite(gO_h.view(np.float32)).all() and np.isfinite(gP.cpu().numpy().view(np.float32)).all()
+    # (3) properties
+    assert abs(lpp_h.astype(np.float64).sum() - loss.item()) <= 1e-6 * abs(loss.item())
+    c = pos / np.float32(cfg.pixel_size) - np.float32(N // 2)               # window corners, reading R2 (float32)
+    r0 = np.floor(c + np.float32(0.5)).astype(np.int64)
+    cover = np.zeros((cfg.obj_n, cfg.obj_n), np.int32)
+    for j in range(J):
+        cover[r0[j, 0]:r0[j, 0] + N, r0[j, 1]:r0[j, 1] + N] += 1
+    assert (gO_h[:, cover == 0] == 0).all()
+    # (1) sampled positions, one by one
+    jc = ptycho.positions_in_flight(pbg, J, J)
+    assert 0 < jc < J                                                     # the pass really runs in several chunks
+    sample = sorted({0, J - 1, jc - 1, jc, J // 2 + 17, 3 * J // 4 + 5})
+    for j in sample:
+        o = orc.gradient(pbo, obj, pr, pos[j:j + 1], inten[j:j + 1])
+        assert abs(lpp_h[j] - o["loss_per_pos"][0]) <= 2e-5 * abs(o["loss_per_pos"][0]), (j, lpp_h[j], o["loss_per_pos"][0])
+        assert rel_l2(gX_h[j], o["grad_pos"][0]) <= TOL_GRAD, (j, gX_h[j], o["grad_pos"][0])
+    # (2) object gradient on a corner patch of the scan footprint
+    y0, x0 = int(r0[:, 0].min()), int(r0[:, 1].min())
+    py, px_ = slice(y0, y0 + 6), slice(x0, x0 + 6)
+    rows = np.array([j for j in range(J) if r0[j, 0] <= y0 + 5 and r0[j, 1] <= x0 + 5 and r0[j, 0] + N > y0 and r0[j, 1] + N > x0])
+    assert 1 <= rows.size <= 16
+    o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
+    assert rel_l2(gO_h[:, py, px_], o["grad_object"][:, py, px_]) <= TOL_GRAD
