@@ -36,11 +36,12 @@ class _Problem(C.Structure):
         ("slice_thickness", C.POINTER(C.c_float)),
         ("tilt_x_mrad", C.c_float), ("tilt_y_mrad", C.c_float), ("bandlimit", C.c_float),
         ("loss", C.c_int32), ("loss_c", C.c_float), ("eps", C.c_float),
-        ("lsqml_delta_o", C.c_float), ("lsqml_delta_p", C.c_float),
+        ("lsqml_delta_o", C.c_float), ("lsqml_delta_p", C.c_float), ("shift_mode", C.c_int32),
     ]
 
 
 LOSS_AMPLITUDE, LOSS_POISSON = 0, 1
+SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
 
 _lib = None
 
@@ -76,6 +77,7 @@ class Problem:
     eps: float = 0.5
     lsqml_delta_o: float = 1.0
     lsqml_delta_p: float = 0.0
+    shift_mode: int = 0
 
     def _c(self, n_pos_total: int, n_batch: int):
         dz = np.ascontiguousarray(np.asarray(self.slice_thickness, dtype=np.float32))
@@ -83,7 +85,8 @@ class Problem:
             dz = np.concatenate([dz, np.zeros(self.n_slices - dz.size, np.float32)])
         s = _Problem(self.n, self.n_modes, self.n_slices, self.obj_ny, self.obj_nx, n_pos_total, n_batch,
                      self.pixel_size, self.wavelength, _p(dz, C.c_float), self.tilt_x_mrad, self.tilt_y_mrad,
-                     self.bandlimit, self.loss, self.loss_c, self.eps, self.lsqml_delta_o, self.lsqml_delta_p)
+                     self.bandlimit, self.loss, self.loss_c, self.eps, self.lsqml_delta_o, self.lsqml_delta_p,
+                     self.shift_mode)
         s._keep = dz
         return s
 
@@ -123,6 +126,25 @@ def position_split(X, px, n):
     r0 = C.c_int32(); d = C.c_float()
     lib().orc_position_split(C.c_float(X), C.c_float(px), n, C.byref(r0), C.byref(d))
     return r0.value, d.value
+
+
+def position_split_floor(X, px, n):
+    i0 = C.c_int32(); f = C.c_float()
+    lib().orc_position_split_floor(C.c_float(X), C.c_float(px), n, C.byref(i0), C.byref(f))
+    return i0.value, f.value
+
+
+def bilinear(n, obj, i0y, i0x, fy, fx, patch=None):
+    """patch = bilinear gather of obj (complex128 [ony][onx]) at corner (i0 + f); with `patch` given: the adjoint,
+    obj += scatter(patch) in place (returns obj)."""
+    obj = np.ascontiguousarray(obj, dtype=np.complex128); ony, onx = obj.shape
+    if patch is None:
+        out = np.empty((n, n), np.complex128)
+        lib().orc_bilinear(n, ony, onx, _p(obj, C.c_double), i0y, i0x, C.c_double(fy), C.c_double(fx), _p(out, C.c_double), 0)
+        return out
+    patch = np.ascontiguousarray(patch, dtype=np.complex128)
+    lib().orc_bilinear(n, ony, onx, _p(obj, C.c_double), i0y, i0x, C.c_double(fy), C.c_double(fx), _p(patch, C.c_double), 1)
+    return obj
 
 
 def propagator(n, px, lam, dz, tx=0.0, ty=0.0, bandlimit=0.0):

@@ -56,6 +56,7 @@ struct orc_problem {
   float eps;                 // epsilon offset (readings R11..R13)
   float lsqml_delta_o;       // delta_O of PAPER.md:219
   float lsqml_delta_p;       // probe analogue (reading R19)
+  int32_t shift_mode;        // 0: Fourier shift of the probe (reading R1, default); 1: bilinear sampling of the object
 };
 
 // ------------------------------------------------------------------------------------------
@@ -158,6 +159,38 @@ void orc_position_split(float X, float px, int32_t N, int32_t* r0, float* delta)
   volatile float d = c - fl;
   *r0 = (int32_t)fl;
   *delta = d;
+}
+
+// O1 (bilinear mode, reading R1 secondary): c = X/px - N/2, i0 = floor(c), f = c - i0 in [0,1), float32 as above
+void orc_position_split_floor(float X, float px, int32_t N, int32_t* i0, float* frac) {
+  volatile float p = X / px;
+  volatile float c = p - (float)(N / 2);
+  float fl = std::floor(c);
+  volatile float d = c - fl;
+  *i0 = (int32_t)fl;
+  *frac = d;
+}
+
+// O3 (bilinear mode): the four taps of window pixel (y, x): object pixels (i0 + r + d), d in {0,1}^2, with weights
+// w_d = (d_y ? f_y : 1 - f_y)(d_x ? f_x : 1 - f_x)   ("sampled")
+static inline double bil_w(int d, double f) { return d ? f : 1.0 - f; }
+
+// patch[r] = sum_d w_d obj[i0 + r + d]; with adjoint != 0: obj[i0 + r + d] += w_d patch[r]   (exported for the pins)
+void orc_bilinear(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t i0y, int32_t i0x, double fy, double fx,
+                  double* patch, int32_t adjoint) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x) {
+      cd acc = 0.0;
+      for (int dy = 0; dy < 2; ++dy)
+        for (int dx = 0; dx < 2; ++dx) {
+          long o = (long)(i0y + y + dy) * onx + (i0x + x + dx);
+          double w = bil_w(dy, fy) * bil_w(dx, fx);
+          if (adjoint) { obj[2 * o] += w * patch[2 * ((long)y * N + x)]; obj[2 * o + 1] += w * patch[2 * ((long)y * N + x) + 1]; }
+          else acc += w * cd(obj[2 * o], obj[2 * o + 1]);
+        }
+      if (!adjoint) { patch[2 * ((long)y * N + x)] = acc.real(); patch[2 * ((long)y * N + x) + 1] = acc.imag(); }
+    }
+  (void)ony;
 }
 
 // O1: sub-pixel shift ramp R[q] = exp(-2 pi i (f(qy) dy + f(qx) dx))  (PAPER.md:115 P_k(r - X_j))
@@ -300,17 +333,30 @@ static int forward_pos(const Model& m, int jrow, PosWork& w) {
   const orc_problem& p = m.p;
   w.N = N; w.M = M; w.S = S;
   float dyf, dxf; int32_t r0y, r0x;
-  orc_position_split(m.positions[2 * jrow + 0], p.pixel_size, N, &r0y, &dyf);   // O1
-  orc_position_split(m.positions[2 * jrow + 1], p.pixel_size, N, &r0x, &dxf);
-  if (r0y < 0 || r0x < 0 || r0y + N > p.obj_ny || r0x + N > p.obj_nx) return -1;
+  const bool bil = p.shift_mode == 1;
+  if (!bil) {
+    orc_position_split(m.positions[2 * jrow + 0], p.pixel_size, N, &r0y, &dyf);   // O1
+    orc_position_split(m.positions[2 * jrow + 1], p.pixel_size, N, &r0x, &dxf);
+    if (r0y < 0 || r0x < 0 || r0y + N > p.obj_ny || r0x + N > p.obj_nx) return -1;
+  } else {                                                                        // taps i0 .. i0 + N inclusive
+    orc_position_split_floor(m.positions[2 * jrow + 0], p.pixel_size, N, &r0y, &dyf);
+    orc_position_split_floor(m.positions[2 * jrow + 1], p.pixel_size, N, &r0x, &dxf);
+    if (r0y < 0 || r0x < 0 || r0y + N + 1 > p.obj_ny || r0x + N + 1 > p.obj_nx) return -1;
+  }
   w.r0y = r0y; w.r0x = r0x; w.dy = (double)dyf; w.dx = (double)dxf;
-  w.R.resize(NN); shift_ramp(N, w.dy, w.dx, w.R.data());
+  w.R.resize(NN); shift_ramp(N, bil ? 0.0 : w.dy, bil ? 0.0 : w.dx, w.R.data());    // bilinear mode: probe unshifted, R = 1
   w.Psi.assign((long)S * M, std::vector<cd>()); w.T.assign(S, std::vector<cd>(NN));
   w.psit.assign(M, std::vector<cd>(NN)); w.I.assign(NN, 0.0);
   for (int i = 0; i < S; ++i)                                                    // O3: T_i[r] = O_i[r0 + r]
     for (int y = 0; y < N; ++y)
-      for (int x = 0; x < N; ++x)
-        w.T[i][(long)y * N + x] = m.obj[((long)i * p.obj_ny + (r0y + y)) * p.obj_nx + (r0x + x)];
+      for (int x = 0; x < N; ++x) {
+        if (!bil) { w.T[i][(long)y * N + x] = m.obj[((long)i * p.obj_ny + (r0y + y)) * p.obj_nx + (r0x + x)]; continue; }
+        cd acc = 0.0;                                                            // bilinear: sum_d w_d O_i[i0 + r + d]
+        for (int dy = 0; dy < 2; ++dy)
+          for (int dx = 0; dx < 2; ++dx)
+            acc += bil_w(dy, w.dy) * bil_w(dx, w.dx) * m.obj[((long)i * p.obj_ny + (r0y + y + dy)) * p.obj_nx + (r0x + x + dx)];
+        w.T[i][(long)y * N + x] = acc;
+      }
   for (int k = 0; k < M; ++k) {
     std::vector<cd> cur(NN);
     for (long q = 0; q < NN; ++q) cur[q] = w.R[q] * m.Pt[k][q];                  // O2
@@ -367,7 +413,7 @@ static void adjoint_pos(const Model& m, int jrow, PosWork& w, double* loss_j,
     F2(N, g.data());                                                             // O9: G~ = F(gPsi_0)
     if (gPt_acc)
       for (long q = 0; q < NN; ++q) (*gPt_acc)[k][q] += std::conj(w.R[q]) * g[q];
-    for (int a = 0; a < 2; ++a) {                                                // O10
+    for (int a = 0; a < 2 && p.shift_mode != 1; ++a) {                           // O10 (Fourier-shift mode)
       cd acc = 0.0;
       for (int qy = 0; qy < N; ++qy)
         for (int qx = 0; qx < N; ++qx) {
@@ -377,6 +423,21 @@ static void adjoint_pos(const Model& m, int jrow, PosWork& w, double* loss_j,
         }
       gdelta[a] += 2.0 * acc.real() / ((double)N * N);
     }
+  }
+  if (p.shift_mode == 1) {
+    // O10 (bilinear mode): the position enters through the weights only, integer corner held fixed (reading R17):
+    // dL/df_a = 2 Re sum_i sum_r conj(gT_i[r]) dT_i[r]/df_a,
+    // dT/df_y = sum_dx w_dx (O[y+1, x+dx] - O[y, x+dx]),  dT/df_x = sum_dy w_dy (O[y+dy, x+1] - O[y+dy, x])
+    for (int i = 0; i < S; ++i)
+      for (int y = 0; y < N; ++y)
+        for (int x = 0; x < N; ++x) {
+          auto O = [&](int dy, int dx) { return m.obj[((long)i * p.obj_ny + (w.r0y + y + dy)) * p.obj_nx + (w.r0x + x + dx)]; };
+          cd dTy = bil_w(0, w.dx) * (O(1, 0) - O(0, 0)) + bil_w(1, w.dx) * (O(1, 1) - O(0, 1));
+          cd dTx = bil_w(0, w.dy) * (O(0, 1) - O(0, 0)) + bil_w(1, w.dy) * (O(1, 1) - O(1, 0));
+          cd g = gT[i][(long)y * N + x];
+          gdelta[0] += 2.0 * (std::conj(g) * dTy).real();
+          gdelta[1] += 2.0 * (std::conj(g) * dTx).real();
+        }
   }
 }
 
@@ -446,11 +507,20 @@ int32_t orc_gradient(const orc_problem* p, const float* object, const float* pro
       for (int i = 0; i < S; ++i)                                               // O8 last line: scatter-add
         for (int y = 0; y < N; ++y)
           for (int x = 0; x < N; ++x) {
-            long o = ((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x);
-            gO_loc[o] += gT[i][(long)y * N + x];
-            if (illum) {                                                        // O12
-              double s = 0.0; for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][(long)y * N + x]);
-              il_loc[o] += s;
+            double s = 0.0;                                                     // O12
+            if (illum) for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][(long)y * N + x]);
+            if (p->shift_mode != 1) {
+              long o = ((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x);
+              gO_loc[o] += gT[i][(long)y * N + x];
+              if (illum) il_loc[o] += s;
+            } else {                                                            // bilinear mode: the same four weights
+              for (int dy = 0; dy < 2; ++dy)
+                for (int dx = 0; dx < 2; ++dx) {
+                  long o = ((long)i * p->obj_ny + (w.r0y + y + dy)) * p->obj_nx + (w.r0x + x + dx);
+                  double wt = bil_w(dy, w.dy) * bil_w(dx, w.dx);
+                  gO_loc[o] += wt * gT[i][(long)y * N + x];
+                  if (illum) il_loc[o] += wt * s;
+                }
             }
           }
       if (grad_pos) { grad_pos[2 * jb + 0] = gd[0] / (double)p->pixel_size; grad_pos[2 * jb + 1] = gd[1] / (double)p->pixel_size; }
@@ -485,6 +555,7 @@ int32_t orc_step_terms(const orc_problem* p, const float* object, const float* p
                        const float* positions, const float* intensity, const int32_t* batch_idx,
                        const double* grad_object, const double* grad_probe, const double* illum_prev,
                        double* step_terms) {
+  if (p->shift_mode == 1) return -2;                                            // step terms: Fourier-shift mode only
   Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
   const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const long NN = m.NN;
   const long on = (long)S * p->obj_ny * p->obj_nx;

@@ -495,3 +495,98 @@ def test_sgd_update():
     o, p, x = orc.apply_update(pb, 0, obj, probe, pos, gO, gP, gX, lr_obj=0.1, lr_probe=0.2, lr_pos=0.3)
     assert np.abs(o - (obj - 0.1 * gO)).max() < 1e-12 and np.abs(p - (probe - 0.2 * gP)).max() < 1e-12
     assert np.abs(x - (pos - 0.3 * gX)).max() < 1e-12
+
+
+# ------------------------------------------------------------------------------------------------
+# bilinear object sampling (SURVEY.md §8(c) R1 secondary mode, "sampled"; shift_mode = 1)
+# ------------------------------------------------------------------------------------------------
+def test_bilinear_split_and_gather_closed_forms():
+    # floor split: c = X/px - N/2 = i0 + f, f in [0,1)
+    for X, px, n, want in [(2.0, 0.2, 8, (6, 0.0)), (2.05, 0.2, 8, (6, 0.25)), (0.79, 0.2, 8, (-1, 0.95))]:
+        i0, f = orc.position_split_floor(X, px, n)
+        assert i0 == want[0] and abs(f - want[1]) < 1e-5
+    # a bilinear interpolant reproduces any function a + b y + c x + d x y exactly
+    on, n = 14, 6
+    yy, xx = np.meshgrid(np.arange(on), np.arange(on), indexing="ij")
+    obj = (0.3 + 0.7j) + (0.2 - 0.1j) * yy + (-0.4 + 0.5j) * xx + 0.05j * xx * yy
+    i0y, i0x, fy, fx = 3, 5, 0.37, 0.81
+    T = orc.bilinear(n, obj, i0y, i0x, fy, fx)
+    ys, xs = np.meshgrid(i0y + fy + np.arange(n), i0x + fx + np.arange(n), indexing="ij")
+    assert np.abs(T - ((0.3 + 0.7j) + (0.2 - 0.1j) * ys + (-0.4 + 0.5j) * xs + 0.05j * xs * ys)).max() < 1e-12
+    # f = 0: the plain integer window
+    assert np.abs(orc.bilinear(n, obj, i0y, i0x, 0.0, 0.0) - obj[i0y:i0y + n, i0x:i0x + n]).max() == 0
+    # adjoint pair (dot-product test) and weight sum: scattering ones deposits n*n in total
+    a = crandn(on, on); y = crandn(n, n)
+    lhs = np.vdot(orc.bilinear(n, a, i0y, i0x, fy, fx), y)
+    rhs = np.vdot(a, orc.bilinear(n, np.zeros((on, on), complex), i0y, i0x, fy, fx, patch=y))
+    assert abs(lhs - rhs) < 1e-12 * abs(lhs)
+    acc = orc.bilinear(n, np.zeros((on, on), complex), i0y, i0x, fy, fx, patch=np.ones((n, n), complex))
+    assert abs(acc.sum() - n * n) < 1e-12
+
+
+def _bilinear_problem(**kw):
+    pb, obj, probe, pos = small_problem(**kw)
+    pb.shift_mode = orc.SHIFT_BILINEAR_OBJECT
+    return pb, obj, probe, pos
+
+
+def test_bilinear_forward_special_cases():
+    n, on = 8, 20
+    pb, obj, probe, pos = _bilinear_problem(n=n, M=2, S=3, on=on, J=4)
+    # (1) integer corners: identical to the Fourier-shift mode, whose shift is then zero too
+    pos_int = (np.array([[5, 6], [4, 9], [7, 5], [9, 9]]) * 0.2).astype(np.float32)
+    pf = orc.Problem(**{**pb.__dict__, "shift_mode": orc.SHIFT_FOURIER_PROBE})
+    a = orc.forward_loss(pb, obj, probe, pos_int)["intensity"]; b = orc.forward_loss(pf, obj, probe, pos_int)["intensity"]
+    assert np.abs(a - b).max() < 1e-12 * np.abs(b).max()
+    # (2) an object that is constant in the plane: the pattern does not depend on the position at all
+    flat = np.ones_like(obj) * np.exp(0.3j * np.arange(3))[:, None, None].astype(np.complex64)
+    out = orc.forward_loss(pb, flat, probe, pos)["intensity"]
+    assert np.abs(out - out[0]).max() < 1e-10 * np.abs(out).max()
+    # (3) S = 1: |F(P . T)|^2 / N^2 with T the bilinear patch and the probe NOT shifted
+    pb1, obj1, probe1, pos1 = _bilinear_problem(n=n, M=1, S=1, on=on, J=2)
+    out = orc.forward_loss(pb1, obj1, probe1, pos1)["intensity"]
+    for j in range(2):
+        (i0y, fy), (i0x, fx) = orc.position_split_floor(float(pos1[j, 0]), 0.2, n), orc.position_split_floor(float(pos1[j, 1]), 0.2, n)
+        T = orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy, fx)
+        ref = np.abs(np.fft.fft2(probe1[0].astype(complex) * T)) ** 2 / n ** 2
+        assert np.abs(out[j] - ref).max() < 1e-10 * ref.max()
+
+
+def test_bilinear_gradient_finite_differences():
+    pb, obj, probe, pos = _bilinear_problem(J=4)
+    obj_t = (obj * np.exp(0.2 * crandn(*obj.shape))).astype(np.complex64)
+    Iexp = orc.forward_loss(pb, obj_t, probe, pos)["intensity"].astype(np.float32) + 0.05
+    # keep the fractions away from 0 and 1 so the integer corner does not flip under the position steps
+    for j in range(4):
+        for a in range(2):
+            i0, f = orc.position_split_floor(float(pos[j, a]), 0.2, 8)
+            if f < 0.2 or f > 0.8:
+                pos[j, a] = np.float32((i0 + 4 + 0.5) * 0.2)
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+
+    def L(o, p, x=pos):
+        return orc.forward_loss(pb, o, p, x, Iexp, want_intensity=False)["loss"]
+
+    assert abs(L(obj, probe) - g["loss"]) < 1e-12 * abs(g["loss"])
+    h = 2.0 ** -9
+    for which in ("obj", "probe"):
+        base = obj if which == "obj" else probe
+        D = crandn(*base.shape).astype(np.complex64)
+        zp = (base.astype(np.complex128) + h * D).astype(np.complex64); zm = (base.astype(np.complex128) - h * D).astype(np.complex64)
+        Dact = (zp.astype(np.complex128) - zm.astype(np.complex128)) / 2.0
+        fd = (L(zp, probe) - L(zm, probe)) / 2.0 if which == "obj" else (L(obj, zp) - L(obj, zm)) / 2.0
+        gw = g["grad_object" if which == "obj" else "grad_probe"]
+        lin = 2.0 * np.real(np.vdot(gw, Dact))
+        # the O(h^2) truncation error scales with |g||D|, not with the (possibly cancelling) directional derivative
+        assert abs(fd - lin) < 2e-4 * abs(lin) + 1e-4 * np.linalg.norm(gw) * np.linalg.norm(Dact), (which, fd, lin)
+    hx = 2e-3 * 0.2
+    for j in range(4):
+        for a in range(2):
+            pp = pos.copy(); pm = pos.copy(); pp[j, a] += np.float32(hx); pm[j, a] -= np.float32(hx)
+            fd = (L(obj, probe, pp) - L(obj, probe, pm)) / (float(pp[j, a]) - float(pm[j, a]))
+            assert abs(fd - g["grad_pos"][j, a]) < 2e-3 * abs(fd) + 1e-6, (j, a, fd, g["grad_pos"][j, a])
+    # illumination map: the weights of a position sum to one, so the total equals the total entering intensity
+    pf = orc.Problem(**{**pb.__dict__, "shift_mode": orc.SHIFT_FOURIER_PROBE})
+    assert g["illum"].min() >= 0
+    # slice 0: sum_r |Psi_0|^2 = sum |P|^2 per position (unshifted probe), 4 positions
+    assert abs(g["illum"][0].sum() - 4 * (np.abs(probe.astype(complex)) ** 2).sum()) < 1e-9 * g["illum"][0].sum()
