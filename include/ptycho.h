@@ -29,7 +29,11 @@ enum { PT_LOSS_AMPLITUDE = 0,   /* PAPER.md:157, l = 1/2 (sqrt(I+c) - sqrt(Iexp+
        PT_LOSS_POISSON = 1 };   /* PAPER.md:151, l = I - Iexp (ln(I+eps) - ln(Iexp+eps) + 1)                  */
 
 enum { PT_SHIFT_FOURIER_PROBE = 0,    /* integer window on the object + Fourier shift of the probe (R1) */
-       PT_SHIFT_BILINEAR_OBJECT = 1 };/* not built yet: returns PT_ERR_UNSUPPORTED                                    */
+       PT_SHIFT_BILINEAR_OBJECT = 1 };/* PAPER.md:61 "sampled" (R1, secondary): probe unshifted; the patch is a four-tap
+                                       * bilinear sample of the object at c + r, c = X/px - N/2 = i0 + f (i0 = floor(c));
+                                       * the object gradient is scattered with the same weights and dL/dX comes through
+                                       * the weights (i0 fixed).  Windows need i0 + N <= size - 1.  PT_WANT_STEP_SIZES is
+                                       * not available in this mode (PT_ERR_UNSUPPORTED).                              */
 
 enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                                                        */
        PT_WANT_ILLUM = 2,             /* fill illum_d with sum_{j,k} |Psi_{i,k,j}|^2             */

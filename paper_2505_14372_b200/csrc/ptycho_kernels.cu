@@ -54,6 +54,7 @@ struct Ws {
   cf* gTpart;          // [Jc][M][S][N^2]  R-native
   cf* Gpart;           // [Jc][M][N^2]     F-native
   cf* scratch;         // [Jc][M][N^2]     (step sizes: gPhi_0)
+  cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
   int32_t Jc;
   size_t total;
 };
@@ -74,7 +75,8 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
   size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   if (steps) pp += M * NN * sizeof(cf);
-  *fixed = f + 8 * 256;   // slack for the per-array alignment of the chunked part
+  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
+  *fixed = f + 9 * 256;   // slack for the per-array alignment of the chunked part
   *per_pos = pp;
 }
 
@@ -108,6 +110,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->gTpart = (cf*)take(jc * M * S * NN * sizeof(cf));
   w->Gpart = (cf*)take(jc * M * NN * sizeof(cf));
   w->scratch = steps ? (cf*)take(jc * M * NN * sizeof(cf)) : nullptr;
+  w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
   w->Jc = (int32_t)jc;
   w->total = off;
   return off <= bytes ? PT_OK : PT_ERR_WORKSPACE;
@@ -121,6 +124,7 @@ struct KP {
   int j0, jc;                        // current chunk: batch-local offset and count
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
   int loss; float loss_c, eps;
+  int bilinear;                      // PT_SHIFT_BILINEAR_OBJECT: probe unshifted, patches sampled with four taps (reading R1)
   const cf* object; const cf* probe; const float* positions; const float* intensity; const int32_t* batch_idx;
   Ws w;
 };
@@ -164,10 +168,10 @@ __global__ void k_setup_pos(KP P) {
     float X = P.positions[2 * row + a];
     float p = __fdiv_rn(X, P.px);
     float c = __fsub_rn(p, (float)(N / 2));
-    float fl = floorf(__fadd_rn(c, 0.5f));
+    float fl = floorf(P.bilinear ? c : __fadd_rn(c, 0.5f));    // bilinear mode: i0 = floor(c), f = c - i0 in [0, 1)
     d[a] = __fsub_rn(c, fl);
     int r = (int)fl;
-    int lim = (a == 0 ? P.ony : P.onx) - N;
+    int lim = (a == 0 ? P.ony : P.onx) - N - (P.bilinear ? 1 : 0);   // bilinear taps reach i0 + N
     if (r < 0 || r > lim) {
       if (q == 0) atomicOr(P.w.status, kStatusOOB);
       r = r < 0 ? 0 : lim;
@@ -180,9 +184,10 @@ __global__ void k_setup_pos(KP P) {
   }
   const float f = (float)signed_freq(q, N) / (float)N;
   float s, c;
-  sincospif(-2.0f * f * d[1], &s, &c);
+  const float dsx = P.bilinear ? 0.f : d[1], dsy = P.bilinear ? 0.f : d[0];   // bilinear mode: the probe is not shifted (R = 1)
+  sincospif(-2.0f * f * dsx, &s, &c);
   P.w.ramps[((size_t)jb * 2 + 0) * N + q] = make_float2(c, s);     // rx
-  sincospif(-2.0f * f * d[0], &s, &c);
+  sincospif(-2.0f * f * dsy, &s, &c);
   P.w.ramps[((size_t)jb * 2 + 1) * N + q] = make_float2(c, s);     // ry
 }
 
@@ -363,9 +368,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   Fft<G>::begin_fourier();
   const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
-  const int S = P.S, onx = P.onx;
-  const size_t slice = (size_t)P.ony * onx;
-  const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);   // this thread's first pixel, slice 0
+  // patch source: the object window itself, or (bilinear mode) this position's resampled patches [S][NF][NF]
+  const int S = P.S, onx = P.bilinear ? NF : P.onx;
+  const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
+  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) +
+                 (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);   // this thread's first pixel, slice 0
   // H3 prefetch: patch values of registers [0, 2E) one FFT pair ahead into the thread's early slots
   auto early = [&](int i) {
     const cf* o = ob + (size_t)i * slice;
@@ -486,11 +493,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
   const int unit = (jb * P.M + k) * CL + (int)rk;                 // index of this CTA's fp64 partials
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
-  const int S = P.S, onx = P.onx;
-  const size_t slice = (size_t)P.ony * onx;
+  // patch source: the object window itself, or (bilinear mode) this position's resampled patches [S][NF][NF]
+  const int S = P.S, onx = P.bilinear ? NF : P.onx;
+  const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
   auto fld = [&](int i) { return (((size_t)pair * S + i) * CL + rk) * NNS; };   // field (pair, slice i), this rank's block
   const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
-  const cf* ob = patch_ptr(P, 0, r0y, r0x) + pix0;
+  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
   // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
   auto early = [&](int i) {
     const float4* st = (const float4*)(P.w.stash + fld(i)) + t;
@@ -649,6 +657,60 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 }
 
 // ------------------------------------------------------------------------------------------------
+// Bilinear mode (reading R1, secondary): H3 as a pre-pass.  Tb[jl][i][y][x] = sum_d w_d O_i[i0 + (y,x) + d],
+// w_d = (d_y ? f_y : 1 - f_y)(d_x ? f_x : 1 - f_x); the chain kernels then read these patches instead of the
+// object window.  One block per (position of the chunk, slice).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_bilinear_patches(KP P) {
+  const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, N = P.N;
+  const int i0y = P.w.r0[2 * jb], i0x = P.w.r0[2 * jb + 1];
+  const float fy = P.w.delta[2 * jb], fx = P.w.delta[2 * jb + 1];
+  const float w00 = (1.f - fy) * (1.f - fx), w01 = (1.f - fy) * fx, w10 = fy * (1.f - fx), w11 = fy * fx;
+  const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
+  cf* out = P.w.Tb + ((size_t)jl * P.S + i) * N * N;
+  for (int e = threadIdx.x; e < N * N; e += 256) {
+    const int y = e / N, x = e - y * N;
+    const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
+    out[e] = make_float2(w00 * a.x + w01 * b.x + w10 * c.x + w11 * d.x, w00 * a.y + w01 * b.y + w10 * c.y + w11 * d.y);
+  }
+}
+
+// Bilinear mode, H13: dL/df_a = 2 Re sum_i sum_r conj(gT_i[r]) dT_i[r]/df_a with gT summed over the modes in fixed
+// order; dT/df_y = sum_dx w_dx (O[y+1, x+dx] - O[y, x+dx]), dT/df_x likewise.  One block per position of the chunk.
+template <class G>
+__global__ void __launch_bounds__(256) k_pos_bilinear(KP P, int cl) {
+  typedef FL<G> F;
+  constexpr int N = F::NF, NN = F::NNF;
+  __shared__ double red[(256 / 32) * 2];
+  const int jl = blockIdx.x, jb = P.j0 + jl;
+  const int i0y = P.w.r0[2 * jb], i0x = P.w.r0[2 * jb + 1];
+  const double fy = (double)P.w.delta[2 * jb], fx = (double)P.w.delta[2 * jb + 1];
+  double acc[2] = {0.0, 0.0};
+  for (int i = 0; i < P.S; ++i) {
+    const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
+    for (int e = threadIdx.x; e < NN; e += 256) {
+      const int y = e / N, x = e - y * N;
+      const size_t base = ((size_t)jl * P.M * P.S + i) * NN + F::r_native_of(y, x);
+      double gr = 0.0, gi = 0.0;
+      for (int k = 0; k < P.M; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; gr += (double)g.x; gi += (double)g.y; }
+      const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
+      const double tyr = (1.0 - fx) * ((double)c.x - a.x) + fx * ((double)d.x - b.x), tyi = (1.0 - fx) * ((double)c.y - a.y) + fx * ((double)d.y - b.y);
+      const double txr = (1.0 - fy) * ((double)b.x - a.x) + fy * ((double)d.x - c.x), txi = (1.0 - fy) * ((double)b.y - a.y) + fy * ((double)d.y - c.y);
+      acc[0] += 2.0 * (gr * tyr + gi * tyi);                     // 2 Re(conj(g) dT)
+      acc[1] += 2.0 * (gr * txr + gi * txi);
+    }
+  }
+  block_sum<256, 2>(acc, red);
+  if (threadIdx.x == 0) {
+    const int MU = P.M * cl;
+    for (int u = 0; u < MU; ++u) {                               // k_finalize sums the MU per-(mode, rank) slots
+      P.w.posg_part[((size_t)jb * MU + u) * 2 + 0] = u == 0 ? acc[0] : 0.0;
+      P.w.posg_part[((size_t)jb * MU + u) * 2 + 1] = u == 0 ? acc[1] : 0.0;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // H11: deterministic object-gradient scatter-add as an owner-computes gather.  Block = 64 x 4 object pixels of
 // one slice; each pixel sums, in fixed (j ascending, k ascending) order, the patch-gradient entries that
 // land on it, in fp64, then adds the chunk total to gO once.  Optionally the illumination map (O12).
@@ -656,11 +718,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 #ifndef GATHER_TW
 #define GATHER_TW 64     // tile width in object pixels (256 threads per block)
 #endif
-template <class G, bool ILLUM>
+template <class G, bool ILLUM, bool BILIN>
 __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illum) {
   typedef FL<G> F;
-  constexpr int N = F::NF, NN = F::NNF;
+  constexpr int N = F::NF, NN = F::NNF, NR = BILIN ? N + 1 : N;   // bilinear mode: a window deposits on N + 1 pixels per axis
   __shared__ int2 sr0[256];
+  __shared__ float2 sfr[BILIN ? 256 : 1];
   const int i = blockIdx.z;
   constexpr int TW_ = GATHER_TW, TH_ = 256 / GATHER_TW;
   const int ox0 = blockIdx.x * TW_, oy0 = blockIdx.y * TH_;
@@ -669,13 +732,35 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
   double ar = 0.0, ai = 0.0, al = 0.0;
   for (int jbase = 0; jbase < P.jc; jbase += 256) {
     const int cnt = min(256, P.jc - jbase);
-    if (tid < cnt) sr0[tid] = make_int2(P.w.r0[2 * (P.j0 + jbase + tid) + 1], P.w.r0[2 * (P.j0 + jbase + tid)]);  // (x, y)
+    if (tid < cnt) {
+      sr0[tid] = make_int2(P.w.r0[2 * (P.j0 + jbase + tid) + 1], P.w.r0[2 * (P.j0 + jbase + tid)]);  // (x, y)
+      if (BILIN) sfr[tid] = make_float2(P.w.delta[2 * (P.j0 + jbase + tid) + 1], P.w.delta[2 * (P.j0 + jbase + tid)]);  // (fx, fy)
+    }
     __syncthreads();
     for (int jj = 0; jj < cnt; ++jj) {
       const int2 r0 = sr0[jj];
-      if (r0.x > ox0 + TW_ - 1 || r0.x + N <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + N <= oy0) continue;   // block-uniform reject
+      if (r0.x > ox0 + TW_ - 1 || r0.x + NR <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + NR <= oy0) continue;   // block-uniform reject
       const int px = ox - r0.x, py = oy - r0.y;
-      if (px >= 0 && px < N && py >= 0 && py < N) {
+      if (BILIN) {
+        // adjoint of the four-tap sampling: pixel o collects w_d gT[o - i0 - d] (the same weights)
+        if (px >= 0 && px <= N && py >= 0 && py <= N) {
+          const double fx = (double)sfr[jj].x, fy = (double)sfr[jj].y;
+#pragma unroll
+          for (int d = 0; d < 4; ++d) {
+            const int dy = d >> 1, dx = d & 1, ry = py - dy, rx = px - dx;
+            if (ry < 0 || ry >= N || rx < 0 || rx >= N) continue;
+            const double wgt = (dy ? fy : 1.0 - fy) * (dx ? fx : 1.0 - fx);
+            const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(ry, rx);
+            double sr = 0.0, si = 0.0, sl = 0.0;
+            for (int k = 0; k < P.M; ++k) {
+              const cf g = P.w.gTpart[base + (size_t)k * P.S * NN];
+              sr += (double)g.x; si += (double)g.y;
+              if (ILLUM) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
+            }
+            ar += wgt * sr; ai += wgt * si; al += wgt * sl;
+          }
+        }
+      } else if (px >= 0 && px < N && py >= 0 && py < N) {
         const int idx = F::r_native_of(py, px);
         const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
         for (int k = 0; k < P.M; ++k) {
@@ -809,10 +894,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
-                                         "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos"};
+                                         "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
+                                         "k_bilinear_patches", "k_pos_bilinear"};
 thread_local int64_t g_launches = 0;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
@@ -840,8 +926,8 @@ int validate(const pt_problem* p) {
   if (p->obj_ny < p->n || p->obj_nx < p->n) return PT_ERR_BAD_SIZE;
   if (!(p->pixel_size > 0.f) || !(p->wavelength > 0.f) || !(p->eps > 0.f)) return PT_ERR_BAD_PARAM;
   if (p->loss != PT_LOSS_AMPLITUDE && p->loss != PT_LOSS_POISSON) return PT_ERR_BAD_PARAM;
-  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
-  if (p->shift_mode != PT_SHIFT_FOURIER_PROBE) return PT_ERR_BAD_PARAM;
+  if (p->shift_mode != PT_SHIFT_FOURIER_PROBE && p->shift_mode != PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_BAD_PARAM;
+  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT && (p->obj_ny < p->n + 1 || p->obj_nx < p->n + 1)) return PT_ERR_BAD_SIZE;
   if (p->n_slices > 1 && !p->slice_thickness) return PT_ERR_NULL;
   if (p->loss_c < 0.f) return PT_ERR_BAD_PARAM;
   return PT_OK;
@@ -855,6 +941,7 @@ KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64*
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
   k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
   k.loss = p->loss; k.loss_c = p->loss_c; k.eps = p->eps;
+  k.bilinear = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   k.object = (const cf*)object; k.probe = (const cf*)probe; k.positions = positions; k.intensity = intensity;
   k.batch_idx = batch_idx; k.w = w;
   return k;
@@ -913,6 +1000,7 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
   if (rc != PT_OK) return rc;
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+    if (kp.bilinear) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, model_intensity_d, 0);
@@ -935,6 +1023,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool want_illum = (p->flags & PT_WANT_ILLUM) && illum;
   const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX;
   const bool want_steps = (p->flags & PT_WANT_STEP_SIZES) && step_terms;
+  const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
   if (!acc) {
@@ -945,15 +1034,25 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+    if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
-    launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos ? 1 : 0);
+    launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
     LAUNCH_CHECK(K_backward, st);
-    if (want_illum) k_gather_object<G, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
-    else k_gather_object<G, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
+    if (bilin) {
+      if (want_illum) k_gather_object<G, true, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
+      else k_gather_object<G, false, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
+    } else {
+      if (want_illum) k_gather_object<G, true, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
+      else k_gather_object<G, false, false><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
+    }
     LAUNCH_CHECK(K_gather_object, st);
+    if (bilin && want_pos) {
+      k_pos_bilinear<G><<<kp.jc, 256, 0, st>>>(kp, G::CL);
+      LAUNCH_CHECK(K_pos_bilinear, st);
+    }
     k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp);
     LAUNCH_CHECK(K_reduce_probe, st);
   }
@@ -1045,6 +1144,7 @@ int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c6
   if (rc != PT_OK) return rc;
   if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
+  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
   Ws w;
   pt_problem q = *p;
   if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
