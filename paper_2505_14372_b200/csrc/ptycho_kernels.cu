@@ -410,7 +410,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     float4* st = (float4*)(P.w.stash + (((size_t)pair * S + i) * CL + rk) * NNS);
 #pragma unroll
     for (int p = 0; p < 16; ++p) {                               // stash Psi_i ; H3+H4: Phi = Psi .* T_i
-      if (STASH) st[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
+      if (STASH) __stcs(st + p * T + t, make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y));
       const cf T0 = p < E ? cs.pf8[(2 * p) * T] : cs.xs8[(2 * p - 2 * E) * 32];
       const cf T1 = p < E ? cs.pf8[(2 * p + 1) * T] : cs.xs8[(2 * p + 1 - 2 * E) * 32];
       v[2 * p] = cmul(v[2 * p], T0);
@@ -547,7 +547,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
         else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
         const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
-        gt[p * T + t] = make_float4(g0.x, g0.y, g1.x, g1.y);    // H10: gT_i contribution conj(Psi) .* gPhi
+        __stcs(gt + p * T + t, make_float4(g0.x, g0.y, g1.x, g1.y));    // H10: gT_i contribution conj(Psi) .* gPhi
         v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
         v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
       }
