@@ -330,6 +330,17 @@ def run_b200(args):
         roof.update(achieved=ach, frac=ach / fp32_peak, nominal_flops_per_launch=fl * units_per_launch,
                     hbm_view={"achieved": achb, "peak": hbm, "unit": "GB/s", "frac": achb / hbm, "peak_source": which,
                               "algorithmic_bytes_per_launch": ab * units_per_launch})
+    # traffic: DRAM bytes of one launch of that kernel from the committed `ncu --set full` capture (profiles/), scaled to
+    # this run's positions per launch; null if the capture is of another kernel or workload
+    try:
+        import csv
+        with open(os.path.join(ROOT, "profiles", "r1d_dominant_kernel_traffic.csv")) as f:
+            tr = next(csv.DictReader(f))
+        if tr["kernel"] == top and tr["workload"] == conf["workload"]:
+            roof["traffic"] = (float(tr["dram_bytes_read"]) + float(tr["dram_bytes_write"])) * units_per_launch / float(tr["positions_per_launch"])
+            roof["traffic_source"] = tr["source"]
+    except (OSError, KeyError, ValueError, StopIteration):
+        pass
     # whole-step view against both roofs of SURVEY §8(d): the io+act byte model and nominal FFT flops on the FP32 ALUs
     rate = J / (ms_step * 1e-3)
     b_model = 2 * cfg.n_modes * cfg.n_slices * cfg.n * cfg.n * 8 + cfg.n * cfg.n * 4
