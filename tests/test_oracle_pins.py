@@ -590,3 +590,24 @@ def test_bilinear_gradient_finite_differences():
     assert g["illum"].min() >= 0
     # slice 0: sum_r |Psi_0|^2 = sum |P|^2 per position (unshifted probe), 4 positions
     assert abs(g["illum"][0].sum() - 4 * (np.abs(probe.astype(complex)) ** 2).sum()) < 1e-9 * g["illum"][0].sum()
+
+
+# ------------------------------------------------------------------------------------------------
+# change detector: stored oracle outputs of a tiny seeded case (tests/golden/, written by make_golden.py from oracle/ only)
+# ------------------------------------------------------------------------------------------------
+def test_golden_oracle_tiny_case():
+    import importlib.util
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mg = importlib.util.module_from_spec(spec); spec.loader.exec_module(mg)
+    want = {}
+    for line in open(os.path.join(here, "oracle_tiny_case.txt")):
+        if line.startswith("#"):
+            continue
+        mode, key, val = line.split()
+        want[(mode, key)] = float(val)
+    assert len(want) == 16
+    for mode, name in ((0, "fourier_probe"), (1, "bilinear_object")):
+        for k, v in mg.checksums(mode):
+            assert abs(float(v) - want[(name, k)]) <= 1e-10 * max(abs(want[(name, k)]), 1e-3), (name, k, v, want[(name, k)])
