@@ -70,20 +70,32 @@ PTK_HD cf twiddle32(cf x, int m) {
 }
 
 // in-register DFT of R = 2^k points, natural order in and out.  DIR = -1 forward (exp(-2 pi i ..)), +1 backward.
-// Decimation in frequency, radix 2, constant twiddles; all indices are compile-time after unrolling.
+// Decimation in time, radix 2, constant twiddles; all indices are compile-time after unrolling.  A butterfly with a
+// non-trivial twiddle w is written in FMA form: y0 = e + w o (4 FMA), y1 = 2 e - y0 (2 FMA) — 6 instructions instead of
+// the 8 of "multiply, then add and subtract".
 template <int R, int DIR>
 struct Dft {
   static PTK_HD void run(cf* x) {
     cf e[R / 2], o[R / 2];
 #pragma unroll
-    for (int k = 0; k < R / 2; ++k) {
-      e[k] = cadd(x[k], x[k + R / 2]);
-      o[k] = twiddle32<DIR>(csub(x[k], x[k + R / 2]), k * (32 / R));
-    }
+    for (int k = 0; k < R / 2; ++k) { e[k] = x[2 * k]; o[k] = x[2 * k + 1]; }
     Dft<R / 2, DIR>::run(e);
     Dft<R / 2, DIR>::run(o);
 #pragma unroll
-    for (int k = 0; k < R / 2; ++k) { x[2 * k] = e[k]; x[2 * k + 1] = o[k]; }
+    for (int k = 0; k < R / 2; ++k) {
+      const int m = k * (32 / R);                                 // twiddle exp(DIR 2 pi i m / 32), m < 16
+      if (m == 0) {
+        x[k] = cadd(e[k], o[k]); x[k + R / 2] = csub(e[k], o[k]);
+      } else if (m == 8) {
+        const cf t = DIR > 0 ? make_float2(-o[k].y, o[k].x) : make_float2(o[k].y, -o[k].x);   // (+-i) o
+        x[k] = cadd(e[k], t); x[k + R / 2] = csub(e[k], t);
+      } else {
+        const float c = c32(m), sn = DIR > 0 ? s32(m) : -s32(m);
+        const cf y0 = make_float2(fmaf(-sn, o[k].y, fmaf(c, o[k].x, e[k].x)), fmaf(sn, o[k].x, fmaf(c, o[k].y, e[k].y)));
+        x[k] = y0;
+        x[k + R / 2] = make_float2(fmaf(2.0f, e[k].x, -y0.x), fmaf(2.0f, e[k].y, -y0.y));
+      }
+    }
   }
 };
 template <int DIR>
