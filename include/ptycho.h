@@ -26,7 +26,8 @@ extern "C" {
 typedef struct { float re, im; } pt_c64;
 
 enum { PT_LOSS_AMPLITUDE = 0,   /* PAPER.md:157, l = 1/2 (sqrt(I+c) - sqrt(Iexp+c))^2 ; c = 3/8 gives Anscombe */
-       PT_LOSS_POISSON = 1 };   /* PAPER.md:151, l = I - Iexp (ln(I+eps) - ln(Iexp+eps) + 1)                  */
+       PT_LOSS_POISSON = 1,     /* PAPER.md:151, l = I - Iexp (ln(I+eps) - ln(Iexp+eps) + 1)                  */
+       PT_LOSS_GAUSSIAN = 2 };  /* PAPER.md:144, l = (I - Iexp)^2 / (2 sigma^2), sigma = loss_c > 0           */
 
 enum { PT_SHIFT_FOURIER_PROBE = 0,    /* integer window on the object + Fourier shift of the probe (R1) */
        PT_SHIFT_BILINEAR_OBJECT = 1 };/* PAPER.md:61 "sampled" (R1, secondary): probe unshifted; the patch is a four-tap
@@ -57,7 +58,7 @@ typedef struct {
   float tilt_x_mrad, tilt_y_mrad; /* propagator tilt (R8: exp(+2 pi i dz (kx tan tx + ky tan ty)))*/
   float bandlimit;                /* fraction of Nyquist of the sharp circular mask (R9); <=0 off */
   int32_t loss;                   /* PT_LOSS_*                                                                   */
-  float loss_c;                   /* c of the variance-stabilising transform                     */
+  float loss_c;                   /* c of the variance-stabilising transform; Gaussian: sigma    */
   float eps;                      /* epsilon > 0 (R11..R13)                                       */
   int32_t shift_mode;             /* PT_SHIFT_*                                                                  */
   int32_t flags;                  /* PT_WANT_* | PT_ACCUMULATE                                                   */

@@ -40,7 +40,7 @@ class _Problem(C.Structure):
     ]
 
 
-LOSS_AMPLITUDE, LOSS_POISSON = 0, 1
+LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
 
 _lib = None

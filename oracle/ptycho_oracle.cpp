@@ -51,8 +51,8 @@ struct orc_problem {
   const float* slice_thickness;  // S entries, last unused (reading R10)
   float tilt_x_mrad, tilt_y_mrad;  // propagator tilt (reading R8)
   float bandlimit;           // fraction of Nyquist, <=0: off (reading R9)
-  int32_t loss;              // 0 amplitude, 1 Poisson
-  float loss_c;              // c of the variance-stabilising transform
+  int32_t loss;              // 0 amplitude, 1 Poisson, 2 Gaussian
+  float loss_c;              // c of the variance-stabilising transform; Gaussian: sigma
   float eps;                 // epsilon offset (readings R11..R13)
   float lsqml_delta_o;       // delta_O of PAPER.md:219
   float lsqml_delta_p;       // probe analogue (reading R19)
@@ -272,8 +272,13 @@ void orc_scatter_add(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t r
 // O6: per-pixel loss l(I, Iexp) and detector weight w = dl/dI
 // Poisson (PAPER.md:151 Stirling form, epsilon inside both logarithms — reading R11; w = PAPER.md:165)
 // Amplitude/Anscombe (PAPER.md:157 as printed; w = its derivative regularised as PAPER.md:167 — reading R12)
+// Gaussian: l = (I - Iexp)^2 / (2 sigma^2), normalisation constant dropped as the paper says;
+// sigma is passed in the c slot; w = (I - Iexp) / sigma^2
 void orc_loss_pixel(int32_t kind, double I, double Iexp, double c, double eps, double* l, double* w) {
-  if (kind == 1) {
+  if (kind == 2) {
+    *l = (I - Iexp) * (I - Iexp) / (2.0 * c * c);
+    *w = (I - Iexp) / (c * c);
+  } else if (kind == 1) {
     *l = I - Iexp * (std::log(I + eps) - std::log(Iexp + eps) + 1.0);
     *w = 1.0 - Iexp / (I + eps);
   } else {

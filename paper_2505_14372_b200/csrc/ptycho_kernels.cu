@@ -455,7 +455,10 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int
     if (Ie) {
       const double Im = (double)I[r], Ix = (double)Ie[qy * NF + qx];
       double l, w;
-      if (P.loss == PT_LOSS_POISSON) {
+      if (P.loss == PT_LOSS_GAUSSIAN) {
+        l = (Im - Ix) * (Im - Ix) / (2.0 * c * c);
+        w = (Im - Ix) / (c * c);
+      } else if (P.loss == PT_LOSS_POISSON) {
         l = Im - Ix * (log(Im + eps) - log(Ix + eps) + 1.0);
         w = 1.0 - Ix / (Im + eps);
       } else {
@@ -925,7 +928,8 @@ int validate(const pt_problem* p) {
   if (p->n_modes < 1 || p->n_slices < 1 || p->n_batch < 1 || p->n_pos_total < p->n_batch) return PT_ERR_BAD_SIZE;
   if (p->obj_ny < p->n || p->obj_nx < p->n) return PT_ERR_BAD_SIZE;
   if (!(p->pixel_size > 0.f) || !(p->wavelength > 0.f) || !(p->eps > 0.f)) return PT_ERR_BAD_PARAM;
-  if (p->loss != PT_LOSS_AMPLITUDE && p->loss != PT_LOSS_POISSON) return PT_ERR_BAD_PARAM;
+  if (p->loss != PT_LOSS_AMPLITUDE && p->loss != PT_LOSS_POISSON && p->loss != PT_LOSS_GAUSSIAN) return PT_ERR_BAD_PARAM;
+  if (p->loss == PT_LOSS_GAUSSIAN && !(p->loss_c > 0.f)) return PT_ERR_BAD_PARAM;
   if (p->shift_mode != PT_SHIFT_FOURIER_PROBE && p->shift_mode != PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_BAD_PARAM;
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT && (p->obj_ny < p->n + 1 || p->obj_nx < p->n + 1)) return PT_ERR_BAD_SIZE;
   if (p->n_slices > 1 && !p->slice_thickness) return PT_ERR_NULL;

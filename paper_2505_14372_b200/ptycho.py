@@ -16,7 +16,7 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 _CSRC = os.path.join(_HERE, "csrc")
 LIB_PATH = os.path.join(_HERE, "libptycho_b200.so")
 
-LOSS_AMPLITUDE, LOSS_POISSON = 0, 1
+LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
 WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE = 1, 2, 4, 16
 UPDATE_SGD, UPDATE_LSQML = 0, 1

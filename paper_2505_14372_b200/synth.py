@@ -18,7 +18,7 @@ from typing import List, Optional, Tuple
 
 import numpy as np
 
-LOSS_AMPLITUDE, LOSS_POISSON = 0, 1
+LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 
 
 @dataclass

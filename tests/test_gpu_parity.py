@@ -144,6 +144,15 @@ def test_bandlimit_and_anscombe():
     check(g, o)
 
 
+def test_gaussian_noise_model():
+    # l = (I - Iexp)^2 / (2 sigma^2), sigma in loss_c; config-3 physics on a small scan
+    cfg = synth.config(3, scan=(3, 4), n_modes=2, n_slices=3, loss=synth.LOSS_GAUSSIAN, loss_c=3.0, eps=0.5)
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
 def test_n64_multislice_multimode():
     cfg = synth.config(3, n=64, scan=(6, 5), n_modes=3, n_slices=4, obj_n=200, pixel_size=0.2, step_px=3.0)
     case = make_case(cfg, start_scale=0.8)

@@ -241,6 +241,14 @@ def test_loss_closed_forms():
             assert abs((lp - lm) / (2 * h) - w0) < 1e-6
             lp, _ = orc.loss_pixel(kind, I0 + 0.25, 5.0, 0.0, eps); lm, _ = orc.loss_pixel(kind, I0 - 0.25, 5.0, 0.0, eps)
             assert lp + lm - 2 * l0 > 0
+    # Gaussian (constant dropped): (I - Iexp)^2 / (2 sigma^2), sigma in the c slot; hand values, and the
+    # printed likelihood: -log P = l + log(sigma sqrt(2 pi)) per pixel
+    l, w = orc.loss_pixel(orc.LOSS_GAUSSIAN, 7.0, 4.0, 1.5, 0.3)
+    assert abs(l - 9.0 / (2 * 2.25)) < 1e-14 and abs(w - 3.0 / 2.25) < 1e-14
+    sig = 1.5
+    nll = -np.log(np.exp(-(7.0 - 4.0) ** 2 / (2 * sig ** 2)) / (sig * np.sqrt(2 * np.pi)))
+    assert abs(nll - (l + np.log(sig * np.sqrt(2 * np.pi)))) < 1e-12
+    assert orc.loss_pixel(orc.LOSS_GAUSSIAN, 5.0, 5.0, 2.0, 0.3) == (0.0, 0.0)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -273,9 +281,9 @@ def test_scatter_add_coverage_map():
 # full gradient: central finite differences (O7..O11; PAPER.md:181-185 Wirtinger convention, reading R15)
 # ------------------------------------------------------------------------------------------------
 @pytest.mark.parametrize("loss,eps,bandlimit", [(orc.LOSS_POISSON, 0.3, 0.0), (orc.LOSS_POISSON, 0.3, 2.0 / 3.0),
-                                                (orc.LOSS_AMPLITUDE, 1e-12, 0.0)])
+                                                (orc.LOSS_AMPLITUDE, 1e-12, 0.0), (orc.LOSS_GAUSSIAN, 0.3, 0.0)])
 def test_gradient_finite_differences(loss, eps, bandlimit):
-    pb, obj, probe, pos = small_problem(loss=loss, eps=eps, bandlimit=bandlimit)
+    pb, obj, probe, pos = small_problem(loss=loss, eps=eps, bandlimit=bandlimit, c=2.0 if loss == orc.LOSS_GAUSSIAN else 0.0)
     obj_t = (obj * np.exp(0.2 * crandn(*obj.shape))).astype(np.complex64)
     Iexp = orc.forward_loss(pb, obj_t, probe, pos)["intensity"].astype(np.float32) + 0.05
     g = orc.gradient(pb, obj, probe, pos, Iexp)
