@@ -453,3 +453,54 @@ def gpu_gradient_raw_steps(case, pbg, st):
     ill = torch.ones(obj_d.shape, dtype=torch.float32, device="cuda")
     ws = ptycho.make_workspace(pbg, cfg.n_pos, cfg.n_pos, ptycho.WANT_STEP_SIZES)
     ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum_prev=ill, step_terms=st)
+
+
+# ------------------------------------------------------------------------------------------------
+# edge cases: non-square odd-sized object, windows flush with every object border, a half-pixel tie of the position
+# split (reading R2), a single-position batch, and both shift modes
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", [0, 1])
+def test_edges_nonsquare_object_border_windows_single_position(mode):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    rng = np.random.default_rng(77)
+    n, M, S, ony, onx, px = 64, 2, 2, 75, 131, 0.5
+    kw = dict(n=n, n_modes=M, n_slices=S, obj_ny=ony, obj_nx=onx, pixel_size=px, wavelength=0.02, slice_thickness=[8.0, 8.0],
+              tilt_x_mrad=2.0, tilt_y_mrad=-1.0, bandlimit=0.0, loss=orc.LOSS_POISSON, loss_c=0.0, eps=0.8, shift_mode=mode)
+    pbo, pbg = orc.Problem(**kw), ptycho.Problem(**kw)
+    obj = np.exp(0.2 * rng.standard_normal((S, ony, onx)) + 0.5j * rng.standard_normal((S, ony, onx))).astype(np.complex64)
+    yy, xx = np.meshgrid(np.arange(n) - n // 2, np.arange(n) - n // 2, indexing="ij")
+    probe = (np.exp(-(yy ** 2 + xx ** 2) / 200.0)[None] * np.exp(1j * rng.standard_normal((M, n, n)) * 0.3) * np.array([3.0, 1.0])[:, None, None]).astype(np.complex64)
+    lim_y, lim_x = ony - n - mode, onx - n - mode               # largest admissible corner (bilinear taps reach corner + N)
+    corners = np.array([[0.0, 0.0], [lim_y, lim_x], [0.0, lim_x], [lim_y, 0.0], [5.5, 20.5], [3.25, 40.75]])   # 5.5: the R2 tie
+    pos = ((corners + n / 2) * px).astype(np.float32)
+    mean = orc.forward_loss(pbo, obj, probe, pos)["intensity"]
+    inten = rng.poisson(mean * 1.1).astype(np.float32)
+    o = orc.gradient(pbo, obj, probe, pos, inten, want_illum=True)
+
+    def run(rows):
+        obj_d, pr_d, pos_d, I_d = _t(obj), _t(probe), _t(pos), _t(inten)
+        b = None if rows is None else _t(np.asarray(rows, np.int32))
+        J = pos.shape[0] if rows is None else len(rows)
+        gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+        gX = torch.full((J, 2), float("nan"), dtype=torch.float32, device="cuda"); lpp = torch.zeros(J, dtype=torch.float32, device="cuda")
+        il = torch.full(obj_d.shape, float("nan"), dtype=torch.float32, device="cuda"); loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+        ws = ptycho.make_workspace(pbg, pos.shape[0], J)
+        ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, b, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il, loss=loss, loss_per_pos=lpp)
+        assert ptycho.status(ws) == 0
+        return dict(loss=loss.item(), loss_per_pos=lpp.cpu().numpy(), grad_object=gO.cpu().numpy(), grad_probe=gP.cpu().numpy(),
+                    grad_pos=gX.cpu().numpy(), illum=il.cpu().numpy())
+
+    g = run(None)
+    check(g, o, pos=True, px=px)
+    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    # a batch of ONE position (the tie case), through the batch index
+    o1 = orc.gradient(pbo, obj, probe, pos, inten, batch_idx=[4])
+    g1 = run([4])
+    check(g1, o1, pos=True, px=px)
+    # one pixel further out is refused with the deferred out-of-bounds status, not computed
+    bad = pos.copy(); bad[1, 1] += np.float32(px)
+    ws = ptycho.make_workspace(pbg, 6, 6)
+    gO = torch.empty_like(_t(obj)); gP = torch.empty_like(_t(probe))
+    ptycho.gradient(pbg, _t(obj), _t(probe), _t(bad), _t(inten), None, workspace=ws, grad_object=gO, grad_probe=gP)
+    assert ptycho.status(ws) == -6                                # PT_ERR_OUT_OF_BOUNDS (include/ptycho.h)
