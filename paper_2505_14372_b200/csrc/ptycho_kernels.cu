@@ -1109,7 +1109,7 @@ int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) 
 size_t ptycho_workspace_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
   size_t f, pp; ws_sizes(p, &f, &pp);
-  const size_t cap = (size_t)32 << 30;
+  const size_t cap = (size_t)64 << 30;
   size_t jc = p->n_batch;
   if (f + jc * pp > cap) {
     jc = (cap - f) / pp;
