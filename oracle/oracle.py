@@ -197,6 +197,21 @@ def forward_loss(pb: Problem, obj, probe, positions, intensity=None, batch_idx=N
     return dict(loss=loss.value, loss_per_pos=lpp, intensity=mi)
 
 
+def epie(pb: Problem, obj, probe, positions, intensity, batch_idx=None):
+    """Multislice ePIE update directions. Returns dict(loss, loss_per_pos, dir_object, dir_probe)."""
+    obj = _c64(obj); probe = _c64(probe); positions = _f32(positions); inten = _f32(intensity)
+    npos = positions.shape[0]; b, J = _batch(batch_idx, npos)
+    cp = pb._c(npos, J)
+    dO = np.zeros((pb.n_slices, pb.obj_ny, pb.obj_nx), np.complex128)
+    dP = np.zeros((pb.n_modes, pb.n, pb.n), np.complex128)
+    loss = C.c_double(); lpp = np.zeros(J, np.float64)
+    rc = lib().orc_epie(C.byref(cp), _p(obj, C.c_float), _p(probe, C.c_float), _p(positions, C.c_float), _p(inten, C.c_float),
+                        _p(b, C.c_int32), _p(dO, C.c_double), _p(dP, C.c_double), C.byref(loss), _p(lpp, C.c_double))
+    if rc != 0:
+        raise RuntimeError(f"orc_epie failed: {rc}")
+    return dict(loss=loss.value, loss_per_pos=lpp, dir_object=dO, dir_probe=dP)
+
+
 def gradient(pb: Problem, obj, probe, positions, intensity, batch_idx=None, want_illum=False):
     """O0..O12. Returns dict(loss, loss_per_pos, grad_object, grad_probe, grad_pos, illum)."""
     obj = _c64(obj); probe = _c64(probe); positions = _f32(positions); inten = _f32(intensity)

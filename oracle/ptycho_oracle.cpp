@@ -673,6 +673,76 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
   return 0;
 }
 
+// ------------------------------------------------------------------------------------------
+// Multislice ePIE ("3PIE") update directions for one group of positions (reading R23).
+//   detector:  chi~_k = ( sqrt(Iexp+c) / (eps + sqrt(I+c)) - 1 ) psi~_k            (amplitude model only;
+//              c = 0 is the classic modulus constraint)
+//   exit:      chi_{S-1,k} = N Finv(chi~_k)                                          (psi~ = F(.)/N, reading R5)
+//   slice i:   dO_{i,k}   = conj(Psi_{i,k}) / max_r |Psi_{i,k}|^2 . chi_{i,k}        (P_i = entering wave)
+//              chi'_{i,k} = conj(T_i)      / max_r |T_i|^2       . chi_{i,k}        (max over the window)
+//              chi_{i-1,k} = Finv( conj(H_{i-1}) F(chi'_{i,k}) )                     ("propagated backwards")
+//   object direction  dO_i[r0 + r] += sum_k dO_{i,k}[r], summed over the group
+//   probe direction   dP_k = (1/J) sum_j shift_j^{-1}( chi'_{0,k,j} )                ("averaged across the group")
+// The caller applies O_i += beta_object dO_i, P_k += beta_probe dP_k.  Fourier-shift mode and amplitude loss only
+// (returns -2 otherwise).  dir_object [S][ony][onx], dir_probe [M][N][N] complex (doubles).
+// ------------------------------------------------------------------------------------------
+int32_t orc_epie(const orc_problem* p, const float* object, const float* probe, const float* positions,
+                 const float* intensity, const int32_t* batch_idx, double* dir_object, double* dir_probe,
+                 double* loss, double* loss_per_pos) {
+  if (p->loss != 0 || p->shift_mode != 0) return -2;
+  Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
+  const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const long NN = m.NN;
+  const long on = (long)S * p->obj_ny * p->obj_nx;
+  std::vector<cd> dO(on, cd(0.0));
+  std::vector<std::vector<cd>> dPt(M, std::vector<cd>(NN, cd(0.0)));           // sum_j conj(R_j) F(chi'_0), Fourier side
+  double L = 0.0; int err = 0;
+  for (int jb = 0; jb < J; ++jb) {                                             // plain loop: fixed summation order
+    PosWork w; int jrow = row_of(m, jb);
+    if (forward_pos(m, jrow, w) != 0) { err = -1; continue; }
+    const float* Iexp = intensity + (long)jrow * NN;
+    std::vector<double> u(NN); double Lj = 0.0;
+    for (long q = 0; q < NN; ++q) {
+      double a = std::sqrt(w.I[q] + (double)p->loss_c), ae = std::sqrt((double)Iexp[q] + (double)p->loss_c);
+      Lj += 0.5 * (a - ae) * (a - ae);
+      u[q] = ae / ((double)p->eps + a) - 1.0;
+    }
+    L += Lj; if (loss_per_pos) loss_per_pos[jb] = Lj;
+    std::vector<double> tmax(S, 0.0);
+    for (int i = 0; i < S; ++i) for (long r = 0; r < NN; ++r) tmax[i] = std::max(tmax[i], std::norm(w.T[i][r]));
+    for (int k = 0; k < M; ++k) {
+      std::vector<cd> chi(NN);
+      for (long q = 0; q < NN; ++q) chi[q] = u[q] * w.psit[k][q];
+      Finv2(N, chi.data());
+      for (long r = 0; r < NN; ++r) chi[r] *= (double)N;
+      for (int i = S - 1; i >= 0; --i) {
+        const std::vector<cd>& Psi = w.Psi[(long)i * M + k];
+        double pmax = 0.0; for (long r = 0; r < NN; ++r) pmax = std::max(pmax, std::norm(Psi[r]));
+        for (int y = 0; y < N; ++y)
+          for (int x = 0; x < N; ++x) {
+            long r = (long)y * N + x;
+            dO[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] += std::conj(Psi[r]) / pmax * chi[r];
+          }
+        for (long r = 0; r < NN; ++r) chi[r] = std::conj(w.T[i][r]) / tmax[i] * chi[r];
+        if (i > 0) {
+          F2(N, chi.data());
+          for (long q = 0; q < NN; ++q) chi[q] *= std::conj(m.H[i - 1][q]);
+          Finv2(N, chi.data());
+        }
+      }
+      F2(N, chi.data());                                                       // undo the sub-pixel shift on the Fourier side
+      for (long q = 0; q < NN; ++q) dPt[k][q] += std::conj(w.R[q]) * chi[q];
+    }
+  }
+  if (dir_object) for (long o = 0; o < on; ++o) { dir_object[2 * o] = dO[o].real(); dir_object[2 * o + 1] = dO[o].imag(); }
+  if (dir_probe)
+    for (int k = 0; k < M; ++k) {
+      Finv2(N, dPt[k].data());
+      for (long r = 0; r < NN; ++r) { dir_probe[2 * (k * NN + r)] = dPt[k][r].real() / J; dir_probe[2 * (k * NN + r) + 1] = dPt[k][r].imag() / J; }
+    }
+  if (loss) *loss = L;
+  return err;
+}
+
 int32_t orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -619,3 +619,64 @@ def test_golden_oracle_tiny_case():
     for mode, name in ((0, "fourier_probe"), (1, "bilinear_object")):
         for k, v in mg.checksums(mode):
             assert abs(float(v) - want[(name, k)]) <= 1e-10 * max(abs(want[(name, k)]), 1e-3), (name, k, v, want[(name, k)])
+
+
+# ------------------------------------------------------------------------------------------------
+# multislice ePIE directions (reading R23)
+# ------------------------------------------------------------------------------------------------
+def test_epie_single_slice_is_classic_epie():
+    # S = 1, one mode, one position, eps -> 0, c = 0: the textbook ePIE step ("classic modulus constraint"):
+    # psi_c = Finv( sqrt(Iexp) F(psi) / |F(psi)| ),  dO|patch = conj(P) / max|P|^2 (psi_c - psi),  dP = conj(O) / max|O|^2 (psi_c - psi)
+    n, on = 16, 40
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=1, loss=orc.LOSS_AMPLITUDE, eps=1e-30)
+    pos[:] = (np.array([[13, 17]]) * 0.2).astype(np.float32)                 # integer corner: no sub-pixel shift
+    Iexp = (RNG.uniform(0.5, 3.0, size=(1, n, n))).astype(np.float32)
+    e = orc.epie(pb, obj, probe, pos, Iexp)
+    (r0y, dy), (r0x, dx) = orc.position_split(float(pos[0, 0]), 0.2, n), orc.position_split(float(pos[0, 1]), 0.2, n)
+    assert (r0y, r0x) == (13 - n // 2, 17 - n // 2) and abs(dy) < 1e-5 and abs(dx) < 1e-5   # float32 X/px: a ~1e-6 px remainder
+    f = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n) / n
+    ramp = np.exp(-2j * np.pi * (f[:, None] * dy + f[None, :] * dx))
+    O = obj[0, r0y:r0y + n, r0x:r0x + n].astype(complex)
+    P = np.fft.ifft2(ramp * np.fft.fft2(probe[0].astype(complex)))           # the probe as placed
+    psi = P * O
+    Fp = np.fft.fft2(psi)
+    psi_c = np.fft.ifft2(np.sqrt(Iexp[0].astype(float)) * n * Fp / np.abs(Fp))   # |F psi|^2 / N^2 = I: amplitude sqrt(Iexp) N
+    dpsi = psi_c - psi
+    ref_dO = np.conj(P) / np.max(np.abs(P) ** 2) * dpsi
+    ref_dP = np.conj(O) / np.max(np.abs(O) ** 2) * dpsi
+    got = e["dir_object"][0, r0y:r0y + n, r0x:r0x + n]
+    assert np.abs(got - ref_dO).max() < 1e-9 * np.abs(ref_dO).max()
+    ref_dP = np.fft.ifft2(np.conj(ramp) * np.fft.fft2(ref_dP))               # back to the un-shifted probe frame
+    assert np.abs(e["dir_probe"][0] - ref_dP).max() < 1e-9 * np.abs(ref_dP).max()
+    outside = e["dir_object"].copy(); outside[0, r0y:r0y + n, r0x:r0x + n] = 0
+    assert np.abs(outside).max() == 0
+
+
+def test_epie_multislice_invariants():
+    pb, obj, probe, pos = small_problem(n=8, M=2, S=3, on=20, J=3, loss=orc.LOSS_AMPLITUDE, eps=1e-30)
+    # (1) noiseless data at the true state: both directions vanish
+    Itrue = orc.forward_loss(pb, obj, probe, pos)["intensity"].astype(np.float64)
+    # float32 storage of the data limits how exactly the modulus constraint is met: compare with the probe's own scale
+    e0 = orc.epie(pb, obj, probe, pos, Itrue.astype(np.float32))
+    assert np.abs(e0["dir_object"]).max() < 1e-6 and np.abs(e0["dir_probe"]).max() < 1e-6 * np.abs(probe).max()
+    # (2) intensity-scaling covariance: P -> a P, Iexp -> a^2 Iexp leaves dO unchanged and scales dP by a
+    Iexp = (Itrue * RNG.uniform(0.5, 1.5, size=Itrue.shape)).astype(np.float32)
+    e1 = orc.epie(pb, obj, probe, pos, Iexp)
+    e2 = orc.epie(pb, obj, (2.0 * probe).astype(np.complex64), pos, (4.0 * Iexp).astype(np.float32))
+    assert np.abs(e2["dir_object"] - e1["dir_object"]).max() < 1e-6 * np.abs(e1["dir_object"]).max()
+    assert np.abs(e2["dir_probe"] - 2.0 * e1["dir_probe"]).max() < 1e-6 * np.abs(e1["dir_probe"]).max()
+    # (3) a small step along the directions lowers the amplitude loss (ePIE as gradient descent with a
+    # variable step), and the loss it reports is the amplitude loss of the forward model
+    L0 = orc.forward_loss(pb, obj, probe, pos, Iexp)["loss"]
+    assert abs(e1["loss"] - L0) < 1e-12 * L0
+    beta = 0.05
+    L1 = orc.forward_loss(pb, (obj + beta * e1["dir_object"]).astype(np.complex64), (probe + beta * e1["dir_probe"]).astype(np.complex64), pos, Iexp)["loss"]
+    assert L1 < L0
+    # (4) relation to the gradient chain for a single slice and mode ("single-slice ePIE can be considered a
+    # gradient descent method"): with eps -> 0, chi = -2 gPhi, hence dO = -2 gO / max|P_shift|^2 for ONE position
+    pb1, obj1, probe1, pos1 = small_problem(n=8, M=1, S=1, on=20, J=1, loss=orc.LOSS_AMPLITUDE, eps=1e-30)
+    I1 = (orc.forward_loss(pb1, obj1, probe1, pos1)["intensity"] * RNG.uniform(0.5, 1.5, size=(1, 8, 8))).astype(np.float32)
+    g = orc.gradient(pb1, obj1, probe1, pos1, I1); e = orc.epie(pb1, obj1, probe1, pos1, I1)
+    r0y, dy = orc.position_split(float(pos1[0, 0]), 0.2, 8); r0x, dx = orc.position_split(float(pos1[0, 1]), 0.2, 8)
+    Ps = orc.shift(probe1[0].astype(complex), dy, dx)
+    assert np.abs(e["dir_object"] + 2.0 * g["grad_object"] / np.max(np.abs(Ps) ** 2)).max() < 1e-9 * np.abs(e["dir_object"]).max()
