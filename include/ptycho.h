@@ -39,7 +39,13 @@ enum { PT_SHIFT_FOURIER_PROBE = 0,    /* integer window on the obj
 enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                                                        */
        PT_WANT_ILLUM = 2,             /* fill illum_d with sum_{j,k} |Psi_{i,k,j}|^2             */
        PT_WANT_STEP_SIZES = 4,        /* fill step_terms_d, needs illum_prev_d               */
-       PT_ACCUMULATE = 16 };          /* add into grad_object_d/grad_probe_d/illum_d/loss_d instead of overwriting */
+       PT_ACCUMULATE = 16,            /* add into grad_object_d/grad_probe_d/illum_d/loss_d instead of overwriting */
+       PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of
+                                       * gradients: grad_object_d <- sum_{j,k} conj(Psi_i,k)/max|Psi_i,k|^2
+                                       * chi_i,k (scattered), grad_probe_d <- (1/J) sum_j shift_j^-1(chi'_0,k), chi~ = (sqrt(Iexp+c)/
+                                       * (eps+sqrt(I+c)) - 1) psi~, chi'_i = conj(T_i)/max|T_i|^2 chi_i back-propagated slice by
+                                       * slice.  To be ADDED with PT_UPDATE_EPIE.  PT_LOSS_AMPLITUDE and PT_SHIFT_FOURIER_PROBE
+                                       * only; no position gradient, no step sizes (PT_ERR_UNSUPPORTED).                  */
 
 enum { PT_OK = 0, PT_ERR_NULL = -1, PT_ERR_BAD_SIZE = -2, PT_ERR_BAD_PARAM = -3, PT_ERR_WORKSPACE = -4,
        PT_ERR_CUDA = -5, PT_ERR_OUT_OF_BOUNDS = -6, PT_ERR_NONFINITE = -7, PT_ERR_UNSUPPORTED = -8 };
@@ -66,10 +72,12 @@ typedef struct {
   float lsqml_delta_p;            /* probe analogue: dPhat = -gP / (delta_p + 1) (R19)                          */
 } pt_problem;
 
-enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1 };
+enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1, PT_UPDATE_EPIE = 2 };
 typedef struct {                  /* HOST struct */
   int32_t mode;                   /* PT_UPDATE_SGD:   z <- z - lr * g   */
                                   /* PT_UPDATE_LSQML: O_i += beta_O alpha_{O,i} dOhat_i etc.   (R18) */
+                                  /* PT_UPDATE_EPIE:  O_i += beta_obj dO_i, P_k += beta_probe dP_k, with
+                                   *                  the directions ptycho_gradient returned under PT_EPIE              */
   float lr_obj, lr_probe, lr_pos;
   float beta_obj, beta_probe;
   float gamma;                    /* step-size regulariser of PAPER.md:221                                      */

@@ -54,6 +54,8 @@ struct Ws {
   cf* gTpart;          // [Jc][M][S][N^2]  R-native
   cf* Gpart;           // [Jc][M][N^2]     F-native
   cf* scratch;         // [Jc][M][N^2]     (step sizes: gPhi_0)
+  float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
+  float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
   cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
   int32_t Jc;
   size_t total;
@@ -76,7 +78,8 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   if (steps) pp += M * NN * sizeof(cf);
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
-  *fixed = f + 9 * 256;   // slack for the per-array alignment of the chunked part
+  if (p->flags & PT_EPIE) pp += (M * CL + 1) * S * sizeof(float) + 64;
+  *fixed = f + 11 * 256;   // slack for the per-array alignment of the chunked part
   *per_pos = pp;
 }
 
@@ -110,6 +113,8 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->gTpart = (cf*)take(jc * M * S * NN * sizeof(cf));
   w->Gpart = (cf*)take(jc * M * NN * sizeof(cf));
   w->scratch = steps ? (cf*)take(jc * M * NN * sizeof(cf)) : nullptr;
+  w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
+  w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
   w->Jc = (int32_t)jc;
   w->total = off;
@@ -288,7 +293,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* i
 
 // H12 tail: gP_k = Finv(gP~_k): Fourier-native double accumulators -> raster complex64 (overwrite or add)
 template <class G>
-__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const double2* acc, cf* out, int accumulate) {
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const double2* acc, cf* out, int accumulate, double extra_scale) {
   typedef Lay<G> L; typedef FL<G> F;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x, k = blockIdx.x / G::CL;
@@ -298,7 +303,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_ifft(const doub
   Fft<G>::begin_fourier();
   __syncthreads();
   cf v[32];
-  const double sc = 1.0 / ((double)F::NF * (double)F::NF);
+  const double sc = extra_scale / ((double)F::NF * (double)F::NF);
   const double2* a0 = acc + ((size_t)k * G::CL + rk) * F::NNS;
 #pragma unroll
   for (int r = 0; r < 32; ++r) { double2 a = a0[L::native(t, r)]; v[r] = make_float2((float)(a.x * sc), (float)(a.y * sc)); }
@@ -516,7 +521,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = N Finv(g~) = F^H(g~) / N
     const float4* ps = (const float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);
     const float2* wd = (const float2*)(P.w.wdet + ((size_t)jl * CL + rk) * NNS);
-    const float sc = 1.0f / (float)NF;
+    const float sc = (MODE == 2 ? -2.0f : 1.0f) / (float)NF;     // ePIE: chi~ = (ae/(eps+a) - 1) psi~ = -2 w psi~
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 q = ps[p * T + t]; const float2 w = wd[p * T + t];
@@ -541,7 +546,14 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
-    if (MODE == 0) {
+    if (MODE != 1) {
+      // ePIE (MODE 2): dO = conj(Psi) / max|Psi|^2 chi ; chi' = conj(T) / max|T|^2 chi
+      float s1 = 1.0f, s2 = 1.0f;
+      if (MODE == 2) {
+        float pm = 0.f;
+        for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pair * S + i) * CL + c]);
+        s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
+      }
       float4* gt = (float4*)(P.w.gTpart + fld(i));
 #pragma unroll
       for (int p = 0; p < 16; ++p) {
@@ -549,7 +561,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         cf T0, T1;
         if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
         else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
-        const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+        cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+        if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
         __stcs(gt + p * T + t, make_float4(g0.x, g0.y, g1.x, g1.y));    // H10: gT_i contribution conj(Psi) .* gPhi
         v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
         v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
@@ -593,7 +606,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
   const cf* ry = rx + NF;
   const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
-  if (MODE == 0) {
+  if (MODE != 1) {
     // v = G~ = F(gPsi_0).  H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
     cf* gp = P.w.Gpart + ((size_t)pair * CL + rk) * NNS;
     cf wxv[F::NXV];
@@ -657,6 +670,37 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       __syncthreads();
     }
   }
+}
+
+// ------------------------------------------------------------------------------------------------
+// ePIE normalisations: tmax[jl][i] = max over the window of |O_i|^2 ; psimax[block] = max |Psi|^2 of
+// one 16384-element block of the stash (one per (pair, slice, rank); the backward kernel takes the max over the ranks).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ float block_max256(float v, float* red) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v = fmaxf(v, __shfl_xor_sync(0xffffffffu, v, o));
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = v;
+  __syncthreads();
+  float m = red[0];
+  for (int w = 1; w < 8; ++w) m = fmaxf(m, red[w]);
+  return m;
+}
+__global__ void __launch_bounds__(256) k_patch_max(KP P) {
+  __shared__ float red[8];
+  const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, N = P.N;
+  const cf* o = P.object + ((size_t)i * P.ony + P.w.r0[2 * jb]) * P.onx + P.w.r0[2 * jb + 1];
+  float m = 0.f;
+  for (int e = threadIdx.x; e < N * N; e += 256) { const cf z = o[(size_t)(e / N) * P.onx + (e % N)]; m = fmaxf(m, fmaf(z.x, z.x, z.y * z.y)); }
+  m = block_max256(m, red);
+  if (threadIdx.x == 0) P.w.tmax[(size_t)jl * P.S + i] = m;
+}
+__global__ void __launch_bounds__(256) k_stash_max(const cf* stash, float* out, int n_per_block) {
+  __shared__ float red[8];
+  const cf* s = stash + (size_t)blockIdx.x * n_per_block;
+  float m = 0.f;
+  for (int e = threadIdx.x; e < n_per_block; e += 256) { const cf z = s[e]; m = fmaxf(m, fmaf(z.x, z.x, z.y * z.y)); }
+  m = block_max256(m, red);
+  if (threadIdx.x == 0) out[blockIdx.x] = m;
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -897,11 +941,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max"};
 thread_local int64_t g_launches = 0;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
@@ -971,6 +1015,7 @@ int set_smem_attrs() {
   if (cudaFuncSetAttribute(k_forward<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   return PT_OK;
@@ -1025,9 +1070,10 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
   const bool acc = (p->flags & PT_ACCUMULATE) != 0;
   const bool want_illum = (p->flags & PT_WANT_ILLUM) && illum;
-  const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX;
+  const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX && !(p->flags & PT_EPIE);
   const bool want_steps = (p->flags & PT_WANT_STEP_SIZES) && step_terms;
   const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
+  const bool epie = (p->flags & PT_EPIE) != 0;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
   if (!acc) {
@@ -1043,7 +1089,14 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
-    launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+    if (epie) {
+      k_patch_max<<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
+      LAUNCH_CHECK(K_epie_max, st);
+      k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
+      LAUNCH_CHECK(K_epie_max, st);
+      launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+    } else
+      launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
     LAUNCH_CHECK(K_backward, st);
     if (bilin) {
       if (want_illum) k_gather_object<G, true, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
@@ -1060,7 +1113,8 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp);
     LAUNCH_CHECK(K_reduce_probe, st);
   }
-  launch_fft<G>(k_probe_ifft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const double2*)kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0);
+  launch_fft<G>(k_probe_ifft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const double2*)kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0,
+                epie ? 1.0 / (double)p->n_batch : 1.0);                         // ePIE: probe direction averaged over the group
   LAUNCH_CHECK(K_probe_ifft, st);
   if (want_steps) {
     // H14 second sweep (O13/O14): needs the batch-aggregated gO, gP
@@ -1149,6 +1203,11 @@ int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c6
   if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
+  // ePIE directions (the optimal wavefront update is given for the amplitude model): amplitude loss,
+  // Fourier-shift mode, no step-size terms, no position gradient
+  if ((p->flags & PT_EPIE) && (p->loss != PT_LOSS_AMPLITUDE || p->shift_mode != PT_SHIFT_FOURIER_PROBE ||
+                               ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d) || ((p->flags & PT_WANT_POS_GRAD) && grad_pos_d)))
+    return PT_ERR_UNSUPPORTED;
   Ws w;
   pt_problem q = *p;
   if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
@@ -1176,6 +1235,11 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
     if (object_d && grad_object_d) { k_axpy<<<(unsigned)((2 * on + 255) / 256), 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, -u->lr_obj, 2 * on); LAUNCH_CHECK(K_axpy, st); }
     if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, -u->lr_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
     if (positions_d && grad_pos_d) { k_pos_sgd<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, grad_pos_d, batch_idx_d, u->lr_pos, p->n_batch); LAUNCH_CHECK(K_pos_sgd, st); }
+    return PT_OK;
+  }
+  if (u->mode == PT_UPDATE_EPIE) {      // O_i += beta_object dO_i ; P_k += beta_probe dP_k
+    if (object_d && grad_object_d) { k_axpy<<<(unsigned)((2 * on + 255) / 256), 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, u->beta_obj, 2 * on); LAUNCH_CHECK(K_axpy, st); }
+    if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, u->beta_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
     return PT_OK;
   }
   if (u->mode != PT_UPDATE_LSQML) return PT_ERR_BAD_PARAM;

@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libptycho_b200.so")
 
 LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
-WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE = 1, 2, 4, 16
-UPDATE_SGD, UPDATE_LSQML = 0, 1
+WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE = 1, 2, 4, 16, 32
+UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE = 0, 1, 2
 OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
            "ptycho_apply_update", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",

@@ -66,7 +66,7 @@ def test_validation_and_workspace_sizes(lib):
     per_pos = (hi - lo) / 63
     assert 2 * 8 * 20 * 128 * 128 * 8 <= per_pos <= 1.1 * 2 * 8 * 20 * 128 * 128 * 8
     big = ptycho.workspace_bytes(pb, 4096, 4096)
-    assert big <= (32 << 30) + (1 << 20)                          # chunked: capped recommendation
+    assert big <= (64 << 30) + (1 << 20)                          # chunked: capped recommendation
     import dataclasses
     for bad in (dict(n=100), dict(n_modes=0), dict(obj_ny=100)):
         with pytest.raises(ptycho.PtychoError):
