@@ -539,3 +539,42 @@ def test_epie_directions_and_update(which):
     # the Poisson model has no ePIE wavefront update in the paper: refused, not improvised
     with pytest.raises(ptycho.PtychoError):
         gpu_gradient(case, gpu_problem(cfg, loss=synth.LOSS_POISSON, eps=0.8), flags=ptycho.EPIE, want_pos=False)
+
+
+# ------------------------------------------------------------------------------------------------
+# the pieces compose into a reconstruction: config 1 (noiseless data from the oracle, vacuum start, true probe),
+# 60 ePIE iterations through the C ABI (object updates summed over groups of 64, beta 0.05: the windows of a group
+# overlap ~16-fold); the amplitude loss must fall by more than 10x and the recovered phase
+# must correlate with the true phase inside the scanned area.  (A property of the method; the
+# per-call numbers are pinned by the parity tests above.)
+# ------------------------------------------------------------------------------------------------
+def test_epie_iterations_reconstruct_config1():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(1, eps=1e-3)                            # a small eps: the eps of PAPER.md:173 biases the fixed point
+    case = make_case(cfg, start_scale=0.0, noise=False)
+    pbg = gpu_problem(cfg)
+    J = cfg.n_pos
+    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(case.positions_true), _t(case.intensity)
+    gO, gP = torch.empty_like(obj_d), torch.empty_like(pr_d)
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ws = ptycho.make_workspace(pbg, J, 64, ptycho.EPIE)
+    rng = np.random.default_rng(5)
+    losses = []
+    for it in range(60):
+        order = rng.permutation(J).astype(np.int32)
+        tot = 0.0
+        for b in range(0, J, 64):                                # groups of 64 positions, sparse grouping
+            bi = _t(order[b:b + 64])
+            ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, bi, workspace=ws, grad_object=gO, grad_probe=gP, loss=loss, flags=ptycho.EPIE)
+            ptycho.apply_update(pbg, obj_d, None, None, grad_object=gO, mode=ptycho.UPDATE_EPIE, beta_obj=0.05, n_batch=64)
+            tot += loss.item()
+        losses.append(tot)
+    assert ptycho.status(ws) == 0
+    assert losses[-1] < 0.1 * losses[0] and losses[-1] < losses[20] < losses[5], (losses[0], losses[5], losses[20], losses[-1])
+    rec = np.angle(obj_d.cpu().numpy()[0]); tru = np.angle(case.obj_true[0])
+    c = cfg.obj_n // 2
+    sl = (slice(c - 24, c + 24), slice(c - 24, c + 24))             # well inside the scanned area
+    a, b_ = rec[sl] - rec[sl].mean(), tru[sl] - tru[sl].mean()
+    corr = float((a * b_).sum() / np.sqrt((a * a).sum() * (b_ * b_).sum()))
+    assert corr > 0.95, corr
