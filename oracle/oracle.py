@@ -264,5 +264,30 @@ def apply_update(pb: Problem, mode, obj, probe, positions, grad_object=None, gra
     return o, pr, x
 
 
+def weighted_illum(pb: Problem, obj, probe, positions, step_terms_, gamma, batch_idx=None):
+    """W_i = sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2 scattered, alpha = numO/(denO+gamma) per position."""
+    obj = _c64(obj); probe = _c64(probe); positions = _f32(positions)
+    npos = positions.shape[0]; b, J = _batch(batch_idx, npos)
+    cp = pb._c(npos, J)
+    st = np.ascontiguousarray(step_terms_, np.float64)
+    out = np.zeros((pb.n_slices, pb.obj_ny, pb.obj_nx), np.float64)
+    rc = lib().orc_weighted_illum(C.byref(cp), _p(obj, C.c_float), _p(probe, C.c_float), _p(positions, C.c_float),
+                                  _p(b, C.c_int32), _p(st, C.c_double), C.c_double(gamma), _p(out, C.c_double))
+    if rc != 0:
+        raise ValueError(f"oracle: weighted_illum failed ({rc})")
+    return out
+
+
+def lsqml_weighted_object(pb: Problem, obj, grad_object, illum_prev, illum_batch, willum, beta_obj=1.0):
+    """O_i += beta_O dOhat_i W_i / I_i (PAPER.md:225 as printed). Returns the updated object (complex128 copy)."""
+    o = np.array(obj, dtype=np.complex128, order="C")
+    f = lambda a, t: np.ascontiguousarray(a, t)
+    gO = f(grad_object, np.complex128); ip = f(illum_prev, np.float64); ib = f(illum_batch, np.float64); wi = f(willum, np.float64)
+    cp = pb._c(1, 1)
+    lib().orc_lsqml_weighted_object(C.byref(cp), _p(o, C.c_double), _p(gO, C.c_double), _p(ip, C.c_double), _p(ib, C.c_double),
+                                    _p(wi, C.c_double), C.c_double(beta_obj))
+    return o
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())

@@ -674,6 +674,50 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
 }
 
 // ------------------------------------------------------------------------------------------
+// LSQML final slice update with PER-POSITION step sizes, exactly as printed at PAPER.md:225 (reading R24):
+//   alpha_{O,i,j} = numO[j,i] / (denO[j,i] + gamma)                       (sums over r and k only)
+//   W_i[r]  = sum_{j in group} alpha_{O,i,j} sum_k |Psi_{i,k,j}[r - r0_j]|^2   (numerator weight of :225)
+//   I_i[r]  = sum_{j in group} sum_k |Psi_{i,k,j}[r - r0_j]|^2                 (denominator of :225 = O12 of this batch)
+//   O_i[r] += beta_O dOhat_i[r] W_i[r] / I_i[r]      where I_i[r] > 0 ; pixels no window of the group covers are left alone
+// dOhat_i does not depend on j, so it leaves the group sum.  orc_weighted_illum returns W; the update is below.
+// ------------------------------------------------------------------------------------------
+int32_t orc_weighted_illum(const orc_problem* p, const float* object, const float* probe, const float* positions,
+                           const int32_t* batch_idx, const double* step_terms, double gamma, double* willum) {
+  if (p->shift_mode == 1) return -2;
+  Model m; model_init(m, p, object, probe, positions, nullptr, batch_idx);
+  const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const int W = 2 * S + 6;
+  const long on = (long)S * p->obj_ny * p->obj_nx;
+  for (long o = 0; o < on; ++o) willum[o] = 0.0;
+  for (int jb = 0; jb < J; ++jb) {                                              // plain serial loop: fixed summation order
+    PosWork w; int jrow = row_of(m, jb);
+    if (forward_pos(m, jrow, w) != 0) return -1;
+    for (int i = 0; i < S; ++i) {
+      const double alpha = step_terms[(long)jb * W + 2 * i] / (step_terms[(long)jb * W + 2 * i + 1] + gamma);
+      for (int y = 0; y < N; ++y)
+        for (int x = 0; x < N; ++x) {
+          double s = 0.0;
+          for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][(long)y * N + x]);
+          willum[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] += alpha * s;
+        }
+    }
+  }
+  return 0;
+}
+
+// object (double complex, in/out) += beta_O dOhat W / I, dOhat = -gO / (illum_prev + delta_O)
+int32_t orc_lsqml_weighted_object(const orc_problem* p, double* object, const double* grad_object, const double* illum_prev,
+                                  const double* illum_batch, const double* willum, double beta_obj) {
+  const long on = (long)p->n_slices * p->obj_ny * p->obj_nx;
+  for (long o = 0; o < on; ++o) {
+    if (!(illum_batch[o] > 0.0)) continue;
+    const double f = beta_obj * (willum[o] / illum_batch[o]) / (illum_prev[o] + (double)p->lsqml_delta_o);
+    object[2 * o] += f * (-grad_object[2 * o]);
+    object[2 * o + 1] += f * (-grad_object[2 * o + 1]);
+  }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
 // Multislice ePIE ("3PIE") update directions for one group of positions (reading R23).
 //   detector:  chi~_k = ( sqrt(Iexp+c) / (eps + sqrt(I+c)) - 1 ) psi~_k            (amplitude model only;
 //              c = 0 is the classic modulus constraint)

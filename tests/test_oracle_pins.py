@@ -497,6 +497,43 @@ def test_lsqml_position_step_recovers_offset():
     assert errs[-1] < 0.3 * errs[0]
 
 
+def test_lsqml_weighted_update_per_position_alpha():
+    # PAPER.md:225 as printed (reading R24): O_i += beta sum_j alpha_{i,j} dOhat_i sum_k|Psi_{i,k,j}|^2 / sum_{j,k}|Psi_{i,k,j}|^2
+    pb, obj, probe, pos = small_problem(n=16, M=2, S=3, on=36, J=4, loss=orc.LOSS_POISSON, eps=0.8)
+    pb.lsqml_delta_o = 0.7
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    illum_prev = g["illum"] * 1.3 + 0.1
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], illum_prev)
+    gamma, S, J = 0.3, 3, 4
+    W = orc.weighted_illum(pb, obj, probe, pos, st, gamma)
+    # (a) linearity route: W = sum_j alpha_{i,j} illum_j with illum_j the (already pinned, O12) map of the one-position batch {j}
+    alpha = st[:, 0:2 * S:2] / (st[:, 1:2 * S:2] + gamma)                       # PAPER.md:221 per position
+    ref = np.zeros_like(W)
+    for j in range(J):
+        ilj = orc.gradient(pb, obj, probe, pos, Iexp, batch_idx=[j], want_illum=True)["illum"]
+        ref += alpha[j][:, None, None] * ilj
+    assert np.abs(W - ref).max() < 1e-12 * np.abs(ref).max()
+    # (b) equal step sizes for every position collapse :225 to the per-group form O_i += beta alpha_i dOhat_i (reading R18)
+    st_eq = st.copy(); a_i = np.array([0.4, -0.2, 1.1])
+    st_eq[:, 0:2 * S:2] = a_i[None, :] * (st[:, 1:2 * S:2] + gamma)
+    W_eq = orc.weighted_illum(pb, obj, probe, pos, st_eq, gamma)
+    cov = g["illum"] > 0
+    assert np.abs(W_eq - a_i[:, None, None] * g["illum"]).max() < 1e-12 * np.abs(g["illum"]).max()
+    o_w = orc.lsqml_weighted_object(pb, obj, g["grad_object"], illum_prev, g["illum"], W_eq, beta_obj=0.5)
+    dOhat = -g["grad_object"] / (illum_prev + float(np.float32(0.7)))
+    o_g = obj.astype(np.complex128) + 0.5 * a_i[:, None, None] * dOhat
+    assert np.abs(o_w - o_g)[cov].max() < 1e-12
+    assert np.abs(o_w - obj.astype(np.complex128))[~cov].max() == 0.0          # uncovered pixels are left alone
+    # (c) the printed formula, written out pixel by pixel on one slice (brute force)
+    o_w = orc.lsqml_weighted_object(pb, obj, g["grad_object"], illum_prev, g["illum"], W, beta_obj=0.8)
+    i = 1
+    for (y, x) in [(10, 11), (17, 20), (25, 9)]:
+        assert g["illum"][i, y, x] > 0
+        expect = obj[i, y, x].astype(np.complex128) + 0.8 * dOhat[i, y, x] * ref[i, y, x] / g["illum"][i, y, x]
+        assert abs(o_w[i, y, x] - expect) < 1e-12
+
+
 def test_sgd_update():
     pb, obj, probe, pos = small_problem()
     gO = crandn(*obj.shape); gP = crandn(*probe.shape); gX = RNG.standard_normal(pos.shape)
