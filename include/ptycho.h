@@ -40,6 +40,10 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
        PT_WANT_ILLUM = 2,             /* fill illum_d with sum_{j,k} |Psi_{i,k,j}|^2             */
        PT_WANT_STEP_SIZES = 4,        /* fill step_terms_d, needs illum_prev_d               */
        PT_ACCUMULATE = 16,            /* add into grad_object_d/grad_probe_d/illum_d/loss_d instead of overwriting */
+       PT_WANT_WEIGHTED_ILLUM = 64,   /* with PT_WANT_ILLUM and PT_WANT_STEP_SIZES: illum_d is [2][S][obj_ny][obj_nx]; plane 1 is
+                                       * W_i = sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2, alpha_{O,i,j} = numO[j,i] / (denO[j,i] +
+                                       * lsqml_gamma): the per-position step sizes of PAPER.md:221 weighting the slice update as
+                                       * PAPER.md:225 prints it (reading R24); used by PT_UPDATE_LSQML_WEIGHTED              */
        PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of
                                        * gradients: grad_object_d <- sum_{j,k} conj(Psi_i,k)/max|Psi_i,k|^2
                                        * chi_i,k (scattered), grad_probe_d <- (1/J) sum_j shift_j^-1(chi'_0,k), chi~ = (sqrt(Iexp+c)/
@@ -70,9 +74,10 @@ typedef struct {
   int32_t flags;                  /* PT_WANT_* | PT_ACCUMULATE                                                   */
   float lsqml_delta_o;            /* delta_O of PAPER.md:219 (PT_WANT_STEP_SIZES only)                          */
   float lsqml_delta_p;            /* probe analogue: dPhat = -gP / (delta_p + 1) (R19)                          */
+  float lsqml_gamma;              /* gamma of PAPER.md:221 in the per-position alphas (PT_WANT_WEIGHTED_ILLUM only) */
 } pt_problem;
 
-enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1, PT_UPDATE_EPIE = 2 };
+enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1, PT_UPDATE_EPIE = 2, PT_UPDATE_LSQML_WEIGHTED = 3 };
 typedef struct {                  /* HOST struct */
   int32_t mode;                   /* PT_UPDATE_SGD:   z <- z - lr * g   */
                                   /* PT_UPDATE_LSQML: O_i += beta_O alpha_{O,i} dOhat_i etc.   (R18) */
@@ -80,7 +85,12 @@ typedef struct {                  /* HOST struct */
                                    *                  the directions ptycho_gradient returned under PT_EPIE              */
   float lr_obj, lr_probe, lr_pos;
   float beta_obj, beta_probe;
+                                  /* PT_UPDATE_LSQML_WEIGHTED: object as PAPER.md:225 prints it, with per-position step
+                                   *                  sizes (R24): O_i += beta_obj dOhat_i W_i / I_i where I_i > 0 (pixels no window
+                                   *                  of the batch covers are left alone); probe and positions as PT_UPDATE_LSQML */
   float gamma;                    /* step-size regulariser of PAPER.md:221                                      */
+  const float *illum_batch_d;     /* DEVICE, [2][S][obj_ny][obj_nx]: (I, W) as ptycho_gradient wrote them to illum_d under
+                                   * PT_WANT_WEIGHTED_ILLUM; PT_UPDATE_LSQML_WEIGHTED only, NULL otherwise                */
 } pt_update;
 
 /* Number of floats per position in step_terms_d:  (numO_i, denO_i) i = 0..S-1, (numP, denP),
@@ -118,7 +128,8 @@ int32_t ptycho_forward_loss(const pt_problem *p, const pt_c64 *object_d, const p
  *   grad_object_d [S][obj_ny][obj_nx]  dL/d conj(O_i), deterministic scatter-add over overlapping patches
  *   grad_probe_d  [M][N][N]            dL/d conj(P_k)
  *   grad_pos_d    [n_batch][2]         dL/dX (per Angstrom), PT_WANT_POS_GRAD            (NULL allowed)
- *   illum_d       [S][obj_ny][obj_nx]  float, this batch's sum_{j,k}|Psi_{i,k}|^2, PT_WANT_ILLUM (NULL allowed)
+ *   illum_d       [S][obj_ny][obj_nx]  float, this batch's sum_{j,k}|Psi_{i,k}|^2, PT_WANT_ILLUM (NULL allowed);
+ *                                      [2][S][obj_ny][obj_nx] under PT_WANT_WEIGHTED_ILLUM (plane 1 = W, see the flag)
  *   illum_prev_d  [S][obj_ny][obj_nx]  float, running sum of the previous iteration (R19);
  *                                      needed with PT_WANT_STEP_SIZES
  *   step_terms_d  [n_batch][2S+6]      float, PT_WANT_STEP_SIZES                          (NULL allowed)

@@ -57,6 +57,7 @@ struct Ws {
   float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
   float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
   cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
+  float* alpha_ji;     // [Jc][S]          per-position object step sizes alpha_{O,i,j} (PT_WANT_WEIGHTED_ILLUM only)
   int32_t Jc;
   size_t total;
 };
@@ -76,10 +77,10 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   f += align_up(J * M * CL * (2 * S + 6) * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
   size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
-  if (steps) pp += M * NN * sizeof(cf);
+  if (steps) pp += M * NN * sizeof(cf) + S * sizeof(float);
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
   if (p->flags & PT_EPIE) pp += (M * CL + 1) * S * sizeof(float) + 64;
-  *fixed = f + 11 * 256;   // slack for the per-array alignment of the chunked part
+  *fixed = f + 12 * 256;   // slack for the per-array alignment of the chunked part
   *per_pos = pp;
 }
 
@@ -116,6 +117,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
   w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
+  w->alpha_ji = steps ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Jc = (int32_t)jc;
   w->total = off;
   return off <= bytes ? PT_OK : PT_ERR_WORKSPACE;
@@ -827,6 +829,60 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// LSQML slice update with per-position step sizes (reading R24).
+// k_alpha_pos: alpha_{O,i,j} = numO[j,i] / (denO[j,i] + gamma) from the per-(mode, rank) fp64 partials of the sweep that
+// has just run over this chunk (fixed order).  k_gather_willum: W_i[r] += sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}[r - r0_j]|^2,
+// the same owner-computes gather as k_gather_object over the slice-wave stash (fixed (j, k) order, fp64).
+// ------------------------------------------------------------------------------------------------
+__global__ void k_alpha_pos(KP P, int cl, float gamma) {
+  const int idx = blockIdx.x * blockDim.x + threadIdx.x;
+  if (idx >= P.jc * P.S) return;
+  const int jl = idx / P.S, i = idx - jl * P.S, MU = P.M * cl, W = 2 * P.S + 6;
+  double num = 0.0, den = 0.0;
+  for (int u = 0; u < MU; ++u) {
+    const double* sp = P.w.step_part + ((size_t)(P.j0 + jl) * MU + u) * W;
+    num += sp[2 * i]; den += sp[2 * i + 1];
+  }
+  P.w.alpha_ji[idx] = (float)(num / (den + (double)gamma));
+}
+template <class G>
+__global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
+  typedef FL<G> F;
+  constexpr int N = F::NF, NN = F::NNF, TW_ = GATHER_TW, TH_ = 256 / GATHER_TW;
+  __shared__ int2 sr0[256];
+  __shared__ float sal[256];
+  const int i = blockIdx.z;
+  const int ox0 = blockIdx.x * TW_, oy0 = blockIdx.y * TH_;
+  const int ox = ox0 + threadIdx.x, oy = oy0 + threadIdx.y;
+  const int tid = threadIdx.y * TW_ + threadIdx.x;
+  double acc = 0.0;
+  for (int jbase = 0; jbase < P.jc; jbase += 256) {
+    const int cnt = min(256, P.jc - jbase);
+    if (tid < cnt) {
+      sr0[tid] = make_int2(P.w.r0[2 * (P.j0 + jbase + tid) + 1], P.w.r0[2 * (P.j0 + jbase + tid)]);  // (x, y)
+      sal[tid] = P.w.alpha_ji[(size_t)(jbase + tid) * P.S + i];
+    }
+    __syncthreads();
+    for (int jj = 0; jj < cnt; ++jj) {
+      const int2 r0 = sr0[jj];
+      if (r0.x > ox0 + TW_ - 1 || r0.x + N <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + N <= oy0) continue;   // block-uniform reject
+      const int px = ox - r0.x, py = oy - r0.y;
+      if (px >= 0 && px < N && py >= 0 && py < N) {
+        const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
+        double s = 0.0;
+        for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; s += (double)q.x * q.x + (double)q.y * q.y; }
+        acc += (double)sal[jj] * s;
+      }
+    }
+    __syncthreads();
+  }
+  if (ox < P.onx && oy < P.ony) {
+    const size_t o = ((size_t)i * P.ony + oy) * P.onx + ox;
+    willum[o] = (float)((double)willum[o] + acc);
+  }
+}
+
 // H12: gP~_k[q] += sum_j (chunk) conj(R_j) G~_{k,j}[q], fixed order, fp64
 __global__ void k_reduce_probe(KP P) {
   const int NN = P.N * P.N;
@@ -919,6 +975,16 @@ __global__ void k_lsqml_object(cf* O, const cf* gO, const float* illum_prev, con
   const float a = beta * alpha[i / slice_elems] * (-1.0f / (illum_prev[i] + delta_o));
   O[i] = make_float2(fmaf(a, gO[i].x, O[i].x), fmaf(a, gO[i].y, O[i].y));
 }
+// PAPER.md:225 as printed (R24): O_i += beta dOhat_i W_i / I_i where I_i > 0, dOhat = -gO / (illum_prev + delta_O)
+__global__ void k_lsqml_object_weighted(cf* O, const cf* gO, const float* illum_prev, const float* illum_batch, const float* willum,
+                                        float beta, float delta_o, size_t n) {
+  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float ib = illum_batch[i];
+  if (!(ib > 0.f)) return;
+  const float a = beta * (willum[i] / ib) * (-1.0f / (illum_prev[i] + delta_o));
+  O[i] = make_float2(fmaf(a, gO[i].x, O[i].x), fmaf(a, gO[i].y, O[i].y));
+}
 __global__ void k_lsqml_probe(cf* Pr, const cf* gP, const float* alpha, int S, float beta, float delta_p, size_t n) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
@@ -941,11 +1007,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum"};
 thread_local int64_t g_launches = 0;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
@@ -1072,6 +1138,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool want_illum = (p->flags & PT_WANT_ILLUM) && illum;
   const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX && !(p->flags & PT_EPIE);
   const bool want_steps = (p->flags & PT_WANT_STEP_SIZES) && step_terms;
+  const bool want_w = (p->flags & PT_WANT_WEIGHTED_ILLUM) != 0;     // validated by the caller: needs want_illum && want_steps
   const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   const bool epie = (p->flags & PT_EPIE) != 0;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
@@ -1079,7 +1146,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   if (!acc) {
     k_zero<<<592, 256, 0, st>>>((float*)gO, on * 2);
     LAUNCH_CHECK(K_zero, st);
-    if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, on); LAUNCH_CHECK(K_zero, st); }
+    if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, want_w ? 2 * on : on); LAUNCH_CHECK(K_zero, st); }
   }
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
@@ -1132,6 +1199,12 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       }
       launch_fft<G>(k_backward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
       LAUNCH_CHECK(K_backward, st);
+      if (want_w) {   // PAPER.md:225 with per-position step sizes (R24): W += sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2
+        k_alpha_pos<<<(kp.jc * p->n_slices + 255) / 256, 256, 0, st>>>(kp, G::CL, p->lsqml_gamma);
+        LAUNCH_CHECK(K_alpha_pos, st);
+        k_gather_willum<G><<<ggrid, gblock, 0, st>>>(kp, illum + on);
+        LAUNCH_CHECK(K_gather_willum, st);
+      }
     }
   }
   k_finalize<<<1, 1024, 0, st>>>(kp, G::CL, loss_d, acc ? 1 : 0, loss_per_pos_d, want_pos ? gX : nullptr, want_steps ? step_terms : nullptr);
@@ -1203,6 +1276,11 @@ int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c6
   if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
+  if (p->flags & PT_WANT_WEIGHTED_ILLUM) {
+    if (!(p->flags & PT_WANT_ILLUM) || !(p->flags & PT_WANT_STEP_SIZES) || (p->flags & PT_EPIE)) return PT_ERR_BAD_PARAM;
+    if (!illum_d || !step_terms_d) return PT_ERR_NULL;
+    if (!(p->lsqml_gamma >= 0.f)) return PT_ERR_BAD_PARAM;
+  }
   // ePIE directions (the optimal wavefront update is given for the amplitude model): amplitude loss,
   // Fourier-shift mode, no step-size terms, no position gradient
   if ((p->flags & PT_EPIE) && (p->loss != PT_LOSS_AMPLITUDE || p->shift_mode != PT_SHIFT_FOURIER_PROBE ||
@@ -1242,7 +1320,7 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
     if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, u->beta_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
     return PT_OK;
   }
-  if (u->mode != PT_UPDATE_LSQML) return PT_ERR_BAD_PARAM;
+  if (u->mode != PT_UPDATE_LSQML && u->mode != PT_UPDATE_LSQML_WEIGHTED) return PT_ERR_BAD_PARAM;
   if (!step_terms_d || !workspace_d) return PT_ERR_NULL;
   if (workspace_bytes < 256 + (size_t)(p->n_slices + 1) * sizeof(float)) return PT_ERR_WORKSPACE;
   float* alpha = (float*)((char*)workspace_d + 256);
@@ -1250,6 +1328,11 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
   LAUNCH_CHECK(K_lsqml_alpha, st);
   if (object_d && grad_object_d) {
     if (!illum_prev_d) return PT_ERR_NULL;
+    if (u->mode == PT_UPDATE_LSQML_WEIGHTED) {
+      if (!u->illum_batch_d) return PT_ERR_NULL;
+      k_lsqml_object_weighted<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, u->illum_batch_d,
+                                                                           u->illum_batch_d + on, u->beta_obj, p->lsqml_delta_o, on);
+    } else
     k_lsqml_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, alpha, u->beta_obj, p->lsqml_delta_o, os, on);
     LAUNCH_CHECK(K_lsqml_object, st);
   }

@@ -18,8 +18,8 @@ LIB_PATH = os.path.join(_HERE, "libptycho_b200.so")
 
 LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
-WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE = 1, 2, 4, 16, 32
-UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE = 0, 1, 2
+WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLUM = 1, 2, 4, 16, 32, 64
+UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE, UPDATE_LSQML_WEIGHTED = 0, 1, 2, 3
 OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
            "ptycho_apply_update", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
@@ -47,12 +47,13 @@ class PtProblem(C.Structure):
         ("slice_thickness", C.POINTER(C.c_float)), ("tilt_x_mrad", C.c_float), ("tilt_y_mrad", C.c_float),
         ("bandlimit", C.c_float), ("loss", C.c_int32), ("loss_c", C.c_float), ("eps", C.c_float),
         ("shift_mode", C.c_int32), ("flags", C.c_int32), ("lsqml_delta_o", C.c_float), ("lsqml_delta_p", C.c_float),
+        ("lsqml_gamma", C.c_float),
     ]
 
 
 class PtUpdate(C.Structure):
     _fields_ = [("mode", C.c_int32), ("lr_obj", C.c_float), ("lr_probe", C.c_float), ("lr_pos", C.c_float),
-                ("beta_obj", C.c_float), ("beta_probe", C.c_float), ("gamma", C.c_float)]
+                ("beta_obj", C.c_float), ("beta_probe", C.c_float), ("gamma", C.c_float), ("illum_batch_d", C.c_void_p)]
 
 
 _lib = None
@@ -103,6 +104,7 @@ class Problem:
     shift_mode: int = SHIFT_FOURIER_PROBE
     lsqml_delta_o: float = 1.0
     lsqml_delta_p: float = 0.0
+    lsqml_gamma: float = 0.0
 
     def c_struct(self, n_pos_total: int, n_batch: int, flags: int = 0) -> PtProblem:
         dz = list(self.slice_thickness) + [0.0] * max(0, self.n_slices - len(self.slice_thickness))
@@ -110,7 +112,7 @@ class Problem:
         s = PtProblem(self.n, self.n_modes, self.n_slices, self.obj_ny, self.obj_nx, n_pos_total, n_batch,
                       self.pixel_size, self.wavelength, C.cast(arr, C.POINTER(C.c_float)), self.tilt_x_mrad,
                       self.tilt_y_mrad, self.bandlimit, self.loss, self.loss_c, self.eps, self.shift_mode, flags,
-                      self.lsqml_delta_o, self.lsqml_delta_p)
+                      self.lsqml_delta_o, self.lsqml_delta_p, self.lsqml_gamma)
         s._keep = arr
         return s
 
@@ -204,13 +206,14 @@ def gradient(pb: Problem, obj, probe, positions, intensity, batch_idx=None, *, w
 
 def apply_update(pb: Problem, obj=None, probe=None, positions=None, *, grad_object=None, grad_probe=None, grad_pos=None,
                  illum_prev=None, step_terms=None, batch_idx=None, n_batch: Optional[int] = None, mode=UPDATE_SGD,
-                 lr_obj=0.0, lr_probe=0.0, lr_pos=0.0, beta_obj=1.0, beta_probe=1.0, gamma=0.0, workspace=None):
-    """ptycho_apply_update (in place)."""
+                 lr_obj=0.0, lr_probe=0.0, lr_pos=0.0, beta_obj=1.0, beta_probe=1.0, gamma=0.0, workspace=None, illum_batch=None):
+    """ptycho_apply_update (in place). illum_batch: the [2][S][ny][nx] (I, W) planes of WANT_WEIGHTED_ILLUM (UPDATE_LSQML_WEIGHTED)."""
     import torch
     npos = positions.shape[0] if positions is not None else (n_batch or 1)
     J = batch_idx.numel() if batch_idx is not None else (n_batch if n_batch is not None else npos)
     cs = pb.c_struct(max(npos, J), J, 0)
-    u = PtUpdate(mode, lr_obj, lr_probe, lr_pos, beta_obj, beta_probe, gamma)
+    ib = _dev(illum_batch, torch.float32, "illum_batch")
+    u = PtUpdate(mode, lr_obj, lr_probe, lr_pos, beta_obj, beta_probe, gamma, None if ib is None else ib.data_ptr())
     _check(lib().ptycho_apply_update(C.byref(cs), _ptr(_dev(obj, torch.complex64, "obj")), _ptr(_dev(probe, torch.complex64, "probe")),
                                      _ptr(_dev(positions, torch.float32, "positions")), _ptr(_dev(grad_object, torch.complex64, "grad_object")),
                                      _ptr(_dev(grad_probe, torch.complex64, "grad_probe")), _ptr(_dev(grad_pos, torch.float32, "grad_pos")),

@@ -52,7 +52,13 @@ def test_struct_layout_matches_header(lib):
         first = [n for n in names if n not in ("const", "int32_t", "float")]
         fields += [f.strip(",") for f in first]
     assert fields == [f[0] for f in ptycho.PtProblem._fields_]
-    assert C.sizeof(ptycho.PtProblem) == 88
+    assert C.sizeof(ptycho.PtProblem) == 96
+    # pt_update: seven 4-byte scalars, then the device pointer of PT_UPDATE_LSQML_WEIGHTED (8-byte aligned)
+    ub = hdr[:hdr.index("} pt_update;")]
+    ub = re.sub(r"/\*.*?\*/", "", ub[ub.rindex("typedef struct {") + len("typedef struct {"):], flags=re.S)
+    unames = [n.strip(",") for d in ub.split(";") for n in d.replace("*", " ").split() if n not in ("const", "int32_t", "float")]
+    assert unames == [f[0] for f in ptycho.PtUpdate._fields_]
+    assert C.sizeof(ptycho.PtUpdate) == 40 and ptycho.PtUpdate.illum_batch_d.offset == 32
 
 
 def test_validation_and_workspace_sizes(lib):

@@ -578,3 +578,57 @@ def test_epie_iterations_reconstruct_config1():
     a, b_ = rec[sl] - rec[sl].mean(), tru[sl] - tru[sl].mean()
     corr = float((a * b_).sum() / np.sqrt((a * a).sum() * (b_ * b_).sum()))
     assert corr > 0.95, corr
+
+
+# ------------------------------------------------------------------------------------------------
+# LSQML slice update with per-position step sizes, PAPER.md:225 as printed (reading R24): weighted illumination map W
+# (plane 1 of illum_d under PT_WANT_WEIGHTED_ILLUM) and PT_UPDATE_LSQML_WEIGHTED, against the oracle; whole batch in
+# flight, chunked second sweep, and the N = 256 cluster geometry
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg5", "cfg5_chunked", "n256"])
+def test_lsqml_weighted_update_per_position_alpha(which):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    if which == "n256":
+        cfg = synth.config(4, scan=(2, 3), n_modes=2, n_slices=3, obj_n=300)
+    else:
+        cfg = synth.config(5, scan=(4, 5), n_modes=4, n_slices=6)
+    gamma = 1e-3
+    case = make_case(cfg, start_scale=0.8)
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbo, pbg = oracle_problem(cfg, **kw), gpu_problem(cfg, lsqml_gamma=gamma, **kw)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    illum_prev = (o["illum"] * 0.9).astype(np.float32)
+    J, S = cfg.n_pos, cfg.n_slices
+    st_o = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev)
+    W_o = orc.weighted_illum(pbo, case.obj_start, case.probe, case.positions, st_o, gamma)
+    o_new = orc.lsqml_weighted_object(pbo, case.obj_start, o["grad_object"], illum_prev, o["illum"], W_o, beta_obj=0.9)
+    obj_d, pr_d, pos_d, I_d, ip_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity), _t(illum_prev)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d)
+    il = torch.full((2,) + tuple(obj_d.shape), float("nan"), dtype=torch.float32, device="cuda")
+    st = torch.empty((J, 2 * S + 6), dtype=torch.float32, device="cuda")
+    fl = ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES | ptycho.WANT_WEIGHTED_ILLUM
+    max_ws = None
+    if which == "cfg5_chunked":
+        min_ws = ptycho.workspace_bytes(pbg, J, J, fl, minimum=True); full_ws = ptycho.workspace_bytes(pbg, J, J, fl)
+        max_ws = min_ws + (full_ws - min_ws) * 6 // 19 + 4096
+    ws = ptycho.make_workspace(pbg, J, J, fl, max_bytes=max_ws)
+    if which == "cfg5_chunked":
+        assert ptycho.positions_in_flight(pbg, J, J, fl, ws.numel()) < J
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum=il, illum_prev=ip_d,
+                    step_terms=st, flags=fl)
+    assert ptycho.status(ws) == 0
+    ilg = il.cpu().numpy()
+    assert rel_l2(ilg[0], o["illum"]) <= TOL_GRAD
+    assert rel_l2(ilg[1], W_o) <= 3e-4          # alphas are ratios of fp32 step terms (each within 3e-4 of the oracle's)
+    ptycho.apply_update(pbg, obj_d, grad_object=gO, illum_prev=ip_d, step_terms=st, n_batch=J, mode=ptycho.UPDATE_LSQML_WEIGHTED,
+                        beta_obj=0.9, gamma=gamma, workspace=ws, illum_batch=il)
+    torch.cuda.synchronize()
+    d_g, d_o = obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start
+    assert rel_l2(d_g, d_o) <= 5e-4
+    cov = o["illum"] > 0
+    assert np.all(d_g[~cov] == 0)               # pixels no window covers are left alone
+    # flag combinations the header rules out
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum=il,
+                        flags=ptycho.WANT_WEIGHTED_ILLUM)
