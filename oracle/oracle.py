@@ -230,17 +230,18 @@ def gradient(pb: Problem, obj, probe, positions, intensity, batch_idx=None, want
     return dict(loss=loss.value, loss_per_pos=lpp, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il)
 
 
-def step_terms(pb: Problem, obj, probe, positions, intensity, grad_object, grad_probe, illum_prev, batch_idx=None):
+def step_terms(pb: Problem, obj, probe, positions, intensity, grad_object, grad_probe, illum_prev, batch_idx=None, probe_precond=None):
     """O13/O14. Returns [J][2S+6] float64."""
     obj = _c64(obj); probe = _c64(probe); positions = _f32(positions); inten = _f32(intensity)
     npos = positions.shape[0]; b, J = _batch(batch_idx, npos)
     cp = pb._c(npos, J)
     gO = np.ascontiguousarray(grad_object, np.complex128); gP = np.ascontiguousarray(grad_probe, np.complex128)
     ip = np.ascontiguousarray(illum_prev, np.float64)
+    pc = None if probe_precond is None else np.ascontiguousarray(probe_precond, np.float64)
     out = np.zeros((J, 2 * pb.n_slices + 6), np.float64)
     rc = lib().orc_step_terms(C.byref(cp), _p(obj, C.c_float), _p(probe, C.c_float), _p(positions, C.c_float),
                               _p(inten, C.c_float), _p(b, C.c_int32), _p(gO, C.c_double), _p(gP, C.c_double),
-                              _p(ip, C.c_double), _p(out, C.c_double))
+                              _p(ip, C.c_double), _p(pc, C.c_double), _p(out, C.c_double))
     if rc != 0:
         raise ValueError("oracle: window out of bounds")
     return out
@@ -248,7 +249,7 @@ def step_terms(pb: Problem, obj, probe, positions, intensity, grad_object, grad_
 
 def apply_update(pb: Problem, mode, obj, probe, positions, grad_object=None, grad_probe=None, grad_pos=None,
                  illum_prev=None, step_terms_=None, batch_idx=None, lr_obj=0.0, lr_probe=0.0, lr_pos=0.0,
-                 beta_obj=1.0, beta_probe=1.0, gamma=0.0):
+                 beta_obj=1.0, beta_probe=1.0, gamma=0.0, probe_precond=None):
     """O15/H15. Returns updated (object, probe, positions) as complex128/float64 copies."""
     o = np.array(obj, dtype=np.complex128, order="C"); pr = np.array(probe, dtype=np.complex128, order="C")
     x = np.array(positions, dtype=np.float64, order="C")
@@ -256,12 +257,24 @@ def apply_update(pb: Problem, mode, obj, probe, positions, grad_object=None, gra
     cp = pb._c(npos, J)
     f = lambda a, t: None if a is None else np.ascontiguousarray(a, t)
     gO = f(grad_object, np.complex128); gP = f(grad_probe, np.complex128); gX = f(grad_pos, np.float64)
-    ip = f(illum_prev, np.float64); st = f(step_terms_, np.float64)
+    ip = f(illum_prev, np.float64); st = f(step_terms_, np.float64); pc = f(probe_precond, np.float64)
     lib().orc_apply_update(C.byref(cp), int(mode), _p(o, C.c_double), _p(pr, C.c_double), _p(x, C.c_double),
                            _p(gO, C.c_double), _p(gP, C.c_double), _p(gX, C.c_double), _p(ip, C.c_double),
                            _p(st, C.c_double), _p(b, C.c_int32), C.c_double(lr_obj), C.c_double(lr_probe),
-                           C.c_double(lr_pos), C.c_double(beta_obj), C.c_double(beta_probe), C.c_double(gamma))
+                           C.c_double(lr_pos), C.c_double(beta_obj), C.c_double(beta_probe), C.c_double(gamma), _p(pc, C.c_double))
     return o, pr, x
+
+
+def object_transparency(pb: Problem, obj, positions, batch_idx=None):
+    """sum_j prod_i |O_i|^2 in the probe/cutout view, [N][N] (reading R25)."""
+    obj = _c64(obj); positions = _f32(positions)
+    npos = positions.shape[0]; b, J = _batch(batch_idx, npos)
+    cp = pb._c(npos, J)
+    out = np.zeros((pb.n, pb.n), np.float64)
+    rc = lib().orc_object_transparency(C.byref(cp), _p(obj, C.c_float), _p(positions, C.c_float), _p(b, C.c_int32), _p(out, C.c_double))
+    if rc != 0:
+        raise ValueError("oracle: window out of bounds")
+    return out
 
 
 def weighted_illum(pb: Problem, obj, probe, positions, step_terms_, gamma, batch_idx=None):

@@ -559,6 +559,7 @@ int32_t orc_gradient(const orc_problem* p, const float* object, const float* pro
 int32_t orc_step_terms(const orc_problem* p, const float* object, const float* probe,
                        const float* positions, const float* intensity, const int32_t* batch_idx,
                        const double* grad_object, const double* grad_probe, const double* illum_prev,
+                       const double* probe_precond /* [N][N] or NULL: constant 1 (R19), reading R25 */,
                        double* step_terms) {
   if (p->shift_mode == 1) return -2;                                            // step terms: Fourier-shift mode only
   Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
@@ -569,7 +570,8 @@ int32_t orc_step_terms(const orc_problem* p, const float* object, const float* p
     dOhat[o] = -cd(grad_object[2 * o], grad_object[2 * o + 1]) / (illum_prev[o] + (double)p->lsqml_delta_o);
   std::vector<std::vector<cd>> dPhat_t(M, std::vector<cd>(NN));                 // F(dPhat_k)
   for (int k = 0; k < M; ++k) {
-    for (long r = 0; r < NN; ++r) dPhat_t[k][r] = -cd(grad_probe[2 * (k * NN + r)], grad_probe[2 * (k * NN + r) + 1]) / ((double)p->lsqml_delta_p + 1.0);
+    for (long r = 0; r < NN; ++r)
+      dPhat_t[k][r] = -cd(grad_probe[2 * (k * NN + r)], grad_probe[2 * (k * NN + r) + 1]) / ((probe_precond ? probe_precond[r] : 1.0) + (double)p->lsqml_delta_p);
     F2(N, dPhat_t[k].data());
   }
   int err = 0; const int W = 2 * S + 6;
@@ -635,7 +637,7 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
                          const double* grad_object, const double* grad_probe, const double* grad_pos,
                          const double* illum_prev, const double* step_terms, const int32_t* batch_idx,
                          double lr_obj, double lr_probe, double lr_pos, double beta_obj, double beta_probe,
-                         double gamma) {
+                         double gamma, const double* probe_precond /* [N][N] or NULL, as in orc_step_terms */) {
   const int J = p->n_batch, M = p->n_modes, S = p->n_slices; const long NN = (long)p->n * p->n;
   const long os = (long)p->obj_ny * p->obj_nx;
   if (mode == 0) {
@@ -662,7 +664,8 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
     double num = 0, den = 0;
     for (int jb = 0; jb < J; ++jb) { num += step_terms[(long)jb * W + 2 * S]; den += step_terms[(long)jb * W + 2 * S + 1]; }
     double alpha = num / (den + gamma);
-    for (long r = 0; r < 2 * M * NN; ++r) probe[r] += beta_probe * alpha * (-grad_probe[r] / ((double)p->lsqml_delta_p + 1.0));
+    for (long r = 0; r < 2 * M * NN; ++r)
+      probe[r] += beta_probe * alpha * (-grad_probe[r] / ((probe_precond ? probe_precond[(r / 2) % NN] : 1.0) + (double)p->lsqml_delta_p));
   }
   if (positions)
     for (int jb = 0; jb < J; ++jb) { int row = batch_idx ? batch_idx[jb] : jb;
@@ -670,6 +673,34 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
         double num = step_terms[(long)jb * W + 2 * S + 2 + 2 * a], den = step_terms[(long)jb * W + 2 * S + 3 + 2 * a];
         positions[2 * row + a] += (double)p->pixel_size * num / (den + gamma);
       } }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// LSQML probe preconditioner (reading R25): "the summed object intensity sum prod_i |O_i|^2 is recorded in
+// the probe/cutout view": objtrans[r] = sum_{j in group} prod_i |O_i[r0_j + r]|^2, r in the N x N window.  The caller
+// keeps the running sum over an iteration and hands last iteration's total back as probe_precond (like illum_prev).
+// ------------------------------------------------------------------------------------------
+int32_t orc_object_transparency(const orc_problem* p, const float* object, const float* positions, const int32_t* batch_idx,
+                                double* objtrans /* [N][N] */) {
+  const int N = p->n, S = p->n_slices, J = p->n_batch;
+  for (long r = 0; r < (long)N * N; ++r) objtrans[r] = 0.0;
+  for (int jb = 0; jb < J; ++jb) {
+    const int jrow = batch_idx ? batch_idx[jb] : jb;
+    int32_t r0y, r0x; float dy, dx;
+    orc_position_split(positions[2 * jrow + 0], p->pixel_size, N, &r0y, &dy);
+    orc_position_split(positions[2 * jrow + 1], p->pixel_size, N, &r0x, &dx);
+    if (r0y < 0 || r0x < 0 || r0y + N > p->obj_ny || r0x + N > p->obj_nx) return -1;
+    for (int y = 0; y < N; ++y)
+      for (int x = 0; x < N; ++x) {
+        double t = 1.0;
+        for (int i = 0; i < S; ++i) {
+          const long o = ((long)i * p->obj_ny + (r0y + y)) * p->obj_nx + (r0x + x);
+          t *= (double)object[2 * o] * object[2 * o] + (double)object[2 * o + 1] * object[2 * o + 1];
+        }
+        objtrans[(long)y * N + x] += t;
+      }
+  }
   return 0;
 }
 
