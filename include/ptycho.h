@@ -75,6 +75,9 @@ typedef struct {
   float lsqml_delta_o;            /* delta_O of PAPER.md:219 (PT_WANT_STEP_SIZES only)                          */
   float lsqml_delta_p;            /* probe analogue: dPhat = -gP / (delta_p + 1) (R19)                          */
   float lsqml_gamma;              /* gamma of PAPER.md:221 in the per-position alphas (PT_WANT_WEIGHTED_ILLUM only) */
+  const float *lsqml_probe_precond_d; /* DEVICE [N][N] or NULL: probe preconditioner of PAPER.md:227 (R25), last iteration's
+                                   * sum of ptycho_object_transparency maps: dPhat_k = -gP_k / (precond + delta_p), in the
+                                   * step-size sweep and in PT_UPDATE_LSQML*; NULL: the constant 1 (R19)              */
 } pt_problem;
 
 enum { PT_UPDATE_SGD = 0, PT_UPDATE_LSQML = 1, PT_UPDATE_EPIE = 2, PT_UPDATE_LSQML_WEIGHTED = 3 };
@@ -147,6 +150,14 @@ int32_t ptycho_apply_update(const pt_problem *p, pt_c64 *object_d, pt_c64 *probe
                             const pt_c64 *grad_object_d, const pt_c64 *grad_probe_d, const float *grad_pos_d,
                             const float *illum_prev_d, const float *step_terms_d, const int32_t *batch_idx_d,
                             const pt_update *u, void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* LSQML probe preconditioner ("summed object intensity ... recorded in the probe/cutout view"; R25):
+ *   objtrans_d [N][N] float <- (PT_ACCUMULATE: +=) sum_{j in batch} prod_i |O_i[r0_j + r]|^2, integer windows of R2
+ * (PT_SHIFT_FOURIER_PROBE only, else PT_ERR_UNSUPPORTED).  Fixed summation order.  workspace_d: any workspace of this
+ * problem (only the status word is touched: PT_ERR_OUT_OF_BOUNDS is deferred as in ptycho_forward_loss). */
+int32_t ptycho_object_transparency(const pt_problem *p, const pt_c64 *object_d, const float *positions_d,
+                                   const int32_t *batch_idx_d, float *objtrans_d, void *workspace_d, size_t workspace_bytes,
+                                   void *cuda_stream);
 
 /* End-to-end convenience with HOST buffers (pinned memory recommended): copies object/probe/positions and the
  * batch rows' intensities host->device into the workspace, runs ptycho_gradient, copies gradients and loss

@@ -274,7 +274,7 @@ __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wai
 // in = raster grad_probe, scale = -1 / (delta_p + 1)).  One CTA (CL = 4: one cluster) per mode.
 // ------------------------------------------------------------------------------------------------
 template <class G>
-__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* in, cf* out, float scale) {
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* in, cf* out, float scale, const float* precond, float delta_p) {
   typedef Lay<G> L; typedef FL<G> F;
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x, k = blockIdx.x / G::CL;
@@ -285,7 +285,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_probe_fft(const cf* i
   cf v[32];
   const cf* src = in + (size_t)k * F::NNF;
 #pragma unroll
-  for (int r = 0; r < 32; ++r) v[r] = cscale(src[F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r)], scale);
+  for (int r = 0; r < 32; ++r) {
+    const int pix = F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r);
+    // step-size sweep with the probe-view preconditioner (R25): dPhat = -gP / (precond + delta_p)
+    v[r] = cscale(src[pix], precond ? -1.0f / (precond[pix] + delta_p) : scale);
+  }
   Fft<G>::fwd(v, cs.sm, cs.tw, cs.tw2, t, rk);
   cf* dst = out + ((size_t)k * G::CL + rk) * F::NNS;
 #pragma unroll
@@ -883,6 +887,41 @@ __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
   }
 }
 
+// ------------------------------------------------------------------------------------------------
+// LSQML probe preconditioner (R25): objtrans[r] = sum_j prod_i |O_i[r0_j + r]|^2, one thread per window pixel,
+// positions in fixed order, fp64.  The position split is the fp32 arithmetic of k_setup_pos (R2), clamped + flagged (R4).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) k_objtrans(KP P, float* out, int accumulate) {
+  __shared__ int2 sr0[256];
+  const int N = P.N, e = blockIdx.x * 256 + threadIdx.x, y = e / N, x = e - y * N;
+  double acc = 0.0;
+  for (int jbase = 0; jbase < P.J; jbase += 256) {
+    const int cnt = min(256, P.J - jbase);
+    if ((int)threadIdx.x < cnt) {
+      const int jb = jbase + threadIdx.x, row = P.batch_idx ? P.batch_idx[jb] : jb;
+      int r0[2];
+#pragma unroll
+      for (int a = 0; a < 2; ++a) {
+        const float c = __fsub_rn(__fdiv_rn(P.positions[2 * row + a], P.px), (float)(N / 2));
+        int r = (int)floorf(__fadd_rn(c, 0.5f));
+        const int lim = (a == 0 ? P.ony : P.onx) - N;
+        if (r < 0 || r > lim) { atomicOr(P.w.status, kStatusOOB); r = r < 0 ? 0 : lim; }
+        r0[a] = r;
+      }
+      sr0[threadIdx.x] = make_int2(r0[1], r0[0]);
+    }
+    __syncthreads();
+    for (int jj = 0; jj < cnt; ++jj) {
+      const cf* o = P.object + ((size_t)(sr0[jj].y + y)) * P.onx + sr0[jj].x + x;
+      float tr = 1.0f;
+      for (int i = 0; i < P.S; ++i) { const cf z = o[(size_t)i * P.ony * P.onx]; tr *= fmaf(z.x, z.x, z.y * z.y); }
+      acc += (double)tr;
+    }
+    __syncthreads();
+  }
+  out[e] = (float)((accumulate ? (double)out[e] : 0.0) + acc);
+}
+
 // H12: gP~_k[q] += sum_j (chunk) conj(R_j) G~_{k,j}[q], fixed order, fp64
 __global__ void k_reduce_probe(KP P) {
   const int NN = P.N * P.N;
@@ -985,10 +1024,10 @@ __global__ void k_lsqml_object_weighted(cf* O, const cf* gO, const float* illum_
   const float a = beta * (willum[i] / ib) * (-1.0f / (illum_prev[i] + delta_o));
   O[i] = make_float2(fmaf(a, gO[i].x, O[i].x), fmaf(a, gO[i].y, O[i].y));
 }
-__global__ void k_lsqml_probe(cf* Pr, const cf* gP, const float* alpha, int S, float beta, float delta_p, size_t n) {
+__global__ void k_lsqml_probe(cf* Pr, const cf* gP, const float* alpha, int S, float beta, float delta_p, const float* precond, size_t NN, size_t n) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i >= n) return;
-  const float a = beta * alpha[S] * (-1.0f / (delta_p + 1.0f));
+  const float a = beta * alpha[S] * (-1.0f / ((precond ? precond[i % NN] : 1.0f) + delta_p));
   Pr[i] = make_float2(fmaf(a, gP[i].x, Pr[i].x), fmaf(a, gP[i].y, Pr[i].y));
 }
 __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* idx, int J, int S, float px, float gamma) {
@@ -1007,11 +1046,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans"};
 thread_local int64_t g_launches = 0;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
@@ -1104,7 +1143,7 @@ int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
   }
   k_setup_pos<<<p->n_batch, p->n, 0, st>>>(kp);
   LAUNCH_CHECK(K_setup_pos, st);
-  launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f);
+  launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f, (const float*)nullptr, 0.0f);
   LAUNCH_CHECK(K_probe_fft, st);
   return PT_OK;
 }
@@ -1187,7 +1226,8 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     // H14 second sweep (O13/O14): needs the batch-aggregated gO, gP
     k_dohat<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((const cf*)gO, illum_prev, p->lsqml_delta_o, kp.w.dOhat, on);
     LAUNCH_CHECK(K_dohat, st);
-    launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f));
+    launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f),
+               p->lsqml_probe_precond_d, p->lsqml_delta_p);
     LAUNCH_CHECK(K_probe_fft, st);
     for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
@@ -1337,13 +1377,30 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
     LAUNCH_CHECK(K_lsqml_object, st);
   }
   if (probe_d && grad_probe_d) {
-    k_lsqml_probe<<<(unsigned)((pn + 255) / 256), 256, 0, st>>>((cf*)probe_d, (const cf*)grad_probe_d, alpha, p->n_slices, u->beta_probe, p->lsqml_delta_p, pn);
+    k_lsqml_probe<<<(unsigned)((pn + 255) / 256), 256, 0, st>>>((cf*)probe_d, (const cf*)grad_probe_d, alpha, p->n_slices, u->beta_probe, p->lsqml_delta_p, p->lsqml_probe_precond_d, NN, pn);
     LAUNCH_CHECK(K_lsqml_probe, st);
   }
   if (positions_d) {
     k_lsqml_pos<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, step_terms_d, batch_idx_d, p->n_batch, p->n_slices, p->pixel_size, u->gamma);
     LAUNCH_CHECK(K_lsqml_pos, st);
   }
+  return PT_OK;
+}
+
+int32_t ptycho_object_transparency(const pt_problem* p, const pt_c64* object_d, const float* positions_d, const int32_t* batch_idx_d,
+                                   float* objtrans_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!object_d || !positions_d || !objtrans_d || !workspace_d) return PT_ERR_NULL;
+  if (p->shift_mode != PT_SHIFT_FOURIER_PROBE) return PT_ERR_UNSUPPORTED;
+  if (workspace_bytes < 256) return PT_ERR_WORKSPACE;
+  Ws w; memset(&w, 0, sizeof(w));
+  w.status = (int32_t*)workspace_d;
+  KP kp = make_kp(p, w, object_d, nullptr, positions_d, nullptr, batch_idx_d);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  k_objtrans<<<p->n * p->n / 256, 256, 0, st>>>(kp, objtrans_d, (p->flags & PT_ACCUMULATE) ? 1 : 0);
+  LAUNCH_CHECK(K_objtrans, st);
   return PT_OK;
 }
 

@@ -22,7 +22,7 @@ WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLU
 UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE, UPDATE_LSQML_WEIGHTED = 0, 1, 2, 3
 OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
-           "ptycho_apply_update", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
+           "ptycho_apply_update", "ptycho_object_transparency", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
            "ptycho_launch_count", "ptycho_strerror", "ptycho_profile_enable", "ptycho_profile_num_kernels",
            "ptycho_profile_kernel_name", "ptycho_profile_read"]
 
@@ -47,7 +47,7 @@ class PtProblem(C.Structure):
         ("slice_thickness", C.POINTER(C.c_float)), ("tilt_x_mrad", C.c_float), ("tilt_y_mrad", C.c_float),
         ("bandlimit", C.c_float), ("loss", C.c_int32), ("loss_c", C.c_float), ("eps", C.c_float),
         ("shift_mode", C.c_int32), ("flags", C.c_int32), ("lsqml_delta_o", C.c_float), ("lsqml_delta_p", C.c_float),
-        ("lsqml_gamma", C.c_float),
+        ("lsqml_gamma", C.c_float), ("lsqml_probe_precond_d", C.c_void_p),
     ]
 
 
@@ -72,7 +72,8 @@ def lib():
         l.ptycho_launch_count.restype = C.c_int64
         l.ptycho_strerror.restype = C.c_char_p
         l.ptycho_profile_kernel_name.restype = C.c_char_p
-        for f in ("ptycho_forward_loss", "ptycho_gradient", "ptycho_apply_update", "ptycho_gradient_host", "ptycho_status"):
+        for f in ("ptycho_forward_loss", "ptycho_gradient", "ptycho_apply_update", "ptycho_gradient_host", "ptycho_status",
+                  "ptycho_object_transparency"):
             getattr(l, f).restype = C.c_int32
         _lib = l
     return _lib
@@ -105,6 +106,7 @@ class Problem:
     lsqml_delta_o: float = 1.0
     lsqml_delta_p: float = 0.0
     lsqml_gamma: float = 0.0
+    lsqml_probe_precond: object = None      # CUDA float32 [N][N] tensor or None (include/ptycho.h)
 
     def c_struct(self, n_pos_total: int, n_batch: int, flags: int = 0) -> PtProblem:
         dz = list(self.slice_thickness) + [0.0] * max(0, self.n_slices - len(self.slice_thickness))
@@ -112,9 +114,17 @@ class Problem:
         s = PtProblem(self.n, self.n_modes, self.n_slices, self.obj_ny, self.obj_nx, n_pos_total, n_batch,
                       self.pixel_size, self.wavelength, C.cast(arr, C.POINTER(C.c_float)), self.tilt_x_mrad,
                       self.tilt_y_mrad, self.bandlimit, self.loss, self.loss_c, self.eps, self.shift_mode, flags,
-                      self.lsqml_delta_o, self.lsqml_delta_p, self.lsqml_gamma)
+                      self.lsqml_delta_o, self.lsqml_delta_p, self.lsqml_gamma,
+                      None if self.lsqml_probe_precond is None else _precond_ptr(self.lsqml_probe_precond))
         s._keep = arr
         return s
+
+
+def _precond_ptr(t):
+    import torch
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("lsqml_probe_precond: expected a contiguous CUDA float32 tensor")
+    return t.data_ptr()
 
 
 def _ptr(t):
@@ -220,6 +230,17 @@ def apply_update(pb: Problem, obj=None, probe=None, positions=None, *, grad_obje
                                      _ptr(_dev(illum_prev, torch.float32, "illum_prev")), _ptr(_dev(step_terms, torch.float32, "step_terms")),
                                      _ptr(_dev(batch_idx, torch.int32, "batch_idx")), C.byref(u), _ptr(workspace),
                                      C.c_size_t(0 if workspace is None else workspace.numel()), _stream()))
+
+
+def object_transparency(pb: Problem, obj, positions, batch_idx=None, *, out, workspace, flags: int = 0):
+    """ptycho_object_transparency: out [N][N] float32 <- sum_j prod_i |O_i|^2 in the probe view."""
+    import torch
+    obj = _dev(obj, torch.complex64, "obj"); positions = _dev(positions, torch.float32, "positions")
+    batch_idx = _dev(batch_idx, torch.int32, "batch_idx")
+    npos = positions.shape[0]; J = npos if batch_idx is None else batch_idx.numel()
+    cs = pb.c_struct(npos, J, flags)
+    _check(lib().ptycho_object_transparency(C.byref(cs), _ptr(obj), _ptr(positions), _ptr(batch_idx), _ptr(_dev(out, torch.float32, "out")),
+                                            _ptr(workspace), C.c_size_t(workspace.numel()), _stream()))
 
 
 def gradient_host(pb: Problem, obj_h, probe_h, positions_h, intensity_h, batch_idx_h=None, *, workspace, grad_object_h,

@@ -52,7 +52,7 @@ def test_struct_layout_matches_header(lib):
         first = [n for n in names if n not in ("const", "int32_t", "float")]
         fields += [f.strip(",") for f in first]
     assert fields == [f[0] for f in ptycho.PtProblem._fields_]
-    assert C.sizeof(ptycho.PtProblem) == 96
+    assert C.sizeof(ptycho.PtProblem) == 104
     # pt_update: seven 4-byte scalars, then the device pointer of PT_UPDATE_LSQML_WEIGHTED (8-byte aligned)
     ub = hdr[:hdr.index("} pt_update;")]
     ub = re.sub(r"/\*.*?\*/", "", ub[ub.rindex("typedef struct {") + len("typedef struct {"):], flags=re.S)

@@ -632,3 +632,63 @@ def test_lsqml_weighted_update_per_position_alpha(which):
     with pytest.raises(ptycho.PtychoError):
         ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum=il,
                         flags=ptycho.WANT_WEIGHTED_ILLUM)
+
+
+# ------------------------------------------------------------------------------------------------
+# LSQML probe-view preconditioner (reading R25): ptycho_object_transparency, and the step-size terms and
+# probe update that divide by it
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg5", "n256"])
+def test_lsqml_probe_preconditioner(which):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(4, scan=(2, 3), n_modes=2, n_slices=3, obj_n=300) if which == "n256" else synth.config(5, scan=(4, 5), n_modes=4, n_slices=6)
+    case = make_case(cfg, start_scale=0.8)
+    J, S, n = cfg.n_pos, cfg.n_slices, cfg.n
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbo = oracle_problem(cfg, **kw)
+    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity)
+    fl = ptycho.WANT_STEP_SIZES
+    pbg0 = gpu_problem(cfg, **kw)
+    ws = ptycho.make_workspace(pbg0, J, J, fl)
+    # the map itself: whole batch, then two halves accumulated, bit-identical re-run
+    ot_o = orc.object_transparency(pbo, case.obj_start, case.positions)
+    ot = torch.full((n, n), float("nan"), dtype=torch.float32, device="cuda")
+    ptycho.object_transparency(pbg0, obj_d, pos_d, None, out=ot, workspace=ws)
+    assert ptycho.status(ws) == 0
+    assert rel_l2(ot.cpu().numpy(), ot_o) <= 1e-6
+    ot2 = torch.full((n, n), float("nan"), dtype=torch.float32, device="cuda")
+    half = J // 2
+    ptycho.object_transparency(pbg0, obj_d, pos_d, _t(np.arange(half, dtype=np.int32)), out=ot2, workspace=ws)
+    ptycho.object_transparency(pbg0, obj_d, pos_d, _t(np.arange(half, J, dtype=np.int32)), out=ot2, workspace=ws, flags=ptycho.ACCUMULATE)
+    assert rel_l2(ot2.cpu().numpy(), ot_o) <= 1e-6
+    ot3 = torch.empty_like(ot)
+    ptycho.object_transparency(pbg0, obj_d, pos_d, None, out=ot3, workspace=ws)
+    assert torch.equal(ot, ot3)
+    # step-size terms and the probe update with the preconditioner (last iteration's map: here 0.9 x this one)
+    pc = (0.9 * ot_o).astype(np.float32)
+    pc_d = _t(pc)
+    pbg = gpu_problem(cfg, lsqml_probe_precond=pc_d, **kw)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    illum_prev = (o["illum"] * 0.9).astype(np.float32)
+    st_o = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev,
+                          probe_precond=pc)
+    st_plain = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev)
+    assert rel_l2(st_plain[:, 2 * S], st_o[:, 2 * S]) > 1e-2           # the preconditioner does change the probe terms
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d)
+    st = torch.empty((J, 2 * S + 6), dtype=torch.float32, device="cuda")
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum_prev=_t(illum_prev), step_terms=st)
+    assert ptycho.status(ws) == 0
+    stg = st.cpu().numpy().astype(np.float64)
+    for c in range(2 * S + 6):
+        assert rel_l2(stg[:, c], st_o[:, c]) <= 3e-4, c
+    _, p_new, _ = orc.apply_update(pbo, 1, case.obj_start, case.probe, case.positions, None, o["grad_probe"], None, illum_prev, st_o,
+                                   beta_probe=0.8, gamma=1e-3, probe_precond=pc)
+    ptycho.apply_update(pbg, None, pr_d, None, grad_probe=gP, step_terms=st, n_batch=J, mode=ptycho.UPDATE_LSQML, beta_probe=0.8,
+                        gamma=1e-3, workspace=ws)
+    torch.cuda.synchronize()
+    assert rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe) <= 5e-4
+    # a window off the object raises the deferred flag
+    bad = case.positions.copy(); bad[0, 0] = -5.0
+    ptycho.object_transparency(pbg0, obj_d, _t(bad), None, out=ot3, workspace=ws)
+    assert ptycho.status(ws) == -6      # PT_ERR_OUT_OF_BOUNDS
