@@ -40,17 +40,19 @@ def parse():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--batch", type=int, default=0, help="config 5: mini-batch size of the LSQML sweep (0: sweep 64/256/1024/4096)")
+    ap.add_argument("--bandlimit", type=float, default=0.0, help="timed variant: sharp band-limit mask at this fraction of Nyquist "
+                    "inside the propagator (PAPER.md:117, reading R9); 0 = off, as in BASELINE.json's configs")
     ap.add_argument("--ws-gib", type=float, default=0.0, help="cap of the device workspace in GiB (0: library default)")
     return ap.parse_args()
 
 
-def workload(idx):
+def workload(idx, bandlimit=0.0):
     from paper_2505_14372_b200 import synth
-    cfg = synth.config(idx)
-    return cfg, dict(workload=f"BASELINE.json configs[{idx - 1}] ({cfg.name})", n=cfg.n, positions_per_gpu=cfg.n_pos, modes=cfg.n_modes,
+    cfg = synth.config(idx) if bandlimit <= 0 else synth.config(idx, bandlimit=bandlimit)
+    return cfg, dict(**({} if bandlimit <= 0 else {"variant": f"band-limited propagator, {bandlimit:g} x Nyquist"}), **dict(workload=f"BASELINE.json configs[{idx - 1}] ({cfg.name})", n=cfg.n, positions_per_gpu=cfg.n_pos, modes=cfg.n_modes,
                      slices=cfg.n_slices, object_px=cfg.obj_n, loss="poisson" if cfg.loss == synth.LOSS_POISSON else "amplitude",
                      start_state="O = exp((i-0.05) 0.8 phi_true), true probe, nominal positions",
-                     patterns="seeded closed-form stand-in + Poisson (synth.standin_patterns)")
+                     patterns="seeded closed-form stand-in + Poisson (synth.standin_patterns)"))
 
 
 def problem_kwargs(cfg):
@@ -162,7 +164,7 @@ def run_reference(args):
     if rank != 0:
         return
     from oracle import oracle as orc
-    cfg, conf = workload(args.config)
+    cfg, conf = workload(args.config, args.bandlimit)
     n = args.cpu_sample or {1: 256, 2: 64, 3: 16, 4: 4, 5: 16}[args.config]
     rows = np.arange(n)
     obj, pr, pos, inten = host_inputs(cfg, rows)
@@ -201,7 +203,7 @@ def run_b200(args):
     if world > 1:
         import torch.distributed as dist
         dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg, conf = workload(args.config)
+    cfg, conf = workload(args.config, args.bandlimit)
     J = cfg.n_pos
     obj_h, pr_h, pos_h, I_h = host_inputs(cfg)
     pbg = ptycho.Problem(**problem_kwargs(cfg))

@@ -302,5 +302,39 @@ def lsqml_weighted_object(pb: Problem, obj, grad_object, illum_prev, illum_batch
     return o
 
 
+REG_L2, REG_L1, REG_TIKHONOV, REG_TV, REG_LAYER_TIKHONOV, REG_LAYER_TV = range(6)
+CON_AMPLITUDE_CLAMP, CON_SUPPORT_MASK, CON_LAYER_BLUR, CON_LOWPASS = range(4)
+
+
+def cost_regularizer(kind, weight, field_, ref=1.0, eps=0.0, grad=None):
+    """Cost regulariser R (reading R26) of a [S][ny][nx] complex field; returns (R, grad + dR/dconj(field))."""
+    z = np.ascontiguousarray(field_, np.complex128); S, ny, nx = z.shape
+    g = np.zeros_like(z) if grad is None else np.array(grad, dtype=np.complex128, order="C")
+    f = lib().orc_cost_regularizer; f.restype = C.c_double
+    R = f(int(kind), C.c_double(weight), C.c_double(ref), C.c_double(eps), S, ny, nx, _p(z, C.c_double), _p(g, C.c_double))
+    return float(R), g
+
+
+def apply_constraint(kind, field_, a=0.0, b=0.0, mask=None):
+    """Constraint regulariser (reading R27) on a [S][ny][nx] complex field; returns the new field."""
+    z = np.array(field_, dtype=np.complex128, order="C"); S, ny, nx = z.shape
+    mk = None if mask is None else np.ascontiguousarray(mask, np.float64)
+    rc = lib().orc_apply_constraint(int(kind), C.c_double(a), C.c_double(b), _p(mk, C.c_double), S, ny, nx, _p(z, C.c_double))
+    if rc != 0:
+        raise ValueError(f"oracle: apply_constraint failed ({rc})")
+    return z
+
+
+def adam_update(z, g, m, v, lr, b1=0.9, b2=0.999, eps=1e-8, t=1):
+    """One Adam step (reading R28). Complex z: complex m, real v = EMA of |g|^2. Returns new (z, m, v) copies."""
+    cplx = np.iscomplexobj(z)
+    ty = np.complex128 if cplx else np.float64
+    z2 = np.array(z, dtype=ty, order="C"); m2 = np.array(m, dtype=ty, order="C"); v2 = np.array(v, dtype=np.float64, order="C")
+    g2 = np.ascontiguousarray(g, ty)
+    lib().orc_adam_update(int(cplx), _p(z2, C.c_double), _p(g2, C.c_double), _p(m2, C.c_double), _p(v2, C.c_double),
+                          C.c_int64(z2.size), C.c_double(lr), C.c_double(b1), C.c_double(b2), C.c_double(eps), int(t))
+    return z2, m2, v2
+
+
 def num_threads() -> int:
     return int(lib().orc_num_threads())

@@ -818,6 +818,130 @@ int32_t orc_epie(const orc_problem* p, const float* object, const float* probe, 
   return err;
 }
 
+// ------------------------------------------------------------------------------------------
+// Cost regularisers (the paper lists them by name only — reading R26).  field is [S][ny][nx] complex
+// (object slices, or probe modes with S = M); returns R and ADDS dR/dconj(field) into grad (dR = 2 Re sum conj(g) dz).
+//   kind 0  L2            R = w sum |z - ref|^2                      ("penalizes ... a non-vacuum object": ref = 1; probe: ref = 0)
+//   kind 1  L1            R = w sum sqrt(|z - ref|^2 + eps^2)       (smoothed modulus)
+//   kind 2  Tikhonov      R = w sum_{d in x,y} sum |D_d z|^2        (forward differences inside a slice, no wrap-around)
+//   kind 3  TV            R = w sum_{d in x,y} sum sqrt(|D_d z|^2 + eps^2)
+//   kind 4  layer Tikhonov, kind 5 layer TV: the same with the one difference along the depth axis, D_z z = z_{i+1} - z_i
+// ------------------------------------------------------------------------------------------
+static double reg_phi(int tv, double a2, double eps) { return tv ? std::sqrt(a2 + eps * eps) : a2; }
+static double reg_dphi(int tv, double a2, double eps) { return tv ? 0.5 / std::sqrt(a2 + eps * eps) : 1.0; }   // d phi / d(a2)
+
+double orc_cost_regularizer(int32_t kind, double weight, double ref, double eps, int32_t S, int32_t ny, int32_t nx,
+                            const double* field, double* grad) {
+  const long os = (long)ny * nx, n = (long)S * os;
+  auto Z = [&](long i) { return cd(field[2 * i], field[2 * i + 1]); };
+  auto addg = [&](long i, cd v) { grad[2 * i] += v.real(); grad[2 * i + 1] += v.imag(); };
+  double R = 0.0;
+  if (kind == 0 || kind == 1) {
+    for (long i = 0; i < n; ++i) {
+      cd u = Z(i) - ref; double a2 = std::norm(u);
+      R += weight * reg_phi(kind == 1, a2, eps);
+      addg(i, weight * reg_dphi(kind == 1, a2, eps) * u);              // d phi(|u|^2) / d conj(z) = phi' u
+    }
+    return R;
+  }
+  const int tv = (kind == 3 || kind == 5);
+  const long strides[3] = {1, (long)nx, os};
+  for (int d = 0; d < 3; ++d) {
+    if ((kind == 2 || kind == 3) && d == 2) continue;                  // in-plane kinds: x and y only
+    if ((kind == 4 || kind == 5) && d != 2) continue;                  // layer kinds: depth only
+    for (int s = 0; s < S; ++s)
+      for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) {
+          if ((d == 0 && x + 1 >= nx) || (d == 1 && y + 1 >= ny) || (d == 2 && s + 1 >= S)) continue;
+          long i = (long)s * os + (long)y * nx + x, j = i + strides[d];
+          cd u = Z(j) - Z(i); double a2 = std::norm(u);
+          R += weight * reg_phi(tv, a2, eps);
+          cd c = weight * reg_dphi(tv, a2, eps) * u;
+          addg(j, c); addg(i, -c);
+        }
+  }
+  return R;
+}
+
+// ------------------------------------------------------------------------------------------
+// Constraint regularisers (reading R27).  field [S][ny][nx] complex, in place.
+//   kind 0  amplitude clamp: |z| limited to [a, b], phase kept (a zero pixel with a > 0 becomes the real number a)
+//   kind 1  support mask:    z[s][y][x] *= mask[y][x]   (probe support in real space; mask [ny][nx] real)
+//   kind 2  layer blur:      Gaussian blur along the depth axis, sigma = a slices, REAL-SPACE convolution (the paper's
+//                            reason: no bleeding from top to bottom through periodic boundaries): out[p] = sum_t w_t z[p+t] /
+//                            sum_t w_t over the taps |t| <= ceil(4 sigma) that fall inside, w_t = exp(-t^2 / (2 sigma^2))
+//   kind 3  object low pass: the same blur along x then along y, sigma = a px
+// ------------------------------------------------------------------------------------------
+static void blur_axis(int S, int ny, int nx, int axis, double sigma, std::vector<cd>& z) {
+  const int R = (int)std::ceil(4.0 * sigma);
+  const long os = (long)ny * nx; const long stride = axis == 0 ? 1 : axis == 1 ? nx : os;
+  const int len = axis == 0 ? nx : axis == 1 ? ny : S;
+  std::vector<cd> out(z.size());
+  for (int s = 0; s < S; ++s)
+    for (int y = 0; y < ny; ++y)
+      for (int x = 0; x < nx; ++x) {
+        const long i = (long)s * os + (long)y * nx + x; const int c = axis == 0 ? x : axis == 1 ? y : s;
+        cd acc = 0.0; double wsum = 0.0;
+        for (int t = -R; t <= R; ++t) {
+          if (c + t < 0 || c + t >= len) continue;
+          double w = std::exp(-(double)t * t / (2.0 * sigma * sigma));
+          acc += w * z[i + (long)t * stride]; wsum += w;
+        }
+        out[i] = acc / wsum;
+      }
+  z.swap(out);
+}
+
+int32_t orc_apply_constraint(int32_t kind, double a, double b, const double* mask, int32_t S, int32_t ny, int32_t nx, double* field) {
+  const long os = (long)ny * nx, n = (long)S * os;
+  if (kind == 0) {
+    for (long i = 0; i < n; ++i) {
+      cd z(field[2 * i], field[2 * i + 1]); double m = std::abs(z);
+      double t = m < a ? a : (m > b ? b : m);
+      if (t == m) continue;
+      cd u = m > 0.0 ? z / m : cd(1.0, 0.0);
+      field[2 * i] = t * u.real(); field[2 * i + 1] = t * u.imag();
+    }
+    return 0;
+  }
+  if (kind == 1) {
+    for (long i = 0; i < n; ++i) { field[2 * i] *= mask[i % os]; field[2 * i + 1] *= mask[i % os]; }
+    return 0;
+  }
+  if (!(a > 0.0)) return -3;
+  std::vector<cd> z(n);
+  for (long i = 0; i < n; ++i) z[i] = cd(field[2 * i], field[2 * i + 1]);
+  if (kind == 2) blur_axis(S, ny, nx, 2, a, z);
+  else if (kind == 3) { blur_axis(S, ny, nx, 0, a, z); blur_axis(S, ny, nx, 1, a, z); }
+  else return -3;
+  for (long i = 0; i < n; ++i) { field[2 * i] = z[i].real(); field[2 * i + 1] = z[i].imag(); }
+  return 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// Adam ("SGD, Adam and its variants [62, 63]"; Kingma & Ba's algorithm 1; reading R28: for a complex variable
+// the first moment is complex and the second moment uses |g|^2, the complex-safe form of the library the paper names).
+//   m <- b1 m + (1 - b1) g ;  v <- b2 v + (1 - b2) |g|^2 ;  z <- z - lr (m / (1 - b1^t)) / (sqrt(v / (1 - b2^t)) + eps)
+// is_complex = 0: n real numbers (positions), |g|^2 = g^2.
+// ------------------------------------------------------------------------------------------
+int32_t orc_adam_update(int32_t is_complex, double* z, const double* g, double* m, double* v, int64_t n, double lr, double b1,
+                        double b2, double eps, int32_t t) {
+  const double c1 = 1.0 - std::pow(b1, (double)t), c2 = 1.0 - std::pow(b2, (double)t);
+  for (int64_t i = 0; i < n; ++i) {
+    if (is_complex) {
+      m[2 * i] = b1 * m[2 * i] + (1.0 - b1) * g[2 * i]; m[2 * i + 1] = b1 * m[2 * i + 1] + (1.0 - b1) * g[2 * i + 1];
+      v[i] = b2 * v[i] + (1.0 - b2) * (g[2 * i] * g[2 * i] + g[2 * i + 1] * g[2 * i + 1]);
+      const double d = std::sqrt(v[i] / c2) + eps;
+      z[2 * i] -= lr * (m[2 * i] / c1) / d; z[2 * i + 1] -= lr * (m[2 * i + 1] / c1) / d;
+    } else {
+      m[i] = b1 * m[i] + (1.0 - b1) * g[i];
+      v[i] = b2 * v[i] + (1.0 - b2) * g[i] * g[i];
+      z[i] -= lr * (m[i] / c1) / (std::sqrt(v[i] / c2) + eps);
+    }
+  }
+  return 0;
+}
+
 int32_t orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -751,3 +751,87 @@ def test_epie_multislice_invariants():
     r0y, dy = orc.position_split(float(pos1[0, 0]), 0.2, 8); r0x, dx = orc.position_split(float(pos1[0, 1]), 0.2, 8)
     Ps = orc.shift(probe1[0].astype(complex), dy, dx)
     assert np.abs(e["dir_object"] + 2.0 * g["grad_object"] / np.max(np.abs(Ps) ** 2)).max() < 1e-9 * np.abs(e["dir_object"]).max()
+
+
+# ------------------------------------------------------------------------------------------------
+# cost regularisers (R26), constraint regularisers (R27), Adam
+# (R28)
+# ------------------------------------------------------------------------------------------------
+def test_cost_regularizers_closed_forms_and_finite_differences():
+    S, ny, nx = 3, 5, 6
+    z = 1.0 + 0.3 * crandn(S, ny, nx)
+    # closed forms
+    R, g = orc.cost_regularizer(orc.REG_L2, 0.7, z, ref=1.0)
+    assert abs(R - 0.7 * np.sum(np.abs(z - 1) ** 2)) < 1e-12 and np.abs(g - 0.7 * (z - 1)).max() < 1e-14
+    assert orc.cost_regularizer(orc.REG_L2, 0.7, np.ones_like(z))[0] == 0.0               # vacuum costs nothing
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    ramp = np.broadcast_to(2.0 * x + 3.0j * y, (S, ny, nx))
+    assert abs(orc.cost_regularizer(orc.REG_TIKHONOV, 0.5, ramp)[0] - 0.5 * S * (4.0 * ny * (nx - 1) + 9.0 * (ny - 1) * nx)) < 1e-10
+    step = np.ones((S, ny, nx), complex); step[:, :, 3:] = 1.0 + 0.4j                     # one edge of height 0.4 per row
+    assert abs(orc.cost_regularizer(orc.REG_TV, 2.0, step, eps=0.0)[0] - 2.0 * S * ny * 0.4) < 1e-12
+    layers = np.stack([np.full((ny, nx), v) for v in (1.0, 1.5, 1.5 + 2j)])
+    assert abs(orc.cost_regularizer(orc.REG_LAYER_TIKHONOV, 1.0, layers)[0] - ny * nx * (0.25 + 4.0)) < 1e-12
+    assert abs(orc.cost_regularizer(orc.REG_LAYER_TV, 1.0, layers, eps=0.0)[0] - ny * nx * (0.5 + 2.0)) < 1e-12
+    assert abs(orc.cost_regularizer(orc.REG_L1, 3.0, layers, ref=1.0, eps=0.0)[0] - 3.0 * ny * nx * (0.0 + 0.5 + abs(0.5 + 2j))) < 1e-12
+    # Wirtinger gradient against central finite differences: dR = 2 Re sum conj(g) dz, for every kind; grad is ADDED into
+    for kind in range(6):
+        d = crandn(S, ny, nx); h = 1e-6; g0 = crandn(S, ny, nx)
+        R, g = orc.cost_regularizer(kind, 0.9, z, ref=1.0, eps=0.05, grad=g0)
+        Rp = orc.cost_regularizer(kind, 0.9, z + h * d, ref=1.0, eps=0.05)[0]
+        Rm = orc.cost_regularizer(kind, 0.9, z - h * d, ref=1.0, eps=0.05)[0]
+        assert abs((Rp - Rm) / (2 * h) - 2 * np.real(np.sum(np.conj(g - g0) * d))) < 1e-6 * max(1.0, abs(R)), kind
+
+
+def test_constraints_clamp_mask_blur():
+    S, ny, nx = 6, 9, 10
+    z = crandn(S, ny, nx)
+    c = orc.apply_constraint(orc.CON_AMPLITUDE_CLAMP, z, 0.5, 1.2)
+    assert np.abs(c).min() >= 0.5 - 1e-12 and np.abs(c).max() <= 1.2 + 1e-12
+    assert np.abs(np.angle(c * np.conj(z))).max() < 1e-12                                  # phase kept
+    inside = (np.abs(z) >= 0.5) & (np.abs(z) <= 1.2)
+    assert np.array_equal(c[inside], z[inside]) and inside.any() and (~inside).any()
+    mask = (RNG.uniform(size=(ny, nx)) > 0.4).astype(float)
+    assert np.array_equal(orc.apply_constraint(orc.CON_SUPPORT_MASK, z, mask=mask), z * mask[None])
+    # Gaussian blurs: constants are preserved up to the edges (no wrap-around, renormalised taps)
+    k = 2.0 - 1.5j
+    for kind, sig in ((orc.CON_LAYER_BLUR, 0.8), (orc.CON_LOWPASS, 1.1)):
+        assert np.abs(orc.apply_constraint(kind, np.full((S, ny, nx), k), sig) - k).max() < 1e-14
+    # interior delta response = normalised Gaussian taps; nothing leaks from the top layer to the bottom one
+    sig = 0.8; R = int(np.ceil(4 * sig)); w = np.exp(-np.arange(-R, R + 1) ** 2 / (2 * sig ** 2))
+    S2 = 2 * R + 3; d = np.zeros((S2, 2, 2), complex); d[R + 1] = 1.0
+    out = orc.apply_constraint(orc.CON_LAYER_BLUR, d, sig)
+    # row p of the blur matrix is w_{q-p} / (sum of the taps of p that fall inside): the column of the centre pixel
+    col = np.array([w[(R + 1 - p) + R] / sum(w[t + R] for t in range(-R, R + 1) if 0 <= p + t < S2) if abs(R + 1 - p) <= R else 0.0 for p in range(S2)])
+    assert np.abs(out[:, 0, 0] - col).max() < 1e-14
+    top = np.zeros((12, 1, 1), complex); top[0] = 1.0
+    assert np.abs(orc.apply_constraint(orc.CON_LAYER_BLUR, top, sig)[-1]).max() == 0.0     # periodic filtering would leak here
+    # in-plane low pass is separable: delta -> outer product of the two 1-D responses; layers do not mix
+    d2 = np.zeros((2, 15, 15), complex); d2[0, 7, 7] = 1.0
+    o2 = orc.apply_constraint(orc.CON_LOWPASS, d2, 1.1)
+    R2 = int(np.ceil(4 * 1.1)); w2 = np.exp(-np.arange(-R2, R2 + 1) ** 2 / (2 * 1.1 ** 2))
+    def col1(n, c):
+        return np.array([w2[(c - p) + R2] / sum(w2[t + R2] for t in range(-R2, R2 + 1) if 0 <= p + t < n) if abs(c - p) <= R2 else 0.0 for p in range(n)])
+    assert np.abs(o2[0] - np.outer(col1(15, 7), col1(15, 7))).max() < 1e-14 and np.abs(o2[1]).max() == 0.0
+
+
+def test_adam_closed_forms():
+    z = crandn(4, 5); g = crandn(4, 5)
+    # first step, eps -> 0: bias correction makes m^ = g, v^ = |g|^2, so the step is -lr g/|g| whatever beta1, beta2
+    z1, m1, v1 = orc.adam_update(z, g, np.zeros_like(z), np.zeros(z.shape), lr=0.01, b1=0.9, b2=0.999, eps=0.0, t=1)
+    assert np.abs((z1 - z) + 0.01 * g / np.abs(g)).max() < 1e-13
+    assert np.abs(m1 - 0.1 * g).max() < 1e-15 and np.abs(v1 - 0.001 * np.abs(g) ** 2).max() < 1e-15
+    # constant gradient: every later step is the same -lr g/|g|
+    zc, mc, vc = z1, m1, v1
+    for t in range(2, 6):
+        zc, mc, vc = orc.adam_update(zc, g, mc, vc, lr=0.01, eps=0.0, t=t)
+    assert np.abs((zc - z) + 5 * 0.01 * g / np.abs(g)).max() < 1e-12
+    # sign flip of the gradient at step 2: m^ = (0.09 - 0.1) g / 0.19, v^ = |g|^2
+    z2, _, _ = orc.adam_update(z1, -g, m1, v1, lr=0.01, eps=0.0, t=2)
+    assert np.abs((z2 - z1) - 0.01 * (0.01 / 0.19) * g / np.abs(g)).max() < 1e-13
+    # real variables (positions): per-component form
+    x = RNG.standard_normal(7); gx = RNG.standard_normal(7)
+    x1, _, _ = orc.adam_update(x, gx, np.zeros(7), np.zeros(7), lr=0.1, eps=0.0, t=1)
+    assert np.abs((x1 - x) + 0.1 * np.sign(gx)).max() < 1e-13
+    # eps enters as sqrt(v^) + eps
+    x1e, _, _ = orc.adam_update(x, gx, np.zeros(7), np.zeros(7), lr=0.1, eps=0.5, t=1)
+    assert np.abs((x1e - x) + 0.1 * gx / (np.abs(gx) + 0.5)).max() < 1e-13
