@@ -159,6 +159,49 @@ int32_t ptycho_object_transparency(const pt_problem *p, const pt_c64 *object_d, 
                                    const int32_t *batch_idx_d, float *objtrans_d, void *workspace_d, size_t workspace_bytes,
                                    void *cuda_stream);
 
+/* ---- what completes a usable gradient-descent iteration around ptycho_gradient -------------------
+ * All three work on a complex field [n_slices][ny][nx] (object slices; probe modes with n_slices = M, ny = nx = N),
+ * DEVICE memory, on `cuda_stream`; deterministic (owner-computes, fixed-order fp64 cost sum).                        */
+
+/* Cost regularisers (the paper names them only — reading R26).  ADDS weight * dR/dconj(field) into
+ * grad_d (same shape; may be NULL) and ADDS R into *cost_d (DEVICE double[1]; may be NULL), so both can be chained behind
+ * ptycho_gradient's outputs.
+ *   PT_REG_L2             R = w sum |z - ref|^2                     (ref = 1: "penalizes a non-vacuum object"; 0 for a probe)
+ *   PT_REG_L1             R = w sum sqrt(|z - ref|^2 + eps^2)
+ *   PT_REG_TIKHONOV       R = w sum_{d = x, y} sum |D_d z|^2        forward differences inside a slice, no wrap-around
+ *   PT_REG_TV             R = w sum_{d = x, y} sum sqrt(|D_d z|^2 + eps^2)
+ *   PT_REG_LAYER_TIKHONOV / PT_REG_LAYER_TV   the same with the one difference along depth, z_{i+1} - z_i
+ * workspace_d: at least ptycho_regularizer_workspace_bytes() bytes of scratch (per-block cost partials).
+ * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE (a dimension < 1), PT_ERR_BAD_PARAM (unknown kind, eps < 0), PT_ERR_WORKSPACE. */
+enum { PT_REG_L2 = 0, PT_REG_L1 = 1, PT_REG_TIKHONOV = 2, PT_REG_TV = 3, PT_REG_LAYER_TIKHONOV = 4, PT_REG_LAYER_TV = 5 };
+size_t ptycho_regularizer_workspace_bytes(void);
+int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps, int32_t n_slices, int32_t ny, int32_t nx,
+                                const pt_c64 *field_d, pt_c64 *grad_d, double *cost_d,
+                                void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* Constraint regularisers (reading R27), in place on field_d.
+ *   PT_CON_AMPLITUDE_CLAMP  |z| limited to [a, b], phase kept (a zero pixel with a > 0 becomes the real number a)
+ *   PT_CON_SUPPORT_MASK     z[s][y][x] *= mask_d[y][x]  (probe support in real space; mask_d DEVICE float [ny][nx])
+ *   PT_CON_LAYER_BLUR       Gaussian blur along depth, sigma = a slices, as a REAL-SPACE convolution (the paper: no bleeding
+ *                           from top to bottom through periodic boundaries): out[p] = sum_t w_t z[p+t] / sum_t w_t over the
+ *                           taps |t| <= ceil(4 sigma) that fall inside, w_t = exp(-t^2 / (2 sigma^2))
+ *   PT_CON_LOWPASS          the same blur along x, then along y, sigma = a px
+ * The two blurs need workspace_bytes >= n_slices*ny*nx*8 (one copy of the field); the others none (workspace_d may be NULL).
+ * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE, PT_ERR_BAD_PARAM (unknown kind, a > b, sigma <= 0), PT_ERR_WORKSPACE.          */
+enum { PT_CON_AMPLITUDE_CLAMP = 0, PT_CON_SUPPORT_MASK = 1, PT_CON_LAYER_BLUR = 2, PT_CON_LOWPASS = 3 };
+int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float *mask_d, int32_t n_slices, int32_t ny, int32_t nx,
+                                pt_c64 *field_d, void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* Adam (Kingma & Ba algorithm 1; reading R28: complex first moment, second moment from |g|^2), step >= 1:
+ *   m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) |g|^2 ; z <- z - lr (m / (1 - b1^step)) / (sqrt(v / (1 - b2^step)) + eps)
+ * ptycho_adam_update: n complex numbers (z, g, m complex64; v float).  ptycho_adam_update_real: n floats (positions).
+ * m_d and v_d are caller-owned state, zero before the first step.  Errors: PT_ERR_NULL, PT_ERR_BAD_PARAM (step < 1,
+ * betas outside [0, 1), eps < 0).                                                                                      */
+int32_t ptycho_adam_update(pt_c64 *z_d, const pt_c64 *g_d, pt_c64 *m_d, float *v_d, size_t n, float lr, float beta1,
+                           float beta2, float eps, int32_t step, void *cuda_stream);
+int32_t ptycho_adam_update_real(float *z_d, const float *g_d, float *m_d, float *v_d, size_t n, float lr, float beta1,
+                                float beta2, float eps, int32_t step, void *cuda_stream);
+
 /* End-to-end convenience with HOST buffers (pinned memory recommended): copies object/probe/positions and the
  * batch rows' intensities host->device into the workspace, runs ptycho_gradient, copies gradients and loss
  * back, and synchronises the stream.  Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL. */

@@ -16,6 +16,7 @@
 // The CPU oracle under oracle/ shares nothing with this file.
 #include <cuda_runtime.h>
 #include <math_constants.h>
+#include <math.h>
 #include <stdint.h>
 #include <string.h>
 
@@ -1046,11 +1047,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_regularizer, K_constraint, K_adam, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam"};
 thread_local int64_t g_launches = 0;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
@@ -1515,3 +1516,5 @@ const char* ptycho_strerror(int32_t code) {
 }
 
 }  // extern "C"
+
+#include "regularizers.cuh"

@@ -1,0 +1,226 @@
+// regularizers.cuh — SURVEY §8(f) rank 3: cost regularisers (reading R26), constraint regularisers
+// (R27) and the Adam update (R28).  Object-sized elementwise / stencil kernels, HBM-bound:
+// one read of the field (+ neighbours from L1/L2) and one read-modify-write of the gradient per call.  Included at the end of
+// ptycho_kernels.cu (it uses that file's launch accounting); the C ABI is declared in include/ptycho.h.
+// Owner-computes everywhere (no atomics); the cost is a fixed-grid, fixed-order fp64 sum, so results are bitwise reproducible.
+#pragma once
+
+namespace {
+
+constexpr int kRegBlocks = 1024, kRegThreads = 256;
+
+__device__ __forceinline__ float reg_phi(bool tv, float a2, float eps2) { return tv ? sqrtf(a2 + eps2) : a2; }
+__device__ __forceinline__ float reg_dphi(bool tv, float a2, float eps2) { return tv ? 0.5f * rsqrtf(a2 + eps2) : 1.0f; }
+
+// kinds L2 / L1: pointwise
+__global__ void __launch_bounds__(kRegThreads) k_reg_point(int l1, float w, float ref, float eps2, size_t n, const cf* z, cf* g, double* part) {
+  __shared__ double red[kRegThreads / 32];
+  double acc[1] = {0.0};
+  for (size_t i = (size_t)blockIdx.x * kRegThreads + threadIdx.x; i < n; i += (size_t)kRegBlocks * kRegThreads) {
+    const cf u = make_float2(z[i].x - ref, z[i].y);
+    const float a2 = fmaf(u.x, u.x, u.y * u.y);
+    if (l1 && a2 + eps2 == 0.f) continue;                            // |0| with eps = 0: subgradient 0
+    acc[0] += (double)(w * reg_phi(l1, a2, eps2));
+    if (g) { const float c = w * reg_dphi(l1, a2, eps2); g[i] = make_float2(fmaf(c, u.x, g[i].x), fmaf(c, u.y, g[i].y)); }
+  }
+  block_sum<kRegThreads, 1>(acc, red);
+  if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
+}
+
+// kinds Tikhonov / TV (in-plane: directions x, y) and their layer versions (direction z): every pixel owns the pair
+// (p, p + stride) for the cost and collects, for its gradient, the pair before it and the pair after it
+__global__ void __launch_bounds__(kRegThreads) k_reg_diff(int tv, int layer, float w, float eps2, int S, int ny, int nx, const cf* z, cf* g,
+                                                        double* part) {
+  __shared__ double red[kRegThreads / 32];
+  const size_t os = (size_t)ny * nx, n = (size_t)S * os;
+  double acc[1] = {0.0};
+  for (size_t i = (size_t)blockIdx.x * kRegThreads + threadIdx.x; i < n; i += (size_t)kRegBlocks * kRegThreads) {
+    const int s = (int)(i / os), y = (int)((i - (size_t)s * os) / nx), x = (int)(i - (size_t)s * os - (size_t)y * nx);
+    const cf c0 = z[i];
+    float gx = 0.f, gy = 0.f;
+#pragma unroll
+    for (int d = 0; d < 3; ++d) {
+      if (layer ? d != 2 : d == 2) continue;
+      const size_t stride = d == 0 ? 1 : d == 1 ? (size_t)nx : os;
+      const int c = d == 0 ? x : d == 1 ? y : s, len = d == 0 ? nx : d == 1 ? ny : S;
+      if (c + 1 < len) {                                             // pair (i, i + stride): u = z[i + stride] - z[i]
+        const cf q = z[i + stride]; const float ux = q.x - c0.x, uy = q.y - c0.y, a2 = fmaf(ux, ux, uy * uy);
+        if (!(tv && a2 + eps2 == 0.f)) {
+          acc[0] += (double)(w * reg_phi(tv, a2, eps2));
+          const float k = w * reg_dphi(tv, a2, eps2); gx -= k * ux; gy -= k * uy;
+        }
+      }
+      if (c > 0) {                                                   // pair (i - stride, i): u = z[i] - z[i - stride]
+        const cf q = z[i - stride]; const float ux = c0.x - q.x, uy = c0.y - q.y, a2 = fmaf(ux, ux, uy * uy);
+        if (!(tv && a2 + eps2 == 0.f)) { const float k = w * reg_dphi(tv, a2, eps2); gx += k * ux; gy += k * uy; }
+      }
+    }
+    if (g) g[i] = make_float2(g[i].x + gx, g[i].y + gy);
+  }
+  block_sum<kRegThreads, 1>(acc, red);
+  if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
+}
+
+__global__ void k_reg_final(const double* part, double* cost) {
+  if (threadIdx.x != 0 || blockIdx.x != 0) return;
+  double s = 0.0;
+  for (int b = 0; b < kRegBlocks; ++b) s += part[b];
+  *cost += s;
+}
+
+// ---- constraints -------------------------------------------------------------------------------------------------
+__global__ void k_con_clamp(cf* z, size_t n, float lo, float hi) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const cf v = z[i];
+  const float m = sqrtf(fmaf(v.x, v.x, v.y * v.y));
+  const float t = m < lo ? lo : (m > hi ? hi : m);
+  if (t == m) return;
+  z[i] = m > 0.f ? make_float2(v.x * (t / m), v.y * (t / m)) : make_float2(t, 0.f);
+}
+__global__ void k_con_mask(cf* z, size_t n, size_t os, const float* mask) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float m = mask[i % os];
+  z[i] = make_float2(z[i].x * m, z[i].y * m);
+}
+struct BlurW { int R; float w[65]; };                                 // taps w[t + R], |t| <= R <= 32
+__global__ void k_con_blur(const cf* in, cf* out, int S, int ny, int nx, int axis, BlurW bw) {
+  const size_t os = (size_t)ny * nx, n = (size_t)S * os, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int s = (int)(i / os), y = (int)((i - (size_t)s * os) / nx), x = (int)(i - (size_t)s * os - (size_t)y * nx);
+  const long stride = axis == 0 ? 1 : axis == 1 ? nx : (long)os;
+  const int c = axis == 0 ? x : axis == 1 ? y : s, len = axis == 0 ? nx : axis == 1 ? ny : S;
+  float ar = 0.f, ai = 0.f, ws = 0.f;
+  for (int t = -bw.R; t <= bw.R; ++t) {
+    if (c + t < 0 || c + t >= len) continue;
+    const float w = bw.w[t + bw.R]; const cf q = in[(long)i + t * stride];
+    ar = fmaf(w, q.x, ar); ai = fmaf(w, q.y, ai); ws += w;
+  }
+  out[i] = make_float2(ar / ws, ai / ws);
+}
+
+// ---- Adam ----------------------------------------------------------------------------------------------------------
+// o1 = 1 - b1, o2 = 1 - b2 formed in double on the host (1 - 0.999f in float is off by 6e-5 relative)
+__global__ void k_adam_c(cf* z, const cf* g, cf* m, float* v, size_t n, float lr, float b1, float b2, float o1, float o2, float eps, float ic1, float ic2) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const cf gi = g[i];
+  const cf mi = make_float2(fmaf(b1, m[i].x, o1 * gi.x), fmaf(b1, m[i].y, o1 * gi.y));
+  const float vi = fmaf(b2, v[i], o2 * fmaf(gi.x, gi.x, gi.y * gi.y));
+  m[i] = mi; v[i] = vi;
+  const float d = lr * ic1 / (sqrtf(vi * ic2) + eps);
+  z[i] = make_float2(fmaf(-d, mi.x, z[i].x), fmaf(-d, mi.y, z[i].y));
+}
+__global__ void k_adam_r(float* z, const float* g, float* m, float* v, size_t n, float lr, float b1, float b2, float o1, float o2, float eps, float ic1, float ic2) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const float mi = fmaf(b1, m[i], o1 * g[i]), vi = fmaf(b2, v[i], o2 * g[i] * g[i]);
+  m[i] = mi; v[i] = vi;
+  z[i] = fmaf(-lr * ic1 / (sqrtf(vi * ic2) + eps), mi, z[i]);
+}
+
+}  // namespace
+
+extern "C" {
+
+size_t ptycho_regularizer_workspace_bytes(void) { return 256 + (size_t)kRegBlocks * sizeof(double); }
+
+int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps, int32_t n_slices, int32_t ny, int32_t nx,
+                                const pt_c64* field_d, pt_c64* grad_d, double* cost_d, void* workspace_d, size_t workspace_bytes,
+                                void* cuda_stream) {
+  if (!field_d || !workspace_d) return PT_ERR_NULL;
+  if (n_slices < 1 || ny < 1 || nx < 1) return PT_ERR_BAD_SIZE;
+  if (kind < PT_REG_L2 || kind > PT_REG_LAYER_TV || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
+  if (workspace_bytes < ptycho_regularizer_workspace_bytes()) return PT_ERR_WORKSPACE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  double* part = (double*)((char*)workspace_d + 256);
+  const size_t n = (size_t)n_slices * ny * nx;
+  if (kind == PT_REG_L2 || kind == PT_REG_L1)
+    k_reg_point<<<kRegBlocks, kRegThreads, 0, st>>>(kind == PT_REG_L1, weight, ref, eps * eps, n, (const cf*)field_d, (cf*)grad_d, part);
+  else
+    k_reg_diff<<<kRegBlocks, kRegThreads, 0, st>>>(kind == PT_REG_TV || kind == PT_REG_LAYER_TV, kind >= PT_REG_LAYER_TIKHONOV, weight,
+                                                   eps * eps, n_slices, ny, nx, (const cf*)field_d, (cf*)grad_d, part);
+  LAUNCH_CHECK(K_regularizer, st);
+  if (cost_d) { k_reg_final<<<1, 32, 0, st>>>(part, cost_d); LAUNCH_CHECK(K_regularizer, st); }
+  return PT_OK;
+}
+
+int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float* mask_d, int32_t n_slices, int32_t ny, int32_t nx,
+                                pt_c64* field_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
+  if (!field_d) return PT_ERR_NULL;
+  if (n_slices < 1 || ny < 1 || nx < 1) return PT_ERR_BAD_SIZE;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  const size_t os = (size_t)ny * nx, n = (size_t)n_slices * os;
+  const unsigned grid = (unsigned)((n + 255) / 256);
+  prof_mark(-1, st);
+  if (kind == PT_CON_AMPLITUDE_CLAMP) {
+    if (!(a >= 0.f) || !(b >= a)) return PT_ERR_BAD_PARAM;
+    k_con_clamp<<<grid, 256, 0, st>>>((cf*)field_d, n, a, b);
+    LAUNCH_CHECK(K_constraint, st);
+    return PT_OK;
+  }
+  if (kind == PT_CON_SUPPORT_MASK) {
+    if (!mask_d) return PT_ERR_NULL;
+    k_con_mask<<<grid, 256, 0, st>>>((cf*)field_d, n, os, mask_d);
+    LAUNCH_CHECK(K_constraint, st);
+    return PT_OK;
+  }
+  if (kind != PT_CON_LAYER_BLUR && kind != PT_CON_LOWPASS) return PT_ERR_BAD_PARAM;
+  if (!(a > 0.f) || a > 8.0f) return PT_ERR_BAD_PARAM;                 // taps |t| <= ceil(4 sigma) <= 32
+  if (!workspace_d) return PT_ERR_NULL;
+  if (workspace_bytes < n * sizeof(cf)) return PT_ERR_WORKSPACE;
+  BlurW bw;
+  bw.R = (int)ceil(4.0 * (double)a);
+  for (int t = -bw.R; t <= bw.R; ++t) bw.w[t + bw.R] = (float)exp(-(double)t * t / (2.0 * (double)a * (double)a));
+  cf* tmp = (cf*)workspace_d;
+  if (kind == PT_CON_LAYER_BLUR) {
+    k_con_blur<<<grid, 256, 0, st>>>((const cf*)field_d, tmp, n_slices, ny, nx, 2, bw);
+    LAUNCH_CHECK(K_constraint, st);
+    if (cudaMemcpyAsync(field_d, tmp, n * sizeof(cf), cudaMemcpyDeviceToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
+  } else {
+    k_con_blur<<<grid, 256, 0, st>>>((const cf*)field_d, tmp, n_slices, ny, nx, 0, bw);
+    LAUNCH_CHECK(K_constraint, st);
+    k_con_blur<<<grid, 256, 0, st>>>((const cf*)tmp, (cf*)field_d, n_slices, ny, nx, 1, bw);
+    LAUNCH_CHECK(K_constraint, st);
+  }
+  return PT_OK;
+}
+
+static int adam_params(const void* z, const void* g, const void* m, const void* v, float b1, float b2, float eps, int32_t step,
+                       float* ic1, float* ic2) {
+  if (!z || !g || !m || !v) return PT_ERR_NULL;
+  if (step < 1 || !(b1 >= 0.f && b1 < 1.f) || !(b2 >= 0.f && b2 < 1.f) || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
+  *ic1 = (float)(1.0 / (1.0 - pow((double)b1, (double)step)));
+  *ic2 = (float)(1.0 / (1.0 - pow((double)b2, (double)step)));
+  return PT_OK;
+}
+
+int32_t ptycho_adam_update(pt_c64* z_d, const pt_c64* g_d, pt_c64* m_d, float* v_d, size_t n, float lr, float beta1, float beta2,
+                           float eps, int32_t step, void* cuda_stream) {
+  float ic1, ic2;
+  int rc = adam_params(z_d, g_d, m_d, v_d, beta1, beta2, eps, step, &ic1, &ic2);
+  if (rc != PT_OK) return rc;
+  if (n == 0) return PT_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  k_adam_c<<<(unsigned)((n + 255) / 256), 256, 0, st>>>((cf*)z_d, (const cf*)g_d, (cf*)m_d, v_d, n, lr, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps, ic1, ic2);
+  LAUNCH_CHECK(K_adam, st);
+  return PT_OK;
+}
+
+int32_t ptycho_adam_update_real(float* z_d, const float* g_d, float* m_d, float* v_d, size_t n, float lr, float beta1, float beta2,
+                                float eps, int32_t step, void* cuda_stream) {
+  float ic1, ic2;
+  int rc = adam_params(z_d, g_d, m_d, v_d, beta1, beta2, eps, step, &ic1, &ic2);
+  if (rc != PT_OK) return rc;
+  if (n == 0) return PT_OK;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  k_adam_r<<<(unsigned)((n + 255) / 256), 256, 0, st>>>(z_d, g_d, m_d, v_d, n, lr, beta1, beta2, (float)(1.0 - (double)beta1), (float)(1.0 - (double)beta2), eps, ic1, ic2);
+  LAUNCH_CHECK(K_adam, st);
+  return PT_OK;
+}
+
+}  // extern "C"

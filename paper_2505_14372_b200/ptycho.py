@@ -24,12 +24,13 @@ OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
            "ptycho_apply_update", "ptycho_object_transparency", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
            "ptycho_launch_count", "ptycho_strerror", "ptycho_profile_enable", "ptycho_profile_num_kernels",
-           "ptycho_profile_kernel_name", "ptycho_profile_read"]
+           "ptycho_profile_kernel_name", "ptycho_profile_read", "ptycho_regularizer_workspace_bytes", "ptycho_cost_regularizer",
+           "ptycho_apply_constraint", "ptycho_adam_update", "ptycho_adam_update_real"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
     """nvcc -gencode arch=compute_100a,code=sm_100a -lineinfo ... -> in-tree libptycho_b200.so"""
-    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_kernels.cu", "fft_core.cuh")] + [os.path.join(_HERE, "..", "include", "ptycho.h")]
+    srcs = [os.path.join(_CSRC, f) for f in ("ptycho_kernels.cu", "fft_core.cuh", "regularizers.cuh")] + [os.path.join(_HERE, "..", "include", "ptycho.h")]
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(s) for s in srcs):
         return LIB_PATH
     cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-shared",
@@ -275,3 +276,58 @@ def profile_read() -> dict:
     ms = (C.c_float * n)(); cnt = (C.c_int64 * n)()
     _check(lib().ptycho_profile_read(ms, cnt))
     return {lib().ptycho_profile_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n) if cnt[i]}
+
+
+# ---- cost / constraint regularisers and Adam (include/ptycho.h) -----------------------------------
+REG_L2, REG_L1, REG_TIKHONOV, REG_TV, REG_LAYER_TIKHONOV, REG_LAYER_TV = range(6)
+CON_AMPLITUDE_CLAMP, CON_SUPPORT_MASK, CON_LAYER_BLUR, CON_LOWPASS = range(4)
+
+
+def _field3(t, name):
+    import torch
+    t = _dev(t, torch.complex64, name)
+    if t.dim() != 3:
+        raise TypeError(f"{name}: expected a [n_slices][ny][nx] tensor")
+    return t
+
+
+def regularizer_workspace_bytes() -> int:
+    f = lib().ptycho_regularizer_workspace_bytes
+    f.restype = C.c_size_t
+    return int(f())
+
+
+def cost_regularizer(kind: int, weight: float, field_, *, grad=None, cost=None, ref: float = 1.0, eps: float = 0.0, workspace):
+    """ptycho_cost_regularizer: grad += weight dR/dconj(field), cost[0] += R (both optional, in place)."""
+    import torch
+    z = _field3(field_, "field")
+    S, ny, nx = z.shape
+    f = lib().ptycho_cost_regularizer
+    f.restype = C.c_int32
+    _check(f(int(kind), C.c_float(weight), C.c_float(ref), C.c_float(eps), S, ny, nx, _ptr(z), _ptr(_dev(grad, torch.complex64, "grad")),
+             _ptr(_dev(cost, torch.float64, "cost")), _ptr(workspace), C.c_size_t(workspace.numel()), _stream()))
+
+
+def apply_constraint(kind: int, field_, *, a: float = 0.0, b: float = 0.0, mask=None, workspace=None):
+    """ptycho_apply_constraint (in place)."""
+    import torch
+    z = _field3(field_, "field")
+    S, ny, nx = z.shape
+    f = lib().ptycho_apply_constraint
+    f.restype = C.c_int32
+    _check(f(int(kind), C.c_float(a), C.c_float(b), _ptr(_dev(mask, torch.float32, "mask")), S, ny, nx, _ptr(z), _ptr(workspace),
+             C.c_size_t(0 if workspace is None else workspace.numel()), _stream()))
+
+
+def adam_update(z, g, m, v, *, lr: float, beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, step: int = 1):
+    """ptycho_adam_update (complex64 z, g, m; float32 v) or ptycho_adam_update_real (all float32); in place."""
+    import torch
+    cplx = z.dtype == torch.complex64
+    ty = torch.complex64 if cplx else torch.float32
+    z = _dev(z, ty, "z"); g = _dev(g, ty, "g"); m = _dev(m, ty, "m"); v = _dev(v, torch.float32, "v")
+    if not (g.numel() == z.numel() == m.numel() == v.numel()):
+        raise TypeError("adam_update: z, g, m, v must have the same number of elements")
+    f = lib().ptycho_adam_update if cplx else lib().ptycho_adam_update_real
+    f.restype = C.c_int32
+    _check(f(_ptr(z), _ptr(g), _ptr(m), _ptr(v), C.c_size_t(z.numel()), C.c_float(lr), C.c_float(beta1), C.c_float(beta2),
+             C.c_float(eps), int(step), _stream()))

@@ -692,3 +692,90 @@ def test_lsqml_probe_preconditioner(which):
     bad = case.positions.copy(); bad[0, 0] = -5.0
     ptycho.object_transparency(pbg0, obj_d, _t(bad), None, out=ot3, workspace=ws)
     assert ptycho.status(ws) == -6      # PT_ERR_OUT_OF_BOUNDS
+
+
+# ------------------------------------------------------------------------------------------------
+# cost regularisers (R26), constraint regularisers (R27), Adam (R28) against the oracle on the config-3
+# object geometry (reduced depth) and probe
+# ------------------------------------------------------------------------------------------------
+def _reg_inputs():
+    cfg = synth.config(3, n_slices=5)
+    phi = synth.object_phase(cfg)
+    obj = synth.object_from_phase(phi, 0.8)                       # [5][420][420] complex64
+    rng = np.random.default_rng(77)
+    g0 = (rng.standard_normal(obj.shape) + 1j * rng.standard_normal(obj.shape)).astype(np.complex64)
+    return cfg, obj, g0
+
+
+@pytest.mark.parametrize("kind", range(6))
+def test_cost_regularizers(kind):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg, obj, g0 = _reg_inputs()
+    R_o, g_o = orc.cost_regularizer(kind, 0.37, obj, ref=1.0, eps=0.02, grad=g0)
+    z_d, g_d = _t(obj), _t(g0)
+    cost = torch.full((1,), 5.0, dtype=torch.float64, device="cuda")
+    ws = torch.empty(ptycho.regularizer_workspace_bytes(), dtype=torch.uint8, device="cuda")
+    ptycho.cost_regularizer(kind, 0.37, z_d, grad=g_d, cost=cost, ref=1.0, eps=0.02, workspace=ws)
+    torch.cuda.synchronize()
+    assert abs((cost.item() - 5.0) - R_o) <= 1e-5 * abs(R_o)                       # cost is ADDED
+    assert rel_l2(g_d.cpu().numpy() - g0, g_o - g0) <= 1e-5                         # gradient is ADDED into grad
+    # cost only / gradient only; bitwise reproducible
+    g2 = _t(g0); c2 = torch.full((1,), 5.0, dtype=torch.float64, device="cuda")
+    ptycho.cost_regularizer(kind, 0.37, z_d, grad=g2, ref=1.0, eps=0.02, workspace=ws)
+    ptycho.cost_regularizer(kind, 0.37, z_d, cost=c2, ref=1.0, eps=0.02, workspace=ws)
+    assert torch.equal(g2, g_d) and torch.equal(c2, cost)
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.cost_regularizer(9, 0.37, z_d, grad=g2, workspace=ws)
+
+
+def test_constraints():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg, obj, g0 = _reg_inputs()
+    z = (obj * (1.0 + 0.3 * g0.real)).astype(np.complex64)
+    z[0, 3, 4] = 0.0
+    d = _t(z)
+    ptycho.apply_constraint(ptycho.CON_AMPLITUDE_CLAMP, d, a=0.8, b=1.1)
+    ref = orc.apply_constraint(orc.CON_AMPLITUDE_CLAMP, z, 0.8, 1.1)
+    assert rel_l2(d.cpu().numpy(), ref) <= 1e-6 and abs(d[0, 3, 4].item() - 0.8) < 1e-7
+    pr = synth.probe(cfg)                                          # [8][128][128]
+    yy, xx = np.meshgrid(np.arange(cfg.n), np.arange(cfg.n), indexing="ij")
+    mask = (((yy - 64) ** 2 + (xx - 64) ** 2) <= 40 ** 2).astype(np.float32)
+    d = _t(pr)
+    ptycho.apply_constraint(ptycho.CON_SUPPORT_MASK, d, mask=_t(mask))
+    assert np.array_equal(d.cpu().numpy(), (pr * mask[None]).astype(np.complex64))
+    ws = torch.empty(z.size * 8, dtype=torch.uint8, device="cuda")
+    for kind, okind, sig in ((ptycho.CON_LAYER_BLUR, orc.CON_LAYER_BLUR, 0.9), (ptycho.CON_LOWPASS, orc.CON_LOWPASS, 1.3)):
+        d = _t(z)
+        ptycho.apply_constraint(kind, d, a=sig, workspace=ws)
+        assert rel_l2(d.cpu().numpy(), orc.apply_constraint(okind, z, sig)) <= 1e-6
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.apply_constraint(ptycho.CON_LAYER_BLUR, d, a=0.9, workspace=ws[:100])
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.apply_constraint(ptycho.CON_AMPLITUDE_CLAMP, d, a=1.2, b=1.0)
+
+
+def test_adam_updates():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg, obj, g0 = _reg_inputs()
+    rng = np.random.default_rng(78)
+    z_o, m_o, v_o = obj.astype(np.complex128), np.zeros(obj.shape, np.complex128), np.zeros(obj.shape)
+    z_d = _t(obj); m_d = torch.zeros_like(z_d); v_d = torch.zeros(obj.shape, dtype=torch.float32, device="cuda")
+    x = rng.standard_normal((300, 2)).astype(np.float32)
+    x_o, mx_o, vx_o = x.astype(np.float64), np.zeros(x.shape), np.zeros(x.shape)
+    x_d = _t(x); mx_d = torch.zeros_like(x_d); vx_d = torch.zeros_like(x_d)
+    for t in range(1, 5):                                          # a few steps with changing gradients
+        g = (g0 * (1.0 + 0.5 * np.cos(t))).astype(np.complex64) + (0.3 * t) * np.roll(g0, t, axis=2)
+        gx = rng.standard_normal(x.shape).astype(np.float32)
+        f32 = lambda v: float(np.float32(v))                       # the oracle gets the float32 scalars the C ABI receives
+        z_o, m_o, v_o = orc.adam_update(z_o, g, m_o, v_o, lr=f32(1e-2), b1=f32(0.9), b2=f32(0.999), eps=f32(1e-8), t=t)
+        x_o, mx_o, vx_o = orc.adam_update(x_o, gx, mx_o, vx_o, lr=f32(1e-2), b1=f32(0.8), b2=f32(0.99), eps=f32(1e-3), t=t)
+        ptycho.adam_update(z_d, _t(g.astype(np.complex64)), m_d, v_d, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, step=t)
+        ptycho.adam_update(x_d, _t(gx), mx_d, vx_d, lr=1e-2, beta1=0.8, beta2=0.99, eps=1e-3, step=t)
+    assert rel_l2(z_d.cpu().numpy() - obj, z_o - obj) <= 1e-5
+    assert rel_l2(m_d.cpu().numpy(), m_o) <= 1e-6 and rel_l2(v_d.cpu().numpy(), v_o) <= 1e-6
+    assert rel_l2(x_d.cpu().numpy() - x, x_o - x) <= 1e-5
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.adam_update(z_d, z_d, m_d, v_d, lr=1e-2, step=0)
