@@ -779,3 +779,61 @@ def test_adam_updates():
     assert rel_l2(x_d.cpu().numpy() - x, x_o - x) <= 1e-5
     with pytest.raises(ptycho.PtychoError):
         ptycho.adam_update(z_d, z_d, m_d, v_d, lr=1e-2, step=0)
+
+
+# ------------------------------------------------------------------------------------------------
+# Full-size config 4 in the launch configuration bench.py times (N = 256 cluster geometry, 10 modes, 30 slices, the 1100 px
+# object, mini-batches of 1024 positions from the seeded permutation accumulated with PT_ACCUMULATE, library-default
+# workspace): the first two mini-batches.  The oracle needs ~1 core-minute per position here, so it sees a handful:
+#   (1) per-position loss and position gradient of sampled positions on both sides of a chunk boundary of each batch;
+#   (2) the object gradient on a corner patch of the two batches' footprint (few windows reach it: the oracle's gradient over
+#       exactly those positions is the whole accumulated sum there);
+#   (3) properties: sum of per-position losses = accumulated loss; zero gradient where no window reaches; finite everywhere.
+# ------------------------------------------------------------------------------------------------
+def test_cfg4_full_size_minibatches_sampled():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(4)
+    N, mb = cfg.n, 1024
+    obj = synth.object_from_phase(synth.object_phase(cfg), 0.8)
+    pr = synth.probe(cfg)
+    bl = synth.batches(cfg, mb)[:2]
+    rows_all = np.concatenate(bl)
+    pos = synth.positions(cfg)[rows_all]                                    # compacted: row r of these arrays = scan row rows_all[r]
+    inten = synth.standin_patterns(cfg, rows_all)
+    pbg, pbo = gpu_problem(cfg), oracle_problem(cfg)
+    obj_d, pr_d, pos_d, I_d = _t(obj), _t(pr), _t(pos), _t(inten)
+    gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+    gX = torch.full((2 * mb, 2), float("nan"), dtype=torch.float32, device="cuda")
+    lpp = torch.full((2 * mb,), float("nan"), dtype=torch.float32, device="cuda")
+    loss = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda")
+    ws = ptycho.make_workspace(pbg, cfg.n_pos, mb)                          # what bench.py --config 4 allocates
+    jc = ptycho.positions_in_flight(pbg, cfg.n_pos, mb)
+    assert 0 < jc < mb                                                      # each mini-batch really runs in several chunks
+    for i in range(2):
+        b = _t(np.arange(i * mb, (i + 1) * mb, dtype=np.int32))
+        ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, b, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX[i * mb:(i + 1) * mb],
+                        loss=loss, loss_per_pos=lpp[i * mb:(i + 1) * mb], flags=ptycho.ACCUMULATE if i else 0)
+    assert ptycho.status(ws) == 0
+    gO_h, gX_h, lpp_h = gO.cpu().numpy(), gX.cpu().numpy(), lpp.cpu().numpy()
+    assert np.isfinite(gO_h.view(np.float32)).all() and np.isfinite(gP.cpu().numpy().view(np.float32)).all()
+    assert abs(lpp_h.astype(np.float64).sum() - loss.item()) <= 1e-6 * abs(loss.item())
+    c = pos / np.float32(cfg.pixel_size) - np.float32(N // 2)
+    r0 = np.floor(c + np.float32(0.5)).astype(np.int64)
+    cover = np.zeros((cfg.obj_n, cfg.obj_n), np.int32)
+    for j in range(2 * mb):
+        cover[r0[j, 0]:r0[j, 0] + N, r0[j, 1]:r0[j, 1] + N] += 1
+    assert (gO_h[:, cover == 0] == 0).all()
+    y0, x0 = int(r0[:, 0].min()), int(r0[:, 1].min())
+    reach = lambda j: r0[j, 0] <= y0 + 3 and r0[j, 1] <= x0 + 3 and r0[j, 0] + N > y0 and r0[j, 1] + N > x0
+    corner = [j for j in range(2 * mb) if reach(j)]
+    assert 1 <= len(corner) <= 8
+    extra = [j for j in (jc - 1, jc, mb + jc - 1, mb + jc) if not reach(j)]
+    rows = np.array(corner + extra)
+    o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
+    for n, j in enumerate(rows):
+        assert abs(lpp_h[j] - o["loss_per_pos"][n]) <= 2e-5 * abs(o["loss_per_pos"][n]), (j, lpp_h[j], o["loss_per_pos"][n])
+        assert rel_l2(gX_h[j], o["grad_pos"][n]) <= TOL_GRAD, (j, gX_h[j], o["grad_pos"][n])
+    o = orc.gradient(pbo, obj, pr, pos[corner], inten[corner]) if extra else o
+    py, px_ = slice(y0, y0 + 4), slice(x0, x0 + 4)
+    assert rel_l2(gO_h[:, py, px_], o["grad_object"][:, py, px_]) <= TOL_GRAD
