@@ -871,6 +871,7 @@ double orc_cost_regularizer(int32_t kind, double weight, double ref, double eps,
 //                            reason: no bleeding from top to bottom through periodic boundaries): out[p] = sum_t w_t z[p+t] /
 //                            sum_t w_t over the taps |t| <= ceil(4 sigma) that fall inside, w_t = exp(-t^2 / (2 sigma^2))
 //   kind 3  object low pass: the same blur along x then along y, sigma = a px
+//   kind 4  probe support in reciprocal space, kind 5 object phase deramp: see the code below
 // ------------------------------------------------------------------------------------------
 static void blur_axis(int S, int ny, int nx, int axis, double sigma, std::vector<cd>& z) {
   const int R = (int)std::ceil(4.0 * sigma);
@@ -906,6 +907,44 @@ int32_t orc_apply_constraint(int32_t kind, double a, double b, const double* mas
   }
   if (kind == 1) {
     for (long i = 0; i < n; ++i) { field[2 * i] *= mask[i % os]; field[2 * i + 1] *= mask[i % os]; }
+    return 0;
+  }
+  if (kind == 4) {
+    // probe support in RECIPROCAL space: z <- Finv(mask .* F(z)), mask [n][n] real, zero frequency at [0][0]
+    if (ny != nx) return -3;
+    std::vector<cd> f(os);
+    for (int s = 0; s < S; ++s) {
+      for (long r = 0; r < os; ++r) f[r] = cd(field[2 * (s * os + r)], field[2 * (s * os + r) + 1]);
+      F2(nx, f.data());
+      for (long q = 0; q < os; ++q) f[q] *= mask[q];
+      Finv2(nx, f.data());
+      for (long r = 0; r < os; ++r) { field[2 * (s * os + r)] = f[r].real(); field[2 * (s * os + r) + 1] = f[r].imag(); }
+    }
+    return 0;
+  }
+  if (kind == 5) {
+    // object phase deramp ("removes an affine phase ramp from the object"; reading R29, no phase unwrapping):
+    // per slice, slopes from the amplitude-weighted mean phase step b = arg sum z[y+1,x] conj(z[y,x]), c likewise along x;
+    // offset a = arg sum z exp(-i(b (y - yc) + c (x - xc))) about the centre; z <- z exp(-i(a + b (y - yc) + c (x - xc)))
+    const double yc = 0.5 * (ny - 1), xc = 0.5 * (nx - 1);
+    for (int s = 0; s < S; ++s) {
+      auto Zs = [&](int y, int x) { long i = (long)s * os + (long)y * nx + x; return cd(field[2 * i], field[2 * i + 1]); };
+      cd sy = 0.0, sx = 0.0, sa = 0.0;
+      for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) {
+          if (y + 1 < ny) sy += Zs(y + 1, x) * std::conj(Zs(y, x));
+          if (x + 1 < nx) sx += Zs(y, x + 1) * std::conj(Zs(y, x));
+        }
+      const double bb = std::arg(sy), cc = std::arg(sx);
+      for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) sa += Zs(y, x) * std::polar(1.0, -(bb * (y - yc) + cc * (x - xc)));
+      const double aa = std::arg(sa);
+      for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) {
+          cd v = Zs(y, x) * std::polar(1.0, -(aa + bb * (y - yc) + cc * (x - xc)));
+          long i = (long)s * os + (long)y * nx + x; field[2 * i] = v.real(); field[2 * i + 1] = v.imag();
+        }
+    }
     return 0;
   }
   if (!(a > 0.0)) return -3;

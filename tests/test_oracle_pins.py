@@ -835,3 +835,33 @@ def test_adam_closed_forms():
     # eps enters as sqrt(v^) + eps
     x1e, _, _ = orc.adam_update(x, gx, np.zeros(7), np.zeros(7), lr=0.1, eps=0.5, t=1)
     assert np.abs((x1e - x) + 0.1 * gx / (np.abs(gx) + 0.5)).max() < 1e-13
+
+
+def test_constraints_fourier_support_and_phase_deramp():
+    # reciprocal-space probe support: z <- Finv(mask F z), against numpy.fft; all-ones = identity; 0/1 mask idempotent
+    n = 16
+    z = crandn(2, n, n)
+    s = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n)
+    mask = ((s[:, None] ** 2 + s[None, :] ** 2) <= 25).astype(float)
+    out = orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, z, mask=mask)
+    assert np.abs(out - np.fft.ifft2(np.fft.fft2(z) * mask[None])).max() < 1e-12
+    assert np.abs(orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, z, mask=np.ones((n, n))) - z).max() < 1e-13
+    assert np.abs(orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, out, mask=mask) - out).max() < 1e-13
+    # phase deramp (reading R29): a pure ramp becomes a positive real constant; an object without a ramp is
+    # unchanged; the result does not depend on a ramp put on top (the ambiguity of PAPER.md:125 is removed)
+    ny, nx = 12, 15
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    ramp = np.exp(1j * (0.7 + 0.21 * y - 0.13 * x))
+    flat = orc.apply_constraint(orc.CON_PHASE_DERAMP, (2.5 * ramp)[None])
+    assert np.abs(flat - 2.5).max() < 1e-12
+    amp = 1.0 + 0.3 * RNG.uniform(size=(1, ny, nx))                            # real positive object: nothing to remove
+    assert np.abs(orc.apply_constraint(orc.CON_PHASE_DERAMP, amp.astype(complex)) - amp).max() < 1e-12
+    obj = amp * np.exp(1j * 0.2 * np.sin(2 * np.pi * x / nx) * np.cos(2 * np.pi * y / ny))[None]
+    d0 = orc.apply_constraint(orc.CON_PHASE_DERAMP, obj)
+    d1 = orc.apply_constraint(orc.CON_PHASE_DERAMP, obj * ramp[None])
+    assert np.abs(d0 - d1).max() < 1e-12
+    assert np.abs(np.abs(d0) - np.abs(obj)).max() < 1e-13                      # a pure phase factor
+    # slices are treated one by one
+    two = np.concatenate([obj * ramp[None], obj * np.conj(ramp)[None]])
+    d2 = orc.apply_constraint(orc.CON_PHASE_DERAMP, two)
+    assert np.abs(d2[0] - d0[0]).max() < 1e-12 and np.abs(d2[1] - d0[0]).max() < 1e-12
