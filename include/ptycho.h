@@ -2,7 +2,7 @@
  * (arxiv 2505.14372, "phaser").  One call = one batched forward(+adjoint) pass of the model of
  * PAPER.md:113-123 over a group of probe positions, on one GPU, on the caller's stream.
  *
- * Conventions (DESIGN.md §2/§3 give the citations and the readings R1..R22 of the paper):
+ * Conventions (DESIGN.md §2/§3 give the citations and the readings R1..R29 of the paper):
  *   - complex64 is interleaved (re, im) float32; all arrays are C-contiguous, row-major, last index fastest.
  *   - F is the unnormalised forward DFT with kernel exp(-2 pi i q.r/N); zero frequency at index [0][0].
  *   - gradients are g = dL/d conj(z); a descent step is z <- z - lr*g.
@@ -186,9 +186,16 @@ int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps
  *                           from top to bottom through periodic boundaries): out[p] = sum_t w_t z[p+t] / sum_t w_t over the
  *                           taps |t| <= ceil(4 sigma) that fall inside, w_t = exp(-t^2 / (2 sigma^2))
  *   PT_CON_LOWPASS          the same blur along x, then along y, sigma = a px
- * The two blurs need workspace_bytes >= n_slices*ny*nx*8 (one copy of the field); the others none (workspace_d may be NULL).
+ *   PT_CON_SUPPORT_MASK_FOURIER  probe support in reciprocal space: z <- Finv(mask_d .* F(z)), mask_d DEVICE float [n][n], zero
+ *                           frequency at [0][0]; ny = nx = n in {64, 128, 256} (the chain kernels' register FFT)
+ *   PT_CON_PHASE_DERAMP     removes an affine phase ramp per slice (reading R29, no unwrapping): slopes
+ *                           b = arg sum z[y+1,x] conj(z[y,x]), c likewise along x, offset a = arg sum z exp(-i(b(y-yc) + c(x-xc)))
+ *                           about the centre; z <- z exp(-i(a + b(y-yc) + c(x-xc))).  Fixed-order fp64 sums.
+ * The two blurs need workspace_bytes >= n_slices*ny*nx*8 (one copy of the field), the deramp 256 + n_slices*2080 bytes; the
+ * others none (workspace_d may be NULL).
  * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE, PT_ERR_BAD_PARAM (unknown kind, a > b, sigma <= 0), PT_ERR_WORKSPACE.          */
-enum { PT_CON_AMPLITUDE_CLAMP = 0, PT_CON_SUPPORT_MASK = 1, PT_CON_LAYER_BLUR = 2, PT_CON_LOWPASS = 3 };
+enum { PT_CON_AMPLITUDE_CLAMP = 0, PT_CON_SUPPORT_MASK = 1, PT_CON_LAYER_BLUR = 2, PT_CON_LOWPASS = 3,
+       PT_CON_SUPPORT_MASK_FOURIER = 4, PT_CON_PHASE_DERAMP = 5 };
 int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float *mask_d, int32_t n_slices, int32_t ny, int32_t nx,
                                 pt_c64 *field_d, void *workspace_d, size_t workspace_bytes, void *cuda_stream);
 

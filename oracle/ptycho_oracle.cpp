@@ -2,7 +2,7 @@
 //
 // Plain, slow, double-precision CPU restatement of one forward+adjoint iteration of the
 // mixed-state multislice ptychography model of arxiv 2505.14372 ("phaser"), written from the
-// paper and from the readings R1..R22 listed in DESIGN.md §3.  It shares no code,
+// paper and from the readings R1..R29 listed in DESIGN.md §3.  It shares no code,
 // header, table or constant generator with the CUDA path in paper_2505_14372_b200/csrc and
 // neither side includes the other.  Only tests/, __graft_entry__.smoke() and bench.py's
 // cpu_baseline / --impl reference leg may load this library.
@@ -15,7 +15,9 @@
 // propagator at dz=0, propagator composition, integer tilt shift, vacuum-object invariant, SPOA
 // special case, phase-ramp object, loss closed forms, dot-product adjoint tests, central finite
 // differences of the whole loss, zero gradient at the truth, torch.fft+autograd (complex128)
-// cross-check, LSQML line-search optimum.  "Absolute values vs the paper": parity unpinned —
+// cross-check, LSQML line-search optimum, and for the later additions (ePIE, per-position-alpha LSQML update, probe
+// preconditioner, regularisers, constraints, Adam) the closed forms, finite differences and numpy restatements named
+// beside each function.  "Absolute values vs the paper": parity unpinned —
 // the paper prints no numeric example.
 //
 // Notation follows PAPER.md §III: probe modes P_k, object slices O_i with gaps dz_i, positions

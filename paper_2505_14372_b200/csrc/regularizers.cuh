@@ -100,6 +100,77 @@ __global__ void k_con_blur(const cf* in, cf* out, int S, int ny, int nx, int axi
   out[i] = make_float2(ar / ws, ai / ws);
 }
 
+// probe support in reciprocal space: z <- Finv(mask .* F(z)); one CTA (CL = 4: one cluster) per mode, the field in
+// registers between the two transforms (the chain kernels' FFT)
+template <class G>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_con_fourier_mask(cf* field, const float* mask) {
+  typedef FL<G> F;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int t = threadIdx.x, k = blockIdx.x / G::CL;
+  const unsigned rk = Fft<G>::rank();
+  ChainSmem<G> cs(smem_raw, t);
+  cs.fill_tables(t);
+  __syncthreads();
+  cf v[32];
+  cf* f = field + (size_t)k * F::NNF;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) v[r] = f[F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r)];
+  Fft<G>::fwd(v, cs.sm, cs.tw, cs.tw2, t, rk);
+  const float sc = 1.0f / ((float)F::NF * (float)F::NF);
+#pragma unroll
+  for (int r = 0; r < 32; ++r) v[r] = cscale(v[r], sc * mask[F::fq_y(rk, t, r) * F::NF + F::fq_x(rk, t, r)]);
+  Fft<G>::inv(v, cs.sm, cs.tw, cs.tw2, t, rk);
+#pragma unroll
+  for (int r = 0; r < 32; ++r) f[F::pix_y(rk, t, r) * F::NF + F::pix_x(rk, t, r)] = v[r];
+}
+
+// object phase deramp (reading R29), per slice.  Pass 0: block partials of sum z[y+1,x] conj(z[y,x]) and
+// sum z[y,x+1] conj(z[y,x]); pass 1 (slopes known): partials of sum z exp(-i(b (y-yc) + c (x-xc))); k_deramp_final sums the
+// partials of a slice in fixed order (fp64) and takes the arguments; k_deramp_apply multiplies by the conjugate ramp.
+constexpr int kDerampBlocks = 64;                                     // per slice
+struct DerampOut { double b, c, a; };
+__global__ void __launch_bounds__(256) k_deramp_sums(const cf* z, int ny, int nx, int pass, const DerampOut* slope, double* part /* [S][64][4] */) {
+  __shared__ double red[(256 / 32) * 4];
+  const int s = blockIdx.y;
+  const size_t os = (size_t)ny * nx;
+  const cf* zs = z + (size_t)s * os;
+  double acc[4] = {0.0, 0.0, 0.0, 0.0};
+  const double yc = 0.5 * (ny - 1), xc = 0.5 * (nx - 1);
+  const double bb = pass ? slope[s].b : 0.0, cc = pass ? slope[s].c : 0.0;
+  for (size_t i = (size_t)blockIdx.x * 256 + threadIdx.x; i < os; i += (size_t)kDerampBlocks * 256) {
+    const int y = (int)(i / nx), x = (int)(i - (size_t)y * nx);
+    const cf c0 = zs[i];
+    if (!pass) {
+      if (y + 1 < ny) { const cf q = zs[i + nx]; acc[0] += (double)q.x * c0.x + (double)q.y * c0.y; acc[1] += (double)q.y * c0.x - (double)q.x * c0.y; }
+      if (x + 1 < nx) { const cf q = zs[i + 1]; acc[2] += (double)q.x * c0.x + (double)q.y * c0.y; acc[3] += (double)q.y * c0.x - (double)q.x * c0.y; }
+    } else {
+      double sn, cs_; sincos(-(bb * (y - yc) + cc * (x - xc)), &sn, &cs_);
+      acc[0] += (double)c0.x * cs_ - (double)c0.y * sn; acc[1] += (double)c0.x * sn + (double)c0.y * cs_;
+    }
+  }
+  block_sum<256, 4>(acc, red);
+  if (threadIdx.x == 0)
+    for (int c = 0; c < 4; ++c) part[((size_t)s * kDerampBlocks + blockIdx.x) * 4 + c] = acc[c];
+}
+__global__ void k_deramp_final(const double* part, int pass, DerampOut* out) {
+  const int s = blockIdx.x;
+  if (threadIdx.x != 0) return;
+  double a[4] = {0.0, 0.0, 0.0, 0.0};
+  for (int b = 0; b < kDerampBlocks; ++b)
+    for (int c = 0; c < 4; ++c) a[c] += part[((size_t)s * kDerampBlocks + b) * 4 + c];
+  if (!pass) { out[s].b = atan2(a[1], a[0]); out[s].c = atan2(a[3], a[2]); }
+  else out[s].a = atan2(a[1], a[0]);
+}
+__global__ void k_deramp_apply(cf* z, int ny, int nx, size_t n, const DerampOut* o) {
+  const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const size_t os = (size_t)ny * nx;
+  const int s = (int)(i / os), y = (int)((i - (size_t)s * os) / nx), x = (int)(i - (size_t)s * os - (size_t)y * nx);
+  double sn, cs_; sincos(-(o[s].a + o[s].b * (y - 0.5 * (ny - 1)) + o[s].c * (x - 0.5 * (nx - 1))), &sn, &cs_);
+  const cf v = z[i];
+  z[i] = make_float2((float)((double)v.x * cs_ - (double)v.y * sn), (float)((double)v.x * sn + (double)v.y * cs_));
+}
+
 // ---- Adam ----------------------------------------------------------------------------------------------------------
 // o1 = 1 - b1, o2 = 1 - b2 formed in double on the host (1 - 0.999f in float is off by 6e-5 relative)
 __global__ void k_adam_c(cf* z, const cf* g, cf* m, float* v, size_t n, float lr, float b1, float b2, float o1, float o2, float eps, float ic1, float ic2) {
@@ -164,6 +235,40 @@ int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float* mas
   if (kind == PT_CON_SUPPORT_MASK) {
     if (!mask_d) return PT_ERR_NULL;
     k_con_mask<<<grid, 256, 0, st>>>((cf*)field_d, n, os, mask_d);
+    LAUNCH_CHECK(K_constraint, st);
+    return PT_OK;
+  }
+  if (kind == PT_CON_SUPPORT_MASK_FOURIER) {
+    if (!mask_d) return PT_ERR_NULL;
+    if (ny != nx || (nx != 64 && nx != 128 && nx != 256)) return PT_ERR_BAD_SIZE;      // the probe sizes of the chain kernels
+    cudaError_t e;
+    if (nx == 128) {
+      if (cudaFuncSetAttribute(k_con_fourier_mask<Geo<128>>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes<Geo<128>>()) != cudaSuccess) return PT_ERR_CUDA;
+      e = launch_fft<Geo<128>>(k_con_fourier_mask<Geo<128>>, n_slices * Geo<128>::CL, fft_smem_bytes<Geo<128>>(), st, (cf*)field_d, mask_d);
+    } else if (nx == 64) {
+      if (cudaFuncSetAttribute(k_con_fourier_mask<Geo<64>>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes<Geo<64>>()) != cudaSuccess) return PT_ERR_CUDA;
+      e = launch_fft<Geo<64>>(k_con_fourier_mask<Geo<64>>, n_slices * Geo<64>::CL, fft_smem_bytes<Geo<64>>(), st, (cf*)field_d, mask_d);
+    } else {
+      if (cudaFuncSetAttribute(k_con_fourier_mask<Geo<256>>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)fft_smem_bytes<Geo<256>>()) != cudaSuccess) return PT_ERR_CUDA;
+      e = launch_fft<Geo<256>>(k_con_fourier_mask<Geo<256>>, n_slices * Geo<256>::CL, fft_smem_bytes<Geo<256>>(), st, (cf*)field_d, mask_d);
+    }
+    if (e != cudaSuccess) return PT_ERR_CUDA;
+    LAUNCH_CHECK(K_constraint, st);
+    return PT_OK;
+  }
+  if (kind == PT_CON_PHASE_DERAMP) {
+    if (!workspace_d) return PT_ERR_NULL;
+    const size_t need = 256 + (size_t)n_slices * (kDerampBlocks * 4 * sizeof(double) + sizeof(DerampOut));
+    if (workspace_bytes < need) return PT_ERR_WORKSPACE;
+    double* part = (double*)((char*)workspace_d + 256);
+    DerampOut* out = (DerampOut*)(part + (size_t)n_slices * kDerampBlocks * 4);
+    for (int pass = 0; pass < 2; ++pass) {
+      k_deramp_sums<<<dim3(kDerampBlocks, n_slices), 256, 0, st>>>((const cf*)field_d, ny, nx, pass, out, part);
+      LAUNCH_CHECK(K_constraint, st);
+      k_deramp_final<<<n_slices, 32, 0, st>>>(part, pass, out);
+      LAUNCH_CHECK(K_constraint, st);
+    }
+    k_deramp_apply<<<grid, 256, 0, st>>>((cf*)field_d, ny, nx, n, out);
     LAUNCH_CHECK(K_constraint, st);
     return PT_OK;
   }

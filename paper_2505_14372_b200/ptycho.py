@@ -280,7 +280,7 @@ def profile_read() -> dict:
 
 # ---- cost / constraint regularisers and Adam (include/ptycho.h) -----------------------------------
 REG_L2, REG_L1, REG_TIKHONOV, REG_TV, REG_LAYER_TIKHONOV, REG_LAYER_TV = range(6)
-CON_AMPLITUDE_CLAMP, CON_SUPPORT_MASK, CON_LAYER_BLUR, CON_LOWPASS = range(4)
+CON_AMPLITUDE_CLAMP, CON_SUPPORT_MASK, CON_LAYER_BLUR, CON_LOWPASS, CON_SUPPORT_MASK_FOURIER, CON_PHASE_DERAMP = range(6)
 
 
 def _field3(t, name):

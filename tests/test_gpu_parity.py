@@ -878,3 +878,42 @@ def test_adam_iterations_with_regularisers_reconstruct_config1():
     a, b_ = rec[sl] - rec[sl].mean(), tru[sl] - tru[sl].mean()
     corr = float((a * b_).sum() / np.sqrt((a * a).sum() * (b_ * b_).sum()))
     assert corr > 0.98, corr
+
+
+@pytest.mark.parametrize("n", [64, 128, 256])
+def test_constraint_probe_support_fourier(n):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    rng = np.random.default_rng(90 + n)
+    pr = (rng.standard_normal((3, n, n)) + 1j * rng.standard_normal((3, n, n))).astype(np.complex64)
+    s = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n)
+    mask = ((s[:, None] ** 2 + s[None, :] ** 2) <= (0.3 * n) ** 2).astype(np.float32)
+    mask[1, 2] = 0.5                                               # not only 0/1, and not symmetric: catches a transposed mask
+    d = _t(pr)
+    ptycho.apply_constraint(ptycho.CON_SUPPORT_MASK_FOURIER, d, mask=_t(mask))
+    torch.cuda.synchronize()
+    assert rel_l2(d.cpu().numpy(), orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, pr, mask=mask)) <= 2e-6
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.apply_constraint(ptycho.CON_SUPPORT_MASK_FOURIER, _t(pr[:, :, : n // 2].copy()), mask=_t(mask))
+
+
+def test_constraint_phase_deramp():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg, obj, g0 = _reg_inputs()
+    ny, nx = obj.shape[1:]
+    y, x = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    ramps = np.stack([np.exp(1j * (0.3 * i + 0.004 * (i + 1) * y - 0.003 * (5 - i) * x)) for i in range(obj.shape[0])])
+    z = (obj * ramps).astype(np.complex64)
+    d = _t(z)
+    ws = torch.empty(256 + obj.shape[0] * 2080, dtype=torch.uint8, device="cuda")
+    ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d, workspace=ws)
+    torch.cuda.synchronize()
+    ref = orc.apply_constraint(orc.CON_PHASE_DERAMP, z)
+    assert rel_l2(d.cpu().numpy(), ref) <= 2e-6
+    assert rel_l2(ref, orc.apply_constraint(orc.CON_PHASE_DERAMP, obj)) <= 1e-5      # the ramp is what was removed (float32 input rounding)
+    d2 = _t(z)
+    ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d2, workspace=ws)
+    assert torch.equal(d, d2)                                                         # bitwise reproducible
+    with pytest.raises(ptycho.PtychoError):
+        ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d2, workspace=ws[:300])
