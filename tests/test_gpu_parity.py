@@ -917,3 +917,57 @@ def test_constraint_phase_deramp():
     assert torch.equal(d, d2)                                                         # bitwise reproducible
     with pytest.raises(ptycho.PtychoError):
         ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d2, workspace=ws[:300])
+
+
+# ------------------------------------------------------------------------------------------------
+# Full-size config 5 in the launch configuration bench.py times (4096-position scan with position errors, one mini-batch of
+# 1024 from the seeded permutation, flags POS_GRAD | ILLUM | STEP_SIZES, library-default workspace).  The step-size terms need
+# the batch-aggregated gradients, which the oracle cannot produce for 1024 positions in a test's time, so this checks
+#   (1) sampled positions one by one against the oracle (per-position loss, position gradient);
+#   (2) properties that hold at any size and tie the second sweep to the first: numX = -1/2 px dL/dX, all
+#       denominators >= 0, sum over pixels of the slice-0 illumination = J sum_k ||P_k||^2 (the Fourier shift is unitary),
+#       everything finite, zero illumination where no window reaches.
+# ------------------------------------------------------------------------------------------------
+def test_cfg5_full_size_minibatch_properties():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(5)
+    N, S, mb = cfg.n, cfg.n_slices, 1024
+    obj = synth.object_from_phase(synth.object_phase(cfg), 0.8)
+    pr = synth.probe(cfg)
+    pos = synth.positions(cfg)
+    inten = synth.standin_patterns(cfg)
+    b = synth.batches(cfg, mb)[0]
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbg, pbo = gpu_problem(cfg, **kw), oracle_problem(cfg, **kw)
+    obj_d, pr_d, pos_d, I_d, b_d = _t(obj), _t(pr), _t(pos), _t(inten), _t(b.astype(np.int32))
+    gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+    gX = torch.full((mb, 2), float("nan"), dtype=torch.float32, device="cuda")
+    lpp = torch.full((mb,), float("nan"), dtype=torch.float32, device="cuda")
+    il = torch.full(obj_d.shape, float("nan"), dtype=torch.float32, device="cuda")
+    ilp = torch.full(obj_d.shape, float(cfg.dose) / (cfg.step_px ** 2), dtype=torch.float32, device="cuda")
+    st = torch.full((mb, 2 * S + 6), float("nan"), dtype=torch.float32, device="cuda")
+    loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    fl = ptycho.WANT_POS_GRAD | ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES
+    ws = ptycho.make_workspace(pbg, cfg.n_pos, cfg.n_pos, fl)                # what bench.py --config 5 allocates
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, b_d, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il,
+                    illum_prev=ilp, step_terms=st, loss=loss, loss_per_pos=lpp)
+    assert ptycho.status(ws) == 0
+    st_h, gX_h, il_h, lpp_h = st.cpu().numpy().astype(np.float64), gX.cpu().numpy().astype(np.float64), il.cpu().numpy(), lpp.cpu().numpy()
+    assert np.isfinite(st_h).all() and np.isfinite(il_h).all() and np.isfinite(gO.cpu().numpy().view(np.float32)).all()
+    px = float(np.float32(cfg.pixel_size))
+    assert rel_l2(st_h[:, 2 * S + 2], -0.5 * px * gX_h[:, 0]) <= 3e-4 and rel_l2(st_h[:, 2 * S + 4], -0.5 * px * gX_h[:, 1]) <= 3e-4
+    assert (st_h[:, 1::2] >= 0).all()
+    pn = float(np.sum(np.abs(pr.astype(np.complex128)) ** 2))
+    assert abs(il_h[0].astype(np.float64).sum() - mb * pn) <= 1e-5 * mb * pn
+    c = pos[b] / np.float32(cfg.pixel_size) - np.float32(N // 2)
+    r0 = np.floor(c + np.float32(0.5)).astype(np.int64)
+    cover = np.zeros((cfg.obj_n, cfg.obj_n), bool)
+    for j in range(mb):
+        cover[r0[j, 0]:r0[j, 0] + N, r0[j, 1]:r0[j, 1] + N] = True
+    assert (il_h[:, ~cover] == 0).all() and (il_h[0][cover] > 0).all()
+    rows = np.array([0, 1, mb // 2, mb - 1])
+    o = orc.gradient(pbo, obj, pr, pos[b[rows]], inten[b[rows]])
+    for n, j in enumerate(rows):
+        assert abs(lpp_h[j] - o["loss_per_pos"][n]) <= 2e-5 * abs(o["loss_per_pos"][n])
+        assert rel_l2(gX_h[j], o["grad_pos"][n]) <= TOL_GRAD
