@@ -18,6 +18,7 @@
 #include <math_constants.h>
 #include <math.h>
 #include <stdint.h>
+#include <stdlib.h>
 #include <string.h>
 
 #include <vector>
@@ -129,6 +130,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
 // ------------------------------------------------------------------------------------------------
 struct KP {
   int N, M, S, ony, onx, J;          // J = batch size
+  int Mg;                            // patch-gradient planes per position in the staging buffer: M, or M/2 after k_backward_pair
   int j0, jc;                        // current chunk: batch-local offset and count
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
   int loss; float loss_c, eps;
@@ -680,6 +682,198 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 }
 
 // ------------------------------------------------------------------------------------------------
+// Tensor memory (TMEM, 256 KB per SM, otherwise unused by this library) as a per-thread parking space: a warp may touch
+// the 32 lanes of its own quarter (warp % 4) and any column; each warp gets 128 columns (64 for a parked field, 64 for the
+// first mode's patch gradient).  Measured on B200 (148 CTAs x 512 threads): swapping 64 registers per thread with TMEM costs
+// 576 cycles per CTA, a 64-register load 371.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void tmem_st4(uint32_t a, cf x, cf y) {
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};" ::"r"(a), "r"(__float_as_uint(x.x)), "r"(__float_as_uint(x.y)),
+               "r"(__float_as_uint(y.x)), "r"(__float_as_uint(y.y)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld4(uint32_t a, cf& x, cf& y) {
+  uint32_t r0, r1, r2, r3;
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x4.b32 {%0,%1,%2,%3}, [%4];" : "=r"(r0), "=r"(r1), "=r"(r2), "=r"(r3) : "r"(a) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+  x = make_float2(__uint_as_float(r0), __uint_as_float(r1)); y = make_float2(__uint_as_float(r2), __uint_as_float(r3));
+}
+__device__ __forceinline__ void tmem_st16(uint32_t a, const cf* v) {   // 8 complex = 16 columns
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x16.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16};" ::"r"(a),
+               "r"(__float_as_uint(v[0].x)), "r"(__float_as_uint(v[0].y)), "r"(__float_as_uint(v[1].x)), "r"(__float_as_uint(v[1].y)),
+               "r"(__float_as_uint(v[2].x)), "r"(__float_as_uint(v[2].y)), "r"(__float_as_uint(v[3].x)), "r"(__float_as_uint(v[3].y)),
+               "r"(__float_as_uint(v[4].x)), "r"(__float_as_uint(v[4].y)), "r"(__float_as_uint(v[5].x)), "r"(__float_as_uint(v[5].y)),
+               "r"(__float_as_uint(v[6].x)), "r"(__float_as_uint(v[6].y)), "r"(__float_as_uint(v[7].x)), "r"(__float_as_uint(v[7].y)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld16(uint32_t a, cf* v) {
+  uint32_t r[16];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x16.b32 {%0,%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15}, [%16];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]), "=r"(r[8]), "=r"(r[9]),
+                 "=r"(r[10]), "=r"(r[11]), "=r"(r[12]), "=r"(r[13]), "=r"(r[14]), "=r"(r[15]) : "r"(a) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 8; ++i) v[i] = make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
+}
+__device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
+// v <-> parked field (columns [0, 64) of the warp's block), eight complex at a time
+__device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
+#pragma unroll
+  for (int c = 0; c < 4; ++c) {
+    cf tmp[8];
+    tmem_ld16(tb + c * 16, tmp);
+    tmem_st16(tb + c * 16, &v[8 * c]);
+#pragma unroll
+    for (int i = 0; i < 8; ++i) v[8 * c + i] = tmp[i];
+  }
+  tmem_wait_st();
+}
+
+// ------------------------------------------------------------------------------------------------
+// H9, H10, H12, H13 backward for TWO modes per CTA (M even, CL = 1): the two adjoint chains advance slice by slice in turn,
+// the field of the mode that is not being worked on parked in TMEM, so that the patch gradients of the pair are summed on
+// chip (first mode's gT_i kept in TMEM until the second mode reaches slice i) and only the sum goes to the staging buffer:
+// half the staging writes here and half the reads in k_gather_object.  Same arithmetic per mode as k_backward (MODE 0 / 2);
+// the sum over the pair is taken in float32 in fixed order (first + second), the gather then sums the pairs in fp64.
+// Staging layout: [Jc][M/2][S][N^2].
+// ------------------------------------------------------------------------------------------------
+template <class G, int MODE>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos) {
+  typedef Lay<G> L; typedef FL<G> F;
+  static_assert(G::CL == 1, "paired backward: one CTA per field only");
+  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int t = threadIdx.x, wp = t >> 5;
+  ChainSmem<G> cs(smem_raw, t);
+  cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
+  uint32_t* tmem_slot = (uint32_t*)((unsigned char*)red + 1000);                  // beyond what block_sum uses of the 1 KB scratch
+  cs.fill_tables(t);
+  if (wp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(tmem_slot)), "n"(TCOLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  const int MP = P.M >> 1, jl = blockIdx.x / MP, kp = blockIdx.x - jl * MP, jb = P.j0 + jl;
+  const int pair0 = jl * P.M + 2 * kp;                                            // (position, mode) index of the pair's first mode
+  const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const int S = P.S, onx = P.bilinear ? NF : P.onx;
+  const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
+  auto fld = [&](int pr, int i) { return ((size_t)pr * S + i) * NNS; };           // field (pair index pr, slice i)
+  const size_t pix0 = (size_t)F::pix_y(0, t, 0) * onx + F::pix_x(0, t, 0);
+  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
+  // half step s = 0 .. 2S-1: mode h = s & 1 of the pair at slice i = S-1 - (s >> 1)
+  auto early = [&](int s) {
+    const int h = s & 1, i = S - 1 - (s >> 1);
+    const float4* st = (const float4*)(P.w.stash + fld(pair0 + h, i)) + t;
+#pragma unroll
+    for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+    if (h == 0 && i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);   // serves both modes at slice i
+    cp_async_commit();
+  };
+  early(0);
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tb = *tmem_slot + ((uint32_t)((wp & 3) * 32) << 16) + (uint32_t)((wp >> 2) * 128);
+  cf v[32];
+  auto init = [&](int pr) {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = F^H(g~) / N
+    const float4* ps = (const float4*)(P.w.psit + (size_t)pr * NNS);
+    const float2* wd = (const float2*)(P.w.wdet + (size_t)jl * NNS);
+    const float sc = (MODE == 2 ? -2.0f : 1.0f) / (float)NF;
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+      const float4 q = ps[p * T + t]; const float2 w = wd[p * T + t];
+      v[2 * p] = make_float2(q.x * (w.x * sc), q.y * (w.x * sc));
+      v[2 * p + 1] = make_float2(q.z * (w.y * sc), q.w * (w.y * sc));
+    }
+  };
+  init(pair0 + 1);
+#pragma unroll
+  for (int c = 0; c < 4; ++c) tmem_st16(tb + c * 16, &v[8 * c]);                  // park the second mode
+  tmem_wait_st();
+  init(pair0);
+#pragma unroll 1
+  for (int s = 0; s < 2 * S; ++s) {
+    const int h = s & 1, i = S - 1 - (s >> 1), pr = pair0 + h;
+    Fft<G>::inv_head(v, sm, cs.tw2, t, 0);
+    const cf* o = ob + (size_t)i * slice;
+    {
+      const float4* st = (const float4*)(P.w.stash + fld(pr, i)) + t;
+#pragma unroll
+      for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
+#pragma unroll
+      for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
+      cp_async_commit();
+    }
+    cf Tr[32 - 2 * E];
+#pragma unroll
+    for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
+    L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
+    cp_async_wait_all();
+    float s1 = 1.0f, s2 = 1.0f;
+    if (MODE == 2) { s1 = 1.0f / P.w.psimax[(size_t)pr * S + i]; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i]; }
+    float4* gt = (float4*)(P.w.gTpart + fld(jl * MP + kp, i));
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+      const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+      cf T0, T1;
+      if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
+      else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+      if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
+      if (h == 0) tmem_st4(tb + 64 + 4 * p, g0, g1);             // first mode: keep gT_i on chip
+      else {                                                     // second mode: the pair's sum goes to the staging buffer
+        cf a0, a1;
+        tmem_ld4(tb + 64 + 4 * p, a0, a1);
+        __stcs(gt + p * T + t, make_float4(a0.x + g0.x, a0.y + g0.y, a1.x + g1.x, a1.y + g1.y));
+      }
+      v[2 * p] = cmulc(v[2 * p], T0);                            // gPsi = conj(T) .* gPhi
+      v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
+    }
+    if (h == 0) tmem_wait_st();
+    if (s + 1 < 2 * S) early(s + 1);
+    Fft<G>::fwd(v, sm, tw, cs.tw2, t, 0);                        // F(gPsi_i)
+    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, 0);
+    tmem_swap_field(tb, v);                                      // the other mode's turn
+  }
+  // v = G~ of the first mode, the second mode's is parked.  H12 / H13 per mode as in k_backward.
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
+  const cf* ry = rx + NF;
+#pragma unroll 1
+  for (int h = 0; h < 2; ++h) {
+    if (h == 1) {
+#pragma unroll
+      for (int c = 0; c < 4; ++c) tmem_ld16(tb + c * 16, &v[8 * c]);
+    }
+    const int pr = pair0 + h, k = 2 * kp + h;
+    const cf* pt = P.w.Pt + (size_t)k * NNS;
+    cf* gp = P.w.Gpart + (size_t)pr * NNS;
+    cf wxv[F::NXV];
+    load_xv<G>(wxv, rx, t, 1.0f);
+    float sy = 0.f, sx = 0.f;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+      const int qy = F::fq_y(0, t, r);
+      const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
+      gp[L::native(t, r)] = cmulc(v[r], R);
+      if (want_pos) {
+        const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);
+        const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(0, t, r), NF) / (float)NF;
+        sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
+      }
+    }
+    if (want_pos) {
+      double acc[2] = {(double)sy, (double)sx};
+      block_sum<G::T, 2>(acc, red);
+      if (t == 0) {
+        const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
+        P.w.posg_part[((size_t)jb * P.M + k) * 2 + 0] = f * acc[0];
+        P.w.posg_part[((size_t)jb * P.M + k) * 2 + 1] = f * acc[1];
+      }
+    }
+  }
+  __syncthreads();
+  if (wp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "n"(TCOLS));
+}
+
+// ------------------------------------------------------------------------------------------------
 // ePIE normalisations: tmax[jl][i] = max over the window of |O_i|^2 ; psimax[block] = max |Psi|^2 of
 // one 16384-element block of the stash (one per (pair, slice, rank); the backward kernel takes the max over the ranks).
 // ------------------------------------------------------------------------------------------------
@@ -744,9 +938,9 @@ __global__ void __launch_bounds__(256) k_pos_bilinear(KP P, int cl) {
     const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
     for (int e = threadIdx.x; e < NN; e += 256) {
       const int y = e / N, x = e - y * N;
-      const size_t base = ((size_t)jl * P.M * P.S + i) * NN + F::r_native_of(y, x);
+      const size_t base = ((size_t)jl * P.Mg * P.S + i) * NN + F::r_native_of(y, x);
       double gr = 0.0, gi = 0.0;
-      for (int k = 0; k < P.M; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; gr += (double)g.x; gi += (double)g.y; }
+      for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; gr += (double)g.x; gi += (double)g.y; }
       const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
       const double tyr = (1.0 - fx) * ((double)c.x - a.x) + fx * ((double)d.x - b.x), tyi = (1.0 - fx) * ((double)c.y - a.y) + fx * ((double)d.y - b.y);
       const double txr = (1.0 - fy) * ((double)b.x - a.x) + fy * ((double)d.x - c.x), txi = (1.0 - fy) * ((double)b.y - a.y) + fy * ((double)d.y - c.y);
@@ -804,23 +998,24 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
             const int dy = d >> 1, dx = d & 1, ry = py - dy, rx = px - dx;
             if (ry < 0 || ry >= N || rx < 0 || rx >= N) continue;
             const double wgt = (dy ? fy : 1.0 - fy) * (dx ? fx : 1.0 - fx);
-            const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(ry, rx);
+            const int nat = F::r_native_of(ry, rx);
+            const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + nat;
             double sr = 0.0, si = 0.0, sl = 0.0;
-            for (int k = 0; k < P.M; ++k) {
-              const cf g = P.w.gTpart[base + (size_t)k * P.S * NN];
-              sr += (double)g.x; si += (double)g.y;
-              if (ILLUM) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
+            for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
+            if (ILLUM) {
+              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat;
+              for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
             }
             ar += wgt * sr; ai += wgt * si; al += wgt * sl;
           }
         }
       } else if (px >= 0 && px < N && py >= 0 && py < N) {
         const int idx = F::r_native_of(py, px);
-        const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
-        for (int k = 0; k < P.M; ++k) {
-          const cf g = P.w.gTpart[base + (size_t)k * P.S * NN];
-          ar += (double)g.x; ai += (double)g.y;
-          if (ILLUM) { const cf s = P.w.stash[base + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
+        const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + idx;
+        for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
+        if (ILLUM) {
+          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
+          for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
       }
     }
@@ -1090,7 +1285,7 @@ int validate(const pt_problem* p) {
 KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64* probe, const float* positions,
            const float* intensity, const int32_t* batch_idx) {
   KP k;
-  k.N = p->n; k.M = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch;
+  k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch;
   k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
   k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
@@ -1122,6 +1317,10 @@ int set_smem_attrs() {
   if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if constexpr (G::CL == 1) {
+    if (cudaFuncSetAttribute(k_backward_pair<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+    if (cudaFuncSetAttribute(k_backward_pair<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  }
   if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   return PT_OK;
@@ -1181,6 +1380,9 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool want_w = (p->flags & PT_WANT_WEIGHTED_ILLUM) != 0;     // validated by the caller: needs want_illum && want_steps
   const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   const bool epie = (p->flags & PT_EPIE) != 0;
+  // two modes per CTA, their patch gradients summed on chip (k_backward_pair): an even number of modes, one CTA per field
+  const bool paired = G::CL == 1 && (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR");
+  kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
   if (!acc) {
@@ -1201,9 +1403,16 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
-      launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
-    } else
-      launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      if constexpr (G::CL == 1) {
+        if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2), chain_smem_bytes<G>(), st, kp, 0);
+      }
+      if (!paired) launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+    } else {
+      if constexpr (G::CL == 1) {
+        if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2), chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      }
+      if (!paired) launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+    }
     LAUNCH_CHECK(K_backward, st);
     if (bilin) {
       if (want_illum) k_gather_object<G, true, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
