@@ -985,9 +985,19 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
       if (BILIN) sfr[tid] = make_float2(P.w.delta[2 * (P.j0 + jbase + tid) + 1], P.w.delta[2 * (P.j0 + jbase + tid)]);  // (fx, fy)
     }
     __syncthreads();
-    for (int jj = 0; jj < cnt; ++jj) {
+    // which windows reach this tile: every lane tests one window of a group of 32 (the test is block-uniform, so all
+    // warps get the same mask), then the warp walks the set bits in ascending order — the summation order is unchanged
+    for (int grp = 0; grp < cnt; grp += 32) {
+      bool hit = false;
+      if (grp + (tid & 31) < cnt) {
+        const int2 q = sr0[grp + (tid & 31)];
+        hit = !(q.x > ox0 + TW_ - 1 || q.x + NR <= ox0 || q.y > oy0 + TH_ - 1 || q.y + NR <= oy0);
+      }
+      unsigned hits = __ballot_sync(0xffffffffu, hit);
+      while (hits) {
+      const int jj = grp + __ffs(hits) - 1;
+      hits &= hits - 1;
       const int2 r0 = sr0[jj];
-      if (r0.x > ox0 + TW_ - 1 || r0.x + NR <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + NR <= oy0) continue;   // block-uniform reject
       const int px = ox - r0.x, py = oy - r0.y;
       if (BILIN) {
         // adjoint of the four-tap sampling: pixel o collects w_d gT[o - i0 - d] (the same weights)
@@ -1017,6 +1027,7 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
           const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
           for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
+      }
       }
     }
     __syncthreads();
@@ -1064,15 +1075,24 @@ __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
       sal[tid] = P.w.alpha_ji[(size_t)(jbase + tid) * P.S + i];
     }
     __syncthreads();
-    for (int jj = 0; jj < cnt; ++jj) {
-      const int2 r0 = sr0[jj];
-      if (r0.x > ox0 + TW_ - 1 || r0.x + N <= ox0 || r0.y > oy0 + TH_ - 1 || r0.y + N <= oy0) continue;   // block-uniform reject
-      const int px = ox - r0.x, py = oy - r0.y;
-      if (px >= 0 && px < N && py >= 0 && py < N) {
-        const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
-        double s = 0.0;
-        for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; s += (double)q.x * q.x + (double)q.y * q.y; }
-        acc += (double)sal[jj] * s;
+    for (int g = 0; g < cnt; g += 32) {                          // as in k_gather_object: ballot over a group of 32 windows
+      bool hit = false;
+      if (g + (tid & 31) < cnt) {
+        const int2 q = sr0[g + (tid & 31)];
+        hit = !(q.x > ox0 + TW_ - 1 || q.x + N <= ox0 || q.y > oy0 + TH_ - 1 || q.y + N <= oy0);
+      }
+      unsigned hits = __ballot_sync(0xffffffffu, hit);
+      while (hits) {
+        const int jj = g + __ffs(hits) - 1;
+        hits &= hits - 1;
+        const int2 r0 = sr0[jj];
+        const int px = ox - r0.x, py = oy - r0.y;
+        if (px >= 0 && px < N && py >= 0 && py < N) {
+          const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
+          double s = 0.0;
+          for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; s += (double)q.x * q.x + (double)q.y * q.y; }
+          acc += (double)sal[jj] * s;
+        }
       }
     }
     __syncthreads();
