@@ -728,7 +728,7 @@ __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// H9, H10, H12, H13 backward for TWO modes per CTA (M even, CL = 1): the two adjoint chains advance slice by slice in turn,
+// H9, H10, H12, H13 backward for TWO modes per CTA (or cluster of four at N = 256); M even: the two adjoint chains advance slice by slice in turn,
 // the field of the mode that is not being worked on parked in TMEM, so that the patch gradients of the pair are summed on
 // chip (first mode's gT_i kept in TMEM until the second mode reaches slice i) and only the sum goes to the staging buffer:
 // half the staging writes here and half the reads in k_gather_object.  Same arithmetic per mode as k_backward (MODE 0 / 2);
@@ -738,25 +738,26 @@ __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 template <class G, int MODE>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos) {
   typedef Lay<G> L; typedef FL<G> F;
-  static_assert(G::CL == 1, "paired backward: one CTA per field only");
-  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
+  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
   extern __shared__ __align__(16) unsigned char smem_raw[];
   const int t = threadIdx.x, wp = t >> 5;
+  const unsigned rk = Fft<G>::rank();
   ChainSmem<G> cs(smem_raw, t);
   cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
   uint32_t* tmem_slot = (uint32_t*)((unsigned char*)red + 1000);                  // beyond what block_sum uses of the 1 KB scratch
   cs.fill_tables(t);
+  Fft<G>::begin_fourier();
   if (wp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(tmem_slot)), "n"(TCOLS));
     asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
   }
-  const int MP = P.M >> 1, jl = blockIdx.x / MP, kp = blockIdx.x - jl * MP, jb = P.j0 + jl;
+  const int MP = P.M >> 1, pp = blockIdx.x / CL, jl = pp / MP, kp = pp - jl * MP, jb = P.j0 + jl;
   const int pair0 = jl * P.M + 2 * kp;                                            // (position, mode) index of the pair's first mode
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int S = P.S, onx = P.bilinear ? NF : P.onx;
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
-  auto fld = [&](int pr, int i) { return ((size_t)pr * S + i) * NNS; };           // field (pair index pr, slice i)
-  const size_t pix0 = (size_t)F::pix_y(0, t, 0) * onx + F::pix_x(0, t, 0);
+  auto fld = [&](int pr, int i) { return (((size_t)pr * S + i) * CL + rk) * NNS; };   // field (index pr, slice i), this rank's block
+  const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
   const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
   // half step s = 0 .. 2S-1: mode h = s & 1 of the pair at slice i = S-1 - (s >> 1)
   auto early = [&](int s) {
@@ -774,8 +775,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   const uint32_t tb = *tmem_slot + ((uint32_t)((wp & 3) * 32) << 16) + (uint32_t)((wp >> 2) * 128);
   cf v[32];
   auto init = [&](int pr) {   // H9: g~ = w .* psi~ ; gPhi_{S-1} = F^H(g~) / N
-    const float4* ps = (const float4*)(P.w.psit + (size_t)pr * NNS);
-    const float2* wd = (const float2*)(P.w.wdet + (size_t)jl * NNS);
+    const float4* ps = (const float4*)(P.w.psit + ((size_t)pr * CL + rk) * NNS);
+    const float2* wd = (const float2*)(P.w.wdet + ((size_t)jl * CL + rk) * NNS);
     const float sc = (MODE == 2 ? -2.0f : 1.0f) / (float)NF;
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
@@ -792,7 +793,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
 #pragma unroll 1
   for (int s = 0; s < 2 * S; ++s) {
     const int h = s & 1, i = S - 1 - (s >> 1), pr = pair0 + h;
-    Fft<G>::inv_head(v, sm, cs.tw2, t, 0);
+    Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
     {
       const float4* st = (const float4*)(P.w.stash + fld(pr, i)) + t;
@@ -808,8 +809,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     float s1 = 1.0f, s2 = 1.0f;
-    if (MODE == 2) { s1 = 1.0f / P.w.psimax[(size_t)pr * S + i]; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i]; }
-    float4* gt = (float4*)(P.w.gTpart + fld(jl * MP + kp, i));
+    if (MODE == 2) {
+      float pm = 0.f;
+      for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pr * S + i) * CL + c]);
+      s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
+    }
+    float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
@@ -829,8 +834,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     }
     if (h == 0) tmem_wait_st();
     if (s + 1 < 2 * S) early(s + 1);
-    Fft<G>::fwd(v, sm, tw, cs.tw2, t, 0);                        // F(gPsi_i)
-    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, 0);
+    Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                        // F(gPsi_i)
+    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
     tmem_swap_field(tb, v);                                      // the other mode's turn
   }
   // v = G~ of the first mode, the second mode's is parked.  H12 / H13 per mode as in k_backward.
@@ -843,19 +848,19 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       for (int c = 0; c < 4; ++c) tmem_ld16(tb + c * 16, &v[8 * c]);
     }
     const int pr = pair0 + h, k = 2 * kp + h;
-    const cf* pt = P.w.Pt + (size_t)k * NNS;
-    cf* gp = P.w.Gpart + (size_t)pr * NNS;
+    const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
+    cf* gp = P.w.Gpart + ((size_t)pr * CL + rk) * NNS;
     cf wxv[F::NXV];
     load_xv<G>(wxv, rx, t, 1.0f);
     float sy = 0.f, sx = 0.f;
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
-      const int qy = F::fq_y(0, t, r);
+      const int qy = F::fq_y(rk, t, r);
       const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
       gp[L::native(t, r)] = cmulc(v[r], R);
       if (want_pos) {
         const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);
-        const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(0, t, r), NF) / (float)NF;
+        const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(rk, t, r), NF) / (float)NF;
         sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
       }
     }
@@ -864,11 +869,13 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       block_sum<G::T, 2>(acc, red);
       if (t == 0) {
         const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
-        P.w.posg_part[((size_t)jb * P.M + k) * 2 + 0] = f * acc[0];
-        P.w.posg_part[((size_t)jb * P.M + k) * 2 + 1] = f * acc[1];
+        const size_t unit = ((size_t)jb * P.M + k) * CL + rk;       // index of this CTA's fp64 partials
+        P.w.posg_part[unit * 2 + 0] = f * acc[0];
+        P.w.posg_part[unit * 2 + 1] = f * acc[1];
       }
     }
   }
+  Fft<G>::end_fourier();
   __syncthreads();
   if (wp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "n"(TCOLS));
 }
@@ -1337,10 +1344,8 @@ int set_smem_attrs() {
   if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if constexpr (G::CL == 1) {
-    if (cudaFuncSetAttribute(k_backward_pair<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-    if (cudaFuncSetAttribute(k_backward_pair<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  }
+  if (cudaFuncSetAttribute(k_backward_pair<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward_pair<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   return PT_OK;
@@ -1400,8 +1405,8 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool want_w = (p->flags & PT_WANT_WEIGHTED_ILLUM) != 0;     // validated by the caller: needs want_illum && want_steps
   const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   const bool epie = (p->flags & PT_EPIE) != 0;
-  // two modes per CTA, their patch gradients summed on chip (k_backward_pair): an even number of modes, one CTA per field
-  const bool paired = G::CL == 1 && (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR");
+  // two modes per CTA (cluster), their patch gradients summed on chip (k_backward_pair): needs an even number of modes
+  const bool paired = (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR");
   kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
@@ -1423,15 +1428,11 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
-      if constexpr (G::CL == 1) {
-        if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2), chain_smem_bytes<G>(), st, kp, 0);
-      }
-      if (!paired) launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      else launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
     } else {
-      if constexpr (G::CL == 1) {
-        if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2), chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
-      }
-      if (!paired) launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      else launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
     }
     LAUNCH_CHECK(K_backward, st);
     if (bilin) {

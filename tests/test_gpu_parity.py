@@ -153,8 +153,9 @@ def test_gaussian_noise_model():
     check(g, o)
 
 
-def test_n64_multislice_multimode():
-    cfg = synth.config(3, n=64, scan=(6, 5), n_modes=3, n_slices=4, obj_n=200, pixel_size=0.2, step_px=3.0)
+@pytest.mark.parametrize("n_modes", [3, 4])                  # odd: one mode per CTA; even: two per CTA (k_backward_pair, four CTAs per SM)
+def test_n64_multislice_multimode(n_modes):
+    cfg = synth.config(3, n=64, scan=(6, 5), n_modes=n_modes, n_slices=4, obj_n=200, pixel_size=0.2, step_px=3.0)
     case = make_case(cfg, start_scale=0.8)
     o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
     g = gpu_gradient(case, gpu_problem(cfg))
@@ -217,8 +218,9 @@ def test_batches_accumulate():
     assert rel_l2(g["grad_probe"], o_all["grad_probe"]) <= TOL_GRAD
 
 
-def test_deterministic_bitwise():
-    cfg = synth.config(3, scan=(4, 5), n_modes=3, n_slices=4)
+@pytest.mark.parametrize("n_modes", [3, 4])                  # one mode per CTA / two modes per CTA with the pair sum taken in TMEM
+def test_deterministic_bitwise(n_modes):
+    cfg = synth.config(3, scan=(4, 5), n_modes=n_modes, n_slices=4)
     case = make_case(cfg, start_scale=0.8)
     pbg = gpu_problem(cfg)
     a = gpu_gradient(case, pbg)
@@ -227,6 +229,22 @@ def test_deterministic_bitwise():
         for k in ("grad_object", "grad_probe", "grad_pos", "loss_per_pos"):
             assert a[k].tobytes() == b[k].tobytes()
         assert a["loss"] == b["loss"]
+
+
+def test_paired_and_unpaired_backward_agree(monkeypatch):
+    # even mode counts run two modes per CTA (the pair's patch gradients summed on chip in float32); PTYCHO_NO_PAIR=1 forces
+    # the one-mode-per-CTA kernel.  Both must match the oracle (checked above); against each other they differ only by the
+    # rounding of that one float32 addition.
+    cfg = synth.config(3, scan=(4, 5), n_modes=4, n_slices=5)
+    case = make_case(cfg, start_scale=0.8)
+    pbg = gpu_problem(cfg)
+    a = gpu_gradient(case, pbg, want_illum=True)
+    monkeypatch.setenv("PTYCHO_NO_PAIR", "1")
+    b = gpu_gradient(case, pbg, want_illum=True)
+    assert rel_l2(a["grad_object"], b["grad_object"]) <= 2e-7
+    for k in ("grad_probe", "grad_pos", "loss_per_pos", "illum"):
+        assert a[k].tobytes() == b[k].tobytes(), k
+    assert a["grad_object"].tobytes() != b["grad_object"].tobytes()        # the switch really selected another kernel
 
 
 # ------------------------------------------------------------------------------------------------
