@@ -101,7 +101,7 @@ typedef struct {                  /* HOST struct */
 #define PT_STEP_TERMS_PER_POS(S) (2 * (S) + 6)
 
 /* Device scratch the caller must supply.  ptycho_workspace_bytes returns the RECOMMENDED size (positions are
- * processed in chunks; a larger workspace means larger chunks, capped at 64 GiB); ptycho_workspace_min_bytes the
+ * processed in chunks; a larger workspace means larger chunks, capped at 49 GiB); ptycho_workspace_min_bytes the
  * smallest size the calls accept.  The first 64 bytes hold the deferred status word. */
 size_t ptycho_workspace_bytes(const pt_problem *p);
 size_t ptycho_workspace_min_bytes(const pt_problem *p);

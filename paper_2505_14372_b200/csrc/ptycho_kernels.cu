@@ -53,7 +53,7 @@ struct Ws {
   cf* psit;            // [Jc][M][N^2]  F-native
   float* wdet;         // [Jc][N^2]     F-native
   cf* stash;           // [Jc][M][S][N^2]  R-native
-  cf* gTpart;          // [Jc][M][S][N^2]  R-native
+  cf* gTpart;          // [Jc][M or M/2][S][N^2]  R-native (staged_planes)
   cf* Gpart;           // [Jc][M][N^2]     F-native
   cf* scratch;         // [Jc][M][N^2]     (step sizes: gPhi_0)
   float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
@@ -65,6 +65,10 @@ struct Ws {
 };
 
 inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
+// Two modes per CTA in the backward pass (k_backward_pair: the pair's patch gradients are summed on chip and staged once)
+// whenever the number of modes is even; PTYCHO_NO_PAIR in the environment forces one mode per CTA (a debugging switch).
+inline bool use_pairs(const pt_problem* p) { return (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR"); }
+inline size_t staged_planes(const pt_problem* p) { return use_pairs(p) ? p->n_modes / 2 : p->n_modes; }   // gT planes per position
 inline size_t cluster_of(int n) { return n == 256 ? 4 : 1; }   // CTAs per field (Geo<n>::CL)
 
 // per-chunk-position bytes and fixed bytes
@@ -78,7 +82,7 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
   f += align_up(J * M * CL * (2 * S + 6) * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
-  size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + 2 * M * S * NN * sizeof(cf) + M * NN * sizeof(cf);
+  size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + (M + staged_planes(p)) * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   if (steps) pp += M * NN * sizeof(cf) + S * sizeof(float);
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
   if (p->flags & PT_EPIE) pp += (M * CL + 1) * S * sizeof(float) + 64;
@@ -113,7 +117,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->psit = (cf*)take(jc * M * NN * sizeof(cf));
   w->wdet = (float*)take(jc * NN * sizeof(float));
   w->stash = (cf*)take(jc * M * S * NN * sizeof(cf));
-  w->gTpart = (cf*)take(jc * M * S * NN * sizeof(cf));
+  w->gTpart = (cf*)take(jc * staged_planes(p) * S * NN * sizeof(cf));
   w->Gpart = (cf*)take(jc * M * NN * sizeof(cf));
   w->scratch = steps ? (cf*)take(jc * M * NN * sizeof(cf)) : nullptr;
   w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
@@ -1406,7 +1410,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool bilin = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT;
   const bool epie = (p->flags & PT_EPIE) != 0;
   // two modes per CTA (cluster), their patch gradients summed on chip (k_backward_pair): needs an even number of modes
-  const bool paired = (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR");
+  const bool paired = use_pairs(p);
   kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
@@ -1507,14 +1511,16 @@ int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) 
 size_t ptycho_workspace_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
   size_t f, pp; ws_sizes(p, &f, &pp);
-  const size_t cap = (size_t)64 << 30;
+  const size_t cap = (size_t)49 << 30;   // config 3: 1554 positions = 84 / 42 whole waves of forward / paired-backward CTAs
   size_t jc = p->n_batch;
   if (f + jc * pp > cap) {
     jc = (cap - f) / pp;
     // whole waves of 148 CTAs per chunk where possible
     const size_t wave = 148;
-    size_t pairs = jc * p->n_modes * cluster_of(p->n);
-    if (pairs > wave) { pairs -= pairs % wave; jc = pairs / (p->n_modes * cluster_of(p->n)); }
+    // (the paired backward kernel launches half as many CTAs: keep that count a whole number of waves too)
+    const size_t per_pos_ctas = staged_planes(p) * cluster_of(p->n);
+    size_t pairs = jc * per_pos_ctas;
+    if (pairs > wave) { pairs -= pairs % wave; jc = pairs / per_pos_ctas; }
     if (jc < 1) jc = 1;
   }
   return f + jc * pp;
