@@ -211,7 +211,9 @@ int32_t ptycho_adam_update_real(float *z_d, const float *g_d, float *m_d, float 
 
 /* End-to-end convenience with HOST buffers (pinned memory recommended): copies object/probe/positions and the
  * batch rows' intensities host->device into the workspace, runs ptycho_gradient, copies gradients and loss
- * back, and synchronises the stream.  Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL. */
+ * back, and synchronises the stream.  The patterns are copied chunk by chunk on a second stream that lives for the duration
+ * of the call, in the order the pass consumes them, so the copies overlap the chain kernels (use pinned host memory).
+ * Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL. */
 size_t ptycho_workspace_host_bytes(const pt_problem *p);
 int32_t ptycho_gradient_host(const pt_problem *p, const pt_c64 *object_h, const pt_c64 *probe_h,
                              const float *positions_h, const float *intensity_h, const int32_t *batch_idx_h,

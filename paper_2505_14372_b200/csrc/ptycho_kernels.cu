@@ -9,10 +9,14 @@
 //   k_loss           H7,H8 mode-summed intensity, per-pixel loss in fp64, detector weight w
 //   k_backward       H9,H10,H12,H13 one CTA per (j,k): adjoint chain, per-(j,k,i) patch gradients,
 //                    per-(j,k) probe-gradient spectra and position-gradient terms
+//   k_backward_pair  the same for TWO modes per CTA (even mode counts): the idle mode's field and the first mode's
+//                    patch gradient live in tensor memory (TMEM), only the pair's sum is staged
 //   k_gather_object  H11 deterministic owner-computes scatter-add: every object pixel sums the patch
 //                    gradients that cover it in fixed (j,k) order — no float atomics
 //   k_reduce_probe / k_probe_ifft / k_finalize   H12 tail, loss and position-gradient sums
-//   k_step_*         H14 LSQML-style step-size terms (second sweep), k_update_* H15
+//   k_backward<.,1>  H14 LSQML-style step-size terms (second sweep); k_alpha_pos / k_gather_willum / k_objtrans: the
+//                    per-position-alpha weights and the probe-view preconditioner of LSQML; k_axpy / k_lsqml_* H15
+//   regularizers.cuh cost / constraint regularisers and Adam
 // The CPU oracle under oracle/ shares nothing with this file.
 #include <cuda_runtime.h>
 #include <math_constants.h>
@@ -1279,6 +1283,9 @@ const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
                                          "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam"};
 thread_local int64_t g_launches = 0;
+// ptycho_gradient_host only: one event per chunk, recorded on its copy stream when that chunk's measured patterns have
+// arrived on the device; the gradient pass waits for chunk c's event before the first kernel that reads them (k_loss)
+thread_local cudaEvent_t* g_chunk_ready = nullptr;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
 thread_local std::vector<ProfMark> g_prof;
@@ -1425,6 +1432,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
+    if (g_chunk_ready && cudaStreamWaitEvent(st, g_chunk_ready[j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
     if (epie) {
@@ -1666,32 +1674,58 @@ int32_t ptycho_gradient_host(const pt_problem* p, const pt_c64* object_h, const 
   float* int_d = (float*)take(J * NN * 4); float* lpp_d = (float*)take(J * 4);
   double* loss_d = (double*)take(256);
   void* ws = c + off;
-  // the batch rows are compacted on the way in: the device sees rows 0..J-1
-  if (cudaMemcpyAsync(obj_d, object_h, on * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaMemcpyAsync(pr_d, probe_h, pn * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (!batch_idx_h) {
-    if (cudaMemcpyAsync(pos_d, positions_h, J * 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-    if (cudaMemcpyAsync(int_d, intensity_h, J * NN * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-  } else {
-    for (size_t j = 0; j < J; ++j) {
-      const size_t row = batch_idx_h[j];
-      if (cudaMemcpyAsync(pos_d + 2 * j, positions_h + 2 * row, 8, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-      if (cudaMemcpyAsync(int_d + j * NN, intensity_h + row * NN, NN * 4, cudaMemcpyHostToDevice, st) != cudaSuccess) return PT_ERR_CUDA;
-    }
-  }
   pt_problem q = *p;
-  q.n_pos_total = (int32_t)J; q.flags &= ~(PT_ACCUMULATE | PT_WANT_STEP_SIZES | PT_WANT_ILLUM);
+  q.n_pos_total = (int32_t)J; q.flags &= ~(PT_ACCUMULATE | PT_WANT_STEP_SIZES | PT_WANT_ILLUM | PT_WANT_WEIGHTED_ILLUM | PT_EPIE);
   if (grad_pos_h) q.flags |= PT_WANT_POS_GRAD;
+  // The measured patterns (the bulk of the input) travel on a second stream, chunk by chunk in the order the gradient pass
+  // consumes them, so that all but the first chunk's copy overlaps the chain kernels; object, probe and positions go first
+  // on the caller's stream.  The batch rows are compacted on the way in: the device sees rows 0..J-1.
+  const size_t Jc = (size_t)ptycho_positions_in_flight(&q, workspace_bytes - off);
+  if (Jc == 0) return PT_ERR_WORKSPACE;
+  const size_t nchunk = (J + Jc - 1) / Jc;
+  cudaStream_t cs2 = nullptr;
+  cudaEvent_t start_ev = nullptr;
+  std::vector<cudaEvent_t> ready(nchunk, nullptr);
+  bool ok = cudaStreamCreateWithFlags(&cs2, cudaStreamNonBlocking) == cudaSuccess &&
+            cudaEventCreateWithFlags(&start_ev, cudaEventDisableTiming) == cudaSuccess;
+  for (size_t c = 0; ok && c < nchunk; ++c) ok = cudaEventCreateWithFlags(&ready[c], cudaEventDisableTiming) == cudaSuccess;
+  auto cleanup = [&]() {
+    g_chunk_ready = nullptr;
+    for (auto e : ready) if (e) cudaEventDestroy(e);
+    if (start_ev) cudaEventDestroy(start_ev);
+    if (cs2) cudaStreamDestroy(cs2);
+  };
+  if (!ok) { cleanup(); return PT_ERR_CUDA; }
+  // the copy stream starts after whatever the caller's stream has queued so far (the buffers may still be in use)
+  ok = cudaEventRecord(start_ev, st) == cudaSuccess && cudaStreamWaitEvent(cs2, start_ev, 0) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(obj_d, object_h, on * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(pr_d, probe_h, pn * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  if (!batch_idx_h) ok = ok && cudaMemcpyAsync(pos_d, positions_h, J * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  else
+    for (size_t j = 0; ok && j < J; ++j)
+      ok = cudaMemcpyAsync(pos_d + 2 * j, positions_h + 2 * (size_t)batch_idx_h[j], 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
+  for (size_t c = 0; ok && c < nchunk; ++c) {
+    const size_t j0 = c * Jc, j1 = j0 + Jc < J ? j0 + Jc : J;
+    if (!batch_idx_h) ok = cudaMemcpyAsync(int_d + j0 * NN, intensity_h + j0 * NN, (j1 - j0) * NN * 4, cudaMemcpyHostToDevice, cs2) == cudaSuccess;
+    else
+      for (size_t j = j0; ok && j < j1; ++j)
+        ok = cudaMemcpyAsync(int_d + j * NN, intensity_h + (size_t)batch_idx_h[j] * NN, NN * 4, cudaMemcpyHostToDevice, cs2) == cudaSuccess;
+    ok = ok && cudaEventRecord(ready[c], cs2) == cudaSuccess;
+  }
+  if (!ok) { cudaStreamSynchronize(cs2); cleanup(); return PT_ERR_CUDA; }
+  g_chunk_ready = ready.data();
   rc = ptycho_gradient(&q, obj_d, pr_d, pos_d, int_d, nullptr, gO_d, gP_d, grad_pos_h ? gX_d : nullptr, nullptr, nullptr, nullptr,
                        loss_d, lpp_d, ws, workspace_bytes - off, st);
-  if (rc != PT_OK) return rc;
-  if (cudaMemcpyAsync(grad_object_h, gO_d, on * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaMemcpyAsync(grad_probe_h, gP_d, pn * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (grad_pos_h && cudaMemcpyAsync(grad_pos_h, gX_d, J * 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (loss_h && cudaMemcpyAsync(loss_h, loss_d, 8, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (loss_per_pos_h && cudaMemcpyAsync(loss_per_pos_h, lpp_d, J * 4, cudaMemcpyDeviceToHost, st) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaStreamSynchronize(st) != cudaSuccess) return PT_ERR_CUDA;
-  return PT_OK;
+  g_chunk_ready = nullptr;
+  if (rc != PT_OK) { cudaStreamSynchronize(cs2); cudaStreamSynchronize(st); cleanup(); return rc; }
+  ok = cudaMemcpyAsync(grad_object_h, gO_d, on * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(grad_probe_h, gP_d, pn * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  if (grad_pos_h) ok = ok && cudaMemcpyAsync(grad_pos_h, gX_d, J * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  if (loss_h) ok = ok && cudaMemcpyAsync(loss_h, loss_d, 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  if (loss_per_pos_h) ok = ok && cudaMemcpyAsync(loss_per_pos_h, lpp_d, J * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  const bool synced = cudaStreamSynchronize(st) == cudaSuccess;       // every copy-stream event has been waited for by now
+  cleanup();
+  return ok && synced ? PT_OK : PT_ERR_CUDA;
 }
 
 int32_t ptycho_status(void* workspace_d, void* cuda_stream) {
