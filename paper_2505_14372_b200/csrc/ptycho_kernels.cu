@@ -64,6 +64,7 @@ struct Ws {
   float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
   cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
   float* alpha_ji;     // [Jc][S]          per-position object step sizes alpha_{O,i,j} (PT_WANT_WEIGHTED_ILLUM only)
+  float* ilpart;       // [Jc][M][S][N^2]  R-native |Psi_{i,k}|^2 written by k_backward_pair (PT_WANT_ILLUM with paired modes)
   int32_t Jc;
   size_t total;
 };
@@ -90,16 +91,42 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   if (steps) pp += M * NN * sizeof(cf) + S * sizeof(float);
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
   if (p->flags & PT_EPIE) pp += (M * CL + 1) * S * sizeof(float) + 64;
-  *fixed = f + 12 * 256;   // slack for the per-array alignment of the chunked part
+  *fixed = f + 13 * 256;   // slack for the per-array alignment of the chunked part
   *per_pos = pp;
+}
+// optional per-position bytes: the |Psi|^2 staging of the illumination map (k_backward_pair writes it, the gather then reads
+// 4 bytes per mode instead of the 8-byte stash entries); 0 where it does not apply
+size_t il_bytes_per_pos(const pt_problem* p) {
+  if (!(p->flags & PT_WANT_ILLUM) || !use_pairs(p) || (p->flags & PT_EPIE)) return 0;
+  return (size_t)p->n_modes * p->n_slices * p->n * p->n * sizeof(float);
+}
+// positions in flight for a workspace of `bytes`, and whether the optional staging is used: it is when the whole batch still
+// fits with it, or when the batch is chunked anyway; not when it alone would force chunking (a caller who sized the workspace
+// for the batch without PT_WANT_ILLUM gets the same single chunk as before)
+struct ChunkPlan { size_t jc; bool il; };
+ChunkPlan plan_chunks(const pt_problem* p, size_t bytes) {
+  size_t fixed, pp;
+  ws_sizes(p, &fixed, &pp);
+  ChunkPlan c = {0, false};
+  if (bytes < fixed + pp) return c;
+  const size_t J = (size_t)p->n_batch, pil = il_bytes_per_pos(p);
+  size_t jc0 = (bytes - fixed) / pp;
+  if (jc0 > J) jc0 = J;
+  c.jc = jc0;
+  if (pil) {
+    size_t jc1 = (bytes - fixed) / (pp + pil);
+    if (jc1 > J) jc1 = J;
+    if (jc1 >= 1 && (jc1 == J || jc0 < J)) { c.jc = jc1; c.il = true; }
+  }
+  return c;
 }
 
 int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   size_t fixed, pp;
   ws_sizes(p, &fixed, &pp);
-  if (bytes < fixed + pp) return PT_ERR_WORKSPACE;
-  size_t jc = (bytes - fixed) / pp;
-  if (jc > (size_t)p->n_batch) jc = p->n_batch;
+  const ChunkPlan plan = plan_chunks(p, bytes);
+  if (plan.jc == 0) return PT_ERR_WORKSPACE;
+  const size_t jc = plan.jc;
   const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch, CL = cluster_of(p->n);
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   char* c = (char*)base;
@@ -128,6 +155,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
   w->alpha_ji = steps ? (float*)take(jc * S * sizeof(float)) : nullptr;
+  w->ilpart = plan.il ? (float*)take(jc * M * S * NN * sizeof(float)) : nullptr;
   w->Jc = (int32_t)jc;
   w->total = off;
   return off <= bytes ? PT_OK : PT_ERR_WORKSPACE;
@@ -744,7 +772,7 @@ __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 // Staging layout: [Jc][M/2][S][N^2].
 // ------------------------------------------------------------------------------------------------
 template <class G, int MODE>
-__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos) {
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos, int want_il) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -823,6 +851,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
     }
     float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
+    float2* il = (float2*)(P.w.ilpart + fld(pr, i));             // O12 staging: |Psi_{i,k}|^2 of this mode (only with want_il)
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
@@ -831,6 +860,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
+      if (MODE == 0 && want_il) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
       if (h == 0) tmem_st4(tb + 64 + 4 * p, g0, g1);             // first mode: keep gT_i on chip
       else {                                                     // second mode: the pair's sum goes to the staging buffer
         cf a0, a1;
@@ -1029,7 +1059,8 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
             for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
             if (ILLUM) {
               const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat;
-              for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
+              if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];
+              else for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
             }
             ar += wgt * sr; ai += wgt * si; al += wgt * sl;
           }
@@ -1040,7 +1071,8 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
         for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
         if (ILLUM) {
           const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
-          for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
+          if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];   // staged by k_backward_pair
+          else for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
       }
       }
@@ -1440,10 +1472,11 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
-      if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0, 0);
       else launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
     } else {
-      if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0,
+                              want_illum && kp.w.ilpart ? 1 : 0);
       else launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
     }
     LAUNCH_CHECK(K_backward, st);
@@ -1510,15 +1543,13 @@ size_t ptycho_workspace_min_bytes(const pt_problem* p) {
 
 int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) {
   if (validate(p) != PT_OK) return 0;
-  size_t f, pp; ws_sizes(p, &f, &pp);
-  if (workspace_bytes < f + pp) return 0;
-  size_t jc = (workspace_bytes - f) / pp;
-  return (int32_t)(jc > (size_t)p->n_batch ? (size_t)p->n_batch : jc);
+  return (int32_t)plan_chunks(p, workspace_bytes).jc;
 }
 
 size_t ptycho_workspace_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
   size_t f, pp; ws_sizes(p, &f, &pp);
+  pp += il_bytes_per_pos(p);             // the recommendation includes the optional staging of the illumination map
   const size_t cap = (size_t)49 << 30;   // config 3: 1554 positions = 84 / 42 whole waves of forward / paired-backward CTAs
   size_t jc = p->n_batch;
   if (f + jc * pp > cap) {

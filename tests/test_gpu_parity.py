@@ -242,8 +242,9 @@ def test_paired_and_unpaired_backward_agree(monkeypatch):
     monkeypatch.setenv("PTYCHO_NO_PAIR", "1")
     b = gpu_gradient(case, pbg, want_illum=True)
     assert rel_l2(a["grad_object"], b["grad_object"]) <= 2e-7
-    for k in ("grad_probe", "grad_pos", "loss_per_pos", "illum"):
+    for k in ("grad_probe", "grad_pos", "loss_per_pos"):
         assert a[k].tobytes() == b[k].tobytes(), k
+    assert rel_l2(a["illum"], b["illum"]) <= 2e-7                              # |Psi|^2 formed in float32 by the pair kernel, in fp64 by the gather
     assert a["grad_object"].tobytes() != b["grad_object"].tobytes()        # the switch really selected another kernel
 
 
