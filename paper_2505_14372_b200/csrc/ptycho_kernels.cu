@@ -771,8 +771,8 @@ __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 // the sum over the pair is taken in float32 in fixed order (first + second), the gather then sums the pairs in fp64.
 // Staging layout: [Jc][M/2][S][N^2].
 // ------------------------------------------------------------------------------------------------
-template <class G, int MODE>
-__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos, int want_il) {
+template <class G, int MODE, bool IL>   // IL: also stage |Psi_{i,k}|^2 for the illumination map (O12)
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
   extern __shared__ __align__(16) unsigned char smem_raw[];
@@ -851,7 +851,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
     }
     float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
-    float2* il = (float2*)(P.w.ilpart + fld(pr, i));             // O12 staging: |Psi_{i,k}|^2 of this mode (only with want_il)
+    float2* il = IL ? (float2*)(P.w.ilpart + fld(pr, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
@@ -860,7 +860,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
-      if (MODE == 0 && want_il) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
+      if (IL) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
       if (h == 0) tmem_st4(tb + 64 + 4 * p, g0, g1);             // first mode: keep gT_i on chip
       else {                                                     // second mode: the pair's sum goes to the staging buffer
         cf a0, a1;
@@ -1387,8 +1387,9 @@ int set_smem_attrs() {
   if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_backward<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward_pair<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward_pair<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward_pair<G, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward_pair<G, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
+  if (cudaFuncSetAttribute(k_backward_pair<G, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
   return PT_OK;
@@ -1472,11 +1473,12 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
-      if (paired) launch_fft<G>(k_backward_pair<G, 2>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0, 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 2, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
       else launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
     } else {
-      if (paired) launch_fft<G>(k_backward_pair<G, 0>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0,
-                              want_illum && kp.w.ilpart ? 1 : 0);
+      if (paired && want_illum && kp.w.ilpart)
+        launch_fft<G>(k_backward_pair<G, 0, true>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      else if (paired) launch_fft<G>(k_backward_pair<G, 0, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
       else launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
     }
     LAUNCH_CHECK(K_backward, st);
