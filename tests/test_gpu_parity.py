@@ -366,6 +366,15 @@ def test_gradient_host_matches_device_path():
     assert gP_h.numpy().tobytes() == g["grad_probe"].tobytes()
     assert gX_h.numpy().tobytes() == g["grad_pos"].tobytes()
     assert loss_h.item() == g["loss"]
+    # a batch through the index list (rows compacted on the way in), twice in a row on the same workspace
+    rows = np.array([7, 2, 11, 5, 14], np.int32)
+    gb = gpu_gradient(case, pbg, batch_idx=rows)
+    gXb = torch.empty((rows.size, 2), dtype=torch.float32).pin_memory()
+    for _ in range(2):
+        ptycho.gradient_host(pbg, obj_h, pr_h, pos_h, I_h, torch.from_numpy(rows), workspace=ws, grad_object_h=gO_h, grad_probe_h=gP_h,
+                             grad_pos_h=gXb, loss_h=loss_h)
+        assert gO_h.numpy().tobytes() == gb["grad_object"].tobytes() and gXb.numpy().tobytes() == gb["grad_pos"].tobytes()
+        assert loss_h.item() == gb["loss"]
 
 
 # ------------------------------------------------------------------------------------------------
@@ -423,6 +432,18 @@ def test_cfg3_full_size_sampled():
     assert 1 <= rows.size <= 16
     o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
     assert rel_l2(gO_h[:, py, px_], o["grad_object"][:, py, px_]) <= TOL_GRAD
+    # (4) the end-to-end entry bench.py times (host buffers, patterns copied chunk by chunk on a second stream while the chain
+    #     kernels run) gives bit for bit what the device-resident path gave
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    gO_p = torch.empty(obj.shape, dtype=torch.complex64).pin_memory(); gP_p = torch.empty(pr.shape, dtype=torch.complex64).pin_memory()
+    gX_p = torch.empty((J, 2), dtype=torch.float32).pin_memory(); loss_p = torch.zeros(1, dtype=torch.float64).pin_memory()
+    del ws
+    torch.cuda.empty_cache()
+    wsh = ptycho.make_workspace(pbg, J, J, host=True)
+    ptycho.gradient_host(pbg, pin(obj), pin(pr), pin(pos), pin(inten), workspace=wsh, grad_object_h=gO_p, grad_probe_h=gP_p, grad_pos_h=gX_p,
+                         loss_h=loss_p)
+    assert gO_p.numpy().tobytes() == gO_h.tobytes() and gX_p.numpy().tobytes() == gX_h.tobytes()
+    assert gP_p.numpy().tobytes() == gP.cpu().numpy().tobytes() and loss_p.item() == loss.item()
 
 
 # ------------------------------------------------------------------------------------------------
