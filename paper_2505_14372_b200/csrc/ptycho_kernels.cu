@@ -377,9 +377,48 @@ __device__ __forceinline__ void load_xv(cf (&wxv)[FL<G>::NXV], const cf* row, in
 }
 
 // v *= hx[qx] * hy[qy] (optionally conjugated) with the sharp band-limit mask (reading R9); hy from shared memory.
-// The mask test is hoisted out of the unrolled loop (block-uniform branch): the five configs run with the mask off.
+// Which of the thread's 32 Fourier pixels lie inside the band does not change from slice to slice: band_mask is formed once
+// per kernel (bit r = register r is inside), the mask test is a bit test, and the branch on "mask on / off" is block-uniform
+// and hoisted out of the unrolled loop (the five configs run with the mask off).
+template <class G>
+__device__ __forceinline__ uint32_t band_mask(float bandlim2, int t, unsigned rk) {
+  typedef FL<G> F;
+  uint32_t m = 0xffffffffu;
+  if (bandlim2 >= 0.0f) {
+    m = 0u;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+      const int sx = signed_freq(F::fq_x(rk, t, r), F::NF), sy = signed_freq(F::fq_y(rk, t, r), F::NF);
+      if (!((float)(sx * sx + sy * sy) > bandlim2)) m |= 1u << r;
+    }
+  }
+  return m;
+}
 template <class G, bool CONJ, bool MASK>
-__device__ __forceinline__ void apply_prop_body(cf (&v)[32], const cf (&wxv)[FL<G>::NXV], const cf* hyS, float bandlim2, int t, unsigned rk) {
+__device__ __forceinline__ void apply_prop_body(cf (&v)[32], const cf (&wxv)[FL<G>::NXV], const cf* hyS, uint32_t inside, int t, unsigned rk) {
+  typedef FL<G> F;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int qy = F::fq_y(rk, t, r);
+    cf wx = wxv[F::fq_xsel(r)], wy = hyS[qy];
+    if (CONJ) { wx.y = -wx.y; wy.y = -wy.y; }
+    cf h = cmul(wx, wy);
+    if (MASK && !((inside >> r) & 1u)) h = make_float2(0.f, 0.f);
+    v[r] = cmul(v[r], h);
+  }
+}
+template <class G, bool CONJ>
+__device__ __forceinline__ void apply_prop_s(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, uint32_t inside, int t, unsigned rk) {
+  cf wxv[FL<G>::NXV];
+  load_xv<G>(wxv, hxrow, t, 1.0f);
+  if (bandlim2 >= 0.0f) apply_prop_body<G, CONJ, true>(v, wxv, hyS, inside, t, rk);
+  else apply_prop_body<G, CONJ, false>(v, wxv, hyS, inside, t, rk);
+}
+
+// The backward kernels keep the mask test inside the loop: one more register live across their slice loop costs them more
+// (spills: 57.5 -> 59.5 ms per step at config 3) than the test costs in the band-limited variant.
+template <class G, bool CONJ, bool MASK>
+__device__ __forceinline__ void apply_prop_body_t(cf (&v)[32], const cf (&wxv)[FL<G>::NXV], const cf* hyS, float bandlim2, int t, unsigned rk) {
   typedef FL<G> F;
 #pragma unroll
   for (int r = 0; r < 32; ++r) {
@@ -395,11 +434,11 @@ __device__ __forceinline__ void apply_prop_body(cf (&v)[32], const cf (&wxv)[FL<
   }
 }
 template <class G, bool CONJ>
-__device__ __forceinline__ void apply_prop_s(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, int t, unsigned rk) {
+__device__ __forceinline__ void apply_prop_t(cf (&v)[32], const cf* hxrow, const cf* hyS, float bandlim2, int t, unsigned rk) {
   cf wxv[FL<G>::NXV];
   load_xv<G>(wxv, hxrow, t, 1.0f);
-  if (bandlim2 >= 0.0f) apply_prop_body<G, CONJ, true>(v, wxv, hyS, bandlim2, t, rk);
-  else apply_prop_body<G, CONJ, false>(v, wxv, hyS, bandlim2, t, rk);
+  if (bandlim2 >= 0.0f) apply_prop_body_t<G, CONJ, true>(v, wxv, hyS, bandlim2, t, rk);
+  else apply_prop_body_t<G, CONJ, false>(v, wxv, hyS, bandlim2, t, rk);
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -447,6 +486,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
       v[2 * p + 1] = cmul(make_float2(q.z, q.w), cmul(wxv[F::fq_xsel(2 * p + 1)], ry[F::fq_y(rk, t, 2 * p + 1)]));
     }
   }
+  const uint32_t inside = band_mask<G>(P.bandlim2, t, rk);
   for (int i = 0; i < S; ++i) {
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     {   // registers [2E, 32) of T_i into the warp's idle X1 region
@@ -468,7 +508,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     }
     if (i + 1 < S) early(i + 1);
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(Phi)    (Fourier layout)
-    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, t, rk);   // H5
+    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, inside, t, rk);   // H5
   }
   float4* out = (float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);   // H6: psi~ = F(Phi_{S-1}) / N
   const float sc = 1.0f / (float)NF;
@@ -646,7 +686,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       if (i == 0) break;                                         // probe / position terms handled below
     }
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(gPsi_i)  (Fourier layout)
-    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
+    if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
   }
   const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
   const cf* ry = rx + NF;
@@ -873,7 +913,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     if (h == 0) tmem_wait_st();
     if (s + 1 < 2 * S) early(s + 1);
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                        // F(gPsi_i)
-    if (i > 0) apply_prop_s<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
+    if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
     tmem_swap_field(tb, v);                                      // the other mode's turn
   }
   // v = G~ of the first mode, the second mode's is parked.  H12 / H13 per mode as in k_backward.
