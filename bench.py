@@ -336,7 +336,7 @@ def run_b200(args):
     # this run's positions per launch; null if the capture is of another kernel or workload
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1g_dominant_kernel_traffic.csv")) as f:
+        with open(os.path.join(ROOT, "profiles", "r1i_dominant_kernel_traffic.csv")) as f:
             tr = next(csv.DictReader(f))
         if tr["kernel"] == top and tr["workload"] == conf["workload"]:
             roof["traffic"] = (float(tr["dram_bytes_read"]) + float(tr["dram_bytes_write"])) * units_per_launch / float(tr["positions_per_launch"])
