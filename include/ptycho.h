@@ -12,6 +12,9 @@
  *   - all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*); nothing synchronises except
  *     ptycho_status() and the *_host convenience entry point.
  *   - every function returns int32 status: 0 = PT_OK, < 0 = error.  No exceptions, no printing, no abort.
+ *   - resources: the chain kernels take a whole SM each (up to 227 KB of shared memory, the full register file) and, with an
+ *     even number of modes, the backward kernel allocates the SM's tensor memory (tcgen05.alloc, all 512 columns at N >= 128)
+ *     for the duration of the kernel; PTYCHO_NO_PAIR=1 in the environment selects the kernel that does not (debugging aid).
  */
 #ifndef PTYCHO_H_
 #define PTYCHO_H_
