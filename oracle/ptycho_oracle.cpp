@@ -24,6 +24,7 @@
 // X_j, exit waves Psi_{i,k}, measured I_exp.  F is the unnormalised forward DFT
 // (F a)[q] = sum_r a[r] exp(-2 pi i (qy y + qx x)/N), Finv = F^H / N^2.
 
+#include <algorithm>
 #include <cmath>
 #include <complex>
 #include <cstdint>
@@ -177,24 +178,6 @@ void orc_position_split_floor(float X, float px, int32_t N, int32_t* i0, float* 
 // w_d = (d_y ? f_y : 1 - f_y)(d_x ? f_x : 1 - f_x)   ("sampled")
 static inline double bil_w(int d, double f) { return d ? f : 1.0 - f; }
 
-// patch[r] = sum_d w_d obj[i0 + r + d]; with adjoint != 0: obj[i0 + r + d] += w_d patch[r]   (exported for the pins)
-void orc_bilinear(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t i0y, int32_t i0x, double fy, double fx,
-                  double* patch, int32_t adjoint) {
-  for (int y = 0; y < N; ++y)
-    for (int x = 0; x < N; ++x) {
-      cd acc = 0.0;
-      for (int dy = 0; dy < 2; ++dy)
-        for (int dx = 0; dx < 2; ++dx) {
-          long o = (long)(i0y + y + dy) * onx + (i0x + x + dx);
-          double w = bil_w(dy, fy) * bil_w(dx, fx);
-          if (adjoint) { obj[2 * o] += w * patch[2 * ((long)y * N + x)]; obj[2 * o + 1] += w * patch[2 * ((long)y * N + x) + 1]; }
-          else acc += w * cd(obj[2 * o], obj[2 * o + 1]);
-        }
-      if (!adjoint) { patch[2 * ((long)y * N + x)] = acc.real(); patch[2 * ((long)y * N + x) + 1] = acc.imag(); }
-    }
-  (void)ony;
-}
-
 // O1: sub-pixel shift ramp R[q] = exp(-2 pi i (f(qy) dy + f(qx) dx))  (PAPER.md:115 P_k(r - X_j))
 static void shift_ramp(int N, double dy, double dx, cd* R) {
   for (int qy = 0; qy < N; ++qy)
@@ -232,43 +215,102 @@ void orc_propagator(int32_t N, double px, double lambda, double dz, double tx_mr
   for (long i = 0; i < (long)N * N; ++i) { H_out[2 * i] = H[i].real(); H_out[2 * i + 1] = H[i].imag(); }
 }
 
-// the linear pieces, exported so that the dot-product tests pin the very code the model uses -----
-// out = Finv(R(dy,dx) .* F(in))        (O2 with in = P_k)
+// ------------------------------------------------------------------------------------------
+// The linear pieces of the model.  forward_pos / adjoint_pos / orc_gradient below call exactly these
+// helpers, and the exported orc_shift / orc_propagate / orc_gather / orc_scatter_add wrappers call them
+// too, so the dot-product and coverage-map pins (tests/test_oracle_pins.py) run the model's own code.
+// ------------------------------------------------------------------------------------------
+// a[q] *= R[q]  (adjoint: conj(R[q]))                    — Fourier side of O2 / O9
+static void mul_ramp(long NN, cd* a, const cd* R, bool adjoint) {
+  for (long q = 0; q < NN; ++q) a[q] *= adjoint ? std::conj(R[q]) : R[q];
+}
+// a <- Finv(H .* F(a))  (adjoint: Finv(conj(H) .* F(a)))  — O3 / O8
+static void propagate_field(int N, cd* a, const cd* H, bool adjoint) {
+  F2(N, a);
+  for (long q = 0; q < (long)N * N; ++q) a[q] *= adjoint ? std::conj(H[q]) : H[q];
+  Finv2(N, a);
+}
+// patch[r] = slice[r0 + r]   (O3); slice = one object slice [ony][onx]
+static void gather_window(int N, int onx, const cd* slice, int r0y, int r0x, cd* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x) patch[(long)y * N + x] = slice[(long)(r0y + y) * onx + (r0x + x)];
+}
+// slice[r0 + r] += patch[r]  (O8 last line)
+static void scatter_add_window(int N, int onx, cd* slice, int r0y, int r0x, const cd* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x) slice[(long)(r0y + y) * onx + (r0x + x)] += patch[(long)y * N + x];
+}
+// bilinear variants (reading R1 secondary): patch[r] = sum_d w_d slice[i0 + r + d] and its adjoint
+static void gather_window_bilinear(int N, int onx, const cd* slice, int i0y, int i0x, double fy, double fx, cd* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x) {
+      cd acc = 0.0;
+      for (int dy = 0; dy < 2; ++dy)
+        for (int dx = 0; dx < 2; ++dx)
+          acc += bil_w(dy, fy) * bil_w(dx, fx) * slice[(long)(i0y + y + dy) * onx + (i0x + x + dx)];
+      patch[(long)y * N + x] = acc;
+    }
+}
+static void scatter_add_window_bilinear(int N, int onx, cd* slice, int i0y, int i0x, double fy, double fx, const cd* patch) {
+  for (int y = 0; y < N; ++y)
+    for (int x = 0; x < N; ++x)
+      for (int dy = 0; dy < 2; ++dy)
+        for (int dx = 0; dx < 2; ++dx)
+          slice[(long)(i0y + y + dy) * onx + (i0x + x + dx)] += bil_w(dy, fy) * bil_w(dx, fx) * patch[(long)y * N + x];
+}
+
+static std::vector<cd> to_cd(const double* in, long n) {
+  std::vector<cd> a(n);
+  for (long i = 0; i < n; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  return a;
+}
+static void from_cd(const std::vector<cd>& a, double* out) {
+  for (size_t i = 0; i < a.size(); ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+}
+// exported for the pins ---------------------------------------------------------------------
+// out = Finv(R(dy,dx) .* F(in))        (O2 with in = P_k; adjoint: conj(R))
 void orc_shift(int32_t N, const double* in, double dy, double dx, double* out, int32_t adjoint) {
-  std::vector<cd> a((long)N * N), R((long)N * N);
-  for (long i = 0; i < (long)N * N; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  std::vector<cd> a = to_cd(in, (long)N * N), R((long)N * N);
   shift_ramp(N, dy, dx, R.data());
   F2(N, a.data());
-  for (long i = 0; i < (long)N * N; ++i) a[i] *= adjoint ? std::conj(R[i]) : R[i];
+  mul_ramp((long)N * N, a.data(), R.data(), adjoint != 0);
   Finv2(N, a.data());
-  for (long i = 0; i < (long)N * N; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+  from_cd(a, out);
 }
 // out = Finv(H .* F(in)), or with adjoint: Finv(conj(H) .* F(in))   (O3 / O8)
 void orc_propagate(int32_t N, const double* in, double px, double lambda, double dz, double tx_mrad,
                    double ty_mrad, double bandlimit, double* out, int32_t adjoint) {
-  std::vector<cd> a((long)N * N), H((long)N * N);
-  for (long i = 0; i < (long)N * N; ++i) a[i] = cd(in[2 * i], in[2 * i + 1]);
+  std::vector<cd> a = to_cd(in, (long)N * N), H((long)N * N);
   propagator(N, px, lambda, dz, tx_mrad, ty_mrad, bandlimit, H.data());
-  F2(N, a.data());
-  for (long i = 0; i < (long)N * N; ++i) a[i] *= adjoint ? std::conj(H[i]) : H[i];
-  Finv2(N, a.data());
-  for (long i = 0; i < (long)N * N; ++i) { out[2 * i] = a[i].real(); out[2 * i + 1] = a[i].imag(); }
+  propagate_field(N, a.data(), H.data(), adjoint != 0);
+  from_cd(a, out);
 }
 // patch[r] = obj[r0 + r]   (O3)
 void orc_gather(int32_t N, int32_t ony, int32_t onx, const double* obj, int32_t r0y, int32_t r0x, double* patch) {
-  for (int y = 0; y < N; ++y)
-    for (int x = 0; x < N; ++x)
-      for (int c = 0; c < 2; ++c)
-        patch[2 * ((long)y * N + x) + c] = obj[2 * ((long)(r0y + y) * onx + (r0x + x)) + c];
-  (void)ony;
+  std::vector<cd> o = to_cd(obj, (long)ony * onx), pt((long)N * N);
+  gather_window(N, onx, o.data(), r0y, r0x, pt.data());
+  from_cd(pt, patch);
 }
 // obj[r0 + r] += patch[r]  (O8 last line)
 void orc_scatter_add(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t r0y, int32_t r0x, const double* patch) {
-  for (int y = 0; y < N; ++y)
-    for (int x = 0; x < N; ++x)
-      for (int c = 0; c < 2; ++c)
-        obj[2 * ((long)(r0y + y) * onx + (r0x + x)) + c] += patch[2 * ((long)y * N + x) + c];
-  (void)ony;
+  std::vector<cd> o = to_cd(obj, (long)ony * onx), pt = to_cd(patch, (long)N * N);
+  scatter_add_window(N, onx, o.data(), r0y, r0x, pt.data());
+  from_cd(o, obj);
+}
+
+// patch[r] = sum_d w_d obj[i0 + r + d]; with adjoint != 0: obj[i0 + r + d] += w_d patch[r]   (exported for the pins)
+void orc_bilinear(int32_t N, int32_t ony, int32_t onx, double* obj, int32_t i0y, int32_t i0x, double fy, double fx,
+                  double* patch, int32_t adjoint) {
+  std::vector<cd> o = to_cd(obj, (long)ony * onx);
+  if (adjoint) {
+    std::vector<cd> pt = to_cd(patch, (long)N * N);
+    scatter_add_window_bilinear(N, onx, o.data(), i0y, i0x, fy, fx, pt.data());
+    from_cd(o, obj);
+  } else {
+    std::vector<cd> pt((long)N * N);
+    gather_window_bilinear(N, onx, o.data(), i0y, i0x, fy, fx, pt.data());
+    from_cd(pt, patch);
+  }
 }
 
 // O6: per-pixel loss l(I, Iexp) and detector weight w = dl/dI
@@ -354,28 +396,19 @@ static int forward_pos(const Model& m, int jrow, PosWork& w) {
   w.R.resize(NN); shift_ramp(N, bil ? 0.0 : w.dy, bil ? 0.0 : w.dx, w.R.data());    // bilinear mode: probe unshifted, R = 1
   w.Psi.assign((long)S * M, std::vector<cd>()); w.T.assign(S, std::vector<cd>(NN));
   w.psit.assign(M, std::vector<cd>(NN)); w.I.assign(NN, 0.0);
-  for (int i = 0; i < S; ++i)                                                    // O3: T_i[r] = O_i[r0 + r]
-    for (int y = 0; y < N; ++y)
-      for (int x = 0; x < N; ++x) {
-        if (!bil) { w.T[i][(long)y * N + x] = m.obj[((long)i * p.obj_ny + (r0y + y)) * p.obj_nx + (r0x + x)]; continue; }
-        cd acc = 0.0;                                                            // bilinear: sum_d w_d O_i[i0 + r + d]
-        for (int dy = 0; dy < 2; ++dy)
-          for (int dx = 0; dx < 2; ++dx)
-            acc += bil_w(dy, w.dy) * bil_w(dx, w.dx) * m.obj[((long)i * p.obj_ny + (r0y + y + dy)) * p.obj_nx + (r0x + x + dx)];
-        w.T[i][(long)y * N + x] = acc;
-      }
+  const long os = (long)p.obj_ny * p.obj_nx;
+  for (int i = 0; i < S; ++i) {                                                  // O3: T_i[r] = O_i[r0 + r]
+    if (!bil) gather_window(N, p.obj_nx, m.obj.data() + i * os, r0y, r0x, w.T[i].data());
+    else gather_window_bilinear(N, p.obj_nx, m.obj.data() + i * os, r0y, r0x, w.dy, w.dx, w.T[i].data());
+  }
   for (int k = 0; k < M; ++k) {
-    std::vector<cd> cur(NN);
-    for (long q = 0; q < NN; ++q) cur[q] = w.R[q] * m.Pt[k][q];                  // O2
+    std::vector<cd> cur = m.Pt[k];
+    mul_ramp(NN, cur.data(), w.R.data(), false);                                 // O2: Psi_0 = Finv(R .* P~_k)
     Finv2(N, cur.data());
     for (int i = 0; i < S; ++i) {
       w.Psi[(long)i * M + k] = cur;                                              // entering wave Psi_{i,k}
       for (long r = 0; r < NN; ++r) cur[r] *= w.T[i][r];                         // Phi_{i,k} = Psi .* T
-      if (i < S - 1) {                                                           // O3 propagate (reading R10: none after the last slice)
-        F2(N, cur.data());
-        for (long q = 0; q < NN; ++q) cur[q] *= m.H[i][q];
-        Finv2(N, cur.data());
-      }
+      if (i < S - 1) propagate_field(N, cur.data(), m.H[i].data(), false);       // O3 propagate (reading R10: none after the last slice)
     }
     F2(N, cur.data());                                                           // O5 far field, orthonormal (reading R5)
     for (long q = 0; q < NN; ++q) { cur[q] /= (double)N; w.I[q] += std::norm(cur[q]); }
@@ -411,15 +444,14 @@ static void adjoint_pos(const Model& m, int jrow, PosWork& w, double* loss_j,
       const std::vector<cd>& Psi = w.Psi[(long)i * M + k];
       for (long r = 0; r < NN; ++r) gT[i][r] += std::conj(Psi[r]) * g[r];        // gT_i += conj(Psi) .* gPhi
       for (long r = 0; r < NN; ++r) g[r] = std::conj(w.T[i][r]) * g[r];          // gPsi = conj(T) .* gPhi
-      if (i > 0) {
-        F2(N, g.data());
-        for (long q = 0; q < NN; ++q) g[q] *= std::conj(m.H[i - 1][q]);
-        Finv2(N, g.data());                                                      // gPhi_{i-1}
-      }
+      if (i > 0) propagate_field(N, g.data(), m.H[i - 1].data(), true);          // gPhi_{i-1} = Finv(conj(H_{i-1}) .* F(gPsi_i))
     }
     F2(N, g.data());                                                             // O9: G~ = F(gPsi_0)
-    if (gPt_acc)
-      for (long q = 0; q < NN; ++q) (*gPt_acc)[k][q] += std::conj(w.R[q]) * g[q];
+    if (gPt_acc) {
+      std::vector<cd> c = g;
+      mul_ramp(NN, c.data(), w.R.data(), true);                                  //     gP~_k += conj(R) .* G~
+      for (long q = 0; q < NN; ++q) (*gPt_acc)[k][q] += c[q];
+    }
     for (int a = 0; a < 2 && p.shift_mode != 1; ++a) {                           // O10 (Fourier-shift mode)
       cd acc = 0.0;
       for (int qy = 0; qy < N; ++qy)
@@ -511,25 +543,22 @@ int32_t orc_gradient(const orc_problem* p, const float* object, const float* pro
       }
       std::vector<std::vector<cd>> gT; double gd[2];
       adjoint_pos(m, jrow, w, &Lj[jb], gT, &gPt_loc, gd, false);
-      for (int i = 0; i < S; ++i)                                               // O8 last line: scatter-add
-        for (int y = 0; y < N; ++y)
-          for (int x = 0; x < N; ++x) {
-            double s = 0.0;                                                     // O12
-            if (illum) for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][(long)y * N + x]);
-            if (p->shift_mode != 1) {
-              long o = ((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x);
-              gO_loc[o] += gT[i][(long)y * N + x];
-              if (illum) il_loc[o] += s;
-            } else {                                                            // bilinear mode: the same four weights
-              for (int dy = 0; dy < 2; ++dy)
-                for (int dx = 0; dx < 2; ++dx) {
-                  long o = ((long)i * p->obj_ny + (w.r0y + y + dy)) * p->obj_nx + (w.r0x + x + dx);
-                  double wt = bil_w(dy, w.dy) * bil_w(dx, w.dx);
-                  gO_loc[o] += wt * gT[i][(long)y * N + x];
-                  if (illum) il_loc[o] += wt * s;
-                }
-            }
-          }
+      const long os = (long)p->obj_ny * p->obj_nx;
+      std::vector<cd> il_patch(illum ? NN : 0), il_slice(illum ? os : 0);
+      for (int i = 0; i < S; ++i) {                                             // O8 last line: scatter-add
+        if (illum) {                                                            // O12: sum_k |Psi_{i,k}|^2, scattered like gT_i
+          for (long r = 0; r < NN; ++r) { double s = 0.0; for (int k = 0; k < M; ++k) s += std::norm(w.Psi[(long)i * M + k][r]); il_patch[r] = s; }
+          std::fill(il_slice.begin(), il_slice.end(), cd(0.0));
+        }
+        if (p->shift_mode != 1) {
+          scatter_add_window(N, p->obj_nx, gO_loc.data() + i * os, w.r0y, w.r0x, gT[i].data());
+          if (illum) scatter_add_window(N, p->obj_nx, il_slice.data(), w.r0y, w.r0x, il_patch.data());
+        } else {                                                                // bilinear mode: the same four weights
+          scatter_add_window_bilinear(N, p->obj_nx, gO_loc.data() + i * os, w.r0y, w.r0x, w.dy, w.dx, gT[i].data());
+          if (illum) scatter_add_window_bilinear(N, p->obj_nx, il_slice.data(), w.r0y, w.r0x, w.dy, w.dx, il_patch.data());
+        }
+        if (illum) for (long o = 0; o < os; ++o) il_loc[i * os + o] += il_slice[o].real();
+      }
       if (grad_pos) { grad_pos[2 * jb + 0] = gd[0] / (double)p->pixel_size; grad_pos[2 * jb + 1] = gd[1] / (double)p->pixel_size; }
     }
 #pragma omp critical

@@ -454,6 +454,48 @@ def test_lsqml_terms_vs_torch_intermediates():
     assert np.abs(st[:, 1:2 * S:2] - den).max() < 1e-9 * np.abs(den).max()
 
 
+@pytest.mark.parametrize("S", [1, 2])
+def test_lsqml_probe_and_position_terms_numpy_restatement(S):
+    # O14 probe / position terms written out in numpy (PAPER.md:221 applied to the probe and to the shift, readings R19, R21):
+    #   v_k = shift_j(dPhat_k) T_0,  s_{a,k} = Finv(-2 pi i f_a R P~_k) T_0,  chi_{0,k} = -gPhi_{0,k}
+    #   numP = sum_k Re<chi, v>, denP = sum_k |v|^2, numX_a = sum_k Re<chi, s_a>, denX_a = sum_k |s_a|^2
+    # S = 1: chi_0 is the numpy one-liner -N Finv(w psi~), so num and den are both pinned; S = 2: the denominators only
+    # (they must use the FIRST slice's patch and sum over both modes).
+    n, on, M, J = 16, 40, 2, 3
+    pb, obj, probe, pos = small_problem(n=n, M=M, S=S, on=on, J=J, loss=orc.LOSS_POISSON, eps=0.8)
+    pb.lsqml_delta_o = 0.7; pb.lsqml_delta_p = 0.2
+    Iexp = orc.forward_loss(pb, (obj * 1.05).astype(np.complex64), probe, pos)["intensity"].astype(np.float32) + 0.1
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], g["illum"] + 0.5)
+    f = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n) / n
+    dPhat = -g["grad_probe"] / (1.0 + float(np.float32(0.2)))
+    Pt = np.fft.fft2(probe.astype(complex))
+    for j in range(J):
+        r0y, dy = orc.position_split(float(pos[j, 0]), pb.pixel_size, n); r0x, dx = orc.position_split(float(pos[j, 1]), pb.pixel_size, n)
+        R = np.exp(-2j * np.pi * (f[:, None] * dy + f[None, :] * dx))
+        T0 = obj[0, r0y:r0y + n, r0x:r0x + n].astype(complex)
+        numP = denP = 0.0; numX = np.zeros(2); denX = np.zeros(2)
+        if S == 1:
+            psit = np.stack([np.fft.fft2(np.fft.ifft2(R * Pt[k]) * T0) / n for k in range(M)])
+            w = 1 - Iexp[j] / ((np.abs(psit) ** 2).sum(0) + float(np.float32(0.8)))
+        for k in range(M):
+            v = np.fft.ifft2(R * np.fft.fft2(dPhat[k])) * T0
+            sa = [np.fft.ifft2(-2j * np.pi * fa * R * Pt[k]) * T0 for fa in (f[:, None] + 0 * f[None, :], f[None, :] + 0 * f[:, None])]
+            denP += np.sum(np.abs(v) ** 2)
+            for a in range(2):
+                denX[a] += np.sum(np.abs(sa[a]) ** 2)
+            if S == 1:
+                chi = -n * np.fft.ifft2(w * psit[k])
+                numP += np.sum(np.real(chi * np.conj(v)))
+                for a in range(2):
+                    numX[a] += np.sum(np.real(chi * np.conj(sa[a])))
+        assert abs(st[j, 2 * S + 1] - denP) < 1e-10 * denP
+        assert abs(st[j, 2 * S + 3] - denX[0]) < 1e-10 * denX[0] and abs(st[j, 2 * S + 5] - denX[1]) < 1e-10 * denX[1]
+        if S == 1:
+            assert abs(st[j, 2 * S] - numP) < 1e-9 * abs(numP)
+            assert abs(st[j, 2 * S + 2] - numX[0]) < 1e-9 * abs(numX[0]) and abs(st[j, 2 * S + 4] - numX[1]) < 1e-9 * abs(numX[1])
+
+
 def test_lsqml_alpha_closed_form_single_position():
     # single position, single slice, one mode, illum_prev = this position's |Psi|^2, delta_O -> 0, gamma = 0:
     # dOhat|patch = conj(Psi) chi / |Psi|^2, so dOhat Psi = chi and alpha_O = sum|chi|^2 / sum|chi|^2 = 1,
