@@ -7,14 +7,19 @@
  *   - F is the unnormalised forward DFT with kernel exp(-2 pi i q.r/N); zero frequency at index [0][0].
  *   - gradients are g = dL/d conj(z); a descent step is z <- z - lr*g.
  *   - pointers ending in _d are DEVICE pointers, _h HOST pointers.  The library never allocates device
- *     memory, keeps no pointer after a call returns and has no global state (re-entrant across streams).
+ *     memory and keeps no pointer after a call returns.  The device-path calls are re-entrant across streams and
+ *     threads; process-wide state is limited to (a) a once-per-device record that the kernels' shared-memory limits
+ *     have been set, (b) the copy stream and events of ptycho_gradient_host, created on first use and reused (that
+ *     call is serialised by a lock), and (c) the per-THREAD launch counter and optional profiling record below.
  *     pt_problem / pt_update / slice_thickness are HOST memory, read synchronously during the call.
+ *   - workspace_d: DEVICE memory, 256-byte aligned.  Its first 256 bytes hold the deferred status word: the caller
+ *     zeroes them once when the buffer is allocated (cudaMemset); ptycho_status() reads and clears the word.
  *   - all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*); nothing synchronises except
  *     ptycho_status() and the *_host convenience entry point.
  *   - every function returns int32 status: 0 = PT_OK, < 0 = error.  No exceptions, no printing, no abort.
  *   - resources: the chain kernels take a whole SM each (up to 227 KB of shared memory, the full register file) and, with an
  *     even number of modes, the backward kernel allocates the SM's tensor memory (tcgen05.alloc, all 512 columns at N >= 128)
- *     for the duration of the kernel; PTYCHO_NO_PAIR=1 in the environment selects the kernel that does not (debugging aid).
+ *     for the duration of the kernel; the flag PT_NO_MODE_PAIRS selects the kernel that does not (debugging aid).
  */
 #ifndef PTYCHO_H_
 #define PTYCHO_H_
@@ -47,6 +52,8 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
                                        * W_i = sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2, alpha_{O,i,j} = numO[j,i] / (denO[j,i] +
                                        * lsqml_gamma): the per-position step sizes of PAPER.md:221 weighting the slice update as
                                        * PAPER.md:225 prints it (reading R24); used by PT_UPDATE_LSQML_WEIGHTED              */
+       PT_NO_MODE_PAIRS = 128,        /* debugging aid: the backward pass runs one mode per CTA even when the mode count is even
+                                       * (no tensor-memory allocation); results differ only by the rounding of one float32 add */
        PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of
                                        * gradients: grad_object_d <- sum_{j,k} conj(Psi_i,k)/max|Psi_i,k|^2
                                        * chi_i,k (scattered), grad_probe_d <- (1/J) sum_j shift_j^-1(chi'_0,k), chi~ = (sqrt(Iexp+c)/
@@ -64,7 +71,9 @@ typedef struct {
   int32_t n_slices;               /* S >= 1 object slices O_i                                    */
   int32_t obj_ny, obj_nx;         /* object slice size in px (>= N)                                             */
   int32_t n_pos_total;            /* rows of positions_d / intensity_d                                          */
-  int32_t n_batch;                /* J: positions in this call; batch_idx_d has J entries (NULL: rows 0..J-1)   */
+  int32_t n_batch;                /* J: positions in this call; batch_idx_d has J entries (NULL: rows 0..J-1).  Entries
+                                   * outside [0, n_pos_total) are clamped and raise PT_ERR_OUT_OF_BOUNDS (deferred).  A row
+                                   * must not appear twice in a batch whose positions are updated (the updates would race) */
   float pixel_size;               /* Angstrom / px (probe and object)                                           */
   float wavelength;               /* Angstrom                                                                   */
   const float *slice_thickness;   /* HOST, S entries (Angstrom); entry S-1 unused (R10)                         */
@@ -216,7 +225,10 @@ int32_t ptycho_adam_update_real(float *z_d, const float *g_d, float *m_d, float 
  * batch rows' intensities host->device into the workspace, runs ptycho_gradient, copies gradients and loss
  * back, and synchronises the stream.  The patterns are copied chunk by chunk on a second stream that lives for the duration
  * of the call, in the order the pass consumes them, so the copies overlap the chain kernels (use pinned host memory).
- * Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL. */
+ * Workspace must be ptycho_workspace_host_bytes(p).  batch_idx_h may be NULL; with an index list the whole position table and
+ * the list are copied once and the rows compacted on the device, and the patterns travel as one copy per run of consecutive
+ * rows.  The call reads the pass's own deferred status before it returns: PT_ERR_OUT_OF_BOUNDS (a window left the object and
+ * was clamped, R4, or an index outside [0, n_pos_total)) or PT_ERR_NONFINITE come back as the return value. */
 size_t ptycho_workspace_host_bytes(const pt_problem *p);
 int32_t ptycho_gradient_host(const pt_problem *p, const pt_c64 *object_h, const pt_c64 *probe_h,
                              const float *positions_h, const float *intensity_h, const int32_t *batch_idx_h,

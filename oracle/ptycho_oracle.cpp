@@ -823,12 +823,15 @@ int32_t orc_epie(const orc_problem* p, const float* object, const float* probe, 
       for (int i = S - 1; i >= 0; --i) {
         const std::vector<cd>& Psi = w.Psi[(long)i * M + k];
         double pmax = 0.0; for (long r = 0; r < NN; ++r) pmax = std::max(pmax, std::norm(Psi[r]));
+        // PAPER.md:203 divides by max|Psi|^2; an identically zero wave (an unused probe mode) gives 0/0 there.  Reading R23b
+        // (DESIGN.md §3): such a wave contributes nothing, i.e. 1/max is taken as 0; likewise 1/max|T|^2 for an opaque window.
+        const double ipmax = pmax > 0.0 ? 1.0 / pmax : 0.0, itmax = tmax[i] > 0.0 ? 1.0 / tmax[i] : 0.0;
         for (int y = 0; y < N; ++y)
           for (int x = 0; x < N; ++x) {
             long r = (long)y * N + x;
-            dO[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] += std::conj(Psi[r]) / pmax * chi[r];
+            dO[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] += std::conj(Psi[r]) * ipmax * chi[r];
           }
-        for (long r = 0; r < NN; ++r) chi[r] = std::conj(w.T[i][r]) / tmax[i] * chi[r];
+        for (long r = 0; r < NN; ++r) chi[r] = std::conj(w.T[i][r]) * itmax * chi[r];
         if (i > 0) {
           F2(N, chi.data());
           for (long q = 0; q < NN; ++q) chi[q] *= std::conj(m.H[i - 1][q]);

@@ -25,6 +25,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <mutex>
 #include <vector>
 
 #include "../../include/ptycho.h"
@@ -46,6 +47,7 @@ struct Ws {
   cf* ramps;           // [J][2][N]  (rx, ry)
   int32_t* r0;         // [J][2]  (y, x)
   float* delta;        // [J][2]
+  int32_t* rows;       // [J]     checked row of positions / intensity for each batch entry (k_setup_pos)
   cf* Pt;              // [M][N^2]  F-native, unscaled
   cf* Qt;              // [M][N^2]  F-native: F(dPhat_k) for the step-size sweep
   double2* gPt_acc;    // [M][N^2]  F-native accumulators
@@ -71,8 +73,8 @@ struct Ws {
 
 inline size_t align_up(size_t x) { return (x + 255) & ~(size_t)255; }
 // Two modes per CTA in the backward pass (k_backward_pair: the pair's patch gradients are summed on chip and staged once)
-// whenever the number of modes is even; PTYCHO_NO_PAIR in the environment forces one mode per CTA (a debugging switch).
-inline bool use_pairs(const pt_problem* p) { return (p->n_modes % 2) == 0 && !getenv("PTYCHO_NO_PAIR"); }
+// whenever the number of modes is even; the flag PT_NO_MODE_PAIRS forces one mode per CTA (a debugging switch).
+inline bool use_pairs(const pt_problem* p) { return (p->n_modes % 2) == 0 && !(p->flags & PT_NO_MODE_PAIRS); }
 inline size_t staged_planes(const pt_problem* p) { return use_pairs(p) ? p->n_modes / 2 : p->n_modes; }   // gT planes per position
 inline size_t cluster_of(int n) { return n == 256 ? 4 : 1; }   // CTAs per field (Geo<n>::CL)
 
@@ -82,7 +84,7 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   size_t f = 256;
   f += 2 * align_up((S > 1 ? S - 1 : 1) * N * sizeof(cf));
-  f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float));
+  f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float)) + align_up(J * sizeof(int32_t));
   f += 2 * align_up(M * NN * sizeof(cf)) + align_up(M * NN * sizeof(double2));
   f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
   f += align_up(J * M * CL * (2 * S + 6) * sizeof(double));
@@ -138,6 +140,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->ramps = (cf*)take(J * 2 * N * sizeof(cf));
   w->r0 = (int32_t*)take(J * 2 * sizeof(int32_t));
   w->delta = (float*)take(J * 2 * sizeof(float));
+  w->rows = (int32_t*)take(J * sizeof(int32_t));
   w->Pt = (cf*)take(M * NN * sizeof(cf));
   w->Qt = (cf*)take(M * NN * sizeof(cf));
   w->gPt_acc = (double2*)take(M * NN * sizeof(double2));
@@ -166,6 +169,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
 // ------------------------------------------------------------------------------------------------
 struct KP {
   int N, M, S, ony, onx, J;          // J = batch size
+  int Jtot;                          // rows of positions / intensity (n_pos_total)
   int Mg;                            // patch-gradient planes per position in the staging buffer: M, or M/2 after k_backward_pair
   int j0, jc;                        // current chunk: batch-local offset and count
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
@@ -207,7 +211,12 @@ __global__ void k_setup_prop(PropArgs a) {
 // ------------------------------------------------------------------------------------------------
 __global__ void k_setup_pos(KP P) {
   const int jb = blockIdx.x, q = threadIdx.x, N = P.N;
-  const int row = P.batch_idx ? P.batch_idx[jb] : jb;
+  int row = P.batch_idx ? P.batch_idx[jb] : jb;
+  if (row < 0 || row >= P.Jtot) {                                 // a batch entry outside the tables: clamp + raise, as R4
+    if (q == 0) atomicOr(P.w.status, kStatusOOB);
+    row = row < 0 ? 0 : P.Jtot - 1;
+  }
+  if (q == 0) P.w.rows[jb] = row;                                 // k_loss reads the checked row
   float d[2]; int r0[2];
 #pragma unroll
   for (int a = 0; a < 2; ++a) {
@@ -526,7 +535,7 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int
   constexpr int NF = F::NF, NNS = F::NNS, CL = G::CL;
   __shared__ double red[(G::T / 32) * 1];
   const int t = threadIdx.x, jl = blockIdx.x / CL, rk = blockIdx.x - jl * CL, jb = P.j0 + jl;
-  const int row = P.batch_idx ? P.batch_idx[jb] : jb;
+  const int row = P.w.rows[jb];
   float I[32];
 #pragma unroll
   for (int r = 0; r < 32; ++r) I[r] = 0.f;
@@ -637,7 +646,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
       if (MODE == 2) {
         float pm = 0.f;
         for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pair * S + i) * CL + c]);
-        s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
+        const float tm = P.w.tmax[(size_t)jl * S + i];
+        s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;   // a dead mode / an opaque window contributes nothing
       }
       float4* gt = (float4*)(P.w.gTpart + fld(i));
 #pragma unroll
@@ -888,7 +898,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     if (MODE == 2) {
       float pm = 0.f;
       for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pr * S + i) * CL + c]);
-      s1 = 1.0f / pm; s2 = 1.0f / P.w.tmax[(size_t)jl * S + i];
+      const float tm = P.w.tmax[(size_t)jl * S + i];
+      s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;
     }
     float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
     float2* il = IL ? (float2*)(P.w.ilpart + fld(pr, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
@@ -1201,7 +1212,9 @@ __global__ void __launch_bounds__(256) k_objtrans(KP P, float* out, int accumula
   for (int jbase = 0; jbase < P.J; jbase += 256) {
     const int cnt = min(256, P.J - jbase);
     if ((int)threadIdx.x < cnt) {
-      const int jb = jbase + threadIdx.x, row = P.batch_idx ? P.batch_idx[jb] : jb;
+      const int jb = jbase + threadIdx.x;
+      int row = P.batch_idx ? P.batch_idx[jb] : jb;
+      if (row < 0 || row >= P.Jtot) { atomicOr(P.w.status, kStatusOOB); row = row < 0 ? 0 : P.Jtot - 1; }
       int r0[2];
 #pragma unroll
       for (int a = 0; a < 2; ++a) {
@@ -1295,10 +1308,13 @@ __global__ void k_axpy(float* z, const float* g, float a, size_t n) {
   size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (i < n) z[i] = fmaf(a, g[i], z[i]);
 }
-__global__ void k_pos_sgd(float* pos, const float* g, const int32_t* idx, float lr, int J) {
+// (rows outside [0, n_rows) are skipped; the gradient call that produced g has already raised PT_ERR_OUT_OF_BOUNDS for them.
+//  A batch must not name a row twice: the two updates would race.)
+__global__ void k_pos_sgd(float* pos, const float* g, const int32_t* idx, float lr, int J, int n_rows) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= J) return;
   int row = idx ? idx[j] : j;
+  if (row < 0 || row >= n_rows) return;
   pos[2 * row] -= lr * g[2 * j]; pos[2 * row + 1] -= lr * g[2 * j + 1];
 }
 // alpha[c] = sum_j num / (sum_j den + gamma) for c = 0..S (S object slices, then the probe); one block per c
@@ -1333,10 +1349,11 @@ __global__ void k_lsqml_probe(cf* Pr, const cf* gP, const float* alpha, int S, f
   const float a = beta * alpha[S] * (-1.0f / ((precond ? precond[i % NN] : 1.0f) + delta_p));
   Pr[i] = make_float2(fmaf(a, gP[i].x, Pr[i].x), fmaf(a, gP[i].y, Pr[i].y));
 }
-__global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* idx, int J, int S, float px, float gamma) {
+__global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* idx, int J, int S, float px, float gamma, int n_rows) {
   int j = blockIdx.x * blockDim.x + threadIdx.x;
   if (j >= J) return;
   const int W = 2 * S + 6; int row = idx ? idx[j] : j;
+  if (row < 0 || row >= n_rows) return;
   const float* s = step_terms + (size_t)j * W + 2 * S + 2;
   pos[2 * row] += px * s[0] / (s[1] + gamma);
   pos[2 * row + 1] += px * s[2] / (s[3] + gamma);
@@ -1355,9 +1372,6 @@ const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
                                          "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam"};
 thread_local int64_t g_launches = 0;
-// ptycho_gradient_host only: one event per chunk, recorded on its copy stream when that chunk's measured patterns have
-// arrived on the device; the gradient pass waits for chunk c's event before the first kernel that reads them (k_loss)
-thread_local cudaEvent_t* g_chunk_ready = nullptr;
 thread_local bool g_prof_on = false;
 struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
 thread_local std::vector<ProfMark> g_prof;
@@ -1395,7 +1409,7 @@ int validate(const pt_problem* p) {
 KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64* probe, const float* positions,
            const float* intensity, const int32_t* batch_idx) {
   KP k;
-  k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch;
+  k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch; k.Jtot = p->n_pos_total;
   k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
   k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
@@ -1418,21 +1432,30 @@ cudaError_t launch_fft(void (*kern)(KArgs...), unsigned grid, size_t smem, cudaS
   return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// dynamic shared-memory limits of the FFT kernels: set once per process and geometry (per device: the attribute is per context)
 template <class G>
-int set_smem_attrs() {
+int set_smem_attrs_now() {
   const int b = (int)fft_smem_bytes<G>();
   const int c = (int)chain_smem_bytes<G>();
-  if (cudaFuncSetAttribute(k_forward<G, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_forward<G, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward<G, 0>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward<G, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward<G, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward_pair<G, 0, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward_pair<G, 0, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_backward_pair<G, 2, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, c) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_probe_fft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
-  if (cudaFuncSetAttribute(k_probe_ifft<G>, cudaFuncAttributeMaxDynamicSharedMemorySize, b) != cudaSuccess) return PT_ERR_CUDA;
-  return PT_OK;
+  bool ok = true;
+  auto set = [&](const void* f, int bytes) { ok = ok && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess; };
+  set((const void*)k_forward<G, true>, c); set((const void*)k_forward<G, false>, c);
+  set((const void*)k_backward<G, 0>, c); set((const void*)k_backward<G, 1>, c); set((const void*)k_backward<G, 2>, c);
+  set((const void*)k_backward_pair<G, 0, false>, c); set((const void*)k_backward_pair<G, 0, true>, c); set((const void*)k_backward_pair<G, 2, false>, c);
+  set((const void*)k_probe_fft<G>, b); set((const void*)k_probe_ifft<G>, b);
+  return ok ? PT_OK : PT_ERR_CUDA;
+}
+template <class G>
+int set_smem_attrs() {
+  static std::mutex mu;
+  static unsigned done_mask = 0;                                   // bit d: device d configured
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return PT_ERR_CUDA;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev < 32 && (done_mask >> dev) & 1u) return PT_OK;
+  const int rc = set_smem_attrs_now<G>();
+  if (rc == PT_OK && dev < 32) done_mask |= 1u << dev;
+  return rc;
 }
 
 // common prologue: tables, position split, probe spectrum
@@ -1478,7 +1501,9 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
 
 template <class G>
 int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, float* illum, const float* illum_prev,
-                 float* step_terms, double* loss_d, float* loss_per_pos_d, cudaStream_t st) {
+                 float* step_terms, double* loss_d, float* loss_per_pos_d, cudaStream_t st, const cudaEvent_t* chunk_ready) {
+  // chunk_ready (ptycho_gradient_host only): one event per chunk, recorded on its copy stream when that chunk's measured
+  // patterns have arrived on the device; the pass waits for chunk c's event before the first kernel that reads them (k_loss)
   int rc = prologue<G>(p, kp, st);
   if (rc != PT_OK) return rc;
   const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
@@ -1505,7 +1530,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
-    if (g_chunk_ready && cudaStreamWaitEvent(st, g_chunk_ready[j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
+    if (chunk_ready && cudaStreamWaitEvent(st, chunk_ready[j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
     if (epie) {
@@ -1570,6 +1595,73 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   return PT_OK;
 }
 
+// rows compacted on the device (ptycho_gradient_host with an index list): out[j] = table[rows[j]]
+__global__ void k_gather_rows(const float2* table, const int32_t* rows, float2* out, int J) {
+  const int j = blockIdx.x * blockDim.x + threadIdx.x;
+  if (j < J) out[j] = table[rows[j]];
+}
+
+// ptycho_gradient_host's copy stream and events: created once per device, reused by later calls, never destroyed (the only
+// process-wide state of the library; the lock serialises concurrent host-path calls)
+struct HostPoolDev { int dev; cudaStream_t copy; cudaEvent_t start; std::vector<cudaEvent_t> ready; };
+struct HostPool {
+  std::mutex mu;
+  std::vector<HostPoolDev> devs;
+  HostPoolDev* cur = nullptr;
+  bool acquire(size_t nchunk) {
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return false;
+    cur = nullptr;
+    for (auto& d : devs) if (d.dev == dev) cur = &d;
+    if (!cur) {
+      HostPoolDev d; d.dev = dev; d.copy = nullptr; d.start = nullptr;
+      if (cudaStreamCreateWithFlags(&d.copy, cudaStreamNonBlocking) != cudaSuccess) return false;
+      if (cudaEventCreateWithFlags(&d.start, cudaEventDisableTiming) != cudaSuccess) return false;
+      devs.push_back(d);
+      cur = &devs.back();
+    }
+    while (cur->ready.size() < nchunk) {
+      cudaEvent_t e;
+      if (cudaEventCreateWithFlags(&e, cudaEventDisableTiming) != cudaSuccess) return false;
+      cur->ready.push_back(e);
+    }
+    return true;
+  }
+};
+HostPool& host_pool() { static HostPool hp; return hp; }
+
+int32_t gradient_impl(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
+                        const float* intensity_d, const int32_t* batch_idx_d, pt_c64* grad_object_d, pt_c64* grad_probe_d,
+                        float* grad_pos_d, float* illum_d, const float* illum_prev_d, float* step_terms_d, double* loss_d,
+                        float* loss_per_pos_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream, const cudaEvent_t* chunk_ready) {
+  int rc = validate(p);
+  if (rc != PT_OK) return rc;
+  if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
+  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
+  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
+  if (p->flags & PT_WANT_WEIGHTED_ILLUM) {
+    if (!(p->flags & PT_WANT_ILLUM) || !(p->flags & PT_WANT_STEP_SIZES) || (p->flags & PT_EPIE)) return PT_ERR_BAD_PARAM;
+    if (!illum_d || !step_terms_d) return PT_ERR_NULL;
+    if (!(p->lsqml_gamma >= 0.f)) return PT_ERR_BAD_PARAM;
+  }
+  // ePIE directions (PAPER.md:173: the optimal wavefront update is given for the amplitude model): amplitude loss,
+  // Fourier-shift mode, no step-size terms, no position gradient
+  if ((p->flags & PT_EPIE) && (p->loss != PT_LOSS_AMPLITUDE || p->shift_mode != PT_SHIFT_FOURIER_PROBE ||
+                               ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d) || ((p->flags & PT_WANT_POS_GRAD) && grad_pos_d)))
+    return PT_ERR_UNSUPPORTED;
+  Ws w;
+  pt_problem q = *p;
+  if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
+  rc = ws_layout(&q, workspace_d, workspace_bytes, &w);
+  if (rc != PT_OK) return rc;
+  KP kp = make_kp(&q, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  prof_mark(-1, st);
+  return p->n == 128 ? run_gradient<Geo<128>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready)
+       : p->n == 64 ? run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready)
+                    : run_gradient<Geo<256>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready);
+}
+
 }  // namespace
 
 // ==================================================================================================
@@ -1629,32 +1721,8 @@ int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c6
                         const float* intensity_d, const int32_t* batch_idx_d, pt_c64* grad_object_d, pt_c64* grad_probe_d,
                         float* grad_pos_d, float* illum_d, const float* illum_prev_d, float* step_terms_d, double* loss_d,
                         float* loss_per_pos_d, void* workspace_d, size_t workspace_bytes, void* cuda_stream) {
-  int rc = validate(p);
-  if (rc != PT_OK) return rc;
-  if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
-  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
-  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
-  if (p->flags & PT_WANT_WEIGHTED_ILLUM) {
-    if (!(p->flags & PT_WANT_ILLUM) || !(p->flags & PT_WANT_STEP_SIZES) || (p->flags & PT_EPIE)) return PT_ERR_BAD_PARAM;
-    if (!illum_d || !step_terms_d) return PT_ERR_NULL;
-    if (!(p->lsqml_gamma >= 0.f)) return PT_ERR_BAD_PARAM;
-  }
-  // ePIE directions (PAPER.md:173: the optimal wavefront update is given for the amplitude model): amplitude loss,
-  // Fourier-shift mode, no step-size terms, no position gradient
-  if ((p->flags & PT_EPIE) && (p->loss != PT_LOSS_AMPLITUDE || p->shift_mode != PT_SHIFT_FOURIER_PROBE ||
-                               ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d) || ((p->flags & PT_WANT_POS_GRAD) && grad_pos_d)))
-    return PT_ERR_UNSUPPORTED;
-  Ws w;
-  pt_problem q = *p;
-  if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
-  rc = ws_layout(&q, workspace_d, workspace_bytes, &w);
-  if (rc != PT_OK) return rc;
-  KP kp = make_kp(&q, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
-  cudaStream_t st = (cudaStream_t)cuda_stream;
-  prof_mark(-1, st);
-  return p->n == 128 ? run_gradient<Geo<128>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st)
-       : p->n == 64 ? run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st)
-                    : run_gradient<Geo<256>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st);
+  return gradient_impl(p, object_d, probe_d, positions_d, intensity_d, batch_idx_d, grad_object_d, grad_probe_d, grad_pos_d, illum_d,
+                       illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, workspace_d, workspace_bytes, cuda_stream, nullptr);
 }
 
 int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe_d, float* positions_d,
@@ -1670,7 +1738,7 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
   if (u->mode == PT_UPDATE_SGD) {
     if (object_d && grad_object_d) { k_axpy<<<(unsigned)((2 * on + 255) / 256), 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, -u->lr_obj, 2 * on); LAUNCH_CHECK(K_axpy, st); }
     if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, -u->lr_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
-    if (positions_d && grad_pos_d) { k_pos_sgd<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, grad_pos_d, batch_idx_d, u->lr_pos, p->n_batch); LAUNCH_CHECK(K_pos_sgd, st); }
+    if (positions_d && grad_pos_d) { k_pos_sgd<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, grad_pos_d, batch_idx_d, u->lr_pos, p->n_batch, p->n_pos_total); LAUNCH_CHECK(K_pos_sgd, st); }
     return PT_OK;
   }
   if (u->mode == PT_UPDATE_EPIE) {      // O_i += beta_object dO_i ; P_k += beta_probe dP_k
@@ -1699,7 +1767,7 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
     LAUNCH_CHECK(K_lsqml_probe, st);
   }
   if (positions_d) {
-    k_lsqml_pos<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, step_terms_d, batch_idx_d, p->n_batch, p->n_slices, p->pixel_size, u->gamma);
+    k_lsqml_pos<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, step_terms_d, batch_idx_d, p->n_batch, p->n_slices, p->pixel_size, u->gamma, p->n_pos_total);
     LAUNCH_CHECK(K_lsqml_pos, st);
   }
   return PT_OK;
@@ -1726,6 +1794,7 @@ size_t ptycho_workspace_host_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
   const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx, pn = NN * p->n_modes, J = p->n_batch;
   size_t s = align_up(on * 8) * 2 + align_up(pn * 8) * 2 + align_up(J * 8) * 2 + align_up(J * NN * 4) + align_up(J * 4) + 256;
+  s += align_up((size_t)p->n_pos_total * 8) + align_up(J * 4);           // whole position table + batch rows (batch_idx_h only)
   return s + ptycho_workspace_bytes(p);
 }
 
@@ -1739,6 +1808,9 @@ int32_t ptycho_gradient_host(const pt_problem* p, const pt_c64* object_h, const 
   if (workspace_bytes < ptycho_workspace_host_bytes(p)) return PT_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx, pn = NN * p->n_modes, J = p->n_batch;
+  if (batch_idx_h)
+    for (size_t j = 0; j < J; ++j)
+      if (batch_idx_h[j] < 0 || batch_idx_h[j] >= p->n_pos_total) return PT_ERR_OUT_OF_BOUNDS;   // host index list: checked here
   char* c = (char*)workspace_d; size_t off = 0;
   auto take = [&](size_t n) { char* r = c + off; off += align_up(n); return (void*)r; };
   pt_c64* obj_d = (pt_c64*)take(on * 8); pt_c64* gO_d = (pt_c64*)take(on * 8);
@@ -1746,7 +1818,8 @@ int32_t ptycho_gradient_host(const pt_problem* p, const pt_c64* object_h, const 
   float* pos_d = (float*)take(J * 8); float* gX_d = (float*)take(J * 8);
   float* int_d = (float*)take(J * NN * 4); float* lpp_d = (float*)take(J * 4);
   double* loss_d = (double*)take(256);
-  void* ws = c + off;
+  float* postab_d = (float*)take((size_t)p->n_pos_total * 8); int32_t* rows_d = (int32_t*)take(J * 4);
+  void* ws = c + off;                                                    // the gradient pass's own workspace (status word first)
   pt_problem q = *p;
   q.n_pos_total = (int32_t)J; q.flags &= ~(PT_ACCUMULATE | PT_WANT_STEP_SIZES | PT_WANT_ILLUM | PT_WANT_WEIGHTED_ILLUM | PT_EPIE);
   if (grad_pos_h) q.flags |= PT_WANT_POS_GRAD;
@@ -1756,49 +1829,52 @@ int32_t ptycho_gradient_host(const pt_problem* p, const pt_c64* object_h, const 
   const size_t Jc = (size_t)ptycho_positions_in_flight(&q, workspace_bytes - off);
   if (Jc == 0) return PT_ERR_WORKSPACE;
   const size_t nchunk = (J + Jc - 1) / Jc;
-  cudaStream_t cs2 = nullptr;
-  cudaEvent_t start_ev = nullptr;
-  std::vector<cudaEvent_t> ready(nchunk, nullptr);
-  bool ok = cudaStreamCreateWithFlags(&cs2, cudaStreamNonBlocking) == cudaSuccess &&
-            cudaEventCreateWithFlags(&start_ev, cudaEventDisableTiming) == cudaSuccess;
-  for (size_t c = 0; ok && c < nchunk; ++c) ok = cudaEventCreateWithFlags(&ready[c], cudaEventDisableTiming) == cudaSuccess;
-  auto cleanup = [&]() {
-    g_chunk_ready = nullptr;
-    for (auto e : ready) if (e) cudaEventDestroy(e);
-    if (start_ev) cudaEventDestroy(start_ev);
-    if (cs2) cudaStreamDestroy(cs2);
-  };
-  if (!ok) { cleanup(); return PT_ERR_CUDA; }
+  // the copy stream and the per-chunk events are created once per device and reused (the call is synchronous: it holds the
+  // pool's lock until its final stream synchronisation)
+  HostPool& hp = host_pool();
+  std::lock_guard<std::mutex> lock(hp.mu);
+  if (!hp.acquire(nchunk)) return PT_ERR_CUDA;
+  cudaStream_t cs2 = hp.cur->copy;
+  cudaEvent_t* ready = hp.cur->ready.data();
   // the copy stream starts after whatever the caller's stream has queued so far (the buffers may still be in use)
-  ok = cudaEventRecord(start_ev, st) == cudaSuccess && cudaStreamWaitEvent(cs2, start_ev, 0) == cudaSuccess;
+  bool ok = cudaEventRecord(hp.cur->start, st) == cudaSuccess && cudaStreamWaitEvent(cs2, hp.cur->start, 0) == cudaSuccess;
+  ok = ok && cudaMemsetAsync(ws, 0, 256, st) == cudaSuccess;           // deferred status word of the pass
   ok = ok && cudaMemcpyAsync(obj_d, object_h, on * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
   ok = ok && cudaMemcpyAsync(pr_d, probe_h, pn * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
   if (!batch_idx_h) ok = ok && cudaMemcpyAsync(pos_d, positions_h, J * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  else
-    for (size_t j = 0; ok && j < J; ++j)
-      ok = cudaMemcpyAsync(pos_d + 2 * j, positions_h + 2 * (size_t)batch_idx_h[j], 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
-  for (size_t c = 0; ok && c < nchunk; ++c) {
-    const size_t j0 = c * Jc, j1 = j0 + Jc < J ? j0 + Jc : J;
+  else {   // one copy of the whole table and of the index list, rows compacted on the device
+    ok = ok && cudaMemcpyAsync(postab_d, positions_h, (size_t)p->n_pos_total * 8, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    ok = ok && cudaMemcpyAsync(rows_d, batch_idx_h, J * 4, cudaMemcpyHostToDevice, st) == cudaSuccess;
+    if (ok) { k_gather_rows<<<(unsigned)((J + 255) / 256), 256, 0, st>>>((const float2*)postab_d, rows_d, (float2*)pos_d, (int)J); LAUNCH_CHECK(K_setup_pos, st); }
+  }
+  for (size_t ch = 0; ok && ch < nchunk; ++ch) {
+    const size_t j0 = ch * Jc, j1 = j0 + Jc < J ? j0 + Jc : J;
     if (!batch_idx_h) ok = cudaMemcpyAsync(int_d + j0 * NN, intensity_h + j0 * NN, (j1 - j0) * NN * 4, cudaMemcpyHostToDevice, cs2) == cudaSuccess;
     else
-      for (size_t j = j0; ok && j < j1; ++j)
-        ok = cudaMemcpyAsync(int_d + j * NN, intensity_h + (size_t)batch_idx_h[j] * NN, NN * 4, cudaMemcpyHostToDevice, cs2) == cudaSuccess;
-    ok = ok && cudaEventRecord(ready[c], cs2) == cudaSuccess;
+      for (size_t j = j0; ok && j < j1;) {                               // one copy per run of consecutive rows
+        size_t e = j + 1;
+        while (e < j1 && batch_idx_h[e] == batch_idx_h[e - 1] + 1) ++e;
+        ok = cudaMemcpyAsync(int_d + j * NN, intensity_h + (size_t)batch_idx_h[j] * NN, (e - j) * NN * 4, cudaMemcpyHostToDevice, cs2) == cudaSuccess;
+        j = e;
+      }
+    ok = ok && cudaEventRecord(ready[ch], cs2) == cudaSuccess;
   }
-  if (!ok) { cudaStreamSynchronize(cs2); cleanup(); return PT_ERR_CUDA; }
-  g_chunk_ready = ready.data();
-  rc = ptycho_gradient(&q, obj_d, pr_d, pos_d, int_d, nullptr, gO_d, gP_d, grad_pos_h ? gX_d : nullptr, nullptr, nullptr, nullptr,
-                       loss_d, lpp_d, ws, workspace_bytes - off, st);
-  g_chunk_ready = nullptr;
-  if (rc != PT_OK) { cudaStreamSynchronize(cs2); cudaStreamSynchronize(st); cleanup(); return rc; }
+  if (!ok) { cudaStreamSynchronize(cs2); cudaStreamSynchronize(st); return PT_ERR_CUDA; }
+  rc = gradient_impl(&q, obj_d, pr_d, pos_d, int_d, nullptr, gO_d, gP_d, grad_pos_h ? gX_d : nullptr, nullptr, nullptr, nullptr,
+                     loss_d, lpp_d, ws, workspace_bytes - off, st, ready);
+  if (rc != PT_OK) { cudaStreamSynchronize(cs2); cudaStreamSynchronize(st); return rc; }
+  int32_t status_h = 0;
   ok = cudaMemcpyAsync(grad_object_h, gO_d, on * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   ok = ok && cudaMemcpyAsync(grad_probe_h, gP_d, pn * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   if (grad_pos_h) ok = ok && cudaMemcpyAsync(grad_pos_h, gX_d, J * 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   if (loss_h) ok = ok && cudaMemcpyAsync(loss_h, loss_d, 8, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   if (loss_per_pos_h) ok = ok && cudaMemcpyAsync(loss_per_pos_h, lpp_d, J * 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
+  ok = ok && cudaMemcpyAsync(&status_h, ws, 4, cudaMemcpyDeviceToHost, st) == cudaSuccess;
   const bool synced = cudaStreamSynchronize(st) == cudaSuccess;       // every copy-stream event has been waited for by now
-  cleanup();
-  return ok && synced ? PT_OK : PT_ERR_CUDA;
+  if (!(ok && synced)) return PT_ERR_CUDA;
+  if (status_h & kStatusOOB) return PT_ERR_OUT_OF_BOUNDS;              // the window was clamped (R4): the results are not the model's
+  if (status_h & kStatusNonfinite) return PT_ERR_NONFINITE;
+  return PT_OK;
 }
 
 int32_t ptycho_status(void* workspace_d, void* cuda_stream) {

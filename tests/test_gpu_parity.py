@@ -1,6 +1,8 @@
-"""Parity of the CUDA path (through the C ABI, include/ptycho.h) against the CPU oracle, element by element,
-on the same seeded inputs.  Tolerances are north_star's: loss <= 1e-5 relative, gradients <= 1e-4 relative L2
-(fp32 complex on the GPU vs fp64 in the oracle).  Everything here needs a B200: marked gpu.
+"""Parity of the CUDA path (through the C ABI, include/ptycho.h) against the CPU oracle on the same seeded inputs.
+Tolerances are north_star's: loss <= 1e-5 relative, gradients <= 1e-4 relative L2 per array (fp32 complex on the GPU vs
+fp64 in the oracle); beside every norm the largest element error is bounded against the largest element (TOL_MAX) and
+every mode / slice plane against its own norm (check_array).  Tolerances that differ from north_star's are derived in
+DESIGN.md §3 ("tolerances").  Everything here needs a B200: marked gpu.
 """
 import numpy as np
 import pytest
@@ -14,6 +16,8 @@ pytestmark = pytest.mark.gpu
 TOL_LOSS = 1e-5     # relative (north_star)
 TOL_GRAD = 1e-4     # relative L2 per array (north_star)
 TOL_INT = 2e-6      # model intensity, relative L2 (fp32 FFT chain)
+TOL_STEP = 1e-4     # LSQML step-size numerators / denominators per column, and the LSQML updates: north_star's gradient bar
+TOL_POS_UPDATE = 1e-3  # updated fp32 positions minus the old ones: ulp(20 A) = 1.9e-6 A on steps of ~1e-2 A (DESIGN.md §3 "tolerances")
 
 
 def _t(a, dtype=None):
@@ -53,13 +57,42 @@ def gpu_gradient(case, pbg, batch_idx=None, flags=0, want_pos=True, want_illum=F
     return out
 
 
+TOL_MAX = 2e-4      # max |g - o| / max |o| per array (element by element; DESIGN.md §3 "tolerances")
+
+
+def margin(name, err, tol):
+    """Assert err <= tol and, when gpurun_out/ exists, append the measured margin to gpurun_out/parity_margins.txt."""
+    import os
+    d = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "gpurun_out")
+    if os.path.isdir(d):
+        test = os.environ.get("PYTEST_CURRENT_TEST", "").split("::")[-1].split(" ")[0]
+        with open(os.path.join(d, "parity_margins.txt"), "a") as f:
+            f.write(f"{test}\t{name}\t{err:.3e}\t{tol:.1e}\n")
+    assert err <= tol, (name, err, tol)
+
+
+def max_rel(a, b) -> float:
+    """max |a - b| / max |b|: the element-by-element companion of rel_l2."""
+    a = np.asarray(a).astype(np.complex128); b = np.asarray(b).astype(np.complex128)
+    return float(np.max(np.abs(a - b)) / max(np.max(np.abs(b)), 1e-300))
+
+
+def check_array(name, g, o, tol_l2=TOL_GRAD, tol_max=TOL_MAX, planes=True):
+    """Whole-array relative L2 (north_star's bar), the largest element error against the largest element, and — so that a
+    weak mode or a thin slice cannot hide inside the norm of the others — the relative L2 of every leading-index plane."""
+    margin(name + " rel_l2", rel_l2(g, o), tol_l2)
+    margin(name + " max_rel", max_rel(g, o), tol_max)
+    if planes and np.asarray(o).ndim == 3 and o.shape[0] > 1:
+        margin(name + " worst-plane rel_l2", max(rel_l2(g[i], o[i]) for i in range(o.shape[0])), 2 * tol_l2)
+
+
 def check(g, o, tol_grad=TOL_GRAD, pos=True, px=1.0):
-    assert abs(g["loss"] - o["loss"]) <= TOL_LOSS * abs(o["loss"]), (g["loss"], o["loss"])
-    assert np.max(np.abs(g["loss_per_pos"] - o["loss_per_pos"]) / np.maximum(np.abs(o["loss_per_pos"]), 1e-30)) <= 2e-5
-    assert rel_l2(g["grad_object"], o["grad_object"]) <= tol_grad
-    assert rel_l2(g["grad_probe"], o["grad_probe"]) <= tol_grad
+    margin("loss", abs(g["loss"] - o["loss"]) / abs(o["loss"]), TOL_LOSS)
+    margin("loss_per_pos", float(np.max(np.abs(g["loss_per_pos"] - o["loss_per_pos"]) / np.maximum(np.abs(o["loss_per_pos"]), 1e-30))), 2e-5)
+    check_array("grad_object", g["grad_object"], o["grad_object"], tol_grad)
+    check_array("grad_probe", g["grad_probe"], o["grad_probe"], tol_grad)
     if pos:
-        assert rel_l2(g["grad_pos"], o["grad_pos"]) <= tol_grad
+        check_array("grad_pos", g["grad_pos"], o["grad_pos"], tol_grad)
     else:
         # vacuum start: the pattern does not depend on the position (vacuum invariant), so dL/dX == 0 exactly and
         # the oracle returns ~1e-10; a relative error is undefined.  Bound the fp32 noise against the natural
@@ -93,7 +126,7 @@ def test_cfg1_forward_intensity():
                         workspace=ws, loss=loss, loss_per_pos=lpp, model_intensity=mi)
     assert ptycho.status(ws) == 0
     o = orc.forward_loss(oracle_problem(cfg), case.obj_true, case.probe, case.positions_true, case.intensity)
-    assert rel_l2(mi.cpu().numpy(), o["intensity"]) <= TOL_INT
+    margin("mi.cpu().numpy()", rel_l2(mi.cpu().numpy(), o["intensity"]), TOL_INT)
     # noiseless data at the true state: the loss is ~0 on both sides (absolute check, electrons)
     assert abs(loss.item() - o["loss"]) <= 1e-5 * cfg.dose * J * 1e-3
     # and without measured data only the model intensity is produced
@@ -130,7 +163,7 @@ def test_cfg3_reduced_chunked(start):
     cap = min_ws + (full_ws - min_ws) * 7 // 29 + 4096          # room for 8 positions per chunk: 30 = 8+8+8+6
     g = gpu_gradient(case, pbg, want_illum=True, max_ws=cap)
     check(g, o, pos=start > 0, px=cfg.pixel_size)
-    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    margin("g['illum']", rel_l2(g["illum"], o["illum"]), TOL_GRAD)
     g1 = gpu_gradient(case, pbg, want_illum=True)                # one chunk
     check(g1, o, pos=start > 0, px=cfg.pixel_size)
 
@@ -174,7 +207,7 @@ def test_cfg4_reduced_n256(start):
     pbg = gpu_problem(cfg)
     g = gpu_gradient(case, pbg, want_illum=True)
     check(g, o, pos=start > 0, px=cfg.pixel_size)
-    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    margin("g['illum']", rel_l2(g["illum"], o["illum"]), TOL_GRAD)
     min_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos, minimum=True)
     full_ws = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos)
     g2 = gpu_gradient(case, pbg, max_ws=min_ws + (full_ws - min_ws) * 4 // 11 + 4096)   # 5 + 5 + 2 positions
@@ -193,7 +226,7 @@ def test_n256_forward_intensity_bandlimit():
     ptycho.forward_loss(pbg, _t(case.obj_true), _t(case.probe), _t(case.positions_true), None, workspace=ws, model_intensity=mi)
     assert ptycho.status(ws) == 0
     o = orc.forward_loss(oracle_problem(cfg), case.obj_true, case.probe, case.positions_true, case.intensity)
-    assert rel_l2(mi.cpu().numpy(), o["intensity"]) <= TOL_INT
+    margin("mi.cpu().numpy()", rel_l2(mi.cpu().numpy(), o["intensity"]), TOL_INT)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -211,11 +244,11 @@ def test_batches_accumulate():
         ob = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, batch_idx=b)
         g = gpu_gradient(case, pbg, batch_idx=b, flags=(ptycho.ACCUMULATE if i else 0), acc_into=acc)
         acc = g["_dev"]
-        assert rel_l2(g["grad_pos"], ob["grad_pos"]) <= TOL_GRAD
+        margin("g['grad_pos']", rel_l2(g["grad_pos"], ob["grad_pos"]), TOL_GRAD)
         assert np.max(np.abs(g["loss_per_pos"] - ob["loss_per_pos"]) / np.abs(ob["loss_per_pos"])) <= 2e-5
     assert abs(g["loss"] - o_all["loss"]) <= TOL_LOSS * abs(o_all["loss"])
-    assert rel_l2(g["grad_object"], o_all["grad_object"]) <= TOL_GRAD
-    assert rel_l2(g["grad_probe"], o_all["grad_probe"]) <= TOL_GRAD
+    margin("g['grad_object']", rel_l2(g["grad_object"], o_all["grad_object"]), TOL_GRAD)
+    margin("g['grad_probe']", rel_l2(g["grad_probe"], o_all["grad_probe"]), TOL_GRAD)
 
 
 @pytest.mark.parametrize("n_modes", [3, 4])                  # one mode per CTA / two modes per CTA with the pair sum taken in TMEM
@@ -231,20 +264,20 @@ def test_deterministic_bitwise(n_modes):
         assert a["loss"] == b["loss"]
 
 
-def test_paired_and_unpaired_backward_agree(monkeypatch):
-    # even mode counts run two modes per CTA (the pair's patch gradients summed on chip in float32); PTYCHO_NO_PAIR=1 forces
+def test_paired_and_unpaired_backward_agree():
+    from paper_2505_14372_b200 import ptycho
+    # even mode counts run two modes per CTA (the pair's patch gradients summed on chip in float32); PT_NO_MODE_PAIRS forces
     # the one-mode-per-CTA kernel.  Both must match the oracle (checked above); against each other they differ only by the
     # rounding of that one float32 addition.
     cfg = synth.config(3, scan=(4, 5), n_modes=4, n_slices=5)
     case = make_case(cfg, start_scale=0.8)
     pbg = gpu_problem(cfg)
     a = gpu_gradient(case, pbg, want_illum=True)
-    monkeypatch.setenv("PTYCHO_NO_PAIR", "1")
-    b = gpu_gradient(case, pbg, want_illum=True)
-    assert rel_l2(a["grad_object"], b["grad_object"]) <= 2e-7
+    b = gpu_gradient(case, pbg, want_illum=True, flags=ptycho.NO_MODE_PAIRS)
+    margin("a['grad_object']", rel_l2(a["grad_object"], b["grad_object"]), 2e-7)
     for k in ("grad_probe", "grad_pos", "loss_per_pos"):
         assert a[k].tobytes() == b[k].tobytes(), k
-    assert rel_l2(a["illum"], b["illum"]) <= 2e-7                              # |Psi|^2 formed in float32 by the pair kernel, in fp64 by the gather
+    margin("a['illum']", rel_l2(a["illum"], b["illum"]), 2e-7)                              # |Psi|^2 formed in float32 by the pair kernel, in fp64 by the gather
     assert a["grad_object"].tobytes() != b["grad_object"].tobytes()        # the switch really selected another kernel
 
 
@@ -273,22 +306,22 @@ def test_cfg5_step_terms_and_lsqml_update():
     ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il,
                     illum_prev=ip_d, step_terms=st, loss=loss)
     assert ptycho.status(ws) == 0
-    assert rel_l2(gO.cpu().numpy(), o["grad_object"]) <= TOL_GRAD
-    assert rel_l2(gX.cpu().numpy(), o["grad_pos"]) <= TOL_GRAD
-    assert rel_l2(il.cpu().numpy(), o["illum"]) <= TOL_GRAD
+    margin("gO.cpu().numpy()", rel_l2(gO.cpu().numpy(), o["grad_object"]), TOL_GRAD)
+    margin("gX.cpu().numpy()", rel_l2(gX.cpu().numpy(), o["grad_pos"]), TOL_GRAD)
+    margin("il.cpu().numpy()", rel_l2(il.cpu().numpy(), o["illum"]), TOL_GRAD)
     stg = st.cpu().numpy().astype(np.float64)
     # numerators / denominators column by column (each an L2 over positions)
     for c in range(2 * S + 6):
-        assert rel_l2(stg[:, c], st_o[:, c]) <= 3e-4, c
+        margin("stg[:", rel_l2(stg[:, c], st_o[:, c]), TOL_STEP)
     # the update itself, from the GPU's own gradients and step terms, against the oracle's from its own
     o_new, p_new, x_new = orc.apply_update(pbo, 1, case.obj_start, case.probe, case.positions, o["grad_object"], o["grad_probe"],
                                            None, illum_prev, st_o, beta_obj=0.9, beta_probe=0.8, gamma=1e-3)
     ptycho.apply_update(pbg, obj_d, pr_d, pos_d, grad_object=gO, grad_probe=gP, illum_prev=ip_d, step_terms=st,
                         mode=ptycho.UPDATE_LSQML, beta_obj=0.9, beta_probe=0.8, gamma=1e-3, workspace=ws)
     torch.cuda.synchronize()
-    assert rel_l2(obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start) <= 5e-4
-    assert rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe) <= 5e-4
-    assert rel_l2(pos_d.cpu().numpy() - case.positions, x_new - case.positions) <= 5e-3   # fp32 positions: ulp(20 A) ~ 2e-6 on steps ~ 1e-2
+    margin("obj_d.cpu().numpy() - case.obj_start", rel_l2(obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start), TOL_STEP)
+    margin("pr_d.cpu().numpy() - case.probe", rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe), TOL_STEP)
+    margin("pos_d.cpu().numpy() - case.positions", rel_l2(pos_d.cpu().numpy() - case.positions, x_new - case.positions), TOL_POS_UPDATE)
     # chunked second sweep (the stash is recomputed per chunk) gives the same step terms
     min_ws = ptycho.workspace_bytes(pbg, J, J, fl, minimum=True)
     full_ws = ptycho.workspace_bytes(pbg, J, J, fl)
@@ -298,7 +331,7 @@ def test_cfg5_step_terms_and_lsqml_update():
                     grad_probe=gP, grad_pos=gX, illum=il, illum_prev=ip_d, step_terms=st2, loss=loss)
     assert ptycho.status(ws2) == 0
     for c in range(2 * S + 6):
-        assert rel_l2(st2.cpu().numpy()[:, c], st_o[:, c]) <= 3e-4, c
+        margin("st2.cpu().numpy()[:", rel_l2(st2.cpu().numpy()[:, c], st_o[:, c]), TOL_STEP)
 
 
 def test_sgd_update():
@@ -317,8 +350,8 @@ def test_sgd_update():
                         grad_probe=_t(o["grad_probe"].astype(np.complex64)), grad_pos=_t(gX.astype(np.float32)),
                         batch_idx=_t(b), mode=ptycho.UPDATE_SGD, lr_obj=1e-3, lr_probe=2e-3, lr_pos=1e-4)
     torch.cuda.synchronize()
-    assert rel_l2(obj_d.cpu().numpy(), o_new) <= 1e-6
-    assert rel_l2(pr_d.cpu().numpy(), p_new) <= 1e-6
+    margin("obj_d.cpu().numpy()", rel_l2(obj_d.cpu().numpy(), o_new), 1e-6)
+    margin("pr_d.cpu().numpy()", rel_l2(pr_d.cpu().numpy(), p_new), 1e-6)
     assert np.max(np.abs(pos_d.cpu().numpy() - x_new)) <= 4e-6
 
 
@@ -431,7 +464,37 @@ def test_cfg3_full_size_sampled():
     rows = np.array([j for j in range(J) if r0[j, 0] <= y0 + 5 and r0[j, 1] <= x0 + 5 and r0[j, 0] + N > y0 and r0[j, 1] + N > x0])
     assert 1 <= rows.size <= 16
     o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
-    assert rel_l2(gO_h[:, py, px_], o["grad_object"][:, py, px_]) <= TOL_GRAD
+    check_array("gO first-corner patch", gO_h[:, py, px_], o["grad_object"][:, py, px_])
+    # (2b) the LAST corner of the footprint: reached only by windows of the last chunk, found in the gather's later groups of 256
+    y1, x1 = int(r0[:, 0].max()) + N, int(r0[:, 1].max()) + N
+    py, px_ = slice(y1 - 6, y1), slice(x1 - 6, x1)
+    rows = np.array([j for j in range(J) if r0[j, 0] + N > y1 - 6 and r0[j, 1] + N > x1 - 6])
+    assert 1 <= rows.size <= 16 and rows.min() >= (J // jc) * jc + 256      # last chunk, beyond its first group of 256 windows
+    o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
+    check_array("gO last-corner patch", gO_h[:, py, px_], o["grad_object"][:, py, px_])
+    # (2c) an interior 2 x 2 patch: ~1024 windows from every chunk overlap there (the oracle needs ~2 minutes for them)
+    yc, xc = cfg.obj_n // 2 + 1, cfg.obj_n // 2 - 2
+    py, px_ = slice(yc, yc + 2), slice(xc, xc + 2)
+    rows = np.array([j for j in range(J) if r0[j, 0] <= yc + 1 and r0[j, 1] <= xc + 1 and r0[j, 0] + N > yc and r0[j, 1] + N > xc])
+    assert rows.size >= 900 and len({int(j) // jc for j in rows}) == (J + jc - 1) // jc
+    o = orc.gradient(pbo, obj, pr, pos[rows], inten[rows])
+    check_array("gO interior patch", gO_h[:, py, px_], o["grad_object"][:, py, px_])
+    # (2d) probe gradient at full size: a 64-row batch of the full tables through batch_idx, forced into several chunks, every
+    #      output array against the oracle
+    brows = np.sort(np.random.Generator(np.random.PCG64(77)).permutation(J)[:64]).astype(np.int32)
+    ob = orc.gradient(pbo, obj, pr, pos, inten, batch_idx=brows)
+    min_ws = ptycho.workspace_bytes(pbg, J, 64, minimum=True); full_ws = ptycho.workspace_bytes(pbg, J, 64)
+    wsb = ptycho.make_workspace(pbg, J, 64, max_bytes=min_ws + (full_ws - min_ws) * 24 // 63 + 4096)
+    assert ptycho.positions_in_flight(pbg, J, 64, 0, wsb.numel()) < 32
+    gOb = torch.full_like(obj_d, float("nan")); gPb = torch.full_like(pr_d, float("nan"))
+    gXb = torch.full((64, 2), float("nan"), dtype=torch.float32, device="cuda")
+    lossb = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda"); lppb = torch.full((64,), float("nan"), dtype=torch.float32, device="cuda")
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, _t(brows), workspace=wsb, grad_object=gOb, grad_probe=gPb, grad_pos=gXb, loss=lossb,
+                    loss_per_pos=lppb)
+    assert ptycho.status(wsb) == 0
+    check(dict(loss=lossb.item(), loss_per_pos=lppb.cpu().numpy(), grad_object=gOb.cpu().numpy(), grad_probe=gPb.cpu().numpy(),
+               grad_pos=gXb.cpu().numpy()), ob)
+    del wsb
     # (4) the end-to-end entry bench.py times (host buffers, patterns copied chunk by chunk on a second stream while the chain
     #     kernels run) gives bit for bit what the device-resident path gave
     pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -476,7 +539,7 @@ def test_bilinear_mode(which):
         max_ws = min_ws + (full_ws - min_ws) * 7 // 19 + 4096
     g = gpu_gradient(case, pbg, want_illum=True, max_ws=max_ws)
     check(g, o, pos=True, px=cfg.pixel_size)
-    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    margin("g['illum']", rel_l2(g["illum"], o["illum"]), TOL_GRAD)
     # step sizes are not built for this mode: the call says so instead of computing something else
     import torch
     st = torch.zeros((cfg.n_pos, 2 * cfg.n_slices + 6), dtype=torch.float32, device="cuda")
@@ -533,7 +596,7 @@ def test_edges_nonsquare_object_border_windows_single_position(mode):
 
     g = run(None)
     check(g, o, pos=True, px=px)
-    assert rel_l2(g["illum"], o["illum"]) <= TOL_GRAD
+    margin("g['illum']", rel_l2(g["illum"], o["illum"]), TOL_GRAD)
     # a batch of ONE position (the tie case), through the batch index
     o1 = orc.gradient(pbo, obj, probe, pos, inten, batch_idx=[4])
     g1 = run([4])
@@ -567,15 +630,15 @@ def test_epie_directions_and_update(which):
         max_ws = min_ws + (full_ws - min_ws) * 7 // 19 + 4096
     g = gpu_gradient(case, pbg, flags=ptycho.EPIE, want_pos=False, max_ws=max_ws)
     assert abs(g["loss"] - o["loss"]) <= TOL_LOSS * abs(o["loss"])
-    assert rel_l2(g["grad_object"], o["dir_object"]) <= TOL_GRAD
-    assert rel_l2(g["grad_probe"], o["dir_probe"]) <= TOL_GRAD
+    margin("g['grad_object']", rel_l2(g["grad_object"], o["dir_object"]), TOL_GRAD)
+    margin("g['grad_probe']", rel_l2(g["grad_probe"], o["dir_probe"]), TOL_GRAD)
     # the update: O += beta_obj dO, P += beta_probe dP
     gO, gP, _, _ = g["_dev"]
     obj_d, pr_d = _t(case.obj_start), _t(case.probe)
     ptycho.apply_update(pbg, obj_d, pr_d, None, grad_object=gO, grad_probe=gP, mode=ptycho.UPDATE_EPIE, beta_obj=0.3, beta_probe=0.2,
                         n_batch=cfg.n_pos)
-    assert rel_l2(obj_d.cpu().numpy(), case.obj_start + 0.3 * o["dir_object"]) <= 1e-5
-    assert rel_l2(pr_d.cpu().numpy(), case.probe + 0.2 * o["dir_probe"]) <= 1e-5
+    margin("obj_d.cpu().numpy()", rel_l2(obj_d.cpu().numpy(), case.obj_start + 0.3 * o["dir_object"]), 1e-5)
+    margin("pr_d.cpu().numpy()", rel_l2(pr_d.cpu().numpy(), case.probe + 0.2 * o["dir_probe"]), 1e-5)
     # the Poisson model has no ePIE wavefront update in the paper: refused, not improvised
     with pytest.raises(ptycho.PtychoError):
         gpu_gradient(case, gpu_problem(cfg, loss=synth.LOSS_POISSON, eps=0.8), flags=ptycho.EPIE, want_pos=False)
@@ -659,13 +722,13 @@ def test_lsqml_weighted_update_per_position_alpha(which):
                     step_terms=st, flags=fl)
     assert ptycho.status(ws) == 0
     ilg = il.cpu().numpy()
-    assert rel_l2(ilg[0], o["illum"]) <= TOL_GRAD
-    assert rel_l2(ilg[1], W_o) <= 3e-4          # alphas are ratios of fp32 step terms (each within 3e-4 of the oracle's)
+    margin("ilg[0]", rel_l2(ilg[0], o["illum"]), TOL_GRAD)
+    margin("ilg[1]", rel_l2(ilg[1], W_o), TOL_STEP)          # alphas are ratios of fp32 step terms
     ptycho.apply_update(pbg, obj_d, grad_object=gO, illum_prev=ip_d, step_terms=st, n_batch=J, mode=ptycho.UPDATE_LSQML_WEIGHTED,
                         beta_obj=0.9, gamma=gamma, workspace=ws, illum_batch=il)
     torch.cuda.synchronize()
     d_g, d_o = obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start
-    assert rel_l2(d_g, d_o) <= 5e-4
+    margin("d_g", rel_l2(d_g, d_o), TOL_STEP)
     cov = o["illum"] > 0
     assert np.all(d_g[~cov] == 0)               # pixels no window covers are left alone
     # flag combinations the header rules out
@@ -696,12 +759,12 @@ def test_lsqml_probe_preconditioner(which):
     ot = torch.full((n, n), float("nan"), dtype=torch.float32, device="cuda")
     ptycho.object_transparency(pbg0, obj_d, pos_d, None, out=ot, workspace=ws)
     assert ptycho.status(ws) == 0
-    assert rel_l2(ot.cpu().numpy(), ot_o) <= 1e-6
+    margin("ot.cpu().numpy()", rel_l2(ot.cpu().numpy(), ot_o), 1e-6)
     ot2 = torch.full((n, n), float("nan"), dtype=torch.float32, device="cuda")
     half = J // 2
     ptycho.object_transparency(pbg0, obj_d, pos_d, _t(np.arange(half, dtype=np.int32)), out=ot2, workspace=ws)
     ptycho.object_transparency(pbg0, obj_d, pos_d, _t(np.arange(half, J, dtype=np.int32)), out=ot2, workspace=ws, flags=ptycho.ACCUMULATE)
-    assert rel_l2(ot2.cpu().numpy(), ot_o) <= 1e-6
+    margin("ot2.cpu().numpy()", rel_l2(ot2.cpu().numpy(), ot_o), 1e-6)
     ot3 = torch.empty_like(ot)
     ptycho.object_transparency(pbg0, obj_d, pos_d, None, out=ot3, workspace=ws)
     assert torch.equal(ot, ot3)
@@ -721,13 +784,13 @@ def test_lsqml_probe_preconditioner(which):
     assert ptycho.status(ws) == 0
     stg = st.cpu().numpy().astype(np.float64)
     for c in range(2 * S + 6):
-        assert rel_l2(stg[:, c], st_o[:, c]) <= 3e-4, c
+        margin("stg[:", rel_l2(stg[:, c], st_o[:, c]), TOL_STEP)
     _, p_new, _ = orc.apply_update(pbo, 1, case.obj_start, case.probe, case.positions, None, o["grad_probe"], None, illum_prev, st_o,
                                    beta_probe=0.8, gamma=1e-3, probe_precond=pc)
     ptycho.apply_update(pbg, None, pr_d, None, grad_probe=gP, step_terms=st, n_batch=J, mode=ptycho.UPDATE_LSQML, beta_probe=0.8,
                         gamma=1e-3, workspace=ws)
     torch.cuda.synchronize()
-    assert rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe) <= 5e-4
+    margin("pr_d.cpu().numpy() - case.probe", rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe), TOL_STEP)
     # a window off the object raises the deferred flag
     bad = case.positions.copy(); bad[0, 0] = -5.0
     ptycho.object_transparency(pbg0, obj_d, _t(bad), None, out=ot3, workspace=ws)
@@ -759,7 +822,7 @@ def test_cost_regularizers(kind):
     ptycho.cost_regularizer(kind, 0.37, z_d, grad=g_d, cost=cost, ref=1.0, eps=0.02, workspace=ws)
     torch.cuda.synchronize()
     assert abs((cost.item() - 5.0) - R_o) <= 1e-5 * abs(R_o)                       # cost is ADDED
-    assert rel_l2(g_d.cpu().numpy() - g0, g_o - g0) <= 1e-5                         # gradient is ADDED into grad
+    margin("g_d.cpu().numpy() - g0", rel_l2(g_d.cpu().numpy() - g0, g_o - g0), 1e-5)                         # gradient is ADDED into grad
     # cost only / gradient only; bitwise reproducible
     g2 = _t(g0); c2 = torch.full((1,), 5.0, dtype=torch.float64, device="cuda")
     ptycho.cost_regularizer(kind, 0.37, z_d, grad=g2, ref=1.0, eps=0.02, workspace=ws)
@@ -789,7 +852,7 @@ def test_constraints():
     for kind, okind, sig in ((ptycho.CON_LAYER_BLUR, orc.CON_LAYER_BLUR, 0.9), (ptycho.CON_LOWPASS, orc.CON_LOWPASS, 1.3)):
         d = _t(z)
         ptycho.apply_constraint(kind, d, a=sig, workspace=ws)
-        assert rel_l2(d.cpu().numpy(), orc.apply_constraint(okind, z, sig)) <= 1e-6
+        margin("d.cpu().numpy()", rel_l2(d.cpu().numpy(), orc.apply_constraint(okind, z, sig)), 1e-6)
     with pytest.raises(ptycho.PtychoError):
         ptycho.apply_constraint(ptycho.CON_LAYER_BLUR, d, a=0.9, workspace=ws[:100])
     with pytest.raises(ptycho.PtychoError):
@@ -814,9 +877,9 @@ def test_adam_updates():
         x_o, mx_o, vx_o = orc.adam_update(x_o, gx, mx_o, vx_o, lr=f32(1e-2), b1=f32(0.8), b2=f32(0.99), eps=f32(1e-3), t=t)
         ptycho.adam_update(z_d, _t(g.astype(np.complex64)), m_d, v_d, lr=1e-2, beta1=0.9, beta2=0.999, eps=1e-8, step=t)
         ptycho.adam_update(x_d, _t(gx), mx_d, vx_d, lr=1e-2, beta1=0.8, beta2=0.99, eps=1e-3, step=t)
-    assert rel_l2(z_d.cpu().numpy() - obj, z_o - obj) <= 1e-5
+    margin("z_d.cpu().numpy() - obj", rel_l2(z_d.cpu().numpy() - obj, z_o - obj), 1e-5)
     assert rel_l2(m_d.cpu().numpy(), m_o) <= 1e-6 and rel_l2(v_d.cpu().numpy(), v_o) <= 1e-6
-    assert rel_l2(x_d.cpu().numpy() - x, x_o - x) <= 1e-5
+    margin("x_d.cpu().numpy() - x", rel_l2(x_d.cpu().numpy() - x, x_o - x), 1e-5)
     with pytest.raises(ptycho.PtychoError):
         ptycho.adam_update(z_d, z_d, m_d, v_d, lr=1e-2, step=0)
 
@@ -876,7 +939,14 @@ def test_cfg4_full_size_minibatches_sampled():
         assert rel_l2(gX_h[j], o["grad_pos"][n]) <= TOL_GRAD, (j, gX_h[j], o["grad_pos"][n])
     o = orc.gradient(pbo, obj, pr, pos[corner], inten[corner]) if extra else o
     py, px_ = slice(y0, y0 + 4), slice(x0, x0 + 4)
-    assert rel_l2(gO_h[:, py, px_], o["grad_object"][:, py, px_]) <= TOL_GRAD
+    check_array("gO first-corner patch", gO_h[:, py, px_], o["grad_object"][:, py, px_])
+    # the opposite corner of the footprint of these two mini-batches
+    jl = int(np.argmax(r0[:, 0] + r0[:, 1]))                                # (a random subset has no window at the box corner)
+    y1, x1 = int(r0[jl, 0]) + N, int(r0[jl, 1]) + N
+    last = np.array([j for j in range(2 * mb) if r0[j, 0] <= y1 - 1 and r0[j, 1] <= x1 - 1 and r0[j, 0] + N > y1 - 4 and r0[j, 1] + N > x1 - 4])
+    assert 1 <= last.size <= 12
+    o = orc.gradient(pbo, obj, pr, pos[last], inten[last])
+    check_array("gO last-corner patch", gO_h[:, y1 - 4:y1, x1 - 4:x1], o["grad_object"][:, y1 - 4:y1, x1 - 4:x1])
 
 
 # ------------------------------------------------------------------------------------------------
@@ -932,7 +1002,7 @@ def test_constraint_probe_support_fourier(n):
     d = _t(pr)
     ptycho.apply_constraint(ptycho.CON_SUPPORT_MASK_FOURIER, d, mask=_t(mask))
     torch.cuda.synchronize()
-    assert rel_l2(d.cpu().numpy(), orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, pr, mask=mask)) <= 2e-6
+    margin("d.cpu().numpy()", rel_l2(d.cpu().numpy(), orc.apply_constraint(orc.CON_SUPPORT_MASK_FOURIER, pr, mask=mask)), 2e-6)
     with pytest.raises(ptycho.PtychoError):
         ptycho.apply_constraint(ptycho.CON_SUPPORT_MASK_FOURIER, _t(pr[:, :, : n // 2].copy()), mask=_t(mask))
 
@@ -950,8 +1020,8 @@ def test_constraint_phase_deramp():
     ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d, workspace=ws)
     torch.cuda.synchronize()
     ref = orc.apply_constraint(orc.CON_PHASE_DERAMP, z)
-    assert rel_l2(d.cpu().numpy(), ref) <= 2e-6
-    assert rel_l2(ref, orc.apply_constraint(orc.CON_PHASE_DERAMP, obj)) <= 1e-5      # the ramp is what was removed (float32 input rounding)
+    margin("d.cpu().numpy()", rel_l2(d.cpu().numpy(), ref), 2e-6)
+    margin("ref", rel_l2(ref, orc.apply_constraint(orc.CON_PHASE_DERAMP, obj)), 1e-5)      # the ramp is what was removed (float32 input rounding)
     d2 = _t(z)
     ptycho.apply_constraint(ptycho.CON_PHASE_DERAMP, d2, workspace=ws)
     assert torch.equal(d, d2)                                                         # bitwise reproducible
@@ -996,7 +1066,7 @@ def test_cfg5_full_size_minibatch_properties():
     st_h, gX_h, il_h, lpp_h = st.cpu().numpy().astype(np.float64), gX.cpu().numpy().astype(np.float64), il.cpu().numpy(), lpp.cpu().numpy()
     assert np.isfinite(st_h).all() and np.isfinite(il_h).all() and np.isfinite(gO.cpu().numpy().view(np.float32)).all()
     px = float(np.float32(cfg.pixel_size))
-    assert rel_l2(st_h[:, 2 * S + 2], -0.5 * px * gX_h[:, 0]) <= 3e-4 and rel_l2(st_h[:, 2 * S + 4], -0.5 * px * gX_h[:, 1]) <= 3e-4
+    assert rel_l2(st_h[:, 2 * S + 2], -0.5 * px * gX_h[:, 0]) <= TOL_STEP and rel_l2(st_h[:, 2 * S + 4], -0.5 * px * gX_h[:, 1]) <= TOL_STEP
     assert (st_h[:, 1::2] >= 0).all()
     pn = float(np.sum(np.abs(pr.astype(np.complex128)) ** 2))
     assert abs(il_h[0].astype(np.float64).sum() - mb * pn) <= 1e-5 * mb * pn
@@ -1010,4 +1080,160 @@ def test_cfg5_full_size_minibatch_properties():
     o = orc.gradient(pbo, obj, pr, pos[b[rows]], inten[b[rows]])
     for n, j in enumerate(rows):
         assert abs(lpp_h[j] - o["loss_per_pos"][n]) <= 2e-5 * abs(o["loss_per_pos"][n])
-        assert rel_l2(gX_h[j], o["grad_pos"][n]) <= TOL_GRAD
+        margin("gX_h[j]", rel_l2(gX_h[j], o["grad_pos"][n]), TOL_GRAD)
+
+
+
+# ------------------------------------------------------------------------------------------------
+# More than 256 windows in one chunk: the gather kernels (k_gather_object, its illumination branch, k_gather_willum) walk
+# a chunk's windows in groups of 256; every array against the oracle (N = 64, 2 modes, 2 slices, 20 x 20 scan, one chunk).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("mode", ["fourier", "bilinear"])
+def test_gather_window_groups_beyond_256(mode):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(5, n=64, scan=(20, 20), n_modes=2, n_slices=2, obj_n=200, pixel_size=0.2, step_px=3.0)
+    J, S = cfg.n_pos, cfg.n_slices
+    if mode == "bilinear":
+        case = _bilinear_case(cfg, 0.8)
+        pbo = oracle_problem(cfg, shift_mode=orc.SHIFT_BILINEAR_OBJECT)
+        pbg = gpu_problem(cfg, shift_mode=ptycho.SHIFT_BILINEAR_OBJECT)
+        o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+        g = gpu_gradient(case, pbg, want_illum=True)
+        assert ptycho.positions_in_flight(pbg, J, J, ptycho.WANT_ILLUM) == J
+        check(g, o)
+        check_array("illum", g["illum"], o["illum"])
+        return
+    gamma = 1e-3
+    case = make_case(cfg, start_scale=0.8)
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbo, pbg = oracle_problem(cfg, **kw), gpu_problem(cfg, lsqml_gamma=gamma, **kw)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    illum_prev = (o["illum"] * 0.9).astype(np.float32)
+    st_o = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev)
+    W_o = orc.weighted_illum(pbo, case.obj_start, case.probe, case.positions, st_o, gamma)
+    obj_d, pr_d, pos_d, I_d, ip_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity), _t(illum_prev)
+    gO = torch.full_like(obj_d, float("nan")); gP = torch.full_like(pr_d, float("nan"))
+    gX = torch.full((J, 2), float("nan"), dtype=torch.float32, device="cuda")
+    il = torch.full((2,) + tuple(obj_d.shape), float("nan"), dtype=torch.float32, device="cuda")
+    st = torch.full((J, 2 * S + 6), float("nan"), dtype=torch.float32, device="cuda")
+    loss = torch.full((1,), float("nan"), dtype=torch.float64, device="cuda"); lpp = torch.full((J,), float("nan"), dtype=torch.float32, device="cuda")
+    fl = ptycho.WANT_POS_GRAD | ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES | ptycho.WANT_WEIGHTED_ILLUM
+    ws = ptycho.make_workspace(pbg, J, J, fl)
+    assert ptycho.positions_in_flight(pbg, J, J, fl) == J > 256                 # one chunk, two groups of windows
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il,
+                    illum_prev=ip_d, step_terms=st, loss=loss, loss_per_pos=lpp, flags=fl)
+    assert ptycho.status(ws) == 0
+    check(dict(loss=loss.item(), loss_per_pos=lpp.cpu().numpy(), grad_object=gO.cpu().numpy(), grad_probe=gP.cpu().numpy(),
+               grad_pos=gX.cpu().numpy()), o)
+    ilg = il.cpu().numpy()
+    check_array("illum", ilg[0], o["illum"])
+    check_array("weighted illum", ilg[1], W_o, TOL_STEP, 2 * TOL_STEP)
+    stg = st.cpu().numpy().astype(np.float64)
+    for c in range(2 * S + 6):
+        margin(f"step term column {c}", rel_l2(stg[:, c], st_o[:, c]), TOL_STEP)
+
+
+# ------------------------------------------------------------------------------------------------
+# config 2 at its FULL size (1024 positions, N = 128, 4 modes): every array against the oracle
+# ------------------------------------------------------------------------------------------------
+def test_cfg2_full():
+    cfg = synth.config(2)
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    g = gpu_gradient(case, gpu_problem(cfg), want_illum=True)
+    check(g, o)
+    check_array("illum", g["illum"], o["illum"])
+
+
+# ------------------------------------------------------------------------------------------------
+# more boundary behaviour: index lists that leave the tables, the host path's own status, non-finite losses, and more than
+# 64 propagators (the table kernel is then launched twice)
+# ------------------------------------------------------------------------------------------------
+def test_batch_index_out_of_range_and_host_path_status():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(1, scan=(3, 3))
+    case = make_case(cfg, noise=False)
+    pbg = gpu_problem(cfg)
+    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d)
+    ws = ptycho.make_workspace(pbg, 9, 3)
+    for bad in ([1, 9, 2], [1, -1, 2]):                                    # a row beyond the tables / a negative row
+        ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, _t(np.array(bad, np.int32)), workspace=ws, grad_object=gO, grad_probe=gP)
+        assert ptycho.status(ws) == -6 and ptycho.status(ws) == 0
+        assert torch.isfinite(torch.view_as_real(gO)).all()
+        pos2 = pos_d.clone()
+        ptycho.apply_update(pbg, None, None, pos2, grad_pos=torch.ones((3, 2), device="cuda"), batch_idx=_t(np.array(bad, np.int32)),
+                            mode=ptycho.UPDATE_SGD, lr_pos=1.0)
+        torch.cuda.synchronize()
+        changed = (pos2 != pos_d).any(dim=1).cpu().numpy()
+        assert changed.tolist() == [False, True, True] + [False] * 6        # rows 1 and 2 moved, the bad entry touched nothing
+    # host path: a window that leaves the object comes back as the call's own return value, and the same
+    # workspace then serves a good call
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    badpos = case.positions.copy(); badpos[4, 0] = 5.0
+    gO_h = torch.empty(case.obj_start.shape, dtype=torch.complex64).pin_memory(); gP_h = torch.empty(case.probe.shape, dtype=torch.complex64).pin_memory()
+    wsh = ptycho.make_workspace(pbg, 9, 9, host=True)
+    with pytest.raises(ptycho.PtychoError) as e:
+        ptycho.gradient_host(pbg, pin(case.obj_start), pin(case.probe), pin(badpos), pin(case.intensity), workspace=wsh, grad_object_h=gO_h, grad_probe_h=gP_h)
+    assert e.value.code == -6
+    with pytest.raises(ptycho.PtychoError) as e:                           # index list checked on the host
+        ptycho.gradient_host(pbg, pin(case.obj_start), pin(case.probe), pin(case.positions), pin(case.intensity), torch.tensor([0, 9], dtype=torch.int32),
+                             workspace=wsh, grad_object_h=gO_h, grad_probe_h=gP_h)
+    assert e.value.code == -6
+    g = gpu_gradient(case, pbg)
+    ptycho.gradient_host(pbg, pin(case.obj_start), pin(case.probe), pin(case.positions), pin(case.intensity), workspace=wsh, grad_object_h=gO_h, grad_probe_h=gP_h)
+    assert gO_h.numpy().tobytes() == g["grad_object"].tobytes() and gP_h.numpy().tobytes() == g["grad_probe"].tobytes()
+    # runs of consecutive rows and single rows mixed in one index list
+    rows = np.array([3, 4, 5, 1, 7, 8], np.int32)
+    gb = gpu_gradient(case, pbg, batch_idx=rows)
+    gX_h = torch.empty((rows.size, 2), dtype=torch.float32).pin_memory()
+    ptycho.gradient_host(pbg, pin(case.obj_start), pin(case.probe), pin(case.positions), pin(case.intensity), torch.from_numpy(rows), workspace=wsh,
+                         grad_object_h=gO_h, grad_probe_h=gP_h, grad_pos_h=gX_h)
+    assert gO_h.numpy().tobytes() == gb["grad_object"].tobytes() and gX_h.numpy().tobytes() == gb["grad_pos"].tobytes()
+
+
+def test_nonfinite_loss_flag():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(1, scan=(2, 2))
+    case = make_case(cfg, noise=False)
+    pbg = gpu_problem(cfg)
+    obj = case.obj_start.copy(); obj[0, 64, 64] = np.inf                   # inside every window
+    obj_d, pr_d, pos_d, I_d = _t(obj), _t(case.probe), _t(case.positions), _t(case.intensity)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d)
+    ws = ptycho.make_workspace(pbg, 4, 4)
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP)
+    assert ptycho.status(ws) == -7 and ptycho.status(ws) == 0              # PT_ERR_NONFINITE, deferred, then cleared
+    pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
+    wsh = ptycho.make_workspace(pbg, 4, 4, host=True)
+    with pytest.raises(ptycho.PtychoError) as e:
+        ptycho.gradient_host(pbg, pin(obj), pin(case.probe), pin(case.positions), pin(case.intensity), workspace=wsh,
+                             grad_object_h=torch.empty(obj.shape, dtype=torch.complex64).pin_memory(),
+                             grad_probe_h=torch.empty(case.probe.shape, dtype=torch.complex64).pin_memory())
+    assert e.value.code == -7
+
+
+def test_more_than_64_propagators():
+    cfg = synth.config(3, n=64, scan=(2, 2), n_modes=1, n_slices=67, obj_n=100, pixel_size=0.2, step_px=3.0, dz=2.0)
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, gpu_problem(cfg))
+    check(g, o)
+
+
+def test_epie_dead_mode_contributes_nothing():
+    # an identically zero probe mode: 1 / max|Psi|^2 is guarded, so the directions stay finite and equal the oracle's
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(2, scan=(3, 3), n_modes=2)
+    case = make_case(cfg, start_scale=0.8)
+    case.probe[1] = 0
+    pbo, pbg = oracle_problem(cfg), gpu_problem(cfg)
+    o = orc.epie(pbo, case.obj_start, case.probe, case.positions, case.intensity)
+    g = gpu_gradient(case, pbg, want_pos=False, flags=ptycho.EPIE)
+    assert np.isfinite(g["grad_object"].view(np.float32)).all() and np.isfinite(g["grad_probe"].view(np.float32)).all()
+    check_array("epie object direction", g["grad_object"], o["dir_object"])
+    check_array("epie probe direction", g["grad_probe"][:1], o["dir_probe"][:1])
+    assert not g["grad_probe"][1].any() and not o["dir_probe"][1].any()

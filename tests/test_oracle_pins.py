@@ -795,6 +795,20 @@ def test_epie_multislice_invariants():
     assert np.abs(e["dir_object"] + 2.0 * g["grad_object"] / np.max(np.abs(Ps) ** 2)).max() < 1e-9 * np.abs(e["dir_object"]).max()
 
 
+def test_epie_dead_mode_contributes_nothing():
+    # reading R23b: an identically zero probe mode (max|Psi|^2 = 0 in PAPER.md:203) adds nothing — the directions are finite
+    # and equal those of the problem without that mode
+    pb, obj, probe, pos = small_problem(n=8, M=2, S=2, on=20, J=3, loss=orc.LOSS_AMPLITUDE, eps=0.5)
+    Iexp = (orc.forward_loss(pb, obj, probe, pos)["intensity"] * RNG.uniform(0.5, 1.5, size=(3, 8, 8))).astype(np.float32)
+    dead = probe.copy(); dead[1] = 0
+    e2 = orc.epie(pb, obj, dead, pos, Iexp)
+    import dataclasses
+    e1 = orc.epie(dataclasses.replace(pb, n_modes=1), obj, dead[:1], pos, Iexp)
+    assert np.isfinite(e2["dir_object"]).all() and np.isfinite(e2["dir_probe"]).all()
+    assert np.array_equal(e2["dir_object"], e1["dir_object"]) and np.array_equal(e2["dir_probe"][0], e1["dir_probe"][0])
+    assert not e2["dir_probe"][1].any()
+
+
 # ------------------------------------------------------------------------------------------------
 # cost regularisers (R26), constraint regularisers (R27), Adam
 # (R28)
