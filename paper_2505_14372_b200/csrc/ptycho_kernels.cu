@@ -31,7 +31,42 @@
 #include "../../include/ptycho.h"
 #include "fft_core.cuh"
 
+// Build units.  The file compiles either as one translation unit (PTK_ONLY_GEO undefined) or as four that the build compiles in
+// parallel (ptycho.build): PTK_ONLY_GEO = 64 / 128 / 256 holds the chain kernels of that geometry and their launch sequences
+// (run_forward / run_gradient), PTK_ONLY_GEO = 0 the C ABI, the geometry-independent kernels and regularizers.cuh.
+#ifndef PTK_ONLY_GEO
+#define PTK_ONLY_GEO -1
+#endif
+#define PTK_HAS_GEO(n) (PTK_ONLY_GEO == -1 || PTK_ONLY_GEO == (n))
+#define PTK_HAS_ABI (PTK_ONLY_GEO <= 0)
+
 using namespace ptk;
+
+// per-thread launch counter and optional profiling record (ptycho_launch_count, ptycho_profile_*): shared by all build units
+struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
+namespace ptk_state {
+extern thread_local int64_t g_launches;
+extern thread_local bool g_prof_on;
+extern thread_local std::vector<ProfMark> g_prof;
+#if PTK_HAS_ABI
+thread_local int64_t g_launches = 0;
+thread_local bool g_prof_on = false;
+thread_local std::vector<ProfMark> g_prof;
+#endif
+}  // namespace ptk_state
+using namespace ptk_state;
+
+// launch sequences of one geometry (defined in that geometry's build unit); kp points at the caller's KP
+struct GradArgs { pt_c64* gO; pt_c64* gP; float* gX; float* illum; const float* illum_prev; float* step_terms; double* loss; float* loss_per_pos;
+                  const cudaEvent_t* chunk_ready; };
+namespace ptk_geo {
+int run_forward_64(const pt_problem* p, const void* kp, double* loss_d, float* loss_per_pos_d, float* model_intensity_d, cudaStream_t st);
+int run_forward_128(const pt_problem* p, const void* kp, double* loss_d, float* loss_per_pos_d, float* model_intensity_d, cudaStream_t st);
+int run_forward_256(const pt_problem* p, const void* kp, double* loss_d, float* loss_per_pos_d, float* model_intensity_d, cudaStream_t st);
+int run_gradient_64(const pt_problem* p, const void* kp, const GradArgs* a, cudaStream_t st);
+int run_gradient_128(const pt_problem* p, const void* kp, const GradArgs* a, cudaStream_t st);
+int run_gradient_256(const pt_problem* p, const void* kp, const GradArgs* a, cudaStream_t st);
+}  // namespace ptk_geo
 
 namespace {
 
@@ -1371,10 +1406,6 @@ const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
                                          "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam"};
-thread_local int64_t g_launches = 0;
-thread_local bool g_prof_on = false;
-struct ProfMark { cudaEvent_t ev; int kind; };          // kind < 0: start-of-call marker
-thread_local std::vector<ProfMark> g_prof;
 
 inline void prof_mark(int kind, cudaStream_t st) {
   if (!g_prof_on) return;
@@ -1657,13 +1688,33 @@ int32_t gradient_impl(const pt_problem* p, const pt_c64* object_d, const pt_c64*
   KP kp = make_kp(&q, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
-  return p->n == 128 ? run_gradient<Geo<128>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready)
-       : p->n == 64 ? run_gradient<Geo<64>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready)
-                    : run_gradient<Geo<256>>(&q, kp, grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, st, chunk_ready);
+  const GradArgs ga = {grad_object_d, grad_probe_d, grad_pos_d, illum_d, illum_prev_d, step_terms_d, loss_d, loss_per_pos_d, chunk_ready};
+  return p->n == 128 ? ptk_geo::run_gradient_128(&q, &kp, &ga, st) : p->n == 64 ? ptk_geo::run_gradient_64(&q, &kp, &ga, st)
+                                                                                 : ptk_geo::run_gradient_256(&q, &kp, &ga, st);
 }
 
 }  // namespace
 
+#define PTK_DEFINE_GEO(n)                                                                                                          \
+  int ptk_geo::run_forward_##n(const pt_problem* p, const void* kp, double* loss_d, float* loss_per_pos_d, float* model_intensity_d, \
+                               cudaStream_t st) {                                                                                  \
+    return run_forward<Geo<n>>(p, *(const KP*)kp, loss_d, loss_per_pos_d, model_intensity_d, st);                                   \
+  }                                                                                                                                \
+  int ptk_geo::run_gradient_##n(const pt_problem* p, const void* kp, const GradArgs* a, cudaStream_t st) {                          \
+    return run_gradient<Geo<n>>(p, *(const KP*)kp, a->gO, a->gP, a->gX, a->illum, a->illum_prev, a->step_terms, a->loss,            \
+                                a->loss_per_pos, st, a->chunk_ready);                                                               \
+  }
+#if PTK_HAS_GEO(64)
+PTK_DEFINE_GEO(64)
+#endif
+#if PTK_HAS_GEO(128)
+PTK_DEFINE_GEO(128)
+#endif
+#if PTK_HAS_GEO(256)
+PTK_DEFINE_GEO(256)
+#endif
+
+#if PTK_HAS_ABI
 // ==================================================================================================
 // C ABI
 // ==================================================================================================
@@ -1712,9 +1763,9 @@ int32_t ptycho_forward_loss(const pt_problem* p, const pt_c64* object_d, const p
   KP kp = make_kp(p, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
-  return p->n == 128 ? run_forward<Geo<128>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st)
-       : p->n == 64 ? run_forward<Geo<64>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st)
-                    : run_forward<Geo<256>>(p, kp, loss_d, loss_per_pos_d, model_intensity_d, st);
+  return p->n == 128 ? ptk_geo::run_forward_128(p, &kp, loss_d, loss_per_pos_d, model_intensity_d, st)
+       : p->n == 64 ? ptk_geo::run_forward_64(p, &kp, loss_d, loss_per_pos_d, model_intensity_d, st)
+                    : ptk_geo::run_forward_256(p, &kp, loss_d, loss_per_pos_d, model_intensity_d, st);
 }
 
 int32_t ptycho_gradient(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
@@ -1937,3 +1988,4 @@ const char* ptycho_strerror(int32_t code) {
 }  // extern "C"
 
 #include "regularizers.cuh"
+#endif  // PTK_HAS_ABI

@@ -33,11 +33,17 @@ def build(force: bool = False, verbose: bool = False) -> str:
     srcs = [os.path.join(_CSRC, f) for f in ("ptycho_kernels.cu", "fft_core.cuh", "regularizers.cuh")] + [os.path.join(_HERE, "..", "include", "ptycho.h")]
     if not force and os.path.exists(LIB_PATH) and all(os.path.getmtime(LIB_PATH) >= os.path.getmtime(s) for s in srcs):
         return LIB_PATH
-    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-shared",
-           "-Xcompiler", "-fPIC", "-o", LIB_PATH, os.path.join(_CSRC, "ptycho_kernels.cu")]
+    # four build units compiled side by side (csrc/ptycho_kernels.cu, PTK_ONLY_GEO): the C ABI and one per FFT geometry
+    base = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-std=c++17", "-lineinfo", "-Xcompiler", "-fPIC"]
     if verbose:
-        cmd.insert(1, "-Xptxas=-v")
-    subprocess.run(cmd, check=True)
+        base.append("-Xptxas=-v")
+    bdir = os.path.join(_HERE, "build")
+    os.makedirs(bdir, exist_ok=True)
+    units = [(g, os.path.join(bdir, f"ptycho_geo{g}.o")) for g in (0, 64, 128, 256)]
+    procs = [subprocess.Popen(base + [f"-DPTK_ONLY_GEO={g}", "-c", "-o", o, os.path.join(_CSRC, "ptycho_kernels.cu")]) for g, o in units]
+    if any(pr.wait() != 0 for pr in procs):
+        raise RuntimeError("nvcc failed")
+    subprocess.run(["nvcc", "-shared", "-o", LIB_PATH] + [o for _, o in units], check=True)
     return LIB_PATH
 
 

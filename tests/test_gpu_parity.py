@@ -1095,8 +1095,7 @@ def test_gather_window_groups_beyond_256(mode):
     cfg = synth.config(5, n=64, scan=(20, 20), n_modes=2, n_slices=2, obj_n=200, pixel_size=0.2, step_px=3.0)
     J, S = cfg.n_pos, cfg.n_slices
     if mode == "bilinear":
-        case = _bilinear_case(cfg, 0.8)
-        pbo = oracle_problem(cfg, shift_mode=orc.SHIFT_BILINEAR_OBJECT)
+        case, pbo = _bilinear_case(cfg, 0.8)
         pbg = gpu_problem(cfg, shift_mode=ptycho.SHIFT_BILINEAR_OBJECT)
         o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
         g = gpu_gradient(case, pbg, want_illum=True)
