@@ -8,7 +8,8 @@ A step = one pass of the whole hot path over ALL posi
 ptycho_gradient (loss + object / probe / position gradients) then ptycho_apply_update (SGD), through the C ABI.
 Workload at N=1: BASELINE.json config 3 (128x128 patterns, 64x64 scan = 4096 positions, 8 modes, 20 slices, tilt,
 Poisson loss), the configuration north_star's target is quoted on.  Inputs are seeded and synthetic.
-Rank 0 prints ONE JSON line.
+After the headline workload the default invocation also times, briefly, configs 1, 2, 4, 5 (batch 1024) and the band-limited
+variant of config 3 and attaches them as "secondary" (--no-secondary skips them).  Rank 0 prints ONE JSON line.
 """
 import argparse
 import json
@@ -43,6 +44,7 @@ def parse():
     ap.add_argument("--bandlimit", type=float, default=0.0, help="timed variant: sharp band-limit mask at this fraction of Nyquist "
                     "inside the propagator (PAPER.md:117, reading R9); 0 = off, as in BASELINE.json's configs")
     ap.add_argument("--ws-gib", type=float, default=0.0, help="cap of the device workspace in GiB (0: library default)")
+    ap.add_argument("--no-secondary", action="store_true", help="config 3 only: skip the short runs of the other configurations")
     return ap.parse_args()
 
 
@@ -191,19 +193,14 @@ def run_reference(args):
         "e2e": {"value": v, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}))
 
 
-def run_b200(args):
+def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit=0.0, batch=0, want_e2e=True, want_cpu=True,
+            min_seconds=0.0, want_sweep=True, prof_steps=None):
+    """One workload through the C ABI: K timed steps (CUDA events on the launching stream, clocks sampled meanwhile), then the
+    per-kernel device times over the same steps, the host-buffer end-to-end loop and the oracle sample.  Returns a dict."""
     import torch
     from paper_2505_14372_b200 import ptycho, shard
-    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
-    torch.cuda.set_device(local)
-    dist = None
-    if world > 1:
-        import torch.distributed as dist
-        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
-    cfg, conf = workload(args.config, args.bandlimit)
+    from paper_2505_14372_b200 import synth as _synth
+    cfg, conf = workload(cfg_idx, bandlimit)
     J = cfg.n_pos
     obj_h, pr_h, pos_h, I_h = host_inputs(cfg)
     pbg = ptycho.Problem(**problem_kwargs(cfg))
@@ -213,24 +210,23 @@ def run_b200(args):
     gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
     loss = torch.zeros(1, dtype=torch.float64, device="cuda")
     cap = int(args.ws_gib * (1 << 30)) if args.ws_gib > 0 else None
-    mb = MINIBATCH.get(args.config)
-    lsqml = args.config == 5
+    mb = MINIBATCH.get(cfg_idx)
+    lsqml = cfg_idx == 5
     if lsqml:
-        mb = args.batch or 1024
-    from paper_2505_14372_b200 import synth as _synth
+        mb = batch or 1024
     batches = None if mb is None else [torch.from_numpy(b).cuda() for b in _synth.batches(cfg, mb)]
     fl = ptycho.WANT_POS_GRAD | ((ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES) if lsqml else 0)
     ws = ptycho.make_workspace(pbg, J, J if lsqml else (mb or J), fl, max_bytes=cap)
     if batches is not None and not lsqml:
         conf.update(minibatch=mb, grouping="seeded permutation (sparse), gradients accumulated over the batches, one update")
-        args.no_e2e = True      # the host-buffer entry point takes one batch per call: no whole-iteration e2e at this size
+        want_e2e = False        # the host-buffer entry point takes one batch per call: no whole-iteration e2e at this size
     if lsqml:
         # config 5: per batch, gradient + illumination map + step-size sweep (second pass over the chain) + LSQML update
         conf.update(minibatch=mb, grouping="seeded permutation (sparse); per batch: gradient, step-size sweep, LSQML update",
                     flags="POS_GRAD | ILLUM | STEP_SIZES")
         illum = torch.zeros(obj.shape, dtype=torch.float32, device="cuda")
         illum_prev = torch.full(obj.shape, float(cfg.dose) / (cfg.step_px ** 2), dtype=torch.float32, device="cuda")   # ~ dose per scan-step area
-        args.no_e2e = True      # the host-buffer entry point has no step-size outputs
+        want_e2e = False        # the host-buffer entry point has no step-size outputs
         st_terms = torch.empty((J, 2 * cfg.n_slices + 6), dtype=torch.float32, device="cuda")
         LS = dict(mode=ptycho.UPDATE_LSQML, beta_obj=1e-3, beta_probe=1e-3, gamma=1e-2)
 
@@ -241,6 +237,8 @@ def run_b200(args):
                             illum_prev=illum_prev, step_terms=st_terms[:nb], loss=loss)
             ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, illum_prev=illum_prev, step_terms=st_terms[:nb],
                                 batch_idx=b, workspace=ws, **LS)
+
+    order = None if batches is None else torch.cat(batches)
 
     def step():
         # weak scaling over ranks: every rank owns J positions of the scan; object / probe are replicated, so the
@@ -262,37 +260,53 @@ def run_b200(args):
         else:
             ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, batch_idx=order, **LR)
 
-    order = None if batches is None else torch.cat(batches)
-
     def barrier():
         torch.cuda.synchronize()
         if dist is not None:
             dist.barrier()
         torch.cuda.synchronize()
 
-    for _ in range(args.warmup):
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    for _ in range(warmup):
         step()
     assert ptycho.status(ws) == 0, "device-side error flag set during warm-up"
+    if min_seconds > 0:
+        # short workloads: enough steps for the timed region to last min_seconds, so that the 100 ms clock sampler sees it
+        torch.cuda.synchronize(); e0.record(); step(); e1.record(); torch.cuda.synchronize()
+        steps = max(steps, int(np.ceil(min_seconds * 1e3 / max(e0.elapsed_time(e1), 1e-3))))
+    # timing rule: inputs larger than L2, or L2 flushed between timed iterations.  The per-step working set (patterns + stash +
+    # staging + far fields) of configs 2-5 is far beyond the 126 MB L2; config 1's is not, so there every step is timed with
+    # its own pair of events and a 512 MB buffer is overwritten between steps.
+    wset = J * cfg.n * cfg.n * (4 + 8 * cfg.n_modes * (2 * cfg.n_slices + 2))
+    flush = torch.empty(512 << 20, dtype=torch.uint8, device="cuda") if wset < 400e6 else None
     clocks = ClockSampler(local) if rank == 0 else None
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     barrier()
     n0 = ptycho.launch_count()
-    e0.record()
-    for _ in range(args.steps):
-        step()
-    e1.record()
-    barrier()
+    if flush is None:
+        e0.record()
+        for _ in range(steps):
+            step()
+        e1.record()
+        barrier()
+        total_ms = e0.elapsed_time(e1)
+    else:
+        evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+        for a, b in evs:
+            flush.zero_()
+            a.record(); step(); b.record()
+        barrier()
+        total_ms = sum(a.elapsed_time(b) for a, b in evs)
     launches = ptycho.launch_count() - n0
-    ms = torch.tensor([e0.elapsed_time(e1)], dtype=torch.float64, device="cuda")
+    ms = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(ms, op=dist.ReduceOp.MAX)
-    ms_step = ms.item() / args.steps
+    ms_step = ms.item() / steps
     clk = clocks.stop() if clocks else None
     loss_val = loss.item()
     assert np.isfinite(loss_val) and ptycho.status(ws) == 0
 
     sweep = None
-    if lsqml and not args.batch:
+    if lsqml and not batch and want_sweep:
         # the paper's grouping sweep: whole-iteration rate at each mini-batch size, one timed iteration each
         sweep = {str(mb): J / (ms_step * 1e-3)}
         for bsz in (64, 256, 4096):
@@ -302,10 +316,11 @@ def run_b200(args):
             sweep[str(bsz)] = J / (e0.elapsed_time(e1) * 1e-3)
         conf.update(batch_sweep_positions_per_s=sweep)
 
-    # per-kernel device time over the same K steps (CUDA events on the launching stream, inside the library)
+    # per-kernel device time (CUDA events on the launching stream, inside the library)
+    psteps = min(steps, prof_steps) if prof_steps else steps
     ptycho.profile_enable(True)
     torch.cuda.synchronize()
-    for _ in range(args.steps):
+    for _ in range(psteps):
         step()
     prof = ptycho.profile_read()
     ptycho.profile_enable(False)
@@ -313,34 +328,42 @@ def run_b200(args):
     top = max(prof, key=lambda k: prof[k][0])
     top_ms, top_n = prof[top]
     hbm, which, sm_max = measured_peaks()
-    units_per_launch = J * args.steps / top_n
+    units_per_launch = J * psteps / top_n
     ab = algorithmic_bytes_per_position(cfg, top)
     # The FFT chain kernels are bound by plain FP32 arithmetic (19.5 flop/B against a machine balance of
     # 11.4), so the line reports "alu": nominal FFT flops (5 N^2 log2 N^2 per 2-D FFT + pointwise) per launch over the
-    # launch duration, against 148 SM x 128 lanes x 2 flop x max SM clock.  The HBM view of the same kernel
-    # (algorithmic bytes: stash + far field) is given beside it.
+    # launch duration, against 148 SM x 128 lanes x 2 flop x max SM clock (peak) and against the FFMA rate measured on this
+    # device in this run (peak_measured, ptycho_profile_fp32_peak).  The HBM view of the same kernel (algorithmic bytes:
+    # stash + far field) is given beside it.
     fp32_peak = 148 * 128 * 2 * sm_max * 1e6 / 1e12
+    fp32_meas = ptycho.profile_fp32_peak(ws)
     roof = {"bound": "alu", "kernel": top, "achieved": None, "peak": fp32_peak, "unit": "TFLOP/s", "frac": None, "traffic": None,
             "peak_source": "derived: 148 SM x 128 FP32 lanes x 2 flop x sm_max_mhz (DESIGN.md §6)",
+            "peak_measured": fp32_meas, "peak_measured_source": "FFMA micro-benchmark in this run (ptycho_profile_fp32_peak)",
             "share_of_step": top_ms / tot, "avg_launch_ms": top_ms / top_n,
-            "kernel_ms_per_step": {k: v[0] / args.steps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
-    if ab is not None:
+            "kernel_ms_per_step": {k: v[0] / psteps for k, v in sorted(prof.items(), key=lambda kv: -kv[1][0])}}
+    # flops of one launch of the dominant kernel: the forward and the backward chain each do half of the FFTs; the fused
+    # single-slice kernel does all of them
+    share = {"k_forward": 0.5, "k_backward": 0.5, "k_single": 1.0}.get(top)
+    if share is not None:
         sec = top_ms / top_n * 1e-3
-        fl = 0.5 * nominal_flops_per_position(cfg)              # the forward and the backward chain each do half of the FFTs
+        fl = share * nominal_flops_per_position(cfg)
         ach = fl * units_per_launch / sec / 1e12
-        achb = ab * units_per_launch / sec / 1e9
-        roof.update(achieved=ach, frac=ach / fp32_peak, nominal_flops_per_launch=fl * units_per_launch,
-                    hbm_view={"achieved": achb, "peak": hbm, "unit": "GB/s", "frac": achb / hbm, "peak_source": which,
-                              "algorithmic_bytes_per_launch": ab * units_per_launch})
+        roof.update(achieved=ach, frac=ach / fp32_peak, frac_of_measured_peak=ach / fp32_meas if fp32_meas > 0 else None,
+                    nominal_flops_per_launch=fl * units_per_launch)
+        if ab is not None:
+            achb = ab * units_per_launch / sec / 1e9
+            roof.update(hbm_view={"achieved": achb, "peak": hbm, "unit": "GB/s", "frac": achb / hbm, "peak_source": which,
+                                  "algorithmic_bytes_per_launch": ab * units_per_launch})
     # traffic: DRAM bytes of one launch of that kernel from the committed `ncu --set full` capture (profiles/), scaled to
     # this run's positions per launch; null if the capture is of another kernel or workload
     try:
         import csv
-        with open(os.path.join(ROOT, "profiles", "r1i_dominant_kernel_traffic.csv")) as f:
-            tr = next(csv.DictReader(f))
-        if tr["kernel"] == top and tr["workload"] == conf["workload"]:
-            roof["traffic"] = (float(tr["dram_bytes_read"]) + float(tr["dram_bytes_write"])) * units_per_launch / float(tr["positions_per_launch"])
-            roof["traffic_source"] = tr["source"]
+        with open(os.path.join(ROOT, "profiles", TRAFFIC_FILE)) as f:
+            for tr in csv.DictReader(f):
+                if tr["kernel"] == top and tr["workload"] == conf["workload"] and not bandlimit:
+                    roof["traffic"] = (float(tr["dram_bytes_read"]) + float(tr["dram_bytes_write"])) * units_per_launch / float(tr["positions_per_launch"])
+                    roof["traffic_source"] = tr["source"]
     except (OSError, KeyError, ValueError, StopIteration):
         pass
     # whole-step view against both roofs of SURVEY §8(d): the io+act byte model and nominal FFT flops on the FP32 ALUs
@@ -352,7 +375,7 @@ def run_b200(args):
 
     # end to end through the host-buffer entry point: pinned host memory in, gradients + loss back, every step
     e2e = None
-    if not args.no_e2e:
+    if want_e2e:
         del ws
         torch.cuda.empty_cache()
         pin = lambda a: torch.from_numpy(np.ascontiguousarray(a)).pin_memory()
@@ -365,11 +388,11 @@ def run_b200(args):
             ptycho.gradient_host(pbg, obj_p, pr_p, pos_p, I_p, workspace=wsh, grad_object_h=gO_p, grad_probe_h=gP_p,
                                  grad_pos_h=gX_p, loss_h=loss_p)
 
-        for _ in range(max(1, min(args.warmup, 2))):
+        for _ in range(max(1, min(warmup, 2))):
             step_host()
         barrier()
         e0.record()
-        for _ in range(args.steps):
+        for _ in range(steps):
             step_host()
         e1.record()
         barrier()
@@ -378,13 +401,16 @@ def run_b200(args):
             dist.all_reduce(msh, op=dist.ReduceOp.MAX)
         h2d = obj_p.numel() * 8 + pr_p.numel() * 8 + pos_p.numel() * 4 + I_p.numel() * 4
         d2h = gO_p.numel() * 8 + gP_p.numel() * 8 + gX_p.numel() * 4 + 8
-        e2e = {"value": world * J / (msh.item() / args.steps * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
-               "d2h_bytes_per_step": d2h, "api": "ptycho_gradient_host (loss + gradients; pinned host buffers)"}
+        e2e = {"value": world * J / (msh.item() / steps * 1e-3), "unit": UNIT, "h2d_bytes_per_step": h2d,
+               "d2h_bytes_per_step": d2h,
+               "api": "ptycho_gradient_host: loss + object / probe / position gradients from and to pinned host buffers; GRADIENT ONLY - "
+                      "the SGD update of `value`'s step (ptycho_apply_update, ~0.04 ms on device arrays) is not part of this loop"}
+        del wsh
 
     cpu = None
-    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+    if rank == 0 and world == 1 and want_cpu:
         from oracle import oracle as orc
-        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 4: 4, 5: 24}[args.config]
+        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 4: 4, 5: 24}[cfg_idx]
         pbo = orc.Problem(**problem_kwargs(cfg))
         t0 = time.perf_counter()
         g = orc.gradient(pbo, obj_h, pr_h, pos_h, I_h, batch_idx=np.arange(n, dtype=np.int32))
@@ -392,16 +418,59 @@ def run_b200(args):
         dt = time.perf_counter() - t0
         cpu = {"value": n / dt, "unit": UNIT, "cores": orc.num_threads(), "kind": "oracle",
                "sample": f"first {n} of {J} positions, one forward+adjoint+update, {dt:.1f} s"}
+    conf.update(parallelism=f"positions sharded over {world} GPU(s), gradients all-reduced" if world > 1 else "1 GPU",
+                global_positions=world * J,
+                l2_policy=(f"per-step working set {wset / 1e6:.0f} MB (patterns + stash + staging) > 126 MB L2, no flush" if flush is None else
+                           f"per-step working set {wset / 1e6:.0f} MB fits L2: a 512 MB buffer is overwritten between timed steps, each "
+                           "step timed with its own pair of CUDA events"),
+                context=PAPER_CONTEXT)
+    return dict(value=world * rate, ms_per_step=ms_step, steps=steps, warmup=warmup, config=conf, clocks=clk, e2e=e2e,
+                gpu_launches=launches, roofline=roof, cpu_baseline=cpu, loss=loss_val)
 
+
+TRAFFIC_FILE = "r2_dominant_kernel_traffic.csv"
+# what the default invocation times after the headline workload: (key, config, keyword overrides)
+SECONDARY = [("config1", 1, {}), ("config2", 2, {}), ("config3_bandlimit_0.667", 3, dict(bandlimit=2.0 / 3.0)),
+             ("config5_batch1024", 5, dict(batch=1024)), ("config4", 4, {})]
+
+
+def run_b200(args):
+    import torch
+    rank = int(os.environ.get("RANK", "0")); world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (there is no CPU fallback)")
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1 or "RANK" in os.environ:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+    common = dict(dist=dist, rank=rank, world=world, local=local)
+    r = measure(args, args.config, steps=args.steps, warmup=args.warmup, bandlimit=args.bandlimit, batch=args.batch,
+                want_e2e=not args.no_e2e, want_cpu=not args.no_cpu_baseline, **common)
+    secondary = None
+    if args.config == 3 and not args.bandlimit and not args.no_secondary and world == 1:
+        # the other configurations of BASELINE.json and the band-limited variant, short runs (1 warm-up + >= 2 timed steps,
+        # at least one second of timed region each), device-resident only
+        secondary = {}
+        for key, idx, over in SECONDARY:
+            torch.cuda.empty_cache()
+            s = measure(args, idx, steps=2, warmup=1, want_e2e=idx in (1, 2), want_cpu=False, min_seconds=1.0, want_sweep=False,
+                        prof_steps=2, **common, **over)
+            rf = s["roofline"]
+            secondary[key] = {"value": s["value"], "unit": UNIT, "ms_per_step": s["ms_per_step"], "steps": s["steps"], "warmup": s["warmup"],
+                              "e2e": None if s["e2e"] is None else s["e2e"]["value"], "gpu_launches_per_step": s["gpu_launches"] / s["steps"],
+                              "dominant_kernel": rf["kernel"], "frac": rf["frac"], "frac_of_measured_peak": rf.get("frac_of_measured_peak"),
+                              "fp32_frac_whole_step": rf["step_model"]["fp32_frac_nominal_fft_flops"],
+                              "kernel_ms_per_step": rf["kernel_ms_per_step"], "clocks": s["clocks"],
+                              "workload": s["config"]["workload"], "minibatch": s["config"].get("minibatch"),
+                              "variant": s["config"].get("variant")}
     if rank == 0:
-        conf.update(parallelism=f"positions sharded over {world} GPU(s), gradients all-reduced" if world > 1 else "1 GPU",
-                    global_positions=world * J, l2_policy="inputs larger than L2 (268 MB patterns + multi-GB stash per step), no flush",
-                    context=PAPER_CONTEXT)
         print(json.dumps({
-            "metric": METRIC, "value": world * rate, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 (complex64)",
-            "data": "synthetic", "config": conf, "clocks": clk, "e2e": e2e, "gpu_launches": launches, "roofline": roof,
-            "cpu_baseline": cpu, "loss": loss_val}))
+            "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": world, "steps": r["steps"], "warmup": r["warmup"],
+            "ms_per_step": r["ms_per_step"], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f32 (complex64)",
+            "data": "synthetic", "config": r["config"], "clocks": r["clocks"], "e2e": r["e2e"], "gpu_launches": r["gpu_launches"],
+            "roofline": r["roofline"], "cpu_baseline": r["cpu_baseline"], "loss": r["loss"], "secondary": secondary}))
     if dist is not None:
         dist.destroy_process_group()
 

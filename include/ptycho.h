@@ -253,6 +253,11 @@ int32_t ptycho_profile_num_kernels(void);
 const char *ptycho_profile_kernel_name(int32_t kind);
 int32_t ptycho_profile_read(float *ms_h, int64_t *launches_h);
 
+/* Measured FP32 FMA throughput of the current device in TFLOP/s (2 flop per FMA), for bench.py's roofline.peak_measured:
+ * a register-only kernel of independent FFMA chains on every SM, best of five launches timed with CUDA events on
+ * `cuda_stream`; synchronises.  workspace_d: any device buffer of >= 512 bytes (never written in practice). */
+int32_t ptycho_profile_fp32_peak(double *tflops_h, void *workspace_d, void *cuda_stream);
+
 const char *ptycho_strerror(int32_t code);
 
 #ifdef __cplusplus

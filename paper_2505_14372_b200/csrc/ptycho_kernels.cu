@@ -1950,6 +1950,47 @@ int32_t ptycho_profile_enable(int32_t on) {
   return PT_OK;
 }
 
+// Measured FP32 FMA throughput (bench.py's roofline.peak_measured): register-only FFMA chains, 16 independent accumulators
+// per thread, 1024 threads x 2 blocks per SM; best of five launches timed with CUDA events.
+__global__ void __launch_bounds__(1024, 2) k_ffma_peak(float* out, float a, float b, int iters) {
+  float x[16];
+#pragma unroll
+  for (int i = 0; i < 16; ++i) x[i] = (float)(threadIdx.x + i);
+  for (int it = 0; it < iters; ++it) {
+#pragma unroll
+    for (int u = 0; u < 4; ++u)
+#pragma unroll
+      for (int i = 0; i < 16; ++i) x[i] = fmaf(x[i], a, b);
+  }
+  float s = 0.f;
+#pragma unroll
+  for (int i = 0; i < 16; ++i) s += x[i];
+  if (s == 12345.678f) out[0] = s;                                  // never true for the a, b passed: keeps the chains alive
+}
+int32_t ptycho_profile_fp32_peak(double* tflops_h, void* workspace_d, void* cuda_stream) {
+  if (!tflops_h || !workspace_d) return PT_ERR_NULL;
+  cudaStream_t st = (cudaStream_t)cuda_stream;
+  int dev = 0, sms = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess || cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) return PT_ERR_CUDA;
+  cudaEvent_t e0, e1;
+  if (cudaEventCreate(&e0) != cudaSuccess || cudaEventCreate(&e1) != cudaSuccess) return PT_ERR_CUDA;
+  const int iters = 8192, blocks = 2 * sms;
+  double best = 0.0;
+  for (int rep = 0; rep < 6; ++rep) {
+    cudaEventRecord(e0, st);
+    k_ffma_peak<<<blocks, 1024, 0, st>>>((float*)workspace_d + 64, 0.999f, 0.001f, iters);
+    cudaEventRecord(e1, st);
+    if (cudaEventSynchronize(e1) != cudaSuccess) { cudaEventDestroy(e0); cudaEventDestroy(e1); return PT_ERR_CUDA; }
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, e0, e1);
+    const double fl = 2.0 * 64.0 * iters * 1024.0 * blocks;
+    if (rep > 0 && ms > 0.f && fl / (ms * 1e-3) / 1e12 > best) best = fl / (ms * 1e-3) / 1e12;
+  }
+  cudaEventDestroy(e0); cudaEventDestroy(e1);
+  *tflops_h = best;
+  return PT_OK;
+}
+
 int32_t ptycho_profile_num_kernels(void) { return K_COUNT; }
 
 const char* ptycho_profile_kernel_name(int32_t kind) { return kind >= 0 && kind < K_COUNT ? kKindNames[kind] : ""; }

@@ -24,7 +24,7 @@ OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
            "ptycho_apply_update", "ptycho_object_transparency", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
            "ptycho_launch_count", "ptycho_strerror", "ptycho_profile_enable", "ptycho_profile_num_kernels",
-           "ptycho_profile_kernel_name", "ptycho_profile_read", "ptycho_regularizer_workspace_bytes", "ptycho_cost_regularizer",
+           "ptycho_profile_kernel_name", "ptycho_profile_read", "ptycho_profile_fp32_peak", "ptycho_regularizer_workspace_bytes", "ptycho_cost_regularizer",
            "ptycho_apply_constraint", "ptycho_adam_update", "ptycho_adam_update_real"]
 
 
@@ -282,6 +282,15 @@ def profile_read() -> dict:
     ms = (C.c_float * n)(); cnt = (C.c_int64 * n)()
     _check(lib().ptycho_profile_read(ms, cnt))
     return {lib().ptycho_profile_kernel_name(i).decode(): (float(ms[i]), int(cnt[i])) for i in range(n) if cnt[i]}
+
+
+def profile_fp32_peak(workspace) -> float:
+    """ptycho_profile_fp32_peak: measured FP32 FMA throughput of the current device, TFLOP/s."""
+    v = C.c_double(0.0)
+    f = lib().ptycho_profile_fp32_peak
+    f.restype = C.c_int32
+    _check(f(C.byref(v), _ptr(workspace), _stream()))
+    return float(v.value)
 
 
 # ---- SURVEY §8(f) rank 3: cost / constraint regularisers and Adam (include/ptycho.h) -----------------------------------
