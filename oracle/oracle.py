@@ -37,6 +37,7 @@ class _Problem(C.Structure):
         ("tilt_x_mrad", C.c_float), ("tilt_y_mrad", C.c_float), ("bandlimit", C.c_float),
         ("loss", C.c_int32), ("loss_c", C.c_float), ("eps", C.c_float),
         ("lsqml_delta_o", C.c_float), ("lsqml_delta_p", C.c_float), ("shift_mode", C.c_int32),
+        ("lsqml_chi_scale", C.c_float),
     ]
 
 
@@ -78,6 +79,7 @@ class Problem:
     lsqml_delta_o: float = 1.0
     lsqml_delta_p: float = 0.0
     shift_mode: int = 0
+    lsqml_chi_scale: float = 1.0    # chi = -lsqml_chi_scale gPhi: 1 steepest descent (R20), 2 modulus-constraint update (R31)
 
     def _c(self, n_pos_total: int, n_batch: int):
         dz = np.ascontiguousarray(np.asarray(self.slice_thickness, dtype=np.float32))
@@ -86,7 +88,7 @@ class Problem:
         s = _Problem(self.n, self.n_modes, self.n_slices, self.obj_ny, self.obj_nx, n_pos_total, n_batch,
                      self.pixel_size, self.wavelength, _p(dz, C.c_float), self.tilt_x_mrad, self.tilt_y_mrad,
                      self.bandlimit, self.loss, self.loss_c, self.eps, self.lsqml_delta_o, self.lsqml_delta_p,
-                     self.shift_mode)
+                     self.shift_mode, self.lsqml_chi_scale)
         s._keep = dz
         return s
 
@@ -242,6 +244,8 @@ def step_terms(pb: Problem, obj, probe, positions, intensity, grad_object, grad_
     rc = lib().orc_step_terms(C.byref(cp), _p(obj, C.c_float), _p(probe, C.c_float), _p(positions, C.c_float),
                               _p(inten, C.c_float), _p(b, C.c_int32), _p(gO, C.c_double), _p(gP, C.c_double),
                               _p(ip, C.c_double), _p(pc, C.c_double), _p(out, C.c_double))
+    if rc == -2:
+        raise ValueError("oracle: the modulus-constraint wavefront update (PAPER.md:173) is defined for the amplitude loss only")
     if rc != 0:
         raise ValueError("oracle: window out of bounds")
     return out

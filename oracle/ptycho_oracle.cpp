@@ -60,6 +60,9 @@ struct orc_problem {
   float lsqml_delta_o;       // delta_O of PAPER.md:219
   float lsqml_delta_p;       // probe analogue (reading R19)
   int32_t shift_mode;        // 0: Fourier shift of the probe (reading R1, default); 1: bilinear sampling of the object
+  float lsqml_chi_scale;     // LSQML wavefront update chi = -lsqml_chi_scale * gPhi: 1 = steepest descent (reading R20);
+                             // 2 = the modulus-constraint update of PAPER.md:173, (ae/(eps+a) - 1) psi~ = -2 w psi~ (reading R31,
+                             // amplitude loss only)
 };
 
 // ------------------------------------------------------------------------------------------
@@ -585,24 +588,31 @@ int32_t orc_gradient(const orc_problem* p, const float* object, const float* pro
 //   grad_object/grad_probe: the batch-aggregated gradients (double, as returned by orc_gradient)
 //   illum_prev: [S][ony][onx] running probe-intensity sum of the previous iteration
 //   step_terms: [J][2S+6]:  (numO,denO) per slice, (numP,denP), (numX_y,denX_y), (numX_x,denX_x)
-// chi_{i,k} := -gPhi_{i,k} (steepest-descent wavefront update, reading R20)
+// chi_{i,k} := -c gPhi_{i,k}, c = lsqml_chi_scale: steepest-descent wavefront update (c = 1, reading R20) or the
+// modulus-constraint update of PAPER.md:173 (c = 2, reading R31); the directions dOhat, dPhat are built from the same chi
+// (PAPER.md:213-219), so they carry the factor c too.
+// Bilinear mode (readings R1, R30): the patch of dOhat is the same four-tap sample as the patch of O; the position enters through
+// the patches of every slice, so numX_a = sum_{i,k,r} Re[chi_{i,k} conj(Psi_{i,k} dT_i/df_a)], denX_a = sum_{i,k,r} |Psi_{i,k} dT_i/df_a|^2
+// (f in px), the least-squares step of the exit waves' first-order change, slice by slice as PAPER.md:221 does for the object.
 // ------------------------------------------------------------------------------------------
 int32_t orc_step_terms(const orc_problem* p, const float* object, const float* probe,
                        const float* positions, const float* intensity, const int32_t* batch_idx,
                        const double* grad_object, const double* grad_probe, const double* illum_prev,
                        const double* probe_precond /* [N][N] or NULL: constant 1 (R19), reading R25 */,
                        double* step_terms) {
-  if (p->shift_mode == 1) return -2;                                            // step terms: Fourier-shift mode only
+  if (p->lsqml_chi_scale != 1.0f && p->loss != 0) return -2;                    // PAPER.md:173 gives the update for the amplitude model
   Model m; model_init(m, p, object, probe, positions, intensity, batch_idx);
   const int J = p->n_batch, N = m.N, M = m.M, S = m.S; const long NN = m.NN;
-  const long on = (long)S * p->obj_ny * p->obj_nx;
+  const long on = (long)S * p->obj_ny * p->obj_nx, os = (long)p->obj_ny * p->obj_nx;
+  const double cs = (double)p->lsqml_chi_scale;
+  const bool bil = p->shift_mode == 1;
   std::vector<cd> dOhat(on);
   for (long o = 0; o < on; ++o)                                                 // O13
-    dOhat[o] = -cd(grad_object[2 * o], grad_object[2 * o + 1]) / (illum_prev[o] + (double)p->lsqml_delta_o);
+    dOhat[o] = -cs * cd(grad_object[2 * o], grad_object[2 * o + 1]) / (illum_prev[o] + (double)p->lsqml_delta_o);
   std::vector<std::vector<cd>> dPhat_t(M, std::vector<cd>(NN));                 // F(dPhat_k)
   for (int k = 0; k < M; ++k) {
     for (long r = 0; r < NN; ++r)
-      dPhat_t[k][r] = -cd(grad_probe[2 * (k * NN + r)], grad_probe[2 * (k * NN + r) + 1]) / ((probe_precond ? probe_precond[r] : 1.0) + (double)p->lsqml_delta_p);
+      dPhat_t[k][r] = -cs * cd(grad_probe[2 * (k * NN + r)], grad_probe[2 * (k * NN + r) + 1]) / ((probe_precond ? probe_precond[r] : 1.0) + (double)p->lsqml_delta_p);
     F2(N, dPhat_t[k].data());
   }
   int err = 0; const int W = 2 * S + 6;
@@ -617,28 +627,42 @@ int32_t orc_step_terms(const orc_problem* p, const float* object, const float* p
     std::vector<std::vector<cd>> gT; double gd[2], Lj;
     adjoint_pos(m, jrow, w, &Lj, gT, nullptr, gd, true);
     double* out = step_terms + (long)jb * W;
+    double numP = 0, denP = 0, numX[2] = {0, 0}, denX[2] = {0, 0};
     for (int i = 0; i < S; ++i) {                                               // O14 object
       double num = 0.0, den = 0.0;
+      std::vector<cd> dOp(NN);                                                  // dOhat_i in the probe view: the patch, sampled like T_i
+      if (!bil) gather_window(N, p->obj_nx, dOhat.data() + i * os, w.r0y, w.r0x, dOp.data());
+      else gather_window_bilinear(N, p->obj_nx, dOhat.data() + i * os, w.r0y, w.r0x, w.dy, w.dx, dOp.data());
       for (int k = 0; k < M; ++k)
+        for (long r = 0; r < NN; ++r) {
+          cd u = dOp[r] * w.Psi[(long)i * M + k][r];
+          cd chi = -cs * w.gPhi[(long)i * M + k][r];
+          num += (chi * std::conj(u)).real(); den += std::norm(u);
+        }
+      out[2 * i] = num; out[2 * i + 1] = den;
+      if (bil)                                                                  // position terms through the patch (R30)
         for (int y = 0; y < N; ++y)
           for (int x = 0; x < N; ++x) {
-            long r = (long)y * N + x;
-            cd u = dOhat[((long)i * p->obj_ny + (w.r0y + y)) * p->obj_nx + (w.r0x + x)] * w.Psi[(long)i * M + k][r];
-            cd chi = -w.gPhi[(long)i * M + k][r];
-            num += (chi * std::conj(u)).real(); den += std::norm(u);
+            auto O = [&](int dy, int dx) { return m.obj[((long)i * p->obj_ny + (w.r0y + y + dy)) * p->obj_nx + (w.r0x + x + dx)]; };
+            const cd dT[2] = {bil_w(0, w.dx) * (O(1, 0) - O(0, 0)) + bil_w(1, w.dx) * (O(1, 1) - O(0, 1)),
+                              bil_w(0, w.dy) * (O(0, 1) - O(0, 0)) + bil_w(1, w.dy) * (O(1, 1) - O(1, 0))};
+            const long r = (long)y * N + x;
+            for (int k = 0; k < M; ++k)
+              for (int a = 0; a < 2; ++a) {
+                cd ss = w.Psi[(long)i * M + k][r] * dT[a]; cd chi = -cs * w.gPhi[(long)i * M + k][r];
+                numX[a] += (chi * std::conj(ss)).real(); denX[a] += std::norm(ss);
+              }
           }
-      out[2 * i] = num; out[2 * i + 1] = den;
     }
-    double numP = 0, denP = 0, numX[2] = {0, 0}, denX[2] = {0, 0};
     for (int k = 0; k < M; ++k) {
       std::vector<cd> v(NN);
       for (long q = 0; q < NN; ++q) v[q] = w.R[q] * dPhat_t[k][q];              // shift_j(dPhat_k)
       Finv2(N, v.data());
       for (long r = 0; r < NN; ++r) {
-        cd vv = v[r] * w.T[0][r]; cd chi = -w.gPhi[k][r];                       // slice 0: index 0*M+k
+        cd vv = v[r] * w.T[0][r]; cd chi = -cs * w.gPhi[k][r];                  // slice 0: index 0*M+k
         numP += (chi * std::conj(vv)).real(); denP += std::norm(vv);
       }
-      for (int a = 0; a < 2; ++a) {
+      for (int a = 0; a < 2 && !bil; ++a) {
         std::vector<cd> s(NN);
         for (int qy = 0; qy < N; ++qy)
           for (int qx = 0; qx < N; ++qx) {
@@ -647,7 +671,7 @@ int32_t orc_step_terms(const orc_problem* p, const float* object, const float* p
           }
         Finv2(N, s.data());
         for (long r = 0; r < NN; ++r) {
-          cd ss = s[r] * w.T[0][r]; cd chi = -w.gPhi[k][r];
+          cd ss = s[r] * w.T[0][r]; cd chi = -cs * w.gPhi[k][r];
           numX[a] += (chi * std::conj(ss)).real(); denX[a] += std::norm(ss);
         }
       }
@@ -680,6 +704,7 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
     return 0;
   }
   const int W = 2 * S + 6;
+  const double cs = (double)p->lsqml_chi_scale;
   if (object && grad_object)
     for (int i = 0; i < S; ++i) {
       double num = 0, den = 0;
@@ -687,8 +712,8 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
       double alpha = num / (den + gamma);
       for (long o = 0; o < os; ++o) {
         long g = (long)i * os + o; double d = illum_prev[g] + (double)p->lsqml_delta_o;
-        object[2 * g] += beta_obj * alpha * (-grad_object[2 * g] / d);
-        object[2 * g + 1] += beta_obj * alpha * (-grad_object[2 * g + 1] / d);
+        object[2 * g] += beta_obj * alpha * (-cs * grad_object[2 * g] / d);      // dOhat = -c gO / d (O13)
+        object[2 * g + 1] += beta_obj * alpha * (-cs * grad_object[2 * g + 1] / d);
       }
     }
   if (probe && grad_probe) {
@@ -696,7 +721,7 @@ int32_t orc_apply_update(const orc_problem* p, int32_t mode, double* object, dou
     for (int jb = 0; jb < J; ++jb) { num += step_terms[(long)jb * W + 2 * S]; den += step_terms[(long)jb * W + 2 * S + 1]; }
     double alpha = num / (den + gamma);
     for (long r = 0; r < 2 * M * NN; ++r)
-      probe[r] += beta_probe * alpha * (-grad_probe[r] / ((probe_precond ? probe_precond[(r / 2) % NN] : 1.0) + (double)p->lsqml_delta_p));
+      probe[r] += beta_probe * alpha * (-cs * grad_probe[r] / ((probe_precond ? probe_precond[(r / 2) % NN] : 1.0) + (double)p->lsqml_delta_p));
   }
   if (positions)
     for (int jb = 0; jb < J; ++jb) { int row = batch_idx ? batch_idx[jb] : jb;
@@ -772,7 +797,7 @@ int32_t orc_lsqml_weighted_object(const orc_problem* p, double* object, const do
   const long on = (long)p->n_slices * p->obj_ny * p->obj_nx;
   for (long o = 0; o < on; ++o) {
     if (!(illum_batch[o] > 0.0)) continue;
-    const double f = beta_obj * (willum[o] / illum_batch[o]) / (illum_prev[o] + (double)p->lsqml_delta_o);
+    const double f = (double)p->lsqml_chi_scale * beta_obj * (willum[o] / illum_batch[o]) / (illum_prev[o] + (double)p->lsqml_delta_o);
     object[2 * o] += f * (-grad_object[2 * o]);
     object[2 * o + 1] += f * (-grad_object[2 * o + 1]);
   }

@@ -713,6 +713,108 @@ def test_bilinear_gradient_finite_differences():
     assert abs(g["illum"][0].sum() - 4 * (np.abs(probe.astype(complex)) ** 2).sum()) < 1e-9 * g["illum"][0].sum()
 
 
+def test_bilinear_step_terms():
+    # readings R1 / R30: LSQML step-size terms with the patches sampled bilinearly.
+    n, on, M, S, J = 8, 20, 2, 3, 4
+    pb, obj, probe, pos = _bilinear_problem(n=n, M=M, S=S, on=on, J=J)
+    pb.lsqml_delta_o = 0.7; pb.lsqml_delta_p = 0.2
+    obj_t = (obj * np.exp(0.2 * crandn(*obj.shape))).astype(np.complex64)
+    Iexp = orc.forward_loss(pb, obj_t, probe, pos)["intensity"].astype(np.float32) + 0.05
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    illum_prev = g["illum"] * 1.3 + 0.1
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], illum_prev)
+    px = float(np.float32(pb.pixel_size))
+    # (1) numX_a = -1/2 dL/df_a (f in px; grad_pos is per Angstrom and is itself pinned by finite differences above)
+    assert np.abs(st[:, 2 * S + 2] + 0.5 * g["grad_pos"][:, 0] * px).max() < 1e-9 * np.abs(g["grad_pos"] * px).max()
+    assert np.abs(st[:, 2 * S + 4] + 0.5 * g["grad_pos"][:, 1] * px).max() < 1e-9 * np.abs(g["grad_pos"] * px).max()
+    # (2) denominators restated in numpy from the illumination of ONE position: sum_k |Psi_{i,k}|^2 in the probe view is the
+    # oracle's own illumination map of that position sampled back... instead use S = 1, where Psi_0 = P_k (unshifted probe):
+    pb1, obj1, probe1, pos1 = _bilinear_problem(n=n, M=M, S=1, on=on, J=2)
+    pb1.lsqml_delta_o = 0.7; pb1.lsqml_delta_p = 0.2
+    I1 = orc.forward_loss(pb1, (obj1 * 1.05).astype(np.complex64), probe1, pos1)["intensity"].astype(np.float32) + 0.1
+    g1 = orc.gradient(pb1, obj1, probe1, pos1, I1, want_illum=True)
+    ip1 = g1["illum"] + 0.5
+    st1 = orc.step_terms(pb1, obj1, probe1, pos1, I1, g1["grad_object"], g1["grad_probe"], ip1)
+    dOhat = -g1["grad_object"] / (ip1 + float(np.float32(0.7)))
+    dPhat = -g1["grad_probe"] / (1.0 + float(np.float32(0.2)))
+    P2 = (np.abs(probe1.astype(complex)) ** 2).sum(0)
+    for j in range(2):
+        (i0y, fy), (i0x, fx) = orc.position_split_floor(float(pos1[j, 0]), 0.2, n), orc.position_split_floor(float(pos1[j, 1]), 0.2, n)
+        T = orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy, fx)
+        dT = orc.bilinear(n, dOhat[0], i0y, i0x, fy, fx)                       # dOhat sampled like the patch
+        psit = np.stack([np.fft.fft2(probe1[k].astype(complex) * T) / n for k in range(M)])
+        w = 1 - I1[j] / ((np.abs(psit) ** 2).sum(0) + float(np.float32(pb1.eps)))
+        chi = np.stack([-n * np.fft.ifft2(w * psit[k]) for k in range(M)])
+        num = sum(np.sum(np.real(chi[k] * np.conj(dT * probe1[k]))) for k in range(M))
+        assert abs(st1[j, 0] - num) < 1e-9 * abs(num) and abs(st1[j, 1] - np.sum(np.abs(dT) ** 2 * P2)) < 1e-10 * st1[j, 1]
+        numP = sum(np.sum(np.real(chi[k] * np.conj(dPhat[k] * T))) for k in range(M))
+        denP = sum(np.sum(np.abs(dPhat[k] * T) ** 2) for k in range(M))
+        assert abs(st1[j, 2] - numP) < 1e-9 * abs(numP) and abs(st1[j, 3] - denP) < 1e-10 * denP
+        # dT/df by central differences of the sampler itself (bilinear sampling is bilinear in f: exact)
+        h = 1e-3
+        dTy = (orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy + h, fx) - orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy - h, fx)) / (2 * h)
+        dTx = (orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy, fx + h) - orc.bilinear(n, obj1[0].astype(complex), i0y, i0x, fy, fx - h)) / (2 * h)
+        for a, d in enumerate((dTy, dTx)):
+            den = np.sum(np.abs(d) ** 2 * P2)
+            numx = sum(np.sum(np.real(chi[k] * np.conj(probe1[k] * d))) for k in range(M))
+            assert abs(st1[j, 5 + 2 * a] - den) < 1e-8 * den and abs(st1[j, 4 + 2 * a] - numx) < 1e-8 * abs(numx) + 1e-12
+    # (3) integer corners: object and probe terms equal those of the Fourier-shift mode (both reduce to the integer window and the
+    # unshifted probe)
+    pos_int = (np.array([[5, 6], [4, 9], [7, 5], [9, 9]]) * 0.2).astype(np.float32)
+    pf = orc.Problem(**{**pb.__dict__, "shift_mode": orc.SHIFT_FOURIER_PROBE})
+    gb = orc.gradient(pb, obj, probe, pos_int, Iexp, want_illum=True)
+    sb = orc.step_terms(pb, obj, probe, pos_int, Iexp, gb["grad_object"], gb["grad_probe"], illum_prev)
+    sf = orc.step_terms(pf, obj, probe, pos_int, Iexp, gb["grad_object"], gb["grad_probe"], illum_prev)
+    assert np.abs(sb[:, :2 * S + 2] - sf[:, :2 * S + 2]).max() < 1e-10 * np.abs(sf[:, :2 * S + 2]).max()
+
+
+def test_lsqml_modulus_constraint_chi():
+    # reading R31: lsqml_chi_scale = 2 makes chi the modulus-constraint wavefront update of PAPER.md:173 (amplitude model).
+    # (1) one position, one slice, one mode, illum_prev = this position's |Psi|^2, delta_O -> 0, gamma = 0, eps -> 0, c = 0: the
+    #     LSQML object step with beta = 1 turns the exit wave into the modulus-projected one, Finv(sqrt(Iexp) F(psi) / |F(psi)|)
+    #     ("the classic modulus constraint"), wherever the probe is non-zero
+    n, on = 16, 40
+    pb, obj, probe, pos = small_problem(n=n, M=1, S=1, on=on, J=1, loss=orc.LOSS_AMPLITUDE, eps=1e-30)
+    pb.lsqml_delta_o = 1e-30; pb.lsqml_chi_scale = 2.0
+    pos[:] = (np.array([[21, 18]]) * 0.2).astype(np.float32)                 # integer corner
+    Iexp = RNG.uniform(0.5, 3.0, size=(1, n, n)).astype(np.float32)
+    g = orc.gradient(pb, obj, probe, pos, Iexp, want_illum=True)
+    illum_prev = np.where(g["illum"] > 0, g["illum"], 1.0)
+    st = orc.step_terms(pb, obj, probe, pos, Iexp, g["grad_object"], g["grad_probe"], illum_prev)
+    assert abs(st[0, 0] / st[0, 1] - 1.0) < 1e-9                             # alpha_O = 1
+    o2, _, _ = orc.apply_update(pb, 1, obj, probe, pos, g["grad_object"], None, None, illum_prev, st, beta_obj=1.0)
+    r0y, r0x = 21 - n // 2, 18 - n // 2
+    f = np.where(np.arange(n) < n // 2, np.arange(n), np.arange(n) - n) / n
+    (_, dy), (_, dx) = orc.position_split(float(pos[0, 0]), 0.2, n), orc.position_split(float(pos[0, 1]), 0.2, n)
+    P = np.fft.ifft2(np.exp(-2j * np.pi * (f[:, None] * dy + f[None, :] * dx)) * np.fft.fft2(probe[0].astype(complex)))
+    psi = P * obj[0, r0y:r0y + n, r0x:r0x + n].astype(complex)
+    Fp = np.fft.fft2(psi)
+    psi_c = np.fft.ifft2(np.sqrt(Iexp[0].astype(float)) * n * Fp / np.abs(Fp))
+    assert np.abs(P * o2[0, r0y:r0y + n, r0x:r0x + n] - psi_c).max() < 1e-8 * np.abs(psi_c).max()
+    # (2) against chi_scale = 1 on a multislice, two-mode case: object / probe terms x4, position numerators x2, position
+    #     denominators unchanged; the update direction doubles
+    pb2, obj2, probe2, pos2 = small_problem(n=8, M=2, S=3, on=20, J=3, loss=orc.LOSS_AMPLITUDE, eps=0.5)
+    pb2.lsqml_delta_o = 0.7; pb2.lsqml_delta_p = 0.2
+    I2 = orc.forward_loss(pb2, (obj2 * 1.05).astype(np.complex64), probe2, pos2)["intensity"].astype(np.float32) + 0.1
+    g2 = orc.gradient(pb2, obj2, probe2, pos2, I2, want_illum=True)
+    ip = g2["illum"] + 0.5
+    s1 = orc.step_terms(pb2, obj2, probe2, pos2, I2, g2["grad_object"], g2["grad_probe"], ip)
+    import dataclasses
+    pbm = dataclasses.replace(pb2, lsqml_chi_scale=2.0)
+    s2 = orc.step_terms(pbm, obj2, probe2, pos2, I2, g2["grad_object"], g2["grad_probe"], ip)
+    S = 3
+    scale = np.array([4.0] * (2 * S + 2) + [2.0, 1.0, 2.0, 1.0])
+    assert np.abs(s2 - s1 * scale).max() < 1e-12 * np.abs(s2).max()
+    a1 = orc.apply_update(pb2, 1, obj2, probe2, pos2, g2["grad_object"], g2["grad_probe"], None, ip, s1, beta_obj=0.5, beta_probe=0.5)
+    a2 = orc.apply_update(pbm, 1, obj2, probe2, pos2, g2["grad_object"], g2["grad_probe"], None, ip, s2, beta_obj=0.5, beta_probe=0.5)
+    assert np.abs((a2[0] - obj2) - 2 * (a1[0] - obj2)).max() < 1e-9 * np.abs(a1[0] - obj2).max()
+    assert np.abs((a2[1] - probe2) - 2 * (a1[1] - probe2)).max() < 1e-9 * np.abs(a1[1] - probe2).max()
+    assert np.abs((a2[2] - pos2) - 2 * (a1[2] - pos2)).max() < 1e-9 * np.abs(a1[2] - pos2).max()
+    # (3) the paper gives the modulus-constraint update for the amplitude model only
+    with pytest.raises(ValueError):
+        orc.step_terms(dataclasses.replace(pbm, loss=orc.LOSS_POISSON), obj2, probe2, pos2, I2, g2["grad_object"], g2["grad_probe"], ip)
+
+
 # ------------------------------------------------------------------------------------------------
 # change detector: stored oracle outputs of a tiny seeded case (tests/golden/, written by make_golden.py from oracle/ only)
 # ------------------------------------------------------------------------------------------------
