@@ -41,8 +41,9 @@ enum { PT_SHIFT_FOURIER_PROBE = 0,    /* integer window on the obj
        PT_SHIFT_BILINEAR_OBJECT = 1 };/* PAPER.md:61 "sampled" (R1, secondary): probe unshifted; the patch is a four-tap
                                        * bilinear sample of the object at c + r, c = X/px - N/2 = i0 + f (i0 = floor(c));
                                        * the object gradient is scattered with the same weights and dL/dX comes through
-                                       * the weights (i0 fixed).  Windows need i0 + N <= size - 1.  PT_WANT_STEP_SIZES is
-                                       * not available in this mode (PT_ERR_UNSUPPORTED).                              */
+                                       * the weights (i0 fixed).  Windows need i0 + N <= size - 1.  Step-size terms (R30): dOhat is
+                                       * sampled with the same four taps; the position terms come through the patch,
+                                       * numX_a = -1/2 dL/df_a, denX_a = sum_{i,k,r} |Psi_{i,k} dT_i/df_a|^2 (f in px).            */
 
 enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                                                        */
        PT_WANT_ILLUM = 2,             /* fill illum_d with sum_{j,k} |Psi_{i,k,j}|^2             */
@@ -52,6 +53,11 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
                                        * W_i = sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2, alpha_{O,i,j} = numO[j,i] / (denO[j,i] +
                                        * lsqml_gamma): the per-position step sizes of PAPER.md:221 weighting the slice update as
                                        * PAPER.md:225 prints it (reading R24); used by PT_UPDATE_LSQML_WEIGHTED              */
+       PT_LSQML_MODULUS_CHI = 256,    /* with PT_WANT_STEP_SIZES / PT_UPDATE_LSQML*: the LSQML wavefront update is the modulus-constraint
+                                       * update of PAPER.md:173, chi~ = (sqrt(Iexp+c)/(eps+sqrt(I+c)) - 1) psi~ = -2 gPhi~ (reading R31), instead
+                                       * of the steepest-descent chi = -gPhi (R20): numerators and denominators of the object and probe
+                                       * terms x4, position numerators x2, update directions x2.  PT_LOSS_AMPLITUDE only (the paper gives
+                                       * that update for the amplitude model), else PT_ERR_UNSUPPORTED                          */
        PT_NO_MODE_PAIRS = 128,        /* debugging aid: the backward pass runs one mode per CTA even when the mode count is even
                                        * (no tensor-memory allocation); results differ only by the rounding of one float32 add */
        PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of
@@ -113,8 +119,11 @@ typedef struct {                  /* HOST struct */
 #define PT_STEP_TERMS_PER_POS(S) (2 * (S) + 6)
 
 /* Device scratch the caller must supply.  ptycho_workspace_bytes returns the RECOMMENDED size (positions are
- * processed in chunks; a larger workspace means larger chunks, capped at 49 GiB); ptycho_workspace_min_bytes the
- * smallest size the calls accept.  The first 64 bytes hold the deferred status word. */
+ * processed in chunks; a larger workspace means larger chunks, capped at 49 GiB — with PT_WANT_STEP_SIZES the patch
+ * gradients, probe partials and |Psi|^2 the backward pass stages are kept for the whole batch on top of that, up to 150 GiB
+ * in total, so that the step-size sweep needs no second pass through the chain); ptycho_workspace_min_bytes the smallest
+ * size the calls accept (with step sizes and a batch that does not fit, each chunk is then recomputed for the sweep).
+ * The first 256 bytes hold the deferred status word. */
 size_t ptycho_workspace_bytes(const pt_problem *p);
 size_t ptycho_workspace_min_bytes(const pt_problem *p);
 /* Positions kept in flight per chunk (the memory unit, as opposed to the mini-batch p->n_batch, the optimisation

@@ -88,20 +88,22 @@ struct Ws {
   double2* gPt_acc;    // [M][N^2]  F-native accumulators
   double* loss_pp;     // [J][CL]
   double* posg_part;   // [J][M][CL][2]
-  double* step_part;   // [J][M][CL][2S+6]
+  double* step_oi;     // [J][S][6]       step-size sweep: (numO, denO) of slice i; bilinear mode also (numX_y, denX_y, numX_x, denX_x)
+  double* step_pp;     // [J][M][CL][6]   step-size sweep: (numP, denP, numX_y, denX_y, numX_x, denX_x) of one mode (and rank)
   cf* dOhat;           // [S][ony][onx]      (step sizes only)
   // chunked
   cf* psit;            // [Jc][M][N^2]  F-native
   float* wdet;         // [Jc][N^2]     F-native
   cf* stash;           // [Jc][M][S][N^2]  R-native
-  cf* gTpart;          // [Jc][M or M/2][S][N^2]  R-native (staged_planes)
-  cf* Gpart;           // [Jc][M][N^2]     F-native
-  cf* scratch;         // [Jc][M][N^2]     (step sizes: gPhi_0)
+  // staged by the backward pass, indexed by (jl + KP::js): per chunk, or per BATCH position when stage_all (step sizes)
+  cf* gTpart;          // [Jc|J][M or M/2][S][N^2]  R-native (staged_planes)
+  cf* Gpart;           // [Jc|J][M][N^2]     F-native
   float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
   float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
   cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
   float* alpha_ji;     // [Jc][S]          per-position object step sizes alpha_{O,i,j} (PT_WANT_WEIGHTED_ILLUM only)
-  float* ilpart;       // [Jc][M][S][N^2]  R-native |Psi_{i,k}|^2 written by k_backward_pair (PT_WANT_ILLUM with paired modes)
+  float* ilpart;       // [Jc|J][M][S][N^2]  R-native |Psi_{i,k}|^2 written by the backward kernels (step sizes; PT_WANT_ILLUM with paired modes)
+  int32_t stage_all;   // the three staged arrays hold the whole batch (the step-size sweep reads them after the last chunk)
   int32_t Jc;
   size_t total;
 };
@@ -113,8 +115,10 @@ inline bool use_pairs(const pt_problem* p) { return (p->n_modes % 2) == 0 && !(p
 inline size_t staged_planes(const pt_problem* p) { return use_pairs(p) ? p->n_modes / 2 : p->n_modes; }   // gT planes per position
 inline size_t cluster_of(int n) { return n == 256 ? 4 : 1; }   // CTAs per field (Geo<n>::CL)
 
-// per-chunk-position bytes and fixed bytes
-void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
+// fixed bytes, bytes per position in flight (chunk), bytes per position of what the backward pass stages (patch gradients,
+// probe partials), and the optional |Psi|^2 staging (illumination map with paired modes; mandatory for the step-size sweep)
+struct WsSizes { size_t fixed, per_chunk, per_staged, per_il; bool il_needed; };
+WsSizes ws_sizes(const pt_problem* p) {
   const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch, CL = cluster_of(p->n);
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   size_t f = 256;
@@ -122,36 +126,51 @@ void ws_sizes(const pt_problem* p, size_t* fixed, size_t* per_pos) {
   f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float)) + align_up(J * sizeof(int32_t));
   f += 2 * align_up(M * NN * sizeof(cf)) + align_up(M * NN * sizeof(double2));
   f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
-  f += align_up(J * M * CL * (2 * S + 6) * sizeof(double));
+  f += align_up(J * S * 6 * sizeof(double)) + align_up(J * M * CL * 6 * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
-  size_t pp = M * NN * sizeof(cf) + NN * sizeof(float) + (M + staged_planes(p)) * S * NN * sizeof(cf) + M * NN * sizeof(cf);
-  if (steps) pp += M * NN * sizeof(cf) + S * sizeof(float);
-  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) pp += S * NN * sizeof(cf);
-  if (p->flags & PT_EPIE) pp += (M * CL + 1) * S * sizeof(float) + 64;
-  *fixed = f + 13 * 256;   // slack for the per-array alignment of the chunked part
-  *per_pos = pp;
+  WsSizes z;
+  z.fixed = f + 13 * 256;   // slack for the per-array alignment of the chunked part
+  z.per_chunk = M * NN * sizeof(cf) + NN * sizeof(float) + M * S * NN * sizeof(cf);
+  if (steps) z.per_chunk += S * sizeof(float);
+  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) z.per_chunk += S * NN * sizeof(cf);
+  if (p->flags & PT_EPIE) z.per_chunk += (M * CL + 1) * S * sizeof(float) + 64;
+  z.per_staged = staged_planes(p) * S * NN * sizeof(cf) + M * NN * sizeof(cf);
+  z.il_needed = steps;
+  z.per_il = 0;
+  if (!(p->flags & PT_EPIE) && (steps || ((p->flags & PT_WANT_ILLUM) && use_pairs(p)))) z.per_il = M * S * NN * sizeof(float);
+  return z;
 }
-// optional per-position bytes: the |Psi|^2 staging of the illumination map (k_backward_pair writes it, the gather then reads
-// 4 bytes per mode instead of the 8-byte stash entries); 0 where it does not apply
-size_t il_bytes_per_pos(const pt_problem* p) {
-  if (!(p->flags & PT_WANT_ILLUM) || !use_pairs(p) || (p->flags & PT_EPIE)) return 0;
-  return (size_t)p->n_modes * p->n_slices * p->n * p->n * sizeof(float);
-}
-// positions in flight for a workspace of `bytes`, and whether the optional staging is used: it is when the whole batch still
-// fits with it, or when the batch is chunked anyway; not when it alone would force chunking (a caller who sized the workspace
-// for the batch without PT_WANT_ILLUM gets the same single chunk as before)
-struct ChunkPlan { size_t jc; bool il; };
+// Positions in flight for a workspace of `bytes`.  Without step sizes everything is per chunk; the optional |Psi|^2 staging is
+// used when the whole batch still fits with it, or when the batch is chunked anyway, not when it alone would force chunking (a
+// caller who sized the workspace for the batch without PT_WANT_ILLUM gets the same single chunk as before).  With step sizes
+// the staged arrays are kept for the WHOLE batch when the workspace allows (stage_all): the sweep then reads them after the last
+// chunk; otherwise each chunk is recomputed for the sweep.
+struct ChunkPlan { size_t jc; bool il; bool stage_all; };
 ChunkPlan plan_chunks(const pt_problem* p, size_t bytes) {
-  size_t fixed, pp;
-  ws_sizes(p, &fixed, &pp);
-  ChunkPlan c = {0, false};
-  if (bytes < fixed + pp) return c;
-  const size_t J = (size_t)p->n_batch, pil = il_bytes_per_pos(p);
-  size_t jc0 = (bytes - fixed) / pp;
+  const WsSizes z = ws_sizes(p);
+  ChunkPlan c = {0, false, false};
+  const size_t J = (size_t)p->n_batch;
+  if (z.il_needed) {
+    const size_t pp = z.per_chunk + z.per_staged + z.per_il;
+    if (bytes < z.fixed + pp) return c;
+    c.il = true;
+    c.jc = (bytes - z.fixed) / pp;
+    if (c.jc >= J) { c.jc = J; return c; }
+    const size_t staged = J * (z.per_staged + z.per_il), floor_jc = J < 64 ? J : 64;
+    if (bytes >= z.fixed + staged + floor_jc * z.per_chunk) {
+      c.stage_all = true;
+      c.jc = (bytes - z.fixed - staged) / z.per_chunk;
+      if (c.jc > J) c.jc = J;
+    }
+    return c;
+  }
+  const size_t pp = z.per_chunk + z.per_staged;
+  if (bytes < z.fixed + pp) return c;
+  size_t jc0 = (bytes - z.fixed) / pp;
   if (jc0 > J) jc0 = J;
   c.jc = jc0;
-  if (pil) {
-    size_t jc1 = (bytes - fixed) / (pp + pil);
+  if (z.per_il) {
+    size_t jc1 = (bytes - z.fixed) / (pp + z.per_il);
     if (jc1 > J) jc1 = J;
     if (jc1 >= 1 && (jc1 == J || jc0 < J)) { c.jc = jc1; c.il = true; }
   }
@@ -159,12 +178,11 @@ ChunkPlan plan_chunks(const pt_problem* p, size_t bytes) {
 }
 
 int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
-  size_t fixed, pp;
-  ws_sizes(p, &fixed, &pp);
   const ChunkPlan plan = plan_chunks(p, bytes);
   if (plan.jc == 0) return PT_ERR_WORKSPACE;
   const size_t jc = plan.jc;
   const size_t N = p->n, NN = N * N, M = p->n_modes, S = p->n_slices, J = p->n_batch, CL = cluster_of(p->n);
+  const size_t js = plan.stage_all ? J : jc;                       // positions the staged arrays hold
   const bool steps = (p->flags & PT_WANT_STEP_SIZES) != 0;
   char* c = (char*)base;
   size_t off = 0;
@@ -181,19 +199,20 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->gPt_acc = (double2*)take(M * NN * sizeof(double2));
   w->loss_pp = (double*)take(J * CL * sizeof(double));
   w->posg_part = (double*)take(J * M * CL * 2 * sizeof(double));
-  w->step_part = (double*)take(J * M * CL * (2 * S + 6) * sizeof(double));
+  w->step_oi = (double*)take(J * S * 6 * sizeof(double));
+  w->step_pp = (double*)take(J * M * CL * 6 * sizeof(double));
   w->dOhat = steps ? (cf*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf)) : nullptr;
   w->psit = (cf*)take(jc * M * NN * sizeof(cf));
   w->wdet = (float*)take(jc * NN * sizeof(float));
   w->stash = (cf*)take(jc * M * S * NN * sizeof(cf));
-  w->gTpart = (cf*)take(jc * staged_planes(p) * S * NN * sizeof(cf));
-  w->Gpart = (cf*)take(jc * M * NN * sizeof(cf));
-  w->scratch = steps ? (cf*)take(jc * M * NN * sizeof(cf)) : nullptr;
+  w->gTpart = (cf*)take(js * staged_planes(p) * S * NN * sizeof(cf));
+  w->Gpart = (cf*)take(js * M * NN * sizeof(cf));
   w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
   w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
   w->alpha_ji = steps ? (float*)take(jc * S * sizeof(float)) : nullptr;
-  w->ilpart = plan.il ? (float*)take(jc * M * S * NN * sizeof(float)) : nullptr;
+  w->ilpart = plan.il ? (float*)take(js * M * S * NN * sizeof(float)) : nullptr;
+  w->stage_all = plan.stage_all ? 1 : 0;
   w->Jc = (int32_t)jc;
   w->total = off;
   return off <= bytes ? PT_OK : PT_ERR_WORKSPACE;
@@ -207,6 +226,8 @@ struct KP {
   int Jtot;                          // rows of positions / intensity (n_pos_total)
   int Mg;                            // patch-gradient planes per position in the staging buffer: M, or M/2 after k_backward_pair
   int j0, jc;                        // current chunk: batch-local offset and count
+  int js;                            // position offset into the staged arrays (gTpart, Gpart, ilpart): j0 when they hold the whole batch, else 0
+  float chi_scale;                   // step-size sweep: chi = -chi_scale gPhi (1; 2 under PT_LSQML_MODULUS_CHI, reading R31)
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
   int loss; float loss_c, eps;
   int bilinear;                      // PT_SHIFT_BILINEAR_OBJECT: probe unshifted, patches sampled with four taps (reading R1)
@@ -340,6 +361,10 @@ struct ChainSmem {
 };
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
+}
+// one thread asks for `bytes` (a multiple of 16, 16-byte aligned) of global memory to be brought into L2
+__device__ __forceinline__ void l2_prefetch_bulk(const void* src, unsigned bytes) {
+  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
 }
 __device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
@@ -612,11 +637,11 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int
 }
 
 // ------------------------------------------------------------------------------------------------
-// H9, H10, H12, H13 backward: one CTA (CL = 4: one cluster) per (j,k) pair of the chunk.
-// MODE 0: gradient pass — writes gT partials, probe partials, position terms.
-// MODE 1: step-size sweep (H14) — instead accumulates numO/denO per slice and the probe / position terms.
+// H9, H10, H12, H13 backward: one CTA (CL = 4: one cluster) per (j,k) pair of the chunk: writes the patch-gradient partials
+// gT_i, the probe partial conj(R) G~ and the position-gradient terms.  MODE 0: gradients; MODE 2: ePIE directions (R23).
+// IL: also stage |Psi_{i,k}|^2 (illumination map O12; denominators of the step-size sweep).
 // ------------------------------------------------------------------------------------------------
-template <class G, int MODE>
+template <class G, int MODE, bool IL>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int want_pos) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL;   // stash pairs [0,E) early, [E,16) late; T pairs [0,E) late
@@ -628,19 +653,21 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   cs.fill_tables(t);
   Fft<G>::begin_fourier();
   const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  const int spair = (jl + P.js) * P.M + k;                          // the same (position, mode) in the staged arrays
   const int unit = (jb * P.M + k) * CL + (int)rk;                 // index of this CTA's fp64 partials
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   // patch source: the object window itself, or (bilinear mode) this position's resampled patches [S][NF][NF]
   const int S = P.S, onx = P.bilinear ? NF : P.onx;
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
-  auto fld = [&](int i) { return (((size_t)pair * S + i) * CL + rk) * NNS; };   // field (pair, slice i), this rank's block
+  auto fld = [&](int pr, int i) { return (((size_t)pr * S + i) * CL + rk) * NNS; };   // field (index pr, slice i), this rank's block
   const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
   const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
   // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
   auto early = [&](int i) {
-    const float4* st = (const float4*)(P.w.stash + fld(i)) + t;
+    const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
 #pragma unroll
     for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+    if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);               // the late part of the same field: DRAM -> L2 now
     if (i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
     cp_async_commit();
   };
@@ -662,7 +689,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
     {   // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
-      const float4* st = (const float4*)(P.w.stash + fld(i)) + t;
+      const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
 #pragma unroll
       for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
 #pragma unroll
@@ -675,131 +702,201 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
-    if (MODE != 1) {
-      // ePIE (MODE 2): dO = conj(Psi) / max|Psi|^2 chi ; chi' = conj(T) / max|T|^2 chi
-      float s1 = 1.0f, s2 = 1.0f;
-      if (MODE == 2) {
-        float pm = 0.f;
-        for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pair * S + i) * CL + c]);
-        const float tm = P.w.tmax[(size_t)jl * S + i];
-        s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;   // a dead mode / an opaque window contributes nothing
-      }
-      float4* gt = (float4*)(P.w.gTpart + fld(i));
-#pragma unroll
-      for (int p = 0; p < 16; ++p) {
-        const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
-        cf T0, T1;
-        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
-        cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
-        if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
-        __stcs(gt + p * T + t, make_float4(g0.x, g0.y, g1.x, g1.y));    // H10: gT_i contribution conj(Psi) .* gPhi
-        v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
-        v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
-      }
-      if (i > 0) early(i - 1);
-    } else {
-      // H14 object terms: u = dOhat|patch .* Psi ; chi = -gPhi ; num += Re(chi conj(u)) ; den += |u|^2
-      const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x + pix0;
-      float num = 0.f, den = 0.f;
-      if (i == 0) {                                              // keep gPhi_0 for the probe / position terms
-        float4* sc0 = (float4*)(P.w.scratch + ((size_t)pair * CL + rk) * NNS);
-#pragma unroll
-        for (int p = 0; p < 16; ++p) sc0[p * T + t] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
-      }
-#pragma unroll
-      for (int p = 0; p < 16; ++p) {
-        const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
-        cf T0, T1;
-        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
-        const cf u0 = cmul(dO[F::patch_off(2 * p, onx)], make_float2(ps.x, ps.y));
-        const cf u1 = cmul(dO[F::patch_off(2 * p + 1, onx)], make_float2(ps.z, ps.w));
-        num -= fmaf(v[2 * p].x, u0.x, v[2 * p].y * u0.y) + fmaf(v[2 * p + 1].x, u1.x, v[2 * p + 1].y * u1.y);
-        den = fmaf(u0.x, u0.x, fmaf(u0.y, u0.y, den));
-        den = fmaf(u1.x, u1.x, fmaf(u1.y, u1.y, den));
-        v[2 * p] = cmulc(v[2 * p], T0);
-        v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
-      }
-      if (i > 0) early(i - 1);
-      double acc[2] = {(double)num, (double)den};
-      block_sum<G::T, 2>(acc, red);
-      if (t == 0) {
-        double* sp = P.w.step_part + (size_t)unit * (2 * S + 6);
-        sp[2 * i] = acc[0]; sp[2 * i + 1] = acc[1];
-      }
-      if (i == 0) break;                                         // probe / position terms handled below
+    // ePIE (MODE 2): dO = conj(Psi) / max|Psi|^2 chi ; chi' = conj(T) / max|T|^2 chi
+    float s1 = 1.0f, s2 = 1.0f;
+    if (MODE == 2) {
+      float pm = 0.f;
+      for (int c = 0; c < CL; ++c) pm = fmaxf(pm, P.w.psimax[((size_t)pair * S + i) * CL + c]);
+      const float tm = P.w.tmax[(size_t)jl * S + i];
+      s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;   // a dead mode / an opaque window contributes nothing (R23b)
     }
+    float4* gt = (float4*)(P.w.gTpart + fld(spair, i));
+    float2* il = IL ? (float2*)(P.w.ilpart + fld(spair, i)) : nullptr;
+#pragma unroll
+    for (int p = 0; p < 16; ++p) {
+      const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+      cf T0, T1;
+      if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
+      else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+      if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
+      if (IL) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
+      __stcs(gt + p * T + t, make_float4(g0.x, g0.y, g1.x, g1.y));    // H10: gT_i contribution conj(Psi) .* gPhi
+      v[2 * p] = cmulc(v[2 * p], T0);                          //      gPsi = conj(T) .* gPhi
+      v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
+    }
+    if (i > 0) early(i - 1);
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(gPsi_i)  (Fourier layout)
     if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
   }
   const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
   const cf* ry = rx + NF;
   const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
-  if (MODE != 1) {
-    // v = G~ = F(gPsi_0).  H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
-    cf* gp = P.w.Gpart + ((size_t)pair * CL + rk) * NNS;
-    cf wxv[F::NXV];
-    load_xv<G>(wxv, rx, t, 1.0f);
-    float sy = 0.f, sx = 0.f;
+  // v = G~ = F(gPsi_0).  H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
+  cf* gp = P.w.Gpart + ((size_t)spair * CL + rk) * NNS;
+  cf wxv[F::NXV];
+  load_xv<G>(wxv, rx, t, 1.0f);
+  float sy = 0.f, sx = 0.f;
+#pragma unroll
+  for (int r = 0; r < 32; ++r) {
+    const int qy = F::fq_y(rk, t, r);
+    const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
+    gp[L::native(t, r)] = cmulc(v[r], R);
+    if (want_pos) {
+      const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);  // conj(G~) R P~
+      const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(rk, t, r), NF) / (float)NF;
+      sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
+    }
+  }
+  if (want_pos) {
+    double acc[2] = {(double)sy, (double)sx};
+    block_sum<G::T, 2>(acc, red);
+    if (t == 0) {
+      const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
+      P.w.posg_part[(size_t)unit * 2 + 0] = f * acc[0];
+      P.w.posg_part[(size_t)unit * 2 + 1] = f * acc[1];
+    }
+  }
+  Fft<G>::end_fourier();
+}
+
+// ------------------------------------------------------------------------------------------------
+// H14, LSQML-style step-size terms from what the gradient pass has staged.  With
+// chi_{i,k} = -c gPhi_{i,k} (c = KP::chi_scale) and u = dOhat|patch .* Psi_{i,k}:
+//   numO_i = sum_{k,r} Re(chi conj(u)) = -c Re sum_r conj(dOhat[r0 + r]) sum_k gT_{i,k}[r]        (gT = conj(Psi) gPhi, staged)
+//   denO_i = sum_{k,r} |u|^2          = sum_r |dOhat[r0 + r]|^2 sum_k |Psi_{i,k}[r]|^2            (|Psi|^2 staged)
+// i.e. the sums of the paper's formula in another order: no second pass through the FFT chain.  One block per (position of
+// the chunk, slice); fp64 sums in fixed order.  Bilinear mode (R1, R30): dOhat is sampled with the four taps, and the position
+// terms come through the patch: numX_a = -c Re sum_i sum_r conj(dT_i/df_a) gT_i, denX_a = sum_i sum_r |dT_i/df_a|^2 sum_k |Psi|^2.
+// ------------------------------------------------------------------------------------------------
+template <class G, bool BILIN>
+__global__ void __launch_bounds__(256) k_step_object(KP P) {
+  typedef Lay<G> L; typedef FL<G> F;
+  constexpr int NNS = F::NNS, T = G::T, CL = G::CL, NV = BILIN ? 6 : 2;
+  __shared__ double red[(256 / 32) * NV];
+  const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, sj = jl + P.js;
+  const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const size_t onx = P.onx;
+  const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x;
+  const cf* ob = P.object + ((size_t)i * P.ony + r0y) * onx + r0x;
+  float w00 = 1.f, w01 = 0.f, w10 = 0.f, w11 = 0.f, fy = 0.f, fx = 0.f;
+  if (BILIN) {
+    fy = P.w.delta[2 * jb]; fx = P.w.delta[2 * jb + 1];
+    w00 = (1.f - fy) * (1.f - fx); w01 = (1.f - fy) * fx; w10 = fy * (1.f - fx); w11 = fy * fx;
+  }
+  double acc[NV];
+#pragma unroll
+  for (int c = 0; c < NV; ++c) acc[c] = 0.0;
+  for (int e = threadIdx.x; e < CL * NNS; e += 256) {              // e: element of the field in storage order [rank][native]
+    const int rank = e / NNS, n = e - rank * NNS, m = n >> 1, t = m % T, r = ((m / T) << 1) | (n & 1);
+    const int y = F::pix_y(rank, t, r), x = F::pix_x(rank, t, r);
+    double gr = 0.0, gi = 0.0, il = 0.0;
+    const size_t gb = ((size_t)sj * P.Mg * P.S + i) * (CL * NNS) + e;
+    for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[gb + (size_t)k * P.S * (CL * NNS)]; gr += (double)g.x; gi += (double)g.y; }
+    const size_t ib = ((size_t)sj * P.M * P.S + i) * (CL * NNS) + e;
+    for (int k = 0; k < P.M; ++k) il += (double)P.w.ilpart[ib + (size_t)k * P.S * (CL * NNS)];
+    const size_t o = (size_t)y * onx + x;
+    double dr, di;
+    if (BILIN) {
+      const cf a = dO[o], b = dO[o + 1], c = dO[o + onx], d = dO[o + onx + 1];
+      dr = (double)(w00 * a.x + w01 * b.x + w10 * c.x + w11 * d.x); di = (double)(w00 * a.y + w01 * b.y + w10 * c.y + w11 * d.y);
+      const cf oa = ob[o], obb = ob[o + 1], oc = ob[o + onx], od = ob[o + onx + 1];
+      const double tyr = (1.0 - fx) * ((double)oc.x - oa.x) + fx * ((double)od.x - obb.x), tyi = (1.0 - fx) * ((double)oc.y - oa.y) + fx * ((double)od.y - obb.y);
+      const double txr = (1.0 - fy) * ((double)obb.x - oa.x) + fy * ((double)od.x - oc.x), txi = (1.0 - fy) * ((double)obb.y - oa.y) + fy * ((double)od.y - oc.y);
+      acc[2] -= tyr * gr + tyi * gi; acc[3] += (tyr * tyr + tyi * tyi) * il;
+      acc[4] -= txr * gr + txi * gi; acc[5] += (txr * txr + txi * txi) * il;
+    } else {
+      const cf d = dO[o];
+      dr = (double)d.x; di = (double)d.y;
+    }
+    acc[0] -= dr * gr + di * gi;                                    // -Re(conj(dOhat) gT)
+    acc[1] += (dr * dr + di * di) * il;
+  }
+  block_sum<256, NV>(acc, red);
+  if (threadIdx.x == 0) {
+    const double c = (double)P.chi_scale;
+    double* out = P.w.step_oi + ((size_t)jb * P.S + i) * 6;
+    out[0] = c * c * acc[0]; out[1] = c * c * acc[1];               // dOhat carries one factor c, chi the other
+#pragma unroll
+    for (int q = 2; q < 6; ++q) out[q] = 0.0;
+    if (BILIN) { out[2] = c * acc[2]; out[3] = acc[3]; out[4] = c * acc[4]; out[5] = acc[5]; }
+  }
+}
+
+// Probe and (Fourier-shift mode) position terms of the step-size sweep, one CTA (cluster) per (position of the chunk, mode).
+// With G~ = F(conj(T_0) gPhi_0) from the gradient pass (staged as Gpart = conj(R) G~) the numerators are dot products on the
+// Fourier side (Parseval):  numP = -c^2/N^2 Re sum_q conj(Q~_k) Gpart,  numX_a = c 2 pi / N^2 sum_q f_a Im(conj(P~_k) Gpart);
+// the denominators need the fields in real space: denP = c^2 sum_r |shift_j(dPhat_k) T_0|^2, denX_a = sum_r |dPsi_0/d delta_a T_0|^2
+// — three inverse transforms instead of a second pass through the 2S transforms of the chain.
+template <class G>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_step_probe(KP P) {
+  typedef Lay<G> L; typedef FL<G> F;
+  constexpr int NF = F::NF, NNS = F::NNS, CL = G::CL;
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int t = threadIdx.x;
+  const unsigned rk = Fft<G>::rank();
+  ChainSmem<G> cs(smem_raw, t);
+  cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
+  cs.fill_tables(t);
+  const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
+  const int spair = (jl + P.js) * P.M + k;
+  const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+  const int onx = P.bilinear ? NF : P.onx;
+  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * P.S * F::NNF : patch_ptr(P, 0, r0y, r0x)) +
+                 (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);          // T_0, this thread's first pixel
+  const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
+  const cf* ry = rx + NF;
+  const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
+  const cf* qt = P.w.Qt + ((size_t)k * CL + rk) * NNS;
+  const cf* gp = P.w.Gpart + ((size_t)spair * CL + rk) * NNS;
+  const double c = (double)P.chi_scale, inn = 1.0 / ((double)NF * (double)NF);
+  double* sp = P.w.step_pp + ((size_t)(jb * P.M + k) * CL + rk) * 6;
+  __syncthreads();
+  {   // numerators
+    float np = 0.f, ny = 0.f, nx = 0.f;
+#pragma unroll
+    for (int r = 0; r < 32; ++r) {
+      const cf g = gp[L::native(t, r)], q = qt[L::native(t, r)], pp = pt[L::native(t, r)];
+      np -= fmaf(q.x, g.x, q.y * g.y);                               // -Re(conj(Q~) Gpart)
+      const float im = fmaf(pp.x, g.y, -(pp.y * g.x));              // Im(conj(P~) Gpart)
+      ny = fmaf((float)signed_freq(F::fq_y(rk, t, r), NF) / (float)NF, im, ny);
+      nx = fmaf((float)signed_freq(F::fq_x(rk, t, r), NF) / (float)NF, im, nx);
+    }
+    double acc[3] = {(double)np, (double)ny, (double)nx};
+    block_sum<G::T, 3>(acc, red);
+    if (t == 0) { sp[0] = c * c * inn * acc[0]; sp[2] = c * 2.0 * CUDART_PI * inn * acc[1]; sp[4] = c * 2.0 * CUDART_PI * inn * acc[2]; }
+  }
+  cf wxv[F::NXV];
+  load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
+  const int nterm = P.bilinear ? 1 : 3;                             // bilinear mode: the position terms come from k_step_object
+  cf v[32];
+  for (int term = 0; term < nterm; ++term) {
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
       const int qy = F::fq_y(rk, t, r);
       const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
-      gp[L::native(t, r)] = cmulc(v[r], R);
-      if (want_pos) {
-        const cf z = cmulc(cmul(R, pt[L::native(t, r)]), v[r]);  // conj(G~) R P~
-        const float fy = (float)signed_freq(qy, NF) / (float)NF, fx = (float)signed_freq(F::fq_x(rk, t, r), NF) / (float)NF;
-        sy = fmaf(fy, z.y, sy); sx = fmaf(fx, z.y, sx);
+      if (term == 0) v[r] = cmul(R, qt[L::native(t, r)]);                       // shift_j(dPhat_k)
+      else {
+        const float f = (float)signed_freq(term == 1 ? qy : F::fq_x(rk, t, r), NF) / (float)NF;   // d Psi_0 / d delta_a
+        const cf z = cmul(R, pt[L::native(t, r)]);
+        const float g = -2.0f * CUDART_PI_F * f;
+        v[r] = make_float2(-g * z.y, g * z.x);                                  // (i g) z
       }
     }
-    if (want_pos) {
-      double acc[2] = {(double)sy, (double)sx};
-      block_sum<G::T, 2>(acc, red);
-      if (t == 0) {
-        const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
-        P.w.posg_part[(size_t)unit * 2 + 0] = f * acc[0];
-        P.w.posg_part[(size_t)unit * 2 + 1] = f * acc[1];
-      }
-    }
-    Fft<G>::end_fourier();
-  } else {
-    // H14 probe and position terms at slice 0 (O14): three more fields from the Fourier side, each
-    // compared with chi_0 = -gPhi_0 (kept in scratch) after multiplication by T_0.
-    const cf* sc0 = P.w.scratch + ((size_t)pair * CL + rk) * NNS;
-    const cf* qt = P.w.Qt + ((size_t)k * CL + rk) * NNS;
-    cf wxv[F::NXV];
-    load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
-    double* sp = P.w.step_part + (size_t)unit * (2 * S + 6) + 2 * S;
-    for (int term = 0; term < 3; ++term) {
+    Fft<G>::begin_fourier();
+    Fft<G>::inv(v, sm, tw, cs.tw2, t, rk);
+    float den = 0.f;
 #pragma unroll
-      for (int r = 0; r < 32; ++r) {
-        const int qy = F::fq_y(rk, t, r);
-        const cf R = cmul(wxv[F::fq_xsel(r)], ry[qy]);
-        if (term == 0) v[r] = cmul(R, qt[L::native(t, r)]);                       // shift_j(dPhat_k)
-        else {
-          const float f = (float)signed_freq(term == 1 ? qy : F::fq_x(rk, t, r), NF) / (float)NF;   // d Psi_0 / d delta_a
-          const cf z = cmul(R, pt[L::native(t, r)]);
-          const float g = -2.0f * CUDART_PI_F * f;
-          v[r] = make_float2(-g * z.y, g * z.x);                                  // (i g) z
-        }
-      }
-      Fft<G>::begin_fourier();
-      Fft<G>::inv(v, sm, tw, cs.tw2, t, rk);
-      float num = 0.f, den = 0.f;
-#pragma unroll
-      for (int r = 0; r < 32; ++r) {
-        const cf u = cmul(v[r], ob[F::patch_off(r, onx)]);
-        const cf g = sc0[L::native(t, r)];
-        num -= fmaf(g.x, u.x, g.y * u.y);
-        den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
-      }
-      double acc[2] = {(double)num, (double)den};
-      block_sum<G::T, 2>(acc, red);
-      if (t == 0) { sp[2 * term] = acc[0]; sp[2 * term + 1] = acc[1]; }
-      __syncthreads();
+    for (int r = 0; r < 32; ++r) {
+      const cf u = cmul(v[r], ob[F::patch_off(r, onx)]);
+      den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
     }
+    double acc[1] = {(double)den};
+    block_sum<G::T, 1>(acc, red);
+    if (t == 0) sp[2 * term + 1] = (term == 0 ? c * c : 1.0) * acc[0];
+    __syncthreads();
   }
+  if (t == 0 && P.bilinear) { sp[2] = 0.0; sp[3] = 0.0; sp[4] = 0.0; sp[5] = 0.0; }
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -874,6 +971,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   }
   const int MP = P.M >> 1, pp = blockIdx.x / CL, jl = pp / MP, kp = pp - jl * MP, jb = P.j0 + jl;
   const int pair0 = jl * P.M + 2 * kp;                                            // (position, mode) index of the pair's first mode
+  const int spair0 = (jl + P.js) * P.M + 2 * kp, spp = (jl + P.js) * MP + kp;     // the same pair in the staged arrays
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int S = P.S, onx = P.bilinear ? NF : P.onx;
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
@@ -886,6 +984,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     const float4* st = (const float4*)(P.w.stash + fld(pair0 + h, i)) + t;
 #pragma unroll
     for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+    if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);               // the late part of the same field: DRAM -> L2 now
     if (h == 0 && i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);   // serves both modes at slice i
     cp_async_commit();
   };
@@ -936,8 +1035,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       const float tm = P.w.tmax[(size_t)jl * S + i];
       s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;
     }
-    float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
-    float2* il = IL ? (float2*)(P.w.ilpart + fld(pr, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
+    float4* gt = (float4*)(P.w.gTpart + fld(spp, i));
+    float2* il = IL ? (float2*)(P.w.ilpart + fld(spair0 + h, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
       const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
@@ -973,7 +1072,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     }
     const int pr = pair0 + h, k = 2 * kp + h;
     const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
-    cf* gp = P.w.Gpart + ((size_t)pr * CL + rk) * NNS;
+    cf* gp = P.w.Gpart + ((size_t)(spair0 + h) * CL + rk) * NNS;
     cf wxv[F::NXV];
     load_xv<G>(wxv, rx, t, 1.0f);
     float sy = 0.f, sx = 0.f;
@@ -1069,7 +1168,7 @@ __global__ void __launch_bounds__(256) k_pos_bilinear(KP P, int cl) {
     const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
     for (int e = threadIdx.x; e < NN; e += 256) {
       const int y = e / N, x = e - y * N;
-      const size_t base = ((size_t)jl * P.Mg * P.S + i) * NN + F::r_native_of(y, x);
+      const size_t base = ((size_t)(jl + P.js) * P.Mg * P.S + i) * NN + F::r_native_of(y, x);
       double gr = 0.0, gi = 0.0;
       for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; gr += (double)g.x; gi += (double)g.y; }
       const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
@@ -1140,12 +1239,12 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
             if (ry < 0 || ry >= N || rx < 0 || rx >= N) continue;
             const double wgt = (dy ? fy : 1.0 - fy) * (dx ? fx : 1.0 - fx);
             const int nat = F::r_native_of(ry, rx);
-            const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + nat;
+            const size_t base = ((size_t)(jbase + jj + P.js) * P.Mg * P.S + i) * NN + nat;
             double sr = 0.0, si = 0.0, sl = 0.0;
             for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
             if (ILLUM) {
-              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat;
-              if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];
+              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat, sbs = sb + (size_t)P.js * P.M * P.S * NN;
+              if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
               else for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
             }
             ar += wgt * sr; ai += wgt * si; al += wgt * sl;
@@ -1153,11 +1252,11 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
         }
       } else if (px >= 0 && px < N && py >= 0 && py < N) {
         const int idx = F::r_native_of(py, px);
-        const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + idx;
+        const size_t base = ((size_t)(jbase + jj + P.js) * P.Mg * P.S + i) * NN + idx;
         for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
         if (ILLUM) {
-          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx;
-          if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];   // staged by k_backward_pair
+          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx, sbs = sb + (size_t)P.js * P.M * P.S * NN;
+          if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];   // staged by the backward kernel
           else for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
       }
@@ -1177,18 +1276,14 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
 // LSQML slice update with per-position step sizes (reading R24).
 // k_alpha_pos: alpha_{O,i,j} = numO[j,i] / (denO[j,i] + gamma) from the per-(mode, rank) fp64 partials of the sweep that
 // has just run over this chunk (fixed order).  k_gather_willum: W_i[r] += sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}[r - r0_j]|^2,
-// the same owner-computes gather as k_gather_object over the slice-wave stash (fixed (j, k) order, fp64).
+// the same owner-computes gather as k_gather_object over the staged |Psi|^2 (fixed (j, k) order, fp64).
 // ------------------------------------------------------------------------------------------------
-__global__ void k_alpha_pos(KP P, int cl, float gamma) {
+__global__ void k_alpha_pos(KP P, float gamma) {
   const int idx = blockIdx.x * blockDim.x + threadIdx.x;
   if (idx >= P.jc * P.S) return;
-  const int jl = idx / P.S, i = idx - jl * P.S, MU = P.M * cl, W = 2 * P.S + 6;
-  double num = 0.0, den = 0.0;
-  for (int u = 0; u < MU; ++u) {
-    const double* sp = P.w.step_part + ((size_t)(P.j0 + jl) * MU + u) * W;
-    num += sp[2 * i]; den += sp[2 * i + 1];
-  }
-  P.w.alpha_ji[idx] = (float)(num / (den + (double)gamma));
+  const int jl = idx / P.S, i = idx - jl * P.S;
+  const double* sp = P.w.step_oi + ((size_t)(P.j0 + jl) * P.S + i) * 6;
+  P.w.alpha_ji[idx] = (float)(sp[0] / (sp[1] + (double)gamma));
 }
 template <class G>
 __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
@@ -1221,9 +1316,9 @@ __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
         const int2 r0 = sr0[jj];
         const int px = ox - r0.x, py = oy - r0.y;
         if (px >= 0 && px < N && py >= 0 && py < N) {
-          const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
+          const size_t base = ((size_t)(jbase + jj + P.js) * P.M * P.S + i) * NN + F::r_native_of(py, px);
           double s = 0.0;
-          for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[base + (size_t)k * P.S * NN]; s += (double)q.x * q.x + (double)q.y * q.y; }
+          for (int k = 0; k < P.M; ++k) s += (double)P.w.ilpart[base + (size_t)k * P.S * NN];      // |Psi_{i,k}|^2 staged by the backward kernel
           acc += (double)sal[jj] * s;
         }
       }
@@ -1280,7 +1375,7 @@ __global__ void k_reduce_probe(KP P) {
   if (e >= NN) return;
   double ar = 0.0, ai = 0.0;
   for (int jl = 0; jl < P.jc; ++jl) {
-    const cf g = P.w.Gpart[(size_t)(jl * P.M + k) * NN + e];
+    const cf g = P.w.Gpart[(size_t)((jl + P.js) * P.M + k) * NN + e];
     ar += (double)g.x; ai += (double)g.y;
   }
   double2 a = P.w.gPt_acc[(size_t)k * NN + e];
@@ -1312,11 +1407,15 @@ __global__ void k_finalize(KP P, int cl, double* loss, int accumulate, float* lo
       grad_pos[2 * j + 1] = (float)(sx / (double)P.px);
     }
   if (step_terms) {
+    // object terms per (position, slice); probe terms summed over the modes (and ranks); position terms likewise, or (bilinear
+    // mode, where they come through the patch) summed over the slices
     const int W = 2 * P.S + 6;
     for (int idx = t; idx < P.J * W; idx += 1024) {
       const int j = idx / W, c = idx - j * W;
       double s = 0.0;
-      for (int k = 0; k < MU; ++k) s += P.w.step_part[((size_t)j * MU + k) * W + c];
+      if (c < 2 * P.S) s = P.w.step_oi[((size_t)j * P.S + (c >> 1)) * 6 + (c & 1)];
+      else if (c >= 2 * P.S + 2 && P.bilinear) for (int i = 0; i < P.S; ++i) s += P.w.step_oi[((size_t)j * P.S + i) * 6 + (c - 2 * P.S)];
+      else for (int k = 0; k < MU; ++k) s += P.w.step_pp[((size_t)j * MU + k) * 6 + (c - 2 * P.S)];
       step_terms[idx] = (float)s;
     }
   }
@@ -1401,11 +1500,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_regularizer, K_constraint, K_adam, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_regularizer, K_constraint, K_adam, K_step_object, K_step_probe, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam", "k_step_object", "k_step_probe"};
 
 inline void prof_mark(int kind, cudaStream_t st) {
   if (!g_prof_on) return;
@@ -1441,7 +1540,8 @@ KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64*
            const float* intensity, const int32_t* batch_idx) {
   KP k;
   k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch; k.Jtot = p->n_pos_total;
-  k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
+  k.j0 = 0; k.jc = 0; k.js = 0; k.px = p->pixel_size;
+  k.chi_scale = (p->flags & PT_LSQML_MODULUS_CHI) ? 2.0f : 1.0f;
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
   k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
   k.loss = p->loss; k.loss_c = p->loss_c; k.eps = p->eps;
@@ -1471,9 +1571,9 @@ int set_smem_attrs_now() {
   bool ok = true;
   auto set = [&](const void* f, int bytes) { ok = ok && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess; };
   set((const void*)k_forward<G, true>, c); set((const void*)k_forward<G, false>, c);
-  set((const void*)k_backward<G, 0>, c); set((const void*)k_backward<G, 1>, c); set((const void*)k_backward<G, 2>, c);
+  set((const void*)k_backward<G, 0, false>, c); set((const void*)k_backward<G, 0, true>, c); set((const void*)k_backward<G, 2, false>, c);
   set((const void*)k_backward_pair<G, 0, false>, c); set((const void*)k_backward_pair<G, 0, true>, c); set((const void*)k_backward_pair<G, 2, false>, c);
-  set((const void*)k_probe_fft<G>, b); set((const void*)k_probe_ifft<G>, b);
+  set((const void*)k_probe_fft<G>, b); set((const void*)k_probe_ifft<G>, b); set((const void*)k_step_probe<G>, b);
   return ok ? PT_OK : PT_ERR_CUDA;
 }
 template <class G>
@@ -1547,6 +1647,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool epie = (p->flags & PT_EPIE) != 0;
   // two modes per CTA (cluster), their patch gradients summed on chip (k_backward_pair): needs an even number of modes
   const bool paired = use_pairs(p);
+  const bool stage_il = kp.w.ilpart != nullptr && !epie;            // |Psi|^2 staged by the backward kernel (step sizes; illumination map)
   kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
@@ -1556,28 +1657,36 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, want_w ? 2 * on : on); LAUNCH_CHECK(K_zero, st); }
   }
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
-  for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
-    kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+  // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
+  auto chains = [&](bool wait_patterns) -> int {
     if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
-    if (chunk_ready && cudaStreamWaitEvent(st, chunk_ready[j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
+    if (wait_patterns && chunk_ready && cudaStreamWaitEvent(st, chunk_ready[kp.j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
     LAUNCH_CHECK(K_loss, st);
+    const int wp = want_pos && !bilin ? 1 : 0;
     if (epie) {
       k_patch_max<<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
       if (paired) launch_fft<G>(k_backward_pair<G, 2, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
-      else launch_fft<G>(k_backward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      else launch_fft<G>(k_backward<G, 2, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+    } else if (paired) {
+      if (stage_il) launch_fft<G>(k_backward_pair<G, 0, true>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, wp);
+      else launch_fft<G>(k_backward_pair<G, 0, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, wp);
     } else {
-      if (paired && want_illum && kp.w.ilpart)
-        launch_fft<G>(k_backward_pair<G, 0, true>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
-      else if (paired) launch_fft<G>(k_backward_pair<G, 0, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
-      else launch_fft<G>(k_backward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, want_pos && !bilin ? 1 : 0);
+      if (stage_il) launch_fft<G>(k_backward<G, 0, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, wp);
+      else launch_fft<G>(k_backward<G, 0, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, wp);
     }
     LAUNCH_CHECK(K_backward, st);
+    return PT_OK;
+  };
+  for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
+    kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
+    kp.js = kp.w.stage_all ? j0 : 0;
+    if ((rc = chains(true)) != PT_OK) return rc;
     if (bilin) {
       if (want_illum) k_gather_object<G, true, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
       else k_gather_object<G, false, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, nullptr);
@@ -1597,24 +1706,25 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
                 epie ? 1.0 / (double)p->n_batch : 1.0);                         // ePIE: probe direction averaged over the group
   LAUNCH_CHECK(K_probe_ifft, st);
   if (want_steps) {
-    // H14 second sweep (O13/O14): needs the batch-aggregated gO, gP
+    // H14 (O13/O14): needs the batch-aggregated gO, gP, and what the backward pass staged for every position of the batch
     k_dohat<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((const cf*)gO, illum_prev, p->lsqml_delta_o, kp.w.dOhat, on);
     LAUNCH_CHECK(K_dohat, st);
     launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const cf*)gP, kp.w.Qt, -1.0f / (p->lsqml_delta_p + 1.0f),
                p->lsqml_probe_precond_d, p->lsqml_delta_p);
     LAUNCH_CHECK(K_probe_fft, st);
+    const bool recompute = kp.w.Jc < p->n_batch && !kp.w.stage_all;      // the staged arrays hold the last chunk only
     for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-      if (kp.w.Jc < p->n_batch) {   // stash of this chunk was overwritten: recompute it
-        launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
-        LAUNCH_CHECK(K_forward, st);
-        k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
-        LAUNCH_CHECK(K_loss, st);
-      }
-      launch_fft<G>(k_backward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
-      LAUNCH_CHECK(K_backward, st);
+      kp.js = kp.w.stage_all ? j0 : 0;
+      if (recompute) { if ((rc = chains(false)) != PT_OK) return rc; }
+      else if (bilin && kp.w.Jc < p->n_batch) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
+      if (bilin) k_step_object<G, true><<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
+      else k_step_object<G, false><<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
+      LAUNCH_CHECK(K_step_object, st);
+      launch_fft<G>(k_step_probe<G>, kp.jc * p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp);
+      LAUNCH_CHECK(K_step_probe, st);
       if (want_w) {   // PAPER.md:225 with per-position step sizes (R24): W += sum_j alpha_{O,i,j} sum_k |Psi_{i,k,j}|^2
-        k_alpha_pos<<<(kp.jc * p->n_slices + 255) / 256, 256, 0, st>>>(kp, G::CL, p->lsqml_gamma);
+        k_alpha_pos<<<(kp.jc * p->n_slices + 255) / 256, 256, 0, st>>>(kp, p->lsqml_gamma);
         LAUNCH_CHECK(K_alpha_pos, st);
         k_gather_willum<G><<<ggrid, gblock, 0, st>>>(kp, illum + on);
         LAUNCH_CHECK(K_gather_willum, st);
@@ -1669,9 +1779,11 @@ int32_t gradient_impl(const pt_problem* p, const pt_c64* object_d, const pt_c64*
   if (rc != PT_OK) return rc;
   if (!object_d || !probe_d || !positions_d || !intensity_d || !grad_object_d || !grad_probe_d || !workspace_d) return PT_ERR_NULL;
   if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && !illum_prev_d) return PT_ERR_NULL;
-  if ((p->flags & PT_WANT_STEP_SIZES) && step_terms_d && p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;
+  // PT_LSQML_MODULUS_CHI: the wavefront update of PAPER.md:173 is given for the amplitude model only
+  if ((p->flags & PT_LSQML_MODULUS_CHI) && p->loss != PT_LOSS_AMPLITUDE) return PT_ERR_UNSUPPORTED;
   if (p->flags & PT_WANT_WEIGHTED_ILLUM) {
     if (!(p->flags & PT_WANT_ILLUM) || !(p->flags & PT_WANT_STEP_SIZES) || (p->flags & PT_EPIE)) return PT_ERR_BAD_PARAM;
+    if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) return PT_ERR_UNSUPPORTED;   // the weighted map is gathered over integer windows
     if (!illum_d || !step_terms_d) return PT_ERR_NULL;
     if (!(p->lsqml_gamma >= 0.f)) return PT_ERR_BAD_PARAM;
   }
@@ -1722,8 +1834,8 @@ extern "C" {
 
 size_t ptycho_workspace_min_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
-  size_t f, pp; ws_sizes(p, &f, &pp);
-  return f + pp;
+  const WsSizes z = ws_sizes(p);
+  return z.fixed + z.per_chunk + z.per_staged + (z.il_needed ? z.per_il : 0);
 }
 
 int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) {
@@ -1733,21 +1845,32 @@ int32_t ptycho_positions_in_flight(const pt_problem* p, size_t workspace_bytes) 
 
 size_t ptycho_workspace_bytes(const pt_problem* p) {
   if (validate(p) != PT_OK) return 0;
-  size_t f, pp; ws_sizes(p, &f, &pp);
-  pp += il_bytes_per_pos(p);             // the recommendation includes the optional staging of the illumination map
+  const WsSizes z = ws_sizes(p);
+  const size_t pp = z.per_chunk + z.per_staged + z.per_il;   // the recommendation includes the optional staging of the illumination map
   const size_t cap = (size_t)49 << 30;   // config 3: 1554 positions = 84 / 42 whole waves of forward / paired-backward CTAs
-  size_t jc = p->n_batch;
-  if (f + jc * pp > cap) {
-    jc = (cap - f) / pp;
-    // whole waves of 148 CTAs per chunk where possible
-    const size_t wave = 148;
-    // (the paired backward kernel launches half as many CTAs: keep that count a whole number of waves too)
-    const size_t per_pos_ctas = staged_planes(p) * cluster_of(p->n);
+  const size_t J = p->n_batch;
+  if (z.fixed + J * pp <= cap) return z.fixed + J * pp;
+  // whole waves of 148 CTAs per chunk where possible (the paired backward kernel launches half as many CTAs: keep that count a
+  // whole number of waves too)
+  auto whole_waves = [&](size_t jc) {
+    const size_t wave = 148, per_pos_ctas = staged_planes(p) * cluster_of(p->n);
     size_t pairs = jc * per_pos_ctas;
     if (pairs > wave) { pairs -= pairs % wave; jc = pairs / per_pos_ctas; }
-    if (jc < 1) jc = 1;
+    return jc < 1 ? (size_t)1 : jc;
+  };
+  if (z.il_needed) {
+    // step sizes: what the backward pass stages is kept for the WHOLE batch (the sweep then needs no second pass through the
+    // chain) as long as the total stays below 150 GiB; the positions in flight get the usual 49 GiB on top
+    const size_t staged = J * (z.per_staged + z.per_il), big = (size_t)150 << 30;
+    if (z.fixed + staged < big) {
+      size_t jc = whole_waves(cap / pp);
+      if (jc > J) jc = J;
+      size_t room = big - z.fixed - staged;
+      if (jc * z.per_chunk > room) jc = room / z.per_chunk;
+      if (jc >= (J < 64 ? J : 64)) return z.fixed + staged + jc * z.per_chunk;
+    }
   }
-  return f + jc * pp;
+  return z.fixed + whole_waves((cap - z.fixed) / pp) * pp;
 }
 
 int32_t ptycho_forward_loss(const pt_problem* p, const pt_c64* object_d, const pt_c64* probe_d, const float* positions_d,
@@ -1801,6 +1924,9 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
   if (!step_terms_d || !workspace_d) return PT_ERR_NULL;
   if (workspace_bytes < 256 + (size_t)(p->n_slices + 1) * sizeof(float)) return PT_ERR_WORKSPACE;
   float* alpha = (float*)((char*)workspace_d + 256);
+  // under PT_LSQML_MODULUS_CHI (R31) the update directions dOhat, dPhat carry the factor 2 of chi = -2 gPhi
+  const float cs = (p->flags & PT_LSQML_MODULUS_CHI) ? 2.0f : 1.0f;
+  if ((p->flags & PT_LSQML_MODULUS_CHI) && p->loss != PT_LOSS_AMPLITUDE) return PT_ERR_UNSUPPORTED;
   k_lsqml_alpha<<<p->n_slices + 1, 256, 0, st>>>(step_terms_d, p->n_batch, p->n_slices, u->gamma, alpha);
   LAUNCH_CHECK(K_lsqml_alpha, st);
   if (object_d && grad_object_d) {
@@ -1808,13 +1934,13 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
     if (u->mode == PT_UPDATE_LSQML_WEIGHTED) {
       if (!u->illum_batch_d) return PT_ERR_NULL;
       k_lsqml_object_weighted<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, u->illum_batch_d,
-                                                                           u->illum_batch_d + on, u->beta_obj, p->lsqml_delta_o, on);
+                                                                           u->illum_batch_d + on, cs * u->beta_obj, p->lsqml_delta_o, on);
     } else
-    k_lsqml_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, alpha, u->beta_obj, p->lsqml_delta_o, os, on);
+    k_lsqml_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>((cf*)object_d, (const cf*)grad_object_d, illum_prev_d, alpha, cs * u->beta_obj, p->lsqml_delta_o, os, on);
     LAUNCH_CHECK(K_lsqml_object, st);
   }
   if (probe_d && grad_probe_d) {
-    k_lsqml_probe<<<(unsigned)((pn + 255) / 256), 256, 0, st>>>((cf*)probe_d, (const cf*)grad_probe_d, alpha, p->n_slices, u->beta_probe, p->lsqml_delta_p, p->lsqml_probe_precond_d, NN, pn);
+    k_lsqml_probe<<<(unsigned)((pn + 255) / 256), 256, 0, st>>>((cf*)probe_d, (const cf*)grad_probe_d, alpha, p->n_slices, cs * u->beta_probe, p->lsqml_delta_p, p->lsqml_probe_precond_d, NN, pn);
     LAUNCH_CHECK(K_lsqml_probe, st);
   }
   if (positions_d) {

@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libptycho_b200.so")
 
 LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
-WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLUM, NO_MODE_PAIRS = 1, 2, 4, 16, 32, 64, 128
+WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLUM, NO_MODE_PAIRS, LSQML_MODULUS_CHI = 1, 2, 4, 16, 32, 64, 128, 256
 UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE, UPDATE_LSQML_WEIGHTED = 0, 1, 2, 3
 OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",
@@ -223,12 +223,12 @@ def gradient(pb: Problem, obj, probe, positions, intensity, batch_idx=None, *, w
 
 def apply_update(pb: Problem, obj=None, probe=None, positions=None, *, grad_object=None, grad_probe=None, grad_pos=None,
                  illum_prev=None, step_terms=None, batch_idx=None, n_batch: Optional[int] = None, mode=UPDATE_SGD,
-                 lr_obj=0.0, lr_probe=0.0, lr_pos=0.0, beta_obj=1.0, beta_probe=1.0, gamma=0.0, workspace=None, illum_batch=None):
+                 lr_obj=0.0, lr_probe=0.0, lr_pos=0.0, beta_obj=1.0, beta_probe=1.0, gamma=0.0, workspace=None, illum_batch=None, flags: int = 0):
     """ptycho_apply_update (in place). illum_batch: the [2][S][ny][nx] (I, W) planes of WANT_WEIGHTED_ILLUM (UPDATE_LSQML_WEIGHTED)."""
     import torch
     npos = positions.shape[0] if positions is not None else (n_batch or 1)
     J = batch_idx.numel() if batch_idx is not None else (n_batch if n_batch is not None else npos)
-    cs = pb.c_struct(max(npos, J), J, 0)
+    cs = pb.c_struct(max(npos, J), J, flags)
     ib = _dev(illum_batch, torch.float32, "illum_batch")
     u = PtUpdate(mode, lr_obj, lr_probe, lr_pos, beta_obj, beta_probe, gamma, None if ib is None else ib.data_ptr())
     _check(lib().ptycho_apply_update(C.byref(cs), _ptr(_dev(obj, torch.complex64, "obj")), _ptr(_dev(probe, torch.complex64, "probe")),

@@ -540,22 +540,43 @@ def test_bilinear_mode(which):
     g = gpu_gradient(case, pbg, want_illum=True, max_ws=max_ws)
     check(g, o, pos=True, px=cfg.pixel_size)
     margin("g['illum']", rel_l2(g["illum"], o["illum"]), TOL_GRAD)
-    # step sizes are not built for this mode: the call says so instead of computing something else
+    # LSQML step-size terms in this mode (reading R30) and the update built on them, against the oracle; config 3 chunked
+    # (the staged arrays then hold the whole batch, or each chunk is recomputed, depending on the cap)
     import torch
-    st = torch.zeros((cfg.n_pos, 2 * cfg.n_slices + 6), dtype=torch.float32, device="cuda")
-    with pytest.raises(ptycho.PtychoError):
-        gpu_gradient_raw_steps(case, pbg, st)
-
-
-def gpu_gradient_raw_steps(case, pbg, st):
-    import torch
-    from paper_2505_14372_b200 import ptycho
-    cfg = case.cfg
-    obj_d, pr_d, pos_d, I_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity)
-    gO, gP = torch.empty_like(obj_d), torch.empty_like(pr_d)
-    ill = torch.ones(obj_d.shape, dtype=torch.float32, device="cuda")
-    ws = ptycho.make_workspace(pbg, cfg.n_pos, cfg.n_pos, ptycho.WANT_STEP_SIZES)
-    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, illum_prev=ill, step_terms=st)
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbo2 = oracle_problem(cfg, shift_mode=orc.SHIFT_BILINEAR_OBJECT, **kw)
+    pbg2 = gpu_problem(cfg, shift_mode=ptycho.SHIFT_BILINEAR_OBJECT, **kw)
+    J, S = cfg.n_pos, cfg.n_slices
+    illum_prev = (o["illum"] * 0.9 + 1.0).astype(np.float32)
+    st_o = orc.step_terms(pbo2, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev)
+    fl = ptycho.WANT_POS_GRAD | ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES
+    caps = [None]
+    if which == "cfg3":
+        lo = ptycho.workspace_bytes(pbg2, J, J, fl, minimum=True); hi = ptycho.workspace_bytes(pbg2, J, J, fl)
+        caps = [None, lo + (hi - lo) * 6 // 19 + 4096, hi - (hi - lo) // 4]     # one chunk / recompute per chunk / staged for the whole batch
+    for cap in caps:
+        obj_d, pr_d, pos_d, I_d, ip_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity), _t(illum_prev)
+        gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d); gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
+        il = torch.empty(obj_d.shape, dtype=torch.float32, device="cuda")
+        st = torch.full((J, 2 * S + 6), float("nan"), dtype=torch.float32, device="cuda")
+        ws = ptycho.make_workspace(pbg2, J, J, fl, max_bytes=cap)
+        if cap is not None:
+            assert ptycho.positions_in_flight(pbg2, J, J, fl, ws.numel()) < J
+        ptycho.gradient(pbg2, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum=il,
+                        illum_prev=ip_d, step_terms=st)
+        assert ptycho.status(ws) == 0
+        margin("gO with steps", rel_l2(gO.cpu().numpy(), o["grad_object"]), TOL_GRAD)
+        stg = st.cpu().numpy().astype(np.float64)
+        for c in range(2 * S + 6):
+            margin(f"bilinear step term column {c}", rel_l2(stg[:, c], st_o[:, c]), TOL_STEP)
+    o_new, p_new, x_new = orc.apply_update(pbo2, 1, case.obj_start, case.probe, case.positions, o["grad_object"], o["grad_probe"],
+                                           None, illum_prev, st_o, beta_obj=0.9, beta_probe=0.8, gamma=1e-3)
+    ptycho.apply_update(pbg2, obj_d, pr_d, pos_d, grad_object=gO, grad_probe=gP, illum_prev=ip_d, step_terms=st,
+                        mode=ptycho.UPDATE_LSQML, beta_obj=0.9, beta_probe=0.8, gamma=1e-3, workspace=ws)
+    torch.cuda.synchronize()
+    margin("object update", rel_l2(obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start), TOL_STEP)
+    margin("probe update", rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe), TOL_STEP)
+    margin("position update", rel_l2(pos_d.cpu().numpy() - case.positions, x_new - case.positions), TOL_POS_UPDATE)
 
 
 # ------------------------------------------------------------------------------------------------
@@ -1236,3 +1257,44 @@ def test_epie_dead_mode_contributes_nothing():
     check_array("epie object direction", g["grad_object"], o["dir_object"])
     check_array("epie probe direction", g["grad_probe"][:1], o["dir_probe"][:1])
     assert not g["grad_probe"][1].any() and not o["dir_probe"][1].any()
+
+
+
+# ------------------------------------------------------------------------------------------------
+# PT_LSQML_MODULUS_CHI (reading R31): LSQML driven by the modulus-constraint wavefront update of PAPER.md:173
+# ------------------------------------------------------------------------------------------------
+def test_lsqml_modulus_constraint_chi():
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(5, scan=(4, 5), n_modes=4, n_slices=6, loss=synth.LOSS_AMPLITUDE, loss_c=0.0, eps=0.5)
+    case = make_case(cfg, start_scale=0.8)
+    kw = dict(lsqml_delta_o=50.0, lsqml_delta_p=0.5)
+    pbo, pbg = oracle_problem(cfg, lsqml_chi_scale=2.0, **kw), gpu_problem(cfg, **kw)
+    o = orc.gradient(pbo, case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    illum_prev = (o["illum"] * 0.9).astype(np.float32)
+    J, S = cfg.n_pos, cfg.n_slices
+    st_o = orc.step_terms(pbo, case.obj_start, case.probe, case.positions, case.intensity, o["grad_object"], o["grad_probe"], illum_prev)
+    obj_d, pr_d, pos_d, I_d, ip_d = _t(case.obj_start), _t(case.probe), _t(case.positions), _t(case.intensity), _t(illum_prev)
+    gO = torch.empty_like(obj_d); gP = torch.empty_like(pr_d); gX = torch.empty((J, 2), dtype=torch.float32, device="cuda")
+    st = torch.empty((J, 2 * S + 6), dtype=torch.float32, device="cuda")
+    fl = ptycho.WANT_POS_GRAD | ptycho.WANT_STEP_SIZES | ptycho.LSQML_MODULUS_CHI
+    ws = ptycho.make_workspace(pbg, J, J, fl)
+    ptycho.gradient(pbg, obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, illum_prev=ip_d,
+                    step_terms=st, flags=fl)
+    assert ptycho.status(ws) == 0
+    stg = st.cpu().numpy().astype(np.float64)
+    for c in range(2 * S + 6):
+        margin(f"step term column {c}", rel_l2(stg[:, c], st_o[:, c]), TOL_STEP)
+    o_new, p_new, x_new = orc.apply_update(pbo, 1, case.obj_start, case.probe, case.positions, o["grad_object"], o["grad_probe"],
+                                           None, illum_prev, st_o, beta_obj=0.9, beta_probe=0.8, gamma=1e-3)
+    ptycho.apply_update(pbg, obj_d, pr_d, pos_d, grad_object=gO, grad_probe=gP, illum_prev=ip_d, step_terms=st,
+                        mode=ptycho.UPDATE_LSQML, beta_obj=0.9, beta_probe=0.8, gamma=1e-3, workspace=ws, flags=ptycho.LSQML_MODULUS_CHI)
+    torch.cuda.synchronize()
+    margin("object update", rel_l2(obj_d.cpu().numpy() - case.obj_start, o_new - case.obj_start), TOL_STEP)
+    margin("probe update", rel_l2(pr_d.cpu().numpy() - case.probe, p_new - case.probe), TOL_STEP)
+    margin("position update", rel_l2(pos_d.cpu().numpy() - case.positions, x_new - case.positions), TOL_POS_UPDATE)
+    # the paper gives that wavefront update for the amplitude model only
+    with pytest.raises(ptycho.PtychoError) as e:
+        ptycho.gradient(gpu_problem(cfg, loss=synth.LOSS_POISSON, eps=0.8, **kw), obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO,
+                        grad_probe=gP, illum_prev=ip_d, step_terms=st, flags=fl)
+    assert e.value.code == -8
