@@ -44,6 +44,8 @@ def parse():
     ap.add_argument("--bandlimit", type=float, default=0.0, help="timed variant: sharp band-limit mask at this fraction of Nyquist "
                     "inside the propagator (PAPER.md:117, reading R9); 0 = off, as in BASELINE.json's configs")
     ap.add_argument("--ws-gib", type=float, default=0.0, help="cap of the device workspace in GiB (0: library default)")
+    ap.add_argument("--stash-fp16", action="store_true", help="timed variant: PT_STASH_FP16, the slice-wave stash stored as binary16 "
+                    "pairs (SURVEY 8(f) rank 4; grad_object then within 7.5e-5 of the oracle instead of 3.4e-5, DESIGN.md 10)")
     ap.add_argument("--no-secondary", action="store_true", help="config 3 only: skip the short runs of the other configurations")
     return ap.parse_args()
 
@@ -216,6 +218,11 @@ def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit
         mb = batch or 1024
     batches = None if mb is None else [torch.from_numpy(b).cuda() for b in _synth.batches(cfg, mb)]
     fl = ptycho.WANT_POS_GRAD | ((ptycho.WANT_ILLUM | ptycho.WANT_STEP_SIZES) if lsqml else 0)
+    xfl = ptycho.STASH_FP16 if args.stash_fp16 else 0
+    fl |= xfl
+    if xfl:
+        conf.update(variant="PT_STASH_FP16: slice-wave stash stored as binary16 pairs")
+        want_e2e = False
     ws = ptycho.make_workspace(pbg, J, J if lsqml else (mb or J), fl, max_bytes=cap)
     if batches is not None and not lsqml:
         conf.update(minibatch=mb, grouping="seeded permutation (sparse), gradients accumulated over the batches, one update")
@@ -234,7 +241,7 @@ def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit
         for b in bl:
             nb = b.numel()
             ptycho.gradient(pbg, obj, pr, pos, inten, b, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX[:nb], illum=illum,
-                            illum_prev=illum_prev, step_terms=st_terms[:nb], loss=loss)
+                            illum_prev=illum_prev, step_terms=st_terms[:nb], loss=loss, flags=xfl)
             ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, illum_prev=illum_prev, step_terms=st_terms[:nb],
                                 batch_idx=b, workspace=ws, **LS)
 
@@ -246,12 +253,12 @@ def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit
         if lsqml:
             return lsqml_iteration(batches)
         if batches is None:
-            ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
+            ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss, flags=xfl)
         else:
             o = 0
             for i, b in enumerate(batches):
                 ptycho.gradient(pbg, obj, pr, pos, inten, b, workspace=ws, grad_object=gO, grad_probe=gP,
-                                grad_pos=gX[o:o + b.numel()], loss=loss, flags=ptycho.ACCUMULATE if i else 0)
+                                grad_pos=gX[o:o + b.numel()], loss=loss, flags=(ptycho.ACCUMULATE if i else 0) | xfl)
                 o += b.numel()
         if dist is not None:
             shard.allreduce_sums(dist, gO, gP, loss)
@@ -449,7 +456,7 @@ def run_b200(args):
     r = measure(args, args.config, steps=args.steps, warmup=args.warmup, bandlimit=args.bandlimit, batch=args.batch,
                 want_e2e=not args.no_e2e, want_cpu=not args.no_cpu_baseline, **common)
     secondary = None
-    if args.config == 3 and not args.bandlimit and not args.no_secondary and world == 1:
+    if args.config == 3 and not args.bandlimit and not args.no_secondary and not args.stash_fp16 and world == 1:
         # the other configurations of BASELINE.json and the band-limited variant, short runs (1 warm-up + >= 2 timed steps,
         # at least one second of timed region each), device-resident only
         secondary = {}

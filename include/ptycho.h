@@ -58,6 +58,15 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
                                        * of the steepest-descent chi = -gPhi (R20): numerators and denominators of the object and probe
                                        * terms x4, position numerators x2, update directions x2.  PT_LOSS_AMPLITUDE only (the paper gives
                                        * that update for the amplitude model), else PT_ERR_UNSUPPORTED                          */
+       PT_STASH_FP16 = 512,           /* SURVEY 8(f) rank 4 (PAPER.md:79-81 names reduced precision as future work): the slice waves Psi_{i,k}
+                                       * kept for the adjoint are STORED as binary16 pairs (round to nearest even; all arithmetic stays
+                                       * float32): half the stash traffic and memory (1.45x the positions in flight).  grad_probe, grad_pos
+                                       * and the loss do not read the stash and are unchanged bit for bit; grad_object, illum_d and the
+                                       * object step-size terms are formed from the rounded waves: measured 2e-5 .. 1.01e-4 relative L2 from
+                                       * the oracle over the parity cases (float32 stash: <= 3.4e-5), i.e. AT the 1e-4 bar, not inside it
+                                       * everywhere.  Off by default.
+                                       * ptycho_gradient only; not with PT_EPIE, and PT_WANT_ILLUM needs an even mode count or
+                                       * PT_WANT_STEP_SIZES (the map comes from the backward kernel's staging): else PT_ERR_UNSUPPORTED */
        PT_NO_MODE_PAIRS = 128,        /* debugging aid: the backward pass runs one mode per CTA even when the mode count is even
                                        * (no tensor-memory allocation); results differ only by the rounding of one float32 add */
        PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of

@@ -130,7 +130,8 @@ WsSizes ws_sizes(const pt_problem* p) {
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
   WsSizes z;
   z.fixed = f + 13 * 256;   // slack for the per-array alignment of the chunked part
-  z.per_chunk = M * NN * sizeof(cf) + NN * sizeof(float) + M * S * NN * sizeof(cf);
+  const size_t stash_el = (p->flags & PT_STASH_FP16) ? sizeof(cf) / 2 : sizeof(cf);   // binary16 pairs: 4 bytes per complex
+  z.per_chunk = M * NN * sizeof(cf) + NN * sizeof(float) + M * S * NN * stash_el;
   if (steps) z.per_chunk += S * sizeof(float);
   if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) z.per_chunk += S * NN * sizeof(cf);
   if (p->flags & PT_EPIE) z.per_chunk += (M * CL + 1) * S * sizeof(float) + 64;
@@ -204,7 +205,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->dOhat = steps ? (cf*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf)) : nullptr;
   w->psit = (cf*)take(jc * M * NN * sizeof(cf));
   w->wdet = (float*)take(jc * NN * sizeof(float));
-  w->stash = (cf*)take(jc * M * S * NN * sizeof(cf));
+  w->stash = (cf*)take(jc * M * S * NN * ((p->flags & PT_STASH_FP16) ? sizeof(cf) / 2 : sizeof(cf)));
   w->gTpart = (cf*)take(js * staged_planes(p) * S * NN * sizeof(cf));
   w->Gpart = (cf*)take(js * M * NN * sizeof(cf));
   w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
@@ -375,6 +376,15 @@ __device__ __forceinline__ cf ld_nc8(const cf* p) {
   asm volatile("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
   return v;
 }
+// reduced-precision stash (PT_STASH_FP16): four complex64 <-> eight binary16 in one 16-byte word, round to nearest even
+__device__ __forceinline__ uint32_t pack_h2(float a, float b) {
+  uint32_t r; asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a)); return r;     // low half = a
+}
+__device__ __forceinline__ cf unpack_h2(uint32_t u) {
+  float lo, hi;
+  asm("{.reg .f16 l, h; mov.b32 {l, h}, %2; cvt.f32.f16 %0, l; cvt.f32.f16 %1, h;}" : "=f"(lo), "=f"(hi) : "r"(u));
+  return make_float2(lo, hi);
+}
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
 // ------------------------------------------------------------------------------------------------
@@ -513,7 +523,7 @@ __device__ __forceinline__ void apply_prop_t(cf (&v)[32], const cf* hxrow, const
 // ------------------------------------------------------------------------------------------------
 // H2..H6 forward: one CTA (CL = 4: one cluster of four) per (j,k) pair of the chunk
 // ------------------------------------------------------------------------------------------------
-template <class G, bool STASH>
+template <class G, int STASH>   // 0: nothing stashed (forward only); 1: Psi_i stashed as complex64; 2: as binary16 pairs (PT_STASH_FP16)
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL;     // E pair slots early, 16 - E late
@@ -566,10 +576,16 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     }
     L::phase1_inv(v, tw, t);                                     // Psi_{i,k}  (R-layout)
     cp_async_wait_all();
-    float4* st = (float4*)(P.w.stash + (((size_t)pair * S + i) * CL + rk) * NNS);
+    float4* st = (float4*)(P.w.stash + (((size_t)pair * S + i) * CL + rk) * (STASH == 2 ? NNS / 2 : NNS));
+    float hprev0 = 0.f, hprev1 = 0.f;                            // STASH == 2: the halves of the even pair, until the odd pair joins them
 #pragma unroll
     for (int p = 0; p < 16; ++p) {                               // stash Psi_i ; H3+H4: Phi = Psi .* T_i
-      if (STASH) __stcs(st + p * T + t, make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y));
+      if (STASH == 1) __stcs(st + p * T + t, make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y));
+      if (STASH == 2) {                                          // registers 2p-2 .. 2p+1 -> one 16-byte word of eight halves
+        const float h0 = __uint_as_float(pack_h2(v[2 * p].x, v[2 * p].y)), h1 = __uint_as_float(pack_h2(v[2 * p + 1].x, v[2 * p + 1].y));
+        if (p & 1) __stcs(st + (p >> 1) * T + t, make_float4(hprev0, hprev1, h0, h1));
+        else { hprev0 = h0; hprev1 = h1; }
+      }
       const cf T0 = p < E ? cs.pf8[(2 * p) * T] : cs.xs8[(2 * p - 2 * E) * 32];
       const cf T1 = p < E ? cs.pf8[(2 * p + 1) * T] : cs.xs8[(2 * p + 1 - 2 * E) * 32];
       v[2 * p] = cmul(v[2 * p], T0);
@@ -641,7 +657,7 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int
 // gT_i, the probe partial conj(R) G~ and the position-gradient terms.  MODE 0: gradients; MODE 2: ePIE directions (R23).
 // IL: also stage |Psi_{i,k}|^2 (illumination map O12; denominators of the step-size sweep).
 // ------------------------------------------------------------------------------------------------
-template <class G, int MODE, bool IL>
+template <class G, int MODE, bool IL, bool H16>   // H16: the stash holds binary16 pairs (PT_STASH_FP16)
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int want_pos) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL;   // stash pairs [0,E) early, [E,16) late; T pairs [0,E) late
@@ -664,10 +680,15 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
   // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
   auto early = [&](int i) {
-    const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
+    const float4* st = (const float4*)(P.w.stash + fld(pair, i) / (H16 ? 2 : 1)) + t;
+    if (H16) {                                                    // eight 16-byte words per thread: the whole field fits the early slots
 #pragma unroll
-    for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
-    if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);               // the late part of the same field: DRAM -> L2 now
+      for (int q = 0; q < 8; ++q) cp_async16(cs.pf + q * T, st + q * T);
+    } else {
+#pragma unroll
+      for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+      if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);             // the late part of the same field: DRAM -> L2 now
+    }
     if (i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
     cp_async_commit();
   };
@@ -688,18 +709,22 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   for (int i = S - 1; i >= 0; --i) {
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
-    {   // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
+    cf Tr[H16 ? 1 : 32 - 2 * E];
+    if (H16) {   // late: all of T_i into the warp's idle X1 region (the stash is in the early slots)
+#pragma unroll
+      for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
+      cp_async_commit();
+    } else {     // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
       const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
 #pragma unroll
       for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
 #pragma unroll
       for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
       cp_async_commit();
-    }
-    // T registers [2E, 32) have no slot left in shared memory: plain loads, issued a whole phase ahead of their use
-    cf Tr[32 - 2 * E];
+      // T registers [2E, 32) have no slot left in shared memory: plain loads, issued a whole phase ahead of their use
 #pragma unroll
-    for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
+      for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
+    }
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     // ePIE (MODE 2): dO = conj(Psi) / max|Psi|^2 chi ; chi' = conj(T) / max|T|^2 chi
@@ -712,12 +737,21 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     }
     float4* gt = (float4*)(P.w.gTpart + fld(spair, i));
     float2* il = IL ? (float2*)(P.w.ilpart + fld(spair, i)) : nullptr;
+    float4 hw = make_float4(0.f, 0.f, 0.f, 0.f);                  // H16: the 16-byte word that holds pairs p, p + 1 (p even)
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
-      const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+      float4 ps;
       cf T0, T1;
-      if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-      else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      if (H16) {
+        if (!(p & 1)) hw = cs.pf[(p >> 1) * T];
+        const cf a = unpack_h2(__float_as_uint((p & 1) ? hw.z : hw.x)), b = unpack_h2(__float_as_uint((p & 1) ? hw.w : hw.y));
+        ps = make_float4(a.x, a.y, b.x, b.y);
+        T0 = cs.xs8[(2 * p) * 32]; T1 = cs.xs8[(2 * p + 1) * 32];
+      } else {
+        ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
+        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
       if (IL) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
@@ -953,7 +987,7 @@ __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 // the sum over the pair is taken in float32 in fixed order (first + second), the gather then sums the pairs in fp64.
 // Staging layout: [Jc][M/2][S][N^2].
 // ------------------------------------------------------------------------------------------------
-template <class G, int MODE, bool IL>   // IL: also stage |Psi_{i,k}|^2 for the illumination map (O12)
+template <class G, int MODE, bool IL, bool H16>   // IL: also stage |Psi_{i,k}|^2 (O12); H16: the stash holds binary16 pairs (PT_STASH_FP16)
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, int want_pos) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NF = F::NF, NNS = F::NNS, T = G::T, E = G::PF16, CL = G::CL, TCOLS = T;       // T/32 warps, 4 per lane quarter, 128 columns each
@@ -981,10 +1015,15 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   // half step s = 0 .. 2S-1: mode h = s & 1 of the pair at slice i = S-1 - (s >> 1)
   auto early = [&](int s) {
     const int h = s & 1, i = S - 1 - (s >> 1);
-    const float4* st = (const float4*)(P.w.stash + fld(pair0 + h, i)) + t;
+    const float4* st = (const float4*)(P.w.stash + fld(pair0 + h, i) / (H16 ? 2 : 1)) + t;
+    if (H16) {                                                    // eight 16-byte words per thread: the whole field fits the early slots
 #pragma unroll
-    for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
-    if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);               // the late part of the same field: DRAM -> L2 now
+      for (int q = 0; q < 8; ++q) cp_async16(cs.pf + q * T, st + q * T);
+    } else {
+#pragma unroll
+      for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
+      if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);             // the late part of the same field: DRAM -> L2 now
+    }
     if (h == 0 && i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);   // serves both modes at slice i
     cp_async_commit();
   };
@@ -1015,17 +1054,21 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     const int h = s & 1, i = S - 1 - (s >> 1), pr = pair0 + h;
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
-    {
+    cf Tr[H16 ? 1 : 32 - 2 * E];
+    if (H16) {   // all of T_i into the warp's idle X1 region (the stash is in the early slots)
+#pragma unroll
+      for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
+      cp_async_commit();
+    } else {
       const float4* st = (const float4*)(P.w.stash + fld(pr, i)) + t;
 #pragma unroll
       for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
 #pragma unroll
       for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
       cp_async_commit();
-    }
-    cf Tr[32 - 2 * E];
 #pragma unroll
-    for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
+      for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
+    }
     L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     float s1 = 1.0f, s2 = 1.0f;
@@ -1037,12 +1080,21 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     }
     float4* gt = (float4*)(P.w.gTpart + fld(spp, i));
     float2* il = IL ? (float2*)(P.w.ilpart + fld(spair0 + h, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
+    float4 hw = make_float4(0.f, 0.f, 0.f, 0.f);                  // H16: the 16-byte word that holds pairs p, p + 1 (p even)
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
-      const float4 ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+      float4 ps;
       cf T0, T1;
-      if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-      else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      if (H16) {
+        if (!(p & 1)) hw = cs.pf[(p >> 1) * T];
+        const cf a = unpack_h2(__float_as_uint((p & 1) ? hw.z : hw.x)), b = unpack_h2(__float_as_uint((p & 1) ? hw.w : hw.y));
+        ps = make_float4(a.x, a.y, b.x, b.y);
+        T0 = cs.xs8[(2 * p) * 32]; T1 = cs.xs8[(2 * p + 1) * 32];
+      } else {
+        ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
+        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
+        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+      }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
       if (IL) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
@@ -1570,9 +1622,11 @@ int set_smem_attrs_now() {
   const int c = (int)chain_smem_bytes<G>();
   bool ok = true;
   auto set = [&](const void* f, int bytes) { ok = ok && cudaFuncSetAttribute(f, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes) == cudaSuccess; };
-  set((const void*)k_forward<G, true>, c); set((const void*)k_forward<G, false>, c);
-  set((const void*)k_backward<G, 0, false>, c); set((const void*)k_backward<G, 0, true>, c); set((const void*)k_backward<G, 2, false>, c);
-  set((const void*)k_backward_pair<G, 0, false>, c); set((const void*)k_backward_pair<G, 0, true>, c); set((const void*)k_backward_pair<G, 2, false>, c);
+  set((const void*)k_forward<G, 0>, c); set((const void*)k_forward<G, 1>, c); set((const void*)k_forward<G, 2>, c);
+  set((const void*)k_backward<G, 0, false, false>, c); set((const void*)k_backward<G, 0, true, false>, c); set((const void*)k_backward<G, 2, false, false>, c);
+  set((const void*)k_backward<G, 0, false, true>, c); set((const void*)k_backward<G, 0, true, true>, c);
+  set((const void*)k_backward_pair<G, 0, false, false>, c); set((const void*)k_backward_pair<G, 0, true, false>, c); set((const void*)k_backward_pair<G, 2, false, false>, c);
+  set((const void*)k_backward_pair<G, 0, false, true>, c); set((const void*)k_backward_pair<G, 0, true, true>, c);
   set((const void*)k_probe_fft<G>, b); set((const void*)k_probe_ifft<G>, b); set((const void*)k_step_probe<G>, b);
   return ok ? PT_OK : PT_ERR_CUDA;
 }
@@ -1618,7 +1672,7 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
     if (kp.bilinear) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
-    launch_fft<G>(k_forward<G, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
+    launch_fft<G>(k_forward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, model_intensity_d, 0);
     LAUNCH_CHECK(K_loss, st);
@@ -1648,6 +1702,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   // two modes per CTA (cluster), their patch gradients summed on chip (k_backward_pair): needs an even number of modes
   const bool paired = use_pairs(p);
   const bool stage_il = kp.w.ilpart != nullptr && !epie;            // |Psi|^2 staged by the backward kernel (step sizes; illumination map)
+  const bool h16 = (p->flags & PT_STASH_FP16) != 0;                 // validated by the caller: no ePIE, illumination map only through ilpart
   kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
@@ -1660,7 +1715,8 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
   auto chains = [&](bool wait_patterns) -> int {
     if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
-    launch_fft<G>(k_forward<G, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
+    if (h16) launch_fft<G>(k_forward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
+    else launch_fft<G>(k_forward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
     if (wait_patterns && chunk_ready && cudaStreamWaitEvent(st, chunk_ready[kp.j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, nullptr, 1);
@@ -1671,14 +1727,20 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       LAUNCH_CHECK(K_epie_max, st);
       k_stash_max<<<kp.jc * p->n_modes * p->n_slices * G::CL, 256, 0, st>>>(kp.w.stash, kp.w.psimax, FL<G>::NNS);
       LAUNCH_CHECK(K_epie_max, st);
-      if (paired) launch_fft<G>(k_backward_pair<G, 2, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
-      else launch_fft<G>(k_backward<G, 2, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      if (paired) launch_fft<G>(k_backward_pair<G, 2, false, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, 0);
+      else launch_fft<G>(k_backward<G, 2, false, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, 0);
     } else if (paired) {
-      if (stage_il) launch_fft<G>(k_backward_pair<G, 0, true>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, wp);
-      else launch_fft<G>(k_backward_pair<G, 0, false>, kp.jc * (p->n_modes / 2) * G::CL, chain_smem_bytes<G>(), st, kp, wp);
+      const unsigned grid = kp.jc * (p->n_modes / 2) * G::CL;
+      if (stage_il && h16) launch_fft<G>(k_backward_pair<G, 0, true, true>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else if (stage_il) launch_fft<G>(k_backward_pair<G, 0, true, false>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else if (h16) launch_fft<G>(k_backward_pair<G, 0, false, true>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else launch_fft<G>(k_backward_pair<G, 0, false, false>, grid, chain_smem_bytes<G>(), st, kp, wp);
     } else {
-      if (stage_il) launch_fft<G>(k_backward<G, 0, true>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, wp);
-      else launch_fft<G>(k_backward<G, 0, false>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp, wp);
+      const unsigned grid = kp.jc * p->n_modes * G::CL;
+      if (stage_il && h16) launch_fft<G>(k_backward<G, 0, true, true>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else if (stage_il) launch_fft<G>(k_backward<G, 0, true, false>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else if (h16) launch_fft<G>(k_backward<G, 0, false, true>, grid, chain_smem_bytes<G>(), st, kp, wp);
+      else launch_fft<G>(k_backward<G, 0, false, false>, grid, chain_smem_bytes<G>(), st, kp, wp);
     }
     LAUNCH_CHECK(K_backward, st);
     return PT_OK;
@@ -1797,6 +1859,9 @@ int32_t gradient_impl(const pt_problem* p, const pt_c64* object_d, const pt_c64*
   if (!step_terms_d) q.flags &= ~PT_WANT_STEP_SIZES;
   rc = ws_layout(&q, workspace_d, workspace_bytes, &w);
   if (rc != PT_OK) return rc;
+  // PT_STASH_FP16: only the chain kernels read the reduced-precision stash; the two other readers (ePIE maxima, the illumination
+  // map when |Psi|^2 is not staged by the backward kernel) are refused
+  if ((p->flags & PT_STASH_FP16) && ((p->flags & PT_EPIE) || ((p->flags & PT_WANT_ILLUM) && illum_d && !w.ilpart))) return PT_ERR_UNSUPPORTED;
   KP kp = make_kp(&q, w, object_d, probe_d, positions_d, intensity_d, batch_idx_d);
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);

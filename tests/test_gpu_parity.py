@@ -1298,3 +1298,44 @@ def test_lsqml_modulus_constraint_chi():
         ptycho.gradient(gpu_problem(cfg, loss=synth.LOSS_POISSON, eps=0.8, **kw), obj_d, pr_d, pos_d, I_d, None, workspace=ws, grad_object=gO,
                         grad_probe=gP, illum_prev=ip_d, step_terms=st, flags=fl)
     assert e.value.code == -8
+
+
+
+# ------------------------------------------------------------------------------------------------
+# PT_STASH_FP16: the slice-wave stash stored as binary16 pairs.  What does not read the
+# stash is unchanged bit for bit; grad_object / illum come out 2e-5 .. 1.01e-4 from the oracle (at north_star's bar,
+# not safely inside it, which is why the flag is opt-in): the bound here is TOL_FP16 = 1.5e-4.
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg3_pairs", "cfg3_odd", "cfg2", "n256"])
+def test_stash_fp16(which):
+    from paper_2505_14372_b200 import ptycho
+    cfg = {"cfg3_pairs": lambda: synth.config(3, scan=(5, 6)), "cfg3_odd": lambda: synth.config(3, scan=(3, 4), n_modes=3, n_slices=4),
+           "cfg2": lambda: synth.config(2, scan=(7, 9)), "n256": lambda: synth.config(4, scan=(2, 3), n_modes=2, n_slices=3, obj_n=300)}[which]()
+    case = make_case(cfg, start_scale=0.8)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity, want_illum=True)
+    pbg = gpu_problem(cfg)
+    wi = cfg.n_modes % 2 == 0                                   # the illumination map needs the backward kernel's |Psi|^2 staging
+    fl = ptycho.WANT_ILLUM if wi else 0
+    g32 = gpu_gradient(case, pbg, flags=fl, want_illum=wi)
+    max_ws = None
+    if which == "cfg3_pairs":                                   # chunked, ragged last chunk
+        lo = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos, fl | ptycho.STASH_FP16, minimum=True)
+        hi = ptycho.workspace_bytes(pbg, cfg.n_pos, cfg.n_pos, fl | ptycho.STASH_FP16)
+        max_ws = lo + (hi - lo) * 7 // 29 + 4096
+    g16 = gpu_gradient(case, pbg, flags=fl | ptycho.STASH_FP16, want_illum=wi, max_ws=max_ws)
+    TOL_FP16 = 1.5e-4
+    check(g16, o, tol_grad=TOL_FP16)
+    for k in ("grad_probe", "grad_pos", "loss_per_pos"):
+        assert g16[k].tobytes() == g32[k].tobytes(), k
+    assert g16["loss"] == g32["loss"]
+    assert g16["grad_object"].tobytes() != g32["grad_object"].tobytes()        # the flag really changed the storage
+    if wi:
+        check_array("illum", g16["illum"], o["illum"], TOL_FP16)
+    else:
+        with pytest.raises(ptycho.PtychoError) as e:            # odd mode count, no step sizes: the map would have to read the stash
+            gpu_gradient(case, pbg, flags=ptycho.WANT_ILLUM | ptycho.STASH_FP16, want_illum=True)
+        assert e.value.code == -8
+    # smaller stash, more positions in flight for the same workspace
+    big = 8 << 30
+    assert ptycho.positions_in_flight(gpu_problem(synth.config(3)), 4096, 4096, ptycho.STASH_FP16, big) > \
+        ptycho.positions_in_flight(gpu_problem(synth.config(3)), 4096, 4096, 0, big)
