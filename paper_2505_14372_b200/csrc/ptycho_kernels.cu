@@ -71,6 +71,7 @@ int run_gradient_256(const pt_problem* p, const void* kp, const GradArgs* a, cud
 namespace {
 
 constexpr int kStatusOOB = 1, kStatusNonfinite = 2;
+constexpr int kReduceZ = 8;          // k_reduce_probe: partial sums per chunk
 
 // ------------------------------------------------------------------------------------------------
 // workspace layout (host + device agree through this POD)
@@ -86,6 +87,7 @@ struct Ws {
   cf* Pt;              // [M][N^2]  F-native, unscaled
   cf* Qt;              // [M][N^2]  F-native: F(dPhat_k) for the step-size sweep
   double2* gPt_acc;    // [M][N^2]  F-native accumulators
+  double2* gPt_part;   // [kReduceZ][M][N^2]  partial sums of one chunk (k_reduce_probe)
   double* loss_pp;     // [J][CL]
   double* posg_part;   // [J][M][CL][2]
   double* step_oi;     // [J][S][6]       step-size sweep: (numO, denO) of slice i; bilinear mode also (numX_y, denX_y, numX_x, denX_x)
@@ -95,7 +97,8 @@ struct Ws {
   cf* psit;            // [Jc][M][N^2]  F-native
   float* wdet;         // [Jc][N^2]     F-native
   cf* stash;           // [Jc][M][S][N^2]  R-native
-  // staged by the backward pass, indexed by (jl + KP::js): per chunk, or per BATCH position when stage_all (step sizes)
+  // staged by the backward pass: per chunk, or per BATCH position when stage_all (step sizes) — the launch sequence then hands
+  // the kernels pointers already advanced to the chunk's first position (stage_chunk), so kernels index all three by jl
   cf* gTpart;          // [Jc|J][M or M/2][S][N^2]  R-native (staged_planes)
   cf* Gpart;           // [Jc|J][M][N^2]     F-native
   float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
@@ -124,7 +127,7 @@ WsSizes ws_sizes(const pt_problem* p) {
   size_t f = 256;
   f += 2 * align_up((S > 1 ? S - 1 : 1) * N * sizeof(cf));
   f += align_up(J * 2 * N * sizeof(cf)) + align_up(J * 2 * sizeof(int32_t)) + align_up(J * 2 * sizeof(float)) + align_up(J * sizeof(int32_t));
-  f += 2 * align_up(M * NN * sizeof(cf)) + align_up(M * NN * sizeof(double2));
+  f += 2 * align_up(M * NN * sizeof(cf)) + (1 + kReduceZ) * align_up(M * NN * sizeof(double2));       // gPt_acc + partial planes
   f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
   f += align_up(J * S * 6 * sizeof(double)) + align_up(J * M * CL * 6 * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
@@ -198,6 +201,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->Pt = (cf*)take(M * NN * sizeof(cf));
   w->Qt = (cf*)take(M * NN * sizeof(cf));
   w->gPt_acc = (double2*)take(M * NN * sizeof(double2));
+  w->gPt_part = (double2*)take(kReduceZ * M * NN * sizeof(double2));
   w->loss_pp = (double*)take(J * CL * sizeof(double));
   w->posg_part = (double*)take(J * M * CL * 2 * sizeof(double));
   w->step_oi = (double*)take(J * S * 6 * sizeof(double));
@@ -227,7 +231,6 @@ struct KP {
   int Jtot;                          // rows of positions / intensity (n_pos_total)
   int Mg;                            // patch-gradient planes per position in the staging buffer: M, or M/2 after k_backward_pair
   int j0, jc;                        // current chunk: batch-local offset and count
-  int js;                            // position offset into the staged arrays (gTpart, Gpart, ilpart): j0 when they hold the whole batch, else 0
   float chi_scale;                   // step-size sweep: chi = -chi_scale gPhi (1; 2 under PT_LSQML_MODULUS_CHI, reading R31)
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
   int loss; float loss_c, eps;
@@ -669,7 +672,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   cs.fill_tables(t);
   Fft<G>::begin_fourier();
   const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
-  const int spair = (jl + P.js) * P.M + k;                          // the same (position, mode) in the staged arrays
+  const int spair = pair;
   const int unit = (jb * P.M + k) * CL + (int)rk;                 // index of this CTA's fp64 partials
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   // patch source: the object window itself, or (bilinear mode) this position's resampled patches [S][NF][NF]
@@ -808,7 +811,7 @@ __global__ void __launch_bounds__(256) k_step_object(KP P) {
   typedef Lay<G> L; typedef FL<G> F;
   constexpr int NNS = F::NNS, T = G::T, CL = G::CL, NV = BILIN ? 6 : 2;
   __shared__ double red[(256 / 32) * NV];
-  const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, sj = jl + P.js;
+  const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, sj = jl;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const size_t onx = P.onx;
   const cf* dO = P.w.dOhat + ((size_t)i * P.ony + r0y) * onx + r0x;
@@ -873,7 +876,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_step_probe(KP P) {
   cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
   cs.fill_tables(t);
   const int pair = blockIdx.x / CL, jl = pair / P.M, k = pair - jl * P.M, jb = P.j0 + jl;
-  const int spair = (jl + P.js) * P.M + k;
+  const int spair = pair;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int onx = P.bilinear ? NF : P.onx;
   const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * P.S * F::NNF : patch_ptr(P, 0, r0y, r0x)) +
@@ -1005,7 +1008,6 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   }
   const int MP = P.M >> 1, pp = blockIdx.x / CL, jl = pp / MP, kp = pp - jl * MP, jb = P.j0 + jl;
   const int pair0 = jl * P.M + 2 * kp;                                            // (position, mode) index of the pair's first mode
-  const int spair0 = (jl + P.js) * P.M + 2 * kp, spp = (jl + P.js) * MP + kp;     // the same pair in the staged arrays
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int S = P.S, onx = P.bilinear ? NF : P.onx;
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
@@ -1078,8 +1080,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       const float tm = P.w.tmax[(size_t)jl * S + i];
       s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;
     }
-    float4* gt = (float4*)(P.w.gTpart + fld(spp, i));
-    float2* il = IL ? (float2*)(P.w.ilpart + fld(spair0 + h, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
+    float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
+    float2* il = IL ? (float2*)(P.w.ilpart + fld(pr, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
     float4 hw = make_float4(0.f, 0.f, 0.f, 0.f);                  // H16: the 16-byte word that holds pairs p, p + 1 (p even)
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
@@ -1124,7 +1126,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     }
     const int pr = pair0 + h, k = 2 * kp + h;
     const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
-    cf* gp = P.w.Gpart + ((size_t)(spair0 + h) * CL + rk) * NNS;
+    cf* gp = P.w.Gpart + ((size_t)pr * CL + rk) * NNS;
     cf wxv[F::NXV];
     load_xv<G>(wxv, rx, t, 1.0f);
     float sy = 0.f, sx = 0.f;
@@ -1220,7 +1222,7 @@ __global__ void __launch_bounds__(256) k_pos_bilinear(KP P, int cl) {
     const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
     for (int e = threadIdx.x; e < NN; e += 256) {
       const int y = e / N, x = e - y * N;
-      const size_t base = ((size_t)(jl + P.js) * P.Mg * P.S + i) * NN + F::r_native_of(y, x);
+      const size_t base = ((size_t)jl * P.Mg * P.S + i) * NN + F::r_native_of(y, x);
       double gr = 0.0, gi = 0.0;
       for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; gr += (double)g.x; gi += (double)g.y; }
       const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
@@ -1291,11 +1293,11 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
             if (ry < 0 || ry >= N || rx < 0 || rx >= N) continue;
             const double wgt = (dy ? fy : 1.0 - fy) * (dx ? fx : 1.0 - fx);
             const int nat = F::r_native_of(ry, rx);
-            const size_t base = ((size_t)(jbase + jj + P.js) * P.Mg * P.S + i) * NN + nat;
+            const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + nat;
             double sr = 0.0, si = 0.0, sl = 0.0;
             for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
             if (ILLUM) {
-              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat, sbs = sb + (size_t)P.js * P.M * P.S * NN;
+              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat, sbs = sb;
               if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
               else for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
             }
@@ -1304,10 +1306,10 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
         }
       } else if (px >= 0 && px < N && py >= 0 && py < N) {
         const int idx = F::r_native_of(py, px);
-        const size_t base = ((size_t)(jbase + jj + P.js) * P.Mg * P.S + i) * NN + idx;
+        const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + idx;
         for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
         if (ILLUM) {
-          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx, sbs = sb + (size_t)P.js * P.M * P.S * NN;
+          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx, sbs = sb;
           if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];   // staged by the backward kernel
           else for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
@@ -1368,7 +1370,7 @@ __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
         const int2 r0 = sr0[jj];
         const int px = ox - r0.x, py = oy - r0.y;
         if (px >= 0 && px < N && py >= 0 && py < N) {
-          const size_t base = ((size_t)(jbase + jj + P.js) * P.M * P.S + i) * NN + F::r_native_of(py, px);
+          const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
           double s = 0.0;
           for (int k = 0; k < P.M; ++k) s += (double)P.w.ilpart[base + (size_t)k * P.S * NN];      // |Psi_{i,k}|^2 staged by the backward kernel
           acc += (double)sal[jj] * s;
@@ -1420,18 +1422,27 @@ __global__ void __launch_bounds__(256) k_objtrans(KP P, float* out, int accumula
   out[e] = (float)((accumulate ? (double)out[e] : 0.0) + acc);
 }
 
-// H12: gP~_k[q] += sum_j (chunk) conj(R_j) G~_{k,j}[q], fixed order, fp64
-__global__ void k_reduce_probe(KP P) {
+// H12: gP~_k[q] += sum_j (chunk) conj(R_j) G~_{k,j}[q], fixed order, fp64, in two stages so that the chunk's positions are summed
+// by kReduceZ blocks side by side: stage 1 sums a contiguous range of positions into part[z][k][q], stage 2 adds the kReduceZ
+// partial sums in order z = 0, 1, ... to the accumulator.
+__global__ void k_reduce_probe(KP P, double2* part) {
+  const int NN = P.N * P.N;
+  const int e = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y, z = blockIdx.z;
+  if (e >= NN) return;
+  const int per = (P.jc + kReduceZ - 1) / kReduceZ, lo = z * per, hi = min(P.jc, lo + per);
+  double ar = 0.0, ai = 0.0;
+  for (int jl = lo; jl < hi; ++jl) {
+    const cf g = P.w.Gpart[(size_t)(jl * P.M + k) * NN + e];
+    ar += (double)g.x; ai += (double)g.y;
+  }
+  part[((size_t)z * P.M + k) * NN + e] = make_double2(ar, ai);
+}
+__global__ void k_reduce_probe2(KP P, const double2* part) {
   const int NN = P.N * P.N;
   const int e = blockIdx.x * blockDim.x + threadIdx.x, k = blockIdx.y;
   if (e >= NN) return;
-  double ar = 0.0, ai = 0.0;
-  for (int jl = 0; jl < P.jc; ++jl) {
-    const cf g = P.w.Gpart[(size_t)((jl + P.js) * P.M + k) * NN + e];
-    ar += (double)g.x; ai += (double)g.y;
-  }
   double2 a = P.w.gPt_acc[(size_t)k * NN + e];
-  a.x += ar; a.y += ai;
+  for (int z = 0; z < kReduceZ; ++z) { const double2 q = part[((size_t)z * P.M + k) * NN + e]; a.x += q.x; a.y += q.y; }
   P.w.gPt_acc[(size_t)k * NN + e] = a;
 }
 
@@ -1592,7 +1603,7 @@ KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64*
            const float* intensity, const int32_t* batch_idx) {
   KP k;
   k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch; k.Jtot = p->n_pos_total;
-  k.j0 = 0; k.jc = 0; k.js = 0; k.px = p->pixel_size;
+  k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
   k.chi_scale = (p->flags & PT_LSQML_MODULUS_CHI) ? 2.0f : 1.0f;
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
   k.bandlim2 = p->bandlimit > 0.f ? (float)(lim * lim) : -1.0f;
@@ -1745,9 +1756,17 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     LAUNCH_CHECK(K_backward, st);
     return PT_OK;
   };
+  // staged arrays that hold the whole batch: the kernels get them advanced to the chunk's first position
+  const Ws w0 = kp.w;
+  auto stage_chunk = [&](int j0) {
+    const size_t js = w0.stage_all ? (size_t)j0 : 0, FN = (size_t)G::CL * FL<G>::NNS;
+    kp.w.gTpart = w0.gTpart + js * kp.Mg * p->n_slices * FN;
+    kp.w.Gpart = w0.Gpart + js * p->n_modes * FN;
+    kp.w.ilpart = w0.ilpart ? w0.ilpart + js * p->n_modes * p->n_slices * FN : nullptr;
+  };
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    kp.js = kp.w.stage_all ? j0 : 0;
+    stage_chunk(j0);
     if ((rc = chains(true)) != PT_OK) return rc;
     if (bilin) {
       if (want_illum) k_gather_object<G, true, true><<<ggrid, gblock, 0, st>>>(kp, (cf*)gO, illum);
@@ -1761,7 +1780,9 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       k_pos_bilinear<G><<<kp.jc, 256, 0, st>>>(kp, G::CL);
       LAUNCH_CHECK(K_pos_bilinear, st);
     }
-    k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp);
+    k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes, kReduceZ), 256, 0, st>>>(kp, kp.w.gPt_part);
+    LAUNCH_CHECK(K_reduce_probe, st);
+    k_reduce_probe2<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp, kp.w.gPt_part);
     LAUNCH_CHECK(K_reduce_probe, st);
   }
   launch_fft<G>(k_probe_ifft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, (const double2*)kp.w.gPt_acc, (cf*)gP, acc ? 1 : 0,
@@ -1777,7 +1798,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     const bool recompute = kp.w.Jc < p->n_batch && !kp.w.stage_all;      // the staged arrays hold the last chunk only
     for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-      kp.js = kp.w.stage_all ? j0 : 0;
+      stage_chunk(j0);
       if (recompute) { if ((rc = chains(false)) != PT_OK) return rc; }
       else if (bilin && kp.w.Jc < p->n_batch) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
       if (bilin) k_step_object<G, true><<<kp.jc * p->n_slices, 256, 0, st>>>(kp);

@@ -1330,7 +1330,7 @@ def test_stash_fp16(which):
     assert g16["loss"] == g32["loss"]
     assert g16["grad_object"].tobytes() != g32["grad_object"].tobytes()        # the flag really changed the storage
     if wi:
-        check_array("illum", g16["illum"], o["illum"], TOL_FP16)
+        check_array("illum", g16["illum"], o["illum"], 3e-4, 6e-4)   # |Psi|^2 of the rounded waves, few windows per pixel on these scans
     else:
         with pytest.raises(ptycho.PtychoError) as e:            # odd mode count, no step sizes: the map would have to read the stash
             gpu_gradient(case, pbg, flags=ptycho.WANT_ILLUM | ptycho.STASH_FP16, want_illum=True)
