@@ -435,7 +435,7 @@ def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit
                 gpu_launches=launches, roofline=roof, cpu_baseline=cpu, loss=loss_val)
 
 
-TRAFFIC_FILE = "r2_dominant_kernel_traffic.csv"
+TRAFFIC_FILE = "r2_dominant_kernel_traffic.csv"   # written with profiles/r2_ncu_full_summary.md
 # what the default invocation times after the headline workload: (key, config, keyword overrides)
 SECONDARY = [("config1", 1, {}), ("config2", 2, {}), ("config3_bandlimit_0.667", 3, dict(bandlimit=2.0 / 3.0)),
              ("config5_batch1024", 5, dict(batch=1024)), ("config4", 4, {})]
