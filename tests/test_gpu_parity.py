@@ -1106,14 +1106,16 @@ def test_cfg5_full_size_minibatch_properties():
 
 
 # ------------------------------------------------------------------------------------------------
-# More than 256 windows in one chunk: the gather kernels (k_gather_object, its illumination branch, k_gather_willum) walk
-# a chunk's windows in groups of 256; every array against the oracle (N = 64, 2 modes, 2 slices, 20 x 20 scan, one chunk).
+# More than 256 windows in one chunk: the gather kernels (k_gather_object / k_gather_object_w, their illumination branch,
+# k_gather_willum) walk a chunk's windows in groups; every array against the oracle (N = 64, 2 modes, 20 x 20 scan, one chunk).
 # ------------------------------------------------------------------------------------------------
-@pytest.mark.parametrize("mode", ["fourier", "bilinear"])
-def test_gather_window_groups_beyond_256(mode):
+@pytest.mark.parametrize("mode,n_slices", [("fourier", 2), ("fourier", 12), ("bilinear", 2), ("bilinear", 12)])
+def test_gather_window_groups_beyond_256(mode, n_slices):
+    # n_slices = 2: few object tiles, the windows are split over the warps of a block (k_gather_object_w, eight groups of 32 per
+    # round); n_slices = 12: 2400 tiles, the tile gather (k_gather_object, groups of 256 windows)
     import torch
     from paper_2505_14372_b200 import ptycho
-    cfg = synth.config(5, n=64, scan=(20, 20), n_modes=2, n_slices=2, obj_n=200, pixel_size=0.2, step_px=3.0)
+    cfg = synth.config(5, n=64, scan=(20, 20), n_modes=2, n_slices=n_slices, obj_n=200, pixel_size=0.2, step_px=3.0)
     J, S = cfg.n_pos, cfg.n_slices
     if mode == "bilinear":
         case, pbo = _bilinear_case(cfg, 0.8)
