@@ -366,6 +366,8 @@ struct ChainSmem {
 __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
   asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
 }
+// every thread asks for the 128-byte line at p to be brought into L2 (fire and forget)
+__device__ __forceinline__ void l2_prefetch_line(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
 // one thread asks for `bytes` (a multiple of 16, 16-byte aligned) of global memory to be brought into L2
 __device__ __forceinline__ void l2_prefetch_bulk(const void* src, unsigned bytes) {
   asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
@@ -605,6 +607,70 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   Fft<G>::end_fourier();
 }
 
+// fp64 square root and reciprocal from a float32 seed and Newton steps (two: relative error ~1e-15 from the seed's 2.4e-7; no fp64
+// division or square-root sequence, which cost ~20 dependent instructions each): the per-pixel loss stays an fp64 quantity
+__device__ __forceinline__ double dsqrt_newton(double x) {
+  if (!(x > 1e-30 && x < 1e30)) return sqrt(x);
+  double r = (double)rsqrtf((float)x);
+  r = r * (1.5 - 0.5 * x * r * r);
+  r = r * (1.5 - 0.5 * x * r * r);
+  return x * r;
+}
+__device__ __forceinline__ double drecip_newton(double d) {       // d > 0
+  if (!(d > 1e-30 && d < 1e30)) return 1.0 / d;                   // outside the float32 seed's comfortable range
+  double y = (double)__fdividef(1.0f, (float)d);                   // MUFU.RCP seed: no slow-path subroutine
+  y = y * (2.0 - d * y);
+  y = y * (2.0 - d * y);
+  return y;
+}
+// per-pixel loss l and detector weight w = dl/dI (readings R11, R12, R12b), fp64
+__device__ __forceinline__ void pixel_loss(int loss, double Im, double Ix, double eps, double c, double& l, double& w) {
+  if (loss == PT_LOSS_GAUSSIAN) {
+    const double ic2 = drecip_newton(c * c);
+    l = 0.5 * (Im - Ix) * (Im - Ix) * ic2;
+    w = (Im - Ix) * ic2;
+  } else if (loss == PT_LOSS_POISSON) {
+    const double ri = drecip_newton(Im + eps);
+    l = Im - Ix * (1.0 - log((Ix + eps) * ri));                  // = Im - Ix (ln(Im+eps) - ln(Ix+eps) + 1)
+    w = 1.0 - Ix * ri;
+  } else {
+    const double a = dsqrt_newton(Im + c), ae = dsqrt_newton(Ix + c);
+    l = 0.5 * (a - ae) * (a - ae);
+    w = 0.5 * (1.0 - ae * drecip_newton(a + eps));
+  }
+}
+
+// The same in float32, written so that no difference of nearly equal numbers is formed from ROUNDED quantities other than the
+// inputs themselves (used by the fused single-slice kernel, whose one CTA per SM cannot hide the latency of fp64 sequences — the
+// fp64 pipe of this GPU runs at a small fraction of the fp32 rate; the sum over pixels is still taken in fp64):
+//   amplitude: d = sqrt(I+c) - sqrt(Iexp+c) ; l = d^2 / 2 ; w = (d + eps) / (2 (sqrt(I+c) + eps))   [= (1 - ae/(a+eps)) / 2]
+//   Poisson:   u = (I - Iexp) / (Iexp + eps) ; l = (I - Iexp) - Iexp log1p(u) ; w = (I - Iexp + eps) / (I + eps)
+// float32 square root (x >= 0) and reciprocal (d > 0, normal range) from the MUFU seeds and one Newton step each: within an ulp,
+// and without the slow-path subroutines of sqrtf() and "/" (taken for zeros, of which a diffraction pattern has many: the loop over
+// a thread's 32 pixels cost 33 k cycles with them, 250 instructions per pixel)
+__device__ __forceinline__ float sqrt_newton_f32(float x) {
+  const float r = rsqrtf(x), a0 = x * r;
+  return x > 0.f ? fmaf(0.5f * r, fmaf(-a0, a0, x), a0) : 0.f;
+}
+__device__ __forceinline__ float rcp_newton_f32(float d) {
+  const float y = __fdividef(1.0f, d);
+  return y * fmaf(-d, y, 2.0f);
+}
+__device__ __forceinline__ void pixel_loss_f32(int loss, float Im, float Ix, float eps, float c, float& l, float& w) {
+  if (loss == PT_LOSS_GAUSSIAN) {
+    const float ic2 = rcp_newton_f32(c * c), d = Im - Ix;
+    l = 0.5f * d * d * ic2; w = d * ic2;
+  } else if (loss == PT_LOSS_POISSON) {
+    const float d = Im - Ix;
+    l = d - Ix * log1pf(d * rcp_newton_f32(Ix + eps));
+    w = (d + eps) * rcp_newton_f32(Im + eps);
+  } else {
+    const float a = sqrt_newton_f32(Im + c), d = a - sqrt_newton_f32(Ix + c);
+    l = 0.5f * d * d;
+    w = 0.5f * (d + eps) * rcp_newton_f32(a + eps);
+  }
+}
+
 // ------------------------------------------------------------------------------------------------
 // H7 + H8: I = sum_k |psi~_k|^2 ; per-pixel loss in fp64 ; w = dl/dI.  One CTA per (position of the chunk, rank).
 // ------------------------------------------------------------------------------------------------
@@ -633,17 +699,7 @@ __global__ void __launch_bounds__(G::T) k_loss(KP P, float* model_intensity, int
     if (Ie) {
       const double Im = (double)I[r], Ix = (double)Ie[qy * NF + qx];
       double l, w;
-      if (P.loss == PT_LOSS_GAUSSIAN) {
-        l = (Im - Ix) * (Im - Ix) / (2.0 * c * c);
-        w = (Im - Ix) / (c * c);
-      } else if (P.loss == PT_LOSS_POISSON) {
-        l = Im - Ix * (log(Im + eps) - log(Ix + eps) + 1.0);
-        w = 1.0 - Ix / (Im + eps);
-      } else {
-        const double a = sqrt(Im + c), ae = sqrt(Ix + c);
-        l = 0.5 * (a - ae) * (a - ae);
-        w = 0.5 * (1.0 - ae / (a + eps));
-      }
+      pixel_loss(P.loss, Im, Ix, eps, c, l, w);
       acc[0] += l;
       if (want_w) P.w.wdet[((size_t)jl * CL + rk) * NNS + L::native(t, r)] = (float)w;
     }
@@ -1158,6 +1214,235 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
 }
 
 // ------------------------------------------------------------------------------------------------
+// Single-slice path (S = 1: BASELINE.json configs 1 and 2; "strong phase object approximation"): forward model, loss
+// and adjoint of ONE position in one persistent CTA, all modes in turn — no kernel boundary between H2..H13, no per-mode staging:
+//   pass 1, mode k:  Psi_k = Finv(R P~_k)/N^2 -> scratch ; Phi = Psi_k T ; psi~_k = F(Phi)/N -> scratch ; I += |psi~_k|^2
+//   loss:            l(I, Iexp) per pixel in fp64, w = dl/dI                                   (as k_loss)
+//   pass 2, mode k:  gPhi = F^H(w psi~_k)/N ; gT += conj(Psi_k) gPhi ; G~ = F(conj(T) gPhi) ; probe partial conj(R) G~ ;
+//                    position terms                                                            (as k_backward)
+// On chip for the whole position: the patch T and the mode sum of gT in tensor memory (64 + 64 columns per warp), I (then w) in
+// the thread-private shared-memory slots, the shift ramp ry in the (otherwise idle) propagator-table buffer.  Psi_k and psi~_k
+// pass through the per-position scratch of the workspace (the stash / far-field arrays of the chain path; the CTA reads back what
+// it wrote shortly before, from L2).  Only ONE patch-gradient plane per position is staged (fp32 sum over the modes in order),
+// so the gather reads 1/M of what the per-mode kernels stage.  CTAs stay resident and take positions jl = blockIdx.x, + gridDim.x, ...
+// ------------------------------------------------------------------------------------------------
+template <class G>
+__global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want_pos) {
+  typedef Lay<G> L; typedef FL<G> F;
+  static_assert(G::CL == 1, "single-slice path: one CTA per field");
+  constexpr int NF = F::NF, NNS = F::NNS, T = G::T, TCOLS = (T / 128) * 128;     // 128 columns per warp: T and the gT sum
+  extern __shared__ __align__(16) unsigned char smem_raw[];
+  const int t = threadIdx.x, wp = t >> 5;
+  ChainSmem<G> cs(smem_raw, t);
+  cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
+  uint32_t* tmem_slot = (uint32_t*)((unsigned char*)red + 1000);
+  float* Ib = (float*)(cs.hyS + 2 * NF) + t;                        // I (then w) of register r: Ib[r * T]   (thread-private)
+  cf* ryS = cs.hyS;                                                 // ry of the current position
+  cs.fill_tables(t);
+  if (wp == 0) {
+    asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(tmem_slot)), "n"(TCOLS));
+    asm volatile("tcgen05.relinquish_alloc_permit.cta_group::1.sync.aligned;");
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  asm volatile("tcgen05.fence::after_thread_sync;" ::: "memory");
+  const uint32_t tb = *tmem_slot + ((uint32_t)((wp & 3) * 32) << 16) + (uint32_t)((wp >> 2) * 128);
+  const uint32_t tbT = tb, tbG = tb + 64;                           // columns [0, 64): T ; [64, 128): sum_k gT_k
+  const int onx = P.onx;
+  const float inv_n = 1.0f / (float)NF;
+  cf v[32];
+  for (int jl = blockIdx.x; jl < P.jc; jl += gridDim.x) {
+    const int jb = P.j0 + jl, row = P.w.rows[jb];
+    const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
+    const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)F::pix_y(0, t, 0) * onx + F::pix_x(0, t, 0);
+    const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
+    const cf* ry = rx + NF;
+    __syncthreads();                                                // the previous position's readers of ryS / red are done
+    if (jl == (int)blockIdx.x) {                                    // first position of this CTA: nobody has prefetched P~_0 yet
+      const float4* src = (const float4*)P.w.Pt + t;
+#pragma unroll
+      for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, src + p * T);
+      cp_async_commit();
+    }
+    if (t < NF) ryS[t] = ry[t];
+    for (int b = t * 128; b < F::NNF * 4; b += T * 128)             // this position's measured pattern: DRAM -> L2 now
+      l2_prefetch_line((const char*)(P.intensity + (size_t)row * F::NNF) + b);
+#pragma unroll
+    for (int c = 0; c < 4; ++c) {                                   // H3: the patch, once per position, parked in tensor memory
+      cf tt[8];
+#pragma unroll
+      for (int e = 0; e < 8; ++e) tt[e] = ld_nc8(ob + F::patch_off(8 * c + e, onx));
+      tmem_st16(tbT + 16 * c, tt);
+    }
+    tmem_wait_st();
+    cf wxv[F::NXV];
+    __syncthreads();                                                // ryS visible
+    // One loop over the 2M half steps (pass 1: modes 0..M-1 forward, pass 2: modes 0..M-1 adjoint) so that the kernel holds ONE
+    // inverse and ONE forward transform body: with four inlined transforms (~130 KB of code) the loop did not fit the
+    // instruction cache and ran three times slower.
+#pragma unroll 1
+    for (int hs = 0; hs < 2 * P.M; ++hs) {
+      const bool fwd_pass = hs < P.M;
+      const int k = fwd_pass ? hs : hs - P.M;
+      const size_t fk = ((size_t)jl * P.M + k) * NNS;               // field (position, mode) in the staged arrays
+      const size_t sk = ((size_t)blockIdx.x * P.M + k) * NNS;       // the CTA's scratch field of mode k: the same lines for every position
+                                                                    // the CTA takes, so that they stay in L2 instead of streaming to HBM
+      if (hs == P.M) {
+        // ---------------- H8: loss and detector weight (float32 per pixel in cancellation-free form, fp64 sum)
+        double acc[1] = {0.0};
+        const float* Ie = P.intensity + (size_t)row * F::NNF;
+        float ix[32];                                               // all 32 loads in flight before the first use (v is dead here)
+#pragma unroll
+        for (int r = 0; r < 32; ++r) ix[r] = __ldg(Ie + F::fq_y(0, t, r) * NF + F::fq_x(0, t, r));
+        float ls = 0.f, lc = 0.f;                                   // the thread's 32 terms: compensated float32 sum (fp64 conversions
+#pragma unroll                                                      // and adds are what made this loop cost 35 k cycles), then fp64
+        for (int r = 0; r < 32; ++r) {
+          float l, w;
+          pixel_loss_f32(P.loss, Ib[r * T], ix[r], P.eps, P.loss_c, l, w);
+          const float y = l - lc, s2 = ls + y;
+          lc = (s2 - ls) - y; ls = s2;
+          Ib[r * T] = w;
+        }
+        acc[0] = (double)ls - (double)lc;
+        block_sum<G::T, 1>(acc, red);
+        if (t == 0) {
+          P.w.loss_pp[jb] = acc[0];
+          if (!(acc[0] == acc[0]) || fabs(acc[0]) > 1e300) atomicOr(P.w.status, kStatusNonfinite);
+        }
+      }
+      {   // Fourier-side start: H2  R .* P~_k / N^2   or   H9  g~ = w .* psi~_k / N ; the source field (P~_k, or psi~_k from the
+          // scratch) was asked into the warp's idle X1 region at the end of the previous half step
+        if (fwd_pass) load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
+        cp_async_wait_all();
+#pragma unroll
+        for (int p = 0; p < 16; ++p) {
+          const float4 q = cs.xs[p * 32];
+          if (fwd_pass) {
+            v[2 * p] = cmul(make_float2(q.x, q.y), cmul(wxv[0], ryS[F::fq_y(0, t, 2 * p)]));
+            v[2 * p + 1] = cmul(make_float2(q.z, q.w), cmul(wxv[0], ryS[F::fq_y(0, t, 2 * p + 1)]));
+          } else {
+            const float w0 = Ib[(2 * p) * T] * inv_n, w1 = Ib[(2 * p + 1) * T] * inv_n;
+            v[2 * p] = make_float2(q.x * w0, q.y * w0);
+            v[2 * p + 1] = make_float2(q.z * w1, q.w * w1);
+          }
+        }
+      }
+      __syncthreads();                                              // every warp has read its source slots: the inverse transform's
+                                                                    // CTA-wide exchange may now write into any warp's region
+      Fft<G>::inv_head(v, sm, cs.tw2, t, 0u);
+      if (!fwd_pass) {   // Psi_k back from the scratch into the warp's idle X1 region (16 slots of 16 B per lane) while phase 1 runs
+        const float4* st = (const float4*)(P.w.stash + sk) + t;
+#pragma unroll
+        for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, st + p * T);
+      }
+      cp_async_commit();
+      L::phase1_inv(v, tw, t);                                      // Psi_k   or   gPhi_k   (R-layout)
+      cp_async_wait_all();
+      float4* stw = (float4*)(P.w.stash + sk) + t;
+#pragma unroll
+      for (int c = 0; c < 4; ++c) {
+        cf tt[8], ga[8];
+        tmem_ld16(tbT + 16 * c, tt);
+        if (fwd_pass) {                                             // keep Psi_k for pass 2 ; H4: Phi = Psi_k .* T
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int p = 4 * c + e;
+            stw[p * T] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
+            v[2 * p] = cmul(v[2 * p], tt[2 * e]);
+            v[2 * p + 1] = cmul(v[2 * p + 1], tt[2 * e + 1]);
+          }
+        } else {                                                    // H10: gT += conj(Psi_k) gPhi ; gPsi = conj(T) gPhi
+          if (k > 0) tmem_ld16(tbG + 16 * c, ga);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int p = 4 * c + e;
+            const float4 ps = cs.xs[p * 32];
+            const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
+            ga[2 * e] = k > 0 ? cadd(ga[2 * e], g0) : g0;
+            ga[2 * e + 1] = k > 0 ? cadd(ga[2 * e + 1], g1) : g1;
+            v[2 * p] = cmulc(v[2 * p], tt[2 * e]);
+            v[2 * p + 1] = cmulc(v[2 * p + 1], tt[2 * e + 1]);
+          }
+          if (k + 1 < P.M) tmem_st16(tbG + 16 * c, ga);
+          else {                                                    // last mode: the sum over the modes goes to the staging buffer
+            float4* gt = (float4*)(P.w.gTpart + (size_t)jl * NNS) + t;
+#pragma unroll
+            for (int e = 0; e < 4; ++e) __stcs(gt + (4 * c + e) * T, make_float4(ga[2 * e].x, ga[2 * e].y, ga[2 * e + 1].x, ga[2 * e + 1].y));
+          }
+        }
+      }
+      tmem_wait_st();
+      Fft<G>::fwd(v, sm, tw, cs.tw2, t, 0u);                        // F(Phi)   or   G~ = F(gPsi)
+      // the next half step's source field -> the warp's X1 region (free until that half step's inverse transform): P~ of the next
+      // mode, psi~ of the first / next mode from the scratch, or P~_0 again for the CTA's next position.  Issued before the tail
+      // below so that the copy overlaps it — except when the field is psi~_0 and this half step is about to store it (M = 1)
+      const int hn = hs + 1;
+      auto prefetch_next = [&]() {
+        const cf* nsrc = hn < P.M ? P.w.Pt + (size_t)hn * NNS : hn < 2 * P.M ? P.w.psit + ((size_t)blockIdx.x * P.M + (hn - P.M)) * NNS : P.w.Pt;
+        const float4* src = (const float4*)nsrc + t;
+#pragma unroll
+        for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, src + p * T);
+        cp_async_commit();
+        // and Psi of the next adjoint half step towards L2 (its cp.async is issued only after that half step's inverse-transform head)
+        if (hn >= P.M && hn < 2 * P.M)
+          for (int b = t * 128; b < NNS * 8; b += T * 128) l2_prefetch_line((const char*)(P.w.stash + ((size_t)blockIdx.x * P.M + (hn - P.M)) * NNS) + b);
+      };
+      if (hn != P.M) prefetch_next();
+      if (fwd_pass) {
+        float4* out = (float4*)(P.w.psit + sk) + t;                 // H6: psi~_k = F(Phi) / N ; H7: I += |psi~_k|^2
+#pragma unroll
+        for (int p = 0; p < 16; ++p) {
+          const float4 q = make_float4(v[2 * p].x * inv_n, v[2 * p].y * inv_n, v[2 * p + 1].x * inv_n, v[2 * p + 1].y * inv_n);
+          out[p * T] = q;
+          const float i0 = fmaf(q.x, q.x, q.y * q.y), i1 = fmaf(q.z, q.z, q.w * q.w);
+          Ib[(2 * p) * T] = k == 0 ? i0 : Ib[(2 * p) * T] + i0;
+          Ib[(2 * p + 1) * T] = k == 0 ? i1 : Ib[(2 * p + 1) * T] + i1;
+        }
+        if (hn == P.M) prefetch_next();                             // psi~_0, after this thread's own store of it (M = 1)
+      } else {
+        // H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
+        const float4* pt4 = (const float4*)(P.w.Pt + (size_t)k * NNS) + t;
+        float4* gp4 = (float4*)(P.w.Gpart + fk) + t;
+        load_xv<G>(wxv, rx, t, 1.0f);
+        float sy = 0.f, sx = 0.f;
+        const float fx = (float)signed_freq(F::fq_x(0, t, 0), NF) / (float)NF;
+#pragma unroll
+        for (int c = 0; c < 4; ++c) {
+          float4 q[4];                                              // P~ of four register pairs in flight before their use
+#pragma unroll
+          for (int e = 0; e < 4; ++e) q[e] = want_pos ? __ldg(pt4 + (4 * c + e) * T) : make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int p = 4 * c + e;
+            const int qy0 = F::fq_y(0, t, 2 * p), qy1 = F::fq_y(0, t, 2 * p + 1);
+            const cf R0 = cmul(wxv[0], ryS[qy0]), R1 = cmul(wxv[0], ryS[qy1]);
+            const cf g0 = cmulc(v[2 * p], R0), g1 = cmulc(v[2 * p + 1], R1);
+            gp4[p * T] = make_float4(g0.x, g0.y, g1.x, g1.y);
+            if (want_pos) {
+              const cf z0 = cmulc(cmul(R0, make_float2(q[e].x, q[e].y)), v[2 * p]), z1 = cmulc(cmul(R1, make_float2(q[e].z, q[e].w)), v[2 * p + 1]);
+              sy = fmaf((float)signed_freq(qy0, NF) * (1.0f / (float)NF), z0.y, sy); sx = fmaf(fx, z0.y, sx);
+              sy = fmaf((float)signed_freq(qy1, NF) * (1.0f / (float)NF), z1.y, sy); sx = fmaf(fx, z1.y, sx);
+            }
+          }
+        }
+        if (want_pos) {
+          double acc[2] = {(double)sy, (double)sx};
+          block_sum<G::T, 2>(acc, red);
+          if (t == 0) {
+            const double f = 4.0 * CUDART_PI / ((double)NF * (double)NF);
+            P.w.posg_part[((size_t)jb * P.M + k) * 2 + 0] = f * acc[0];
+            P.w.posg_part[((size_t)jb * P.M + k) * 2 + 1] = f * acc[1];
+          }
+        }
+      }
+    }
+  }
+  asm volatile("tcgen05.fence::before_thread_sync;" ::: "memory");
+  __syncthreads();
+  if (wp == 0) asm volatile("tcgen05.dealloc.cta_group::1.sync.aligned.b32 %0, %1;" ::"r"(*tmem_slot), "n"(TCOLS));
+}
+
+// ------------------------------------------------------------------------------------------------
 // ePIE normalisations: tmax[jl][i] = max over the window of |O_i|^2 ; psimax[block] = max |Psi|^2 of
 // one 16384-element block of the stash (one per (pair, slice, rank); the backward kernel takes the max over the ranks).
 // ------------------------------------------------------------------------------------------------
@@ -1632,11 +1917,11 @@ __global__ void k_lsqml_pos(float* pos, const float* step_terms, const int32_t* 
 // ------------------------------------------------------------------------------------------------
 enum Kind { K_setup_prop, K_setup_pos, K_probe_fft, K_forward, K_loss, K_finalize, K_zero, K_backward, K_gather_object,
             K_reduce_probe, K_probe_ifft, K_dohat, K_axpy, K_pos_sgd, K_lsqml_alpha, K_lsqml_object, K_lsqml_probe,
-            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_regularizer, K_constraint, K_adam, K_step_object, K_step_probe, K_COUNT };
+            K_lsqml_pos, K_bilinear_patches, K_pos_bilinear, K_epie_max, K_alpha_pos, K_gather_willum, K_objtrans, K_regularizer, K_constraint, K_adam, K_step_object, K_step_probe, K_single, K_COUNT };
 const char* const kKindNames[K_COUNT] = {"k_setup_prop", "k_setup_pos", "k_probe_fft", "k_forward", "k_loss", "k_finalize",
                                          "k_zero", "k_backward", "k_gather_object", "k_reduce_probe", "k_probe_ifft", "k_dohat",
                                          "k_axpy", "k_pos_sgd", "k_lsqml_alpha", "k_lsqml_object", "k_lsqml_probe", "k_lsqml_pos",
-                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam", "k_step_object", "k_step_probe"};
+                                         "k_bilinear_patches", "k_pos_bilinear", "k_epie_max", "k_alpha_pos", "k_gather_willum", "k_objtrans", "k_regularizer", "k_constraint", "k_adam", "k_step_object", "k_step_probe", "k_single"};
 
 inline void prof_mark(int kind, cudaStream_t st) {
   if (!g_prof_on) return;
@@ -1695,6 +1980,19 @@ cudaError_t launch_fft(void (*kern)(KArgs...), unsigned grid, size_t smem, cudaS
   return cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
 }
 
+// SMs of the current device (asked once per process and device)
+inline int sm_count() {
+  static std::mutex mu;
+  static int cached[32] = {0};
+  int dev = 0, n = 148;
+  if (cudaGetDevice(&dev) != cudaSuccess) return n;
+  std::lock_guard<std::mutex> lock(mu);
+  if (dev < 32 && cached[dev] > 0) return cached[dev];
+  if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess || n < 1) n = 148;
+  if (dev < 32) cached[dev] = n;
+  return n;
+}
+
 // dynamic shared-memory limits of the FFT kernels: set once per process and geometry (per device: the attribute is per context)
 template <class G>
 int set_smem_attrs_now() {
@@ -1708,6 +2006,7 @@ int set_smem_attrs_now() {
   set((const void*)k_backward_pair<G, 0, false, false>, c); set((const void*)k_backward_pair<G, 0, true, false>, c); set((const void*)k_backward_pair<G, 2, false, false>, c);
   set((const void*)k_backward_pair<G, 0, false, true>, c); set((const void*)k_backward_pair<G, 0, true, true>, c);
   set((const void*)k_probe_fft<G>, b); set((const void*)k_probe_ifft<G>, b); set((const void*)k_step_probe<G>, b);
+  if constexpr (G::CL == 1) set((const void*)k_single<G>, c);
   return ok ? PT_OK : PT_ERR_CUDA;
 }
 template <class G>
@@ -1783,7 +2082,10 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool paired = use_pairs(p);
   const bool stage_il = kp.w.ilpart != nullptr && !epie;            // |Psi|^2 staged by the backward kernel (step sizes; illumination map)
   const bool h16 = (p->flags & PT_STASH_FP16) != 0;                 // validated by the caller: no ePIE, illumination map only through ilpart
-  kp.Mg = paired ? p->n_modes / 2 : p->n_modes;
+  // single slice, plain gradient: forward, loss and adjoint of a position fused in one persistent kernel (k_single)
+  const bool single = G::CL == 1 && p->n_slices == 1 && !bilin && !epie && !want_steps && !want_illum && !h16 && !kp.w.ilpart &&
+                      !(p->flags & PT_NO_SINGLE_SLICE_FUSION);
+  kp.Mg = single ? 1 : paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
   if (!acc) {
@@ -1794,6 +2096,15 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
   auto chains = [&](bool wait_patterns) -> int {
+    if constexpr (G::CL == 1) {
+      if (single) {
+        if (wait_patterns && chunk_ready && cudaStreamWaitEvent(st, chunk_ready[kp.j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
+        const int resident = sm_count() * min_blocks<G>();
+        launch_fft<G>(k_single<G>, kp.jc < resident ? kp.jc : resident, chain_smem_bytes<G>(), st, kp, want_pos ? 1 : 0);
+        LAUNCH_CHECK(K_single, st);
+        return PT_OK;
+      }
+    }
     if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
     if (h16) launch_fft<G>(k_forward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     else launch_fft<G>(k_forward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);

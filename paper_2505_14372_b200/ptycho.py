@@ -18,7 +18,7 @@ LIB_PATH = os.path.join(_HERE, "libptycho_b200.so")
 
 LOSS_AMPLITUDE, LOSS_POISSON, LOSS_GAUSSIAN = 0, 1, 2
 SHIFT_FOURIER_PROBE, SHIFT_BILINEAR_OBJECT = 0, 1
-WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLUM, NO_MODE_PAIRS, LSQML_MODULUS_CHI, STASH_FP16 = 1, 2, 4, 16, 32, 64, 128, 256, 512
+WANT_POS_GRAD, WANT_ILLUM, WANT_STEP_SIZES, ACCUMULATE, EPIE, WANT_WEIGHTED_ILLUM, NO_MODE_PAIRS, LSQML_MODULUS_CHI, STASH_FP16, NO_SINGLE_SLICE_FUSION = 1, 2, 4, 16, 32, 64, 128, 256, 512, 1024
 UPDATE_SGD, UPDATE_LSQML, UPDATE_EPIE, UPDATE_LSQML_WEIGHTED = 0, 1, 2, 3
 OK = 0
 EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_positions_in_flight", "ptycho_forward_loss", "ptycho_gradient",

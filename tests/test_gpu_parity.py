@@ -1341,3 +1341,29 @@ def test_stash_fp16(which):
     big = 8 << 30
     assert ptycho.positions_in_flight(gpu_problem(synth.config(3)), 4096, 4096, ptycho.STASH_FP16, big) > \
         ptycho.positions_in_flight(gpu_problem(synth.config(3)), 4096, 4096, 0, big)
+
+
+
+# ------------------------------------------------------------------------------------------------
+# Single-slice problems run forward, loss and adjoint of a position in one fused kernel (k_single); PT_NO_SINGLE_SLICE_FUSION sends
+# them through the multislice kernel sequence instead.  Both against the oracle, and against each other (they differ only in the
+# order of the float32 sum of the patch gradients over the modes and of the fp64 partial sums of the probe gradient).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg1", "cfg2", "n64_m3"])
+def test_single_slice_fused_and_unfused(which):
+    from paper_2505_14372_b200 import ptycho
+    cfg = {"cfg1": lambda: synth.config(1), "cfg2": lambda: synth.config(2, scan=(13, 14)),       # 182 positions: more than one per resident CTA
+           "n64_m3": lambda: synth.config(2, n=64, scan=(30, 25), n_modes=3, obj_n=200, pixel_size=0.2, step_px=3.0)}[which]()
+    case = make_case(cfg, start_scale=0.0 if which == "cfg1" else 0.8, noise=which != "cfg1")
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    pbg = gpu_problem(cfg)
+    a = gpu_gradient(case, pbg)
+    b = gpu_gradient(case, pbg, flags=ptycho.NO_SINGLE_SLICE_FUSION)
+    check(a, o, pos=which != "cfg1", px=cfg.pixel_size)
+    check(b, o, pos=which != "cfg1", px=cfg.pixel_size)
+    assert a["grad_object"].tobytes() != b["grad_object"].tobytes() or cfg.n_modes == 1      # the flag really selected another path
+    margin("fused vs unfused gO", rel_l2(a["grad_object"], b["grad_object"]), 1e-6)
+    margin("fused vs unfused gP", rel_l2(a["grad_probe"], b["grad_probe"]), 1e-6)
+    a2 = gpu_gradient(case, pbg)
+    for k in ("grad_object", "grad_probe", "grad_pos", "loss_per_pos"):
+        assert a[k].tobytes() == a2[k].tobytes(), k                                           # deterministic
