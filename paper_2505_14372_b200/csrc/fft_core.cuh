@@ -168,18 +168,24 @@ struct Lay {
     tw[idx] = make_float2(c, s);
   }
 
-  // ---- phase 1 (forward): R-layout regs -> (k1y, k1x) regs with twiddles
+  // ---- phase 1 (forward): R-layout regs -> (k1y, k1x) regs with twiddles.  In two pieces so that a caller can run the row
+  // transforms of registers [n1y N1X, (n1y + 1) N1X) as soon as those registers are final (the chain kernels interleave them with
+  // the global stores of the pointwise stretch): phase1_fwd = phase1_fwd_row for every n1y, then phase1_fwd_rest.
+  static PTK_HD void phase1_fwd_row(cf (&v)[32], int n1y) {
+    cf x[G::N1X];
+#pragma unroll
+    for (int i = 0; i < G::N1X; ++i) x[i] = v[n1y * G::N1X + i];
+    Dft<G::N1X, -1>::run(x);
+#pragma unroll
+    for (int i = 0; i < G::N1X; ++i) v[n1y * G::N1X + i] = x[i];
+  }
   static PTK_HD void phase1_fwd(cf (&v)[32], const cf* tw, int t) {
+#pragma unroll
+    for (int n1y = 0; n1y < G::N1Y; ++n1y) phase1_fwd_row(v, n1y);
+    phase1_fwd_rest(v, tw, t);
+  }
+  static PTK_HD void phase1_fwd_rest(cf (&v)[32], const cf* tw, int t) {
     const int a = t & (G::N2X - 1), b = t >> G::LX2;
-#pragma unroll
-    for (int n1y = 0; n1y < G::N1Y; ++n1y) {
-      cf x[G::N1X];
-#pragma unroll
-      for (int i = 0; i < G::N1X; ++i) x[i] = v[n1y * G::N1X + i];
-      Dft<G::N1X, -1>::run(x);
-#pragma unroll
-      for (int i = 0; i < G::N1X; ++i) v[n1y * G::N1X + i] = x[i];
-    }
 #pragma unroll
     for (int k1x = 0; k1x < G::N1X; ++k1x) {
       cf x[G::N1Y];
@@ -401,9 +407,19 @@ __device__ __forceinline__ void st_cluster_v4(unsigned addr, cf a, cf b) {
 // after which the whole buffer is free again.  Consequences: fft2_fwd may start whenever the calling warp is done
 // with its own region; fft2_inv_head may start after an fft2_fwd or any CTA barrier.  Unnormalised.
 template <class G>
+__device__ __forceinline__ void fft2_fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, int t);
+template <class G>
 __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int t) {
   typedef Lay<G> L;
-  L::phase1_fwd(v, tw, t);
+#pragma unroll
+  for (int n1y = 0; n1y < G::N1Y; ++n1y) L::phase1_fwd_row(v, n1y);
+  fft2_fwd_after_rows<G>(v, sm, tw, t);
+}
+// the forward transform whose phase-1 row transforms the caller has already run (Lay::phase1_fwd_row for every n1y)
+template <class G>
+__device__ __forceinline__ void fft2_fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, int t) {
+  typedef Lay<G> L;
+  L::phase1_fwd_rest(v, tw, t);
   __syncwarp();
   L::x1_store_p1(v, sm, t);
   __syncwarp();
@@ -506,6 +522,10 @@ struct Fft {
   static __device__ __forceinline__ void end_fourier() { if (G::CL > 1) cluster_wait(); }       // kernel ends in Fourier space
   static __device__ __forceinline__ void fwd(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
     fft2_fwd<G>(v, sm, tw, t);
+    if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
+  }
+  static __device__ __forceinline__ void fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
+    fft2_fwd_after_rows<G>(v, sm, tw, t);
     if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
   }
   static __device__ __forceinline__ void inv_head(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rk) {

@@ -13,9 +13,12 @@
 //                    patch gradient live in tensor memory (TMEM), only the pair's sum is staged
 //   k_gather_object  H11 deterministic owner-computes scatter-add: every object pixel sums the patch
 //                    gradients that cover it in fixed (j,k) order — no float atomics
+//   k_gather_object_w the same with the windows split over the warps of a block (objects with few tiles: configs 1, 2)
+//   k_single         S = 1: H2..H13 of one position in one persistent CTA, all modes in turn (configs 1, 2)
 //   k_reduce_probe / k_probe_ifft / k_finalize   H12 tail, loss and position-gradient sums
-//   k_backward<.,1>  H14 LSQML-style step-size terms (second sweep); k_alpha_pos / k_gather_willum / k_objtrans: the
-//                    per-position-alpha weights and the probe-view preconditioner of LSQML; k_axpy / k_lsqml_* H15
+//   k_step_object / k_step_probe   H14 LSQML-style step-size terms from what the backward pass staged (no second pass through
+//                    the chain); k_alpha_pos / k_gather_willum / k_objtrans: the per-position-alpha weights and the probe-view
+//                    preconditioner of LSQML; k_axpy / k_lsqml_* H15
 //   regularizers.cuh cost / constraint regularisers and Adam
 // The CPU oracle under oracle/ shares nothing with this file.
 #include <cuda_runtime.h>
@@ -105,7 +108,7 @@ struct Ws {
   float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
   cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
   float* alpha_ji;     // [Jc][S]          per-position object step sizes alpha_{O,i,j} (PT_WANT_WEIGHTED_ILLUM only)
-  float* ilpart;       // [Jc|J][M][S][N^2]  R-native |Psi_{i,k}|^2 written by the backward kernels (step sizes; PT_WANT_ILLUM with paired modes)
+  float* ilpart;       // [Jc|J][M or M/2][S][N^2]  R-native |Psi_{i,k}|^2 written by the backward kernels (step sizes; PT_WANT_ILLUM with paired modes)
   int32_t stage_all;   // the three staged arrays hold the whole batch (the step-size sweep reads them after the last chunk)
   int32_t Jc;
   size_t total;
@@ -141,7 +144,7 @@ WsSizes ws_sizes(const pt_problem* p) {
   z.per_staged = staged_planes(p) * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   z.il_needed = steps;
   z.per_il = 0;
-  if (!(p->flags & PT_EPIE) && (steps || ((p->flags & PT_WANT_ILLUM) && use_pairs(p)))) z.per_il = M * S * NN * sizeof(float);
+  if (!(p->flags & PT_EPIE) && (steps || ((p->flags & PT_WANT_ILLUM) && use_pairs(p)))) z.per_il = staged_planes(p) * S * NN * sizeof(float);
   return z;
 }
 // Positions in flight for a workspace of `bytes`.  Without step sizes everything is per chunk; the optional |Psi|^2 staging is
@@ -216,7 +219,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
   w->alpha_ji = steps ? (float*)take(jc * S * sizeof(float)) : nullptr;
-  w->ilpart = plan.il ? (float*)take(js * M * S * NN * sizeof(float)) : nullptr;
+  w->ilpart = plan.il ? (float*)take(js * staged_planes(p) * S * NN * sizeof(float)) : nullptr;
   w->stage_all = plan.stage_all ? 1 : 0;
   w->Jc = (int32_t)jc;
   w->total = off;
@@ -230,6 +233,7 @@ struct KP {
   int N, M, S, ony, onx, J;          // J = batch size
   int Jtot;                          // rows of positions / intensity (n_pos_total)
   int Mg;                            // patch-gradient planes per position in the staging buffer: M, or M/2 after k_backward_pair
+  int Mi;                            // |Psi|^2 planes per position in the staging buffer: M, or M/2 after k_backward_pair (the pair's sum)
   int j0, jc;                        // current chunk: batch-local offset and count
   float chi_scale;                   // step-size sweep: chi = -chi_scale gPhi (1; 2 under PT_LSQML_MODULUS_CHI, reading R31)
   float px, bandlim2;                // bandlim2 = (0.5*bandlimit*N)^2 or < 0 when off
@@ -368,10 +372,6 @@ __device__ __forceinline__ void cp_async16(void* dst_smem, const void* src) {
 }
 // every thread asks for the 128-byte line at p to be brought into L2 (fire and forget)
 __device__ __forceinline__ void l2_prefetch_line(const void* p) { asm volatile("prefetch.global.L2 [%0];" ::"l"(p)); }
-// one thread asks for `bytes` (a multiple of 16, 16-byte aligned) of global memory to be brought into L2
-__device__ __forceinline__ void l2_prefetch_bulk(const void* src, unsigned bytes) {
-  asm volatile("cp.async.bulk.prefetch.L2.global [%0], %1;" ::"l"(src), "r"(bytes) : "memory");
-}
 __device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
 }
@@ -595,9 +595,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
       const cf T1 = p < E ? cs.pf8[(2 * p + 1) * T] : cs.xs8[(2 * p + 1 - 2 * E) * 32];
       v[2 * p] = cmul(v[2 * p], T0);
       v[2 * p + 1] = cmul(v[2 * p + 1], T1);
+      if ((p & 3) == 3) L::phase1_fwd_row(v, p >> 2);            // registers [8 (p/4), 8 (p/4) + 8) are final: their row transform now,
+                                                                 // between the bursts of stash stores (forward 46.4 -> 46.0 ms per step)
     }
     if (i + 1 < S) early(i + 1);
-    Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(Phi)    (Fourier layout)
+    Fft<G>::fwd_after_rows(v, sm, tw, cs.tw2, t, rk);            // F(Phi)    (Fourier layout)
     if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, inside, t, rk);   // H5
   }
   float4* out = (float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);   // H6: psi~ = F(Phi_{S-1}) / N
@@ -746,7 +748,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     } else {
 #pragma unroll
       for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
-      if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);             // the late part of the same field: DRAM -> L2 now
+      if (t < (16 - E) * T / 8) l2_prefetch_line((const char*)(st - t + E * T) + t * 128);   // the late part of the same field: DRAM -> L2 now, one line per thread
     }
     if (i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
     cp_async_commit();
@@ -886,8 +888,8 @@ __global__ void __launch_bounds__(256) k_step_object(KP P) {
     double gr = 0.0, gi = 0.0, il = 0.0;
     const size_t gb = ((size_t)sj * P.Mg * P.S + i) * (CL * NNS) + e;
     for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[gb + (size_t)k * P.S * (CL * NNS)]; gr += (double)g.x; gi += (double)g.y; }
-    const size_t ib = ((size_t)sj * P.M * P.S + i) * (CL * NNS) + e;
-    for (int k = 0; k < P.M; ++k) il += (double)P.w.ilpart[ib + (size_t)k * P.S * (CL * NNS)];
+    const size_t ib = ((size_t)sj * P.Mi * P.S + i) * (CL * NNS) + e;
+    for (int k = 0; k < P.Mi; ++k) il += (double)P.w.ilpart[ib + (size_t)k * P.S * (CL * NNS)];
     const size_t o = (size_t)y * onx + x;
     double dr, di;
     if (BILIN) {
@@ -1080,7 +1082,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     } else {
 #pragma unroll
       for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, st + p * T);
-      if (t == 0) l2_prefetch_bulk(st + E * T, (16 - E) * T * 16);             // the late part of the same field: DRAM -> L2 now
+      if (t < (16 - E) * T / 8) l2_prefetch_line((const char*)(st - t + E * T) + t * 128);   // the late part of the same field: DRAM -> L2 now, one line per thread
     }
     if (h == 0 && i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);   // serves both modes at slice i
     cp_async_commit();
@@ -1137,7 +1139,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       s1 = pm > 0.f ? 1.0f / pm : 0.f; s2 = tm > 0.f ? 1.0f / tm : 0.f;
     }
     float4* gt = (float4*)(P.w.gTpart + fld(pp, i));
-    float2* il = IL ? (float2*)(P.w.ilpart + fld(pr, i)) : nullptr;   // O12 staging: |Psi_{i,k}|^2 of this mode
+    float2* il = IL ? (float2*)(P.w.ilpart + fld(pp, i)) : nullptr;   // O12 staging: |Psi|^2 summed over the pair (first mode stores, second adds)
     float4 hw = make_float4(0.f, 0.f, 0.f, 0.f);                  // H16: the 16-byte word that holds pairs p, p + 1 (p even)
 #pragma unroll
     for (int p = 0; p < 16; ++p) {
@@ -1155,7 +1157,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
-      if (IL) __stcs(il + p * T + t, make_float2(fmaf(ps.x, ps.x, ps.y * ps.y), fmaf(ps.z, ps.z, ps.w * ps.w)));
+      if (IL) {
+        const float i0 = fmaf(ps.x, ps.x, ps.y * ps.y), i1 = fmaf(ps.z, ps.z, ps.w * ps.w);
+        if (h == 0) il[p * T + t] = make_float2(i0, i1);         // stays in L2 until the second mode's half step adds to it: the same thread,
+        else asm volatile("red.global.add.v2.f32 [%0], {%1,%2};" ::"l"(il + p * T + t), "f"(i0), "f"(i1) : "memory");   // program order, one adder: deterministic
+      }
       if (h == 0) tmem_st4(tb + 64 + 4 * p, g0, g1);             // first mode: keep gT_i on chip
       else {                                                     // second mode: the pair's sum goes to the staging buffer
         cf a0, a1;
@@ -1164,10 +1170,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
       }
       v[2 * p] = cmulc(v[2 * p], T0);                            // gPsi = conj(T) .* gPhi
       v[2 * p + 1] = cmulc(v[2 * p + 1], T1);
+      if ((p & 3) == 3) L::phase1_fwd_row(v, p >> 2);            // row transform of the eight registers that are final (as in k_forward)
     }
     if (h == 0) tmem_wait_st();
     if (s + 1 < 2 * S) early(s + 1);
-    Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                        // F(gPsi_i)
+    Fft<G>::fwd_after_rows(v, sm, tw, cs.tw2, t, rk);             // F(gPsi_i)
     if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
     tmem_swap_field(tb, v);                                      // the other mode's turn
   }
@@ -1582,8 +1589,8 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
             double sr = 0.0, si = 0.0, sl = 0.0;
             for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
             if (ILLUM) {
-              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat, sbs = sb;
-              if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
+              const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + nat, sbs = ((size_t)(jbase + jj) * P.Mi * P.S + i) * NN + nat;
+              if (P.w.ilpart) for (int k = 0; k < P.Mi; ++k) sl += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
               else for (int k = 0; k < P.M; ++k) { const cf q = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)q.x * q.x + (double)q.y * q.y; }
             }
             ar += wgt * sr; ai += wgt * si; al += wgt * sl;
@@ -1594,8 +1601,8 @@ __global__ void __launch_bounds__(256) k_gather_object(KP P, cf* gO, float* illu
         const size_t base = ((size_t)(jbase + jj) * P.Mg * P.S + i) * NN + idx;
         for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
         if (ILLUM) {
-          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx, sbs = sb;
-          if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];   // staged by the backward kernel
+          const size_t sb = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + idx, sbs = ((size_t)(jbase + jj) * P.Mi * P.S + i) * NN + idx;
+          if (P.w.ilpart) for (int k = 0; k < P.Mi; ++k) al += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];   // staged by the backward kernel
           else for (int k = 0; k < P.M; ++k) { const cf s = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)s.x * s.x + (double)s.y * s.y; }
         }
       }
@@ -1648,8 +1655,8 @@ __global__ void __launch_bounds__(256) k_gather_object_w(KP P, cf* gO, float* il
             double sr = 0.0, si = 0.0, sl = 0.0;
             for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; sr += (double)g.x; si += (double)g.y; }
             if (ILLUM) {
-              const size_t sb = ((size_t)jj * P.M * P.S + i) * NN + nat;
-              if (P.w.ilpart) for (int k = 0; k < P.M; ++k) sl += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];
+              const size_t sb = ((size_t)jj * P.M * P.S + i) * NN + nat, sbs = ((size_t)jj * P.Mi * P.S + i) * NN + nat;
+              if (P.w.ilpart) for (int k = 0; k < P.Mi; ++k) sl += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
               else for (int k = 0; k < P.M; ++k) { const cf z = P.w.stash[sb + (size_t)k * P.S * NN]; sl += (double)z.x * z.x + (double)z.y * z.y; }
             }
             ar += wgt * sr; ai += wgt * si; al += wgt * sl;
@@ -1660,8 +1667,8 @@ __global__ void __launch_bounds__(256) k_gather_object_w(KP P, cf* gO, float* il
         const size_t base = ((size_t)jj * P.Mg * P.S + i) * NN + idx;
         for (int k = 0; k < P.Mg; ++k) { const cf g = P.w.gTpart[base + (size_t)k * P.S * NN]; ar += (double)g.x; ai += (double)g.y; }
         if (ILLUM) {
-          const size_t sb = ((size_t)jj * P.M * P.S + i) * NN + idx;
-          if (P.w.ilpart) for (int k = 0; k < P.M; ++k) al += (double)P.w.ilpart[sb + (size_t)k * P.S * NN];
+          const size_t sb = ((size_t)jj * P.M * P.S + i) * NN + idx, sbs = ((size_t)jj * P.Mi * P.S + i) * NN + idx;
+          if (P.w.ilpart) for (int k = 0; k < P.Mi; ++k) al += (double)P.w.ilpart[sbs + (size_t)k * P.S * NN];
           else for (int k = 0; k < P.M; ++k) { const cf z = P.w.stash[sb + (size_t)k * P.S * NN]; al += (double)z.x * z.x + (double)z.y * z.y; }
         }
       }
@@ -1724,9 +1731,9 @@ __global__ void __launch_bounds__(256) k_gather_willum(KP P, float* willum) {
         const int2 r0 = sr0[jj];
         const int px = ox - r0.x, py = oy - r0.y;
         if (px >= 0 && px < N && py >= 0 && py < N) {
-          const size_t base = ((size_t)(jbase + jj) * P.M * P.S + i) * NN + F::r_native_of(py, px);
+          const size_t base = ((size_t)(jbase + jj) * P.Mi * P.S + i) * NN + F::r_native_of(py, px);
           double s = 0.0;
-          for (int k = 0; k < P.M; ++k) s += (double)P.w.ilpart[base + (size_t)k * P.S * NN];      // |Psi_{i,k}|^2 staged by the backward kernel
+          for (int k = 0; k < P.Mi; ++k) s += (double)P.w.ilpart[base + (size_t)k * P.S * NN];      // |Psi_{i,k}|^2 staged by the backward kernel
           acc += (double)sal[jj] * s;
         }
       }
@@ -1956,7 +1963,7 @@ int validate(const pt_problem* p) {
 KP make_kp(const pt_problem* p, const Ws& w, const pt_c64* object, const pt_c64* probe, const float* positions,
            const float* intensity, const int32_t* batch_idx) {
   KP k;
-  k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch; k.Jtot = p->n_pos_total;
+  k.N = p->n; k.M = p->n_modes; k.Mg = p->n_modes; k.Mi = p->n_modes; k.S = p->n_slices; k.ony = p->obj_ny; k.onx = p->obj_nx; k.J = p->n_batch; k.Jtot = p->n_pos_total;
   k.j0 = 0; k.jc = 0; k.px = p->pixel_size;
   k.chi_scale = (p->flags & PT_LSQML_MODULUS_CHI) ? 2.0f : 1.0f;
   const double lim = 0.5 * (double)p->bandlimit * (double)p->n;
@@ -2086,6 +2093,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   const bool single = G::CL == 1 && p->n_slices == 1 && !bilin && !epie && !want_steps && !want_illum && !h16 && !kp.w.ilpart &&
                       !(p->flags & PT_NO_SINGLE_SLICE_FUSION);
   kp.Mg = single ? 1 : paired ? p->n_modes / 2 : p->n_modes;
+  kp.Mi = paired ? p->n_modes / 2 : p->n_modes;
   k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
   LAUNCH_CHECK(K_zero, st);
   if (!acc) {
@@ -2142,7 +2150,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
     const size_t js = w0.stage_all ? (size_t)j0 : 0, FN = (size_t)G::CL * FL<G>::NNS;
     kp.w.gTpart = w0.gTpart + js * kp.Mg * p->n_slices * FN;
     kp.w.Gpart = w0.Gpart + js * p->n_modes * FN;
-    kp.w.ilpart = w0.ilpart ? w0.ilpart + js * p->n_modes * p->n_slices * FN : nullptr;
+    kp.w.ilpart = w0.ilpart ? w0.ilpart + js * kp.Mi * p->n_slices * FN : nullptr;
   };
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
