@@ -126,6 +126,7 @@ template <> struct Geo<256> {
 template <class G>
 struct Lay {
   static constexpr int N = G::N, T = G::T;
+  struct NoHook { PTK_HD void operator()(int) const {} };
   // The exchange buffer is one region of X1_WARP float2 slots per warp.  X1 (warp-local) lives in the calling
   // warp's region; X2 is laid out so that its "p2" side (warp w holds rows b = w*LP2 .. w*LP2+LP2-1 of every
   // k1y plane) also touches ONLY the calling warp's region: slot(b, k1y, qx) = (b / LP2)*X1_WARP +
@@ -184,7 +185,9 @@ struct Lay {
     for (int n1y = 0; n1y < G::N1Y; ++n1y) phase1_fwd_row(v, n1y);
     phase1_fwd_rest(v, tw, t);
   }
-  static PTK_HD void phase1_fwd_rest(cf (&v)[32], const cf* tw, int t) {
+  static PTK_HD void phase1_fwd_rest(cf (&v)[32], const cf* tw, int t) { phase1_fwd_rest_h(v, tw, t, NoHook()); }
+  template <class Hook>
+  static PTK_HD void phase1_fwd_rest_h(cf (&v)[32], const cf* tw, int t, Hook hook) {   // hook(step), step = 0 .. N1X - 1, after each column
     const int a = t & (G::N2X - 1), b = t >> G::LX2;
 #pragma unroll
     for (int k1x = 0; k1x < G::N1X; ++k1x) {
@@ -199,6 +202,7 @@ struct Lay {
       }
 #pragma unroll
       for (int i = 0; i < G::N1Y; ++i) v[i * G::N1X + k1x] = x[i];
+      hook(k1x);
     }
 #pragma unroll
     for (int k1y = 1; k1y < G::N1Y; ++k1y) {
@@ -207,8 +211,12 @@ struct Lay {
       for (int k1x = 0; k1x < G::N1X; ++k1x) v[k1y * G::N1X + k1x] = cmul(v[k1y * G::N1X + k1x], wy);
     }
   }
-  // ---- phase 1 (inverse): (k1y, k1x) regs -> R-layout regs
-  static PTK_HD void phase1_inv(cf (&v)[32], const cf* tw, int t) {
+  // ---- phase 1 (inverse): (k1y, k1x) regs -> R-layout regs.  phase1_inv_h calls hook(step), step = 0 .. N1X + N1Y - 1, between its
+  // column and row transforms: the chain kernels issue their asynchronous copies there, a few per step, instead of in one burst
+  // before the arithmetic (the copy instructions queue behind one another; spread out, the arithmetic issues meanwhile).
+  static PTK_HD void phase1_inv(cf (&v)[32], const cf* tw, int t) { phase1_inv_h(v, tw, t, NoHook()); }
+  template <class Hook>
+  static PTK_HD void phase1_inv_h(cf (&v)[32], const cf* tw, int t, Hook hook) {
     const int a = t & (G::N2X - 1), b = t >> G::LX2;
 #pragma unroll
     for (int k1y = 1; k1y < G::N1Y; ++k1y) {
@@ -229,6 +237,7 @@ struct Lay {
       Dft<G::N1Y, +1>::run(x);
 #pragma unroll
       for (int i = 0; i < G::N1Y; ++i) v[i * G::N1X + k1x] = x[i];
+      hook(k1x);
     }
 #pragma unroll
     for (int n1y = 0; n1y < G::N1Y; ++n1y) {
@@ -238,6 +247,7 @@ struct Lay {
       Dft<G::N1X, +1>::run(x);
 #pragma unroll
       for (int i = 0; i < G::N1X; ++i) v[n1y * G::N1X + i] = x[i];
+      hook(G::N1X + n1y);
     }
   }
   // ---- phase 2: LP2 lines of N2X points (reg = line*N2X + point)
@@ -416,10 +426,16 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   fft2_fwd_after_rows<G>(v, sm, tw, t);
 }
 // the forward transform whose phase-1 row transforms the caller has already run (Lay::phase1_fwd_row for every n1y)
+template <class G, class Hook>
+__device__ __forceinline__ void fft2_fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, int t, Hook hook);
 template <class G>
 __device__ __forceinline__ void fft2_fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, int t) {
+  fft2_fwd_after_rows_h<G>(v, sm, tw, t, typename Lay<G>::NoHook());
+}
+template <class G, class Hook>
+__device__ __forceinline__ void fft2_fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, int t, Hook hook) {
   typedef Lay<G> L;
-  L::phase1_fwd_rest(v, tw, t);
+  L::phase1_fwd_rest_h(v, tw, t, hook);
   __syncwarp();
   L::x1_store_p1(v, sm, t);
   __syncwarp();
@@ -526,6 +542,11 @@ struct Fft {
   }
   static __device__ __forceinline__ void fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
     fft2_fwd_after_rows<G>(v, sm, tw, t);
+    if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
+  }
+  template <class Hook>
+  static __device__ __forceinline__ void fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk, Hook hook) {
+    fft2_fwd_after_rows_h<G>(v, sm, tw, t, hook);
     if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
   }
   static __device__ __forceinline__ void inv_head(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rk) {

@@ -775,18 +775,23 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
 #pragma unroll
       for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
       cp_async_commit();
-    } else {     // late: the rest of the stash, and T pairs [0, E), into the warp's idle X1 region
+      L::phase1_inv(v, tw, t);                                   // gPhi_{i,k}  (R-layout)
+    } else {
+      // late: the rest of the stash and T pairs [0, E) into the warp's idle X1 region, T registers [2E, 32) (no slot left in shared
+      // memory) by plain loads: 38 instructions per thread, a few between the steps of phase 1 instead of one burst before it
       const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
+      constexpr int NQ = (16 - E) + 2 * E + (32 - 2 * E), NH = G::N1X + G::N1Y;
+      auto item = [&](int q) {
+        if (q < 16 - E) cp_async16(cs.xs + q * 32, st + (E + q) * T);
+        else if (q < 16 - E + 2 * E) { const int r = q - (16 - E); cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx)); }
+        else { const int r = 2 * E + (q - (16 - E) - 2 * E); Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx)); }
+      };
+      L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout)
 #pragma unroll
-      for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
-#pragma unroll
-      for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
+        for (int q = 0; q < NQ; ++q) if (q * NH / NQ == step) item(q);
+      });
       cp_async_commit();
-      // T registers [2E, 32) have no slot left in shared memory: plain loads, issued a whole phase ahead of their use
-#pragma unroll
-      for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
     }
-    L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     // ePIE (MODE 2): dO = conj(Psi) / max|Psi|^2 chi ; chi' = conj(T) / max|T|^2 chi
     float s1 = 1.0f, s2 = 1.0f;
@@ -1115,21 +1120,26 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     const cf* o = ob + (size_t)i * slice;
     cf Tr[H16 ? 1 : 32 - 2 * E];
-    if (H16) {   // all of T_i into the warp's idle X1 region (the stash is in the early slots)
+    if (H16) {
 #pragma unroll
       for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
       cp_async_commit();
+      L::phase1_inv(v, tw, t);
     } else {
+      // the late copies and direct loads (38 instructions per thread), a few between the steps of phase 1 instead of one burst before it
       const float4* st = (const float4*)(P.w.stash + fld(pr, i)) + t;
+      constexpr int NQ = (16 - E) + 2 * E + (32 - 2 * E), NH = G::N1X + G::N1Y;
+      auto item = [&](int q) {
+        if (q < 16 - E) cp_async16(cs.xs + q * 32, st + (E + q) * T);
+        else if (q < 16 - E + 2 * E) { const int r = q - (16 - E); cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx)); }
+        else { const int r = 2 * E + (q - (16 - E) - 2 * E); Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx)); }
+      };
+      L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout); backward 56.4 -> 55.5 ms per step
 #pragma unroll
-      for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, st + p * T);
-#pragma unroll
-      for (int r = 0; r < 2 * E; ++r) cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx));
+        for (int q = 0; q < NQ; ++q) if (q * NH / NQ == step) item(q);
+      });
       cp_async_commit();
-#pragma unroll
-      for (int r = 2 * E; r < 32; ++r) Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx));
     }
-    L::phase1_inv(v, tw, t);                                     // gPhi_{i,k}  (R-layout)
     cp_async_wait_all();
     float s1 = 1.0f, s2 = 1.0f;
     if (MODE == 2) {
