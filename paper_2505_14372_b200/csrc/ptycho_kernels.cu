@@ -96,6 +96,8 @@ struct Ws {
   double* step_oi;     // [J][S][6]       step-size sweep: (numO, denO) of slice i; bilinear mode also (numX_y, denX_y, numX_x, denX_x)
   double* step_pp;     // [J][M][CL][6]   step-size sweep: (numP, denP, numX_y, denX_y, numX_x, denX_x) of one mode (and rank)
   cf* dOhat;           // [S][ony][onx]      (step sizes only)
+  float4* O2;          // [S][ony][onx]      the object with its partner: O2[y][x] = (O[y][x], O[y][x + D]), D = the distance of a thread's
+                       //                    registers 2p, 2p + 1 in the patch (k_pair_object): one 16-byte copy brings both
   // chunked
   cf* psit;            // [Jc][M][N^2]  F-native
   float* wdet;         // [Jc][N^2]     F-native
@@ -106,7 +108,8 @@ struct Ws {
   cf* Gpart;           // [Jc|J][M][N^2]     F-native
   float* psimax;       // [Jc][M][S][CL]   ePIE: max |Psi_{i,k}|^2 of each rank's block (PT_EPIE only)
   float* tmax;         // [Jc][S]          ePIE: max |O_i|^2 over the window
-  cf* Tb;              // [Jc][S][N^2]     raster: bilinearly sampled patches (PT_SHIFT_BILINEAR_OBJECT only)
+  float4* Tb;          // [Jc][S][N^2]     raster: bilinearly sampled patches, each with its partner D pixels to the right, as O2
+                       //                  (PT_SHIFT_BILINEAR_OBJECT only)
   float* alpha_ji;     // [Jc][S]          per-position object step sizes alpha_{O,i,j} (PT_WANT_WEIGHTED_ILLUM only)
   float* ilpart;       // [Jc|J][M or M/2][S][N^2]  R-native |Psi_{i,k}|^2 written by the backward kernels (step sizes; PT_WANT_ILLUM with paired modes)
   int32_t stage_all;   // the three staged arrays hold the whole batch (the step-size sweep reads them after the last chunk)
@@ -134,12 +137,13 @@ WsSizes ws_sizes(const pt_problem* p) {
   f += align_up(J * CL * sizeof(double)) + align_up(J * M * CL * 2 * sizeof(double));
   f += align_up(J * S * 6 * sizeof(double)) + align_up(J * M * CL * 6 * sizeof(double));
   if (steps) f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf));
+  f += align_up(S * (size_t)p->obj_ny * p->obj_nx * sizeof(float4));
   WsSizes z;
   z.fixed = f + 13 * 256;   // slack for the per-array alignment of the chunked part
   const size_t stash_el = (p->flags & PT_STASH_FP16) ? sizeof(cf) / 2 : sizeof(cf);   // binary16 pairs: 4 bytes per complex
   z.per_chunk = M * NN * sizeof(cf) + NN * sizeof(float) + M * S * NN * stash_el;
   if (steps) z.per_chunk += S * sizeof(float);
-  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) z.per_chunk += S * NN * sizeof(cf);
+  if (p->shift_mode == PT_SHIFT_BILINEAR_OBJECT) z.per_chunk += S * NN * sizeof(float4);
   if (p->flags & PT_EPIE) z.per_chunk += (M * CL + 1) * S * sizeof(float) + 64;
   z.per_staged = staged_planes(p) * S * NN * sizeof(cf) + M * NN * sizeof(cf);
   z.il_needed = steps;
@@ -210,6 +214,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->step_oi = (double*)take(J * S * 6 * sizeof(double));
   w->step_pp = (double*)take(J * M * CL * 6 * sizeof(double));
   w->dOhat = steps ? (cf*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(cf)) : nullptr;
+  w->O2 = (float4*)take(S * (size_t)p->obj_ny * p->obj_nx * sizeof(float4));
   w->psit = (cf*)take(jc * M * NN * sizeof(cf));
   w->wdet = (float*)take(jc * NN * sizeof(float));
   w->stash = (cf*)take(jc * M * S * NN * ((p->flags & PT_STASH_FP16) ? sizeof(cf) / 2 : sizeof(cf)));
@@ -217,7 +222,7 @@ int ws_layout(const pt_problem* p, void* base, size_t bytes, Ws* w) {
   w->Gpart = (cf*)take(js * M * NN * sizeof(cf));
   w->psimax = (p->flags & PT_EPIE) ? (float*)take(jc * M * S * CL * sizeof(float)) : nullptr;
   w->tmax = (p->flags & PT_EPIE) ? (float*)take(jc * S * sizeof(float)) : nullptr;
-  w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (cf*)take(jc * S * NN * sizeof(cf)) : nullptr;
+  w->Tb = p->shift_mode == PT_SHIFT_BILINEAR_OBJECT ? (float4*)take(jc * S * NN * sizeof(float4)) : nullptr;
   w->alpha_ji = steps ? (float*)take(jc * S * sizeof(float)) : nullptr;
   w->ilpart = plan.il ? (float*)take(js * staged_planes(p) * S * NN * sizeof(float)) : nullptr;
   w->stage_all = plan.stage_all ? 1 : 0;
@@ -310,6 +315,15 @@ __global__ void k_setup_pos(KP P) {
   P.w.ramps[((size_t)jb * 2 + 1) * N + q] = make_float2(c, s);     // ry
 }
 
+// O2[y][x] = (O[y][x], O[y][x + D]) for every slice (zero where x + D leaves the row: no window reads those as a first element)
+__global__ void k_pair_object(KP P, int D) {
+  const size_t n = (size_t)P.S * P.ony * P.onx, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int x = (int)(i % P.onx);
+  const cf a = P.object[i], b = x + D < P.onx ? P.object[i + D] : make_float2(0.f, 0.f);
+  P.w.O2[i] = make_float4(a.x, a.y, b.x, b.y);
+}
+
 // ------------------------------------------------------------------------------------------------
 // block-wide deterministic sum of NV doubles per thread; result valid in thread 0
 // ------------------------------------------------------------------------------------------------
@@ -350,16 +364,13 @@ template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::X
 template <class G> constexpr size_t chain_smem_bytes() { return fft_smem_bytes<G>() + (size_t)2 * G::NF * sizeof(cf) + (size_t)G::PF16 * G::T * 16; }
 template <class G>
 struct ChainSmem {
-  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs; cf* pf8; cf* xs8;
+  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs;
   __device__ __forceinline__ ChainSmem(unsigned char* raw, int t) {
     typedef Lay<G> L;
     sm = (cf*)raw; tw = sm + L::XBUF; tw2 = tw + L::TW; red = (double*)(tw2 + (G::CL > 1 ? G::N : 0));
     hyS = (cf*)((unsigned char*)red + 1024);
     pf = (float4*)(hyS + 2 * G::NF) + t;                                // early 16-byte slot s: pf[s * T]
     xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late 16-byte slot s:  xs[s * 32]
-    // the same two regions viewed as 8-byte slots (lanes 8 bytes apart: conflict-free cp.async writes and reads)
-    pf8 = (cf*)(hyS + 2 * G::NF) + t;                                   // early 8-byte slot s: pf8[s * T]
-    xs8 = sm + (t >> 5) * L::X1_WARP + (t & 31);                        // late 8-byte slot s:  xs8[s * 32]
   }
   // twiddle tables; the caller synchronises the CTA before the first transform
   __device__ __forceinline__ void fill_tables(int t) {
@@ -375,12 +386,6 @@ __device__ __forceinline__ void l2_prefetch_line(const void* p) { asm volatile("
 __device__ __forceinline__ void cp_async8(void* dst_smem, const void* src) {
   asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((unsigned)__cvta_generic_to_shared(dst_smem)), "l"(src) : "memory");
 }
-// 8-byte read-only load pinned where it is written (asm volatile keeps its place among the other memory operations)
-__device__ __forceinline__ cf ld_nc8(const cf* p) {
-  cf v;
-  asm volatile("ld.global.nc.v2.f32 {%0, %1}, [%2];" : "=f"(v.x), "=f"(v.y) : "l"(p));
-  return v;
-}
 // reduced-precision stash (PT_STASH_FP16): four complex64 <-> eight binary16 in one 16-byte word, round to nearest even
 __device__ __forceinline__ uint32_t pack_h2(float a, float b) {
   uint32_t r; asm("cvt.rn.f16x2.f32 %0, %1, %2;" : "=r"(r) : "f"(b), "f"(a)); return r;     // low half = a
@@ -389,6 +394,12 @@ __device__ __forceinline__ cf unpack_h2(uint32_t u) {
   float lo, hi;
   asm("{.reg .f16 l, h; mov.b32 {l, h}, %2; cvt.f32.f16 %0, l; cvt.f32.f16 %1, h;}" : "=f"(lo), "=f"(hi) : "r"(u));
   return make_float2(lo, hi);
+}
+// 16-byte read-only load pinned where it is written (asm volatile keeps its place among the other memory operations)
+__device__ __forceinline__ float4 ld_nc16(const float4* p) {
+  float4 v;
+  asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(v.x), "=f"(v.y), "=f"(v.z), "=f"(v.w) : "l"(p));
+  return v;
 }
 __device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void cp_async_wait_all() { asm volatile("cp.async.wait_all;" ::: "memory"); }
@@ -544,13 +555,13 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   // patch source: the object window itself, or (bilinear mode) this position's resampled patches [S][NF][NF]
   const int S = P.S, onx = P.bilinear ? NF : P.onx;
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
-  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) +
-                 (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);   // this thread's first pixel, slice 0
-  // H3 prefetch: patch values of registers [0, 2E) one FFT pair ahead into the thread's early slots
+  const float4* ob2 = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : P.w.O2 + ((size_t)r0y * P.onx + r0x)) +
+                      (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);   // this thread's first pixel (with its partner), slice 0
+  // H3 prefetch: patch values of register pairs [0, E) one FFT pair ahead into the thread's early slots
   auto early = [&](int i) {
-    const cf* o = ob + (size_t)i * slice;
+    const float4* o2 = ob2 + (size_t)i * slice;
 #pragma unroll
-    for (int r = 0; r < 2 * E; ++r) cp_async8(cs.pf8 + r * T, o + F::patch_off(r, onx));
+    for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, o2 + F::patch_off(2 * p, onx));
     if (i < S - 1 && t < NF) cp_async8(cs.hyS + (i & 1) * NF + t, P.w.hy + (size_t)i * NF + t);
     cp_async_commit();
   };
@@ -574,9 +585,9 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
   for (int i = 0; i < S; ++i) {
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
     {   // registers [2E, 32) of T_i into the warp's idle X1 region
-      const cf* o = ob + (size_t)i * slice;
+      const float4* o2 = ob2 + (size_t)i * slice;
 #pragma unroll
-      for (int r = 2 * E; r < 32; ++r) cp_async8(cs.xs8 + (r - 2 * E) * 32, o + F::patch_off(r, onx));
+      for (int p = E; p < 16; ++p) cp_async16(cs.xs + (p - E) * 32, o2 + F::patch_off(2 * p, onx));
       cp_async_commit();
     }
     L::phase1_inv(v, tw, t);                                     // Psi_{i,k}  (R-layout)
@@ -591,8 +602,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
         if (p & 1) __stcs(st + (p >> 1) * T + t, make_float4(hprev0, hprev1, h0, h1));
         else { hprev0 = h0; hprev1 = h1; }
       }
-      const cf T0 = p < E ? cs.pf8[(2 * p) * T] : cs.xs8[(2 * p - 2 * E) * 32];
-      const cf T1 = p < E ? cs.pf8[(2 * p + 1) * T] : cs.xs8[(2 * p + 1 - 2 * E) * 32];
+      const float4 tt = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];   // (T[2p], T[2p+1]): one 16-byte slot (k_pair_object)
+      const cf T0 = make_float2(tt.x, tt.y), T1 = make_float2(tt.z, tt.w);
       v[2 * p] = cmul(v[2 * p], T0);
       v[2 * p + 1] = cmul(v[2 * p + 1], T1);
       if ((p & 3) == 3) L::phase1_fwd_row(v, p >> 2);            // registers [8 (p/4), 8 (p/4) + 8) are final: their row transform now,
@@ -738,7 +749,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
   auto fld = [&](int pr, int i) { return (((size_t)pr * S + i) * CL + rk) * NNS; };   // field (index pr, slice i), this rank's block
   const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
-  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
+  const float4* ob2 = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : P.w.O2 + ((size_t)r0y * P.onx + r0x)) + pix0;   // first pixel with its partner
   // stash pairs [0, E) of slice i one FFT pair ahead; hy table of the propagation that ends iteration i
   auto early = [&](int i) {
     const float4* st = (const float4*)(P.w.stash + fld(pair, i) / (H16 ? 2 : 1)) + t;
@@ -769,22 +780,22 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
   }
   for (int i = S - 1; i >= 0; --i) {
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
-    const cf* o = ob + (size_t)i * slice;
-    cf Tr[H16 ? 1 : 32 - 2 * E];
+    const float4* o2 = ob2 + (size_t)i * slice;
+    float4 Tr[H16 ? 1 : 16 - E];                                  // patch pairs [E, 16): no slot left in shared memory
     if (H16) {   // late: all of T_i into the warp's idle X1 region (the stash is in the early slots)
 #pragma unroll
-      for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
+      for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, o2 + F::patch_off(2 * p, onx));
       cp_async_commit();
       L::phase1_inv(v, tw, t);                                   // gPhi_{i,k}  (R-layout)
     } else {
       // late: the rest of the stash and T pairs [0, E) into the warp's idle X1 region, T registers [2E, 32) (no slot left in shared
-      // memory) by plain loads: 38 instructions per thread, a few between the steps of phase 1 instead of one burst before it
+      // memory) by plain loads: 22 instructions per thread, a few between the steps of phase 1 instead of one burst before it
       const float4* st = (const float4*)(P.w.stash + fld(pair, i)) + t;
-      constexpr int NQ = (16 - E) + 2 * E + (32 - 2 * E), NH = G::N1X + G::N1Y;
+      constexpr int NQ = (16 - E) + E + (16 - E), NH = G::N1X + G::N1Y;
       auto item = [&](int q) {
         if (q < 16 - E) cp_async16(cs.xs + q * 32, st + (E + q) * T);
-        else if (q < 16 - E + 2 * E) { const int r = q - (16 - E); cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx)); }
-        else { const int r = 2 * E + (q - (16 - E) - 2 * E); Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx)); }
+        else if (q < 16) { const int p = q - (16 - E); cp_async16(cs.xs + (16 - E + p) * 32, o2 + F::patch_off(2 * p, onx)); }
+        else { const int p = E + (q - 16); Tr[p - E] = ld_nc16(o2 + F::patch_off(2 * p, onx)); }
       };
       L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout)
 #pragma unroll
@@ -812,11 +823,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         if (!(p & 1)) hw = cs.pf[(p >> 1) * T];
         const cf a = unpack_h2(__float_as_uint((p & 1) ? hw.z : hw.x)), b = unpack_h2(__float_as_uint((p & 1) ? hw.w : hw.y));
         ps = make_float4(a.x, a.y, b.x, b.y);
-        T0 = cs.xs8[(2 * p) * 32]; T1 = cs.xs8[(2 * p + 1) * 32];
+        const float4 tt = cs.xs[p * 32];
+        T0 = make_float2(tt.x, tt.y); T1 = make_float2(tt.z, tt.w);
       } else {
         ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
-        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+        const float4 tt = p < E ? cs.xs[(16 - E + p) * 32] : Tr[p - E];
+        T0 = make_float2(tt.x, tt.y); T1 = make_float2(tt.z, tt.w);
       }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
@@ -942,8 +954,9 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_step_probe(KP P) {
   const int spair = pair;
   const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
   const int onx = P.bilinear ? NF : P.onx;
-  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * P.S * F::NNF : patch_ptr(P, 0, r0y, r0x)) +
-                 (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);          // T_0, this thread's first pixel
+  const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);     // this thread's first pixel
+  const cf* ob = patch_ptr(P, 0, r0y, r0x) + pix0;                               // T_0: the object window, or (bilinear mode) the first
+  const float4* ob2 = P.bilinear ? P.w.Tb + (size_t)jl * P.S * F::NNF + pix0 : nullptr;   // halves of this position's sampled pairs
   const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
   const cf* ry = rx + NF;
   const cf* pt = P.w.Pt + ((size_t)k * CL + rk) * NNS;
@@ -988,7 +1001,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_step_probe(KP P) {
     float den = 0.f;
 #pragma unroll
     for (int r = 0; r < 32; ++r) {
-      const cf u = cmul(v[r], ob[F::patch_off(r, onx)]);
+      cf T0;
+      if (P.bilinear) { const float4 q = ob2[F::patch_off(r, onx)]; T0 = make_float2(q.x, q.y); }
+      else T0 = ob[F::patch_off(r, onx)];
+      const cf u = cmul(v[r], T0);
       den = fmaf(u.x, u.x, fmaf(u.y, u.y, den));
     }
     double acc[1] = {(double)den};
@@ -1076,7 +1092,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   const size_t slice = P.bilinear ? (size_t)F::NNF : (size_t)P.ony * P.onx;
   auto fld = [&](int pr, int i) { return (((size_t)pr * S + i) * CL + rk) * NNS; };   // field (index pr, slice i), this rank's block
   const size_t pix0 = (size_t)F::pix_y(rk, t, 0) * onx + F::pix_x(rk, t, 0);
-  const cf* ob = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : patch_ptr(P, 0, r0y, r0x)) + pix0;
+  const float4* ob2 = (P.bilinear ? P.w.Tb + (size_t)jl * S * F::NNF : P.w.O2 + ((size_t)r0y * P.onx + r0x)) + pix0;   // first pixel with its partner
   // half step s = 0 .. 2S-1: mode h = s & 1 of the pair at slice i = S-1 - (s >> 1)
   auto early = [&](int s) {
     const int h = s & 1, i = S - 1 - (s >> 1);
@@ -1118,21 +1134,21 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
   for (int s = 0; s < 2 * S; ++s) {
     const int h = s & 1, i = S - 1 - (s >> 1), pr = pair0 + h;
     Fft<G>::inv_head(v, sm, cs.tw2, t, rk);
-    const cf* o = ob + (size_t)i * slice;
-    cf Tr[H16 ? 1 : 32 - 2 * E];
+    const float4* o2 = ob2 + (size_t)i * slice;
+    float4 Tr[H16 ? 1 : 16 - E];                                  // patch pairs [E, 16): no slot left in shared memory
     if (H16) {
 #pragma unroll
-      for (int r = 0; r < 32; ++r) cp_async8(cs.xs8 + r * 32, o + F::patch_off(r, onx));
+      for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, o2 + F::patch_off(2 * p, onx));
       cp_async_commit();
       L::phase1_inv(v, tw, t);
     } else {
-      // the late copies and direct loads (38 instructions per thread), a few between the steps of phase 1 instead of one burst before it
+      // the late copies and direct loads (22 instructions per thread), a few between the steps of phase 1 instead of one burst before it
       const float4* st = (const float4*)(P.w.stash + fld(pr, i)) + t;
-      constexpr int NQ = (16 - E) + 2 * E + (32 - 2 * E), NH = G::N1X + G::N1Y;
+      constexpr int NQ = (16 - E) + E + (16 - E), NH = G::N1X + G::N1Y;
       auto item = [&](int q) {
         if (q < 16 - E) cp_async16(cs.xs + q * 32, st + (E + q) * T);
-        else if (q < 16 - E + 2 * E) { const int r = q - (16 - E); cp_async8(cs.xs8 + (2 * (16 - E) + r) * 32, o + F::patch_off(r, onx)); }
-        else { const int r = 2 * E + (q - (16 - E) - 2 * E); Tr[r - 2 * E] = ld_nc8(o + F::patch_off(r, onx)); }
+        else if (q < 16) { const int p = q - (16 - E); cp_async16(cs.xs + (16 - E + p) * 32, o2 + F::patch_off(2 * p, onx)); }
+        else { const int p = E + (q - 16); Tr[p - E] = ld_nc16(o2 + F::patch_off(2 * p, onx)); }
       };
       L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout); backward 56.4 -> 55.5 ms per step
 #pragma unroll
@@ -1159,11 +1175,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
         if (!(p & 1)) hw = cs.pf[(p >> 1) * T];
         const cf a = unpack_h2(__float_as_uint((p & 1) ? hw.z : hw.x)), b = unpack_h2(__float_as_uint((p & 1) ? hw.w : hw.y));
         ps = make_float4(a.x, a.y, b.x, b.y);
-        T0 = cs.xs8[(2 * p) * 32]; T1 = cs.xs8[(2 * p + 1) * 32];
+        const float4 tt = cs.xs[p * 32];
+        T0 = make_float2(tt.x, tt.y); T1 = make_float2(tt.z, tt.w);
       } else {
         ps = p < E ? cs.pf[p * T] : cs.xs[(p - E) * 32];
-        if (p < E) { T0 = cs.xs8[(2 * (16 - E) + 2 * p) * 32]; T1 = cs.xs8[(2 * (16 - E) + 2 * p + 1) * 32]; }
-        else { T0 = Tr[2 * p - 2 * E]; T1 = Tr[2 * p + 1 - 2 * E]; }
+        const float4 tt = p < E ? cs.xs[(16 - E + p) * 32] : Tr[p - E];
+        T0 = make_float2(tt.x, tt.y); T1 = make_float2(tt.z, tt.w);
       }
       cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
       if (MODE == 2) { g0 = cscale(g0, s1); g1 = cscale(g1, s1); T0 = cscale(T0, s2); T1 = cscale(T1, s2); }
@@ -1271,7 +1288,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
   for (int jl = blockIdx.x; jl < P.jc; jl += gridDim.x) {
     const int jb = P.j0 + jl, row = P.w.rows[jb];
     const int r0y = P.w.r0[2 * jb], r0x = P.w.r0[2 * jb + 1];
-    const cf* ob = patch_ptr(P, 0, r0y, r0x) + (size_t)F::pix_y(0, t, 0) * onx + F::pix_x(0, t, 0);
+    const float4* ob2 = P.w.O2 + ((size_t)r0y * onx + r0x) + (size_t)F::pix_y(0, t, 0) * onx + F::pix_x(0, t, 0);
     const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
     const cf* ry = rx + NF;
     __syncthreads();                                                // the previous position's readers of ryS / red are done
@@ -1288,7 +1305,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
     for (int c = 0; c < 4; ++c) {                                   // H3: the patch, once per position, parked in tensor memory
       cf tt[8];
 #pragma unroll
-      for (int e = 0; e < 8; ++e) tt[e] = ld_nc8(ob + F::patch_off(8 * c + e, onx));
+      for (int e = 0; e < 4; ++e) {
+        const float4 q = ld_nc16(ob2 + F::patch_off(8 * c + 2 * e, onx));
+        tt[2 * e] = make_float2(q.x, q.y); tt[2 * e + 1] = make_float2(q.z, q.w);
+      }
       tmem_st16(tbT + 16 * c, tt);
     }
     tmem_wait_st();
@@ -1495,17 +1515,21 @@ __global__ void __launch_bounds__(256) k_stash_max(const cf* stash, float* out, 
 // w_d = (d_y ? f_y : 1 - f_y)(d_x ? f_x : 1 - f_x); the chain kernels then read these patches instead of the
 // object window.  One block per (position of the chunk, slice).
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) k_bilinear_patches(KP P) {
+__global__ void __launch_bounds__(256) k_bilinear_patches(KP P, int D) {   // D: distance of a pixel's partner (as k_pair_object)
   const int jl = blockIdx.x / P.S, i = blockIdx.x - jl * P.S, jb = P.j0 + jl, N = P.N;
   const int i0y = P.w.r0[2 * jb], i0x = P.w.r0[2 * jb + 1];
   const float fy = P.w.delta[2 * jb], fx = P.w.delta[2 * jb + 1];
   const float w00 = (1.f - fy) * (1.f - fx), w01 = (1.f - fy) * fx, w10 = fy * (1.f - fx), w11 = fy * fx;
   const cf* o = P.object + ((size_t)i * P.ony + i0y) * P.onx + i0x;
-  cf* out = P.w.Tb + ((size_t)jl * P.S + i) * N * N;
+  float4* out = P.w.Tb + ((size_t)jl * P.S + i) * N * N;
+  auto sample = [&](int y, int x) {
+    const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
+    return make_float2(w00 * a.x + w01 * b.x + w10 * c.x + w11 * d.x, w00 * a.y + w01 * b.y + w10 * c.y + w11 * d.y);
+  };
   for (int e = threadIdx.x; e < N * N; e += 256) {
     const int y = e / N, x = e - y * N;
-    const cf a = o[(size_t)y * P.onx + x], b = o[(size_t)y * P.onx + x + 1], c = o[(size_t)(y + 1) * P.onx + x], d = o[(size_t)(y + 1) * P.onx + x + 1];
-    out[e] = make_float2(w00 * a.x + w01 * b.x + w10 * c.x + w11 * d.x, w00 * a.y + w01 * b.y + w10 * c.y + w11 * d.y);
+    const cf u = sample(y, x), w = x + D < N ? sample(y, x + D) : make_float2(0.f, 0.f);
+    out[e] = make_float4(u.x, u.y, w.x, w.y);
   }
 }
 
@@ -2056,6 +2080,11 @@ int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
   }
   k_setup_pos<<<p->n_batch, p->n, 0, st>>>(kp);
   LAUNCH_CHECK(K_setup_pos, st);
+  {
+    const size_t on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
+    k_pair_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X);
+    LAUNCH_CHECK(K_setup_pos, st);
+  }
   launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f, (const float*)nullptr, 0.0f);
   LAUNCH_CHECK(K_probe_fft, st);
   return PT_OK;
@@ -2067,7 +2096,7 @@ int run_forward(const pt_problem* p, KP kp, double* loss_d, float* loss_per_pos_
   if (rc != PT_OK) return rc;
   for (int j0 = 0; j0 < p->n_batch; j0 += kp.w.Jc) {
     kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
-    if (kp.bilinear) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
+    if (kp.bilinear) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X); LAUNCH_CHECK(K_bilinear_patches, st); }
     launch_fft<G>(k_forward<G, 0>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
     k_loss<G><<<kp.jc * G::CL, G::T, 0, st>>>(kp, model_intensity_d, 0);
@@ -2123,7 +2152,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
         return PT_OK;
       }
     }
-    if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
+    if (bilin) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X); LAUNCH_CHECK(K_bilinear_patches, st); }
     if (h16) launch_fft<G>(k_forward<G, 2>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     else launch_fft<G>(k_forward<G, 1>, kp.jc * p->n_modes * G::CL, chain_smem_bytes<G>(), st, kp);
     LAUNCH_CHECK(K_forward, st);
@@ -2212,7 +2241,7 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       kp.j0 = j0; kp.jc = p->n_batch - j0 < kp.w.Jc ? p->n_batch - j0 : kp.w.Jc;
       stage_chunk(j0);
       if (recompute) { if ((rc = chains(false)) != PT_OK) return rc; }
-      else if (bilin && kp.w.Jc < p->n_batch) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp); LAUNCH_CHECK(K_bilinear_patches, st); }
+      else if (bilin && kp.w.Jc < p->n_batch) { k_bilinear_patches<<<kp.jc * p->n_slices, 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X); LAUNCH_CHECK(K_bilinear_patches, st); }
       if (bilin) k_step_object<G, true><<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
       else k_step_object<G, false><<<kp.jc * p->n_slices, 256, 0, st>>>(kp);
       LAUNCH_CHECK(K_step_object, st);
