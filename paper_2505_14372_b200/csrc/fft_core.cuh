@@ -111,16 +111,19 @@ template <> struct Geo<128> {
   static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
   static constexpr int NF = 128, CL = 1;
   static constexpr int PF16 = 10;   // 16-byte prefetch slots per thread beside the exchange buffer (1 CTA / SM)
+  static constexpr int HXS = 1;     // the hx propagator tables are staged in shared memory beside the hy tables (2 KB)
 };
 template <> struct Geo<64> {
   static constexpr int N = 64, LOGN = 6, T = 128, N1X = 8, N2X = 8, N1Y = 4, N2Y = 16, LX2 = 3, LY2 = 4, LP2 = 4, LP3 = 2;
   static constexpr int NF = 64, CL = 1;
   static constexpr int PF16 = 8;    // 4 CTAs / SM: 56 KB each
+  static constexpr int HXS = 0;     // no room for them without losing the fourth CTA per SM: hx is read from global memory
 };
 template <> struct Geo<256> {
   static constexpr int N = 128, LOGN = 7, T = 512, N1X = 8, N2X = 16, N1Y = 4, N2Y = 32, LX2 = 4, LY2 = 5, LP2 = 2, LP3 = 1;
   static constexpr int NF = 256, CL = 4;
   static constexpr int PF16 = 10;
+  static constexpr int HXS = 0;     // 4 KB more would exceed the 227 KB of a CTA: hx is read from global memory
 };
 
 template <class G>

@@ -361,15 +361,16 @@ template <class G> constexpr int min_blocks() { return G::T == 512 ? 1 : 4; }
 // which is idle between the end of fft2_inv_head and the next fft2_fwd (16 slots of 16 B per lane).
 // ------------------------------------------------------------------------------------------------
 template <class G> constexpr size_t fft_smem_bytes() { return (size_t)(Lay<G>::XBUF + Lay<G>::TW + (G::CL > 1 ? G::N : 0)) * sizeof(cf) + 1024; }
-template <class G> constexpr size_t chain_smem_bytes() { return fft_smem_bytes<G>() + (size_t)2 * G::NF * sizeof(cf) + (size_t)G::PF16 * G::T * 16; }
+template <class G> constexpr size_t chain_smem_bytes() { return fft_smem_bytes<G>() + (size_t)(G::HXS ? 4 : 2) * G::NF * sizeof(cf) + (size_t)G::PF16 * G::T * 16; }
 template <class G>
 struct ChainSmem {
-  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; float4* pf; float4* xs;
+  cf* sm; cf* tw; cf* tw2; double* red; cf* hyS; cf* hxS; float4* pf; float4* xs;
   __device__ __forceinline__ ChainSmem(unsigned char* raw, int t) {
     typedef Lay<G> L;
     sm = (cf*)raw; tw = sm + L::XBUF; tw2 = tw + L::TW; red = (double*)(tw2 + (G::CL > 1 ? G::N : 0));
-    hyS = (cf*)((unsigned char*)red + 1024);
-    pf = (float4*)(hyS + 2 * G::NF) + t;                                // early 16-byte slot s: pf[s * T]
+    hyS = (cf*)((unsigned char*)red + 1024);                            // hy tables of two consecutive propagations, then hx likewise
+    hxS = hyS + 2 * G::NF;                                              // (G::HXS only; else the early slots start here)
+    pf = (float4*)(hxS + (G::HXS ? 2 : 0) * G::NF) + t;                                // early 16-byte slot s: pf[s * T]
     xs = (float4*)(sm + (t >> 5) * L::X1_WARP) + (t & 31);              // late 16-byte slot s:  xs[s * 32]
   }
   // twiddle tables; the caller synchronises the CTA before the first transform
@@ -577,7 +578,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     const float4* o2 = ob2 + (size_t)i * slice;
 #pragma unroll
     for (int p = 0; p < E; ++p) cp_async16(cs.pf + p * T, o2 + F::patch_off(2 * p, onx));
-    if (i < S - 1 && t < NF) cp_async8(cs.hyS + (i & 1) * NF + t, P.w.hy + (size_t)i * NF + t);
+    if (i < S - 1 && t < NF) {                                    // both tables of the propagation that ends iteration i (hx from global
+      cp_async8(cs.hyS + (i & 1) * NF + t, P.w.hy + (size_t)i * NF + t);   // memory at its point of use exposed an L2 round trip per slice)
+      if (G::HXS) cp_async8(cs.hxS + (i & 1) * NF + t, P.w.hx + (size_t)i * NF + t);
+    }
     cp_async_commit();
   };
   early(0);
@@ -626,7 +630,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_forward(KP P) {
     }
     if (i + 1 < S) early(i + 1);
     Fft<G>::fwd_after_rows(v, sm, tw, cs.tw2, t, rk);            // F(Phi)    (Fourier layout)
-    if (i < S - 1) apply_prop_s<G, false>(v, P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, inside, t, rk);   // H5
+    if (i < S - 1) apply_prop_s<G, false>(v, G::HXS ? cs.hxS + (i & 1) * NF : P.w.hx + (size_t)i * NF, cs.hyS + (i & 1) * NF, P.bandlim2, inside, t, rk);   // H5
   }
   float4* out = (float4*)(P.w.psit + ((size_t)pair * CL + rk) * NNS);   // H6: psi~ = F(Phi_{S-1}) / N
   const float sc = 1.0f / (float)NF;
@@ -770,7 +774,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     const float4* st = (const float4*)(P.w.stash + fld(pair, i) / (H16 ? 2 : 1)) + t;
     // (the early part itself, pairs [0, E) or the whole binary16 field, arrives by one bulk copy: early_bulk, as in k_backward_pair)
     if (!H16 && t < (16 - E) * T / 8) l2_prefetch_line((const char*)(st - t + E * T) + t * 128);   // the late part of the same field: DRAM -> L2 now, one line per thread
-    if (i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
+    if (i > 0 && t < NF) {
+      cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
+      if (G::HXS) cp_async8(cs.hxS + ((i - 1) & 1) * NF + t, P.w.hx + (size_t)(i - 1) * NF + t);
+    }
     cp_async_commit();
   };
   uint64_t* bar = (uint64_t*)((unsigned char*)red + 512);
@@ -854,7 +861,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
     if (i > 0) early(i - 1);
     Fft<G>::fwd(v, sm, tw, cs.tw2, t, rk);                       // F(gPsi_i)  (Fourier layout)
     if (t == 0 && i > 0) early_bulk(i - 1);                      // behind the forward transform's last CTA barrier: every thread has read its slots
-    if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
+    if (i > 0) apply_prop_t<G, true>(v, G::HXS ? cs.hxS + ((i - 1) & 1) * NF : P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
   }
   const cf* rx = P.w.ramps + (size_t)jb * 2 * NF;
   const cf* ry = rx + NF;
@@ -1114,7 +1121,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     const float4* st = (const float4*)(P.w.stash + fld(pair0 + h, i) / (H16 ? 2 : 1)) + t;
     // (the early part itself, pairs [0, E) or the whole binary16 field, arrives by ONE bulk copy: early_bulk below)
     if (!H16 && t < (16 - E) * T / 8) l2_prefetch_line((const char*)(st - t + E * T) + t * 128);   // the late part of the same field: DRAM -> L2 now, one line per thread
-    if (h == 0 && i > 0 && t < NF) cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);   // serves both modes at slice i
+    if (h == 0 && i > 0 && t < NF) {                              // serves both modes at slice i
+      cp_async8(cs.hyS + ((i - 1) & 1) * NF + t, P.w.hy + (size_t)(i - 1) * NF + t);
+      if (G::HXS) cp_async8(cs.hxS + ((i - 1) & 1) * NF + t, P.w.hx + (size_t)(i - 1) * NF + t);
+    }
     cp_async_commit();
   };
   // The early slots of all threads are one contiguous block [pair][thread] in shared memory and in the stash, so ONE bulk copy
@@ -1222,7 +1232,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
     if (h == 0) tmem_wait_st();
     if (s + 1 < 2 * S) early(s + 1);
     Fft<G>::fwd_after_rows(v, sm, tw, cs.tw2, t, rk);             // F(gPsi_i)
-    if (i > 0) apply_prop_t<G, true>(v, P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
+    if (i > 0) apply_prop_t<G, true>(v, G::HXS ? cs.hxS + ((i - 1) & 1) * NF : P.w.hx + (size_t)(i - 1) * NF, cs.hyS + ((i - 1) & 1) * NF, P.bandlim2, t, rk);
     if (t == 0 && s + 1 < 2 * S) early_bulk(s + 1);               // behind the forward transform's last CTA barrier: every thread has read its slots
     tmem_swap_field(tb, v);                                      // the other mode's turn
   }
@@ -1291,7 +1301,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
   ChainSmem<G> cs(smem_raw, t);
   cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
   uint32_t* tmem_slot = (uint32_t*)((unsigned char*)red + 1000);
-  float* Ib = (float*)(cs.hyS + 2 * NF) + t;                        // I (then w) of register r: Ib[r * T]   (thread-private)
+  float* Ib = (float*)(cs.pf - t) + t;                        // I (then w) of register r: Ib[r * T]   (thread-private)
   cf* ryS = cs.hyS;                                                 // ry of the current position
   cs.fill_tables(t);
   if (wp == 0) {
