@@ -188,9 +188,7 @@ struct Lay {
     for (int n1y = 0; n1y < G::N1Y; ++n1y) phase1_fwd_row(v, n1y);
     phase1_fwd_rest(v, tw, t);
   }
-  static PTK_HD void phase1_fwd_rest(cf (&v)[32], const cf* tw, int t) { phase1_fwd_rest_h(v, tw, t, NoHook()); }
-  template <class Hook>
-  static PTK_HD void phase1_fwd_rest_h(cf (&v)[32], const cf* tw, int t, Hook hook) {   // hook(step), step = 0 .. N1X - 1, after each column
+  static PTK_HD void phase1_fwd_rest(cf (&v)[32], const cf* tw, int t) {
     const int a = t & (G::N2X - 1), b = t >> G::LX2;
 #pragma unroll
     for (int k1x = 0; k1x < G::N1X; ++k1x) {
@@ -205,7 +203,6 @@ struct Lay {
       }
 #pragma unroll
       for (int i = 0; i < G::N1Y; ++i) v[i * G::N1X + k1x] = x[i];
-      hook(k1x);
     }
 #pragma unroll
     for (int k1y = 1; k1y < G::N1Y; ++k1y) {
@@ -429,16 +426,10 @@ __device__ __forceinline__ void fft2_fwd(cf (&v)[32], cf* sm, const cf* tw, int 
   fft2_fwd_after_rows<G>(v, sm, tw, t);
 }
 // the forward transform whose phase-1 row transforms the caller has already run (Lay::phase1_fwd_row for every n1y)
-template <class G, class Hook>
-__device__ __forceinline__ void fft2_fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, int t, Hook hook);
 template <class G>
 __device__ __forceinline__ void fft2_fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, int t) {
-  fft2_fwd_after_rows_h<G>(v, sm, tw, t, typename Lay<G>::NoHook());
-}
-template <class G, class Hook>
-__device__ __forceinline__ void fft2_fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, int t, Hook hook) {
   typedef Lay<G> L;
-  L::phase1_fwd_rest_h(v, tw, t, hook);
+  L::phase1_fwd_rest(v, tw, t);
   __syncwarp();
   L::x1_store_p1(v, sm, t);
   __syncwarp();
@@ -545,11 +536,6 @@ struct Fft {
   }
   static __device__ __forceinline__ void fwd_after_rows(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
     fft2_fwd_after_rows<G>(v, sm, tw, t);
-    if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
-  }
-  template <class Hook>
-  static __device__ __forceinline__ void fwd_after_rows_h(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk, Hook hook) {
-    fft2_fwd_after_rows_h<G>(v, sm, tw, t, hook);
     if (G::CL > 1) Cross<G>::fwd(v, sm, tw2, t, rk);
   }
   static __device__ __forceinline__ void inv_head(cf (&v)[32], cf* sm, const cf* tw2, int t, unsigned rk) {
