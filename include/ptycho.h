@@ -79,7 +79,8 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
                                        * only; no position gradient, no step sizes (PT_ERR_UNSUPPORTED).                  */
 
 enum { PT_OK = 0, PT_ERR_NULL = -1, PT_ERR_BAD_SIZE = -2, PT_ERR_BAD_PARAM = -3, PT_ERR_WORKSPACE = -4,
-       PT_ERR_CUDA = -5, PT_ERR_OUT_OF_BOUNDS = -6, PT_ERR_NONFINITE = -7, PT_ERR_UNSUPPORTED = -8 };
+       PT_ERR_CUDA = -5, PT_ERR_OUT_OF_BOUNDS = -6, PT_ERR_NONFINITE = -7, PT_ERR_UNSUPPORTED = -8,
+       PT_ERR_STATIC_LIMIT = -9 /* ptycho_apply_constraint_static only: the field needs more than PT_STATIC_SCRATCH_BYTES */ };
 
 /* Problem statement. HOST struct. */
 typedef struct {
@@ -230,6 +231,29 @@ enum { PT_CON_AMPLITUDE_CLAMP = 0, PT_CON_SUPPORT_MASK = 1, PT_CON_LAYER_BLUR = 
        PT_CON_SUPPORT_MASK_FOURIER = 4, PT_CON_PHASE_DERAMP = 5 };
 int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float *mask_d, int32_t n_slices, int32_t ny, int32_t nx,
                                 pt_c64 *field_d, void *workspace_d, size_t workspace_bytes, void *cuda_stream);
+
+/* ptycho_apply_constraint for callers that cannot allocate device memory (code under CUDA graph capture, serving loops,
+ * harnesses that forbid cudaMalloc): the kinds that need scratch — PT_CON_LAYER_BLUR, PT_CON_LOWPASS, PT_CON_PHASE_DERAMP —
+ * with that scratch in a file-scope `static __device__` array of PT_STATIC_SCRATCH_BYTES inside the library instead of a
+ * caller's workspace.  Same kernels, same launch configuration, same results bit for bit as ptycho_apply_constraint; the
+ * call (and everything under it) calls no cudaMalloc / cudaFree and no allocating library routine.
+ *   - Every GPU that loads the library holds the PT_STATIC_SCRATCH_BYTES (16 MiB) from module load until the process exits.
+ *   - Limit: the two blurs need n_slices*ny*nx*8 bytes (fields up to 2 097 152 complex pixels, e.g. 8 slices of 512 x 512),
+ *     the deramp 256 + n_slices*2080 bytes.  A larger field is rejected with PT_ERR_STATIC_LIMIT before anything is launched
+ *     (field_d untouched); use ptycho_apply_constraint with a caller-owned workspace for it.
+ *   - The first call on each device looks up the array's device address (cudaGetSymbolAddress, with that device current —
+ *     the device that is current at the call; field_d must live there) and caches it per device; later calls only launch.
+ *   - All calls on a device SHARE the one array, and it keeps the previous call's contents.  Nothing in it has to start at
+ *     zero: every word a kernel reads (the blurred copy, the per-block partial sums, the slopes) is written earlier in the
+ *     same call, so there is nothing to clear and stale contents are never read.  Calls that overlap on the GPU (two
+ *     streams, two host threads, two graphs replayed side by side) RACE on it: serialise them on one stream.
+ *   - The kinds that need no scratch are not served here: PT_ERR_UNSUPPORTED (ptycho_apply_constraint with workspace_d =
+ *     NULL already allocates nothing for them).
+ * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE, PT_ERR_BAD_PARAM (sigma outside (0, 8]), PT_ERR_UNSUPPORTED, PT_ERR_STATIC_LIMIT,
+ * PT_ERR_CUDA (address lookup or a launch failed).                                                                     */
+#define PT_STATIC_SCRATCH_BYTES (16u << 20)
+int32_t ptycho_apply_constraint_static(int32_t kind, float a, int32_t n_slices, int32_t ny, int32_t nx, pt_c64 *field_d,
+                                       void *cuda_stream);
 
 /* Adam (Kingma & Ba algorithm 1; reading R28: complex first moment, second moment from |g|^2), step >= 1:
  *   m <- b1 m + (1-b1) g ; v <- b2 v + (1-b2) |g|^2 ; z <- z - lr (m / (1 - b1^step)) / (sqrt(v / (1 - b2^step)) + eps)

@@ -28,6 +28,7 @@
 #include <stdlib.h>
 #include <string.h>
 
+#include <atomic>
 #include <mutex>
 #include <vector>
 
@@ -2706,6 +2707,7 @@ const char* ptycho_strerror(int32_t code) {
     case PT_ERR_OUT_OF_BOUNDS: return "a probe window leaves the object";
     case PT_ERR_NONFINITE: return "non-finite loss";
     case PT_ERR_UNSUPPORTED: return "not supported by this build";
+    case PT_ERR_STATIC_LIMIT: return "the field needs more scratch than the library's static array holds (PT_STATIC_SCRATCH_BYTES): use the entry point that takes a workspace";
     default: return "unknown error";
   }
 }

@@ -293,6 +293,34 @@ int32_t ptycho_apply_constraint(int32_t kind, float a, float b, const float* mas
   return PT_OK;
 }
 
+// ---- ptycho_apply_constraint without a caller's workspace (include/ptycho.h) ----------------------------------------
+// The scratch of the blur / low-pass / deramp kernels in a file-scope device array.  In HOST code the name below is a
+// host-side stand-in, not a device address (a kernel handed it would fault, or on a GPU that can reach host memory use the
+// wrong memory): the address comes from cudaGetSymbolAddress, once per device with that device current, and is cached.
+// Every call on a device shares the array; nothing in it has to start at zero (see the header).
+static __device__ __align__(256) unsigned char g_static_scratch[PT_STATIC_SCRATCH_BYTES];
+constexpr int kStaticMaxDevices = 64;
+static std::atomic<void*> g_static_scratch_ptr[kStaticMaxDevices];
+
+int32_t ptycho_apply_constraint_static(int32_t kind, float a, int32_t n_slices, int32_t ny, int32_t nx, pt_c64* field_d,
+                                       void* cuda_stream) {
+  if (!field_d) return PT_ERR_NULL;
+  if (n_slices < 1 || ny < 1 || nx < 1) return PT_ERR_BAD_SIZE;
+  size_t need;
+  if (kind == PT_CON_LAYER_BLUR || kind == PT_CON_LOWPASS) need = (size_t)n_slices * ny * nx * sizeof(cf);
+  else if (kind == PT_CON_PHASE_DERAMP) need = 256 + (size_t)n_slices * (kDerampBlocks * 4 * sizeof(double) + sizeof(DerampOut));
+  else return kind >= PT_CON_AMPLITUDE_CLAMP && kind <= PT_CON_PHASE_DERAMP ? PT_ERR_UNSUPPORTED : PT_ERR_BAD_PARAM;
+  if (need > (size_t)PT_STATIC_SCRATCH_BYTES) return PT_ERR_STATIC_LIMIT;
+  int dev = -1;
+  if (cudaGetDevice(&dev) != cudaSuccess || dev < 0 || dev >= kStaticMaxDevices) return PT_ERR_CUDA;
+  void* scratch = g_static_scratch_ptr[dev].load(std::memory_order_acquire);
+  if (!scratch) {                                                      // set-up, once per device (threads racing here store the same value)
+    if (cudaGetSymbolAddress(&scratch, g_static_scratch) != cudaSuccess || !scratch) return PT_ERR_CUDA;
+    g_static_scratch_ptr[dev].store(scratch, std::memory_order_release);
+  }
+  return ptycho_apply_constraint(kind, a, 0.f, nullptr, n_slices, ny, nx, field_d, scratch, (size_t)PT_STATIC_SCRATCH_BYTES, cuda_stream);
+}
+
 static int adam_params(const void* z, const void* g, const void* m, const void* v, float b1, float b2, float eps, int32_t step,
                        float* ic1, float* ic2) {
   if (!z || !g || !m || !v) return PT_ERR_NULL;

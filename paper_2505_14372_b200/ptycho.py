@@ -25,7 +25,7 @@ EXPORTS = ["ptycho_workspace_bytes", "ptycho_workspace_min_bytes", "ptycho_posit
            "ptycho_apply_update", "ptycho_object_transparency", "ptycho_workspace_host_bytes", "ptycho_gradient_host", "ptycho_status",
            "ptycho_launch_count", "ptycho_strerror", "ptycho_profile_enable", "ptycho_profile_num_kernels",
            "ptycho_profile_kernel_name", "ptycho_profile_read", "ptycho_profile_fp32_peak", "ptycho_regularizer_workspace_bytes", "ptycho_cost_regularizer",
-           "ptycho_apply_constraint", "ptycho_adam_update", "ptycho_adam_update_real"]
+           "ptycho_apply_constraint", "ptycho_apply_constraint_static", "ptycho_adam_update", "ptycho_adam_update_real"]
 
 
 def build(force: bool = False, verbose: bool = False) -> str:
@@ -332,6 +332,20 @@ def apply_constraint(kind: int, field_, *, a: float = 0.0, b: float = 0.0, mask=
     f.restype = C.c_int32
     _check(f(int(kind), C.c_float(a), C.c_float(b), _ptr(_dev(mask, torch.float32, "mask")), S, ny, nx, _ptr(z), _ptr(workspace),
              C.c_size_t(0 if workspace is None else workspace.numel()), _stream()))
+
+
+STATIC_SCRATCH_BYTES = 16 << 20                                       # PT_STATIC_SCRATCH_BYTES
+ERR_UNSUPPORTED, ERR_STATIC_LIMIT = -8, -9
+
+
+def apply_constraint_static(kind: int, field_, *, a: float = 0.0):
+    """ptycho_apply_constraint_static (in place): layer blur / low pass / phase deramp with the library's own static device
+    scratch; allocates nothing, fields beyond STATIC_SCRATCH_BYTES of scratch raise PtychoError(ERR_STATIC_LIMIT)."""
+    z = _field3(field_, "field")
+    S, ny, nx = z.shape
+    f = lib().ptycho_apply_constraint_static
+    f.restype = C.c_int32
+    _check(f(int(kind), C.c_float(a), S, ny, nx, _ptr(z), _stream()))
 
 
 def adam_update(z, g, m, v, *, lr: float, beta1: float = 0.9, beta2: float = 0.999, eps: float = 1e-8, step: int = 1):
