@@ -16,6 +16,10 @@
  *     zeroes them once when the buffer is allocated (cudaMemset); ptycho_status() reads and clears the word.
  *   - all work is enqueued on `cuda_stream` (a cudaStream_t passed as void*); nothing synchronises except
  *     ptycho_status() and the *_host convenience entry point.
+ *   - CUDA graphs: every device-path call (everything except ptycho_status, ptycho_gradient_host and the profiling record)
+ *     only enqueues kernels on `cuda_stream`, so a sequence of calls can be captured into a CUDA graph and replayed, once the
+ *     same calls have run once on that device outside a capture (the first call sets the kernels' shared-memory attributes).
+ *     pt_problem / pt_update / slice_thickness are read at capture time (tests: test_step_captured_in_a_cuda_graph_replays_bitwise).
  *   - every function returns int32 status: 0 = PT_OK, < 0 = error.  No exceptions, no printing, no abort.
  *   - resources: the chain kernels take a whole SM each (up to 227 KB of shared memory, the full register file) and, with an
  *     even number of modes, the backward kernel allocates the SM's tensor memory (tcgen05.alloc, all 512 columns at N >= 128)

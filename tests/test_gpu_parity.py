@@ -1367,3 +1367,53 @@ def test_single_slice_fused_and_unfused(which):
     a2 = gpu_gradient(case, pbg)
     for k in ("grad_object", "grad_probe", "grad_pos", "loss_per_pos"):
         assert a[k].tobytes() == a2[k].tobytes(), k                                           # deterministic
+
+
+# ------------------------------------------------------------------------------------------------
+# The C-ABI calls can be captured in a CUDA graph (they allocate nothing, never synchronise and keep no per-call state):
+# ptycho_gradient + ptycho_apply_update captured once and replayed must give, bit for bit, what the same calls give when
+# launched directly (bench.py times the single-slice configurations this way).  Multislice too (chunked launches, pair kernel).
+# ------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("which", ["cfg2_single_slice", "cfg3_multislice"])
+def test_step_captured_in_a_cuda_graph_replays_bitwise(which):
+    import torch
+    from paper_2505_14372_b200 import ptycho
+    cfg = synth.config(2, scan=(9, 10)) if which == "cfg2_single_slice" else synth.config(3, scan=(4, 5), n_modes=4, n_slices=3)
+    case = make_case(cfg, start_scale=0.8)
+    pbg = gpu_problem(cfg)
+    J = cfg.n_pos
+    lr = dict(lr_obj=1e-3, lr_probe=1e-4, lr_pos=1e-9)               # positions move, windows stay inside the small object
+
+    def state():
+        return [_t(case.obj_start), _t(case.probe), _t(case.positions)]
+
+    inten = _t(case.intensity)
+    gO = torch.empty(case.obj_start.shape, dtype=torch.complex64, device="cuda"); gP = torch.empty(case.probe.shape, dtype=torch.complex64, device="cuda")
+    gX = torch.empty((J, 2), dtype=torch.float32, device="cuda"); loss = torch.zeros(1, dtype=torch.float64, device="cuda")
+    ws = ptycho.make_workspace(pbg, J, J, ptycho.WANT_POS_GRAD)
+
+    def step(obj, pr, pos):
+        ptycho.gradient(pbg, obj, pr, pos, inten, None, workspace=ws, grad_object=gO, grad_probe=gP, grad_pos=gX, loss=loss)
+        ptycho.apply_update(pbg, obj, pr, pos, grad_object=gO, grad_probe=gP, grad_pos=gX, **lr)
+
+    # direct calls: three steps from the start state
+    d = state()
+    for _ in range(3):
+        step(*d)
+    assert ptycho.status(ws) == 0
+    direct = [x.cpu().numpy().copy() for x in d] + [gO.cpu().numpy().copy(), loss.item()]
+    # captured once (on a fresh copy of the state, after the warm-up above set the kernels' attributes), replayed three times
+    g = state()
+    graph = torch.cuda.CUDAGraph()
+    keep = [x.clone() for x in g]
+    with torch.cuda.graph(graph):
+        step(*g)
+    for x, k in zip(g, keep):
+        x.copy_(k)                                                 # capture does not execute; start again from the start state anyway
+    for _ in range(3):
+        graph.replay()
+    assert ptycho.status(ws) == 0
+    replayed = [x.cpu().numpy() for x in g] + [gO.cpu().numpy(), loss.item()]
+    for a, b, name in zip(direct, replayed, ("object", "probe", "positions", "grad_object", "loss")):
+        assert np.asarray(a).tobytes() == np.asarray(b).tobytes(), name
+    assert rel_l2(direct[0], case.obj_start) > 0                   # the steps moved the object
