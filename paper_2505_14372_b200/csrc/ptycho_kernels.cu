@@ -1303,7 +1303,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
   cf* sm = cs.sm; cf* tw = cs.tw; double* red = cs.red;
   uint32_t* tmem_slot = (uint32_t*)((unsigned char*)red + 1000);
   float* Ib = (float*)(cs.pf - t) + t;                        // I (then w) of register r: Ib[r * T]   (thread-private)
-  cf* ryS = cs.hyS;                                                 // ry of the current position
+  cf* ryS = cs.hyS;                                                 // ry, then rx, of the current position (2 NF entries)
   cs.fill_tables(t);
   if (wp == 0) {
     asm volatile("tcgen05.alloc.cta_group::1.sync.aligned.shared::cta.b32 [%0], %1;" ::"r"((unsigned)__cvta_generic_to_shared(tmem_slot)), "n"(TCOLS));
@@ -1330,7 +1330,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
       for (int p = 0; p < 16; ++p) cp_async16(cs.xs + p * 32, src + p * T);
       cp_async_commit();
     }
-    if (t < NF) ryS[t] = ry[t];
+    if (t < NF) { ryS[t] = ry[t]; ryS[NF + t] = rx[t]; }            // both shift ramps of the position (read 2M times below)
     for (int b = t * 128; b < F::NNF * 4; b += T * 128)             // this position's measured pattern: DRAM -> L2 now
       l2_prefetch_line((const char*)(P.intensity + (size_t)row * F::NNF) + b);
 #pragma unroll
@@ -1360,17 +1360,29 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
         // ---------------- H8: loss and detector weight (float32 per pixel in cancellation-free form, fp64 sum)
         double acc[1] = {0.0};
         const float* Ie = P.intensity + (size_t)row * F::NNF;
-        float ix[32];                                               // all 32 loads in flight before the first use (v is dead here)
-#pragma unroll
-        for (int r = 0; r < 32; ++r) ix[r] = __ldg(Ie + F::fq_y(0, t, r) * NF + F::fq_x(0, t, r));
         float ls = 0.f, lc = 0.f;                                   // the thread's 32 terms: compensated float32 sum (fp64 conversions
-#pragma unroll                                                      // and adds are what made this loop cost 35 k cycles), then fp64
-        for (int r = 0; r < 32; ++r) {
-          float l, w;
-          pixel_loss_f32(P.loss, Ib[r * T], ix[r], P.eps, P.loss_c, l, w);
-          const float y = l - lc, s2 = ls + y;
-          lc = (s2 - ls) - y; ls = s2;
-          Ib[r * T] = w;
+                                                                    // and adds are what made this loop cost 35 k cycles), then fp64
+        // Four rounds of eight pixels, NOT unrolled across the rounds: run once per position, the fully unrolled loop (3 loss kinds
+        // x 32 pixels, ~3500 instructions = 56 KB) pushed the half-step loop out of the instruction cache (ncu: stall_no_inst was
+        // the kernel's first stall reason).  The pattern is in L2 (prefetched at the start of the position).
+        float cur[8], nxt[8];                                       // the next round's pattern values are in flight during this one
+#pragma unroll
+        for (int e = 0; e < 8; ++e) cur[e] = __ldg(Ie + F::fq_y(0, t, e) * NF + F::fq_x(0, t, e));
+#pragma unroll 1
+        for (int r0 = 0; r0 < 32; r0 += 8) {
+          const int rn = r0 + 8 < 32 ? r0 + 8 : r0;                 // (the last round re-reads its own values: no branch)
+#pragma unroll
+          for (int e = 0; e < 8; ++e) nxt[e] = __ldg(Ie + F::fq_y(0, t, rn + e) * NF + F::fq_x(0, t, rn + e));
+#pragma unroll
+          for (int e = 0; e < 8; ++e) {
+            float l, w;
+            pixel_loss_f32(P.loss, Ib[(r0 + e) * T], cur[e], P.eps, P.loss_c, l, w);
+            const float y = l - lc, s2 = ls + y;
+            lc = (s2 - ls) - y; ls = s2;
+            Ib[(r0 + e) * T] = w;
+          }
+#pragma unroll
+          for (int e = 0; e < 8; ++e) cur[e] = nxt[e];
         }
         acc[0] = (double)ls - (double)lc;
         block_sum<G::T, 1>(acc, red);
@@ -1381,7 +1393,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
       }
       {   // Fourier-side start: H2  R .* P~_k / N^2   or   H9  g~ = w .* psi~_k / N ; the source field (P~_k, or psi~_k from the
           // scratch) was asked into the warp's idle X1 region at the end of the previous half step
-        if (fwd_pass) load_xv<G>(wxv, rx, t, 1.0f / (float)F::NNF);
+        if (fwd_pass) load_xv<G>(wxv, ryS + NF, t, 1.0f / (float)F::NNF);
         cp_async_wait_all();
 #pragma unroll
         for (int p = 0; p < 16; ++p) {
@@ -1472,7 +1484,7 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
         // H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
         const float4* pt4 = (const float4*)(P.w.Pt + (size_t)k * NNS) + t;
         float4* gp4 = (float4*)(P.w.Gpart + fk) + t;
-        load_xv<G>(wxv, rx, t, 1.0f);
+        load_xv<G>(wxv, ryS + NF, t, 1.0f);
         float sy = 0.f, sx = 0.f;
         const float fx = (float)signed_freq(F::fq_x(0, t, 0), NF) / (float)NF;
 #pragma unroll
