@@ -1071,15 +1071,31 @@ __device__ __forceinline__ void tmem_ld16(uint32_t a, cf* v) {
   for (int i = 0; i < 8; ++i) v[i] = make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
 }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
-// v <-> parked field (columns [0, 64) of the warp's block), eight complex at a time
+__device__ __forceinline__ void tmem_st8(uint32_t a, const cf* v) {   // 4 complex = 8 columns
+  asm volatile("tcgen05.st.sync.aligned.32x32b.x8.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8};" ::"r"(a),
+               "r"(__float_as_uint(v[0].x)), "r"(__float_as_uint(v[0].y)), "r"(__float_as_uint(v[1].x)), "r"(__float_as_uint(v[1].y)),
+               "r"(__float_as_uint(v[2].x)), "r"(__float_as_uint(v[2].y)), "r"(__float_as_uint(v[3].x)), "r"(__float_as_uint(v[3].y)) : "memory");
+}
+__device__ __forceinline__ void tmem_ld8(uint32_t a, cf* v) {
+  uint32_t r[8];
+  asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];"
+               : "=r"(r[0]), "=r"(r[1]), "=r"(r[2]), "=r"(r[3]), "=r"(r[4]), "=r"(r[5]), "=r"(r[6]), "=r"(r[7]) : "r"(a) : "memory");
+  asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory");
+#pragma unroll
+  for (int i = 0; i < 4; ++i) v[i] = make_float2(__uint_as_float(r[2 * i]), __uint_as_float(r[2 * i + 1]));
+}
+// v <-> parked field (columns [0, 64) of the warp's block), four complex at a time.  Sixteen-column accesses want sixteen
+// CONSECUTIVE registers on both sides: with them the register allocator spilled one quarter of the incoming field in every half step
+// (16 LDL + 8 STL.64, 4.6 % of the kernel's stall samples; ncu source page); eight-column accesses leave 8 bytes of spill and the
+// backward kernel runs 52.4 -> 50.0 ms per step at config 3.
 __device__ __forceinline__ void tmem_swap_field(uint32_t tb, cf (&v)[32]) {
 #pragma unroll
-  for (int c = 0; c < 4; ++c) {
-    cf tmp[8];
-    tmem_ld16(tb + c * 16, tmp);
-    tmem_st16(tb + c * 16, &v[8 * c]);
+  for (int c = 0; c < 8; ++c) {
+    cf tmp[4];
+    tmem_ld8(tb + c * 8, tmp);
+    tmem_st8(tb + c * 8, &v[4 * c]);
 #pragma unroll
-    for (int i = 0; i < 8; ++i) v[8 * c + i] = tmp[i];
+    for (int i = 0; i < 4; ++i) v[4 * c + i] = tmp[i];
   }
   tmem_wait_st();
 }
