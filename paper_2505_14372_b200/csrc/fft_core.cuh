@@ -402,6 +402,13 @@ struct FL {
 __device__ __forceinline__ unsigned cluster_ctarank() { unsigned r; asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r)); return r; }
 __device__ __forceinline__ void cluster_arrive() { asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory"); }
 __device__ __forceinline__ void cluster_wait() { asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory"); }
+// Arrive that only says "this thread has finished READING its CTA's exchange buffer" (write-after-read protection; it publishes
+// no data).  barrier.cluster.arrive.release compiles to MEMBAR.ALL.CTA + MEMBAR.ALL.GPU + ERRBAR, and the GPU-scope part waits for
+// every global store the thread has in flight (the stash / staging stores of the chain kernels): ncu showed `membar` as 7.7 % of
+// the N = 256 kernels' stalls.  Here the CTA-scope fence alone is enough: once it retires, the thread's shared-memory loads have
+// returned their values, and a load that has completed cannot be affected by a peer's later remote store, which can only be
+// issued after every thread of the cluster has executed this arrive.  (config 4: 7489 -> 7296 ms per step)
+__device__ __forceinline__ void cluster_arrive_war() { asm volatile("fence.acq_rel.cta;\n\tbarrier.cluster.arrive.relaxed.aligned;" ::: "memory"); }
 __device__ __forceinline__ unsigned mapa_u32(unsigned saddr, unsigned rank) {
   unsigned r; asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(saddr), "r"(rank)); return r;
 }
@@ -439,7 +446,7 @@ __device__ __forceinline__ void fft2_fwd_after_rows(cf (&v)[32], cf* sm, const c
   L::x2_store_p2(v, sm, t);
   __syncthreads();
   L::x2_load_p3(v, sm, t);
-  if (G::CL > 1) cluster_arrive();  // this thread no longer reads the exchange buffer: peers may overwrite it (Cross)
+  if (G::CL > 1) cluster_arrive_war();  // this thread no longer reads the exchange buffer: peers may overwrite it (Cross)
   L::template phase3<-1>(v);
   __syncthreads();                 // all p3-side reads are long done: the buffer is free for the next transform.
                                    // Placed after the arithmetic, not after the loads: a barrier behind a burst of
@@ -509,7 +516,7 @@ struct Cross {
     cluster_arrive();
     cluster_wait();
     recv(v, sm, t);
-    cluster_arrive();
+    cluster_arrive_war();
     F::butterfly(v);
   }
   // C-layout -> sub-F-layout (ready for fft2_inv_head); consumes the pending arrive
@@ -528,7 +535,7 @@ struct Cross {
 template <class G>
 struct Fft {
   static __device__ __forceinline__ unsigned rank() { return G::CL > 1 ? cluster_ctarank() : 0u; }
-  static __device__ __forceinline__ void begin_fourier() { if (G::CL > 1) cluster_arrive(); }   // registers (re)start in Fourier space
+  static __device__ __forceinline__ void begin_fourier() { if (G::CL > 1) cluster_arrive_war(); }   // registers (re)start in Fourier space
   static __device__ __forceinline__ void end_fourier() { if (G::CL > 1) cluster_wait(); }       // kernel ends in Fourier space
   static __device__ __forceinline__ void fwd(cf (&v)[32], cf* sm, const cf* tw, const cf* tw2, int t, unsigned rk) {
     fft2_fwd<G>(v, sm, tw, t);
