@@ -1637,7 +1637,7 @@ __global__ void __launch_bounds__(256) k_pos_bilinear(KP P, int cl) {
 #define GATHER_TW 64     // tile width in object pixels (256 threads per block)
 #endif
 template <class G, bool ILLUM, bool BILIN>
-__global__ void __launch_bounds__(256, 8) k_gather_object(KP P, cf* gO, float* illum) {
+__global__ void __launch_bounds__(256, ILLUM ? 8 : 0) k_gather_object(KP P, cf* gO, float* illum) {
   typedef FL<G> F;
   constexpr int N = F::NF, NN = F::NNF, NR = BILIN ? N + 1 : N;   // bilinear mode: a window deposits on N + 1 pixels per axis
   __shared__ int2 sr0[256];
