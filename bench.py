@@ -436,7 +436,7 @@ def measure(args, cfg_idx, *, steps, warmup, dist, rank, world, local, bandlimit
     cpu = None
     if rank == 0 and world == 1 and want_cpu:
         from oracle import oracle as orc
-        n = args.cpu_sample or {1: 256, 2: 64, 3: 24, 4: 4, 5: 24}[cfg_idx]
+        n = args.cpu_sample or {1: 256, 2: 256, 3: 128, 4: 8, 5: 128}[cfg_idx]
         pbo = orc.Problem(**problem_kwargs(cfg))
         t0 = time.perf_counter()
         g = orc.gradient(pbo, obj_h, pr_h, pos_h, I_h, batch_idx=np.arange(n, dtype=np.int32))
