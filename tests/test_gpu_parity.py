@@ -264,6 +264,23 @@ def test_deterministic_bitwise(n_modes):
         assert a["loss"] == b["loss"]
 
 
+def test_n256_repeated_runs_bitwise_and_against_oracle():
+    # N = 256: four CTAs per field exchange sub-lattices over distributed shared memory under cluster barriers whose
+    # write-after-read arrives are relaxed (fft_core.cuh: cluster_arrive_war).  A race there would show as run-to-run
+    # differences: 336 CTAs (more than two waves of clusters), twelve passes, every output bit for bit, and the oracle once.
+    cfg = synth.config(4, scan=(6, 7), n_modes=4, n_slices=3, obj_n=330)
+    case = make_case(cfg, start_scale=0.8)
+    pbg = gpu_problem(cfg)
+    a = gpu_gradient(case, pbg)
+    o = orc.gradient(oracle_problem(cfg), case.obj_start, case.probe, case.positions, case.intensity)
+    check(a, o, pos=True, px=cfg.pixel_size)
+    for _ in range(11):
+        b = gpu_gradient(case, pbg)
+        for k in ("grad_object", "grad_probe", "grad_pos", "loss_per_pos"):
+            assert a[k].tobytes() == b[k].tobytes(), k
+        assert a["loss"] == b["loss"]
+
+
 def test_paired_and_unpaired_backward_agree():
     from paper_2505_14372_b200 import ptycho
     # even mode counts run two modes per CTA (the pair's patch gradients summed on chip in float32); PT_NO_MODE_PAIRS forces
