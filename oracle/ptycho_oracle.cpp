@@ -885,6 +885,10 @@ int32_t orc_epie(const orc_problem* p, const float* object, const float* probe, 
 //   kind 2  Tikhonov      R = w sum_{d in x,y} sum |D_d z|^2        (forward differences inside a slice, no wrap-around)
 //   kind 3  TV            R = w sum_{d in x,y} sum sqrt(|D_d z|^2 + eps^2)
 //   kind 4  layer Tikhonov, kind 5 layer TV: the same with the one difference along the depth axis, D_z z = z_{i+1} - z_i
+//   kind 6  L1 on the object PHASE ("L1 regularization: (object, object phase, ...)"; reading R26b):
+//           R = w sum sqrt(phi^2 + eps^2), phi = arg z in (-pi, pi] (principal value: object slices are weak phase objects,
+//           |phi| << pi).  With phi = Im log z, d phi / d conj(z) = i z / (2 |z|^2), hence
+//           dR/dconj(z) = w phi / sqrt(phi^2 + eps^2) * i z / (2 |z|^2); a zero pixel, and phi = 0 with eps = 0, contribute no gradient
 // ------------------------------------------------------------------------------------------
 static double reg_phi(int tv, double a2, double eps) { return tv ? std::sqrt(a2 + eps * eps) : a2; }
 static double reg_dphi(int tv, double a2, double eps) { return tv ? 0.5 / std::sqrt(a2 + eps * eps) : 1.0; }   // d phi / d(a2)
@@ -900,6 +904,16 @@ double orc_cost_regularizer(int32_t kind, double weight, double ref, double eps,
       cd u = Z(i) - ref; double a2 = std::norm(u);
       R += weight * reg_phi(kind == 1, a2, eps);
       addg(i, weight * reg_dphi(kind == 1, a2, eps) * u);              // d phi(|u|^2) / d conj(z) = phi' u
+    }
+    return R;
+  }
+  if (kind == 6) {
+    for (long i = 0; i < n; ++i) {
+      const cd z = Z(i); const double a2 = std::norm(z);
+      if (a2 == 0.0) continue;
+      const double phi = std::atan2(z.imag(), z.real()), q = std::sqrt(phi * phi + eps * eps);
+      R += weight * q;
+      if (q > 0.0) addg(i, weight * (phi / q) * cd(0.0, 1.0) * z / (2.0 * a2));
     }
     return R;
   }

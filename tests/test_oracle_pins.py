@@ -931,8 +931,22 @@ def test_cost_regularizers_closed_forms_and_finite_differences():
     assert abs(orc.cost_regularizer(orc.REG_LAYER_TIKHONOV, 1.0, layers)[0] - ny * nx * (0.25 + 4.0)) < 1e-12
     assert abs(orc.cost_regularizer(orc.REG_LAYER_TV, 1.0, layers, eps=0.0)[0] - ny * nx * (0.5 + 2.0)) < 1e-12
     assert abs(orc.cost_regularizer(orc.REG_L1, 3.0, layers, ref=1.0, eps=0.0)[0] - 3.0 * ny * nx * (0.0 + 0.5 + abs(0.5 + 2j))) < 1e-12
+    # L1 on the phase (R26b): for z = r exp(i phi), R = w sum |phi| whatever r; the gradient is tangential (no radial part: scaling
+    # a pixel does not change its phase) with modulus w / (2 r); the vacuum and a zero pixel cost nothing
+    r = 0.5 + RNG.uniform(size=(S, ny, nx)); phi = RNG.uniform(-1.0, 1.0, size=(S, ny, nx))
+    zp = r * np.exp(1j * phi)
+    Rph, gph = orc.cost_regularizer(orc.REG_L1_PHASE, 1.7, zp, eps=0.0)
+    assert abs(Rph - 1.7 * np.sum(np.abs(phi))) < 1e-11
+    assert np.abs(np.real(np.conj(zp) * gph)).max() < 1e-13                                # tangential
+    assert np.abs(np.abs(gph) - 1.7 / (2 * r)).max() < 1e-12
+    assert np.abs(np.angle(gph * np.conj(1j * zp * np.sign(phi)))).max() < 1e-12          # along +i z for phi > 0: descent lowers |phi|
+    Rv, gv = orc.cost_regularizer(orc.REG_L1_PHASE, 1.7, np.ones_like(zp), eps=0.0)
+    assert Rv == 0.0 and np.abs(gv).max() == 0.0
+    z0 = zp.copy(); z0[1, 2, 3] = 0.0
+    assert np.isfinite(orc.cost_regularizer(orc.REG_L1_PHASE, 1.7, z0, eps=0.1)[1]).all()
+    assert abs(orc.cost_regularizer(orc.REG_L1_PHASE, 2.0, zp, eps=0.3)[0] - 2.0 * np.sum(np.sqrt(phi ** 2 + 0.09))) < 1e-11
     # Wirtinger gradient against central finite differences: dR = 2 Re sum conj(g) dz, for every kind; grad is ADDED into
-    for kind in range(6):
+    for kind in range(7):
         d = crandn(S, ny, nx); h = 1e-6; g0 = crandn(S, ny, nx)
         R, g = orc.cost_regularizer(kind, 0.9, z, ref=1.0, eps=0.05, grad=g0)
         Rp = orc.cost_regularizer(kind, 0.9, z + h * d, ref=1.0, eps=0.05)[0]
