@@ -27,6 +27,22 @@ __global__ void __launch_bounds__(kRegThreads) k_reg_point(int l1, float w, floa
   if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
 }
 
+// kind L1 on the phase (reading R26b): R = w sum sqrt(phi^2 + eps^2), phi = arg z ; dR/dconj(z) = w phi / sqrt(.) * i z / (2 |z|^2)
+__global__ void __launch_bounds__(kRegThreads) k_reg_phase(float w, float eps2, size_t n, const cf* z, cf* g, double* part) {
+  __shared__ double red[kRegThreads / 32];
+  double acc[1] = {0.0};
+  for (size_t i = (size_t)blockIdx.x * kRegThreads + threadIdx.x; i < n; i += (size_t)kRegBlocks * kRegThreads) {
+    const cf v = z[i];
+    const float a2 = fmaf(v.x, v.x, v.y * v.y);
+    if (a2 == 0.f) continue;
+    const float phi = atan2f(v.y, v.x), q = sqrtf(fmaf(phi, phi, eps2));
+    acc[0] += (double)(w * q);
+    if (g && q > 0.f) { const float c = w * (phi / q) / (2.0f * a2); g[i] = make_float2(fmaf(-c, v.y, g[i].x), fmaf(c, v.x, g[i].y)); }
+  }
+  block_sum<kRegThreads, 1>(acc, red);
+  if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
+}
+
 // kinds Tikhonov / TV (in-plane: directions x, y) and their layer versions (direction z): every pixel owns the pair
 // (p, p + stride) for the cost and collects, for its gradient, the pair before it and the pair after it
 __global__ void __launch_bounds__(kRegThreads) k_reg_diff(int tv, int layer, float w, float eps2, int S, int ny, int nx, const cf* z, cf* g,
@@ -202,13 +218,15 @@ int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps
                                 void* cuda_stream) {
   if (!field_d || !workspace_d) return PT_ERR_NULL;
   if (n_slices < 1 || ny < 1 || nx < 1) return PT_ERR_BAD_SIZE;
-  if (kind < PT_REG_L2 || kind > PT_REG_LAYER_TV || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
+  if (kind < PT_REG_L2 || kind > PT_REG_L1_PHASE || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
   if (workspace_bytes < ptycho_regularizer_workspace_bytes()) return PT_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
   double* part = (double*)((char*)workspace_d + 256);
   const size_t n = (size_t)n_slices * ny * nx;
-  if (kind == PT_REG_L2 || kind == PT_REG_L1)
+  if (kind == PT_REG_L1_PHASE)
+    k_reg_phase<<<kRegBlocks, kRegThreads, 0, st>>>(weight, eps * eps, n, (const cf*)field_d, (cf*)grad_d, part);
+  else if (kind == PT_REG_L2 || kind == PT_REG_L1)
     k_reg_point<<<kRegBlocks, kRegThreads, 0, st>>>(kind == PT_REG_L1, weight, ref, eps * eps, n, (const cf*)field_d, (cf*)grad_d, part);
   else
     k_reg_diff<<<kRegBlocks, kRegThreads, 0, st>>>(kind == PT_REG_TV || kind == PT_REG_LAYER_TV, kind >= PT_REG_LAYER_TIKHONOV, weight,

@@ -848,11 +848,13 @@ def _reg_inputs():
     return cfg, obj, g0
 
 
-@pytest.mark.parametrize("kind", range(6))
+@pytest.mark.parametrize("kind", range(7))
 def test_cost_regularizers(kind):
     import torch
     from paper_2505_14372_b200 import ptycho
     cfg, obj, g0 = _reg_inputs()
+    if kind == ptycho.REG_L1_PHASE:
+        obj = obj.copy(); obj[0, 3, 4] = 0.0; obj[1, 5, 6] = 0.7                  # a zero pixel (skipped) and a pixel of phase 0
     R_o, g_o = orc.cost_regularizer(kind, 0.37, obj, ref=1.0, eps=0.02, grad=g0)
     z_d, g_d = _t(obj), _t(g0)
     cost = torch.full((1,), 5.0, dtype=torch.float64, device="cuda")
