@@ -72,7 +72,10 @@ enum { PT_WANT_POS_GRAD = 1,          /* fill grad_pos_d                        
                                        * ptycho_gradient only; not with PT_EPIE, and PT_WANT_ILLUM needs an even mode count or
                                        * PT_WANT_STEP_SIZES (the map comes from the backward kernel's staging): else PT_ERR_UNSUPPORTED */
        PT_NO_SINGLE_SLICE_FUSION = 1024, /* debugging aid: a single-slice problem runs through the multislice kernel sequence (forward chain,
-                                       * loss, backward chain) instead of the fused single-slice kernel                         */
+                                       * loss, backward chain) instead of the fused single-slice kernel.  The fused kernel sums
+                                       * the probe-gradient partials of the positions one resident CTA takes in float32 before the
+                                       * fp64 reduction: grad_probe is bit-reproducible on a device, its last bits depend on the
+                                       * device's SM count                                                                       */
        PT_NO_MODE_PAIRS = 128,        /* debugging aid: the backward pass runs one mode per CTA even when the mode count is even
                                        * (no tensor-memory allocation); results differ only by the rounding of one float32 add */
        PT_EPIE = 32 };                /* ptycho_gradient returns the multislice ePIE ("3PIE") update DIRECTIONS instead of

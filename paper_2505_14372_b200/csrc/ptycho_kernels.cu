@@ -1306,7 +1306,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
 // the thread-private shared-memory slots, the shift ramp ry in the (otherwise idle) propagator-table buffer.  Psi_k and psi~_k
 // pass through the per-position scratch of the workspace (the stash / far-field arrays of the chain path; the CTA reads back what
 // it wrote shortly before, from L2).  Only ONE patch-gradient plane per position is staged (fp32 sum over the modes in order),
-// so the gather reads 1/M of what the per-mode kernels stage.  CTAs stay resident and take positions jl = blockIdx.x, + gridDim.x, ...
+// so the gather reads 1/M of what the per-mode kernels stage, and ONE probe-partial plane per (CTA, mode): the CTA's positions are
+// added in float32 in the order it takes them.  CTAs stay resident and take positions jl = blockIdx.x, + gridDim.x, ...
 // ------------------------------------------------------------------------------------------------
 template <class G>
 __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want_pos) {
@@ -1369,7 +1370,6 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
     for (int hs = 0; hs < 2 * P.M; ++hs) {
       const bool fwd_pass = hs < P.M;
       const int k = fwd_pass ? hs : hs - P.M;
-      const size_t fk = ((size_t)jl * P.M + k) * NNS;               // field (position, mode) in the staged arrays
       const size_t sk = ((size_t)blockIdx.x * P.M + k) * NNS;       // the CTA's scratch field of mode k: the same lines for every position
                                                                     // the CTA takes, so that they stay in L2 instead of streaming to HBM
       if (hs == P.M) {
@@ -1499,7 +1499,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
       } else {
         // H12: probe partial conj(R) .* G~ ;  H13: (4 pi / N^2) sum_q f_a Im(conj(G~) R P~)
         const float4* pt4 = (const float4*)(P.w.Pt + (size_t)k * NNS) + t;
-        float4* gp4 = (float4*)(P.w.Gpart + fk) + t;
+        // probe partial: ONE plane per (CTA, mode), the CTA's positions added in the order it takes them (float32, one adder per
+        // address, program order: deterministic) — 1/7 of the planes at config 2 for the probe reduction to read
+        float4* gp4 = (float4*)(P.w.Gpart + ((size_t)blockIdx.x * P.M + k) * NNS) + t;
+        const bool first_pos = jl == (int)blockIdx.x;
         load_xv<G>(wxv, ryS + NF, t, 1.0f);
         float sy = 0.f, sx = 0.f;
         const float fx = (float)signed_freq(F::fq_x(0, t, 0), NF) / (float)NF;
@@ -1514,7 +1517,8 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
             const int qy0 = F::fq_y(0, t, 2 * p), qy1 = F::fq_y(0, t, 2 * p + 1);
             const cf R0 = cmul(wxv[0], ryS[qy0]), R1 = cmul(wxv[0], ryS[qy1]);
             const cf g0 = cmulc(v[2 * p], R0), g1 = cmulc(v[2 * p + 1], R1);
-            gp4[p * T] = make_float4(g0.x, g0.y, g1.x, g1.y);
+            if (first_pos) gp4[p * T] = make_float4(g0.x, g0.y, g1.x, g1.y);
+            else asm volatile("red.global.add.v4.f32 [%0], {%1,%2,%3,%4};" ::"l"(gp4 + p * T), "f"(g0.x), "f"(g0.y), "f"(g1.x), "f"(g1.y) : "memory");
             if (want_pos) {
               const cf z0 = cmulc(cmul(R0, make_float2(q[e].x, q[e].y)), v[2 * p]), z1 = cmulc(cmul(R1, make_float2(q[e].z, q[e].w)), v[2 * p + 1]);
               sy = fmaf((float)signed_freq(qy0, NF) * (1.0f / (float)NF), z0.y, sy); sx = fmaf(fx, z0.y, sx);
@@ -2202,12 +2206,14 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
   }
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
+  int single_ctas = 0;                                              // k_single: its CTAs each leave ONE probe-partial plane per mode
   auto chains = [&](bool wait_patterns) -> int {
     if constexpr (G::CL == 1) {
       if (single) {
         if (wait_patterns && chunk_ready && cudaStreamWaitEvent(st, chunk_ready[kp.j0 / kp.w.Jc], 0) != cudaSuccess) return PT_ERR_CUDA;
         const int resident = sm_count() * min_blocks<G>();
-        launch_fft<G>(k_single<G>, kp.jc < resident ? kp.jc : resident, chain_smem_bytes<G>(), st, kp, want_pos ? 1 : 0);
+        single_ctas = kp.jc < resident ? kp.jc : resident;
+        launch_fft<G>(k_single<G>, single_ctas, chain_smem_bytes<G>(), st, kp, want_pos ? 1 : 0);
         LAUNCH_CHECK(K_single, st);
         return PT_OK;
       }
@@ -2281,7 +2287,9 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
       k_pos_bilinear<G><<<kp.jc, 256, 0, st>>>(kp, G::CL);
       LAUNCH_CHECK(K_pos_bilinear, st);
     }
-    k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes, kReduceZ), 256, 0, st>>>(kp, kp.w.gPt_part);
+    KP kr = kp;
+    if (single) kr.jc = single_ctas;                                 // the planes of the fused single-slice kernel are per CTA, not per position
+    k_reduce_probe<<<dim3((unsigned)((NN + 255) / 256), p->n_modes, kReduceZ), 256, 0, st>>>(kr, kp.w.gPt_part);
     LAUNCH_CHECK(K_reduce_probe, st);
     k_reduce_probe2<<<dim3((unsigned)((NN + 255) / 256), p->n_modes), 256, 0, st>>>(kp, kp.w.gPt_part);
     LAUNCH_CHECK(K_reduce_probe, st);
