@@ -1437,22 +1437,22 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
       cp_async_wait_all();
       float4* stw = (float4*)(P.w.stash + sk) + t;
 #pragma unroll
-      for (int c = 0; c < 4; ++c) {
-        cf tt[8], ga[8];
-        tmem_ld16(tbT + 16 * c, tt);
+      for (int c = 0; c < 8; ++c) {                                 // 8-column tensor-memory accesses (4 complex): see tmem_swap_field
+        cf tt[4], ga[4];
+        tmem_ld8(tbT + 8 * c, tt);
         if (fwd_pass) {                                             // keep Psi_k for pass 2 ; H4: Phi = Psi_k .* T
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int p = 4 * c + e;
+          for (int e = 0; e < 2; ++e) {
+            const int p = 2 * c + e;
             stw[p * T] = make_float4(v[2 * p].x, v[2 * p].y, v[2 * p + 1].x, v[2 * p + 1].y);
             v[2 * p] = cmul(v[2 * p], tt[2 * e]);
             v[2 * p + 1] = cmul(v[2 * p + 1], tt[2 * e + 1]);
           }
         } else {                                                    // H10: gT += conj(Psi_k) gPhi ; gPsi = conj(T) gPhi
-          if (k > 0) tmem_ld16(tbG + 16 * c, ga);
+          if (k > 0) tmem_ld8(tbG + 8 * c, ga);
 #pragma unroll
-          for (int e = 0; e < 4; ++e) {
-            const int p = 4 * c + e;
+          for (int e = 0; e < 2; ++e) {
+            const int p = 2 * c + e;
             const float4 ps = cs.xs[p * 32];
             const cf g0 = cmulc(v[2 * p], make_float2(ps.x, ps.y)), g1 = cmulc(v[2 * p + 1], make_float2(ps.z, ps.w));
             ga[2 * e] = k > 0 ? cadd(ga[2 * e], g0) : g0;
@@ -1460,11 +1460,11 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_single(KP P, int want
             v[2 * p] = cmulc(v[2 * p], tt[2 * e]);
             v[2 * p + 1] = cmulc(v[2 * p + 1], tt[2 * e + 1]);
           }
-          if (k + 1 < P.M) tmem_st16(tbG + 16 * c, ga);
+          if (k + 1 < P.M) tmem_st8(tbG + 8 * c, ga);
           else {                                                    // last mode: the sum over the modes goes to the staging buffer
             float4* gt = (float4*)(P.w.gTpart + (size_t)jl * NNS) + t;
 #pragma unroll
-            for (int e = 0; e < 4; ++e) __stcs(gt + (4 * c + e) * T, make_float4(ga[2 * e].x, ga[2 * e].y, ga[2 * e + 1].x, ga[2 * e + 1].y));
+            for (int e = 0; e < 2; ++e) __stcs(gt + (2 * c + e) * T, make_float4(ga[2 * e].x, ga[2 * e].y, ga[2 * e + 1].x, ga[2 * e + 1].y));
           }
         }
       }
