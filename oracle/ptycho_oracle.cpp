@@ -889,6 +889,9 @@ int32_t orc_epie(const orc_problem* p, const float* object, const float* probe, 
 //           R = w sum sqrt(phi^2 + eps^2), phi = arg z in (-pi, pi] (principal value: object slices are weak phase objects,
 //           |phi| << pi).  With phi = Im log z, d phi / d conj(z) = i z / (2 |z|^2), hence
 //           dR/dconj(z) = w phi / sqrt(phi^2 + eps^2) * i z / (2 |z|^2); a zero pixel, and phi = 0 with eps = 0, contribute no gradient
+//   kind 7  L1 on the object's Fourier amplitudes per slice ("object power spectrum ... to bias the reconstruction towards
+//           periodic solutions"; reading R26c: the L1 norm of the power spectrum |Z|^2 itself is N times the L2 regulariser by Parseval, so
+//           the sparsity-promoting form is the L1 norm of its square root): R = w sum_s sum_q sqrt(|Z_s[q]|^2 + eps^2); ref unused
 // ------------------------------------------------------------------------------------------
 static double reg_phi(int tv, double a2, double eps) { return tv ? std::sqrt(a2 + eps * eps) : a2; }
 static double reg_dphi(int tv, double a2, double eps) { return tv ? 0.5 / std::sqrt(a2 + eps * eps) : 1.0; }   // d phi / d(a2)
@@ -914,6 +917,48 @@ double orc_cost_regularizer(int32_t kind, double weight, double ref, double eps,
       const double phi = std::atan2(z.imag(), z.real()), q = std::sqrt(phi * phi + eps * eps);
       R += weight * q;
       if (q > 0.0) addg(i, weight * (phi / q) * cd(0.0, 1.0) * z / (2.0 * a2));
+    }
+    return R;
+  }
+  if (kind == 7) {
+    // R = w sum_s sum_q sqrt(|Z_s[q]|^2 + eps^2), Z_s = F z_s the unnormalised 2-D DFT of slice s over the whole (ny x nx) slice,
+    // any size: rows, then columns, by the definition (twiddle index reduced mod the length exactly).
+    // dR/dconj(Z) = w Z / (2 sqrt(|Z|^2 + eps^2)) and Z is linear in z, so dR/dconj(z) = F^H (dR/dconj(Z)).
+    std::vector<cd> wx(nx), wy(ny);
+    for (int m = 0; m < nx; ++m) wx[m] = std::polar(1.0, -2.0 * M_PI * m / nx);
+    for (int m = 0; m < ny; ++m) wy[m] = std::polar(1.0, -2.0 * M_PI * m / ny);
+    std::vector<cd> A(os), Zq(os);
+    for (int s = 0; s < S; ++s) {
+      for (int y = 0; y < ny; ++y)
+        for (int kx = 0; kx < nx; ++kx) {
+          cd a = 0.0;
+          for (int x = 0; x < nx; ++x) a += Z((long)s * os + (long)y * nx + x) * wx[(long)x * kx % nx];
+          A[(long)y * nx + kx] = a;
+        }
+      for (int ky = 0; ky < ny; ++ky)
+        for (int kx = 0; kx < nx; ++kx) {
+          cd a = 0.0;
+          for (int y = 0; y < ny; ++y) a += A[(long)y * nx + kx] * wy[(long)y * ky % ny];
+          Zq[(long)ky * nx + kx] = a;
+        }
+      for (long q = 0; q < os; ++q) {
+        const double a2 = std::norm(Zq[q]), r = std::sqrt(a2 + eps * eps);
+        R += weight * r;
+        Zq[q] = r > 0.0 ? weight * Zq[q] / (2.0 * r) : cd(0.0);     // dR/dconj(Z); |Z| = 0 with eps = 0: subgradient 0
+      }
+      if (!grad) continue;
+      for (int y = 0; y < ny; ++y)                                    // F^H: conjugate kernels, columns then rows
+        for (int kx = 0; kx < nx; ++kx) {
+          cd a = 0.0;
+          for (int ky = 0; ky < ny; ++ky) a += Zq[(long)ky * nx + kx] * std::conj(wy[(long)y * ky % ny]);
+          A[(long)y * nx + kx] = a;
+        }
+      for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) {
+          cd a = 0.0;
+          for (int kx = 0; kx < nx; ++kx) a += A[(long)y * nx + kx] * std::conj(wx[(long)x * kx % nx]);
+          addg((long)s * os + (long)y * nx + x, a);
+        }
     }
     return R;
   }

@@ -945,8 +945,25 @@ def test_cost_regularizers_closed_forms_and_finite_differences():
     z0 = zp.copy(); z0[1, 2, 3] = 0.0
     assert np.isfinite(orc.cost_regularizer(orc.REG_L1_PHASE, 1.7, z0, eps=0.1)[1]).all()
     assert abs(orc.cost_regularizer(orc.REG_L1_PHASE, 2.0, zp, eps=0.3)[0] - 2.0 * np.sum(np.sqrt(phi ** 2 + 0.09))) < 1e-11
+    # L1 on the Fourier amplitudes per slice (R26c), sizes that are no power of two: a constant slice and a plane wave have ONE
+    # non-zero coefficient of modulus ny nx |c|; a delta has ny nx coefficients of modulus |c|; in general the amplitudes are
+    # numpy's fft2 (a library routine); the gradient of a one-peak spectrum is (w / 2) times the unit-modulus wave itself
+    yy, xx = np.meshgrid(np.arange(ny), np.arange(nx), indexing="ij")
+    c = 0.8 - 0.6j
+    const = np.full((S, ny, nx), c)
+    assert abs(orc.cost_regularizer(orc.REG_L1_FOURIER, 1.3, const, eps=0.0)[0] - 1.3 * S * ny * nx * abs(c)) < 1e-9
+    wave = c * np.exp(2j * np.pi * (2 * xx / nx + 3 * yy / ny))[None].repeat(S, 0)
+    assert abs(orc.cost_regularizer(orc.REG_L1_FOURIER, 1.3, wave, eps=0.0)[0] - 1.3 * S * ny * nx * abs(c)) < 1e-9
+    # gradient with a small eps (at eps = 0 the rounding noise of the empty coefficients has an arbitrary phase): F^H of
+    # (w/2) Z / sqrt(|Z|^2 + eps^2) at the one peak = (w/2) exp(i arg c) x the unit wave, the other coefficients ~1e-12
+    gw = orc.cost_regularizer(orc.REG_L1_FOURIER, 1.3, wave, eps=1e-3)[1]
+    assert np.abs(gw - 0.65 * wave / abs(c)).max() < 1e-8
+    delta = np.zeros((S, ny, nx), complex); delta[:, 2, 4] = c
+    assert abs(orc.cost_regularizer(orc.REG_L1_FOURIER, 1.3, delta, eps=0.0)[0] - 1.3 * S * ny * nx * abs(c)) < 1e-9
+    Rg = orc.cost_regularizer(orc.REG_L1_FOURIER, 0.7, z, eps=0.25)[0]
+    assert abs(Rg - 0.7 * np.sum(np.sqrt(np.abs(np.fft.fft2(z, axes=(1, 2))) ** 2 + 0.0625))) < 1e-9 * Rg
     # Wirtinger gradient against central finite differences: dR = 2 Re sum conj(g) dz, for every kind; grad is ADDED into
-    for kind in range(7):
+    for kind in range(8):
         d = crandn(S, ny, nx); h = 1e-6; g0 = crandn(S, ny, nx)
         R, g = orc.cost_regularizer(kind, 0.9, z, ref=1.0, eps=0.05, grad=g0)
         Rp = orc.cost_regularizer(kind, 0.9, z + h * d, ref=1.0, eps=0.05)[0]
