@@ -212,9 +212,12 @@ int32_t ptycho_object_transparency(const pt_problem *p, const pt_c64 *object_d, 
  *   PT_REG_TV             R = w sum_{d = x, y} sum sqrt(|D_d z|^2 + eps^2)
  *   PT_REG_LAYER_TIKHONOV / PT_REG_LAYER_TV   the same with the one difference along depth, z_{i+1} - z_i
  *   PT_REG_L1_PHASE       R = w sum sqrt(phi^2 + eps^2), phi = arg z (principal value; reading R26b); ref unused; zero pixels skipped
+ *   PT_REG_L1_FOURIER     R = w sum_s sum_q sqrt(|Z_s[q]|^2 + eps^2), Z_s the unnormalised 2-D DFT of the whole slice s (any ny, nx
+ *                         <= 4096; reading R26c: the sparsity-promoting form of "L1 on the object power spectrum"); ref unused;
+ *                         needs workspace_bytes >= ptycho_regularizer_workspace_bytes() + 16 * n_slices*ny*nx
  * workspace_d: at least ptycho_regularizer_workspace_bytes() bytes of scratch (per-block cost partials).
  * Errors: PT_ERR_NULL, PT_ERR_BAD_SIZE (a dimension < 1), PT_ERR_BAD_PARAM (unknown kind, eps < 0), PT_ERR_WORKSPACE. */
-enum { PT_REG_L2 = 0, PT_REG_L1 = 1, PT_REG_TIKHONOV = 2, PT_REG_TV = 3, PT_REG_LAYER_TIKHONOV = 4, PT_REG_LAYER_TV = 5, PT_REG_L1_PHASE = 6 };
+enum { PT_REG_L2 = 0, PT_REG_L1 = 1, PT_REG_TIKHONOV = 2, PT_REG_TV = 3, PT_REG_LAYER_TIKHONOV = 4, PT_REG_LAYER_TV = 5, PT_REG_L1_PHASE = 6, PT_REG_L1_FOURIER = 7 };
 size_t ptycho_regularizer_workspace_bytes(void);
 int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps, int32_t n_slices, int32_t ny, int32_t nx,
                                 const pt_c64 *field_d, pt_c64 *grad_d, double *cost_d,

@@ -43,6 +43,50 @@ __global__ void __launch_bounds__(kRegThreads) k_reg_phase(float w, float eps2, 
   if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
 }
 
+// kind L1 on the Fourier amplitudes of every slice (reading R26c).  The slice has any size, so the transform is the DFT by its
+// definition, one axis at a time: one thread per output coefficient, the len twiddles exp(sign 2 pi i m / len) in shared memory (formed
+// in double), the index x k mod len advanced by addition, fp64 accumulation.  O(n (nx + ny)) per slice: a regulariser evaluated
+// once per iteration on the object (420^2: 0.3 Gflop per slice and pass), not part of the hot path.
+constexpr int kDftMaxLen = 4096;
+__global__ void __launch_bounds__(256) k_dft_axis(const cf* in, cf* out, int S, int ny, int nx, int axis, double sign, int add) {
+  extern __shared__ float2 dft_tw[];
+  const int len = axis == 0 ? nx : ny;
+  for (int m = threadIdx.x; m < len; m += blockDim.x) {
+    double sn, cs_; sincospi(sign * 2.0 * (double)m / (double)len, &sn, &cs_);
+    dft_tw[m] = make_float2((float)cs_, (float)sn);
+  }
+  __syncthreads();
+  const size_t os = (size_t)ny * nx, n = (size_t)S * os, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (i >= n) return;
+  const int s = (int)(i / os), y = (int)((i - (size_t)s * os) / nx), x = (int)(i - (size_t)s * os - (size_t)y * nx);
+  const int k = axis == 0 ? x : y;                                    // output index along the axis
+  const cf* src = in + (size_t)s * os + (axis == 0 ? (size_t)y * nx : (size_t)x);
+  const size_t stride = axis == 0 ? 1 : (size_t)nx;
+  double ar = 0.0, ai = 0.0;
+  int idx = 0;
+  for (int j = 0; j < len; ++j) {
+    const cf v = src[(size_t)j * stride]; const float2 w = dft_tw[idx];
+    ar += (double)v.x * w.x - (double)v.y * w.y; ai += (double)v.x * w.y + (double)v.y * w.x;
+    idx += k; if (idx >= len) idx -= len;
+  }
+  if (add) out[i] = make_float2((float)((double)out[i].x + ar), (float)((double)out[i].y + ai));
+  else out[i] = make_float2((float)ar, (float)ai);
+}
+// R partials and Z <- dR/dconj(Z) = w Z / (2 sqrt(|Z|^2 + eps^2)) in place
+__global__ void __launch_bounds__(kRegThreads) k_reg_fourier_point(float w, float eps2, size_t n, cf* Z, double* part) {
+  __shared__ double red[kRegThreads / 32];
+  double acc[1] = {0.0};
+  for (size_t i = (size_t)blockIdx.x * kRegThreads + threadIdx.x; i < n; i += (size_t)kRegBlocks * kRegThreads) {
+    const cf v = Z[i];
+    const float r = sqrtf(fmaf(v.x, v.x, fmaf(v.y, v.y, eps2)));
+    acc[0] += (double)(w * r);
+    const float c = r > 0.f ? 0.5f * w / r : 0.f;
+    Z[i] = make_float2(c * v.x, c * v.y);
+  }
+  block_sum<kRegThreads, 1>(acc, red);
+  if (threadIdx.x == 0) part[blockIdx.x] = acc[0];
+}
+
 // kinds Tikhonov / TV (in-plane: directions x, y) and their layer versions (direction z): every pixel owns the pair
 // (p, p + stride) for the cost and collects, for its gradient, the pair before it and the pair after it
 __global__ void __launch_bounds__(kRegThreads) k_reg_diff(int tv, int layer, float w, float eps2, int S, int ny, int nx, const cf* z, cf* g,
@@ -218,13 +262,31 @@ int32_t ptycho_cost_regularizer(int32_t kind, float weight, float ref, float eps
                                 void* cuda_stream) {
   if (!field_d || !workspace_d) return PT_ERR_NULL;
   if (n_slices < 1 || ny < 1 || nx < 1) return PT_ERR_BAD_SIZE;
-  if (kind < PT_REG_L2 || kind > PT_REG_L1_PHASE || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
+  if (kind < PT_REG_L2 || kind > PT_REG_L1_FOURIER || !(eps >= 0.f)) return PT_ERR_BAD_PARAM;
   if (workspace_bytes < ptycho_regularizer_workspace_bytes()) return PT_ERR_WORKSPACE;
   cudaStream_t st = (cudaStream_t)cuda_stream;
   prof_mark(-1, st);
   double* part = (double*)((char*)workspace_d + 256);
   const size_t n = (size_t)n_slices * ny * nx;
-  if (kind == PT_REG_L1_PHASE)
+  if (kind == PT_REG_L1_FOURIER) {
+    if (nx > kDftMaxLen || ny > kDftMaxLen) return PT_ERR_BAD_SIZE;
+    if (workspace_bytes < ptycho_regularizer_workspace_bytes() + 2 * n * sizeof(cf)) return PT_ERR_WORKSPACE;
+    cf* A = (cf*)((char*)workspace_d + ptycho_regularizer_workspace_bytes());
+    cf* B = A + n;
+    const unsigned grid = (unsigned)((n + 255) / 256);
+    k_dft_axis<<<grid, 256, (size_t)nx * sizeof(float2), st>>>((const cf*)field_d, A, n_slices, ny, nx, 0, -1.0, 0);
+    LAUNCH_CHECK(K_regularizer, st);
+    k_dft_axis<<<grid, 256, (size_t)ny * sizeof(float2), st>>>(A, B, n_slices, ny, nx, 1, -1.0, 0);
+    LAUNCH_CHECK(K_regularizer, st);
+    k_reg_fourier_point<<<kRegBlocks, kRegThreads, 0, st>>>(weight, eps * eps, n, B, part);
+    LAUNCH_CHECK(K_regularizer, st);
+    if (grad_d) {                                                     // F^H: conjugate kernels, columns then rows, added into grad
+      k_dft_axis<<<grid, 256, (size_t)ny * sizeof(float2), st>>>(B, A, n_slices, ny, nx, 1, 1.0, 0);
+      LAUNCH_CHECK(K_regularizer, st);
+      k_dft_axis<<<grid, 256, (size_t)nx * sizeof(float2), st>>>(A, (cf*)grad_d, n_slices, ny, nx, 0, 1.0, 1);
+      LAUNCH_CHECK(K_regularizer, st);
+    }
+  } else if (kind == PT_REG_L1_PHASE)
     k_reg_phase<<<kRegBlocks, kRegThreads, 0, st>>>(weight, eps * eps, n, (const cf*)field_d, (cf*)grad_d, part);
   else if (kind == PT_REG_L2 || kind == PT_REG_L1)
     k_reg_point<<<kRegBlocks, kRegThreads, 0, st>>>(kind == PT_REG_L1, weight, ref, eps * eps, n, (const cf*)field_d, (cf*)grad_d, part);

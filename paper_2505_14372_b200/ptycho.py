@@ -294,7 +294,7 @@ def profile_fp32_peak(workspace) -> float:
 
 
 # ---- cost / constraint regularisers and Adam (include/ptycho.h) -----------------------------------
-REG_L2, REG_L1, REG_TIKHONOV, REG_TV, REG_LAYER_TIKHONOV, REG_LAYER_TV, REG_L1_PHASE = range(7)
+REG_L2, REG_L1, REG_TIKHONOV, REG_TV, REG_LAYER_TIKHONOV, REG_LAYER_TV, REG_L1_PHASE, REG_L1_FOURIER = range(8)
 CON_AMPLITUDE_CLAMP, CON_SUPPORT_MASK, CON_LAYER_BLUR, CON_LOWPASS, CON_SUPPORT_MASK_FOURIER, CON_PHASE_DERAMP = range(6)
 
 

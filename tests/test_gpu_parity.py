@@ -848,17 +848,22 @@ def _reg_inputs():
     return cfg, obj, g0
 
 
-@pytest.mark.parametrize("kind", range(7))
+@pytest.mark.parametrize("kind", range(8))
 def test_cost_regularizers(kind):
     import torch
     from paper_2505_14372_b200 import ptycho
     cfg, obj, g0 = _reg_inputs()
+    if kind == ptycho.REG_L1_FOURIER:
+        obj, g0 = obj[:2, :150, :173].copy(), g0[:2, :150, :173].copy()        # the oracle's DFT by the definition is O(n^1.5): a ragged 150 x 173 cut
     if kind == ptycho.REG_L1_PHASE:
         obj = obj.copy(); obj[0, 3, 4] = 0.0; obj[1, 5, 6] = 0.7                  # a zero pixel (skipped) and a pixel of phase 0
     R_o, g_o = orc.cost_regularizer(kind, 0.37, obj, ref=1.0, eps=0.02, grad=g0)
     z_d, g_d = _t(obj), _t(g0)
     cost = torch.full((1,), 5.0, dtype=torch.float64, device="cuda")
-    ws = torch.empty(ptycho.regularizer_workspace_bytes(), dtype=torch.uint8, device="cuda")
+    ws = torch.empty(ptycho.regularizer_workspace_bytes() + (16 * obj.size if kind == ptycho.REG_L1_FOURIER else 0), dtype=torch.uint8, device="cuda")
+    if kind == ptycho.REG_L1_FOURIER:
+        with pytest.raises(ptycho.PtychoError):
+            ptycho.cost_regularizer(kind, 0.37, z_d, grad=g_d, workspace=ws[:ptycho.regularizer_workspace_bytes()])
     ptycho.cost_regularizer(kind, 0.37, z_d, grad=g_d, cost=cost, ref=1.0, eps=0.02, workspace=ws)
     torch.cuda.synchronize()
     assert abs((cost.item() - 5.0) - R_o) <= 1e-5 * abs(R_o)                       # cost is ADDED
