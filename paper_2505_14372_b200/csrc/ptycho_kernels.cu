@@ -1948,6 +1948,13 @@ __global__ void k_zero(float* p, size_t n) {
   const size_t stride = (size_t)gridDim.x * blockDim.x;
   for (; i < n; i += stride) p[i] = 0.f;
 }
+// up to three arrays in one launch (a small problem's step is a dozen launches of a few microseconds: every launch saved counts)
+__global__ void k_zero3(float* a, size_t na, float* b, size_t nb, float* c, size_t nc) {
+  const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t i = i0; i < na; i += stride) a[i] = 0.f;
+  for (size_t i = i0; i < nb; i += stride) b[i] = 0.f;
+  for (size_t i = i0; i < nc; i += stride) c[i] = 0.f;
+}
 
 // O13: dOhat = -gO / (illum_prev + delta_O)
 __global__ void k_dohat(const cf* gO, const float* illum_prev, float delta_o, cf* out, size_t n) {
@@ -1966,12 +1973,23 @@ __global__ void k_axpy(float* z, const float* g, float a, size_t n) {
 }
 // (rows outside [0, n_rows) are skipped; the gradient call that produced g has already raised PT_ERR_OUT_OF_BOUNDS for them.
 //  A batch must not name a row twice: the two updates would race.)
-__global__ void k_pos_sgd(float* pos, const float* g, const int32_t* idx, float lr, int J, int n_rows) {
-  int j = blockIdx.x * blockDim.x + threadIdx.x;
-  if (j >= J) return;
-  int row = idx ? idx[j] : j;
-  if (row < 0 || row >= n_rows) return;
-  pos[2 * row] -= lr * g[2 * j]; pos[2 * row + 1] -= lr * g[2 * j + 1];
+// the whole SGD step in one launch: blocks [0, bo) the object, [bo, bo + bp) the probe, the rest the positions (same arithmetic
+// per element as k_axpy; positions: pos[row] -= lr g[j])
+__global__ void k_sgd(float* obj, const float* gO, float ao, size_t no, unsigned bo, float* pr, const float* gP, float ap, size_t np, unsigned bp,
+                      float* pos, const float* gX, const int32_t* idx, float lr, int J, int n_rows) {
+  if (blockIdx.x < bo) {
+    const size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < no) obj[i] = fmaf(ao, gO[i], obj[i]);
+  } else if (blockIdx.x < bo + bp) {
+    const size_t i = (size_t)(blockIdx.x - bo) * blockDim.x + threadIdx.x;
+    if (i < np) pr[i] = fmaf(ap, gP[i], pr[i]);
+  } else {
+    const int j = (int)(blockIdx.x - bo - bp) * blockDim.x + threadIdx.x;
+    if (j >= J) return;
+    const int row = idx ? idx[j] : j;
+    if (row < 0 || row >= n_rows) return;
+    pos[2 * row] -= lr * gX[2 * j]; pos[2 * row + 1] -= lr * gX[2 * j + 1];
+  }
 }
 // alpha[c] = sum_j num / (sum_j den + gamma) for c = 0..S (S object slices, then the probe); one block per c
 __global__ void k_lsqml_alpha(const float* step_terms, int J, int S, float gamma, float* alpha) {
@@ -2197,13 +2215,9 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
                       !(p->flags & PT_NO_SINGLE_SLICE_FUSION);
   kp.Mg = single ? 1 : paired ? p->n_modes / 2 : p->n_modes;
   kp.Mi = paired ? p->n_modes / 2 : p->n_modes;
-  k_zero<<<296, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4);
+  k_zero3<<<592, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4, (float*)gO, acc ? 0 : on * 2, illum,
+                               !acc && want_illum ? (want_w ? 2 * on : on) : 0);
   LAUNCH_CHECK(K_zero, st);
-  if (!acc) {
-    k_zero<<<592, 256, 0, st>>>((float*)gO, on * 2);
-    LAUNCH_CHECK(K_zero, st);
-    if (want_illum) { k_zero<<<592, 256, 0, st>>>(illum, want_w ? 2 * on : on); LAUNCH_CHECK(K_zero, st); }
-  }
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
   int single_ctas = 0;                                              // k_single: its CTAs each leave ONE probe-partial plane per mode
@@ -2505,9 +2519,14 @@ int32_t ptycho_apply_update(const pt_problem* p, pt_c64* object_d, pt_c64* probe
   prof_mark(-1, st);
   const size_t NN = (size_t)p->n * p->n, os = (size_t)p->obj_ny * p->obj_nx, on = os * p->n_slices, pn = NN * p->n_modes;
   if (u->mode == PT_UPDATE_SGD) {
-    if (object_d && grad_object_d) { k_axpy<<<(unsigned)((2 * on + 255) / 256), 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, -u->lr_obj, 2 * on); LAUNCH_CHECK(K_axpy, st); }
-    if (probe_d && grad_probe_d) { k_axpy<<<(unsigned)((2 * pn + 255) / 256), 256, 0, st>>>((float*)probe_d, (const float*)grad_probe_d, -u->lr_probe, 2 * pn); LAUNCH_CHECK(K_axpy, st); }
-    if (positions_d && grad_pos_d) { k_pos_sgd<<<(p->n_batch + 255) / 256, 256, 0, st>>>(positions_d, grad_pos_d, batch_idx_d, u->lr_pos, p->n_batch, p->n_pos_total); LAUNCH_CHECK(K_pos_sgd, st); }
+    const bool uo = object_d && grad_object_d, up = probe_d && grad_probe_d, ux = positions_d && grad_pos_d;
+    const unsigned bo = uo ? (unsigned)((2 * on + 255) / 256) : 0, bp = up ? (unsigned)((2 * pn + 255) / 256) : 0, bx = ux ? (unsigned)((p->n_batch + 255) / 256) : 0;
+    if (bo + bp + bx) {
+      k_sgd<<<bo + bp + bx, 256, 0, st>>>((float*)object_d, (const float*)grad_object_d, -u->lr_obj, uo ? 2 * on : 0, bo, (float*)probe_d,
+                                          (const float*)grad_probe_d, -u->lr_probe, up ? 2 * pn : 0, bp, positions_d, grad_pos_d, batch_idx_d,
+                                          u->lr_pos, ux ? p->n_batch : 0, p->n_pos_total);
+      LAUNCH_CHECK(K_axpy, st);
+    }
     return PT_OK;
   }
   if (u->mode == PT_UPDATE_EPIE) {      // O_i += beta_object dO_i ; P_k += beta_probe dP_k
