@@ -317,8 +317,13 @@ __global__ void k_setup_pos(KP P) {
 }
 
 // O2[y][x] = (O[y][x], O[y][x + D]) for every slice (zero where x + D leaves the row: no window reads those as a first element)
-__global__ void k_pair_object(KP P, int D) {
-  const size_t n = (size_t)P.S * P.ony * P.onx, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
+// The same launch clears up to three arrays of the gradient call (probe-gradient accumulator, grad_object, illumination map): a
+// small problem's step is a dozen launches of a few microseconds each, every launch saved counts.
+__global__ void k_pair_object(KP P, int D, float* za, size_t na, float* zb, size_t nb, float* zc, size_t nc) {
+  const size_t n = (size_t)P.S * P.ony * P.onx, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)gridDim.x * blockDim.x;
+  for (size_t j = i; j < na; j += stride) za[j] = 0.f;
+  for (size_t j = i; j < nb; j += stride) zb[j] = 0.f;
+  for (size_t j = i; j < nc; j += stride) zc[j] = 0.f;
   if (i >= n) return;
   const int x = (int)(i % P.onx);
   const cf a = P.object[i], b = x + D < P.onx ? P.object[i + D] : make_float2(0.f, 0.f);
@@ -1943,18 +1948,6 @@ __global__ void k_finalize(KP P, int cl, double* loss, int accumulate, float* lo
   }
 }
 
-__global__ void k_zero(float* p, size_t n) {
-  size_t i = (size_t)blockIdx.x * blockDim.x + threadIdx.x;
-  const size_t stride = (size_t)gridDim.x * blockDim.x;
-  for (; i < n; i += stride) p[i] = 0.f;
-}
-// up to three arrays in one launch (a small problem's step is a dozen launches of a few microseconds: every launch saved counts)
-__global__ void k_zero3(float* a, size_t na, float* b, size_t nb, float* c, size_t nc) {
-  const size_t i0 = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)gridDim.x * blockDim.x;
-  for (size_t i = i0; i < na; i += stride) a[i] = 0.f;
-  for (size_t i = i0; i < nb; i += stride) b[i] = 0.f;
-  for (size_t i = i0; i < nc; i += stride) c[i] = 0.f;
-}
 
 // O13: dOhat = -gO / (illum_prev + delta_O)
 __global__ void k_dohat(const cf* gO, const float* illum_prev, float delta_o, cf* out, size_t n) {
@@ -2147,7 +2140,7 @@ int set_smem_attrs() {
 
 // common prologue: tables, position split, probe spectrum
 template <class G>
-int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
+int prologue(const pt_problem* p, KP& kp, cudaStream_t st, float* za = nullptr, size_t na = 0, float* zb = nullptr, size_t nb = 0, float* zc = nullptr, size_t nc = 0) {
   int rc = set_smem_attrs<G>();
   if (rc != PT_OK) return rc;
   const int nprop = p->n_slices - 1;
@@ -2164,7 +2157,7 @@ int prologue(const pt_problem* p, KP& kp, cudaStream_t st) {
   LAUNCH_CHECK(K_setup_pos, st);
   {
     const size_t on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
-    k_pair_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X);
+    k_pair_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X, za, na, zb, nb, zc, nc);
     LAUNCH_CHECK(K_setup_pos, st);
   }
   launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f, (const float*)nullptr, 0.0f);
@@ -2196,11 +2189,14 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
                  float* step_terms, double* loss_d, float* loss_per_pos_d, cudaStream_t st, const cudaEvent_t* chunk_ready) {
   // chunk_ready (ptycho_gradient_host only): one event per chunk, recorded on its copy stream when that chunk's measured
   // patterns have arrived on the device; the pass waits for chunk c's event before the first kernel that reads them (k_loss)
-  int rc = prologue<G>(p, kp, st);
-  if (rc != PT_OK) return rc;
   const size_t NN = (size_t)p->n * p->n, on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
   const bool acc = (p->flags & PT_ACCUMULATE) != 0;
   const bool want_illum = (p->flags & PT_WANT_ILLUM) && illum;
+  // tables, position split, probe spectrum; the object pre-pass also clears the probe-gradient accumulator and (unless accumulating)
+  // grad_object and the illumination map(s)
+  int rc = prologue<G>(p, kp, st, (float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4, (float*)gO, acc ? 0 : on * 2, illum,
+                       !acc && want_illum ? ((p->flags & PT_WANT_WEIGHTED_ILLUM) ? 2 * on : on) : 0);
+  if (rc != PT_OK) return rc;
   const bool want_pos = (p->flags & PT_WANT_POS_GRAD) && gX && !(p->flags & PT_EPIE);
   const bool want_steps = (p->flags & PT_WANT_STEP_SIZES) && step_terms;
   const bool want_w = (p->flags & PT_WANT_WEIGHTED_ILLUM) != 0;     // validated by the caller: needs want_illum && want_steps
@@ -2215,9 +2211,6 @@ int run_gradient(const pt_problem* p, KP kp, pt_c64* gO, pt_c64* gP, float* gX, 
                       !(p->flags & PT_NO_SINGLE_SLICE_FUSION);
   kp.Mg = single ? 1 : paired ? p->n_modes / 2 : p->n_modes;
   kp.Mi = paired ? p->n_modes / 2 : p->n_modes;
-  k_zero3<<<592, 256, 0, st>>>((float*)kp.w.gPt_acc, (size_t)p->n_modes * NN * 4, (float*)gO, acc ? 0 : on * 2, illum,
-                               !acc && want_illum ? (want_w ? 2 * on : on) : 0);
-  LAUNCH_CHECK(K_zero, st);
   const dim3 ggrid((p->obj_nx + GATHER_TW - 1) / GATHER_TW, (p->obj_ny + 256 / GATHER_TW - 1) / (256 / GATHER_TW), p->n_slices), gblock(GATHER_TW, 256 / GATHER_TW);
   // forward chain, loss, backward chain of the current chunk (kp.j0, kp.jc); the backward kernels stage gT, conj(R) G~, |Psi|^2
   int single_ctas = 0;                                              // k_single: its CTAs each leave ONE probe-partial plane per mode
