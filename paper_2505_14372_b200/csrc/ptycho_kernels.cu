@@ -823,9 +823,10 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward(KP P, int wa
         else if (q < 16) { const int p = q - (16 - E); cp_async16(cs.xs + (16 - E + p) * 32, o2 + F::patch_off(2 * p, onx)); }
         else { const int p = E + (q - 16); Tr[p - E] = ld_nc16(o2 + F::patch_off(2 * p, onx)); }
       };
+      constexpr int NHU = NH * 2 / 3;                              // within the first two thirds of the steps (see k_backward_pair)
       L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout)
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) if (q * NH / NQ == step) item(q);
+        for (int q = 0; q < NQ; ++q) if (q * NHU / NQ == step) item(q);
       });
       cp_async_commit();
     }
@@ -1201,9 +1202,12 @@ __global__ void __launch_bounds__(G::T, min_blocks<G>()) k_backward_pair(KP P, i
         else if (q < 16) { const int p = q - (16 - E); cp_async16(cs.xs + (16 - E + p) * 32, o2 + F::patch_off(2 * p, onx)); }
         else { const int p = E + (q - 16); Tr[p - E] = ld_nc16(o2 + F::patch_off(2 * p, onx)); }
       };
+      // over the first two thirds of the steps only: spread over all of them, the last copies were issued ~20 instructions before the
+      // wait below in some variants (ncu, illumination-staging kernel: 2.3 % of the samples on that wait); 49.8 -> 49.1 ms per step
+      constexpr int NHU = NH * 2 / 3;
       L::phase1_inv_h(v, tw, t, [&](int step) {                  // gPhi_{i,k}  (R-layout); backward 56.4 -> 55.5 ms per step
 #pragma unroll
-        for (int q = 0; q < NQ; ++q) if (q * NH / NQ == step) item(q);
+        for (int q = 0; q < NQ; ++q) if (q * NHU / NQ == step) item(q);
       });
       cp_async_commit();
     }
