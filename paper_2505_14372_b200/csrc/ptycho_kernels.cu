@@ -2,7 +2,7 @@
 //
 // Path, all on the caller's stream:
 //   k_setup_prop     H5 tables  hx_i[qx], hy_i[qy] (separable Fresnel + tilt phases, fp64 math -> fp32)
-//   k_setup_pos      H0 position split (fp32, reading R2) + H2 shift ramps rx_j, ry_j + bounds flag (R4)
+//   setup_pos_one    H0 position split (fp32, reading R2) + H2 shift ramps rx_j, ry_j + bounds flag (R4)
 //   k_probe_fft      H1 P~_k = F(P_k)
 //   k_forward        H2..H6 one CTA per (position j, mode k): field in registers, 2S in-register 2-D FFTs,
 //                    entering waves Psi_{i,k} stashed for the adjoint, far field psi~_k written out
@@ -277,10 +277,10 @@ __global__ void k_setup_prop(PropArgs a) {
 // ------------------------------------------------------------------------------------------------
 // H0 + H2 tables: position split in fp32 exactly as the reading R2 states it (no FMA contraction), bounds
 // flag (R4: clamp + raise), shift ramps rx[q] = exp(-2 pi i f(q) dx), ry likewise.
-// One block per position, N threads.
+// N threads per position (thread q writes the ramps' entry q); launched inside k_pair_object's grid (below).
 // ------------------------------------------------------------------------------------------------
-__global__ void k_setup_pos(KP P) {
-  const int jb = blockIdx.x, q = threadIdx.x, N = P.N;
+__device__ __forceinline__ void setup_pos_one(const KP& P, int jb, int q) {
+  const int N = P.N;
   int row = P.batch_idx ? P.batch_idx[jb] : jb;
   if (row < 0 || row >= P.Jtot) {                                 // a batch entry outside the tables: clamp + raise, as R4
     if (q == 0) atomicOr(P.w.status, kStatusOOB);
@@ -319,8 +319,15 @@ __global__ void k_setup_pos(KP P) {
 // O2[y][x] = (O[y][x], O[y][x + D]) for every slice (zero where x + D leaves the row: no window reads those as a first element)
 // The same launch clears up to three arrays of the gradient call (probe-gradient accumulator, grad_object, illumination map): a
 // small problem's step is a dozen launches of a few microseconds each, every launch saved counts.
-__global__ void k_pair_object(KP P, int D, float* za, size_t na, float* zb, size_t nb, float* zc, size_t nc) {
-  const size_t n = (size_t)P.S * P.ony * P.onx, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)gridDim.x * blockDim.x;
+// Blocks [nb_obj, gridDim.x) do the position set-up (k_setup_pos of earlier builds: 256 / N positions per block) — one launch for the
+// whole prologue besides the probe transform and the propagator tables.
+__global__ void __launch_bounds__(256) k_pair_object(KP P, int D, float* za, size_t na, float* zb, size_t nb, float* zc, size_t nc, unsigned nb_obj) {
+  if (blockIdx.x >= nb_obj) {
+    const int jb = (int)(blockIdx.x - nb_obj) * (256 / P.N) + (int)threadIdx.x / P.N;
+    if (jb < P.J) setup_pos_one(P, jb, (int)threadIdx.x % P.N);
+    return;
+  }
+  const size_t n = (size_t)P.S * P.ony * P.onx, i = (size_t)blockIdx.x * blockDim.x + threadIdx.x, stride = (size_t)nb_obj * blockDim.x;
   for (size_t j = i; j < na; j += stride) za[j] = 0.f;
   for (size_t j = i; j < nb; j += stride) zb[j] = 0.f;
   for (size_t j = i; j < nc; j += stride) zc[j] = 0.f;
@@ -2157,11 +2164,10 @@ int prologue(const pt_problem* p, KP& kp, cudaStream_t st, float* za = nullptr, 
     k_setup_prop<<<(n + 255) / 256, 256, 0, st>>>(a);
     LAUNCH_CHECK(K_setup_prop, st);
   }
-  k_setup_pos<<<p->n_batch, p->n, 0, st>>>(kp);
-  LAUNCH_CHECK(K_setup_pos, st);
   {
     const size_t on = (size_t)p->n_slices * p->obj_ny * p->obj_nx;
-    k_pair_object<<<(unsigned)((on + 255) / 256), 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X, za, na, zb, nb, zc, nc);
+    const unsigned nb_obj = (unsigned)((on + 255) / 256), per = 256u / (unsigned)p->n, nb_pos = ((unsigned)p->n_batch + per - 1) / per;
+    k_pair_object<<<nb_obj + nb_pos, 256, 0, st>>>(kp, (G::CL == 1 ? 1 : 2) * G::N2X, za, na, zb, nb, zc, nc, nb_obj);
     LAUNCH_CHECK(K_setup_pos, st);
   }
   launch_fft<G>(k_probe_fft<G>, p->n_modes * G::CL, fft_smem_bytes<G>(), st, kp.probe, kp.w.Pt, 1.0f, (const float*)nullptr, 0.0f);
