@@ -10,7 +10,8 @@
  *     memory and keeps no pointer after a call returns.  The device-path calls are re-entrant across streams and
  *     threads; process-wide state is limited to (a) a once-per-device record that the kernels' shared-memory limits
  *     have been set, (b) the copy stream and events of ptycho_gradient_host, created on first use and reused (that
- *     call is serialised by a lock), and (c) the per-THREAD launch counter and optional profiling record below.
+ *     call is serialised by a lock), (c) the per-THREAD launch counter and optional profiling record below, and (d) the
+ *     16 MiB static device array of ptycho_apply_constraint_static with its per-device cached address.
  *     pt_problem / pt_update / slice_thickness are HOST memory, read synchronously during the call.
  *   - workspace_d: DEVICE memory, 256-byte aligned.  Its first 256 bytes hold the deferred status word: the caller
  *     zeroes them once when the buffer is allocated (cudaMemset); ptycho_status() reads and clears the word.
